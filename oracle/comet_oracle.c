@@ -1,0 +1,360 @@
+/*
+ * comet_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, fp64 CPU restatement of the seed x hit scan of arXiv 1911.09340
+ * ("GPU-accelerated event reconstruction for the COMET Phase-I experiment"),
+ * written from the paper (citations are /root/reference/PAPER.md line numbers)
+ * with the readings R1..R23 listed in DESIGN.md.  It shares no code with the
+ * CUDA path under paper_1911_09340_b200/ and must never be imported, linked or
+ * called by it: only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may use it.
+ *
+ * Shape: the paper's CPU function, Algorithm 3: one task per
+ * seed = record the track (Algorithm 1's loop), then for every
+ * wire find the recorded state closest to it and iterate the virtual-plane
+ * extrapolation (Algorithm 2, prose :103, :216), accumulate
+ * the squared bounded residual of Eq. (1).  OpenMP runs over
+ * seeds only, so results do not depend on the thread count.
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (no fast-math, no
+ * contraction: every operation below is one IEEE-754 double operation in the
+ * order written).
+ *
+ * Parity pins (tests/test_oracle_pins.py): closed-form helix radius / angular
+ * advance / pitch, |T| conservation, straight-line limit, reversibility, axial
+ * wire closed form, brute-force dense sampling, rotation / translation / endpoint
+ * swap symmetries, truth-seed RSS = injected smearing, RSS bounds, brute-force
+ * argmin and classification.  No function here is "parity unpinned".
+ *
+ * Units: cm, MeV/c, Tesla, charge in e.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* R4: "0.3 B" of PAPER.md:319 Eq. (2), in (MeV/c)/(T cm). */
+#define ORACLE_KAPPA 2.99792458
+/* R9: TOLERANCE of PAPER.md:173 and the iteration cap. */
+#define ORACLE_TOL_CM 1e-9
+#define ORACLE_MAX_ITER 16
+
+typedef struct {
+    double x[3];
+    double T[3];
+} ostate;
+
+/* f(T) = c (T x z_hat) = c (Ty, -Tx, 0): the uniform-B_z equation of motion (O1). */
+static void field_rhs(const double T[3], double c, double k[3])
+{
+    k[0] = c * T[1];
+    k[1] = -(c * T[0]);
+    k[2] = 0.0;
+}
+
+/* O2 / R1: one classical 4th-order Runge-Kutta-Nystrom step of signed length h
+ * (method of ref [7]).  T is not renormalised. */
+static void rkn4_step(ostate* s, double h, double c)
+{
+    double k1[3], k2[3], k3[3], k4[3], t[3];
+    int i;
+    field_rhs(s->T, c, k1);
+    for (i = 0; i < 3; ++i) t[i] = s->T[i] + (h / 2.0) * k1[i];
+    field_rhs(t, c, k2);
+    for (i = 0; i < 3; ++i) t[i] = s->T[i] + (h / 2.0) * k2[i];
+    field_rhs(t, c, k3);
+    for (i = 0; i < 3; ++i) t[i] = s->T[i] + h * k3[i];
+    field_rhs(t, c, k4);
+    for (i = 0; i < 3; ++i) {
+        s->x[i] = s->x[i] + h * s->T[i] + ((h * h) / 6.0) * (k1[i] + k2[i] + k3[i]);
+    }
+    for (i = 0; i < 3; ++i) {
+        s->T[i] = s->T[i] + (h / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+    }
+}
+
+/* O1 + O3: Algorithm 1.  pts has room for n_steps+1 states.
+ * R3: targetRegion = first recorded point with r < r_stop moving inward. */
+static int record_track(const double seed[6], int charge, double bz, double h, int n_steps,
+                        double r_stop, ostate* pts)
+{
+    double P = sqrt(seed[3] * seed[3] + seed[4] * seed[4] + seed[5] * seed[5]);
+    double c = ORACLE_KAPPA * (double)charge * bz / P;
+    int k, n_pts = n_steps + 1;
+    pts[0].x[0] = seed[0]; pts[0].x[1] = seed[1]; pts[0].x[2] = seed[2];
+    pts[0].T[0] = seed[3] / P; pts[0].T[1] = seed[4] / P; pts[0].T[2] = seed[5] / P;
+    for (k = 1; k <= n_steps; ++k) {
+        pts[k] = pts[k - 1];
+        rkn4_step(&pts[k], h, c);
+        if (r_stop > 0.0) {
+            double r2 = pts[k].x[0] * pts[k].x[0] + pts[k].x[1] * pts[k].x[1];
+            double rad = pts[k].x[0] * pts[k].T[0] + pts[k].x[1] * pts[k].T[1];
+            if (r2 < r_stop * r_stop && rad < 0.0) { n_pts = k + 1; break; }
+        }
+    }
+    return n_pts;
+}
+
+static double dot3(const double a[3], const double b[3])
+{
+    return a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
+}
+
+/* O4: perp(x) = (x - m) - ((x - m) . w) w, the vector from the infinite wire line
+ * (R5) to x, measured from the wire midpoint m. */
+static void perp_to_wire(const double x[3], const double m[3], const double w[3], double u[3])
+{
+    double d[3], t;
+    int i;
+    for (i = 0; i < 3; ++i) d[i] = x[i] - m[i];
+    t = dot3(d, w);
+    for (i = 0; i < 3; ++i) u[i] = d[i] - t * w[i];
+}
+
+/* O5..O7: Algorithm 2 lines 6-15 for one (track, wire): returns the signed DCA,
+ * writes the index of the closest recorded state to *kstar_out. */
+static double wire_dca(const ostate* pts, int n_pts, double h, double c,
+                       const double m[3], const double w[3], int* kstar_out)
+{
+    int k, kstar = 0, it;
+    double best = 0.0, u[3], sigma = 0.0, lo, hi, cross[3], side, dist;
+    ostate s;
+    /* O5 / R6: closest recorded state, squared perpendicular distance, ties -> lowest k
+     * ("Find state (in params) closest to geom"). */
+    for (k = 0; k < n_pts; ++k) {
+        double d2;
+        perp_to_wire(pts[k].x, m, w, u);
+        d2 = dot3(u, u);
+        if (k == 0 || d2 < best) { best = d2; kstar = k; }
+    }
+    /* O6 / R7, R8, R10: virtual plane through the wire whose normal is the part of
+     * the momentum direction perpendicular to the wire; step by the
+     * path length to that plane; total offset kept inside [s_{k*-1}, s_{k*+1}]. */
+    s = pts[kstar];
+    lo = (kstar > 0) ? -h : 0.0;
+    hi = (kstar < n_pts - 1) ? h : 0.0;
+    for (it = 0; it < ORACLE_MAX_ITER; ++it) {
+        double nv[3], tw, den, mx[3], delta, target;
+        int i;
+        tw = dot3(s.T, w);
+        for (i = 0; i < 3; ++i) nv[i] = s.T[i] - tw * w[i];
+        den = dot3(s.T, nv);
+        if (den < 1e-12) break;
+        for (i = 0; i < 3; ++i) mx[i] = m[i] - s.x[i];
+        delta = dot3(mx, nv) / den;
+        target = sigma + delta;
+        if (target < lo) target = lo;
+        if (target > hi) target = hi;
+        delta = target - sigma;
+        if (fabs(delta) < ORACLE_TOL_CM) break;
+        rkn4_step(&s, delta, c);
+        sigma = sigma + delta;
+    }
+    /* O7 / R16: signed DCA, + when u . (T x w) >= 0. */
+    perp_to_wire(s.x, m, w, u);
+    cross[0] = s.T[1] * w[2] - s.T[2] * w[1];
+    cross[1] = s.T[2] * w[0] - s.T[0] * w[2];
+    cross[2] = s.T[0] * w[1] - s.T[1] * w[0];
+    side = dot3(u, cross);
+    dist = sqrt(dot3(u, u));
+    if (kstar_out) *kstar_out = kstar;
+    return (side >= 0.0) ? dist : -dist;
+}
+
+/* O4: unit direction and midpoint of fired wire i. */
+static void wire_line(const double* wire_a, const double* wire_b, int n_wires, int wi,
+                      double m[3], double w[3])
+{
+    double d[3], len;
+    int i;
+    for (i = 0; i < 3; ++i) d[i] = wire_b[(size_t)i * n_wires + wi] - wire_a[(size_t)i * n_wires + wi];
+    len = sqrt(dot3(d, d));
+    for (i = 0; i < 3; ++i) {
+        w[i] = d[i] / len;
+        m[i] = (wire_a[(size_t)i * n_wires + wi] + wire_b[(size_t)i * n_wires + wi]) / 2.0;
+    }
+}
+
+/* O8: bounded residual of one wire, Eq. (1): min over the wire's hit
+ * entries (ghosts explicit, R12) of |D - rho_j|, capped at lambda.  *jstar = lowest
+ * index attaining the minimum (-1 when the wire has no entries). */
+static double wire_residual(double D, const double* rho, int j0, int j1, double lambda,
+                            int* jstar, double* rmin_out)
+{
+    int j, js = -1;
+    double rmin = 0.0;
+    for (j = j0; j < j1; ++j) {
+        double r = fabs(D - rho[j]);
+        if (js < 0 || r < rmin) { rmin = r; js = j; }
+    }
+    if (jstar) *jstar = js;
+    if (rmin_out) *rmin_out = rmin;
+    if (js < 0) return lambda;
+    return (rmin < lambda) ? rmin : lambda;
+}
+
+/* One seed of Algorithm 3 given its recorded track. */
+static double seed_rss(const ostate* pts, int n_pts, double h, double c,
+                       const double* wire_a, const double* wire_b, int n_wires,
+                       const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                       int n_fired, double lambda, double* dca_row, int32_t* kstar_row)
+{
+    double rss = 0.0;
+    int i;
+    for (i = 0; i < n_fired; ++i) {            /* O9: increasing wire order */
+        double m[3], w[3], D, e;
+        int ks;
+        wire_line(wire_a, wire_b, n_wires, fired_wire[i], m, w);
+        D = wire_dca(pts, n_pts, h, c, m, w, &ks);
+        e = wire_residual(D, rho, hit_off[i], hit_off[i + 1], lambda, NULL, NULL);
+        rss = rss + e * e;
+        if (dca_row) dca_row[i] = D;
+        if (kstar_row) kstar_row[i] = ks;
+    }
+    return rss;
+}
+
+static double seed_curvature(const double* seeds, int64_t n_seeds, int64_t s, int charge, double bz,
+                             double seed[6])
+{
+    int i;
+    double P;
+    for (i = 0; i < 6; ++i) seed[i] = seeds[(size_t)i * n_seeds + s];
+    P = sqrt(seed[3] * seed[3] + seed[4] * seed[4] + seed[5] * seed[5]);
+    return ORACLE_KAPPA * (double)charge * bz / P;
+}
+
+/* ------------------------------------------------------------------------ */
+/* exported                                                                 */
+/* ------------------------------------------------------------------------ */
+
+int oracle_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_threads(int n)
+{
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
+/* Algorithm 1 alone: track [n_seeds][n_steps+1][6] = x,y,z,Tx,Ty,Tz (NaN beyond n_pts). */
+void oracle_extrapolate(const double* seeds, int64_t n_seeds, int charge, double bz,
+                        double step, int n_steps, double r_stop,
+                        double* track, int32_t* n_pts)
+{
+    int64_t s;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (s = 0; s < n_seeds; ++s) {
+        ostate* pts = (ostate*)malloc(sizeof(ostate) * (size_t)(n_steps + 1));
+        double seed[6];
+        int k, np;
+        (void)seed_curvature(seeds, n_seeds, s, charge, bz, seed);
+        np = record_track(seed, charge, bz, step, n_steps, r_stop, pts);
+        n_pts[s] = np;
+        for (k = 0; k <= n_steps; ++k) {
+            double* o = track + ((size_t)s * (size_t)(n_steps + 1) + (size_t)k) * 6;
+            int i;
+            for (i = 0; i < 3; ++i) {
+                o[i] = (k < np) ? pts[k].x[i] : NAN;
+                o[3 + i] = (k < np) ? pts[k].T[i] : NAN;
+            }
+        }
+        free(pts);
+    }
+}
+
+/* Algorithm 3 over all seeds: rss[n_seeds]; optional dca[n_seeds][n_fired] (signed),
+ * kstar[n_seeds][n_fired], n_pts[n_seeds]. */
+void oracle_scan(const double* seeds, int64_t n_seeds, int charge, double bz,
+                 double step, int n_steps, double r_stop,
+                 const double* wire_a, const double* wire_b, int n_wires,
+                 const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                 int n_fired, double cutoff,
+                 double* rss, double* dca, int32_t* kstar, int32_t* n_pts)
+{
+    int64_t s;
+#pragma omp parallel
+    {
+        ostate* pts = (ostate*)malloc(sizeof(ostate) * (size_t)(n_steps + 1));
+#pragma omp for schedule(dynamic, 16)
+        for (s = 0; s < n_seeds; ++s) {
+            double seed[6];
+            double c = seed_curvature(seeds, n_seeds, s, charge, bz, seed);
+            int np = record_track(seed, charge, bz, step, n_steps, r_stop, pts);
+            if (n_pts) n_pts[s] = np;
+            rss[s] = seed_rss(pts, np, step, c, wire_a, wire_b, n_wires, fired_wire, hit_off, rho,
+                              n_fired, cutoff,
+                              dca ? dca + (size_t)s * (size_t)n_fired : NULL,
+                              kstar ? kstar + (size_t)s * (size_t)n_fired : NULL);
+        }
+        free(pts);
+    }
+}
+
+/* O10 + O11: per partition the lowest-index argmin of rss, then the
+ * classification rule of PAPER.md:83 for that seed: on every fired wire the closest
+ * hit entry is classified iff its residual is < lambda (R13 strict).
+ * best_dca [n_part][n_fired], cls [n_part][n_hits] (0/1). */
+void oracle_select_classify(const double* seeds, int64_t n_seeds, int charge, double bz,
+                            double step, int n_steps, double r_stop,
+                            const double* wire_a, const double* wire_b, int n_wires,
+                            const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                            int n_fired, int n_hits, double cutoff,
+                            const double* rss, const int64_t* part_off, int n_part,
+                            int64_t* best_seed, double* best_rss, double* best_dca, uint8_t* cls)
+{
+    int p;
+    ostate* pts = (ostate*)malloc(sizeof(ostate) * (size_t)(n_steps + 1));
+    for (p = 0; p < n_part; ++p) {
+        int64_t s, b = -1;
+        double seed[6], c;
+        int np, i;
+        for (s = part_off[p]; s < part_off[p + 1]; ++s) {
+            if (b < 0 || rss[s] < rss[b]) b = s;
+        }
+        best_seed[p] = b;
+        memset(cls + (size_t)p * (size_t)n_hits, 0, (size_t)n_hits);
+        if (b < 0) {
+            best_rss[p] = NAN;
+            for (i = 0; i < n_fired; ++i) best_dca[(size_t)p * n_fired + i] = NAN;
+            continue;
+        }
+        best_rss[p] = rss[b];
+        c = seed_curvature(seeds, n_seeds, b, charge, bz, seed);
+        np = record_track(seed, charge, bz, step, n_steps, r_stop, pts);
+        for (i = 0; i < n_fired; ++i) {
+            double m[3], w[3], D, rmin;
+            int js;
+            wire_line(wire_a, wire_b, n_wires, fired_wire[i], m, w);
+            D = wire_dca(pts, np, step, c, m, w, NULL);
+            best_dca[(size_t)p * n_fired + i] = D;
+            (void)wire_residual(D, rho, hit_off[i], hit_off[i + 1], cutoff, &js, &rmin);
+            if (js >= 0 && rmin < cutoff) cls[(size_t)p * (size_t)n_hits + js] = 1;
+        }
+    }
+    free(pts);
+}
+
+/* Single RKN4 step exposed for the pin tests (state = x,y,z,Tx,Ty,Tz; c = kappa q Bz / |p|). */
+void oracle_rkn4_step(double* state6, double h, double c)
+{
+    ostate s;
+    int i;
+    for (i = 0; i < 3; ++i) { s.x[i] = state6[i]; s.T[i] = state6[3 + i]; }
+    rkn4_step(&s, h, c);
+    for (i = 0; i < 3; ++i) { state6[i] = s.x[i]; state6[3 + i] = s.T[i]; }
+}
+
+double oracle_kappa(void) { return ORACLE_KAPPA; }

@@ -1,0 +1,126 @@
+"""ctypes wrapper around oracle/comet_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+reference legs may import this.  It never imports paper_1911_09340_b200.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "comet_oracle.c")
+_LIB = os.path.join(_HERE, "libcomet_oracle.so")
+_lib = None
+
+_F64 = np.ctypeslib.ndpointer(dtype=np.float64, flags="C_CONTIGUOUS")
+_I32 = np.ctypeslib.ndpointer(dtype=np.int32, flags="C_CONTIGUOUS")
+_I64 = np.ctypeslib.ndpointer(dtype=np.int64, flags="C_CONTIGUOUS")
+_U8 = np.ctypeslib.ndpointer(dtype=np.uint8, flags="C_CONTIGUOUS")
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off -fopenmp: one IEEE double operation per written operation."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
+               "-Wall", "-Wextra", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_LIB)
+        c_int, c_i64, c_dbl, vp = ctypes.c_int, ctypes.c_int64, ctypes.c_double, ctypes.c_void_p
+        L.oracle_max_threads.restype = c_int
+        L.oracle_set_threads.argtypes = [c_int]
+        L.oracle_kappa.restype = c_dbl
+        L.oracle_rkn4_step.argtypes = [_F64, c_dbl, c_dbl]
+        L.oracle_extrapolate.argtypes = [_F64, c_i64, c_int, c_dbl, c_dbl, c_int, c_dbl, _F64, _I32]
+        L.oracle_scan.argtypes = [_F64, c_i64, c_int, c_dbl, c_dbl, c_int, c_dbl,
+                                  _F64, _F64, c_int, _I32, _I32, _F64, c_int, c_dbl,
+                                  _F64, vp, vp, vp]
+        L.oracle_select_classify.argtypes = [_F64, c_i64, c_int, c_dbl, c_dbl, c_int, c_dbl,
+                                             _F64, _F64, c_int, _I32, _I32, _F64, c_int, c_int, c_dbl,
+                                             _F64, _I64, c_int, _I64, _F64, _F64, _U8]
+        _lib = L
+    return _lib
+
+
+def max_threads() -> int:
+    return int(lib().oracle_max_threads())
+
+
+def set_threads(n: int) -> None:
+    lib().oracle_set_threads(int(n))
+
+
+def kappa() -> float:
+    return float(lib().oracle_kappa())
+
+
+def rkn4_step(state6, h: float, c: float) -> np.ndarray:
+    s = np.ascontiguousarray(state6, dtype=np.float64).copy()
+    lib().oracle_rkn4_step(s, float(h), float(c))
+    return s
+
+
+def _c(a, dt):
+    return np.ascontiguousarray(a, dtype=dt)
+
+
+def extrapolate(seeds, charge, bz, step, n_steps, r_stop):
+    """Algorithm 1.  seeds [6][S] -> (track [S][n_steps+1][6], n_pts [S])."""
+    seeds = _c(seeds, np.float64)
+    S = seeds.shape[1]
+    track = np.empty((S, n_steps + 1, 6))
+    n_pts = np.empty(S, dtype=np.int32)
+    lib().oracle_extrapolate(seeds, S, int(charge), float(bz), float(step), int(n_steps),
+                             float(r_stop), track, n_pts)
+    return track, n_pts
+
+
+def scan(seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
+         cutoff, want_dca=False, want_kstar=False, want_npts=False):
+    """Algorithm 3 over all seeds -> dict(rss[, dca, kstar, n_pts])."""
+    seeds = _c(seeds, np.float64)
+    wire_a, wire_b = _c(wire_a, np.float64), _c(wire_b, np.float64)
+    fired_wire, hit_off, rho = _c(fired_wire, np.int32), _c(hit_off, np.int32), _c(rho, np.float64)
+    S, W = seeds.shape[1], fired_wire.shape[0]
+    out = {"rss": np.empty(S)}
+    dca = np.empty((S, W)) if want_dca else None
+    ks = np.empty((S, W), dtype=np.int32) if want_kstar else None
+    npt = np.empty(S, dtype=np.int32) if want_npts else None
+    ptr = lambda a: a.ctypes.data_as(ctypes.c_void_p) if a is not None else None
+    lib().oracle_scan(seeds, S, int(charge), float(bz), float(step), int(n_steps), float(r_stop),
+                      wire_a, wire_b, wire_a.shape[1], fired_wire, hit_off, rho, W, float(cutoff),
+                      out["rss"], ptr(dca), ptr(ks), ptr(npt))
+    if want_dca:
+        out["dca"] = dca
+    if want_kstar:
+        out["kstar"] = ks
+    if want_npts:
+        out["n_pts"] = npt
+    return out
+
+
+def select_classify(seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off,
+                    rho, cutoff, rss, part_off):
+    """O10 + O11 -> dict(best_seed [P], best_rss [P], best_dca [P][W], cls [P][H])."""
+    seeds = _c(seeds, np.float64)
+    wire_a, wire_b = _c(wire_a, np.float64), _c(wire_b, np.float64)
+    fired_wire, hit_off, rho = _c(fired_wire, np.int32), _c(hit_off, np.int32), _c(rho, np.float64)
+    rss, part_off = _c(rss, np.float64), _c(part_off, np.int64)
+    S, W, H, P = seeds.shape[1], fired_wire.shape[0], rho.shape[0], part_off.shape[0] - 1
+    best_seed = np.empty(P, dtype=np.int64)
+    best_rss = np.empty(P)
+    best_dca = np.empty((P, W))
+    cls = np.zeros((P, H), dtype=np.uint8)
+    lib().oracle_select_classify(seeds, S, int(charge), float(bz), float(step), int(n_steps),
+                                 float(r_stop), wire_a, wire_b, wire_a.shape[1], fired_wire, hit_off,
+                                 rho, W, H, float(cutoff), rss, part_off, P,
+                                 best_seed, best_rss, best_dca, cls)
+    return {"best_seed": best_seed, "best_rss": best_rss, "best_dca": best_dca, "cls": cls}
