@@ -1,0 +1,165 @@
+/*
+ * comet.h -- C ABI of the B200-native seed x hit scan of arXiv 1911.09340
+ * ("GPU-accelerated event reconstruction for the COMET Phase-I experiment").
+ *
+ * Citations are /root/reference/PAPER.md line numbers; R<n> are the readings listed in
+ * DESIGN.md section 2.  Units: cm, MeV/c, Tesla, charge in units of e.
+ *
+ * Conventions
+ *   - Every function returns COMET_OK (0) or a negative comet_status.  Nothing throws.
+ *   - "dev" pointers are CUDA device memory owned by the caller, 16-byte aligned, valid until
+ *     the work enqueued on `cuda_stream` has completed.  "host" pointers are ordinary host
+ *     memory read or written before the call returns unless stated otherwise.
+ *   - `cuda_stream` is a cudaStream_t cast to void* (NULL = the legacy default stream).
+ *     The device-buffer calls only enqueue work: no host synchronisation, no allocation.
+ *   - A comet_ctx owns a small device workspace; use one ctx per stream.  Calls on different
+ *     ctx objects / streams are independent.
+ *   - There is no CPU implementation behind this interface.
+ */
+#ifndef COMET_H_
+#define COMET_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct comet_ctx comet_ctx;
+
+typedef enum comet_status {
+    COMET_OK = 0,
+    COMET_EINVAL = -1,   /* null pointer, negative size, bad option, limits exceeded */
+    COMET_ENOMEM = -2,   /* device or host allocation failed */
+    COMET_ECUDA = -3     /* a CUDA runtime call failed; see comet_last_cuda_error */
+} comet_status;
+
+/* Seeds per track chunk: the track buffer is laid out in chunks of 32 consecutive seeds
+ * (one warp of lanes), see comet_track_bytes. */
+#define COMET_CHUNK 32
+/* Limits checked by the entry points. */
+#define COMET_MAX_PARTITIONS 64
+#define COMET_MAX_STEPS 4096
+
+/* Options for comet_set_option. */
+#define COMET_OPT_COARSE_SEARCH 1     /* how step B2 (closest recorded state) is found          */
+#define COMET_COARSE_EXHAUSTIVE 0     /*   every recorded point is evaluated      */
+#define COMET_COARSE_PRUNED 1         /*   strided samples + Lipschitz-bounded windows; same k*  */
+
+/* ---- context ---------------------------------------------------------------------------- */
+
+/* Creates a context on CUDA device `cuda_device` (allocates a few MB of device workspace). */
+int comet_create(comet_ctx** out, int cuda_device);
+/* Frees the workspace.  The caller must have synchronised every stream that used the ctx. */
+int comet_destroy(comet_ctx* ctx);
+/* Static, never freed. */
+const char* comet_status_string(int status);
+/* cudaError_t of the last failing CUDA call made through this ctx (0 if none). */
+int comet_last_cuda_error(const comet_ctx* ctx);
+int comet_set_option(comet_ctx* ctx, int option, int value);
+int comet_get_option(const comet_ctx* ctx, int option, int* value);
+
+/* ---- kernel A: track recording (Algorithm 1) ---------------------------- */
+
+/* Bytes of the opaque track buffer for n_seeds seeds and n_steps steps.
+ * Layout (library-defined): two planes, positions X then unit tangents T, each
+ * [n_chunks][n_steps+1][3][32] doubles with n_chunks = ceil(n_seeds/32): component c of
+ * recorded state k of seed s is at ((s/32 * (n_steps+1) + k) * 3 + c) * 32 + s%32.
+ * Returns 0 for invalid arguments. */
+size_t comet_track_bytes(int64_t n_seeds, int32_t n_steps);
+
+/* Every seed (x,p)_0 is extrapolated as a charged particle in the uniform field (0,0,bz):
+ * T_0 = p/|p|, c = kappa*charge*bz/|p| (kappa = 2.99792458, R4), then n_steps classical
+ * Runge-Kutta-Nystrom steps of length step_cm (R1, R2), every state recorded
+ * (PAPER.md:138).  Recording stops at the first recorded state inside the target region
+ * r < r_stop_cm and moving inward (R3); r_stop_cm = 0 never stops.
+ *   seeds       dev, SoA: component j (x,y,z,px,py,pz) of seed s at seeds[j*seed_stride + s]
+ *   seed_stride distance in doubles between components (>= n_seeds)
+ *   track       dev, comet_track_bytes(n_seeds, n_steps) bytes, written
+ *   n_pts       dev [n_seeds], written: number of recorded states, 2..n_steps+1
+ * Arithmetic: fp64, one IEEE operation per operation of the definition (no contraction). */
+int comet_seed_extrapolate(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                           int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                           double r_stop_cm, void* track, int32_t* n_pts, void* cuda_stream);
+
+/* Copies seeds [seed_begin, seed_end) of a track buffer to the canonical layout
+ * out[(s - seed_begin)][k][6] = x,y,z,Tx,Ty,Tz (dev), NaN for k >= n_pts[s]. */
+int comet_track_export(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64_t n_seeds,
+                       int32_t n_steps, int64_t seed_begin, int64_t seed_end, double* out,
+                       void* cuda_stream);
+
+/* ---- kernel B: DCA finding and RSS (Algorithm 2; Eq. (1), :75-77) -------- */
+
+/* For every seed s and fired wire i: the recorded state closest to the wire line (R5, R6;
+ * PAPER.md:165), the virtual-plane iteration with RKN sub-steps from it (R7-R10; PAPER.md:167-184,
+ * :216), the signed distance of closest approach D (R16); then
+ *   rss[s] = sum_i min( min_{j in [hit_off[i], hit_off[i+1])} |D - rho[j]|, cutoff )^2
+ * accumulated in increasing i (Eq. (1); a wire without entries contributes cutoff^2).
+ *   track, n_pts   as written by comet_seed_extrapolate with the same n_seeds, n_steps,
+ *                  charge, bz_tesla, step_cm
+ *   wire_a, wire_b dev, SoA [3][n_wires]: wire endpoints
+ *   fired_wire     dev [n_fired]: indices into the wire table of the wires that have hits (R11)
+ *   hit_off        dev [n_fired+1]: CSR offsets into rho, non-decreasing, hit_off[n_fired] = n_hits
+ *   rho            dev [n_hits]: signed drift distance of each hit entry, +r and -r for the
+ *                  left/right ghosts (R12)
+ *   rss            dev [n_seeds], written
+ *   dca            dev [n_seeds][n_fired] signed D, written; NULL to skip
+ *   kstar          dev [n_seeds][n_fired] index of the closest recorded state; NULL to skip */
+int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64_t n_seeds,
+                  int32_t n_steps, int32_t charge, double bz_tesla, double step_cm,
+                  const double* seeds, int64_t seed_stride,
+                  const double* wire_a, const double* wire_b, int32_t n_wires,
+                  const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                  int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                  double* rss, double* dca, int32_t* kstar, void* cuda_stream);
+
+/* ---- step C: best seed per turn partition and hit classification -------- */
+
+/* For every partition p (seeds [part_off[p], part_off[p+1])): best_seed[p] = lowest-index argmin
+ * of rss (R15), best_rss[p] its value.  That seed is extrapolated again and, on every fired wire,
+ * the hit entry closest to its D (ties -> lowest index) is classified iff |D - rho| < cutoff
+ * (R13): cls[p][j] = 1, all other entries 0.  best_dca[p][i] = D.
+ *   part_off   HOST [n_part+1], non-decreasing, within [0, n_seeds]; read before returning
+ *   best_seed  dev [n_part] (global seed index, -1 for an empty partition), best_rss dev [n_part],
+ *   best_dca   dev [n_part][n_fired], cls dev [n_part][n_hits]
+ * Limits: n_part <= COMET_MAX_PARTITIONS, n_steps <= COMET_MAX_STEPS. */
+int comet_select_and_classify(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                              int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                              double r_stop_cm,
+                              const double* wire_a, const double* wire_b, int32_t n_wires,
+                              const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                              int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                              const double* rss, const int64_t* part_off, int32_t n_part,
+                              int64_t* best_seed, double* best_rss, double* best_dca, uint8_t* cls,
+                              void* cuda_stream);
+
+/* ---- whole event from host buffers ------------------------------------------------------- */
+
+/* Runs A, B and C for one event whose inputs and outputs live in HOST memory (pinned memory makes
+ * the copies asynchronous): copies the inputs to the device, processes the seeds in slabs that fit
+ * `track_budget_bytes` of track workspace (grown inside the ctx when needed, 0 = 4 GiB), copies
+ * best_seed/best_rss/best_dca/cls (and rss if rss_host != NULL) back and synchronises the stream.
+ * All array arguments have the shapes of the device-buffer calls above. */
+int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, int64_t n_seeds,
+                          int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                          double r_stop_cm,
+                          const double* wire_a_host, const double* wire_b_host, int32_t n_wires,
+                          const int32_t* fired_wire_host, const int32_t* hit_off_host,
+                          const double* rho_host, int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                          const int64_t* part_off_host, int32_t n_part, size_t track_budget_bytes,
+                          int64_t* best_seed_host, double* best_rss_host, double* best_dca_host,
+                          uint8_t* cls_host, double* rss_host, void* cuda_stream);
+
+/* ---- measurement helper ------------------------------------------------------------------ */
+
+/* Enqueues a dependent-free DFMA loop on every SM (`iters` FMAs per thread on 8 chains) and
+ * returns the number of FP64 FMA instructions it executes per launch in *n_fma (host).  Timing it
+ * with CUDA events gives the FP64 pipe peak of the device the roofline is quoted against. */
+int comet_fp64_peak_probe(comet_ctx* ctx, int32_t iters, double* sink_dev, double* n_fma,
+                          void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COMET_H_ */

@@ -1,0 +1,317 @@
+"""ctypes binding of libcomet.so (include/comet.h): argument marshalling only.
+
+torch supplies device memory (`tensor.data_ptr()`) and streams (`torch.cuda.Stream.cuda_stream`);
+every step of the path runs inside the library's CUDA kernels.  There is no fallback: a missing
+library or a failing call raises CometError.
+"""
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+EXPORTED_SYMBOLS = [
+    "comet_create", "comet_destroy", "comet_status_string", "comet_last_cuda_error",
+    "comet_set_option", "comet_get_option", "comet_track_bytes", "comet_seed_extrapolate",
+    "comet_track_export", "comet_dca_rss", "comet_select_and_classify", "comet_scan_event_host",
+    "comet_fp64_peak_probe",
+]
+
+COMET_CHUNK = 32
+OPT_COARSE_SEARCH = 1
+COARSE_EXHAUSTIVE = 0
+COARSE_PRUNED = 1
+
+
+class CometError(RuntimeError):
+    pass
+
+
+def lib_path() -> str:
+    return os.path.join(_HERE, "libcomet.so")
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree libcomet.so and declare the signatures of include/comet.h."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = lib_path()
+    if not os.path.exists(path):
+        raise CometError("%s is missing: build it with `python -m paper_1911_09340_b200.build` "
+                         "(there is no CPU fallback)" % path)
+    L = ctypes.CDLL(path)
+    vp, i32, i64, dbl, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double, ctypes.c_size_t
+    L.comet_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int]
+    L.comet_destroy.argtypes = [vp]
+    L.comet_status_string.argtypes = [ctypes.c_int]
+    L.comet_status_string.restype = ctypes.c_char_p
+    L.comet_last_cuda_error.argtypes = [vp]
+    L.comet_set_option.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+    L.comet_get_option.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
+    L.comet_track_bytes.argtypes = [i64, i32]
+    L.comet_track_bytes.restype = sz
+    L.comet_seed_extrapolate.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl, vp, vp, vp]
+    L.comet_track_export.argtypes = [vp, vp, vp, i64, i32, i64, i64, vp, vp]
+    L.comet_dca_rss.argtypes = [vp, vp, vp, i64, i32, i32, dbl, dbl, vp, i64,
+                                vp, vp, i32, vp, vp, vp, i32, i32, dbl, vp, vp, vp, vp]
+    L.comet_select_and_classify.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
+                                            vp, vp, i32, vp, vp, vp, i32, i32, dbl,
+                                            vp, vp, i32, vp, vp, vp, vp, vp]
+    L.comet_scan_event_host.argtypes = [vp, vp, i64, i32, dbl, dbl, i32, dbl,
+                                        vp, vp, i32, vp, vp, vp, i32, i32, dbl,
+                                        vp, i32, sz, vp, vp, vp, vp, vp, vp]
+    L.comet_fp64_peak_probe.argtypes = [vp, i32, vp, ctypes.POINTER(dbl), vp]
+    for name in EXPORTED_SYMBOLS:
+        if name not in ("comet_status_string", "comet_track_bytes"):
+            getattr(L, name).restype = ctypes.c_int
+    _lib = L
+    return L
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _dev(t: Optional[torch.Tensor], dtype, name: str, device) -> int:
+    """data_ptr of a contiguous CUDA tensor of the given dtype on `device` (0 for None)."""
+    if t is None:
+        return 0
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise CometError("%s must be a contiguous CUDA tensor of dtype %s" % (name, dtype))
+    if t.device.index != device:
+        raise CometError("%s is on cuda:%s, the context is on cuda:%d" % (name, t.device.index, device))
+    return int(t.data_ptr())
+
+
+class Comet:
+    """One comet_ctx (one per stream).  Methods mirror the C entry points."""
+
+    def __init__(self, device: int = 0):
+        self._L = load_library()
+        if not torch.cuda.is_available():
+            raise CometError("no CUDA device: the seed x hit scan has no CPU implementation")
+        self.device = int(device)
+        h = ctypes.c_void_p()
+        self._check(self._L.comet_create(ctypes.byref(h), self.device), None)
+        self._h = h
+
+    # -- plumbing ---------------------------------------------------------------------------
+    def _check(self, rc: int, h=True):
+        if rc != 0:
+            msg = self._L.comet_status_string(rc).decode()
+            cu = self._L.comet_last_cuda_error(self._h) if h and getattr(self, "_h", None) else 0
+            raise CometError("libcomet: %s (status %d, cudaError %d)" % (msg, rc, cu))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            torch.cuda.synchronize(self.device)
+            self._L.comet_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_option(self, option: int, value: int):
+        self._check(self._L.comet_set_option(self._h, int(option), int(value)))
+
+    def get_option(self, option: int) -> int:
+        v = ctypes.c_int()
+        self._check(self._L.comet_get_option(self._h, int(option), ctypes.byref(v)))
+        return v.value
+
+    def track_bytes(self, n_seeds: int, n_steps: int) -> int:
+        return int(self._L.comet_track_bytes(int(n_seeds), int(n_steps)))
+
+    def _tdev(self):
+        return torch.device("cuda", self.device)
+
+    # -- kernel A ---------------------------------------------------------------------------
+    def seed_extrapolate(self, seeds, charge, bz, step, n_steps, r_stop, track=None, n_pts=None,
+                         seed_range=None, stream=None):
+        """seeds: CUDA float64 [6][S].  Returns (track uint8 buffer, n_pts int32 [n])."""
+        S = seeds.shape[1]
+        b, e = (0, S) if seed_range is None else seed_range
+        n = e - b
+        base = _dev(seeds, torch.float64, "seeds", self.device)
+        need = self.track_bytes(n, n_steps)
+        if track is None:
+            track = torch.empty(max(need, 16), dtype=torch.uint8, device=self._tdev())
+        elif track.numel() * track.element_size() < need:
+            raise CometError("track buffer too small: %d < %d bytes" % (track.numel() * track.element_size(), need))
+        if n_pts is None:
+            n_pts = torch.empty(n, dtype=torch.int32, device=self._tdev())
+        self._check(self._L.comet_seed_extrapolate(
+            self._h, base + 8 * b, S, n, int(charge), float(bz), float(step), int(n_steps), float(r_stop),
+            int(track.data_ptr()), _dev(n_pts, torch.int32, "n_pts", self.device), _stream_ptr(stream)))
+        return track, n_pts
+
+    def track_export(self, track, n_pts, n_seeds, n_steps, seed_begin=0, seed_end=None, stream=None):
+        seed_end = n_seeds if seed_end is None else seed_end
+        out = torch.empty((seed_end - seed_begin, n_steps + 1, 6), dtype=torch.float64, device=self._tdev())
+        self._check(self._L.comet_track_export(
+            self._h, int(track.data_ptr()), _dev(n_pts, torch.int32, "n_pts", self.device), int(n_seeds),
+            int(n_steps), int(seed_begin), int(seed_end), int(out.data_ptr()), _stream_ptr(stream)))
+        return out
+
+    # -- kernel B ---------------------------------------------------------------------------
+    def dca_rss(self, track, n_pts, seeds, charge, bz, step, n_steps, wire_a, wire_b, fired_wire, hit_off,
+                rho, cutoff, rss=None, want_dca=False, want_kstar=False, seed_range=None, stream=None):
+        S = seeds.shape[1]
+        b, e = (0, S) if seed_range is None else seed_range
+        n = e - b
+        W, H = int(fired_wire.shape[0]), int(rho.shape[0])
+        d = self.device
+        if rss is None:
+            rss = torch.empty(n, dtype=torch.float64, device=self._tdev())
+        dca = torch.empty((n, W), dtype=torch.float64, device=self._tdev()) if want_dca else None
+        ks = torch.empty((n, W), dtype=torch.int32, device=self._tdev()) if want_kstar else None
+        self._check(self._L.comet_dca_rss(
+            self._h, int(track.data_ptr()), _dev(n_pts, torch.int32, "n_pts", d), n, int(n_steps), int(charge),
+            float(bz), float(step), _dev(seeds, torch.float64, "seeds", d) + 8 * b, S,
+            _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
+            int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d),
+            _dev(hit_off, torch.int32, "hit_off", d), _dev(rho, torch.float64, "rho", d), W, H, float(cutoff),
+            _dev(rss, torch.float64, "rss", d), _dev(dca, torch.float64, "dca", d),
+            _dev(ks, torch.int32, "kstar", d), _stream_ptr(stream)))
+        out = {"rss": rss}
+        if want_dca:
+            out["dca"] = dca
+        if want_kstar:
+            out["kstar"] = ks
+        return out
+
+    # -- step C -----------------------------------------------------------------------------
+    def select_and_classify(self, seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
+                            hit_off, rho, cutoff, rss, part_off: Sequence[int], stream=None):
+        S = seeds.shape[1]
+        W, H = int(fired_wire.shape[0]), int(rho.shape[0])
+        po = np.ascontiguousarray(np.asarray(part_off, dtype=np.int64))
+        P = po.shape[0] - 1
+        d, td = self.device, self._tdev()
+        best_seed = torch.empty(P, dtype=torch.int64, device=td)
+        best_rss = torch.empty(P, dtype=torch.float64, device=td)
+        best_dca = torch.empty((P, W), dtype=torch.float64, device=td)
+        cls = torch.empty((P, H), dtype=torch.uint8, device=td)
+        self._check(self._L.comet_select_and_classify(
+            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, int(charge), float(bz), float(step),
+            int(n_steps), float(r_stop),
+            _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
+            int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d),
+            _dev(hit_off, torch.int32, "hit_off", d), _dev(rho, torch.float64, "rho", d), W, H, float(cutoff),
+            _dev(rss, torch.float64, "rss", d), po.ctypes.data, P,
+            int(best_seed.data_ptr()), int(best_rss.data_ptr()), int(best_dca.data_ptr()), int(cls.data_ptr()),
+            _stream_ptr(stream)))
+        return {"best_seed": best_seed, "best_rss": best_rss, "best_dca": best_dca, "cls": cls}
+
+    # -- whole event, device-resident inputs --------------------------------------------------
+    def scan_event(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
+                   hit_off, rho, cutoff, track=None, n_pts=None, rss=None, slab_seeds=None, stream=None):
+        """A, B (per slab of seeds when the track buffer is smaller than the whole set) and C."""
+        S = seeds.shape[1]
+        if slab_seeds is None:
+            slab_seeds = S
+        slab_seeds = max(COMET_CHUNK, (int(slab_seeds) // COMET_CHUNK) * COMET_CHUNK)
+        if rss is None:
+            rss = torch.empty(S, dtype=torch.float64, device=self._tdev())
+        if n_pts is None:
+            n_pts = torch.empty(S, dtype=torch.int32, device=self._tdev())
+        if track is None:
+            track = torch.empty(self.track_bytes(min(S, slab_seeds), n_steps), dtype=torch.uint8, device=self._tdev())
+        for b in range(0, S, slab_seeds):
+            e = min(S, b + slab_seeds)
+            self.seed_extrapolate(seeds, charge, bz, step, n_steps, r_stop, track=track, n_pts=n_pts[b:e],
+                                  seed_range=(b, e), stream=stream)
+            self.dca_rss(track, n_pts[b:e], seeds, charge, bz, step, n_steps, wire_a, wire_b, fired_wire,
+                         hit_off, rho, cutoff, rss=rss[b:e], seed_range=(b, e), stream=stream)
+        out = self.select_and_classify(seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
+                                       hit_off, rho, cutoff, rss, part_off, stream=stream)
+        out["rss"] = rss
+        out["n_pts"] = n_pts
+        return out
+
+    # -- whole event, host buffers ------------------------------------------------------------
+    def scan_event_host(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
+                        hit_off, rho, cutoff, out=None, want_rss=False, track_budget_bytes=0, stream=None):
+        """All arrays are HOST torch tensors (pinned for asynchronous copies) or numpy arrays."""
+        def host(a, dt):
+            t = a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a))
+            if t.is_cuda or t.dtype != dt or not t.is_contiguous():
+                raise CometError("host array must be a contiguous CPU tensor of dtype %s" % dt)
+            return t
+        seeds, wire_a, wire_b = host(seeds, torch.float64), host(wire_a, torch.float64), host(wire_b, torch.float64)
+        fired_wire, hit_off, rho = host(fired_wire, torch.int32), host(hit_off, torch.int32), host(rho, torch.float64)
+        po = host(np.asarray(part_off, dtype=np.int64) if not isinstance(part_off, torch.Tensor) else part_off,
+                  torch.int64)
+        S, W, H, P = seeds.shape[1], fired_wire.shape[0], rho.shape[0], po.shape[0] - 1
+        if out is None:
+            out = {"best_seed": torch.empty(P, dtype=torch.int64).pin_memory(),
+                   "best_rss": torch.empty(P, dtype=torch.float64).pin_memory(),
+                   "best_dca": torch.empty((P, W), dtype=torch.float64).pin_memory(),
+                   "cls": torch.empty((P, H), dtype=torch.uint8).pin_memory()}
+            if want_rss:
+                out["rss"] = torch.empty(S, dtype=torch.float64).pin_memory()
+        rss_ptr = out["rss"].data_ptr() if "rss" in out else 0
+        self._check(self._L.comet_scan_event_host(
+            self._h, seeds.data_ptr(), S, int(charge), float(bz), float(step), int(n_steps), float(r_stop),
+            wire_a.data_ptr(), wire_b.data_ptr(), int(wire_a.shape[1]), fired_wire.data_ptr(), hit_off.data_ptr(),
+            rho.data_ptr(), W, H, float(cutoff), po.data_ptr(), P, int(track_budget_bytes),
+            out["best_seed"].data_ptr(), out["best_rss"].data_ptr(), out["best_dca"].data_ptr(),
+            out["cls"].data_ptr(), rss_ptr, _stream_ptr(stream)))
+        return out
+
+    # -- measurement helper -------------------------------------------------------------------
+    def fp64_peak_probe(self, iters: int, sink=None, stream=None) -> float:
+        """Enqueues the DFMA loop; returns the number of FP64 FMA instructions (thread-level) it runs."""
+        if sink is None:
+            sink = torch.zeros(1, dtype=torch.float64, device=self._tdev())
+        self._sink = sink
+        n = ctypes.c_double()
+        self._check(self._L.comet_fp64_peak_probe(self._h, int(iters), int(sink.data_ptr()), ctypes.byref(n),
+                                                  _stream_ptr(stream)))
+        return n.value
+
+
+_default = {}
+
+
+def _ctx(device=None) -> Comet:
+    device = torch.cuda.current_device() if device is None else int(device)
+    if device not in _default:
+        _default[device] = Comet(device)
+    return _default[device]
+
+
+def seed_extrapolate(seeds, *a, **k):
+    return _ctx(seeds.device.index).seed_extrapolate(seeds, *a, **k)
+
+
+def track_export(track, *a, **k):
+    return _ctx(track.device.index).track_export(track, *a, **k)
+
+
+def dca_rss(track, *a, **k):
+    return _ctx(track.device.index).dca_rss(track, *a, **k)
+
+
+def select_and_classify(seeds, *a, **k):
+    return _ctx(seeds.device.index).select_and_classify(seeds, *a, **k)
+
+
+def scan_event(seeds, *a, **k):
+    return _ctx(seeds.device.index).scan_event(seeds, *a, **k)
+
+
+def scan_event_host(*a, **k):
+    return _ctx().scan_event_host(*a, **k)

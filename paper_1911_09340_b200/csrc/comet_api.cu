@@ -1,0 +1,459 @@
+// comet_api.cu -- C ABI of include/comet.h on top of the sm_100a kernels (argument checks,
+// workspace, launches).  No torch types, no exceptions, no host synchronisation in the
+// device-buffer entry points.
+#include "../../include/comet.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <new>
+#include <stdio.h>
+#include <string.h>
+
+#include "common.cuh"
+#include "dca.cuh"
+#include "extrapolate.cuh"
+#include "select.cuh"
+
+using namespace comet;
+
+struct comet_ctx {
+    int device;
+    int last_cuda;
+    int opt_coarse;
+    int n_sm;
+    // device workspace
+    double* wt;            // wire table [14][wt_cap]
+    int32_t wt_cap;
+    double* pv;            // argmin partials [MAX_PART][SPLIT]
+    int64_t* pi;
+    // host-buffer entry point workspace (grown on demand)
+    void* hbuf;            // one device slab for the event's inputs and outputs
+    size_t hbuf_bytes;
+    void* tbuf;            // track slab
+    size_t tbuf_bytes;
+};
+
+#define CU(ctx, call)                                  \
+    do {                                               \
+        cudaError_t e__ = (call);                      \
+        if (e__ != cudaSuccess) {                      \
+            (ctx)->last_cuda = (int)e__;               \
+            return COMET_ECUDA;                        \
+        }                                              \
+    } while (0)
+
+static int set_device(comet_ctx* ctx)
+{
+    CU(ctx, cudaSetDevice(ctx->device));
+    return COMET_OK;
+}
+
+extern "C" const char* comet_status_string(int status)
+{
+    switch (status) {
+        case COMET_OK: return "ok";
+        case COMET_EINVAL: return "invalid argument";
+        case COMET_ENOMEM: return "out of memory";
+        case COMET_ECUDA: return "CUDA runtime error";
+        default: return "unknown status";
+    }
+}
+
+extern "C" int comet_last_cuda_error(const comet_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
+
+extern "C" int comet_create(comet_ctx** out, int cuda_device)
+{
+    if (!out || cuda_device < 0) return COMET_EINVAL;
+    *out = nullptr;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || cuda_device >= n_dev) return COMET_ECUDA;
+    comet_ctx* ctx = new (std::nothrow) comet_ctx();
+    if (!ctx) return COMET_ENOMEM;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->device = cuda_device;
+    ctx->opt_coarse = COMET_COARSE_EXHAUSTIVE;
+    cudaError_t e = cudaSetDevice(cuda_device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, cuda_device);
+    ctx->wt_cap = 8192;
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->wt, sizeof(double) * COMET_WT_FIELDS * (size_t)ctx->wt_cap);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->pv, sizeof(double) * COMET_MAX_PARTITIONS * COMET_ARGMIN_SPLIT);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->pi, sizeof(int64_t) * COMET_MAX_PARTITIONS * COMET_ARGMIN_SPLIT);
+    // shared-memory opt-ins (done once here, never on the hot path)
+    const int dca_smem = (2 * COMET_KT * 3 * COMET_LANES + COMET_DCA_WARPS * 4 * 32) * (int)sizeof(double);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_select_classify, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
+    if (e != cudaSuccess) {
+        cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi);
+        delete ctx;
+        return e == cudaErrorMemoryAllocation ? COMET_ENOMEM : COMET_ECUDA;
+    }
+    *out = ctx;
+    return COMET_OK;
+}
+
+extern "C" int comet_destroy(comet_ctx* ctx)
+{
+    if (!ctx) return COMET_EINVAL;
+    cudaSetDevice(ctx->device);
+    cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi);
+    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf);
+    delete ctx;
+    return COMET_OK;
+}
+
+extern "C" int comet_set_option(comet_ctx* ctx, int option, int value)
+{
+    if (!ctx) return COMET_EINVAL;
+    if (option == COMET_OPT_COARSE_SEARCH && (value == COMET_COARSE_EXHAUSTIVE || value == COMET_COARSE_PRUNED)) {
+        ctx->opt_coarse = value;
+        return COMET_OK;
+    }
+    return COMET_EINVAL;
+}
+
+extern "C" int comet_get_option(const comet_ctx* ctx, int option, int* value)
+{
+    if (!ctx || !value) return COMET_EINVAL;
+    if (option == COMET_OPT_COARSE_SEARCH) { *value = ctx->opt_coarse; return COMET_OK; }
+    return COMET_EINVAL;
+}
+
+static inline int64_t n_chunks_of(int64_t n_seeds) { return (n_seeds + COMET_LANES - 1) / COMET_LANES; }
+
+extern "C" size_t comet_track_bytes(int64_t n_seeds, int32_t n_steps)
+{
+    if (n_seeds < 0 || n_steps < 1 || n_steps > COMET_MAX_STEPS) return 0;
+    return 2 * sizeof(double) * track_row(n_chunks_of(n_seeds), n_steps + 1, 0);
+}
+
+static inline double* plane_X(void* track) { return (double*)track; }
+static inline double* plane_T(void* track, int64_t n_seeds, int32_t n_steps)
+{
+    return (double*)track + track_row(n_chunks_of(n_seeds), n_steps + 1, 0);
+}
+
+static bool bad_physics(int32_t charge, double bz, double step, int32_t n_steps)
+{
+    return (charge != 1 && charge != -1) || !isfinite(bz) || !(step > 0.0) || !isfinite(step) ||
+           n_steps < 1 || n_steps > COMET_MAX_STEPS;
+}
+
+extern "C" int comet_seed_extrapolate(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                                      int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                                      double r_stop_cm, void* track, int32_t* n_pts, void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
+        !(r_stop_cm >= 0.0))
+        return COMET_EINVAL;
+    if (n_seeds == 0) return COMET_OK;
+    if (!seeds || !track || !n_pts) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    const double qkb = COMET_KAPPA * (double)charge * bz_tesla;
+    const StepK hk = make_stepk_host(step_cm);
+    const int threads = 128;
+    const int64_t n_thr = n_chunks_of(n_seeds) * COMET_LANES;
+    const unsigned blocks = (unsigned)((n_thr + threads - 1) / threads);
+    k_extrapolate<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>(
+        seeds, seed_stride, n_seeds, qkb, hk, n_steps, r_stop_cm * r_stop_cm, plane_X(track),
+        plane_T(track, n_seeds, n_steps), n_pts);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+extern "C" int comet_track_export(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64_t n_seeds,
+                                  int32_t n_steps, int64_t seed_begin, int64_t seed_end, double* out,
+                                  void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || n_steps < 1 || n_steps > COMET_MAX_STEPS || seed_begin < 0 ||
+        seed_end < seed_begin || seed_end > n_seeds)
+        return COMET_EINVAL;
+    if (seed_end == seed_begin) return COMET_OK;
+    if (!track || !n_pts || !out) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    const int64_t total = (seed_end - seed_begin) * (int64_t)(n_steps + 1);
+    const unsigned blocks = (unsigned)min((int64_t)(ctx->n_sm * 16), (total + 255) / 256);
+    k_track_export<<<blocks, 256, 0, (cudaStream_t)cuda_stream>>>(
+        plane_X((void*)track), plane_T((void*)track, n_seeds, n_steps), n_pts, n_steps, seed_begin, seed_end, out);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+static int launch_wire_prep(comet_ctx* ctx, const double* wire_a, const double* wire_b, int32_t n_wires,
+                            const int32_t* fired_wire, int32_t n_fired, cudaStream_t st)
+{
+    if (n_fired > ctx->wt_cap) return COMET_EINVAL;
+    if (n_fired == 0) return COMET_OK;
+    k_wire_prep<<<(n_fired + 127) / 128, 128, 0, st>>>(wire_a, wire_b, n_wires, fired_wire, n_fired, ctx->wt);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+static bool bad_hits(const double* wire_a, const double* wire_b, int32_t n_wires, const int32_t* fired_wire,
+                     const int32_t* hit_off, const double* rho, int32_t n_fired, int32_t n_hits, double cutoff)
+{
+    if (n_wires < 0 || n_fired < 0 || n_hits < 0 || n_fired > n_wires || !(cutoff >= 0.0) || !isfinite(cutoff))
+        return true;
+    if (n_fired > 0 && (!wire_a || !wire_b || !fired_wire || !hit_off)) return true;
+    if (n_hits > 0 && !rho) return true;
+    return false;
+}
+
+extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64_t n_seeds,
+                             int32_t n_steps, int32_t charge, double bz_tesla, double step_cm,
+                             const double* seeds, int64_t seed_stride,
+                             const double* wire_a, const double* wire_b, int32_t n_wires,
+                             const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                             int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                             double* rss, double* dca, int32_t* kstar, void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
+        bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm))
+        return COMET_EINVAL;
+    if (n_seeds == 0) return COMET_OK;
+    if (!track || !n_pts || !seeds || !rss) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, n_fired, st);
+    if (rc) return rc;
+    DcaArgs a;
+    a.X = plane_X((void*)track);
+    a.T = plane_T((void*)track, n_seeds, n_steps);
+    a.n_pts = n_pts;
+    a.n_seeds = n_seeds;
+    a.n_steps = n_steps;
+    a.qkb = COMET_KAPPA * (double)charge * bz_tesla;
+    a.h = step_cm;
+    a.seeds = seeds;
+    a.stride = seed_stride;
+    a.wt = ctx->wt;
+    a.W = n_fired;
+    a.hit_off = hit_off;
+    a.rho = rho;
+    a.lambda = cutoff_cm;
+    a.rss = rss;
+    a.dca = dca;
+    a.kstar = kstar;
+    // wires per warp per pass: spread n_fired evenly over ceil(n_fired/32) passes of 8 warps
+    const int n_pass = (n_fired + COMET_DCA_WARPS * 4 - 1) / (COMET_DCA_WARPS * 4);
+    int wt = n_pass > 0 ? (n_fired + COMET_DCA_WARPS * n_pass - 1) / (COMET_DCA_WARPS * n_pass) : 1;
+    if (wt < 1) wt = 1;
+    const unsigned blocks = (unsigned)n_chunks_of(n_seeds);
+    const int threads = COMET_DCA_WARPS * 32;
+    const size_t smem = (2 * COMET_KT * 3 * COMET_LANES + (size_t)COMET_DCA_WARPS * wt * 32) * sizeof(double);
+    switch (wt) {
+        case 1: k_dca_rss<1><<<blocks, threads, smem, st>>>(a); break;
+        case 2: k_dca_rss<2><<<blocks, threads, smem, st>>>(a); break;
+        case 3: k_dca_rss<3><<<blocks, threads, smem, st>>>(a); break;
+        default: k_dca_rss<4><<<blocks, threads, smem, st>>>(a); break;
+    }
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                                         int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                                         double r_stop_cm,
+                                         const double* wire_a, const double* wire_b, int32_t n_wires,
+                                         const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                         int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                         const double* rss, const int64_t* part_off, int32_t n_part,
+                                         int64_t* best_seed, double* best_rss, double* best_dca, uint8_t* cls,
+                                         void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
+        !(r_stop_cm >= 0.0) ||
+        bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm) ||
+        n_part < 0 || n_part > COMET_MAX_PARTITIONS)
+        return COMET_EINVAL;
+    if (n_part == 0) return COMET_OK;
+    if (!part_off || !best_seed || !best_rss || (n_fired > 0 && !best_dca) || (n_hits > 0 && !cls)) return COMET_EINVAL;
+    PartOff po;
+    memset(&po, 0, sizeof(po));
+    for (int p = 0; p <= n_part; ++p) {
+        po.off[p] = part_off[p];
+        if (part_off[p] < 0 || part_off[p] > n_seeds || (p > 0 && part_off[p] < part_off[p - 1])) return COMET_EINVAL;
+    }
+    if (po.off[n_part] > 0 && (!seeds || !rss)) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, n_fired, st);
+    if (rc) return rc;
+    k_argmin_stage1<<<dim3(COMET_ARGMIN_SPLIT, n_part), COMET_ARGMIN_THREADS, 0, st>>>(rss, po, ctx->pv, ctx->pi);
+    CU(ctx, cudaGetLastError());
+    ClassifyArgs a;
+    a.seeds = seeds;
+    a.stride = seed_stride;
+    a.qkb = COMET_KAPPA * (double)charge * bz_tesla;
+    a.hk = make_stepk_host(step_cm);
+    a.n_steps = n_steps;
+    a.r_stop2 = r_stop_cm * r_stop_cm;
+    a.wt = ctx->wt;
+    a.W = n_fired;
+    a.hit_off = hit_off;
+    a.rho = rho;
+    a.n_hits = n_hits;
+    a.lambda = cutoff_cm;
+    a.pv = ctx->pv;
+    a.pi = ctx->pi;
+    a.best_seed = best_seed;
+    a.best_rss = best_rss;
+    a.best_dca = best_dca;
+    a.cls = cls;
+    const size_t smem = (size_t)(n_steps + 1) * 6 * sizeof(double);
+    k_select_classify<<<n_part, 256, smem, st>>>(a);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// whole event from host buffers
+// ---------------------------------------------------------------------------------------------
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static int grow(comet_ctx* ctx, void** buf, size_t* have, size_t need)
+{
+    if (need <= *have) return COMET_OK;
+    if (*buf) { CU(ctx, cudaFree(*buf)); *buf = nullptr; *have = 0; }
+    cudaError_t e = cudaMalloc(buf, need);
+    if (e != cudaSuccess) { ctx->last_cuda = (int)e; *buf = nullptr; return COMET_ENOMEM; }
+    *have = need;
+    return COMET_OK;
+}
+
+extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, int64_t n_seeds,
+                                     int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                                     double r_stop_cm,
+                                     const double* wire_a_host, const double* wire_b_host, int32_t n_wires,
+                                     const int32_t* fired_wire_host, const int32_t* hit_off_host,
+                                     const double* rho_host, int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                     const int64_t* part_off_host, int32_t n_part, size_t track_budget_bytes,
+                                     int64_t* best_seed_host, double* best_rss_host, double* best_dca_host,
+                                     uint8_t* cls_host, double* rss_host, void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || bad_physics(charge, bz_tesla, step_cm, n_steps) || !(r_stop_cm >= 0.0) ||
+        bad_hits(wire_a_host, wire_b_host, n_wires, fired_wire_host, hit_off_host, rho_host, n_fired, n_hits,
+                 cutoff_cm) ||
+        n_part < 0 || n_part > COMET_MAX_PARTITIONS || (n_seeds > 0 && !seeds_host) ||
+        (n_part > 0 && (!part_off_host || !best_seed_host || !best_rss_host)) ||
+        (n_part > 0 && n_fired > 0 && !best_dca_host) || (n_part > 0 && n_hits > 0 && !cls_host))
+        return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // ---- carve one device slab: inputs then outputs ------------------------------------------
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    const size_t o_seeds = take(sizeof(double) * 6 * (size_t)n_seeds);
+    const size_t o_wa = take(sizeof(double) * 3 * (size_t)n_wires);
+    const size_t o_wb = take(sizeof(double) * 3 * (size_t)n_wires);
+    const size_t o_fw = take(sizeof(int32_t) * (size_t)n_fired);
+    const size_t o_ho = take(sizeof(int32_t) * ((size_t)n_fired + 1));
+    const size_t o_rho = take(sizeof(double) * (size_t)n_hits);
+    const size_t o_npts = take(sizeof(int32_t) * (size_t)n_seeds);
+    const size_t o_rss = take(sizeof(double) * (size_t)n_seeds);
+    const size_t o_bs = take(sizeof(int64_t) * (size_t)n_part);
+    const size_t o_br = take(sizeof(double) * (size_t)n_part);
+    const size_t o_bd = take(sizeof(double) * (size_t)n_part * (size_t)n_fired);
+    const size_t o_cls = take((size_t)n_part * (size_t)n_hits);
+    rc = grow(ctx, &ctx->hbuf, &ctx->hbuf_bytes, off);
+    if (rc) return rc;
+    char* B = (char*)ctx->hbuf;
+    double* d_seeds = (double*)(B + o_seeds);
+    double* d_wa = (double*)(B + o_wa);
+    double* d_wb = (double*)(B + o_wb);
+    int32_t* d_fw = (int32_t*)(B + o_fw);
+    int32_t* d_ho = (int32_t*)(B + o_ho);
+    double* d_rho = (double*)(B + o_rho);
+    int32_t* d_npts = (int32_t*)(B + o_npts);
+    double* d_rss = (double*)(B + o_rss);
+    int64_t* d_bs = (int64_t*)(B + o_bs);
+    double* d_br = (double*)(B + o_br);
+    double* d_bd = (double*)(B + o_bd);
+    uint8_t* d_cls = (uint8_t*)(B + o_cls);
+    // ---- slab of seeds per A+B round, bounded by the track budget ----------------------------
+    if (track_budget_bytes == 0) track_budget_bytes = (size_t)4 << 30;
+    const size_t per_chunk = comet_track_bytes(COMET_LANES, n_steps);
+    int64_t slab_chunks = (int64_t)(track_budget_bytes / per_chunk);
+    if (slab_chunks < 1) slab_chunks = 1;
+    const int64_t total_chunks = n_chunks_of(n_seeds);
+    if (slab_chunks > total_chunks) slab_chunks = total_chunks;
+    rc = grow(ctx, &ctx->tbuf, &ctx->tbuf_bytes, (size_t)slab_chunks * per_chunk);
+    if (rc) return rc;
+    // ---- H2D ---------------------------------------------------------------------------------
+    if (n_seeds) CU(ctx, cudaMemcpyAsync(d_seeds, seeds_host, sizeof(double) * 6 * (size_t)n_seeds, cudaMemcpyHostToDevice, st));
+    if (n_fired) {
+        CU(ctx, cudaMemcpyAsync(d_wa, wire_a_host, sizeof(double) * 3 * (size_t)n_wires, cudaMemcpyHostToDevice, st));
+        CU(ctx, cudaMemcpyAsync(d_wb, wire_b_host, sizeof(double) * 3 * (size_t)n_wires, cudaMemcpyHostToDevice, st));
+        CU(ctx, cudaMemcpyAsync(d_fw, fired_wire_host, sizeof(int32_t) * (size_t)n_fired, cudaMemcpyHostToDevice, st));
+        CU(ctx, cudaMemcpyAsync(d_ho, hit_off_host, sizeof(int32_t) * ((size_t)n_fired + 1), cudaMemcpyHostToDevice, st));
+    }
+    if (n_hits) CU(ctx, cudaMemcpyAsync(d_rho, rho_host, sizeof(double) * (size_t)n_hits, cudaMemcpyHostToDevice, st));
+    // ---- A + B per slab, then C --------------------------------------------------------------
+    const int64_t slab_seeds = slab_chunks * COMET_LANES;
+    for (int64_t s0 = 0; s0 < n_seeds; s0 += slab_seeds) {
+        const int64_t ns = (n_seeds - s0 < slab_seeds) ? (n_seeds - s0) : slab_seeds;
+        rc = comet_seed_extrapolate(ctx, d_seeds + s0, n_seeds, ns, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+                                    ctx->tbuf, d_npts + s0, st);
+        if (rc) return rc;
+        rc = comet_dca_rss(ctx, ctx->tbuf, d_npts + s0, ns, n_steps, charge, bz_tesla, step_cm, d_seeds + s0, n_seeds,
+                           d_wa, d_wb, n_wires, d_fw, d_ho, d_rho, n_fired, n_hits, cutoff_cm, d_rss + s0, nullptr,
+                           nullptr, st);
+        if (rc) return rc;
+    }
+    rc = comet_select_and_classify(ctx, d_seeds, n_seeds, n_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+                                   d_wa, d_wb, n_wires, d_fw, d_ho, d_rho, n_fired, n_hits, cutoff_cm, d_rss,
+                                   part_off_host, n_part, d_bs, d_br, d_bd, d_cls, st);
+    if (rc) return rc;
+    // ---- D2H ---------------------------------------------------------------------------------
+    if (n_part) {
+        CU(ctx, cudaMemcpyAsync(best_seed_host, d_bs, sizeof(int64_t) * (size_t)n_part, cudaMemcpyDeviceToHost, st));
+        CU(ctx, cudaMemcpyAsync(best_rss_host, d_br, sizeof(double) * (size_t)n_part, cudaMemcpyDeviceToHost, st));
+        if (n_fired) CU(ctx, cudaMemcpyAsync(best_dca_host, d_bd, sizeof(double) * (size_t)n_part * n_fired, cudaMemcpyDeviceToHost, st));
+        if (n_hits) CU(ctx, cudaMemcpyAsync(cls_host, d_cls, (size_t)n_part * n_hits, cudaMemcpyDeviceToHost, st));
+    }
+    if (rss_host && n_seeds) CU(ctx, cudaMemcpyAsync(rss_host, d_rss, sizeof(double) * (size_t)n_seeds, cudaMemcpyDeviceToHost, st));
+    CU(ctx, cudaStreamSynchronize(st));
+    return COMET_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// FP64 pipe peak probe
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_fp64_probe(int iters, double* sink)
+{
+    double a0 = threadIdx.x * 1e-9, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0;
+    double a4 = a0 + 4.0, a5 = a0 + 5.0, a6 = a0 + 6.0, a7 = a0 + 7.0;
+    const double m = 0.999999999, b = 1e-12;
+#pragma unroll 1
+    for (int i = 0; i < iters; i += 8) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            a0 = fma(a0, m, b); a1 = fma(a1, m, b); a2 = fma(a2, m, b); a3 = fma(a3, m, b);
+            a4 = fma(a4, m, b); a5 = fma(a5, m, b); a6 = fma(a6, m, b); a7 = fma(a7, m, b);
+        }
+    }
+    const double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+    if (r == 123.456) sink[0] = r;          // never true: keeps the chains alive
+}
+
+extern "C" int comet_fp64_peak_probe(comet_ctx* ctx, int32_t iters, double* sink_dev, double* n_fma, void* cuda_stream)
+{
+    if (!ctx || iters < 8 || !sink_dev) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    iters = (iters + 7) / 8 * 8;
+    const int blocks = ctx->n_sm * 8, threads = 256;
+    k_fp64_probe<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>(iters, sink_dev);
+    CU(ctx, cudaGetLastError());
+    if (n_fma) *n_fma = (double)blocks * threads * (double)iters * 8.0;
+    return COMET_OK;
+}

@@ -1,0 +1,180 @@
+// common.cuh -- shared device helpers of the CUDA seed x hit scan (sm_100a).
+//
+// Arithmetic policy.  Everything that ends up in a result (track points, k*, DCA, residuals,
+// RSS) is computed with one IEEE-754 double operation per operation of the definition in
+// DESIGN.md section 2, in the order written there -- the __d*_rn intrinsics are never contracted
+// into FMAs by nvcc -- so the results do not depend on compiler flags or on the kernel variant.
+// Only the coarse closest-point *shortlist* (dca.cuh) uses FMAs; its choice is re-decided with
+// the exact distance before it is used.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define COMET_KAPPA 2.99792458      // (MeV/c)/(T cm): "0.3 B" of PAPER.md:319 Eq. (2), reading R4
+#define COMET_TOL_CM 1e-9           // TOLERANCE of PAPER.md:173, reading R9
+#define COMET_MAX_ITER 16
+#define COMET_DEN_MIN 1e-12
+#define COMET_LANES 32              // seeds per track chunk
+
+namespace comet {
+
+__device__ __forceinline__ double xmul(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ double xadd(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ double xsub(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ double xdiv(double a, double b) { return __ddiv_rn(a, b); }
+__device__ __forceinline__ double xsqrt(double a) { return __dsqrt_rn(a); }
+// a0*b0 + a1*b1 + a2*b2 evaluated left to right
+__device__ __forceinline__ double xdot3(double a0, double a1, double a2, double b0, double b1, double b2)
+{
+    return xadd(xadd(xmul(a0, b0), xmul(a1, b1)), xmul(a2, b2));
+}
+
+struct State {          // one recorded track parameter: position (cm) and unit tangent
+    double x0, x1, x2, t0, t1, t2;
+};
+
+// Step constants for a step of signed length h: h, h/2, h*h/6, h/6 (each one IEEE operation).
+struct StepK {
+    double h, hh, hh6, h6;
+};
+__host__ __device__ __forceinline__ StepK make_stepk_host(double h)
+{
+    StepK k;
+    k.h = h;
+    k.hh = h / 2.0;
+    k.hh6 = (h * h) / 6.0;
+    k.h6 = h / 6.0;
+    return k;
+}
+__device__ __forceinline__ StepK make_stepk(double h)
+{
+    StepK k;
+    k.h = h;
+    k.hh = xmul(h, 0.5);                 // == h / 2.0 exactly
+    k.hh6 = xdiv(xmul(h, h), 6.0);
+    k.h6 = xdiv(h, 6.0);
+    return k;
+}
+
+// One classical 4th-order Runge-Kutta-Nystrom step in the uniform field (0,0,B_z)
+// (reading R1):  f(T) = c (T_y, -T_x, 0),
+//   k1=f(T) k2=f(T+h/2 k1) k3=f(T+h/2 k2) k4=f(T+h k3)
+//   x' = x + h T + h^2/6 (k1+k2+k3)      T' = T + h/6 (k1 + 2 k2 + 2 k3 + k4)
+// The z components of k are zero: x2' = x2 + h T2, T2' = T2.  T is not renormalised.
+__device__ __forceinline__ void rkn4_step(State& s, const StepK& k, double c)
+{
+    const double k1x = xmul(c, s.t1), k1y = -xmul(c, s.t0);
+    double ax = xadd(s.t0, xmul(k.hh, k1x)), ay = xadd(s.t1, xmul(k.hh, k1y));
+    const double k2x = xmul(c, ay), k2y = -xmul(c, ax);
+    ax = xadd(s.t0, xmul(k.hh, k2x));
+    ay = xadd(s.t1, xmul(k.hh, k2y));
+    const double k3x = xmul(c, ay), k3y = -xmul(c, ax);
+    ax = xadd(s.t0, xmul(k.h, k3x));
+    ay = xadd(s.t1, xmul(k.h, k3y));
+    const double k4x = xmul(c, ay), k4y = -xmul(c, ax);
+    s.x0 = xadd(xadd(s.x0, xmul(k.h, s.t0)), xmul(k.hh6, xadd(xadd(k1x, k2x), k3x)));
+    s.x1 = xadd(xadd(s.x1, xmul(k.h, s.t1)), xmul(k.hh6, xadd(xadd(k1y, k2y), k3y)));
+    s.x2 = xadd(s.x2, xmul(k.h, s.t2));
+    s.t0 = xadd(s.t0, xmul(k.h6, xadd(xadd(xadd(k1x, xmul(2.0, k2x)), xmul(2.0, k3x)), k4x)));
+    s.t1 = xadd(s.t1, xmul(k.h6, xadd(xadd(xadd(k1y, xmul(2.0, k2y)), xmul(2.0, k3y)), k4y)));
+}
+
+// Seed -> initial state and curvature constant c = kappa q B_z / |p| (A1; qkb = kappa*q*B_z).
+__device__ __forceinline__ double seed_init(const double* __restrict__ seeds, int64_t stride, int64_t s,
+                                            double qkb, State& st)
+{
+    const double px = seeds[3 * stride + s], py = seeds[4 * stride + s], pz = seeds[5 * stride + s];
+    const double P = xsqrt(xdot3(px, py, pz, px, py, pz));
+    st.x0 = seeds[s];
+    st.x1 = seeds[stride + s];
+    st.x2 = seeds[2 * stride + s];
+    st.t0 = xdiv(px, P);
+    st.t1 = xdiv(py, P);
+    st.t2 = xdiv(pz, P);
+    return xdiv(qkb, P);
+}
+
+// target region test of reading R3 on a recorded state
+__device__ __forceinline__ bool in_target_region(const State& s, double r_stop2)
+{
+    const double r2 = xadd(xmul(s.x0, s.x0), xmul(s.x1, s.x1));
+    const double rad = xadd(xmul(s.x0, s.t0), xmul(s.x1, s.t1));
+    return (r2 < r_stop2) && (rad < 0.0);
+}
+
+// Track buffer: plane [n_chunks][n_rows][3][32]; index of (chunk, k, component 0, lane 0).
+__device__ __host__ __forceinline__ size_t track_row(int64_t chunk, int32_t n_rows, int32_t k)
+{
+    return ((size_t)chunk * (size_t)n_rows + (size_t)k) * (size_t)(3 * COMET_LANES);
+}
+
+// Exact wire line (O4): unit direction w and midpoint m.
+struct WireLine {
+    double m0, m1, m2, w0, w1, w2;
+};
+
+// exact squared perpendicular distance from the wire line to x (O4/O5)
+__device__ __forceinline__ double perp2_exact(double x0, double x1, double x2, const WireLine& wl,
+                                              double& u0, double& u1, double& u2)
+{
+    const double d0 = xsub(x0, wl.m0), d1 = xsub(x1, wl.m1), d2 = xsub(x2, wl.m2);
+    const double t = xdot3(d0, d1, d2, wl.w0, wl.w1, wl.w2);
+    u0 = xsub(d0, xmul(t, wl.w0));
+    u1 = xsub(d1, xmul(t, wl.w1));
+    u2 = xsub(d2, xmul(t, wl.w2));
+    return xdot3(u0, u1, u2, u0, u1, u2);
+}
+
+// O6 + O7: virtual-plane iteration from recorded state `s` (index kstar of n_pts) and signed DCA.
+__device__ __forceinline__ double fine_dca(State s, int kstar, int n_pts, double h, double c,
+                                           const WireLine& wl)
+{
+    const double lo = (kstar > 0) ? -h : 0.0;
+    const double hi = (kstar < n_pts - 1) ? h : 0.0;
+    double sigma = 0.0;
+#pragma unroll 1
+    for (int it = 0; it < COMET_MAX_ITER; ++it) {
+        const double tw = xdot3(s.t0, s.t1, s.t2, wl.w0, wl.w1, wl.w2);
+        const double n0 = xsub(s.t0, xmul(tw, wl.w0));
+        const double n1 = xsub(s.t1, xmul(tw, wl.w1));
+        const double n2 = xsub(s.t2, xmul(tw, wl.w2));
+        const double den = xdot3(s.t0, s.t1, s.t2, n0, n1, n2);
+        if (den < COMET_DEN_MIN) break;
+        const double mx0 = xsub(wl.m0, s.x0), mx1 = xsub(wl.m1, s.x1), mx2 = xsub(wl.m2, s.x2);
+        double delta = xdiv(xdot3(mx0, mx1, mx2, n0, n1, n2), den);
+        double target = xadd(sigma, delta);
+        if (target < lo) target = lo;
+        if (target > hi) target = hi;
+        delta = xsub(target, sigma);
+        if (fabs(delta) < COMET_TOL_CM) break;
+        const StepK k = make_stepk(delta);
+        rkn4_step(s, k, c);
+        sigma = xadd(sigma, delta);
+    }
+    double u0, u1, u2;
+    const double d2 = perp2_exact(s.x0, s.x1, s.x2, wl, u0, u1, u2);
+    const double c0 = xsub(xmul(s.t1, wl.w2), xmul(s.t2, wl.w1));
+    const double c1 = xsub(xmul(s.t2, wl.w0), xmul(s.t0, wl.w2));
+    const double c2 = xsub(xmul(s.t0, wl.w1), xmul(s.t1, wl.w0));
+    const double side = xdot3(u0, u1, u2, c0, c1, c2);
+    const double dist = xsqrt(d2);
+    return (side >= 0.0) ? dist : -dist;
+}
+
+// O8: bounded residual of one wire; *jstar = lowest entry index attaining the minimum (-1: none).
+__device__ __forceinline__ double wire_residual(double D, const double* __restrict__ rho, int j0, int j1,
+                                                double lambda, int* jstar, double* rmin_out)
+{
+    int js = -1;
+    double rmin = 0.0;
+    for (int j = j0; j < j1; ++j) {
+        const double r = fabs(xsub(D, __ldg(rho + j)));
+        if (js < 0 || r < rmin) { rmin = r; js = j; }
+    }
+    if (jstar) *jstar = js;
+    if (rmin_out) *rmin_out = rmin;
+    if (js < 0) return lambda;
+    return (rmin < lambda) ? rmin : lambda;
+}
+
+}  // namespace comet

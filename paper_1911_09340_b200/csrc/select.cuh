@@ -1,0 +1,144 @@
+// select.cuh -- step C: per-partition argmin of RSS (reading R15) and hit
+// classification for the winning seed (reading R13), sm_100a.
+#pragma once
+#include "common.cuh"
+
+namespace comet {
+
+struct PartOff {
+    int64_t off[65];            // COMET_MAX_PARTITIONS + 1
+};
+
+#define COMET_ARGMIN_SPLIT 64   // CTAs per partition in the first argmin stage
+#define COMET_ARGMIN_THREADS 256
+
+// (value, index) ordering of R15: smaller rss wins, equal rss -> lower index.  NaN never wins
+// against a number (the comparison is false), exactly as the serial scan "rss[s] < rss[b]".
+__device__ __forceinline__ void argmin_merge(double& v, int64_t& i, double v2, int64_t i2)
+{
+    if (i2 >= 0 && (i < 0 || v2 < v || (v2 == v && i2 < i))) { v = v2; i = i2; }
+}
+
+// A serial scan keeps the first index whose value is strictly smaller than every earlier one.
+// With NaNs: "rss[s] < rss[b]" is false when either is NaN, so a NaN at the first position stays
+// the winner.  We reproduce that by treating the first element of the partition as the initial
+// winner and merging only strictly smaller values; ties resolve to the lower index.
+__global__ void __launch_bounds__(COMET_ARGMIN_THREADS)
+k_argmin_stage1(const double* __restrict__ rss, PartOff po, double* __restrict__ pv, int64_t* __restrict__ pi)
+{
+    const int p = blockIdx.y;
+    const int64_t lo = po.off[p], hi = po.off[p + 1];
+    const int64_t n = hi - lo;
+    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
+    const int64_t b = lo + per * blockIdx.x, e = min(hi, b + per);
+    double v = 0.0;
+    int64_t idx = -1;
+    for (int64_t s = b + threadIdx.x; s < e; s += blockDim.x) {
+        const double r = rss[s];
+        if (idx < 0 || r < v) { v = r; idx = s; }       // increasing s per thread: ties keep lower s
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        const double v2 = __shfl_down_sync(0xffffffffu, v, o);
+        const int64_t i2 = __shfl_down_sync(0xffffffffu, idx, o);
+        argmin_merge(v, idx, v2, i2);
+    }
+    __shared__ double sv[COMET_ARGMIN_THREADS / 32];
+    __shared__ int64_t si[COMET_ARGMIN_THREADS / 32];
+    if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = v; si[threadIdx.x >> 5] = idx; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < COMET_ARGMIN_THREADS / 32; ++w) argmin_merge(v, idx, sv[w], si[w]);
+        pv[p * gridDim.x + blockIdx.x] = v;
+        pi[p * gridDim.x + blockIdx.x] = idx;
+    }
+}
+
+struct ClassifyArgs {
+    const double* seeds;
+    int64_t stride;
+    double qkb;
+    StepK hk;
+    int32_t n_steps;
+    double r_stop2;
+    const double* wt;          // [14][W] from k_wire_prep
+    int32_t W;
+    const int32_t* hit_off;
+    const double* rho;
+    int32_t n_hits;
+    double lambda;
+    const double* pv;          // stage-1 partial minima [n_part][COMET_ARGMIN_SPLIT]
+    const int64_t* pi;
+    int64_t* best_seed;
+    double* best_rss;
+    double* best_dca;
+    uint8_t* cls;
+};
+
+// One CTA per partition: finish the argmin, re-extrapolate the winning seed into shared memory
+// (state k at sm[k*6..]), then one thread per fired wire does O5..O8 + O11 in exact arithmetic.
+__global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
+{
+    extern __shared__ __align__(16) double sm[];       // [(n_steps+1)][6]
+    __shared__ int64_t s_best;
+    __shared__ int32_t s_np;
+    __shared__ double s_c;
+    const int p = blockIdx.x;
+    uint8_t* cls = a.cls + (size_t)p * a.n_hits;
+    for (int j = threadIdx.x; j < a.n_hits; j += blockDim.x) cls[j] = 0;
+    if (threadIdx.x == 0) {
+        double v = 0.0;
+        int64_t idx = -1;
+        for (int b = 0; b < COMET_ARGMIN_SPLIT; ++b)
+            argmin_merge(v, idx, a.pv[p * COMET_ARGMIN_SPLIT + b], a.pi[p * COMET_ARGMIN_SPLIT + b]);
+        s_best = idx;
+        a.best_seed[p] = idx;
+        a.best_rss[p] = (idx >= 0) ? v : __longlong_as_double(0x7ff8000000000000LL);
+        if (idx >= 0) {
+            State st;
+            const double c = seed_init(a.seeds, a.stride, idx, a.qkb, st);
+            s_c = c;
+            int32_t np = a.n_steps + 1;
+            sm[0] = st.x0; sm[1] = st.x1; sm[2] = st.x2; sm[3] = st.t0; sm[4] = st.t1; sm[5] = st.t2;
+            for (int32_t k = 1; k <= a.n_steps; ++k) {
+                rkn4_step(st, a.hk, c);
+                double* o = sm + (size_t)k * 6;
+                o[0] = st.x0; o[1] = st.x1; o[2] = st.x2; o[3] = st.t0; o[4] = st.t1; o[5] = st.t2;
+                if (a.r_stop2 > 0.0 && in_target_region(st, a.r_stop2)) { np = k + 1; break; }
+            }
+            s_np = np;
+        }
+    }
+    __syncthreads();
+    const int64_t best = s_best;
+    const int W = a.W;
+    if (best < 0) {
+        for (int i = threadIdx.x; i < W; i += blockDim.x)
+            a.best_dca[(size_t)p * W + i] = __longlong_as_double(0x7ff8000000000000LL);
+        return;
+    }
+    const int32_t np = s_np;
+    const double c = s_c;
+    for (int i = threadIdx.x; i < W; i += blockDim.x) {
+        WireLine wl;
+        wl.m0 = a.wt[i]; wl.m1 = a.wt[W + i]; wl.m2 = a.wt[2 * W + i];
+        wl.w0 = a.wt[3 * W + i]; wl.w1 = a.wt[4 * W + i]; wl.w2 = a.wt[5 * W + i];
+        int ks = 0;
+        double bd = 0.0;
+        for (int k = 0; k < np; ++k) {
+            double u0, u1, u2;
+            const double d2 = perp2_exact(sm[k * 6], sm[k * 6 + 1], sm[k * 6 + 2], wl, u0, u1, u2);
+            if (k == 0 || d2 < bd) { bd = d2; ks = k; }
+        }
+        State st;
+        st.x0 = sm[ks * 6]; st.x1 = sm[ks * 6 + 1]; st.x2 = sm[ks * 6 + 2];
+        st.t0 = sm[ks * 6 + 3]; st.t1 = sm[ks * 6 + 4]; st.t2 = sm[ks * 6 + 5];
+        const double D = fine_dca(st, ks, np, a.hk.h, c, wl);
+        a.best_dca[(size_t)p * W + i] = D;
+        int js;
+        double rmin;
+        (void)wire_residual(D, a.rho, a.hit_off[i], a.hit_off[i + 1], a.lambda, &js, &rmin);
+        if (js >= 0 && rmin < a.lambda) cls[js] = 1;
+    }
+}
+
+}  // namespace comet

@@ -1,0 +1,291 @@
+"""CUDA path vs CPU oracle, element by element, through the C ABI (needs one B200).
+
+Bars (BASELINE.json north_star; R23):
+  * n_pts, k*, best seed, classified set: identical;
+  * track points: the CUDA extrapolator performs the definition's IEEE operations one by one, so
+    they are compared for bit equality (and reported), with 1e-12 relative as the hard bar;
+  * DCA: |delta| <= 1e-9 * max(|ref|, 1e-3 cm); RSS: 1e-9 relative.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from comet_synth import event_seeds, make_config, truth_seed  # noqa: E402
+from oracle import comet_oracle as O  # noqa: E402
+
+DCA_REL, DCA_FLOOR, RSS_REL = 1e-9, 1e-3, 1e-9
+
+
+@pytest.fixture(scope="module")
+def comet():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_1911_09340_b200 import Comet
+    from paper_1911_09340_b200.build import build
+    build()
+    c = Comet(0)
+    yield c
+    c.close()
+
+
+def _dev(a, dt=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dt is not None:
+        t = t.to(dt)
+    return t.cuda()
+
+
+class DevEvent:
+    def __init__(self, ev, seeds):
+        self.ev = ev
+        self.seeds_h = np.ascontiguousarray(seeds)
+        self.seeds = _dev(seeds)
+        self.wire_a, self.wire_b = _dev(ev.geom.wire_a), _dev(ev.geom.wire_b)
+        self.fired, self.hit_off, self.rho = _dev(ev.fired_wire), _dev(ev.hit_off), _dev(ev.rho)
+
+    def phys(self):
+        ev = self.ev
+        return (ev.charge, ev.bz, ev.step, ev.n_steps)
+
+    def hits(self):
+        return (self.wire_a, self.wire_b, self.fired, self.hit_off, self.rho)
+
+
+def _oracle_scan(ev, seeds, cutoff=None, r_stop=None, **kw):
+    return O.scan(seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop if r_stop is None else r_stop,
+                  ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho,
+                  ev.cutoff if cutoff is None else cutoff, **kw)
+
+
+def _check_dca(got, ref):
+    tol = DCA_REL * np.maximum(np.abs(ref), DCA_FLOOR)
+    bad = np.abs(got - ref) > tol
+    assert not bad.any(), "DCA mismatch: %d of %d, worst %.3e" % (bad.sum(), bad.size, np.abs(got - ref).max())
+
+
+def _check_rss(got, ref):
+    rel = np.abs(got - ref) / np.maximum(np.abs(ref), 1e-300)
+    assert rel.max() <= RSS_REL, "RSS mismatch: worst relative %.3e" % rel.max()
+
+
+# ------------------------------------------------------------------------------------------------
+# kernel A
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("r_stop", [50.0, 0.0])
+def test_extrapolate_matches_oracle_cfg0(comet, cfg0_event, r_stop):
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev)
+    seeds = np.ascontiguousarray(seeds[:, :1000])           # 31 full chunks + a ragged tail of 8
+    d = DevEvent(ev, seeds)
+    track, n_pts = comet.seed_extrapolate(d.seeds, ev.charge, ev.bz, ev.step, ev.n_steps, r_stop)
+    got = comet.track_export(track, n_pts, seeds.shape[1], ev.n_steps).cpu().numpy()
+    ref, ref_n = O.extrapolate(seeds, ev.charge, ev.bz, ev.step, ev.n_steps, r_stop)
+    np.testing.assert_array_equal(n_pts.cpu().numpy(), ref_n)
+    assert np.array_equal(np.isnan(got), np.isnan(ref))
+    m = ~np.isnan(ref)
+    np.testing.assert_allclose(got[m], ref[m], rtol=1e-12, atol=1e-12)
+    assert np.array_equal(got[m], ref[m]), "track not bit-identical (max |d| %.3e)" % np.abs(got[m] - ref[m]).max()
+
+
+def test_extrapolate_seed_range_and_positron(comet, cfg1_event):
+    ev = cfg1_event
+    seeds, _ = event_seeds(ev, shape=(4, 4, 4, 5))          # 3 * 320 seeds
+    d = DevEvent(ev, seeds)
+    S = seeds.shape[1]
+    b, e = 96, 96 + 333
+    track, n_pts = comet.seed_extrapolate(d.seeds, +1, 0.7, ev.step, ev.n_steps, 0.0, seed_range=(b, e))
+    got = comet.track_export(track, n_pts, e - b, ev.n_steps).cpu().numpy()
+    ref, ref_n = O.extrapolate(np.ascontiguousarray(seeds[:, b:e]), +1, 0.7, ev.step, ev.n_steps, 0.0)
+    np.testing.assert_array_equal(n_pts.cpu().numpy(), ref_n)
+    assert np.array_equal(got, ref)
+    assert S == 960
+
+
+# ------------------------------------------------------------------------------------------------
+# kernel B
+# ------------------------------------------------------------------------------------------------
+def _run_b(comet, d, cutoff=None, r_stop=None, **kw):
+    ev = d.ev
+    r_stop = ev.r_stop if r_stop is None else r_stop
+    track, n_pts = comet.seed_extrapolate(d.seeds, ev.charge, ev.bz, ev.step, ev.n_steps, r_stop)
+    out = comet.dca_rss(track, n_pts, d.seeds, *d.phys(), *d.hits(), ev.cutoff if cutoff is None else cutoff,
+                        want_dca=True, want_kstar=True, **kw)
+    torch.cuda.synchronize()
+    return {k: v.cpu().numpy() for k, v in out.items()}, n_pts.cpu().numpy()
+
+
+@pytest.mark.parametrize("r_stop", [50.0, 0.0])
+def test_dca_rss_matches_oracle_cfg0_full(comet, cfg0_event, r_stop):
+    """All 8192 seeds x 32 wires of configs[0]: 256 chunks, 1 pass of 32 wires."""
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev)
+    d = DevEvent(ev, seeds)
+    got, n_pts = _run_b(comet, d, r_stop=r_stop)
+    ref = _oracle_scan(ev, seeds, r_stop=r_stop, want_dca=True, want_kstar=True, want_npts=True)
+    np.testing.assert_array_equal(n_pts, ref["n_pts"])
+    np.testing.assert_array_equal(got["kstar"], ref["kstar"])
+    _check_dca(got["dca"], ref["dca"])
+    _check_rss(got["rss"], ref["rss"])
+    # stronger than the bar: same operations in the same order
+    assert np.array_equal(got["dca"], ref["dca"])
+    assert np.array_equal(got["rss"], ref["rss"])
+
+
+def test_dca_rss_cfg1_ragged(comet, cfg1_event):
+    """71 fired wires (3 passes of 24), truth seeds first, 2000-odd seeds with a ragged last chunk."""
+    ev = cfg1_event
+    seeds, _ = event_seeds(ev)
+    ts = np.stack([truth_seed(ev, i) for i in range(len(ev.partitions))], axis=1)
+    seeds = np.ascontiguousarray(np.concatenate([ts, seeds[:, ::191]], axis=1))
+    assert seeds.shape[1] % 32 != 0
+    d = DevEvent(ev, seeds)
+    got, n_pts = _run_b(comet, d)
+    ref = _oracle_scan(ev, seeds, want_dca=True, want_kstar=True, want_npts=True)
+    np.testing.assert_array_equal(n_pts, ref["n_pts"])
+    np.testing.assert_array_equal(got["kstar"], ref["kstar"])
+    _check_dca(got["dca"], ref["dca"])
+    _check_rss(got["rss"], ref["rss"])
+    assert np.array_equal(got["rss"], ref["rss"])
+
+
+@pytest.mark.parametrize("n_fired", [1, 7, 33, 97])
+def test_dca_rss_wire_counts(comet, cfg1_event, n_fired):
+    """Every wires-per-warp instantiation (1..4) and partly filled last passes."""
+    import copy
+    ev = copy.copy(cfg1_event)
+    ev.fired_wire = cfg1_event.fired_wire[:min(n_fired, cfg1_event.n_fired)].copy()
+    if n_fired > cfg1_event.n_fired:        # pad with unfired wires that carry no entries
+        extra = np.setdiff1d(np.arange(ev.geom.n_wires, dtype=np.int32), cfg1_event.fired_wire)[:n_fired - cfg1_event.n_fired]
+        ev.fired_wire = np.concatenate([cfg1_event.fired_wire, extra]).astype(np.int32)
+        ev.hit_off = np.concatenate([cfg1_event.hit_off, np.full(extra.size, cfg1_event.hit_off[-1], dtype=np.int32)])
+        ev.rho = cfg1_event.rho
+    else:
+        ev.hit_off = cfg1_event.hit_off[:n_fired + 1].copy()
+        ev.rho = cfg1_event.rho[:ev.hit_off[-1]].copy()
+    seeds, _ = event_seeds(ev, shape=(3, 3, 4, 4))
+    d = DevEvent(ev, seeds)
+    got, _ = _run_b(comet, d)
+    ref = _oracle_scan(ev, seeds, want_dca=True, want_kstar=True)
+    np.testing.assert_array_equal(got["kstar"], ref["kstar"])
+    _check_dca(got["dca"], ref["dca"])
+    _check_rss(got["rss"], ref["rss"])
+
+
+def test_dca_rss_no_wires_and_no_seeds(comet, cfg0_event):
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev, shape=(2, 2, 2, 5))
+    d = DevEvent(ev, seeds)
+    track, n_pts = comet.seed_extrapolate(d.seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop)
+    empty_i = torch.zeros(0, dtype=torch.int32, device="cuda")
+    out = comet.dca_rss(track, n_pts, d.seeds, *d.phys(), d.wire_a, d.wire_b, empty_i,
+                        torch.zeros(1, dtype=torch.int32, device="cuda"),
+                        torch.zeros(0, dtype=torch.float64, device="cuda"), ev.cutoff)
+    assert torch.all(out["rss"] == 0.0)
+    # zero seeds: nothing to do, no error
+    z = torch.zeros((6, 0), dtype=torch.float64, device="cuda")
+    t0, n0 = comet.seed_extrapolate(z, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop)
+    assert n0.numel() == 0
+
+
+def test_high_occupancy_cutoff_sweep(comet):
+    """configs[4]: ~1000 noise hits; D is cutoff-independent, RSS and classification are not."""
+    ev = make_config(4)[0]
+    seeds, part_off = event_seeds(ev, shape=(4, 4, 4, 4))
+    d = DevEvent(ev, seeds)
+    ref_d = None
+    for lam in ev.spec["cutoffs"]:
+        got, _ = _run_b(comet, d, cutoff=lam)
+        ref = _oracle_scan(ev, seeds, cutoff=lam, want_dca=True, want_kstar=True)
+        np.testing.assert_array_equal(got["kstar"], ref["kstar"])
+        _check_dca(got["dca"], ref["dca"])
+        _check_rss(got["rss"], ref["rss"])
+        if ref_d is not None:
+            assert np.array_equal(got["dca"], ref_d)
+        ref_d = got["dca"]
+        sel = comet.select_and_classify(d.seeds, *d.phys(), ev.r_stop, *d.hits(), lam,
+                                        torch.from_numpy(got["rss"]).cuda(), part_off)
+        rs = O.select_classify(seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a,
+                               ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho, lam, ref["rss"], part_off)
+        np.testing.assert_array_equal(sel["best_seed"].cpu().numpy(), rs["best_seed"])
+        np.testing.assert_array_equal(sel["cls"].cpu().numpy(), rs["cls"])
+
+
+# ------------------------------------------------------------------------------------------------
+# step C and the whole path
+# ------------------------------------------------------------------------------------------------
+def _check_select(sel, ref, ev, cutoff):
+    np.testing.assert_array_equal(sel["best_seed"].cpu().numpy(), ref["best_seed"])
+    _check_rss(sel["best_rss"].cpu().numpy(), ref["best_rss"])
+    bd, rd = sel["best_dca"].cpu().numpy(), ref["best_dca"]
+    _check_dca(bd, rd)
+    cls, rcls = sel["cls"].cpu().numpy(), ref["cls"]
+    if not np.array_equal(cls, rcls):
+        # only entries whose residual lies within 1e-9 cm of the cutoff may differ
+        for p, j in zip(*np.nonzero(cls != rcls)):
+            i = np.searchsorted(ev.hit_off, j, side="right") - 1
+            assert abs(abs(rd[p, i] - ev.rho[j]) - cutoff) < 1e-9
+
+
+def test_whole_path_cfg0(comet, cfg0_event):
+    ev = cfg0_event
+    seeds, part_off = event_seeds(ev)
+    d = DevEvent(ev, seeds)
+    out = comet.scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    ref = _oracle_scan(ev, seeds)
+    _check_rss(out["rss"].cpu().numpy(), ref["rss"])
+    rs = O.select_classify(seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a,
+                           ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, ref["rss"], part_off)
+    _check_select(out, rs, ev, ev.cutoff)
+    # slabbed processing (track buffer smaller than the seed set) gives the same numbers
+    out2 = comet.scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, slab_seeds=1000)
+    assert torch.equal(out2["rss"], out["rss"]) and torch.equal(out2["cls"], out["cls"])
+    assert torch.equal(out2["best_seed"], out["best_seed"])
+
+
+def test_select_ties_and_empty_partition(comet, cfg0_event):
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev, shape=(3, 2, 2, 2))
+    S = seeds.shape[1]
+    dup = np.ascontiguousarray(np.concatenate([seeds, seeds], axis=1))
+    d = DevEvent(ev, dup)
+    part_off = np.array([0, S, S, 2 * S], dtype=np.int64)      # middle partition is empty
+    out = comet.scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    bs = out["best_seed"].cpu().numpy()
+    assert bs[1] == -1 and bs[2] == bs[0] + S
+    assert torch.all(out["cls"][1] == 0) and torch.isnan(out["best_rss"][1])
+    one = comet.select_and_classify(d.seeds, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, out["rss"],
+                                    np.array([0, 2 * S], dtype=np.int64))
+    assert int(one["best_seed"][0]) == int(bs[0])              # tie between the copies -> lower index
+
+
+def test_whole_path_host_buffers(comet, cfg0_event):
+    ev = cfg0_event
+    seeds, part_off = event_seeds(ev)
+    out = comet.scan_event_host(torch.from_numpy(seeds).pin_memory(), part_off, ev.charge, ev.bz, ev.step,
+                                ev.n_steps, ev.r_stop, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire,
+                                ev.hit_off, ev.rho, ev.cutoff, want_rss=True,
+                                track_budget_bytes=40 << 20)       # forces several slabs
+    ref = _oracle_scan(ev, seeds)
+    _check_rss(out["rss"].numpy(), ref["rss"])
+    rs = O.select_classify(seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a,
+                           ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, ref["rss"], part_off)
+    np.testing.assert_array_equal(out["best_seed"].numpy(), rs["best_seed"])
+    np.testing.assert_array_equal(out["cls"].numpy(), rs["cls"])
+
+
+def test_argument_errors(comet, cfg0_event):
+    from paper_1911_09340_b200 import CometError
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev, shape=(2, 2, 2, 4))
+    d = DevEvent(ev, seeds)
+    with pytest.raises(CometError):
+        comet.seed_extrapolate(d.seeds, ev.charge, ev.bz, -1.0, ev.n_steps, ev.r_stop)      # step <= 0
+    with pytest.raises(CometError):
+        comet.seed_extrapolate(d.seeds, 0, ev.bz, ev.step, ev.n_steps, ev.r_stop)           # charge 0
+    with pytest.raises(CometError):
+        comet.seed_extrapolate(d.seeds, ev.charge, ev.bz, ev.step, 5000, ev.r_stop)         # > COMET_MAX_STEPS
+    with pytest.raises(CometError):
+        comet.seed_extrapolate(d.seeds.cpu(), ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop)
