@@ -1,0 +1,340 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the seed x hit scan on BASELINE.json configs[1], one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A step is one pass of the whole hot path (comet_seed_extrapolate, comet_dca_rss,
+comet_select_and_classify) over one synthetic event whose inputs are resident in HBM.  `value` is
+seed x fired-wire DCA evaluations per second over all ranks (each rank scans its own replica of the
+event: weak scaling, no data-path collective).  `e2e` is the same metric through
+comet_scan_event_host with pinned HOST buffers (H2D of the inputs and D2H of the results inside the
+timed region).  `roofline` is for comet_dca_rss' kernel, timed live with CUDA events on its stream.
+`--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "seed_hit_dca_evals_per_s"
+UNIT = "DCA evals/s (seed x fired-wire pairs)"
+
+# FP64 pipe model of k_dca_rss: per (seed, wire, recorded state) the shortlist
+# issues 9 FP64-pipe instructions (6 DFMA + DMUL + DFMA + DSETP); per (seed, wire) the exact decision
+# + virtual-plane iteration + residual issue about FINE_INSTR more.  FLOPs are pipe slots x 2.
+SHORTLIST_INSTR = 9
+FINE_INSTR = 600
+# 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz)
+FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum of k_dca_rss per launch (profiles/, ncu --set full); None = not captured
+DCA_TRAFFIC_BYTES = None
+
+
+def _event(cfg):
+    from comet_synth import event_seeds, make_config
+    ev = make_config(cfg)[0]
+    seeds, part_off = event_seeds(ev)
+    return ev, seeds, part_off
+
+
+def _workload_name(cfg, ev, seeds, part_off):
+    return ("BASELINE.json configs[%d]: %d partition(s) x %d seeds, %d fired wires / %d hit entries, "
+            "%d steps x %.3g cm, r_stop %.0f cm, cutoff %.3g cm"
+            % (cfg, len(part_off) - 1, seeds.shape[1] // (len(part_off) - 1), ev.n_fired, ev.n_hits,
+               ev.n_steps, ev.step, ev.r_stop, ev.cutoff))
+
+
+# --------------------------------------------------------------------------------------------------
+# CPU oracle legs
+# --------------------------------------------------------------------------------------------------
+def _oracle_time(ev, seeds, part_off, n_sample):
+    """Seconds the oracle needs for A+B on the first n_sample seeds plus C on them."""
+    from oracle import comet_oracle as O
+    sub = np.ascontiguousarray(seeds[:, :n_sample])
+    t0 = time.perf_counter()
+    r = O.scan(sub, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a, ev.geom.wire_b,
+               ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff)
+    O.select_classify(sub, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a, ev.geom.wire_b,
+                      ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, r["rss"],
+                      np.array([0, n_sample], dtype=np.int64))
+    return time.perf_counter() - t0
+
+
+def _oracle_sample_size(ev, seeds, part_off, target_s):
+    S = seeds.shape[1]
+    probe = min(S, 4096)
+    t = _oracle_time(ev, seeds, part_off, probe)
+    n = int(min(S, max(probe, probe * target_s / max(t, 1e-6))))
+    return max(32, n // 32 * 32)
+
+
+def cpu_baseline(ev, seeds, part_off, target_s=15.0):
+    from oracle import comet_oracle as O
+    n = _oracle_sample_size(ev, seeds, part_off, target_s)
+    t = _oracle_time(ev, seeds, part_off, n)
+    return {"value": n * ev.n_fired / t, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle",
+            "sample": "first %d of %d seeds of the same event (A+B+C), %.1f s" % (n, seeds.shape[1], t),
+            "events_per_s_extrapolated": 1.0 / (t * seeds.shape[1] / n)}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import comet_oracle as O
+    ev, seeds, part_off = _event(args.config)
+    n = _oracle_sample_size(ev, seeds, part_off, 4.0)
+    for _ in range(args.warmup):
+        _oracle_time(ev, seeds, part_off, n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _oracle_time(ev, seeds, part_off, n)
+    dt = (time.perf_counter() - t0) / args.steps
+    value = n * ev.n_fired / dt
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": _workload_name(args.config, ev, seeds, part_off),
+                   "note": "CPU oracle (oracle/comet_oracle.c, gcc -O2, OpenMP over seeds) on the host cores; "
+                           "each step scans a bounded sample of the event's seeds"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.max_threads(), "kind": "oracle",
+                         "sample": "first %d of %d seeds per step (A+B+C)" % (n, seeds.shape[1])},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------------------------------
+# clocks
+# --------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.f.read().splitlines():
+            c = [x.strip() for x in ln.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# --------------------------------------------------------------------------------------------------
+# CUDA legs
+# --------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1911_09340_b200 import Comet
+    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH
+    from paper_1911_09340_b200.build import build
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.set_device(local)
+    ev, seeds, part_off = _event(args.config)
+    S, W, H, P = seeds.shape[1], ev.n_fired, ev.n_hits, len(part_off) - 1
+    c = Comet(local)
+    c.set_option(OPT_COARSE_SEARCH, COARSE_PRUNED if args.coarse == "pruned" else COARSE_EXHAUSTIVE)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    d_seeds, d_wa, d_wb = dev(seeds), dev(ev.geom.wire_a), dev(ev.geom.wire_b)
+    d_fw, d_ho, d_rho = dev(ev.fired_wire), dev(ev.hit_off), dev(ev.rho)
+    track = torch.empty(c.track_bytes(S, ev.n_steps), dtype=torch.uint8, device="cuda")
+    n_pts = torch.empty(S, dtype=torch.int32, device="cuda")
+    rss = torch.empty(S, dtype=torch.float64, device="cuda")
+    phys = (ev.charge, ev.bz, ev.step, ev.n_steps)
+    hits = (d_wa, d_wb, d_fw, d_ho, d_rho)
+    stream = torch.cuda.current_stream()
+    b_events = []
+
+    def step(timed):
+        c.seed_extrapolate(d_seeds, *phys, ev.r_stop, track=track, n_pts=n_pts)
+        if timed:
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+        c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss)
+        if timed:
+            e1.record(stream)
+            b_events.append((e0, e1))
+        return c.select_and_classify(d_seeds, *phys, ev.r_stop, *hits, ev.cutoff, rss, part_off)
+
+    for _ in range(args.warmup):
+        step(False)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t0.record(stream)
+    for _ in range(args.steps):
+        out = step(True)
+    t1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop() if sampler else None
+    ms = t0.elapsed_time(t1)
+    ms_b = float(np.mean([a.elapsed_time(b) for a, b in b_events]))
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_per_step = ms / args.steps
+    pairs = float(S) * W
+    value = world * pairs / (ms_per_step * 1e-3)
+    n_states = float(n_pts.sum().item())
+    best = out["best_seed"].cpu().numpy().tolist()
+    n_cls = int(out["cls"].sum().item())
+
+    # ---- e2e: host buffers through comet_scan_event_host -------------------------------------
+    pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
+    h = dict(seeds=pin(seeds, torch.float64), wa=pin(ev.geom.wire_a, torch.float64), wb=pin(ev.geom.wire_b, torch.float64),
+             fw=pin(ev.fired_wire, torch.int32), ho=pin(ev.hit_off, torch.int32), rho=pin(ev.rho, torch.float64))
+    del track
+    torch.cuda.empty_cache()
+    budget = 8 << 30
+    hout = None
+
+    def e2e_step():
+        nonlocal hout
+        hout = c.scan_event_host(h["seeds"], part_off, *phys, ev.r_stop, h["wa"], h["wb"], h["fw"], h["ho"], h["rho"],
+                                 ev.cutoff, out=hout, track_budget_bytes=budget)
+
+    for _ in range(max(1, min(args.warmup, 3))):
+        e2e_step()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    w0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()
+    e2e_s = (time.perf_counter() - w0) / args.steps
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    h2d = sum(int(v.numel() * v.element_size()) for v in h.values())
+    d2h = sum(int(v.numel() * v.element_size()) for v in hout.values())
+    assert hout["best_seed"].numpy().tolist() == best
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+    # ---- FP64 pipe peak, measured live ---------------------------------------------------------
+    n_fma = c.fp64_peak_probe(8 * 4096)
+    torch.cuda.synchronize()
+    pe0, pe1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    best_ms = 1e30
+    for _ in range(5):
+        pe0.record(stream); c.fp64_peak_probe(8 * 4096); pe1.record(stream)
+        torch.cuda.synchronize()
+        best_ms = min(best_ms, pe0.elapsed_time(pe1))
+    peak_measured = 2 * n_fma / (best_ms * 1e-3) / 1e12
+    flops = 2.0 * (SHORTLIST_INSTR * n_states * W + FINE_INSTR * pairs)
+    achieved = flops / (ms_b * 1e-3) / 1e12
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": _workload_name(args.config, ev, seeds, part_off),
+                   "coarse_search": args.coarse,
+                   "l2": "inputs larger than L2: every step rewrites and rereads the %.1f GB track buffer"
+                         % (c.track_bytes(S, ev.n_steps) / 1e9),
+                   "parallelism": "one replica of the event per GPU (event-level sharding, no collective)"},
+        "events_per_s": world / (ms_per_step * 1e-3),
+        "result": {"best_seed": best, "classified_entries": n_cls, "recorded_states_per_seed": n_states / S},
+        "e2e": {"value": world * pairs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_s * 1e3, "api": "comet_scan_event_host, pinned host buffers, %d GiB track slab" % (budget >> 30)},
+        "gpu_launches": 6 * args.steps,
+        "clocks": clocks,
+        "roofline": {"kernel": "k_dca_rss", "bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS,
+                     "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": DCA_TRAFFIC_BYTES,
+                     "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 figure)",
+                     "peak_measured_dfma_probe": peak_measured, "frac_of_measured": achieved / peak_measured,
+                     "ms_per_launch": ms_b, "share_of_step": ms_b / ms_per_step,
+                     "model": "FP64-pipe slots x 2: %d per (seed, wire, recorded state) + %d per (seed, wire)"
+                              % (SHORTLIST_INSTR, FINE_INSTR),
+                     "algorithmic_hbm_bytes": n_states * 24 + n_states * 0 + pairs * 48,
+                     "hbm_gbs_if_read_once": (n_states * 24) / (ms_b * 1e-3) / 1e9},
+    }
+    if args.cpu_baseline and world == 1:
+        line["cpu_baseline"] = cpu_baseline(ev, seeds, part_off)
+    print(json.dumps(line))
+    c.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--coarse", choices=["exhaustive", "pruned"], default="exhaustive")
+    ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
