@@ -172,7 +172,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_1911_09340_b200 import Comet
-    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH
+    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH, OPT_STATS
     from paper_1911_09340_b200.build import build
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -240,6 +240,30 @@ def run_ours(args):
     best = out["best_seed"].cpu().numpy().tolist()
     n_cls = int(out["cls"].sum().item())
 
+    # ---- work counters of the pruned search (one untimed launch) and the other mode's kernel time ---
+    stats = None
+    if args.coarse == "pruned":
+        c.set_option(OPT_STATS, 1)
+        c.read_stats(reset=True)
+        c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss)
+        stats = c.read_stats(reset=True)
+        c.set_option(OPT_STATS, 0)
+    other = "exhaustive" if args.coarse == "pruned" else "pruned"
+    c.set_option(OPT_COARSE_SEARCH, COARSE_EXHAUSTIVE if other == "exhaustive" else COARSE_PRUNED)
+    rss2 = torch.empty_like(rss)
+    o_ev = []
+    for i in range(1 + min(args.steps, 5)):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss2)
+        e1.record(stream)
+        if i:
+            o_ev.append((e0, e1))
+    torch.cuda.synchronize()
+    ms_other = float(np.mean([a.elapsed_time(b) for a, b in o_ev]))
+    modes_agree = bool(torch.equal(rss, rss2))
+    c.set_option(OPT_COARSE_SEARCH, COARSE_PRUNED if args.coarse == "pruned" else COARSE_EXHAUSTIVE)
+
     # ---- e2e: host buffers through comet_scan_event_host -------------------------------------
     pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
     h = dict(seeds=pin(seeds, torch.float64), wa=pin(ev.geom.wire_a, torch.float64), wb=pin(ev.geom.wire_b, torch.float64),
@@ -285,7 +309,20 @@ def run_ours(args):
         torch.cuda.synchronize()
         best_ms = min(best_ms, pe0.elapsed_time(pe1))
     peak_measured = 2 * n_fma / (best_ms * 1e-3) / 1e12
-    flops = 2.0 * (SHORTLIST_INSTR * n_states * W + FINE_INSTR * pairs)
+    flops_exh = 2.0 * (SHORTLIST_INSTR * n_states * W + FINE_INSTR * pairs)
+    if stats is not None:
+        flops = 2.0 * (SHORTLIST_INSTR * (stats["samples"] + stats["rows_needed"]) + FINE_INSTR * stats["fine_needed"])
+        flops_exec = 2.0 * (SHORTLIST_INSTR * (stats["samples"] + stats["rows_executed"]) + FINE_INSTR * stats["fine_executed"])
+        kernel, model = "k_dca_rss_pruned", (
+            "FP64-pipe slots x 2 of the work the pruned search needs (thread-level counters, comet_read_stats): "
+            "%d per block/sub-block sample or row evaluation + %d per (seed, wire) pair that runs the plane iteration"
+            % (SHORTLIST_INSTR, FINE_INSTR))
+        ms_exh, flops_other = ms_other, flops_exh
+    else:
+        flops, flops_exec = flops_exh, flops_exh
+        kernel, model = "k_dca_rss", ("FP64-pipe slots x 2: %d per (seed, wire, recorded state) + %d per (seed, wire)"
+                                      % (SHORTLIST_INSTR, FINE_INSTR))
+        ms_exh, flops_other = ms_b, None
     achieved = flops / (ms_b * 1e-3) / 1e12
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -302,13 +339,19 @@ def run_ours(args):
                 "ms_per_step": e2e_s * 1e3, "api": "comet_scan_event_host, pinned host buffers, %d GiB track slab" % (budget >> 30)},
         "gpu_launches": 6 * args.steps,
         "clocks": clocks,
-        "roofline": {"kernel": "k_dca_rss", "bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS,
+        "roofline": {"kernel": kernel, "bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS,
                      "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": DCA_TRAFFIC_BYTES,
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 figure)",
                      "peak_measured_dfma_probe": peak_measured, "frac_of_measured": achieved / peak_measured,
                      "ms_per_launch": ms_b, "share_of_step": ms_b / ms_per_step,
-                     "model": "FP64-pipe slots x 2: %d per (seed, wire, recorded state) + %d per (seed, wire)"
-                              % (SHORTLIST_INSTR, FINE_INSTR),
+                     "model": model,
+                     "achieved_executed": flops_exec / (ms_b * 1e-3) / 1e12,
+                     "work_counters": stats,
+                     "exhaustive_kernel": {"ms_per_launch": ms_exh, "achieved": flops_exh / (ms_exh * 1e-3) / 1e12,
+                                           "frac": flops_exh / (ms_exh * 1e-3) / 1e12 / FP64_PEAK_NOMINAL_TFLOPS,
+                                           "model": "%d per (seed, wire, recorded state) + %d per (seed, wire)"
+                                                    % (SHORTLIST_INSTR, FINE_INSTR)},
+                     "other_mode": {"coarse_search": other, "ms_per_launch": ms_other, "rss_bit_identical": modes_agree},
                      "algorithmic_hbm_bytes": n_states * 24 + n_states * 0 + pairs * 48,
                      "hbm_gbs_if_read_once": (n_states * 24) / (ms_b * 1e-3) / 1e9},
     }
@@ -327,7 +370,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--coarse", choices=["exhaustive", "pruned"], default="exhaustive")
+    ap.add_argument("--coarse", choices=["exhaustive", "pruned"], default="pruned")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -44,8 +44,11 @@ typedef enum comet_status {
 
 /* Options for comet_set_option. */
 #define COMET_OPT_COARSE_SEARCH 1     /* how step B2 (closest recorded state) is found          */
-#define COMET_COARSE_EXHAUSTIVE 0     /*   every recorded point is evaluated      */
-#define COMET_COARSE_PRUNED 1         /*   strided samples + Lipschitz-bounded windows; same k*  */
+#define COMET_COARSE_EXHAUSTIVE 0     /*   every recorded state is evaluated for every wire         */
+#define COMET_COARSE_PRUNED 1         /*   default: block samples + Lipschitz bounds skip states that cannot be
+                                       *   the closest one, and (when neither dca nor kstar is requested) pairs
+                                       *   whose residual is provably the cutoff; k*, D and rss are identical   */
+#define COMET_OPT_STATS 2             /* 1: comet_dca_rss (pruned) adds its work counters, see comet_read_stats  */
 
 /* ---- context ---------------------------------------------------------------------------- */
 
@@ -59,6 +62,14 @@ const char* comet_status_string(int status);
 int comet_last_cuda_error(const comet_ctx* ctx);
 int comet_set_option(comet_ctx* ctx, int option, int value);
 int comet_get_option(const comet_ctx* ctx, int option, int* value);
+
+/* Copies the work counters accumulated by comet_dca_rss calls made with COMET_OPT_STATS = 1 to
+ * out_host[0..n) (HOST, n <= 6) and synchronises the stream; reset != 0 zeroes them afterwards.
+ * Counters are thread-level: [0] block/sub-block sample evaluations, [1] row evaluations a lane
+ * needed, [2] row evaluations executed (a warp opens a sub-block when any lane needs it),
+ * [3] (seed, wire) pairs that needed the virtual-plane iteration, [4] pairs for which a warp
+ * executed it, [5] all pairs. */
+int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, int32_t reset, void* cuda_stream);
 
 /* ---- kernel A: track recording (Algorithm 1) ---------------------------- */
 

@@ -17,13 +17,15 @@ EXPORTED_SYMBOLS = [
     "comet_create", "comet_destroy", "comet_status_string", "comet_last_cuda_error",
     "comet_set_option", "comet_get_option", "comet_track_bytes", "comet_seed_extrapolate",
     "comet_track_export", "comet_dca_rss", "comet_select_and_classify", "comet_scan_event_host",
-    "comet_fp64_peak_probe",
+    "comet_fp64_peak_probe", "comet_read_stats",
 ]
 
 COMET_CHUNK = 32
 OPT_COARSE_SEARCH = 1
 COARSE_EXHAUSTIVE = 0
 COARSE_PRUNED = 1
+OPT_STATS = 2
+STATS_FIELDS = ("samples", "rows_needed", "rows_executed", "fine_needed", "fine_executed", "pairs")
 
 
 class CometError(RuntimeError):
@@ -68,6 +70,7 @@ def load_library():
                                         vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                         vp, i32, sz, vp, vp, vp, vp, vp, vp]
     L.comet_fp64_peak_probe.argtypes = [vp, i32, vp, ctypes.POINTER(dbl), vp]
+    L.comet_read_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), i32, i32, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("comet_status_string", "comet_track_bytes"):
             getattr(L, name).restype = ctypes.c_int
@@ -130,6 +133,12 @@ class Comet:
         v = ctypes.c_int()
         self._check(self._L.comet_get_option(self._h, int(option), ctypes.byref(v)))
         return v.value
+
+    def read_stats(self, reset: bool = True, stream=None) -> dict:
+        """Work counters of the pruned comet_dca_rss calls made with OPT_STATS = 1 (synchronises)."""
+        buf = (ctypes.c_uint64 * len(STATS_FIELDS))()
+        self._check(self._L.comet_read_stats(self._h, buf, len(STATS_FIELDS), int(bool(reset)), _stream_ptr(stream)))
+        return dict(zip(STATS_FIELDS, (int(v) for v in buf)))
 
     def track_bytes(self, n_seeds: int, n_steps: int) -> int:
         return int(self._L.comet_track_bytes(int(n_seeds), int(n_steps)))

@@ -14,13 +14,17 @@
 #include "extrapolate.cuh"
 #include "select.cuh"
 
+#define COMET_PRUNED_WT 4
+
 using namespace comet;
 
 struct comet_ctx {
     int device;
     int last_cuda;
     int opt_coarse;
+    int opt_stats;
     int n_sm;
+    unsigned long long* stats;   // device [ST_N] work counters of the pruned kernel
     // device workspace
     double* wt;            // wire table [14][wt_cap]
     int32_t wt_cap;
@@ -71,13 +75,18 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (!ctx) return COMET_ENOMEM;
     memset(ctx, 0, sizeof(*ctx));
     ctx->device = cuda_device;
-    ctx->opt_coarse = COMET_COARSE_EXHAUSTIVE;
+    ctx->opt_coarse = COMET_COARSE_PRUNED;
     cudaError_t e = cudaSetDevice(cuda_device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, cuda_device);
     ctx->wt_cap = 8192;
     if (e == cudaSuccess) e = cudaMalloc(&ctx->wt, sizeof(double) * COMET_WT_FIELDS * (size_t)ctx->wt_cap);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->pv, sizeof(double) * COMET_MAX_PARTITIONS * COMET_ARGMIN_SPLIT);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->pi, sizeof(int64_t) * COMET_MAX_PARTITIONS * COMET_ARGMIN_SPLIT);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->stats, sizeof(unsigned long long) * ST_N);
+    if (e == cudaSuccess) e = cudaMemset(ctx->stats, 0, sizeof(unsigned long long) * ST_N);
+    const int pr_smem = COMET_WSUP * 32 * (int)sizeof(double);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss_pruned<COMET_PRUNED_WT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss_pruned<COMET_PRUNED_WT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
     // shared-memory opt-ins (done once here, never on the hot path)
     const int dca_smem = (2 * COMET_KT * 3 * COMET_LANES + COMET_DCA_WARPS * 4 * 32) * (int)sizeof(double);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
@@ -88,7 +97,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
         e = cudaFuncSetAttribute(k_select_classify, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
     if (e != cudaSuccess) {
-        cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi);
+        cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
         delete ctx;
         return e == cudaErrorMemoryAllocation ? COMET_ENOMEM : COMET_ECUDA;
     }
@@ -100,7 +109,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
 {
     if (!ctx) return COMET_EINVAL;
     cudaSetDevice(ctx->device);
-    cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi);
+    cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf);
     delete ctx;
     return COMET_OK;
@@ -113,6 +122,10 @@ extern "C" int comet_set_option(comet_ctx* ctx, int option, int value)
         ctx->opt_coarse = value;
         return COMET_OK;
     }
+    if (option == COMET_OPT_STATS && (value == 0 || value == 1)) {
+        ctx->opt_stats = value;
+        return COMET_OK;
+    }
     return COMET_EINVAL;
 }
 
@@ -120,7 +133,20 @@ extern "C" int comet_get_option(const comet_ctx* ctx, int option, int* value)
 {
     if (!ctx || !value) return COMET_EINVAL;
     if (option == COMET_OPT_COARSE_SEARCH) { *value = ctx->opt_coarse; return COMET_OK; }
+    if (option == COMET_OPT_STATS) { *value = ctx->opt_stats; return COMET_OK; }
     return COMET_EINVAL;
+}
+
+extern "C" int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, int32_t reset, void* cuda_stream)
+{
+    if (!ctx || !out_host || n < 0 || n > ST_N) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(ctx, cudaMemcpyAsync(out_host, ctx->stats, sizeof(uint64_t) * (size_t)n, cudaMemcpyDeviceToHost, st));
+    if (reset) CU(ctx, cudaMemsetAsync(ctx->stats, 0, sizeof(unsigned long long) * ST_N, st));
+    CU(ctx, cudaStreamSynchronize(st));
+    return COMET_OK;
 }
 
 static inline int64_t n_chunks_of(int64_t n_seeds) { return (n_seeds + COMET_LANES - 1) / COMET_LANES; }
@@ -186,11 +212,13 @@ extern "C" int comet_track_export(comet_ctx* ctx, const void* track, const int32
 }
 
 static int launch_wire_prep(comet_ctx* ctx, const double* wire_a, const double* wire_b, int32_t n_wires,
-                            const int32_t* fired_wire, int32_t n_fired, cudaStream_t st)
+                            const int32_t* fired_wire, const int32_t* hit_off, const double* rho, int32_t n_fired,
+                            double cutoff_cm, double step_cm, cudaStream_t st)
 {
     if (n_fired > ctx->wt_cap) return COMET_EINVAL;
     if (n_fired == 0) return COMET_OK;
-    k_wire_prep<<<(n_fired + 127) / 128, 128, 0, st>>>(wire_a, wire_b, n_wires, fired_wire, n_fired, ctx->wt);
+    k_wire_prep<<<(n_fired + 127) / 128, 128, 0, st>>>(wire_a, wire_b, n_wires, fired_wire, n_fired, hit_off, rho,
+                                                       cutoff_cm, step_cm, ctx->wt);
     CU(ctx, cudaGetLastError());
     return COMET_OK;
 }
@@ -221,7 +249,7 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, n_fired, st);
+    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
     if (rc) return rc;
     DcaArgs a;
     a.X = plane_X((void*)track);
@@ -241,18 +269,25 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
     a.rss = rss;
     a.dca = dca;
     a.kstar = kstar;
-    // wires per warp per pass: spread n_fired evenly over ceil(n_fired/32) passes of 8 warps
-    const int n_pass = (n_fired + COMET_DCA_WARPS * 4 - 1) / (COMET_DCA_WARPS * 4);
-    int wt = n_pass > 0 ? (n_fired + COMET_DCA_WARPS * n_pass - 1) / (COMET_DCA_WARPS * n_pass) : 1;
-    if (wt < 1) wt = 1;
+    a.stats = ctx->opt_stats ? ctx->stats : nullptr;
     const unsigned blocks = (unsigned)n_chunks_of(n_seeds);
     const int threads = COMET_DCA_WARPS * 32;
-    const size_t smem = (2 * COMET_KT * 3 * COMET_LANES + (size_t)COMET_DCA_WARPS * wt * 32) * sizeof(double);
-    switch (wt) {
-        case 1: k_dca_rss<1><<<blocks, threads, smem, st>>>(a); break;
-        case 2: k_dca_rss<2><<<blocks, threads, smem, st>>>(a); break;
-        case 3: k_dca_rss<3><<<blocks, threads, smem, st>>>(a); break;
-        default: k_dca_rss<4><<<blocks, threads, smem, st>>>(a); break;
+    if (ctx->opt_coarse == COMET_COARSE_PRUNED) {
+        const size_t smem = (size_t)(n_fired < COMET_WSUP ? (n_fired > 0 ? n_fired : 1) : COMET_WSUP) * 32 * sizeof(double);
+        if (ctx->opt_stats) k_dca_rss_pruned<COMET_PRUNED_WT, true><<<blocks, threads, smem, st>>>(a);
+        else k_dca_rss_pruned<COMET_PRUNED_WT, false><<<blocks, threads, smem, st>>>(a);
+    } else {
+        // wires per warp per pass: spread n_fired evenly over ceil(n_fired/32) passes of 8 warps
+        const int n_pass = (n_fired + COMET_DCA_WARPS * 4 - 1) / (COMET_DCA_WARPS * 4);
+        int wt = n_pass > 0 ? (n_fired + COMET_DCA_WARPS * n_pass - 1) / (COMET_DCA_WARPS * n_pass) : 1;
+        if (wt < 1) wt = 1;
+        const size_t smem = (2 * COMET_KT * 3 * COMET_LANES + (size_t)COMET_DCA_WARPS * wt * 32) * sizeof(double);
+        switch (wt) {
+            case 1: k_dca_rss<1><<<blocks, threads, smem, st>>>(a); break;
+            case 2: k_dca_rss<2><<<blocks, threads, smem, st>>>(a); break;
+            case 3: k_dca_rss<3><<<blocks, threads, smem, st>>>(a); break;
+            default: k_dca_rss<4><<<blocks, threads, smem, st>>>(a); break;
+        }
     }
     CU(ctx, cudaGetLastError());
     return COMET_OK;
@@ -285,7 +320,7 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, n_fired, st);
+    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
     if (rc) return rc;
     k_argmin_stage1<<<dim3(COMET_ARGMIN_SPLIT, n_part), COMET_ARGMIN_THREADS, 0, st>>>(rss, po, ctx->pv, ctx->pi);
     CU(ctx, cudaGetLastError());

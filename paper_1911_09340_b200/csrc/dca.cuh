@@ -21,14 +21,19 @@
 
 namespace comet {
 
-#define COMET_WT_FIELDS 14   // m[3] w[3] | e1[3] -m.e1 | e2[3] -m.e2
+#define COMET_WT_FIELDS 15   // m[3] w[3] | e1[3] -m.e1 | e2[3] -m.e2 | far radius R_i
 #define COMET_KT 32          // recorded states per shared-memory tile
 #define COMET_DCA_WARPS 8
 
 // B1: wire prep, one thread per fired wire (once per event).
+// Field 14 is the wire's "far radius" R_i = max_j |rho_ij| + lambda + 1.01 h + 1e-6 cm (-1 for a
+// wire without entries): a track whose every recorded state is farther than R_i from the wire ends
+// the virtual-plane iteration (at most h of arc away from k*, R10) with |D| - |rho_ij| > lambda for
+// every entry, so its bounded residual is exactly lambda (pruned mode).
 __global__ void k_wire_prep(const double* __restrict__ wire_a, const double* __restrict__ wire_b,
                             int32_t n_wires, const int32_t* __restrict__ fired_wire, int32_t W,
-                            double* __restrict__ wt)
+                            const int32_t* __restrict__ hit_off, const double* __restrict__ rho,
+                            double lambda, double h, double* __restrict__ wt)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= W) return;
@@ -55,6 +60,9 @@ __global__ void k_wire_prep(const double* __restrict__ wire_a, const double* __r
     wt[9 * W + i] = -(m0 * p0 + m1 * p1 + m2 * p2);
     wt[10 * W + i] = q0; wt[11 * W + i] = q1; wt[12 * W + i] = q2;
     wt[13 * W + i] = -(m0 * q0 + m1 * q1 + m2 * q2);
+    double rmax = -1.0;
+    for (int j = hit_off[i]; j < hit_off[i + 1]; ++j) rmax = fmax(rmax, fabs(rho[j]));
+    wt[14 * W + i] = (rmax < 0.0) ? -1.0 : rmax + lambda + 1.01 * h + 1e-6;
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
@@ -84,7 +92,40 @@ struct DcaArgs {
     double* rss;
     double* dca;             // optional
     int32_t* kstar;          // optional
+    unsigned long long* stats;   // optional work counters [ST_N] (pruned kernel, COMET_OPT_STATS)
 };
+
+// B2 decision + B3 + B4 for one (seed, wire) pair given the shortlisted state bk:
+// the exact distance of O5 (the definition's operation order) decides between bk-1, bk, bk+1,
+// then the virtual-plane iteration, the signed DCA and the squared bounded residual.
+__device__ __forceinline__ double pair_exact(const double* __restrict__ Xc, const double* __restrict__ Tc,
+                                             int lane, int bk, int np, const DcaArgs& a, double c, int i,
+                                             double& D, int& ks)
+{
+    constexpr int ROW = 3 * COMET_LANES;
+    const int W = a.W;
+    WireLine wl;
+    wl.m0 = __ldg(a.wt + i); wl.m1 = __ldg(a.wt + W + i); wl.m2 = __ldg(a.wt + 2 * W + i);
+    wl.w0 = __ldg(a.wt + 3 * W + i); wl.w1 = __ldg(a.wt + 4 * W + i); wl.w2 = __ldg(a.wt + 5 * W + i);
+    const int ka = max(bk - 1, 0), kb = min(bk + 1, np - 1);
+    ks = ka;
+    double bd = 0.0;
+    State st;
+    st.x0 = st.x1 = st.x2 = 0.0;
+    for (int k = ka; k <= kb; ++k) {
+        const double* xr = Xc + (size_t)k * ROW + lane;
+        const double x0 = xr[0], x1 = xr[32], x2 = xr[64];
+        double u0, u1, u2;
+        const double d2 = perp2_exact(x0, x1, x2, wl, u0, u1, u2);
+        if (k == ka || d2 < bd) { bd = d2; ks = k; st.x0 = x0; st.x1 = x1; st.x2 = x2; }
+    }
+    const double* tr = Tc + (size_t)ks * ROW + lane;
+    st.t0 = tr[0]; st.t1 = tr[32]; st.t2 = tr[64];
+    D = fine_dca(st, ks, np, a.h, c, wl);
+    const double e = wire_residual(D, a.rho, __ldg(a.hit_off + i), __ldg(a.hit_off + i + 1), a.lambda,
+                                   nullptr, nullptr);
+    return xmul(e, e);
+}
 
 template <int WT>
 __global__ void __launch_bounds__(COMET_DCA_WARPS * 32, 2) k_dca_rss(const DcaArgs a)
@@ -152,13 +193,13 @@ __global__ void __launch_bounds__(COMET_DCA_WARPS * 32, 2) k_dca_rss(const DcaAr
 #pragma unroll 4
             for (int kk = 0; kk < rows; ++kk) {
                 const double x0 = sx[kk * ROW], x1 = sx[kk * ROW + 32], x2 = sx[kk * ROW + 64];
-                const bool in_arc = (k0 + kk) < np;       // rows past this lane's last state hold a sentinel
+                // rows past this lane's last state repeat it (hold-last): never strictly smaller
 #pragma unroll
                 for (int q = 0; q < WT; ++q) {
                     const double u1 = fma(x0, e1x[q], fma(x1, e1y[q], fma(x2, e1z[q], c1[q])));
                     const double u2 = fma(x0, e2x[q], fma(x1, e2y[q], fma(x2, e2z[q], c2[q])));
                     const double d2 = fma(u1, u1, u2 * u2);
-                    if (in_arc && d2 < best[q]) { best[q] = d2; bk[q] = k0 + kk; }
+                    if (d2 < best[q]) { best[q] = d2; bk[q] = k0 + kk; }
                 }
             }
             __syncthreads();
@@ -169,27 +210,9 @@ __global__ void __launch_bounds__(COMET_DCA_WARPS * 32, 2) k_dca_rss(const DcaAr
             double e2 = 0.0;
             if (valid && wi[q] < W) {
                 const int i = wi[q];
-                WireLine wl;
-                wl.m0 = __ldg(a.wt + i); wl.m1 = __ldg(a.wt + W + i); wl.m2 = __ldg(a.wt + 2 * W + i);
-                wl.w0 = __ldg(a.wt + 3 * W + i); wl.w1 = __ldg(a.wt + 4 * W + i); wl.w2 = __ldg(a.wt + 5 * W + i);
-                const int ka = max(bk[q] - 1, 0), kb = min(bk[q] + 1, np - 1);
-                int ks = ka;
-                double bd = 0.0;
-                State st;
-                st.x0 = st.x1 = st.x2 = 0.0;
-                for (int k = ka; k <= kb; ++k) {
-                    const double* xr = Xc + (size_t)k * ROW + lane;
-                    const double x0 = xr[0], x1 = xr[32], x2 = xr[64];
-                    double u0, u1, u2;
-                    const double d2 = perp2_exact(x0, x1, x2, wl, u0, u1, u2);
-                    if (k == ka || d2 < bd) { bd = d2; ks = k; st.x0 = x0; st.x1 = x1; st.x2 = x2; }
-                }
-                const double* tr = Tc + (size_t)ks * ROW + lane;
-                st.t0 = tr[0]; st.t1 = tr[32]; st.t2 = tr[64];
-                const double D = fine_dca(st, ks, np, a.h, c, wl);
-                const double e = wire_residual(D, a.rho, __ldg(a.hit_off + i), __ldg(a.hit_off + i + 1),
-                                               a.lambda, nullptr, nullptr);
-                e2 = xmul(e, e);
+                double D;
+                int ks;
+                e2 = pair_exact(Xc, Tc, lane, bk[q], np, a, c, i, D, ks);
                 if (a.dca) a.dca[(size_t)s * W + i] = D;
                 if (a.kstar) a.kstar[(size_t)s * W + i] = ks;
             }
@@ -204,6 +227,218 @@ __global__ void __launch_bounds__(COMET_DCA_WARPS * 32, 2) k_dca_rss(const DcaAr
         __syncthreads();
     }
     if (warp == 0 && valid) a.rss[s] = rss_acc;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Pruned closest-state search (COMET_COARSE_PRUNED): same k*, D and RSS as the exhaustive scan.
+//
+// Consecutive recorded states are at most L = 1.001 h apart (an RKN step of length h with |c| h
+// <= 0.05 moves the position by less than h (1 + 1e-3); hold-last padding moves it by 0), and the
+// distance to a line is 1-Lipschitz, so a state j rows away from an evaluated state k has
+// D_j >= D_k - j L.  With any upper bound `ub` on the answer, a block of rows whose centre sample
+// has D > ub + (half block) L cannot hold the closest state and is skipped.  Two levels:
+//   level 0: blocks of M0 = 64 rows, sample at row 32; pass 1 takes the minimum over the samples
+//            (ub), pass 2 revisits the samples and opens the blocks that may hold the answer;
+//   level 1: an opened block is cut into sub-blocks of M1 = 8 rows, sample at row 4, the running
+//            minimum tightens ub, and only the sub-blocks that may hold the answer are evaluated
+//            row by row (in increasing k, strict "<": lowest k wins ties, as in the exhaustive scan).
+// ub is also capped by the wire's far radius R_i (k_wire_prep) when neither D nor k* is asked
+// for: a pair whose every state is farther than R_i contributes exactly lambda^2 to RSS and skips
+// the virtual-plane iteration.  All bounds carry an absolute slack of 1e-9 cm for the rounding of
+// the FMA-form distances (~1e-13 cm).  Lanes with |c| h > 0.05 take no shortcut (ub = infinity).
+//
+// Mapping: CTA = one track chunk (lane = seed), warps take groups of WT wires from a CTA-wide
+// counter; rows come straight from global memory / L1 (coalesced 256-byte rows, read-only).
+// e^2 of up to COMET_WSUP wires is staged in shared memory and summed by warp 0 in wire order.
+// ---------------------------------------------------------------------------------------------
+#define COMET_M0 64
+#define COMET_M1 8
+#define COMET_WSUP 256
+#define COMET_CH_MAX 0.05
+#define COMET_LIP 1.001
+#define COMET_SLACK 1e-9
+
+struct EvalC {
+    double e1x, e1y, e1z, c1, e2x, e2y, e2z, c2;
+};
+__device__ __forceinline__ void load_evalc(EvalC& w, const double* __restrict__ wt, int W, int i)
+{
+    w.e1x = __ldg(wt + 6 * W + i); w.e1y = __ldg(wt + 7 * W + i); w.e1z = __ldg(wt + 8 * W + i);
+    w.c1 = __ldg(wt + 9 * W + i);
+    w.e2x = __ldg(wt + 10 * W + i); w.e2y = __ldg(wt + 11 * W + i); w.e2z = __ldg(wt + 12 * W + i);
+    w.c2 = __ldg(wt + 13 * W + i);
+}
+__device__ __forceinline__ double d2_fma(const EvalC& w, double x0, double x1, double x2)
+{
+    const double u1 = fma(x0, w.e1x, fma(x1, w.e1y, fma(x2, w.e1z, w.c1)));
+    const double u2 = fma(x0, w.e2x, fma(x1, w.e2y, fma(x2, w.e2z, w.c2)));
+    return fma(u1, u1, u2 * u2);
+}
+
+// optional work counters (COMET_OPT_STATS): lane-level needed work and warp-level executed work
+enum { ST_SAMPLES = 0, ST_ROWS_NEEDED, ST_ROWS_EXEC, ST_FINE_NEEDED, ST_FINE_EXEC, ST_PAIRS, ST_N };
+
+template <int WT, bool STATS>
+__global__ void __launch_bounds__(COMET_DCA_WARPS * 32, 2) k_dca_rss_pruned(const DcaArgs a)
+{
+    constexpr int ROW = 3 * COMET_LANES;
+    constexpr unsigned FULL = 0xffffffffu;
+    extern __shared__ __align__(16) double e2s[];      // [min(W, WSUP)][32]
+    __shared__ int s_next;
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t chunk = blockIdx.x;
+    const int64_t s = chunk * COMET_LANES + lane;
+    const bool valid = s < a.n_seeds;
+    const int32_t n_rows = a.n_steps + 1;
+    const int32_t np = valid ? a.n_pts[s] : 0;
+    const int32_t kmax = __reduce_max_sync(FULL, np);
+    const int n0 = (kmax + COMET_M0 - 1) / COMET_M0;
+    const size_t base = track_row(chunk, n_rows, 0);
+    const double* __restrict__ Xc = a.X + base;
+    const double* __restrict__ Tc = a.T + base;
+    double c = 0.0;
+    if (valid) {
+        const double px = a.seeds[3 * a.stride + s], py = a.seeds[4 * a.stride + s], pz = a.seeds[5 * a.stride + s];
+        c = xdiv(a.qkb, xsqrt(xdot3(px, py, pz, px, py, pz)));
+    }
+    const int W = a.W;
+    const bool full = (a.dca != nullptr) || (a.kstar != nullptr);
+    const bool lip_ok = fabs(c) * a.h <= COMET_CH_MAX;       // Lipschitz bound valid for this lane
+    const double L = COMET_LIP * a.h;
+    const double INF = 1.7976931348623157e308;
+    const double half0 = (COMET_M0 / 2) * L + COMET_SLACK, half1 = (COMET_M1 / 2) * L + COMET_SLACK;
+    const double lam2 = xmul(a.lambda, a.lambda);
+    double rss_acc = 0.0;
+    unsigned long long st_cnt[ST_N];
+    if (STATS) {
+#pragma unroll
+        for (int j = 0; j < ST_N; ++j) st_cnt[j] = 0;
+    }
+
+    auto load_row = [&](int k, double& x0, double& x1, double& x2) {
+        const double* xr = Xc + (size_t)k * ROW + lane;
+        x0 = __ldg(xr); x1 = __ldg(xr + 32); x2 = __ldg(xr + 64);
+    };
+
+    for (int w_base = 0; w_base < W; w_base += COMET_WSUP) {
+        const int n_here = min(COMET_WSUP, W - w_base);
+        const int n_groups = (n_here + WT - 1) / WT;
+        if (threadIdx.x == 0) s_next = 0;
+        __syncthreads();
+        while (true) {
+            int g = 0;
+            if (lane == 0) g = atomicAdd(&s_next, 1);
+            g = __shfl_sync(FULL, g, 0);
+            if (g >= n_groups) break;
+            const int i0 = w_base + g * WT;
+            // ---- level 0, pass 1: minimum over the block samples, WT wires share the row loads ----
+            EvalC ec[WT];
+            double dmin[WT];
+#pragma unroll
+            for (int q = 0; q < WT; ++q) {
+                load_evalc(ec[q], a.wt, W, min(i0 + q, W - 1));
+                dmin[q] = INF;
+            }
+#pragma unroll 2
+            for (int t = 0; t < n0; ++t) {
+                double x0, x1, x2;
+                load_row(min(t * COMET_M0 + COMET_M0 / 2, kmax - 1), x0, x1, x2);
+#pragma unroll
+                for (int q = 0; q < WT; ++q) dmin[q] = fmin(dmin[q], d2_fma(ec[q], x0, x1, x2));
+            }
+            if (STATS) st_cnt[ST_SAMPLES] += (unsigned long long)n0 * min(WT, W - i0);
+            // ---- per wire: level 0 pass 2, level 1, row sweeps, then B3 ---------------------------
+#pragma unroll 1
+            for (int q = 0; q < WT; ++q) {
+                const int i = i0 + q;
+                if (i >= w_base + n_here) break;
+                EvalC w;
+                load_evalc(w, a.wt, W, i);           // warp-uniform, L1-resident
+                double dm = dmin[0];
+#pragma unroll
+                for (int r = 1; r < WT; ++r)
+                    if (q == r) dm = dmin[r];
+                const double cap = full ? INF : __ldg(a.wt + 14 * W + i);       // far radius R_i
+                double e2 = lam2;
+                if (STATS) st_cnt[ST_PAIRS] += 1;
+                if (cap >= 0.0) {                                              // wire has entries
+                    double ub = lip_ok ? fmin(sqrt(dm), cap) : INF;            // upper bound on min(D*, cap)
+                    const double t0 = ub + half0;
+                    const double thr0 = lip_ok ? t0 * t0 : INF;
+                    double best = INF;
+                    int bk = 0;
+                    for (int t = 0; t < n0; ++t) {
+                        const int r0 = t * COMET_M0;
+                        double x0, x1, x2;
+                        load_row(min(r0 + COMET_M0 / 2, kmax - 1), x0, x1, x2);
+                        const double ds = d2_fma(w, x0, x1, x2);
+                        if (STATS) st_cnt[ST_SAMPLES] += 1;
+                        if (!__any_sync(FULL, ds <= thr0)) continue;
+                        // level 1: sub-block samples of this block
+                        double d1[COMET_M0 / COMET_M1];
+                        double m1 = INF;
+#pragma unroll
+                        for (int j = 0; j < COMET_M0 / COMET_M1; ++j) {
+                            load_row(min(r0 + j * COMET_M1 + COMET_M1 / 2, kmax - 1), x0, x1, x2);
+                            d1[j] = d2_fma(w, x0, x1, x2);
+                            m1 = fmin(m1, d1[j]);
+                        }
+                        if (STATS) st_cnt[ST_SAMPLES] += COMET_M0 / COMET_M1;
+                        ub = fmin(ub, sqrt(m1));
+                        const double t1 = ub + half1;
+                        const double thr1 = lip_ok ? t1 * t1 : INF;
+#pragma unroll
+                        for (int j = 0; j < COMET_M0 / COMET_M1; ++j) {
+                            const int rj = r0 + j * COMET_M1;
+                            const bool need = d1[j] <= thr1;
+                            if (rj < kmax && __any_sync(FULL, need)) {
+                                const int rows = min(COMET_M1, kmax - rj);
+                                if (STATS) { st_cnt[ST_ROWS_EXEC] += rows; if (need) st_cnt[ST_ROWS_NEEDED] += rows; }
+#pragma unroll
+                                for (int kk = 0; kk < COMET_M1; ++kk) {
+                                    if (kk < rows) {
+                                        load_row(rj + kk, x0, x1, x2);
+                                        const double d2 = d2_fma(w, x0, x1, x2);
+                                        if (d2 < best) { best = d2; bk = rj + kk; }
+                                    }
+                                }
+                            }
+                        }
+                    }
+                    // near <=> the closest recorded state is within the far radius (always, in full mode)
+                    const bool near = valid && (best < INF) && (sqrt(best) <= cap || !lip_ok);
+                    if (STATS) { if (near) st_cnt[ST_FINE_NEEDED] += 1; }
+                    if (__any_sync(FULL, near)) {
+                        if (STATS) st_cnt[ST_FINE_EXEC] += 1;
+                        if (near) {
+                            double D;
+                            int ks;
+                            e2 = pair_exact(Xc, Tc, lane, bk, np, a, c, i, D, ks);
+                            if (a.dca) a.dca[(size_t)s * W + i] = D;
+                            if (a.kstar) a.kstar[(size_t)s * W + i] = ks;
+                        }
+                    }
+                }
+                e2s[(i - w_base) * 32 + lane] = e2;
+            }
+        }
+        __syncthreads();
+        // ---- B5: warp 0 adds the staged e^2 in wire order --------------------------------------
+        if (warp == 0) {
+            for (int j = 0; j < n_here; ++j) rss_acc = xadd(rss_acc, e2s[j * 32 + lane]);
+        }
+        __syncthreads();
+    }
+    if (warp == 0 && valid) a.rss[s] = rss_acc;
+    if (STATS) {
+#pragma unroll
+        for (int j = 0; j < ST_N; ++j) {
+            unsigned long long v = st_cnt[j];
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(FULL, v, o);
+            if (lane == 0 && a.stats) atomicAdd(a.stats + j, v);
+        }
+    }
 }
 
 }  // namespace comet

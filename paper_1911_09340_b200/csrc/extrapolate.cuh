@@ -3,14 +3,16 @@
 // One thread per seed, one warp per track chunk of 32 consecutive seeds.  Every step the warp
 // writes six fully coalesced 256-byte rows (3 position + 3 tangent components x 32 lanes), so the
 // stores run at 100 % sector efficiency -- the paper's AoS layout reached 25 %.
-// A lane that has reached the target region keeps writing a far-away sentinel position up to the
-// last row any lane of its chunk records, so kernel B can scan the chunk without a per-lane bound.
+// A lane that has reached the target region keeps writing its LAST recorded position up to the last
+// row any lane of its chunk records ("hold-last" padding).  Kernel B can then scan or sample the
+// chunk's rows without a per-lane bound: a padded row is at the same distance from any wire as the
+// lane's last state, so it never wins the strict "<" of the closest-state search (ties -> lowest k)
+// and it keeps the row-to-row displacement bounded by the step length, which the pruned search
+// relies on.  Lanes beyond n_seeds in a ragged last chunk hold zeros.
 #pragma once
 #include "common.cuh"
 
 namespace comet {
-
-#define COMET_SENTINEL 1.0e30
 
 __global__ void __launch_bounds__(128)
 k_extrapolate(const double* __restrict__ seeds, int64_t stride, int64_t n_seeds, double qkb, StepK hk,
@@ -28,7 +30,7 @@ k_extrapolate(const double* __restrict__ seeds, int64_t stride, int64_t n_seeds,
     if (active) {
         c = seed_init(seeds, stride, s, qkb, st);
     } else {
-        st.x0 = st.x1 = st.x2 = COMET_SENTINEL;
+        st.x0 = st.x1 = st.x2 = 0.0;
         st.t0 = st.t1 = st.t2 = 0.0;
     }
     size_t row = track_row(chunk, n_rows, 0) + lane;
@@ -45,7 +47,7 @@ k_extrapolate(const double* __restrict__ seeds, int64_t stride, int64_t n_seeds,
             T[row] = st.t0; T[row + 32] = st.t1; T[row + 64] = st.t2;
             if (use_stop && in_target_region(st, r_stop2)) { np = k + 1; active = false; }
         } else {
-            X[row] = COMET_SENTINEL; X[row + 32] = COMET_SENTINEL; X[row + 64] = COMET_SENTINEL;
+            X[row] = st.x0; X[row + 32] = st.x1; X[row + 64] = st.x2;      // hold-last padding
         }
     }
     if (s < n_seeds) n_pts[s] = np;

@@ -107,23 +107,36 @@ def test_extrapolate_seed_range_and_positron(comet, cfg1_event):
 # ------------------------------------------------------------------------------------------------
 # kernel B
 # ------------------------------------------------------------------------------------------------
-def _run_b(comet, d, cutoff=None, r_stop=None, **kw):
+MODES = ["pruned", "exhaustive"]
+
+
+def _set_mode(comet, mode):
+    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH
+    comet.set_option(OPT_COARSE_SEARCH, COARSE_PRUNED if mode == "pruned" else COARSE_EXHAUSTIVE)
+
+
+def _run_b(comet, d, cutoff=None, r_stop=None, mode="pruned", full=True, **kw):
+    """Kernel A + kernel B.  full=True asks for D and k* of every pair; full=False is the RSS-only
+    call the whole path makes (in pruned mode it also skips provably-far pairs)."""
     ev = d.ev
     r_stop = ev.r_stop if r_stop is None else r_stop
+    _set_mode(comet, mode)
     track, n_pts = comet.seed_extrapolate(d.seeds, ev.charge, ev.bz, ev.step, ev.n_steps, r_stop)
     out = comet.dca_rss(track, n_pts, d.seeds, *d.phys(), *d.hits(), ev.cutoff if cutoff is None else cutoff,
-                        want_dca=True, want_kstar=True, **kw)
+                        want_dca=full, want_kstar=full, **kw)
     torch.cuda.synchronize()
+    _set_mode(comet, "pruned")
     return {k: v.cpu().numpy() for k, v in out.items()}, n_pts.cpu().numpy()
 
 
+@pytest.mark.parametrize("mode", MODES)
 @pytest.mark.parametrize("r_stop", [50.0, 0.0])
-def test_dca_rss_matches_oracle_cfg0_full(comet, cfg0_event, r_stop):
+def test_dca_rss_matches_oracle_cfg0_full(comet, cfg0_event, r_stop, mode):
     """All 8192 seeds x 32 wires of configs[0]: 256 chunks, 1 pass of 32 wires."""
     ev = cfg0_event
     seeds, _ = event_seeds(ev)
     d = DevEvent(ev, seeds)
-    got, n_pts = _run_b(comet, d, r_stop=r_stop)
+    got, n_pts = _run_b(comet, d, r_stop=r_stop, mode=mode)
     ref = _oracle_scan(ev, seeds, r_stop=r_stop, want_dca=True, want_kstar=True, want_npts=True)
     np.testing.assert_array_equal(n_pts, ref["n_pts"])
     np.testing.assert_array_equal(got["kstar"], ref["kstar"])
@@ -132,9 +145,13 @@ def test_dca_rss_matches_oracle_cfg0_full(comet, cfg0_event, r_stop):
     # stronger than the bar: same operations in the same order
     assert np.array_equal(got["dca"], ref["dca"])
     assert np.array_equal(got["rss"], ref["rss"])
+    # the RSS-only call (pruned mode: far pairs take the cutoff without the plane iteration)
+    got2, _ = _run_b(comet, d, r_stop=r_stop, mode=mode, full=False)
+    assert np.array_equal(got2["rss"], ref["rss"])
 
 
-def test_dca_rss_cfg1_ragged(comet, cfg1_event):
+@pytest.mark.parametrize("mode", MODES)
+def test_dca_rss_cfg1_ragged(comet, cfg1_event, mode):
     """71 fired wires (3 passes of 24), truth seeds first, 2000-odd seeds with a ragged last chunk."""
     ev = cfg1_event
     seeds, _ = event_seeds(ev)
@@ -142,18 +159,22 @@ def test_dca_rss_cfg1_ragged(comet, cfg1_event):
     seeds = np.ascontiguousarray(np.concatenate([ts, seeds[:, ::191]], axis=1))
     assert seeds.shape[1] % 32 != 0
     d = DevEvent(ev, seeds)
-    got, n_pts = _run_b(comet, d)
+    got, n_pts = _run_b(comet, d, mode=mode)
     ref = _oracle_scan(ev, seeds, want_dca=True, want_kstar=True, want_npts=True)
     np.testing.assert_array_equal(n_pts, ref["n_pts"])
     np.testing.assert_array_equal(got["kstar"], ref["kstar"])
     _check_dca(got["dca"], ref["dca"])
     _check_rss(got["rss"], ref["rss"])
     assert np.array_equal(got["rss"], ref["rss"])
+    got2, _ = _run_b(comet, d, mode=mode, full=False)
+    assert np.array_equal(got2["rss"], ref["rss"])
 
 
-@pytest.mark.parametrize("n_fired", [1, 7, 33, 97])
-def test_dca_rss_wire_counts(comet, cfg1_event, n_fired):
-    """Every wires-per-warp instantiation (1..4) and partly filled last passes."""
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("n_fired", [1, 7, 33, 97, 300])
+def test_dca_rss_wire_counts(comet, cfg1_event, n_fired, mode):
+    """Every wires-per-warp instantiation (1..4), partly filled last passes / wire groups, and more
+    wires than one e^2 staging pass of the pruned kernel holds (256)."""
     import copy
     ev = copy.copy(cfg1_event)
     ev.fired_wire = cfg1_event.fired_wire[:min(n_fired, cfg1_event.n_fired)].copy()
@@ -167,11 +188,13 @@ def test_dca_rss_wire_counts(comet, cfg1_event, n_fired):
         ev.rho = cfg1_event.rho[:ev.hit_off[-1]].copy()
     seeds, _ = event_seeds(ev, shape=(3, 3, 4, 4))
     d = DevEvent(ev, seeds)
-    got, _ = _run_b(comet, d)
+    got, _ = _run_b(comet, d, mode=mode)
     ref = _oracle_scan(ev, seeds, want_dca=True, want_kstar=True)
     np.testing.assert_array_equal(got["kstar"], ref["kstar"])
     _check_dca(got["dca"], ref["dca"])
     _check_rss(got["rss"], ref["rss"])
+    got2, _ = _run_b(comet, d, mode=mode, full=False)
+    assert np.array_equal(got2["rss"], ref["rss"])
 
 
 def test_dca_rss_no_wires_and_no_seeds(comet, cfg0_event):
@@ -202,6 +225,9 @@ def test_high_occupancy_cutoff_sweep(comet):
         np.testing.assert_array_equal(got["kstar"], ref["kstar"])
         _check_dca(got["dca"], ref["dca"])
         _check_rss(got["rss"], ref["rss"])
+        for mode in MODES:
+            got2, _ = _run_b(comet, d, cutoff=lam, mode=mode, full=False)
+            assert np.array_equal(got2["rss"], ref["rss"]), mode
         if ref_d is not None:
             assert np.array_equal(got["dca"], ref_d)
         ref_d = got["dca"]
