@@ -37,7 +37,7 @@ FINE_INSTR = 600
 # 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz)
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of k_dca_rss per launch (profiles/, ncu --set full); None = not captured
-DCA_TRAFFIC_BYTES = None
+DCA_TRAFFIC_BYTES = {}
 
 
 def _event(cfg):
@@ -172,7 +172,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_1911_09340_b200 import Comet
-    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH, OPT_STATS
+    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH, OPT_STATS, OPT_TIMING
     from paper_1911_09340_b200.build import build
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -240,14 +240,26 @@ def run_ours(args):
     best = out["best_seed"].cpu().numpy().tolist()
     n_cls = int(out["cls"].sum().item())
 
-    # ---- work counters of the pruned search (one untimed launch) and the other mode's kernel time ---
-    stats = None
+    # ---- work counters and per-kernel device times of the pruned search (untimed extra launches) ---
+    stats, ktimes = None, None
     if args.coarse == "pruned":
         c.set_option(OPT_STATS, 1)
         c.read_stats(reset=True)
         c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss)
         stats = c.read_stats(reset=True)
         c.set_option(OPT_STATS, 0)
+        c.set_option(OPT_TIMING, 1)
+        acc = {}
+        n_t = 1 + min(args.steps, 10)
+        for i in range(n_t):
+            c.seed_extrapolate(d_seeds, *phys, ev.r_stop, track=track, n_pts=n_pts)   # as in a step: track rewritten
+            c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss)
+            t = c.read_timing()
+            if i:
+                for k, v in t.items():
+                    acc[k] = acc.get(k, 0.0) + v / (n_t - 1)
+        c.set_option(OPT_TIMING, 0)
+        ktimes = acc
     other = "exhaustive" if args.coarse == "pruned" else "pruned"
     c.set_option(OPT_COARSE_SEARCH, COARSE_EXHAUSTIVE if other == "exhaustive" else COARSE_PRUNED)
     rss2 = torch.empty_like(rss)
@@ -310,20 +322,30 @@ def run_ours(args):
         best_ms = min(best_ms, pe0.elapsed_time(pe1))
     peak_measured = 2 * n_fma / (best_ms * 1e-3) / 1e12
     flops_exh = 2.0 * (SHORTLIST_INSTR * n_states * W + FINE_INSTR * pairs)
+    peak = FP64_PEAK_NOMINAL_TFLOPS
     if stats is not None:
-        flops = 2.0 * (SHORTLIST_INSTR * (stats["samples"] + stats["rows_needed"]) + FINE_INSTR * stats["fine_needed"])
-        flops_exec = 2.0 * (SHORTLIST_INSTR * (stats["samples"] + stats["rows_executed"]) + FINE_INSTR * stats["fine_executed"])
-        kernel, model = "k_dca_rss_pruned", (
-            "FP64-pipe slots x 2 of the work the pruned search needs (thread-level counters, comet_read_stats): "
-            "%d per block/sub-block sample or row evaluation + %d per (seed, wire) pair that runs the plane iteration"
-            % (SHORTLIST_INSTR, FINE_INSTR))
-        ms_exh, flops_other = ms_other, flops_exh
+        fl = {"k_coarse_pruned": 2.0 * SHORTLIST_INSTR * (stats["samples"] + stats["rows_needed"]),
+              "k_fine": 2.0 * FINE_INSTR * stats["fine_needed"]}
+        fl_exec = {"k_coarse_pruned": 2.0 * SHORTLIST_INSTR * (stats["samples"] + stats["rows_executed"]),
+                   "k_fine": 2.0 * FINE_INSTR * stats["fine_executed"]}
+        kernels = {k: {"ms_per_launch": ktimes[k], "achieved": fl[k] / (ktimes[k] * 1e-3) / 1e12,
+                       "frac": fl[k] / (ktimes[k] * 1e-3) / 1e12 / peak,
+                       "achieved_executed": fl_exec[k] / (ktimes[k] * 1e-3) / 1e12,
+                       "share_of_step": ktimes[k] / ms_per_step} for k in fl}
+        kernels["k_rss_sum"] = {"ms_per_launch": ktimes["k_rss_sum"], "bound": "hbm",
+                                "achieved_gbs": (pairs * 8 + S * 8) / (ktimes["k_rss_sum"] * 1e-3) / 1e9}
+        kernel = max(fl, key=lambda k: ktimes[k])
+        ms_k, achieved = ktimes[kernel], kernels[kernel]["achieved"]
+        model = ("FP64-pipe slots x 2 of the work the pruned search needs (thread-level counters, comet_read_stats): "
+                 "k_coarse_pruned %d per block/sub-block sample or row evaluation; k_fine %d per (seed, wire) pair "
+                 "that runs the plane iteration" % (SHORTLIST_INSTR, FINE_INSTR))
+        ms_exh = ms_other
     else:
-        flops, flops_exec = flops_exh, flops_exh
-        kernel, model = "k_dca_rss", ("FP64-pipe slots x 2: %d per (seed, wire, recorded state) + %d per (seed, wire)"
-                                      % (SHORTLIST_INSTR, FINE_INSTR))
-        ms_exh, flops_other = ms_b, None
-    achieved = flops / (ms_b * 1e-3) / 1e12
+        kernels, kernel, ms_k = None, "k_dca_rss", ms_b
+        achieved = flops_exh / (ms_b * 1e-3) / 1e12
+        model = ("FP64-pipe slots x 2: %d per (seed, wire, recorded state) + %d per (seed, wire)"
+                 % (SHORTLIST_INSTR, FINE_INSTR))
+        ms_exh = ms_b
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -337,23 +359,24 @@ def run_ours(args):
         "result": {"best_seed": best, "classified_entries": n_cls, "recorded_states_per_seed": n_states / S},
         "e2e": {"value": world * pairs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_s * 1e3, "api": "comet_scan_event_host, pinned host buffers, %d GiB track slab" % (budget >> 30)},
-        "gpu_launches": 6 * args.steps,
+        "gpu_launches": (8 if args.coarse == "pruned" else 6) * args.steps,
         "clocks": clocks,
-        "roofline": {"kernel": kernel, "bound": "alu", "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS,
-                     "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": DCA_TRAFFIC_BYTES,
+        "roofline": {"kernel": kernel, "bound": "alu", "achieved": achieved, "peak": peak,
+                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": DCA_TRAFFIC_BYTES.get(kernel),
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 figure)",
                      "peak_measured_dfma_probe": peak_measured, "frac_of_measured": achieved / peak_measured,
-                     "ms_per_launch": ms_b, "share_of_step": ms_b / ms_per_step,
+                     "ms_per_launch": ms_k, "share_of_step": ms_k / ms_per_step,
                      "model": model,
-                     "achieved_executed": flops_exec / (ms_b * 1e-3) / 1e12,
+                     "comet_dca_rss_ms": ms_b, "comet_dca_rss_share_of_step": ms_b / ms_per_step,
+                     "kernels": kernels,
                      "work_counters": stats,
-                     "exhaustive_kernel": {"ms_per_launch": ms_exh, "achieved": flops_exh / (ms_exh * 1e-3) / 1e12,
-                                           "frac": flops_exh / (ms_exh * 1e-3) / 1e12 / FP64_PEAK_NOMINAL_TFLOPS,
+                     "exhaustive_kernel": {"kernel": "k_dca_rss", "ms_per_launch": ms_exh,
+                                           "achieved": flops_exh / (ms_exh * 1e-3) / 1e12,
+                                           "frac": flops_exh / (ms_exh * 1e-3) / 1e12 / peak,
                                            "model": "%d per (seed, wire, recorded state) + %d per (seed, wire)"
                                                     % (SHORTLIST_INSTR, FINE_INSTR)},
                      "other_mode": {"coarse_search": other, "ms_per_launch": ms_other, "rss_bit_identical": modes_agree},
-                     "algorithmic_hbm_bytes": n_states * 24 + n_states * 0 + pairs * 48,
-                     "hbm_gbs_if_read_once": (n_states * 24) / (ms_b * 1e-3) / 1e9},
+                     "track_bytes_read_once": n_states * 24},
     }
     if args.cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(ev, seeds, part_off)

@@ -48,6 +48,7 @@ typedef enum comet_status {
 #define COMET_COARSE_PRUNED 1         /*   default: block samples + Lipschitz bounds skip states that cannot be
                                        *   the closest one, and (when neither dca nor kstar is requested) pairs
                                        *   whose residual is provably the cutoff; k*, D and rss are identical   */
+#define COMET_OPT_TIMING 3            /* 1: comet_dca_rss (pruned) times its kernels, see comet_read_timing      */
 #define COMET_OPT_STATS 2             /* 1: comet_dca_rss (pruned) adds its work counters, see comet_read_stats  */
 
 /* ---- context ---------------------------------------------------------------------------- */
@@ -63,6 +64,19 @@ int comet_last_cuda_error(const comet_ctx* ctx);
 int comet_set_option(comet_ctx* ctx, int option, int value);
 int comet_get_option(const comet_ctx* ctx, int option, int* value);
 
+/* Sets the size of the (seed, wire) pair workspace of the pruned search to max_pairs_per_launch
+ * pairs (12 bytes each; default limit 2^26) and allocates it now, so that later comet_dca_rss calls
+ * never allocate.  comet_dca_rss processes larger problems in seed slabs that fit; without this
+ * call the workspace grows on the first comet_dca_rss that needs it (that call synchronises the
+ * device). */
+int comet_reserve(comet_ctx* ctx, int64_t max_pairs_per_launch);
+
+/* With COMET_OPT_TIMING = 1 the pruned comet_dca_rss records CUDA events on its stream around its
+ * three kernels.  Waits for the last such call and writes the device times in milliseconds of
+ * k_coarse_pruned, k_fine and k_rss_sum (of the call's last seed slab) to ms_host[0..n), n <= 3.
+ * COMET_EINVAL if no timed call was made. */
+int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n);
+
 /* Copies the work counters accumulated by comet_dca_rss calls made with COMET_OPT_STATS = 1 to
  * out_host[0..n) (HOST, n <= 6) and synchronises the stream; reset != 0 zeroes them afterwards.
  * Counters are thread-level: [0] block/sub-block sample evaluations, [1] row evaluations a lane
@@ -75,8 +89,10 @@ int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, int32_t rese
 
 /* Bytes of the opaque track buffer for n_seeds seeds and n_steps steps.
  * Layout (library-defined): two planes, positions X then unit tangents T, each
- * [n_chunks][n_steps+1][3][32] doubles with n_chunks = ceil(n_seeds/32): component c of
- * recorded state k of seed s is at ((s/32 * (n_steps+1) + k) * 3 + c) * 32 + s%32.
+ * [n_chunks][R][3][32] doubles with n_chunks = ceil(n_seeds/32) and R = n_steps+1 rounded up to
+ * a multiple of 8: component c of recorded state k of seed s is at ((s/32 * R + k) * 3 + c) * 32
+ * + s%32.  Position rows between a seed's last state and the end of its chunk's last 8-row group
+ * repeat the last state (padding read by kernel B).
  * Returns 0 for invalid arguments. */
 size_t comet_track_bytes(int64_t n_seeds, int32_t n_steps);
 

@@ -17,7 +17,7 @@ EXPORTED_SYMBOLS = [
     "comet_create", "comet_destroy", "comet_status_string", "comet_last_cuda_error",
     "comet_set_option", "comet_get_option", "comet_track_bytes", "comet_seed_extrapolate",
     "comet_track_export", "comet_dca_rss", "comet_select_and_classify", "comet_scan_event_host",
-    "comet_fp64_peak_probe", "comet_read_stats",
+    "comet_fp64_peak_probe", "comet_read_stats", "comet_reserve", "comet_read_timing",
 ]
 
 COMET_CHUNK = 32
@@ -25,6 +25,7 @@ OPT_COARSE_SEARCH = 1
 COARSE_EXHAUSTIVE = 0
 COARSE_PRUNED = 1
 OPT_STATS = 2
+OPT_TIMING = 3
 STATS_FIELDS = ("samples", "rows_needed", "rows_executed", "fine_needed", "fine_executed", "pairs")
 
 
@@ -70,6 +71,8 @@ def load_library():
                                         vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                         vp, i32, sz, vp, vp, vp, vp, vp, vp]
     L.comet_fp64_peak_probe.argtypes = [vp, i32, vp, ctypes.POINTER(dbl), vp]
+    L.comet_reserve.argtypes = [vp, i64]
+    L.comet_read_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32]
     L.comet_read_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), i32, i32, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("comet_status_string", "comet_track_bytes"):
@@ -133,6 +136,16 @@ class Comet:
         v = ctypes.c_int()
         self._check(self._L.comet_get_option(self._h, int(option), ctypes.byref(v)))
         return v.value
+
+    def reserve(self, max_pairs_per_launch: int):
+        """Pre-allocates the pruned search's (seed, wire) pair workspace (12 bytes per pair)."""
+        self._check(self._L.comet_reserve(self._h, int(max_pairs_per_launch)))
+
+    def read_timing(self) -> dict:
+        """Device milliseconds of the last pruned comet_dca_rss made with OPT_TIMING = 1 (waits for it)."""
+        buf = (ctypes.c_float * 3)()
+        self._check(self._L.comet_read_timing(self._h, buf, 3))
+        return {"k_coarse_pruned": float(buf[0]), "k_fine": float(buf[1]), "k_rss_sum": float(buf[2])}
 
     def read_stats(self, reset: bool = True, stream=None) -> dict:
         """Work counters of the pruned comet_dca_rss calls made with OPT_STATS = 1 (synchronises)."""

@@ -15,6 +15,7 @@
 #include "select.cuh"
 
 #define COMET_PRUNED_WT 4
+#define COMET_PR_CAP_S 96      // sub-block samples staged in shared memory per chunk (72 KB)
 
 using namespace comet;
 
@@ -23,8 +24,16 @@ struct comet_ctx {
     int last_cuda;
     int opt_coarse;
     int opt_stats;
+    int opt_timing;
     int n_sm;
-    unsigned long long* stats;   // device [ST_N] work counters of the pruned kernel
+    cudaEvent_t tev[4];          // COMET_OPT_TIMING: around k_coarse_pruned, k_fine, k_rss_sum
+    int tev_valid;
+    unsigned long long* stats;   // device [ST_N] work counters of the pruned kernels
+    // pair workspace of the pruned path: shortlisted state and e^2 per (wire, seed)
+    int32_t* kb;
+    double* e2;
+    size_t pair_cap;             // pairs the two buffers hold
+    size_t pair_max;             // growth limit (larger problems are processed in seed slabs)
     // device workspace
     double* wt;            // wire table [14][wt_cap]
     int32_t wt_cap;
@@ -84,9 +93,11 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaMalloc(&ctx->pi, sizeof(int64_t) * COMET_MAX_PARTITIONS * COMET_ARGMIN_SPLIT);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->stats, sizeof(unsigned long long) * ST_N);
     if (e == cudaSuccess) e = cudaMemset(ctx->stats, 0, sizeof(unsigned long long) * ST_N);
-    const int pr_smem = COMET_WSUP * 32 * (int)sizeof(double);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss_pruned<COMET_PRUNED_WT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss_pruned<COMET_PRUNED_WT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
+    ctx->pair_max = (size_t)1 << 26;
+    const int pr_smem = COMET_PR_CAP_S * 3 * COMET_LANES * (int)sizeof(double);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coarse_pruned<COMET_PRUNED_WT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coarse_pruned<COMET_PRUNED_WT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
+    for (int j = 0; j < 4 && e == cudaSuccess; ++j) e = cudaEventCreate(&ctx->tev[j]);
     // shared-memory opt-ins (done once here, never on the hot path)
     const int dca_smem = (2 * COMET_KT * 3 * COMET_LANES + COMET_DCA_WARPS * 4 * 32) * (int)sizeof(double);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
@@ -110,6 +121,8 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     if (!ctx) return COMET_EINVAL;
     cudaSetDevice(ctx->device);
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
+    cudaFree(ctx->kb); cudaFree(ctx->e2);
+    for (int j = 0; j < 4; ++j) if (ctx->tev[j]) cudaEventDestroy(ctx->tev[j]);
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf);
     delete ctx;
     return COMET_OK;
@@ -126,6 +139,11 @@ extern "C" int comet_set_option(comet_ctx* ctx, int option, int value)
         ctx->opt_stats = value;
         return COMET_OK;
     }
+    if (option == COMET_OPT_TIMING && (value == 0 || value == 1)) {
+        ctx->opt_timing = value;
+        ctx->tev_valid = 0;
+        return COMET_OK;
+    }
     return COMET_EINVAL;
 }
 
@@ -134,7 +152,19 @@ extern "C" int comet_get_option(const comet_ctx* ctx, int option, int* value)
     if (!ctx || !value) return COMET_EINVAL;
     if (option == COMET_OPT_COARSE_SEARCH) { *value = ctx->opt_coarse; return COMET_OK; }
     if (option == COMET_OPT_STATS) { *value = ctx->opt_stats; return COMET_OK; }
+    if (option == COMET_OPT_TIMING) { *value = ctx->opt_timing; return COMET_OK; }
     return COMET_EINVAL;
+}
+
+extern "C" int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n)
+{
+    if (!ctx || !ms_host || n < 0 || n > 3) return COMET_EINVAL;
+    if (!ctx->tev_valid) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    CU(ctx, cudaEventSynchronize(ctx->tev[3]));
+    for (int j = 0; j < n; ++j) CU(ctx, cudaEventElapsedTime(ms_host + j, ctx->tev[j], ctx->tev[j + 1]));
+    return COMET_OK;
 }
 
 extern "C" int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, int32_t reset, void* cuda_stream)
@@ -151,16 +181,44 @@ extern "C" int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, i
 
 static inline int64_t n_chunks_of(int64_t n_seeds) { return (n_seeds + COMET_LANES - 1) / COMET_LANES; }
 
+// grows the pair workspace to hold `pairs` (seed, wire) pairs (synchronises when it reallocates)
+static int ensure_pairs(comet_ctx* ctx, size_t pairs)
+{
+    if (pairs <= ctx->pair_cap) return COMET_OK;
+    CU(ctx, cudaDeviceSynchronize());
+    cudaFree(ctx->kb); cudaFree(ctx->e2);
+    ctx->kb = nullptr; ctx->e2 = nullptr; ctx->pair_cap = 0;
+    cudaError_t e = cudaMalloc(&ctx->kb, sizeof(int32_t) * pairs);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->e2, sizeof(double) * pairs);
+    if (e != cudaSuccess) {
+        ctx->last_cuda = (int)e;
+        cudaFree(ctx->kb); ctx->kb = nullptr;
+        cudaGetLastError();
+        return COMET_ENOMEM;
+    }
+    ctx->pair_cap = pairs;
+    return COMET_OK;
+}
+
+extern "C" int comet_reserve(comet_ctx* ctx, int64_t max_pairs_per_launch)
+{
+    if (!ctx || max_pairs_per_launch < COMET_LANES) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    ctx->pair_max = (size_t)max_pairs_per_launch;
+    return ensure_pairs(ctx, ctx->pair_max);
+}
+
 extern "C" size_t comet_track_bytes(int64_t n_seeds, int32_t n_steps)
 {
     if (n_seeds < 0 || n_steps < 1 || n_steps > COMET_MAX_STEPS) return 0;
-    return 2 * sizeof(double) * track_row(n_chunks_of(n_seeds), n_steps + 1, 0);
+    return 2 * sizeof(double) * track_row(n_chunks_of(n_seeds), track_rows(n_steps), 0);
 }
 
 static inline double* plane_X(void* track) { return (double*)track; }
 static inline double* plane_T(void* track, int64_t n_seeds, int32_t n_steps)
 {
-    return (double*)track + track_row(n_chunks_of(n_seeds), n_steps + 1, 0);
+    return (double*)track + track_row(n_chunks_of(n_seeds), track_rows(n_steps), 0);
 }
 
 static bool bad_physics(int32_t charge, double bz, double step, int32_t n_steps)
@@ -272,10 +330,58 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
     a.stats = ctx->opt_stats ? ctx->stats : nullptr;
     const unsigned blocks = (unsigned)n_chunks_of(n_seeds);
     const int threads = COMET_DCA_WARPS * 32;
+    (void)threads;
     if (ctx->opt_coarse == COMET_COARSE_PRUNED) {
-        const size_t smem = (size_t)(n_fired < COMET_WSUP ? (n_fired > 0 ? n_fired : 1) : COMET_WSUP) * 32 * sizeof(double);
-        if (ctx->opt_stats) k_dca_rss_pruned<COMET_PRUNED_WT, true><<<blocks, threads, smem, st>>>(a);
-        else k_dca_rss_pruned<COMET_PRUNED_WT, false><<<blocks, threads, smem, st>>>(a);
+        if (n_fired == 0) {
+            CU(ctx, cudaMemsetAsync(rss, 0, sizeof(double) * (size_t)n_seeds, st));
+            return COMET_OK;
+        }
+        // seed slabs so that (wires x padded seeds) fits the pair workspace
+        const int64_t total_chunks = n_chunks_of(n_seeds);
+        int64_t slab_chunks = (int64_t)(ctx->pair_max / ((size_t)COMET_LANES * (size_t)n_fired));
+        if (slab_chunks < 1) slab_chunks = 1;
+        if (slab_chunks > total_chunks) slab_chunks = total_chunks;
+        rc = ensure_pairs(ctx, (size_t)slab_chunks * COMET_LANES * (size_t)n_fired);
+        if (rc) return rc;
+        const int32_t n_rows = track_rows(n_steps);
+        for (int64_t c0 = 0; c0 < total_chunks; c0 += slab_chunks) {
+            const int64_t nc = (total_chunks - c0 < slab_chunks) ? (total_chunks - c0) : slab_chunks;
+            const int64_t s0 = c0 * COMET_LANES;
+            PrunedArgs pa;
+            pa.d = a;
+            pa.d.X = a.X + track_row(c0, n_rows, 0);
+            pa.d.T = a.T + track_row(c0, n_rows, 0);
+            pa.d.n_pts = n_pts + s0;
+            pa.d.seeds = seeds + s0;
+            pa.d.n_seeds = (n_seeds - s0 < nc * COMET_LANES) ? (n_seeds - s0) : nc * COMET_LANES;
+            pa.d.rss = rss + s0;
+            pa.d.dca = dca ? dca + (size_t)s0 * n_fired : nullptr;
+            pa.d.kstar = kstar ? kstar + (size_t)s0 * n_fired : nullptr;
+            pa.n_chunks = nc;
+            pa.SP = nc * COMET_LANES;
+            pa.n_groups = (n_fired + COMET_PRUNED_WT - 1) / COMET_PRUNED_WT;
+            pa.full = (dca || kstar) ? 1 : 0;
+            pa.kb = ctx->kb;
+            pa.e2 = ctx->e2;
+            pa.cap_s = track_rows(n_steps) / COMET_M1;
+            if (pa.cap_s > COMET_PR_CAP_S) pa.cap_s = COMET_PR_CAP_S;
+            const size_t sm1 = (size_t)pa.cap_s * 3 * COMET_LANES * sizeof(double);
+            const int64_t w2 = nc * (int64_t)n_fired;
+            const unsigned b1 = (unsigned)nc;
+            const unsigned b2 = (unsigned)((w2 + COMET_PR_WARPS - 1) / COMET_PR_WARPS);
+            const bool tm = ctx->opt_timing != 0;
+            if (tm) CU(ctx, cudaEventRecord(ctx->tev[0], st));
+            if (ctx->opt_stats) k_coarse_pruned<COMET_PRUNED_WT, true><<<b1, COMET_PR_WARPS * 32, sm1, st>>>(pa);
+            else k_coarse_pruned<COMET_PRUNED_WT, false><<<b1, COMET_PR_WARPS * 32, sm1, st>>>(pa);
+            if (tm) CU(ctx, cudaEventRecord(ctx->tev[1], st));
+            if (ctx->opt_stats) k_fine<true><<<b2, COMET_PR_WARPS * 32, 0, st>>>(pa);
+            else k_fine<false><<<b2, COMET_PR_WARPS * 32, 0, st>>>(pa);
+            if (tm) CU(ctx, cudaEventRecord(ctx->tev[2], st));
+            k_rss_sum<<<(unsigned)((pa.d.n_seeds + 255) / 256), 256, 0, st>>>(pa.e2, pa.SP, n_fired, pa.d.n_seeds, pa.d.rss);
+            if (tm) { CU(ctx, cudaEventRecord(ctx->tev[3], st)); ctx->tev_valid = 1; }
+            CU(ctx, cudaGetLastError());
+        }
+        return COMET_OK;
     } else {
         // wires per warp per pass: spread n_fired evenly over ceil(n_fired/32) passes of 8 warps
         const int n_pass = (n_fired + COMET_DCA_WARPS * 4 - 1) / (COMET_DCA_WARPS * 4);

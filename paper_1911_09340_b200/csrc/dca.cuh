@@ -141,7 +141,7 @@ __global__ void __launch_bounds__(COMET_DCA_WARPS * 32, 2) k_dca_rss(const DcaAr
     const int64_t chunk = blockIdx.x;
     const int64_t s = chunk * COMET_LANES + lane;
     const bool valid = s < a.n_seeds;
-    const int32_t n_rows = a.n_steps + 1;
+    const int32_t n_rows = track_rows(a.n_steps);
     const int32_t np = valid ? a.n_pts[s] : 0;
     const int32_t kmax = __reduce_max_sync(0xffffffffu, np);
     const int n_tiles = (kmax + COMET_KT - 1) / COMET_KT;
@@ -247,16 +247,18 @@ __global__ void __launch_bounds__(COMET_DCA_WARPS * 32, 2) k_dca_rss(const DcaAr
 // the virtual-plane iteration.  All bounds carry an absolute slack of 1e-9 cm for the rounding of
 // the FMA-form distances (~1e-13 cm).  Lanes with |c| h > 0.05 take no shortcut (ub = infinity).
 //
-// Mapping: CTA = one track chunk (lane = seed), warps take groups of WT wires from a CTA-wide
-// counter; rows come straight from global memory / L1 (coalesced 256-byte rows, read-only).
-// e^2 of up to COMET_WSUP wires is staged in shared memory and summed by warp 0 in wire order.
+// Three kernels, no barriers, no atomics in the data path (lane = seed of a track chunk everywhere):
+//   k_coarse_pruned  warp = (chunk, group of WT wires): shortlisted state bk per pair, -1 = far
+//   k_fine           warp = (chunk, wire): exact decision + virtual-plane iteration + residual -> e^2
+//   k_rss_sum        thread = seed: RSS = sum of e^2 in wire order (Eq. (1))
+// bk [W][SP] int32 and e^2 [W][SP] double (SP = 32 * number of chunks) live in the ctx workspace.
 // ---------------------------------------------------------------------------------------------
 #define COMET_M0 64
 #define COMET_M1 8
-#define COMET_WSUP 256
 #define COMET_CH_MAX 0.05
 #define COMET_LIP 1.001
 #define COMET_SLACK 1e-9
+#define COMET_PR_WARPS 8
 
 struct EvalC {
     double e1x, e1y, e1z, c1, e2x, e2y, e2z, c2;
@@ -275,170 +277,243 @@ __device__ __forceinline__ double d2_fma(const EvalC& w, double x0, double x1, d
     return fma(u1, u1, u2 * u2);
 }
 
-// optional work counters (COMET_OPT_STATS): lane-level needed work and warp-level executed work
+// optional work counters (COMET_OPT_STATS), thread-level
 enum { ST_SAMPLES = 0, ST_ROWS_NEEDED, ST_ROWS_EXEC, ST_FINE_NEEDED, ST_FINE_EXEC, ST_PAIRS, ST_N };
 
+struct PrunedArgs {
+    DcaArgs d;
+    int64_t n_chunks;
+    int64_t SP;              // 32 * n_chunks: stride of kb / e2
+    int32_t n_groups;        // ceil(W / WT)
+    int32_t cap_s;           // sub-block samples the shared-memory stage holds
+    int32_t full;            // dca or kstar requested: no far-pair shortcut
+    int32_t* kb;             // [W][SP]
+    double* e2;              // [W][SP]
+};
+
+// CTA = one track chunk.  The sub-block samples (row 8 j + 4 of every 8-row sub-block j, fp64) are
+// staged in shared memory once per CTA (up to `cap_s` of them; the rest is read from global memory);
+// both sampling levels run from there, so only the rows of opened sub-blocks are read from the track
+// buffer.  The level-0 sample of block t is sub-block sample 8 t + 4 (row 64 t + 36, at most 36 rows
+// from any row of the block).  Kernel A pads every chunk to whole sub-blocks (hold-last rows).
 template <int WT, bool STATS>
-__global__ void __launch_bounds__(COMET_DCA_WARPS * 32, 2) k_dca_rss_pruned(const DcaArgs a)
+__global__ void __launch_bounds__(COMET_PR_WARPS * 32) k_coarse_pruned(const PrunedArgs pa)
 {
     constexpr int ROW = 3 * COMET_LANES;
+    constexpr int NSUB = COMET_M0 / COMET_M1;               // sub-blocks per block
     constexpr unsigned FULL = 0xffffffffu;
-    extern __shared__ __align__(16) double e2s[];      // [min(W, WSUP)][32]
+    extern __shared__ __align__(16) double ssm[];           // [cap_s][ROW]
     __shared__ int s_next;
-
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const DcaArgs& a = pa.d;
+    const int lane = threadIdx.x & 31;
     const int64_t chunk = blockIdx.x;
     const int64_t s = chunk * COMET_LANES + lane;
     const bool valid = s < a.n_seeds;
-    const int32_t n_rows = a.n_steps + 1;
+    const int32_t n_rows = track_rows(a.n_steps);
     const int32_t np = valid ? a.n_pts[s] : 0;
     const int32_t kmax = __reduce_max_sync(FULL, np);
-    const int n0 = (kmax + COMET_M0 - 1) / COMET_M0;
-    const size_t base = track_row(chunk, n_rows, 0);
-    const double* __restrict__ Xc = a.X + base;
-    const double* __restrict__ Tc = a.T + base;
-    double c = 0.0;
+    const int nS = (kmax + COMET_M1 - 1) / COMET_M1;        // sub-blocks (all complete: kernel A pads)
+    const int n0 = (nS + NSUB - 1) / NSUB;                  // blocks (the last one may be partial)
+    const double* __restrict__ Xl = a.X + track_row(chunk, n_rows, 0) + lane;
+    const int nS_sm = min(nS, pa.cap_s);
+    // ---- stage the sub-block samples --------------------------------------------------------------
+    for (int v = threadIdx.x; v < nS_sm * (ROW / 2); v += COMET_PR_WARPS * 32) {
+        const int j = v / (ROW / 2), o = (v - j * (ROW / 2)) * 2;
+        cp_async16(ssm + j * ROW + o, Xl - lane + (size_t)(j * COMET_M1 + COMET_M1 / 2) * ROW + o);
+    }
+    cp_async_commit();
+    if (threadIdx.x == 0) s_next = 0;
+    double ch = 0.0;                                        // |c| h of this lane
     if (valid) {
         const double px = a.seeds[3 * a.stride + s], py = a.seeds[4 * a.stride + s], pz = a.seeds[5 * a.stride + s];
-        c = xdiv(a.qkb, xsqrt(xdot3(px, py, pz, px, py, pz)));
+        ch = fabs(a.qkb) * a.h / sqrt(px * px + py * py + pz * pz);
     }
     const int W = a.W;
-    const bool full = (a.dca != nullptr) || (a.kstar != nullptr);
-    const bool lip_ok = fabs(c) * a.h <= COMET_CH_MAX;       // Lipschitz bound valid for this lane
+    const bool lip_ok = ch <= COMET_CH_MAX;                 // Lipschitz bound valid for this lane
     const double L = COMET_LIP * a.h;
     const double INF = 1.7976931348623157e308;
-    const double half0 = (COMET_M0 / 2) * L + COMET_SLACK, half1 = (COMET_M1 / 2) * L + COMET_SLACK;
-    const double lam2 = xmul(a.lambda, a.lambda);
-    double rss_acc = 0.0;
+    const double half0 = (COMET_M0 / 2 + COMET_M1 / 2) * L + COMET_SLACK, half1 = (COMET_M1 / 2) * L + COMET_SLACK;
     unsigned long long st_cnt[ST_N];
     if (STATS) {
 #pragma unroll
         for (int j = 0; j < ST_N; ++j) st_cnt[j] = 0;
     }
-
-    auto load_row = [&](int k, double& x0, double& x1, double& x2) {
-        const double* xr = Xc + (size_t)k * ROW + lane;
-        x0 = __ldg(xr); x1 = __ldg(xr + 32); x2 = __ldg(xr + 64);
+    cp_async_wait<0>();
+    __syncthreads();
+    // sample of sub-block j (warp-uniform j)
+    auto load_sample = [&](int j, double& x0, double& x1, double& x2) {
+        if (j < nS_sm) {
+            const double* p = ssm + j * ROW + lane;
+            x0 = p[0]; x1 = p[32]; x2 = p[64];
+        } else {
+            const double* p = Xl + (size_t)(j * COMET_M1 + COMET_M1 / 2) * ROW;
+            x0 = __ldg(p); x1 = __ldg(p + 32); x2 = __ldg(p + 64);
+        }
     };
 
-    for (int w_base = 0; w_base < W; w_base += COMET_WSUP) {
-        const int n_here = min(COMET_WSUP, W - w_base);
-        const int n_groups = (n_here + WT - 1) / WT;
-        if (threadIdx.x == 0) s_next = 0;
-        __syncthreads();
-        while (true) {
-            int g = 0;
-            if (lane == 0) g = atomicAdd(&s_next, 1);
-            g = __shfl_sync(FULL, g, 0);
-            if (g >= n_groups) break;
-            const int i0 = w_base + g * WT;
-            // ---- level 0, pass 1: minimum over the block samples, WT wires share the row loads ----
+    while (true) {
+        int g = 0;
+        if (lane == 0) g = atomicAdd(&s_next, 1);
+        g = __shfl_sync(FULL, g, 0);
+        if (g >= pa.n_groups) break;
+        const int i0 = g * WT;
+        // ---- level 0: minimum over the block samples, then the blocks within reach of it ------------
+        double thr0[WT];
+        unsigned long long mask[WT];                        // bit t: block t may hold the closest state
+        {
             EvalC ec[WT];
             double dmin[WT];
 #pragma unroll
             for (int q = 0; q < WT; ++q) {
                 load_evalc(ec[q], a.wt, W, min(i0 + q, W - 1));
                 dmin[q] = INF;
+                mask[q] = 0ull;
             }
 #pragma unroll 2
             for (int t = 0; t < n0; ++t) {
                 double x0, x1, x2;
-                load_row(min(t * COMET_M0 + COMET_M0 / 2, kmax - 1), x0, x1, x2);
+                load_sample(min(t * NSUB + NSUB / 2, nS - 1), x0, x1, x2);
 #pragma unroll
                 for (int q = 0; q < WT; ++q) dmin[q] = fmin(dmin[q], d2_fma(ec[q], x0, x1, x2));
             }
-            if (STATS) st_cnt[ST_SAMPLES] += (unsigned long long)n0 * min(WT, W - i0);
-            // ---- per wire: level 0 pass 2, level 1, row sweeps, then B3 ---------------------------
-#pragma unroll 1
+#pragma unroll
             for (int q = 0; q < WT; ++q) {
-                const int i = i0 + q;
-                if (i >= w_base + n_here) break;
+                const double cap = pa.full ? INF : __ldg(a.wt + 14 * W + min(i0 + q, W - 1));   // far radius R_i
+                const double ub = fmin(sqrt(dmin[q]), cap);          // upper bound on min(D*, cap)
+                const double t0 = ub + half0;
+                thr0[q] = lip_ok ? t0 * t0 : INF;
+                if (cap < 0.0) thr0[q] = -1.0;                       // wire without entries: nothing to find
+            }
+            for (int t = 0; t < n0; ++t) {
+                double x0, x1, x2;
+                load_sample(min(t * NSUB + NSUB / 2, nS - 1), x0, x1, x2);
+#pragma unroll
+                for (int q = 0; q < WT; ++q)
+                    if (d2_fma(ec[q], x0, x1, x2) <= thr0[q]) mask[q] |= 1ull << (t & 63);
+            }
+            if (STATS) st_cnt[ST_SAMPLES] += 2ull * n0 * min(WT, W - i0);
+        }
+        // ---- per wire: level 1 in the opened blocks, row sweeps of the opened sub-blocks ------------
+#pragma unroll 1
+        for (int q = 0; q < WT; ++q) {
+            const int i = i0 + q;
+            if (i >= W) break;
+            unsigned long long mq = mask[0];
+            double th0 = thr0[0];
+#pragma unroll
+            for (int r = 1; r < WT; ++r)
+                if (q == r) { mq = mask[r]; th0 = thr0[r]; }
+            // blocks any lane wants (n0 <= 64 always fits; beyond that the bit is shared, still a superset)
+            unsigned mlo = __reduce_or_sync(FULL, (unsigned)mq), mhi = __reduce_or_sync(FULL, (unsigned)(mq >> 32));
+            const unsigned long long wm = ((unsigned long long)mhi << 32) | mlo;
+            if (STATS) st_cnt[ST_PAIRS] += 1;
+            int bk = -1;
+            if (wm) {
+                const double cap = pa.full ? INF : __ldg(a.wt + 14 * W + i);
                 EvalC w;
-                load_evalc(w, a.wt, W, i);           // warp-uniform, L1-resident
-                double dm = dmin[0];
+                load_evalc(w, a.wt, W, i);                           // warp-uniform, L1-resident
+                double best = INF;
+                double ub = lip_ok ? sqrt(th0) - half0 : INF;        // = min(sqrt(dmin), cap)
+                for (int t = 0; t < n0; ++t) {
+                    if (!((wm >> (t & 63)) & 1ull)) continue;
+                    const int j0 = t * NSUB;
+                    const int nj = min(NSUB, nS - j0);
+                    double d1[NSUB];
+                    double m1 = INF;
 #pragma unroll
-                for (int r = 1; r < WT; ++r)
-                    if (q == r) dm = dmin[r];
-                const double cap = full ? INF : __ldg(a.wt + 14 * W + i);       // far radius R_i
-                double e2 = lam2;
-                if (STATS) st_cnt[ST_PAIRS] += 1;
-                if (cap >= 0.0) {                                              // wire has entries
-                    double ub = lip_ok ? fmin(sqrt(dm), cap) : INF;            // upper bound on min(D*, cap)
-                    const double t0 = ub + half0;
-                    const double thr0 = lip_ok ? t0 * t0 : INF;
-                    double best = INF;
-                    int bk = 0;
-                    for (int t = 0; t < n0; ++t) {
-                        const int r0 = t * COMET_M0;
+                    for (int j = 0; j < NSUB; ++j) {
                         double x0, x1, x2;
-                        load_row(min(r0 + COMET_M0 / 2, kmax - 1), x0, x1, x2);
-                        const double ds = d2_fma(w, x0, x1, x2);
-                        if (STATS) st_cnt[ST_SAMPLES] += 1;
-                        if (!__any_sync(FULL, ds <= thr0)) continue;
-                        // level 1: sub-block samples of this block
-                        double d1[COMET_M0 / COMET_M1];
-                        double m1 = INF;
+                        load_sample(min(j0 + j, nS - 1), x0, x1, x2);
+                        d1[j] = d2_fma(w, x0, x1, x2);
+                        m1 = fmin(m1, d1[j]);
+                    }
+                    if (STATS) st_cnt[ST_SAMPLES] += nj;
+                    ub = fmin(ub, sqrt(m1));
+                    const double t1 = ub + half1;
+                    const double thr1 = lip_ok ? t1 * t1 : INF;
 #pragma unroll
-                        for (int j = 0; j < COMET_M0 / COMET_M1; ++j) {
-                            load_row(min(r0 + j * COMET_M1 + COMET_M1 / 2, kmax - 1), x0, x1, x2);
-                            d1[j] = d2_fma(w, x0, x1, x2);
-                            m1 = fmin(m1, d1[j]);
-                        }
-                        if (STATS) st_cnt[ST_SAMPLES] += COMET_M0 / COMET_M1;
-                        ub = fmin(ub, sqrt(m1));
-                        const double t1 = ub + half1;
-                        const double thr1 = lip_ok ? t1 * t1 : INF;
+                    for (int j = 0; j < NSUB; ++j) {
+                        const bool need = d1[j] <= thr1;
+                        if (j < nj && __any_sync(FULL, need)) {
+                            if (STATS) { st_cnt[ST_ROWS_EXEC] += COMET_M1; if (need) st_cnt[ST_ROWS_NEEDED] += COMET_M1; }
+                            const int rj = (j0 + j) * COMET_M1;
+                            const double* p = Xl + (size_t)rj * ROW;
+                            double xr[COMET_M1][3];
 #pragma unroll
-                        for (int j = 0; j < COMET_M0 / COMET_M1; ++j) {
-                            const int rj = r0 + j * COMET_M1;
-                            const bool need = d1[j] <= thr1;
-                            if (rj < kmax && __any_sync(FULL, need)) {
-                                const int rows = min(COMET_M1, kmax - rj);
-                                if (STATS) { st_cnt[ST_ROWS_EXEC] += rows; if (need) st_cnt[ST_ROWS_NEEDED] += rows; }
+                            for (int kk = 0; kk < COMET_M1; ++kk) {
+                                xr[kk][0] = __ldg(p + kk * ROW); xr[kk][1] = __ldg(p + kk * ROW + 32);
+                                xr[kk][2] = __ldg(p + kk * ROW + 64);
+                            }
 #pragma unroll
-                                for (int kk = 0; kk < COMET_M1; ++kk) {
-                                    if (kk < rows) {
-                                        load_row(rj + kk, x0, x1, x2);
-                                        const double d2 = d2_fma(w, x0, x1, x2);
-                                        if (d2 < best) { best = d2; bk = rj + kk; }
-                                    }
-                                }
+                            for (int kk = 0; kk < COMET_M1; ++kk) {
+                                const double d2 = d2_fma(w, xr[kk][0], xr[kk][1], xr[kk][2]);
+                                if (d2 < best) { best = d2; bk = rj + kk; }
                             }
                         }
                     }
-                    // near <=> the closest recorded state is within the far radius (always, in full mode)
-                    const bool near = valid && (best < INF) && (sqrt(best) <= cap || !lip_ok);
-                    if (STATS) { if (near) st_cnt[ST_FINE_NEEDED] += 1; }
-                    if (__any_sync(FULL, near)) {
-                        if (STATS) st_cnt[ST_FINE_EXEC] += 1;
-                        if (near) {
-                            double D;
-                            int ks;
-                            e2 = pair_exact(Xc, Tc, lane, bk, np, a, c, i, D, ks);
-                            if (a.dca) a.dca[(size_t)s * W + i] = D;
-                            if (a.kstar) a.kstar[(size_t)s * W + i] = ks;
-                        }
-                    }
                 }
-                e2s[(i - w_base) * 32 + lane] = e2;
+                // near <=> the closest recorded state is within the far radius (always, in full mode)
+                const bool near = (bk >= 0) && (sqrt(best) <= cap || !lip_ok);
+                if (!near) bk = -1;
             }
+            if (STATS && bk >= 0) st_cnt[ST_FINE_NEEDED] += 1;
+            pa.kb[(size_t)i * pa.SP + s] = bk;
         }
-        __syncthreads();
-        // ---- B5: warp 0 adds the staged e^2 in wire order --------------------------------------
-        if (warp == 0) {
-            for (int j = 0; j < n_here; ++j) rss_acc = xadd(rss_acc, e2s[j * 32 + lane]);
-        }
-        __syncthreads();
     }
-    if (warp == 0 && valid) a.rss[s] = rss_acc;
     if (STATS) {
 #pragma unroll
         for (int j = 0; j < ST_N; ++j) {
             unsigned long long v = st_cnt[j];
             for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(FULL, v, o);
-            if (lane == 0 && a.stats) atomicAdd(a.stats + j, v);
+            if (lane == 0 && a.stats && v) atomicAdd(a.stats + j, v);
         }
     }
+}
+
+// warp = (chunk, wire): B2 decision + B3 + B4 for the pairs the coarse search kept
+template <bool STATS>
+__global__ void __launch_bounds__(COMET_PR_WARPS * 32) k_fine(const PrunedArgs pa)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    const DcaArgs& a = pa.d;
+    const int lane = threadIdx.x & 31;
+    const int64_t wid = (int64_t)blockIdx.x * COMET_PR_WARPS + (threadIdx.x >> 5);
+    const int W = a.W;
+    if (wid >= pa.n_chunks * W) return;
+    const int64_t chunk = wid / W;
+    const int i = (int)(wid - chunk * W);
+    const int64_t s = chunk * COMET_LANES + lane;
+    const bool valid = s < a.n_seeds;
+    const int bk = pa.kb[(size_t)i * pa.SP + s];
+    const bool near = valid && bk >= 0;
+    double e2 = xmul(a.lambda, a.lambda);
+    if (__any_sync(FULL, near)) {
+        if (STATS) { if (lane == 0 && a.stats) atomicAdd(a.stats + ST_FINE_EXEC, 32ull); }
+        if (near) {
+            const int32_t n_rows = track_rows(a.n_steps);
+            const size_t base = track_row(chunk, n_rows, 0);
+            const double px = a.seeds[3 * a.stride + s], py = a.seeds[4 * a.stride + s], pz = a.seeds[5 * a.stride + s];
+            const double c = xdiv(a.qkb, xsqrt(xdot3(px, py, pz, px, py, pz)));
+            double D;
+            int ks;
+            e2 = pair_exact(a.X + base, a.T + base, lane, bk, a.n_pts[s], a, c, i, D, ks);
+            if (a.dca) a.dca[(size_t)s * W + i] = D;
+            if (a.kstar) a.kstar[(size_t)s * W + i] = ks;
+        }
+    }
+    pa.e2[(size_t)i * pa.SP + s] = e2;
+}
+
+// B5: RSS_s = sum_i e^2_i in increasing wire order (Eq. (1); no atomics, cf. :374)
+__global__ void __launch_bounds__(256) k_rss_sum(const double* __restrict__ e2, int64_t SP, int32_t W,
+                                                 int64_t n_seeds, double* __restrict__ rss)
+{
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n_seeds) return;
+    double acc = 0.0;
+#pragma unroll 4
+    for (int i = 0; i < W; ++i) acc = xadd(acc, e2[(size_t)i * SP + s]);
+    rss[s] = acc;
 }
 
 }  // namespace comet

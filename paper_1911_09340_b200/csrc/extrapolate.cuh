@@ -22,7 +22,7 @@ k_extrapolate(const double* __restrict__ seeds, int64_t stride, int64_t n_seeds,
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31;
     const int64_t chunk = s >> 5;
-    const int32_t n_rows = n_steps + 1;
+    const int32_t n_rows = track_rows(n_steps);
     if (chunk * COMET_LANES >= n_seeds) return;          // whole warp out of range
     bool active = s < n_seeds;
     State st;
@@ -36,9 +36,10 @@ k_extrapolate(const double* __restrict__ seeds, int64_t stride, int64_t n_seeds,
     size_t row = track_row(chunk, n_rows, 0) + lane;
     X[row] = st.x0; X[row + 32] = st.x1; X[row + 64] = st.x2;
     T[row] = st.t0; T[row + 32] = st.t1; T[row + 64] = st.t2;
-    int32_t np = n_rows;
+    int32_t np = n_steps + 1;
     const bool use_stop = r_stop2 > 0.0;
-    for (int32_t k = 1; k <= n_steps; ++k) {
+    int32_t k = 1;
+    for (; k <= n_steps; ++k) {
         if (!__any_sync(0xffffffffu, active)) break;
         row += 3 * COMET_LANES;
         if (active) {
@@ -50,6 +51,11 @@ k_extrapolate(const double* __restrict__ seeds, int64_t stride, int64_t n_seeds,
             X[row] = st.x0; X[row + 32] = st.x1; X[row + 64] = st.x2;      // hold-last padding
         }
     }
+    // pad the chunk to whole 8-row sub-blocks (rows k .. next multiple of 8; they exist: n_rows % 8 == 0)
+    for (; k & 7; ++k) {
+        row += 3 * COMET_LANES;
+        X[row] = st.x0; X[row + 32] = st.x1; X[row + 64] = st.x2;
+    }
     if (s < n_seeds) n_pts[s] = np;
 }
 
@@ -58,13 +64,13 @@ __global__ void k_track_export(const double* __restrict__ X, const double* __res
                                const int32_t* __restrict__ n_pts, int32_t n_steps, int64_t seed_begin,
                                int64_t seed_end, double* __restrict__ out)
 {
-    const int32_t n_rows = n_steps + 1;
-    const int64_t total = (seed_end - seed_begin) * (int64_t)n_rows;
+    const int32_t n_out = n_steps + 1;
+    const int64_t total = (seed_end - seed_begin) * (int64_t)n_out;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total;
          i += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t s = seed_begin + i / n_rows;
-        const int32_t k = (int32_t)(i % n_rows);
-        const size_t row = track_row(s >> 5, n_rows, k) + (size_t)(s & 31);
+        const int64_t s = seed_begin + i / n_out;
+        const int32_t k = (int32_t)(i % n_out);
+        const size_t row = track_row(s >> 5, track_rows(n_steps), k) + (size_t)(s & 31);
         const bool ok = k < n_pts[s];
         const double nan = __longlong_as_double(0x7ff8000000000000LL);
         double* o = out + (size_t)i * 6;
