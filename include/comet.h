@@ -90,8 +90,8 @@ int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, int32_t rese
 /* Bytes of the opaque track buffer for n_seeds seeds and n_steps steps.
  * Layout (library-defined): two planes, positions X then unit tangents T, each
  * [n_chunks][R][3][32] doubles with n_chunks = ceil(n_seeds/32) and R = n_steps+1 rounded up to
- * a multiple of 8: component c of recorded state k of seed s is at ((s/32 * R + k) * 3 + c) * 32
- * + s%32.  Position rows between a seed's last state and the end of its chunk's last 8-row group
+ * a multiple of 64: component c of recorded state k of seed s is at ((s/32 * R + k) * 3 + c) * 32
+ * + s%32.  Position rows between a seed's last state and the end of its chunk's last 64-row block
  * repeat the last state (padding read by kernel B).
  * Returns 0 for invalid arguments. */
 size_t comet_track_bytes(int64_t n_seeds, int32_t n_steps);

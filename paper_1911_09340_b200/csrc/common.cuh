@@ -103,9 +103,13 @@ __device__ __forceinline__ bool in_target_region(const State& s, double r_stop2)
 }
 
 // Track buffer: plane [n_chunks][n_rows][3][32]; index of (chunk, k, component 0, lane 0).
-// n_rows = track_rows(n_steps): n_steps + 1 recorded states rounded up to a multiple of 8 rows, so
-// that kernel A can pad every chunk to whole 8-row sub-blocks (hold-last) for the pruned search.
-__device__ __host__ __forceinline__ int32_t track_rows(int32_t n_steps) { return (n_steps + 8) & ~7; }
+// n_rows = track_rows(n_steps): n_steps + 1 recorded states rounded up to a multiple of 64 rows, so
+// that kernel A can pad every chunk to whole 64-row blocks (hold-last) for the pruned search.
+#define COMET_ROW_PAD 64
+__device__ __host__ __forceinline__ int32_t track_rows(int32_t n_steps)
+{
+    return (n_steps + COMET_ROW_PAD) & ~(COMET_ROW_PAD - 1);
+}
 __device__ __host__ __forceinline__ size_t track_row(int64_t chunk, int32_t n_rows, int32_t k)
 {
     return ((size_t)chunk * (size_t)n_rows + (size_t)k) * (size_t)(3 * COMET_LANES);

@@ -292,120 +292,91 @@ struct PrunedArgs {
 };
 
 // CTA = one track chunk.  The sub-block samples (row 8 j + 4 of every 8-row sub-block j, fp64) are
-// staged in shared memory once per CTA (up to `cap_s` of them; the rest is read from global memory);
-// both sampling levels run from there, so only the rows of opened sub-blocks are read from the track
-// buffer.  The level-0 sample of block t is sub-block sample 8 t + 4 (row 64 t + 36, at most 36 rows
-// from any row of the block).  Kernel A pads every chunk to whole sub-blocks (hold-last rows).
-template <int WT, bool STATS>
-__global__ void __launch_bounds__(COMET_PR_WARPS * 32) k_coarse_pruned(const PrunedArgs pa)
+// staged in shared memory once per CTA when they fit (`cap_s` of them; else they are read from
+// global memory): both sampling levels run from there, only the rows of opened sub-blocks are read
+// from the track buffer.  The level-0 sample of block t is sub-block sample 8 t + 4 (row 64 t + 36,
+// at most 36 rows from any row of the block).  Kernel A pads every chunk to whole 64-row blocks
+// (hold-last rows), so no index is ever clamped.
+//
+// Thresholds are compared on the high 32 bits of the (non-negative) squared distances: hi(d) <=
+// hi(thr) whenever d <= thr, so the integer test accepts a superset -- still a correct pruning --
+// and the minimum over samples is tracked as the integer minimum of the high words, rounded up.
+template <int WT, bool STATS, bool SMEM>
+__device__ __forceinline__ void coarse_groups(const PrunedArgs& pa, const double* __restrict__ Xl,
+                                              const double* sbase, int n0, int lane, int64_t s, bool lip_ok,
+                                              int* s_next, unsigned long long* st_cnt)
 {
     constexpr int ROW = 3 * COMET_LANES;
     constexpr int NSUB = COMET_M0 / COMET_M1;               // sub-blocks per block
+    constexpr int SST = SMEM ? ROW : COMET_M1 * ROW;        // distance between sub-block samples (doubles)
     constexpr unsigned FULL = 0xffffffffu;
-    extern __shared__ __align__(16) double ssm[];           // [cap_s][ROW]
-    __shared__ int s_next;
+    constexpr int IMAX = 0x7fffffff;
     const DcaArgs& a = pa.d;
-    const int lane = threadIdx.x & 31;
-    const int64_t chunk = blockIdx.x;
-    const int64_t s = chunk * COMET_LANES + lane;
-    const bool valid = s < a.n_seeds;
-    const int32_t n_rows = track_rows(a.n_steps);
-    const int32_t np = valid ? a.n_pts[s] : 0;
-    const int32_t kmax = __reduce_max_sync(FULL, np);
-    const int nS = (kmax + COMET_M1 - 1) / COMET_M1;        // sub-blocks (all complete: kernel A pads)
-    const int n0 = (nS + NSUB - 1) / NSUB;                  // blocks (the last one may be partial)
-    const double* __restrict__ Xl = a.X + track_row(chunk, n_rows, 0) + lane;
-    const int nS_sm = min(nS, pa.cap_s);
-    // ---- stage the sub-block samples --------------------------------------------------------------
-    for (int v = threadIdx.x; v < nS_sm * (ROW / 2); v += COMET_PR_WARPS * 32) {
-        const int j = v / (ROW / 2), o = (v - j * (ROW / 2)) * 2;
-        cp_async16(ssm + j * ROW + o, Xl - lane + (size_t)(j * COMET_M1 + COMET_M1 / 2) * ROW + o);
-    }
-    cp_async_commit();
-    if (threadIdx.x == 0) s_next = 0;
-    double ch = 0.0;                                        // |c| h of this lane
-    if (valid) {
-        const double px = a.seeds[3 * a.stride + s], py = a.seeds[4 * a.stride + s], pz = a.seeds[5 * a.stride + s];
-        ch = fabs(a.qkb) * a.h / sqrt(px * px + py * py + pz * pz);
-    }
     const int W = a.W;
-    const bool lip_ok = ch <= COMET_CH_MAX;                 // Lipschitz bound valid for this lane
     const double L = COMET_LIP * a.h;
     const double INF = 1.7976931348623157e308;
     const double half0 = (COMET_M0 / 2 + COMET_M1 / 2) * L + COMET_SLACK, half1 = (COMET_M1 / 2) * L + COMET_SLACK;
-    unsigned long long st_cnt[ST_N];
-    if (STATS) {
-#pragma unroll
-        for (int j = 0; j < ST_N; ++j) st_cnt[j] = 0;
-    }
-    cp_async_wait<0>();
-    __syncthreads();
-    // sample of sub-block j (warp-uniform j)
-    auto load_sample = [&](int j, double& x0, double& x1, double& x2) {
-        if (j < nS_sm) {
-            const double* p = ssm + j * ROW + lane;
-            x0 = p[0]; x1 = p[32]; x2 = p[64];
-        } else {
-            const double* p = Xl + (size_t)(j * COMET_M1 + COMET_M1 / 2) * ROW;
-            x0 = __ldg(p); x1 = __ldg(p + 32); x2 = __ldg(p + 64);
-        }
-    };
 
     while (true) {
         int g = 0;
-        if (lane == 0) g = atomicAdd(&s_next, 1);
+        if (lane == 0) g = atomicAdd(s_next, 1);
         g = __shfl_sync(FULL, g, 0);
         if (g >= pa.n_groups) break;
         const int i0 = g * WT;
         // ---- level 0: minimum over the block samples, then the blocks within reach of it ------------
-        double thr0[WT];
-        unsigned long long mask[WT];                        // bit t: block t may hold the closest state
+        double ub0[WT];                                     // min(sqrt(min sample), far radius)
+        unsigned mask[WT];                                  // bit t % 32: block t may hold the closest state
+        bool any_cand = false;
         {
             EvalC ec[WT];
-            double dmin[WT];
+            int dh[WT], thi[WT];
 #pragma unroll
             for (int q = 0; q < WT; ++q) {
                 load_evalc(ec[q], a.wt, W, min(i0 + q, W - 1));
-                dmin[q] = INF;
-                mask[q] = 0ull;
+                dh[q] = IMAX;
+                mask[q] = 0u;
             }
+            const double* p = sbase + (NSUB / 2) * SST;
 #pragma unroll 2
-            for (int t = 0; t < n0; ++t) {
-                double x0, x1, x2;
-                load_sample(min(t * NSUB + NSUB / 2, nS - 1), x0, x1, x2);
+            for (int t = 0; t < n0; ++t, p += NSUB * SST) {
+                const double x0 = p[0], x1 = p[32], x2 = p[64];
 #pragma unroll
-                for (int q = 0; q < WT; ++q) dmin[q] = fmin(dmin[q], d2_fma(ec[q], x0, x1, x2));
+                for (int q = 0; q < WT; ++q) dh[q] = min(dh[q], __double2hiint(d2_fma(ec[q], x0, x1, x2)));
             }
 #pragma unroll
             for (int q = 0; q < WT; ++q) {
                 const double cap = pa.full ? INF : __ldg(a.wt + 14 * W + min(i0 + q, W - 1));   // far radius R_i
-                const double ub = fmin(sqrt(dmin[q]), cap);          // upper bound on min(D*, cap)
-                const double t0 = ub + half0;
-                thr0[q] = lip_ok ? t0 * t0 : INF;
-                if (cap < 0.0) thr0[q] = -1.0;                       // wire without entries: nothing to find
+                const double dm = __hiloint2double(dh[q] + 1, 0);    // >= the smallest sample
+                ub0[q] = lip_ok ? fmin(sqrt(dm), cap) : INF;
+                const double t0 = ub0[q] + half0;
+                thi[q] = lip_ok ? __double2hiint(t0 * t0) : IMAX;
+                if (cap < 0.0 || i0 + q >= W) thi[q] = -1;           // wire without entries / past the end
+                any_cand |= dh[q] <= thi[q];
             }
-            for (int t = 0; t < n0; ++t) {
-                double x0, x1, x2;
-                load_sample(min(t * NSUB + NSUB / 2, nS - 1), x0, x1, x2);
+            if (STATS) st_cnt[ST_SAMPLES] += (unsigned long long)n0 * min(WT, W - i0);
+            if (__any_sync(FULL, any_cand)) {
+                p = sbase + (NSUB / 2) * SST;
+                for (int t = 0; t < n0; ++t, p += NSUB * SST) {
+                    const double x0 = p[0], x1 = p[32], x2 = p[64];
+                    const unsigned bit = 1u << (t & 31);
 #pragma unroll
-                for (int q = 0; q < WT; ++q)
-                    if (d2_fma(ec[q], x0, x1, x2) <= thr0[q]) mask[q] |= 1ull << (t & 63);
+                    for (int q = 0; q < WT; ++q)
+                        if (__double2hiint(d2_fma(ec[q], x0, x1, x2)) <= thi[q]) mask[q] |= bit;
+                }
+                if (STATS) st_cnt[ST_SAMPLES] += (unsigned long long)n0 * min(WT, W - i0);
             }
-            if (STATS) st_cnt[ST_SAMPLES] += 2ull * n0 * min(WT, W - i0);
         }
         // ---- per wire: level 1 in the opened blocks, row sweeps of the opened sub-blocks ------------
 #pragma unroll 1
         for (int q = 0; q < WT; ++q) {
             const int i = i0 + q;
             if (i >= W) break;
-            unsigned long long mq = mask[0];
-            double th0 = thr0[0];
+            unsigned mq = mask[0];
+            double ub = ub0[0];
 #pragma unroll
             for (int r = 1; r < WT; ++r)
-                if (q == r) { mq = mask[r]; th0 = thr0[r]; }
-            // blocks any lane wants (n0 <= 64 always fits; beyond that the bit is shared, still a superset)
-            unsigned mlo = __reduce_or_sync(FULL, (unsigned)mq), mhi = __reduce_or_sync(FULL, (unsigned)(mq >> 32));
-            const unsigned long long wm = ((unsigned long long)mhi << 32) | mlo;
+                if (q == r) { mq = mask[r]; ub = ub0[r]; }
+            unsigned wm = __reduce_or_sync(FULL, mq);       // blocks any lane of the warp wants
             if (STATS) st_cnt[ST_PAIRS] += 1;
             int bk = -1;
             if (wm) {
@@ -413,36 +384,38 @@ __global__ void __launch_bounds__(COMET_PR_WARPS * 32) k_coarse_pruned(const Pru
                 EvalC w;
                 load_evalc(w, a.wt, W, i);                           // warp-uniform, L1-resident
                 double best = INF;
-                double ub = lip_ok ? sqrt(th0) - half0 : INF;        // = min(sqrt(dmin), cap)
-                for (int t = 0; t < n0; ++t) {
-                    if (!((wm >> (t & 63)) & 1ull)) continue;
-                    const int j0 = t * NSUB;
-                    const int nj = min(NSUB, nS - j0);
-                    double d1[NSUB];
-                    double m1 = INF;
+                while (wm) {
+                    const int tb = __ffs(wm) - 1;
+                    wm &= wm - 1;
+                    for (int t = tb; t < n0; t += 32) {              // blocks that share the mask bit
+                        const double* ps = sbase + t * (NSUB * SST);
+                        int d1h[NSUB];
+                        int m1 = IMAX;
 #pragma unroll
-                    for (int j = 0; j < NSUB; ++j) {
-                        double x0, x1, x2;
-                        load_sample(min(j0 + j, nS - 1), x0, x1, x2);
-                        d1[j] = d2_fma(w, x0, x1, x2);
-                        m1 = fmin(m1, d1[j]);
-                    }
-                    if (STATS) st_cnt[ST_SAMPLES] += nj;
-                    ub = fmin(ub, sqrt(m1));
-                    const double t1 = ub + half1;
-                    const double thr1 = lip_ok ? t1 * t1 : INF;
+                        for (int j = 0; j < NSUB; ++j) {
+                            d1h[j] = __double2hiint(d2_fma(w, ps[j * SST], ps[j * SST + 32], ps[j * SST + 64]));
+                            m1 = min(m1, d1h[j]);
+                        }
+                        if (STATS) st_cnt[ST_SAMPLES] += NSUB;
+                        ub = fmin(ub, sqrt(__hiloint2double(m1 + 1, 0)));
+                        const double t1 = ub + half1;
+                        const int t1h = lip_ok ? __double2hiint(t1 * t1) : IMAX;
+                        unsigned sub = 0u;
 #pragma unroll
-                    for (int j = 0; j < NSUB; ++j) {
-                        const bool need = d1[j] <= thr1;
-                        if (j < nj && __any_sync(FULL, need)) {
-                            if (STATS) { st_cnt[ST_ROWS_EXEC] += COMET_M1; if (need) st_cnt[ST_ROWS_NEEDED] += COMET_M1; }
-                            const int rj = (j0 + j) * COMET_M1;
-                            const double* p = Xl + (size_t)rj * ROW;
+                        for (int j = 0; j < NSUB; ++j)
+                            if (d1h[j] <= t1h) sub |= 1u << j;
+                        unsigned wsub = __reduce_or_sync(FULL, sub);
+                        while (wsub) {
+                            const int j = __ffs(wsub) - 1;
+                            wsub &= wsub - 1;
+                            if (STATS) { st_cnt[ST_ROWS_EXEC] += COMET_M1; if ((sub >> j) & 1u) st_cnt[ST_ROWS_NEEDED] += COMET_M1; }
+                            const int rj = (t * NSUB + j) * COMET_M1;
+                            const double* pr = Xl + (size_t)(unsigned)(rj * ROW);
                             double xr[COMET_M1][3];
 #pragma unroll
                             for (int kk = 0; kk < COMET_M1; ++kk) {
-                                xr[kk][0] = __ldg(p + kk * ROW); xr[kk][1] = __ldg(p + kk * ROW + 32);
-                                xr[kk][2] = __ldg(p + kk * ROW + 64);
+                                xr[kk][0] = __ldg(pr + kk * ROW); xr[kk][1] = __ldg(pr + kk * ROW + 32);
+                                xr[kk][2] = __ldg(pr + kk * ROW + 64);
                             }
 #pragma unroll
                             for (int kk = 0; kk < COMET_M1; ++kk) {
@@ -460,6 +433,49 @@ __global__ void __launch_bounds__(COMET_PR_WARPS * 32) k_coarse_pruned(const Pru
             pa.kb[(size_t)i * pa.SP + s] = bk;
         }
     }
+}
+
+template <int WT, bool STATS>
+__global__ void __launch_bounds__(COMET_PR_WARPS * 32, 2) k_coarse_pruned(const PrunedArgs pa)
+{
+    constexpr int ROW = 3 * COMET_LANES;
+    constexpr unsigned FULL = 0xffffffffu;
+    extern __shared__ __align__(16) double ssm[];           // [cap_s][ROW]
+    __shared__ int s_next;
+    const DcaArgs& a = pa.d;
+    const int lane = threadIdx.x & 31;
+    const int64_t chunk = blockIdx.x;
+    const int64_t s = chunk * COMET_LANES + lane;
+    const bool valid = s < a.n_seeds;
+    const int32_t np = valid ? a.n_pts[s] : 0;
+    const int32_t kmax = __reduce_max_sync(FULL, np);
+    const int n0 = (kmax + COMET_M0 - 1) / COMET_M0;        // blocks (all complete: kernel A pads)
+    const int nS = n0 * (COMET_M0 / COMET_M1);
+    const double* __restrict__ Xc = a.X + track_row(chunk, track_rows(a.n_steps), 0);
+    const bool in_smem = nS <= pa.cap_s;                    // CTA-uniform
+    if (in_smem) {
+        for (int v = threadIdx.x; v < nS * (ROW / 2); v += COMET_PR_WARPS * 32) {
+            const int j = v / (ROW / 2), o = (v - j * (ROW / 2)) * 2;
+            cp_async16(ssm + j * ROW + o, Xc + (size_t)(j * COMET_M1 + COMET_M1 / 2) * ROW + o);
+        }
+        cp_async_commit();
+    }
+    if (threadIdx.x == 0) s_next = 0;
+    double ch = 0.0;                                        // |c| h of this lane
+    if (valid) {
+        const double px = a.seeds[3 * a.stride + s], py = a.seeds[4 * a.stride + s], pz = a.seeds[5 * a.stride + s];
+        ch = fabs(a.qkb) * a.h / sqrt(px * px + py * py + pz * pz);
+    }
+    const bool lip_ok = ch <= COMET_CH_MAX;                 // Lipschitz bound valid for this lane
+    unsigned long long st_cnt[ST_N];
+    if (STATS) {
+#pragma unroll
+        for (int j = 0; j < ST_N; ++j) st_cnt[j] = 0;
+    }
+    cp_async_wait<0>();
+    __syncthreads();
+    if (in_smem) coarse_groups<WT, STATS, true>(pa, Xc + lane, ssm + lane, n0, lane, s, lip_ok, &s_next, st_cnt);
+    else coarse_groups<WT, STATS, false>(pa, Xc + lane, Xc + lane + (COMET_M1 / 2) * ROW, n0, lane, s, lip_ok, &s_next, st_cnt);
     if (STATS) {
 #pragma unroll
         for (int j = 0; j < ST_N; ++j) {

@@ -51,8 +51,8 @@ k_extrapolate(const double* __restrict__ seeds, int64_t stride, int64_t n_seeds,
             X[row] = st.x0; X[row + 32] = st.x1; X[row + 64] = st.x2;      // hold-last padding
         }
     }
-    // pad the chunk to whole 8-row sub-blocks (rows k .. next multiple of 8; they exist: n_rows % 8 == 0)
-    for (; k & 7; ++k) {
+    // pad the chunk to whole 64-row blocks (rows k .. next multiple of 64; they exist: n_rows % 64 == 0)
+    for (; k & (COMET_ROW_PAD - 1); ++k) {
         row += 3 * COMET_LANES;
         X[row] = st.x0; X[row + 32] = st.x1; X[row + 64] = st.x2;
     }

@@ -41,10 +41,11 @@ def test_host_only_entry_points(libpath):
     assert L.comet_status_string(-1) == b"invalid argument"
     L.comet_track_bytes.restype = ctypes.c_size_t
     L.comet_track_bytes.argtypes = [ctypes.c_int64, ctypes.c_int32]
-    # two planes x ceil(S/32) chunks x (n_steps+1 rounded up to 8) rows x 3 components x 32 lanes x 8 bytes
-    assert L.comet_track_bytes(8192, 400) == 2 * 256 * 408 * 3 * 32 * 8
-    assert L.comet_track_bytes(33, 10) == 2 * 2 * 16 * 3 * 32 * 8
-    assert L.comet_track_bytes(33, 7) == 2 * 2 * 8 * 3 * 32 * 8
+    # two planes x ceil(S/32) chunks x (n_steps+1 rounded up to 64) rows x 3 components x 32 lanes x 8 bytes
+    assert L.comet_track_bytes(8192, 400) == 2 * 256 * 448 * 3 * 32 * 8
+    assert L.comet_track_bytes(33, 10) == 2 * 2 * 64 * 3 * 32 * 8
+    assert L.comet_track_bytes(33, 63) == 2 * 2 * 64 * 3 * 32 * 8
+    assert L.comet_track_bytes(33, 64) == 2 * 2 * 128 * 3 * 32 * 8
     assert L.comet_track_bytes(0, 10) == 0
     assert L.comet_track_bytes(10, 0) == 0 and L.comet_track_bytes(-1, 10) == 0
     # argument errors are reported before any CUDA call
