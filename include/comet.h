@@ -72,10 +72,11 @@ int comet_get_option(const comet_ctx* ctx, int option, int* value);
 int comet_reserve(comet_ctx* ctx, int64_t max_pairs_per_launch);
 
 /* With COMET_OPT_TIMING = 1 the pruned comet_dca_rss records CUDA events on its stream around its
- * three kernels.  Waits for the last such call and writes the device times in milliseconds of
- * k_coarse_pruned, k_fine and k_rss_sum (of the call's last seed slab) to ms_host[0..n), n <= 3.
- * COMET_EINVAL if no timed call was made. */
-int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n);
+ * three kernels (once per seed slab).  Waits for the timed slabs and writes the mean device time in
+ * milliseconds of k_coarse_pruned, k_fine and k_rss_sum over the most recent ones (at most 64 since
+ * the option was set or the last read) to ms_host[0..n), n <= 3, their number to *n_calls (may be
+ * NULL), and restarts the count.  COMET_EINVAL if no timed call was made. */
+int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n, int32_t* n_calls);
 
 /* Copies the work counters accumulated by comet_dca_rss calls made with COMET_OPT_STATS = 1 to
  * out_host[0..n) (HOST, n <= 6) and synchronises the stream; reset != 0 zeroes them afterwards.

@@ -72,7 +72,7 @@ def load_library():
                                         vp, i32, sz, vp, vp, vp, vp, vp, vp]
     L.comet_fp64_peak_probe.argtypes = [vp, i32, vp, ctypes.POINTER(dbl), vp]
     L.comet_reserve.argtypes = [vp, i64]
-    L.comet_read_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32]
+    L.comet_read_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32, ctypes.POINTER(i32)]
     L.comet_read_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), i32, i32, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("comet_status_string", "comet_track_bytes"):
@@ -142,10 +142,13 @@ class Comet:
         self._check(self._L.comet_reserve(self._h, int(max_pairs_per_launch)))
 
     def read_timing(self) -> dict:
-        """Device milliseconds of the last pruned comet_dca_rss made with OPT_TIMING = 1 (waits for it)."""
+        """Mean device milliseconds per kernel of the latest (<= 64) pruned comet_dca_rss slabs made with
+        OPT_TIMING = 1 (waits for them)."""
         buf = (ctypes.c_float * 3)()
-        self._check(self._L.comet_read_timing(self._h, buf, 3))
-        return {"k_coarse_pruned": float(buf[0]), "k_fine": float(buf[1]), "k_rss_sum": float(buf[2])}
+        n = ctypes.c_int32()
+        self._check(self._L.comet_read_timing(self._h, buf, 3, ctypes.byref(n)))
+        return {"k_coarse_pruned": float(buf[0]), "k_fine": float(buf[1]), "k_rss_sum": float(buf[2]),
+                "n_calls": int(n.value)}
 
     def read_stats(self, reset: bool = True, stream=None) -> dict:
         """Work counters of the pruned comet_dca_rss calls made with OPT_STATS = 1 (synchronises)."""

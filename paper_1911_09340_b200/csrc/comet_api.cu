@@ -15,6 +15,7 @@
 #include "select.cuh"
 
 #define COMET_PRUNED_WT 4
+#define COMET_TEV_RING 64
 #define COMET_PR_CAP_S 96      // sub-block samples staged in shared memory per chunk (72 KB)
 
 using namespace comet;
@@ -26,8 +27,8 @@ struct comet_ctx {
     int opt_stats;
     int opt_timing;
     int n_sm;
-    cudaEvent_t tev[4];          // COMET_OPT_TIMING: around k_coarse_pruned, k_fine, k_rss_sum
-    int tev_valid;
+    cudaEvent_t tev[COMET_TEV_RING][4];   // COMET_OPT_TIMING: around k_coarse_pruned, k_fine, k_rss_sum
+    long long tev_count;         // timed comet_dca_rss slabs since the option was set / last read
     unsigned long long* stats;   // device [ST_N] work counters of the pruned kernels
     // pair workspace of the pruned path: shortlisted state and e^2 per (wire, seed)
     int32_t* kb;
@@ -97,7 +98,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     const int pr_smem = COMET_PR_CAP_S * 3 * COMET_LANES * (int)sizeof(double);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coarse_pruned<COMET_PRUNED_WT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coarse_pruned<COMET_PRUNED_WT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
-    for (int j = 0; j < 4 && e == cudaSuccess; ++j) e = cudaEventCreate(&ctx->tev[j]);
+    for (int j = 0; j < COMET_TEV_RING * 4 && e == cudaSuccess; ++j) e = cudaEventCreate(&ctx->tev[j / 4][j % 4]);
     // shared-memory opt-ins (done once here, never on the hot path)
     const int dca_smem = (2 * COMET_KT * 3 * COMET_LANES + COMET_DCA_WARPS * 4 * 32) * (int)sizeof(double);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
@@ -122,7 +123,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaSetDevice(ctx->device);
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
     cudaFree(ctx->kb); cudaFree(ctx->e2);
-    for (int j = 0; j < 4; ++j) if (ctx->tev[j]) cudaEventDestroy(ctx->tev[j]);
+    for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf);
     delete ctx;
     return COMET_OK;
@@ -141,7 +142,7 @@ extern "C" int comet_set_option(comet_ctx* ctx, int option, int value)
     }
     if (option == COMET_OPT_TIMING && (value == 0 || value == 1)) {
         ctx->opt_timing = value;
-        ctx->tev_valid = 0;
+        ctx->tev_count = 0;
         return COMET_OK;
     }
     return COMET_EINVAL;
@@ -156,14 +157,26 @@ extern "C" int comet_get_option(const comet_ctx* ctx, int option, int* value)
     return COMET_EINVAL;
 }
 
-extern "C" int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n)
+extern "C" int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n, int32_t* n_calls)
 {
     if (!ctx || !ms_host || n < 0 || n > 3) return COMET_EINVAL;
-    if (!ctx->tev_valid) return COMET_EINVAL;
+    if (ctx->tev_count <= 0) return COMET_EINVAL;
     int rc = set_device(ctx);
     if (rc) return rc;
-    CU(ctx, cudaEventSynchronize(ctx->tev[3]));
-    for (int j = 0; j < n; ++j) CU(ctx, cudaEventElapsedTime(ms_host + j, ctx->tev[j], ctx->tev[j + 1]));
+    const long long have = ctx->tev_count < COMET_TEV_RING ? ctx->tev_count : COMET_TEV_RING;
+    double acc[3] = {0.0, 0.0, 0.0};
+    for (long long r = ctx->tev_count - have; r < ctx->tev_count; ++r) {
+        cudaEvent_t* ev = ctx->tev[r % COMET_TEV_RING];
+        CU(ctx, cudaEventSynchronize(ev[3]));
+        for (int j = 0; j < n; ++j) {
+            float ms = 0.f;
+            CU(ctx, cudaEventElapsedTime(&ms, ev[j], ev[j + 1]));
+            acc[j] += ms;
+        }
+    }
+    for (int j = 0; j < n; ++j) ms_host[j] = (float)(acc[j] / (double)have);
+    if (n_calls) *n_calls = (int32_t)have;
+    ctx->tev_count = 0;
     return COMET_OK;
 }
 
@@ -370,15 +383,16 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
             const unsigned b1 = (unsigned)nc;
             const unsigned b2 = (unsigned)((w2 + COMET_PR_WARPS - 1) / COMET_PR_WARPS);
             const bool tm = ctx->opt_timing != 0;
-            if (tm) CU(ctx, cudaEventRecord(ctx->tev[0], st));
+            cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
+            if (tm) CU(ctx, cudaEventRecord(tev[0], st));
             if (ctx->opt_stats) k_coarse_pruned<COMET_PRUNED_WT, true><<<b1, COMET_PR_WARPS * 32, sm1, st>>>(pa);
             else k_coarse_pruned<COMET_PRUNED_WT, false><<<b1, COMET_PR_WARPS * 32, sm1, st>>>(pa);
-            if (tm) CU(ctx, cudaEventRecord(ctx->tev[1], st));
+            if (tm) CU(ctx, cudaEventRecord(tev[1], st));
             if (ctx->opt_stats) k_fine<true><<<b2, COMET_PR_WARPS * 32, 0, st>>>(pa);
             else k_fine<false><<<b2, COMET_PR_WARPS * 32, 0, st>>>(pa);
-            if (tm) CU(ctx, cudaEventRecord(ctx->tev[2], st));
+            if (tm) CU(ctx, cudaEventRecord(tev[2], st));
             k_rss_sum<<<(unsigned)((pa.d.n_seeds + 255) / 256), 256, 0, st>>>(pa.e2, pa.SP, n_fired, pa.d.n_seeds, pa.d.rss);
-            if (tm) { CU(ctx, cudaEventRecord(ctx->tev[3], st)); ctx->tev_valid = 1; }
+            if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }
             CU(ctx, cudaGetLastError());
         }
         return COMET_OK;

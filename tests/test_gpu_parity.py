@@ -315,3 +315,144 @@ def test_argument_errors(comet, cfg0_event):
         comet.seed_extrapolate(d.seeds, ev.charge, ev.bz, ev.step, 5000, ev.r_stop)         # > COMET_MAX_STEPS
     with pytest.raises(CometError):
         comet.seed_extrapolate(d.seeds.cpu(), ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop)
+
+
+# ------------------------------------------------------------------------------------------------
+# full-size configurations (the launch configuration bench.py times) and the remaining configs
+# ------------------------------------------------------------------------------------------------
+def _oracle_select(ev, seeds, rss, part_off, cutoff=None):
+    return O.select_classify(seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a,
+                             ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho,
+                             ev.cutoff if cutoff is None else cutoff, rss, part_off)
+
+
+def test_full_cfg1_as_benchmarked(comet, cfg1_event):
+    """configs[1] at full size (3 x 131072 seeds x 71 wires), default (pruned) mode, device-resident
+    inputs exactly as bench.py runs it: every RSS, the best seeds and the classified set."""
+    ev = cfg1_event
+    seeds, part_off = event_seeds(ev)
+    assert seeds.shape[1] == 3 * 131072
+    d = DevEvent(ev, seeds)
+    out = comet.scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    torch.cuda.synchronize()
+    ref = _oracle_scan(ev, seeds, want_npts=True)
+    np.testing.assert_array_equal(out["n_pts"].cpu().numpy(), ref["n_pts"])
+    got = out["rss"].cpu().numpy()
+    _check_rss(got, ref["rss"])
+    assert np.array_equal(got, ref["rss"])
+    _check_select(out, _oracle_select(ev, seeds, ref["rss"], part_off), ev, ev.cutoff)
+
+
+def test_pair_workspace_slabs(comet, cfg0_event):
+    """A pair workspace smaller than the problem: comet_dca_rss walks seed slabs, same numbers."""
+    from paper_1911_09340_b200 import Comet
+    ev = cfg0_event
+    seeds, part_off = event_seeds(ev)
+    d = DevEvent(ev, seeds)
+    c2 = Comet(0)
+    try:
+        c2.reserve(5 * 32 * ev.n_fired)                    # 5 chunks per slab -> 52 slabs, ragged last one
+        out = c2.scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+        ref = comet.scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+        assert torch.equal(out["rss"], ref["rss"]) and torch.equal(out["cls"], ref["cls"])
+        assert torch.equal(out["best_seed"], ref["best_seed"])
+        track, n_pts = c2.seed_extrapolate(d.seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop)
+        full = c2.dca_rss(track, n_pts, d.seeds, *d.phys(), *d.hits(), ev.cutoff, want_dca=True, want_kstar=True)
+        oref = _oracle_scan(ev, seeds, want_dca=True, want_kstar=True)
+        np.testing.assert_array_equal(full["kstar"].cpu().numpy(), oref["kstar"])
+        assert np.array_equal(full["dca"].cpu().numpy(), oref["dca"])
+    finally:
+        c2.close()
+
+
+def test_cfg2_batch_of_events_on_streams():
+    """configs[2]: independent events (1-4 turns, |p| in [60,105]) in flight on several streams, one
+    context per stream; reduced seed grid so that the oracle finishes in seconds."""
+    from paper_1911_09340_b200 import Comet
+    events = make_config(2, n_events=6)
+    n_str = 3
+    ctxs = [Comet(0) for _ in range(n_str)]
+    streams = [torch.cuda.Stream() for _ in range(n_str)]
+    try:
+        outs, inputs = [], []
+        for k, ev in enumerate(events):
+            seeds, part_off = event_seeds(ev, shape=(6, 4, 4, 6))
+            d = DevEvent(ev, seeds)
+            st = streams[k % n_str]
+            st.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(st):
+                outs.append(ctxs[k % n_str].scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(),
+                                                       ev.cutoff, stream=st))
+            inputs.append((ev, seeds, part_off, d))
+        torch.cuda.synchronize()
+        assert len({len(ev.partitions) for ev in events}) > 1          # a mix of turn counts
+        for (ev, seeds, part_off, _), out in zip(inputs, outs):
+            ref = _oracle_scan(ev, seeds)
+            assert np.array_equal(out["rss"].cpu().numpy(), ref["rss"])
+            _check_select(out, _oracle_select(ev, seeds, ref["rss"], part_off), ev, ev.cutoff)
+    finally:
+        for c in ctxs:
+            c.close()
+
+
+def test_cfg3_large_scan_in_slabs(comet):
+    """configs[3] (4 turns, 1600 steps of 0.2 cm): the track buffer of the full grid does not fit in
+    HBM, so seeds go through a bounded track workspace.  Reduced grid, element by element."""
+    ev = make_config(3)[0]
+    assert len(ev.partitions) == 4 and ev.n_steps == 1600
+    seeds, part_off = event_seeds(ev, shape=(8, 4, 8, 16))             # 4 x 4096 seeds
+    out = comet.scan_event_host(torch.from_numpy(seeds).pin_memory(), part_off, ev.charge, ev.bz, ev.step,
+                                ev.n_steps, ev.r_stop, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire,
+                                ev.hit_off, ev.rho, ev.cutoff, want_rss=True,
+                                track_budget_bytes=300 << 20)          # ~3800 seeds per slab
+    ref = _oracle_scan(ev, seeds)
+    assert np.array_equal(out["rss"].numpy(), ref["rss"])
+    rs = _oracle_select(ev, seeds, ref["rss"], part_off)
+    np.testing.assert_array_equal(out["best_seed"].numpy(), rs["best_seed"])
+    np.testing.assert_array_equal(out["cls"].numpy(), rs["cls"])
+
+
+def _sampled_full_size_check(comet, ev, seeds, part_off, n_sample, cutoff=None, budget=8 << 30):
+    """Whole path at full size through the host-buffer entry point; RSS of a strided sample of seeds
+    against the oracle, the argmin recomputed from the device RSS, and the winners' D / classified
+    sets against the oracle (which needs only the winning seeds)."""
+    cutoff = ev.cutoff if cutoff is None else cutoff
+    S = seeds.shape[1]
+    out = comet.scan_event_host(torch.from_numpy(seeds).pin_memory(), part_off, ev.charge, ev.bz, ev.step,
+                                ev.n_steps, ev.r_stop, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire,
+                                ev.hit_off, ev.rho, cutoff, want_rss=True, track_budget_bytes=budget)
+    rss = out["rss"].numpy()
+    idx = np.unique(np.concatenate([np.arange(0, S, max(1, S // n_sample)), out["best_seed"].numpy()]))
+    sub = np.ascontiguousarray(seeds[:, idx])
+    ref = _oracle_scan(ev, sub, cutoff=cutoff)
+    assert np.array_equal(rss[idx], ref["rss"])
+    W = ev.n_fired
+    assert rss.min() >= 0.0 and rss.max() <= W * cutoff * cutoff * (1 + 1e-12)
+    for p in range(len(part_off) - 1):
+        lo, hi = int(part_off[p]), int(part_off[p + 1])
+        b = lo + int(np.argmin(rss[lo:hi]))                               # first minimum = lowest index
+        assert int(out["best_seed"][p]) == b
+        one = np.ascontiguousarray(seeds[:, b:b + 1])
+        r1 = _oracle_scan(ev, one, cutoff=cutoff)
+        rs = _oracle_select(ev, one, r1["rss"], np.array([0, 1], dtype=np.int64), cutoff=cutoff)
+        assert float(out["best_rss"][p]) == float(r1["rss"][0])
+        _check_dca(out["best_dca"][p].numpy(), rs["best_dca"][0])
+        np.testing.assert_array_equal(out["cls"][p].numpy(), rs["cls"][0])
+    return out
+
+
+def test_full_cfg3_sampled(comet):
+    """configs[3] at full size: 4 x 1048576 seeds, 1600 steps; 8 GiB track slabs."""
+    ev = make_config(3)[0]
+    seeds, part_off = event_seeds(ev)
+    assert seeds.shape[1] == 4 * 1048576
+    _sampled_full_size_check(comet, ev, seeds, part_off, n_sample=4096)
+
+
+def test_full_cfg4_sampled(comet):
+    """configs[4] at full size: 3 x 131072 seeds against ~970 fired wires, three cutoffs."""
+    ev = make_config(4)[0]
+    seeds, part_off = event_seeds(ev)
+    assert seeds.shape[1] == 3 * 131072 and ev.n_fired > 900
+    for lam in ev.spec["cutoffs"]:
+        _sampled_full_size_check(comet, ev, seeds, part_off, n_sample=1024, cutoff=lam)
