@@ -456,3 +456,34 @@ def test_full_cfg4_sampled(comet):
     assert seeds.shape[1] == 3 * 131072 and ev.n_fired > 900
     for lam in ev.spec["cutoffs"]:
         _sampled_full_size_check(comet, ev, seeds, part_off, n_sample=1024, cutoff=lam)
+
+
+def test_seed_sharded_scan_two_ranks_emulated(comet, cfg1_event):
+    """The seed-sharded N > 1 flow on one GPU: each 'rank' scans only its chunk-aligned seed ranges
+    (one after the other here, no kernel waits on another), the local winners are merged with the
+    rule of sharding.merge_best, every rank classifies the winners itself.  Same result as one rank."""
+    from paper_1911_09340_b200.sharding import local_best, shard_partitions
+    ev = cfg1_event
+    seeds, part_off = event_seeds(ev, shape=(5, 4, 4, 7))             # 560 seeds per partition: ragged chunks
+    d = DevEvent(ev, seeds)
+    one = comet.scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    world, P = 2, len(part_off) - 1
+    loc = []
+    for rank in range(world):
+        ranges = shard_partitions(part_off, rank, world)
+        rss = torch.full((seeds.shape[1],), float("nan"), dtype=torch.float64, device="cuda")
+        for b, e in ranges:
+            if e > b:
+                track, n_pts = comet.seed_extrapolate(d.seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop,
+                                                      seed_range=(b, e))
+                comet.dca_rss(track, n_pts, d.seeds, *d.phys(), *d.hits(), ev.cutoff, rss=rss[b:e],
+                              seed_range=(b, e))
+        loc.append(local_best(rss, ranges))
+    gv = torch.minimum(loc[0][0], loc[1][0])
+    big = torch.iinfo(torch.int64).max
+    gi = torch.minimum(torch.where(loc[0][0] == gv, loc[0][1], big), torch.where(loc[1][0] == gv, loc[1][1], big))
+    assert torch.equal(gi, one["best_seed"]) and torch.equal(gv, one["best_rss"])
+    winners = d.seeds[:, gi].contiguous()                              # [6][P]
+    sel = comet.select_and_classify(winners, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, gv.contiguous(),
+                                    np.arange(P + 1, dtype=np.int64))
+    assert torch.equal(sel["cls"], one["cls"]) and torch.equal(sel["best_dca"], one["best_dca"])
