@@ -14,7 +14,9 @@
 #include "extrapolate.cuh"
 #include "select.cuh"
 
-#define COMET_PRUNED_WT 4
+#ifndef COMET_PRUNED_WT
+#define COMET_PRUNED_WT 3
+#endif
 #define COMET_TEV_RING 64
 #define COMET_PR_CAP_S 96      // sub-block samples staged in shared memory per chunk (72 KB)
 
@@ -33,6 +35,9 @@ struct comet_ctx {
     // pair workspace of the pruned path: shortlisted state and e^2 per (wire, seed)
     int32_t* kb;
     double* e2;
+    unsigned long long* items;   // [pair_cap / 32] work list of k_fine
+    unsigned int* n_items;
+    int fine_blocks;             // persistent grid of k_fine
     size_t pair_cap;             // pairs the two buffers hold
     size_t pair_max;             // growth limit (larger problems are processed in seed slabs)
     // device workspace
@@ -95,6 +100,12 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaMalloc(&ctx->stats, sizeof(unsigned long long) * ST_N);
     if (e == cudaSuccess) e = cudaMemset(ctx->stats, 0, sizeof(unsigned long long) * ST_N);
     ctx->pair_max = (size_t)1 << 26;
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int));
+    if (e == cudaSuccess) {
+        int per_sm = 0;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fine<false>, COMET_FINE_THREADS, 0);
+        ctx->fine_blocks = ctx->n_sm * (per_sm > 0 ? per_sm : 1);
+    }
     const int pr_smem = COMET_PR_CAP_S * 3 * COMET_LANES * (int)sizeof(double);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coarse_pruned<COMET_PRUNED_WT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coarse_pruned<COMET_PRUNED_WT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
@@ -109,7 +120,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
         e = cudaFuncSetAttribute(k_select_classify, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
     if (e != cudaSuccess) {
-        cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
+        cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats); cudaFree(ctx->n_items);
         delete ctx;
         return e == cudaErrorMemoryAllocation ? COMET_ENOMEM : COMET_ECUDA;
     }
@@ -122,7 +133,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     if (!ctx) return COMET_EINVAL;
     cudaSetDevice(ctx->device);
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
-    cudaFree(ctx->kb); cudaFree(ctx->e2);
+    cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items);
     for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf);
     delete ctx;
@@ -199,13 +210,15 @@ static int ensure_pairs(comet_ctx* ctx, size_t pairs)
 {
     if (pairs <= ctx->pair_cap) return COMET_OK;
     CU(ctx, cudaDeviceSynchronize());
-    cudaFree(ctx->kb); cudaFree(ctx->e2);
-    ctx->kb = nullptr; ctx->e2 = nullptr; ctx->pair_cap = 0;
+    cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items);
+    ctx->kb = nullptr; ctx->e2 = nullptr; ctx->items = nullptr; ctx->pair_cap = 0;
     cudaError_t e = cudaMalloc(&ctx->kb, sizeof(int32_t) * pairs);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->e2, sizeof(double) * pairs);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->items, sizeof(unsigned long long) * (pairs / COMET_LANES + 1));
     if (e != cudaSuccess) {
         ctx->last_cuda = (int)e;
         cudaFree(ctx->kb); ctx->kb = nullptr;
+        cudaFree(ctx->e2); ctx->e2 = nullptr;
         cudaGetLastError();
         return COMET_ENOMEM;
     }
@@ -376,20 +389,24 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
             pa.full = (dca || kstar) ? 1 : 0;
             pa.kb = ctx->kb;
             pa.e2 = ctx->e2;
+            pa.items = ctx->items;
+            pa.n_items = ctx->n_items;
+            CU(ctx, cudaMemsetAsync(ctx->n_items, 0, sizeof(unsigned int), st));
             pa.cap_s = track_rows(n_steps) / COMET_M1;
             if (pa.cap_s > COMET_PR_CAP_S) pa.cap_s = COMET_PR_CAP_S;
             const size_t sm1 = (size_t)pa.cap_s * 3 * COMET_LANES * sizeof(double);
-            const int64_t w2 = nc * (int64_t)n_fired;
+            const int64_t w2 = nc * (int64_t)n_fired;          // upper bound on the work list
             const unsigned b1 = (unsigned)nc;
-            const unsigned b2 = (unsigned)((w2 + COMET_PR_WARPS - 1) / COMET_PR_WARPS);
+            const int64_t b2_all = (w2 + COMET_FINE_THREADS / 32 - 1) / (COMET_FINE_THREADS / 32);
+            const unsigned b2 = (unsigned)(b2_all < ctx->fine_blocks ? b2_all : ctx->fine_blocks);
             const bool tm = ctx->opt_timing != 0;
             cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
             if (tm) CU(ctx, cudaEventRecord(tev[0], st));
             if (ctx->opt_stats) k_coarse_pruned<COMET_PRUNED_WT, true><<<b1, COMET_PR_WARPS * 32, sm1, st>>>(pa);
             else k_coarse_pruned<COMET_PRUNED_WT, false><<<b1, COMET_PR_WARPS * 32, sm1, st>>>(pa);
             if (tm) CU(ctx, cudaEventRecord(tev[1], st));
-            if (ctx->opt_stats) k_fine<true><<<b2, COMET_PR_WARPS * 32, 0, st>>>(pa);
-            else k_fine<false><<<b2, COMET_PR_WARPS * 32, 0, st>>>(pa);
+            if (ctx->opt_stats) k_fine<true><<<b2, COMET_FINE_THREADS, 0, st>>>(pa);
+            else k_fine<false><<<b2, COMET_FINE_THREADS, 0, st>>>(pa);
             if (tm) CU(ctx, cudaEventRecord(tev[2], st));
             k_rss_sum<<<(unsigned)((pa.d.n_seeds + 255) / 256), 256, 0, st>>>(pa.e2, pa.SP, n_fired, pa.d.n_seeds, pa.d.rss);
             if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }

@@ -253,12 +253,28 @@ __global__ void __launch_bounds__(COMET_DCA_WARPS * 32, 2) k_dca_rss(const DcaAr
 //   k_rss_sum        thread = seed: RSS = sum of e^2 in wire order (Eq. (1))
 // bk [W][SP] int32 and e^2 [W][SP] double (SP = 32 * number of chunks) live in the ctx workspace.
 // ---------------------------------------------------------------------------------------------
+#ifndef COMET_M0
 #define COMET_M0 64
+#endif
+#ifndef COMET_M1
 #define COMET_M1 8
+#endif
 #define COMET_CH_MAX 0.05
 #define COMET_LIP 1.001
 #define COMET_SLACK 1e-9
 #define COMET_PR_WARPS 8
+#ifndef COMET_COARSE_MINB
+#define COMET_COARSE_MINB 3
+#endif
+#ifndef COMET_SWEEP_B
+#define COMET_SWEEP_B 8           // rows loaded per batch in a sub-block sweep
+#endif
+#ifndef COMET_FINE_MINB
+#define COMET_FINE_MINB 4
+#endif
+#ifndef COMET_FINE_THREADS
+#define COMET_FINE_THREADS 256
+#endif
 
 struct EvalC {
     double e1x, e1y, e1z, c1, e2x, e2y, e2z, c2;
@@ -289,6 +305,8 @@ struct PrunedArgs {
     int32_t full;            // dca or kstar requested: no far-pair shortcut
     int32_t* kb;             // [W][SP]
     double* e2;              // [W][SP]
+    unsigned long long* items;   // work list of k_fine: (chunk << 16 | wire) of every warp-item with a near lane
+    unsigned int* n_items;       // its length (zeroed before k_coarse_pruned)
 };
 
 // CTA = one track chunk.  The sub-block samples (row 8 j + 4 of every 8-row sub-block j, fp64) are
@@ -316,6 +334,7 @@ __device__ __forceinline__ void coarse_groups(const PrunedArgs& pa, const double
     const double L = COMET_LIP * a.h;
     const double INF = 1.7976931348623157e308;
     const double half0 = (COMET_M0 / 2 + COMET_M1 / 2) * L + COMET_SLACK, half1 = (COMET_M1 / 2) * L + COMET_SLACK;
+    const double lam2 = xmul(a.lambda, a.lambda);
 
     while (true) {
         int g = 0;
@@ -326,7 +345,6 @@ __device__ __forceinline__ void coarse_groups(const PrunedArgs& pa, const double
         // ---- level 0: minimum over the block samples, then the blocks within reach of it ------------
         double ub0[WT];                                     // min(sqrt(min sample), far radius)
         unsigned mask[WT];                                  // bit t % 32: block t may hold the closest state
-        bool any_cand = false;
         {
             EvalC ec[WT];
             int dh[WT], thi[WT];
@@ -336,35 +354,37 @@ __device__ __forceinline__ void coarse_groups(const PrunedArgs& pa, const double
                 dh[q] = IMAX;
                 mask[q] = 0u;
             }
+            // RSS-only calls know an upper bound before looking at anything: the far radius.  One pass.
+            // Calls that want D / k* of every pair first take the minimum over the block samples.
             const double* p = sbase + (NSUB / 2) * SST;
+            if (pa.full) {
 #pragma unroll 2
-            for (int t = 0; t < n0; ++t, p += NSUB * SST) {
-                const double x0 = p[0], x1 = p[32], x2 = p[64];
+                for (int t = 0; t < n0; ++t, p += NSUB * SST) {
+                    const double x0 = p[0], x1 = p[32], x2 = p[64];
 #pragma unroll
-                for (int q = 0; q < WT; ++q) dh[q] = min(dh[q], __double2hiint(d2_fma(ec[q], x0, x1, x2)));
+                    for (int q = 0; q < WT; ++q) dh[q] = min(dh[q], __double2hiint(d2_fma(ec[q], x0, x1, x2)));
+                }
+                if (STATS) st_cnt[ST_SAMPLES] += (unsigned long long)n0 * min(WT, W - i0);
             }
 #pragma unroll
             for (int q = 0; q < WT; ++q) {
                 const double cap = pa.full ? INF : __ldg(a.wt + 14 * W + min(i0 + q, W - 1));   // far radius R_i
-                const double dm = __hiloint2double(dh[q] + 1, 0);    // >= the smallest sample
+                const double dm = pa.full ? __hiloint2double(dh[q] + 1, 0) : INF;   // >= the smallest sample
                 ub0[q] = lip_ok ? fmin(sqrt(dm), cap) : INF;
                 const double t0 = ub0[q] + half0;
                 thi[q] = lip_ok ? __double2hiint(t0 * t0) : IMAX;
                 if (cap < 0.0 || i0 + q >= W) thi[q] = -1;           // wire without entries / past the end
-                any_cand |= dh[q] <= thi[q];
+            }
+            p = sbase + (NSUB / 2) * SST;
+#pragma unroll 2
+            for (int t = 0; t < n0; ++t, p += NSUB * SST) {
+                const double x0 = p[0], x1 = p[32], x2 = p[64];
+                const unsigned bit = 1u << (t & 31);
+#pragma unroll
+                for (int q = 0; q < WT; ++q)
+                    if (__double2hiint(d2_fma(ec[q], x0, x1, x2)) <= thi[q]) mask[q] |= bit;
             }
             if (STATS) st_cnt[ST_SAMPLES] += (unsigned long long)n0 * min(WT, W - i0);
-            if (__any_sync(FULL, any_cand)) {
-                p = sbase + (NSUB / 2) * SST;
-                for (int t = 0; t < n0; ++t, p += NSUB * SST) {
-                    const double x0 = p[0], x1 = p[32], x2 = p[64];
-                    const unsigned bit = 1u << (t & 31);
-#pragma unroll
-                    for (int q = 0; q < WT; ++q)
-                        if (__double2hiint(d2_fma(ec[q], x0, x1, x2)) <= thi[q]) mask[q] |= bit;
-                }
-                if (STATS) st_cnt[ST_SAMPLES] += (unsigned long long)n0 * min(WT, W - i0);
-            }
         }
         // ---- per wire: level 1 in the opened blocks, row sweeps of the opened sub-blocks ------------
 #pragma unroll 1
@@ -411,16 +431,19 @@ __device__ __forceinline__ void coarse_groups(const PrunedArgs& pa, const double
                             if (STATS) { st_cnt[ST_ROWS_EXEC] += COMET_M1; if ((sub >> j) & 1u) st_cnt[ST_ROWS_NEEDED] += COMET_M1; }
                             const int rj = (t * NSUB + j) * COMET_M1;
                             const double* pr = Xl + (size_t)(unsigned)(rj * ROW);
-                            double xr[COMET_M1][3];
 #pragma unroll
-                            for (int kk = 0; kk < COMET_M1; ++kk) {
-                                xr[kk][0] = __ldg(pr + kk * ROW); xr[kk][1] = __ldg(pr + kk * ROW + 32);
-                                xr[kk][2] = __ldg(pr + kk * ROW + 64);
-                            }
+                            for (int k0 = 0; k0 < COMET_M1; k0 += COMET_SWEEP_B) {
+                                double xr[COMET_SWEEP_B][3];
 #pragma unroll
-                            for (int kk = 0; kk < COMET_M1; ++kk) {
-                                const double d2 = d2_fma(w, xr[kk][0], xr[kk][1], xr[kk][2]);
-                                if (d2 < best) { best = d2; bk = rj + kk; }
+                                for (int kk = 0; kk < COMET_SWEEP_B; ++kk) {
+                                    xr[kk][0] = __ldg(pr + (k0 + kk) * ROW); xr[kk][1] = __ldg(pr + (k0 + kk) * ROW + 32);
+                                    xr[kk][2] = __ldg(pr + (k0 + kk) * ROW + 64);
+                                }
+#pragma unroll
+                                for (int kk = 0; kk < COMET_SWEEP_B; ++kk) {
+                                    const double d2 = d2_fma(w, xr[kk][0], xr[kk][1], xr[kk][2]);
+                                    if (d2 < best) { best = d2; bk = rj + k0 + kk; }
+                                }
                             }
                         }
                     }
@@ -430,13 +453,20 @@ __device__ __forceinline__ void coarse_groups(const PrunedArgs& pa, const double
                 if (!near) bk = -1;
             }
             if (STATS && bk >= 0) st_cnt[ST_FINE_NEEDED] += 1;
-            pa.kb[(size_t)i * pa.SP + s] = bk;
+            // a (chunk, wire) item with a near lane goes to k_fine's work list; the others are done here
+            if (__any_sync(FULL, bk >= 0)) {
+                pa.kb[(size_t)i * pa.SP + s] = bk;
+                if (lane == 0)
+                    pa.items[atomicAdd(pa.n_items, 1u)] = ((unsigned long long)(s >> 5) << 16) | (unsigned)i;
+            } else {
+                pa.e2[(size_t)i * pa.SP + s] = lam2;
+            }
         }
     }
 }
 
 template <int WT, bool STATS>
-__global__ void __launch_bounds__(COMET_PR_WARPS * 32, 2) k_coarse_pruned(const PrunedArgs pa)
+__global__ void __launch_bounds__(COMET_PR_WARPS * 32, COMET_COARSE_MINB) k_coarse_pruned(const PrunedArgs pa)
 {
     constexpr int ROW = 3 * COMET_LANES;
     constexpr unsigned FULL = 0xffffffffu;
@@ -486,27 +516,28 @@ __global__ void __launch_bounds__(COMET_PR_WARPS * 32, 2) k_coarse_pruned(const 
     }
 }
 
-// warp = (chunk, wire): B2 decision + B3 + B4 for the pairs the coarse search kept
+// Persistent warps walk the work list of (chunk, wire) items that have at least one near lane:
+// B2 decision + B3 + B4 for the near lanes, lambda^2 for the others.
 template <bool STATS>
-__global__ void __launch_bounds__(COMET_PR_WARPS * 32) k_fine(const PrunedArgs pa)
+__global__ void __launch_bounds__(COMET_FINE_THREADS, COMET_FINE_MINB) k_fine(const PrunedArgs pa)
 {
-    constexpr unsigned FULL = 0xffffffffu;
     const DcaArgs& a = pa.d;
     const int lane = threadIdx.x & 31;
-    const int64_t wid = (int64_t)blockIdx.x * COMET_PR_WARPS + (threadIdx.x >> 5);
+    const unsigned n_items = *pa.n_items;
+    const unsigned n_warps = gridDim.x * (COMET_FINE_THREADS / 32);
     const int W = a.W;
-    if (wid >= pa.n_chunks * W) return;
-    const int64_t chunk = wid / W;
-    const int i = (int)(wid - chunk * W);
-    const int64_t s = chunk * COMET_LANES + lane;
-    const bool valid = s < a.n_seeds;
-    const int bk = pa.kb[(size_t)i * pa.SP + s];
-    const bool near = valid && bk >= 0;
-    double e2 = xmul(a.lambda, a.lambda);
-    if (__any_sync(FULL, near)) {
+    const int32_t n_rows = track_rows(a.n_steps);
+    const double lam2 = xmul(a.lambda, a.lambda);
+    for (unsigned it = blockIdx.x * (COMET_FINE_THREADS / 32) + (threadIdx.x >> 5); it < n_items; it += n_warps) {
+        const unsigned long long item = pa.items[it];
+        const int64_t chunk = (int64_t)(item >> 16);
+        const int i = (int)(item & 0xffffu);
+        const int64_t s = chunk * COMET_LANES + lane;
+        const bool valid = s < a.n_seeds;
+        const int bk = pa.kb[(size_t)i * pa.SP + s];
+        double e2 = lam2;
         if (STATS) { if (lane == 0 && a.stats) atomicAdd(a.stats + ST_FINE_EXEC, 32ull); }
-        if (near) {
-            const int32_t n_rows = track_rows(a.n_steps);
+        if (valid && bk >= 0) {
             const size_t base = track_row(chunk, n_rows, 0);
             const double px = a.seeds[3 * a.stride + s], py = a.seeds[4 * a.stride + s], pz = a.seeds[5 * a.stride + s];
             const double c = xdiv(a.qkb, xsqrt(xdot3(px, py, pz, px, py, pz)));
@@ -516,8 +547,8 @@ __global__ void __launch_bounds__(COMET_PR_WARPS * 32) k_fine(const PrunedArgs p
             if (a.dca) a.dca[(size_t)s * W + i] = D;
             if (a.kstar) a.kstar[(size_t)s * W + i] = ks;
         }
+        pa.e2[(size_t)i * pa.SP + s] = e2;
     }
-    pa.e2[(size_t)i * pa.SP + s] = e2;
 }
 
 // B5: RSS_s = sum_i e^2_i in increasing wire order (Eq. (1); no atomics, cf. :374)
