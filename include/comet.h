@@ -142,6 +142,26 @@ int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64
                   int32_t n_fired, int32_t n_hits, double cutoff_cm,
                   double* rss, double* dca, int32_t* kstar, void* cuda_stream);
 
+/* ---- kernels A + B fused, track kept on chip (Algorithms 1 + 2) ------------ */
+
+/* rss[s] (and n_pts[s]) exactly as comet_seed_extrapolate followed by comet_dca_rss(dca = kstar =
+ * NULL) would produce them -- same operations, bit-identical -- but the recorded track never goes
+ * to HBM: a warp extrapolates a chunk of 32 seeds tile by tile into shared memory, searches the
+ * tile for the states closest to every fired wire, and keeps only every 4th recorded state in a
+ * checkpoint workspace from which the virtual-plane iteration restarts.
+ * Arguments as in the two calls above;
+ *   n_pts   dev [n_seeds], written; NULL to skip.
+ * Workspace (pair buffers and checkpoints, 12 bytes per recorded state + 12 per (seed, wire) pair)
+ * lives in the ctx and grows on the first call that needs it (that call synchronises the device);
+ * larger problems are processed in seed slabs bounded by comet_reserve's pair limit and by 8 GiB of
+ * checkpoints.  COMET_OPT_TIMING applies (k_scan_fused, k_fine_ck, k_rss_sum). */
+int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                   int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                   const double* wire_a, const double* wire_b, int32_t n_wires,
+                   const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                   int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                   double* rss, int32_t* n_pts, void* cuda_stream);
+
 /* ---- step C: best seed per turn partition and hit classification -------- */
 
 /* For every partition p (seeds [part_off[p], part_off[p+1])): best_seed[p] = lowest-index argmin
@@ -165,8 +185,9 @@ int comet_select_and_classify(comet_ctx* ctx, const double* seeds, int64_t seed_
 /* ---- whole event from host buffers ------------------------------------------------------- */
 
 /* Runs A, B and C for one event whose inputs and outputs live in HOST memory (pinned memory makes
- * the copies asynchronous): copies the inputs to the device, processes the seeds in slabs that fit
- * `track_budget_bytes` of track workspace (grown inside the ctx when needed, 0 = 4 GiB), copies
+ * the copies asynchronous): copies the inputs to the device, runs comet_scan_rss (track on chip) when
+ * track_budget_bytes == 0, else comet_seed_extrapolate + comet_dca_rss over slabs of seeds that fit
+ * `track_budget_bytes` of track workspace (grown inside the ctx when needed), copies
  * best_seed/best_rss/best_dca/cls (and rss if rss_host != NULL) back and synchronises the stream.
  * All array arguments have the shapes of the device-buffer calls above. */
 int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, int64_t n_seeds,

@@ -5,7 +5,7 @@ into it.  Nothing here has a CPU implementation: without the built library, or w
 device, the calls raise.
 """
 from .binding import (Comet, CometError, lib_path, load_library, seed_extrapolate, track_export,
-                      dca_rss, select_and_classify, scan_event, scan_event_host, EXPORTED_SYMBOLS)
+                      dca_rss, scan_rss, select_and_classify, scan_event, scan_event_host, EXPORTED_SYMBOLS)
 
 __all__ = ["Comet", "CometError", "lib_path", "load_library", "seed_extrapolate", "track_export",
-           "dca_rss", "select_and_classify", "scan_event", "scan_event_host", "EXPORTED_SYMBOLS"]
+           "dca_rss", "scan_rss", "select_and_classify", "scan_event", "scan_event_host", "EXPORTED_SYMBOLS"]

