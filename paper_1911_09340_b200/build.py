@@ -10,7 +10,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libcomet.so")
 _SOURCES = ["comet_api.cu"]
-_DEPS = ["comet_api.cu", "common.cuh", "extrapolate.cuh", "dca.cuh", "select.cuh",
+_DEPS = ["comet_api.cu", "common.cuh", "extrapolate.cuh", "dca.cuh", "select.cuh", "scan_fused.cuh",
          os.path.join("..", "..", "include", "comet.h")]
 
 NVCC_FLAGS = [

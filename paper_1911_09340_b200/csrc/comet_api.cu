@@ -518,11 +518,10 @@ extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_
         a.n_ck = n_ck;
         a.ck = ctx->ck;
         a.bd = ctx->e2;
-        a.kb = ctx->kb;
         a.n_pts = n_pts ? n_pts + s0 : ctx->npw;
         a.items = ctx->items;
         a.n_items = ctx->n_items;
-        a.stats = nullptr;
+        a.stats = ctx->opt_stats ? ctx->stats : nullptr;
         CU(ctx, cudaMemsetAsync(ctx->n_items, 0, sizeof(unsigned int), st));
         const unsigned b1 = (unsigned)((nc + COMET_FUSED_WARPS - 1) / COMET_FUSED_WARPS);
         const int64_t w2 = nc * (int64_t)n_fired;

@@ -7,15 +7,19 @@
 //   generate   TR RKN4 steps per lane (the definition's operations, common.cuh), the positions of the
 //              TR rows go to a warp-private shared-memory tile [TR][3][32] fp64 (conflict-free, never
 //              to HBM); every CK-th recorded state (x, T) is written to a small checkpoint buffer;
-//   level 0    one sample per tile (row TR/2) against every fired wire.  This is the dense part, so
-//              it runs with lane = WIRE: the wire's shortlist constants stay in registers for the
-//              whole chunk, the 32 seeds' samples are broadcast from shared memory, and each lane
-//              builds a 32-bit mask of the seeds whose tile may hold that wire's closest state
-//              (Lipschitz bound of dca.cuh with the wire's far radius as the upper bound);
-//   level 1    per wire with a non-empty mask (lane = seed again): the 8-row sub-block samples of
-//              the tile, then row sweeps of the sub-blocks within reach, all from the tile; the best
-//              (squared distance, row) of the pair so far lives in the pair workspace (L2-resident,
-//              touched only by this warp);
+//   level 0    one evaluation per (8-row sub-block, wire) with lane = WIRE: the wire's shortlist
+//              constants stay in registers for the whole chunk; the sub-block sample of one
+//              representative seed and the largest offset of the other seeds' samples from it bound
+//              every seed's distance from below (Lipschitz bound of dca.cuh with the wire's far radius
+//              as the upper bound), so a sub-block is opened for a wire only if some seed may have its
+//              closest state there;
+//   sweeps     per wire with candidate sub-blocks (lane = seed again, the wire's constants arrive by
+//              warp shuffles): their rows are evaluated from the tile; the tile's
+//              best (squared distance, row) of the pair is merged into the pair workspace with one
+//              fire-and-forget 64-bit atomic min on a packed key (no read-modify-write round trip to
+//              L2): key = bits(d^2) with the low 13 bits replaced by the row, so keys order by d^2
+//              (to 2^-39 relative) and then by row -- enough for a shortlist whose choice is re-decided
+//              exactly between bk-1, bk, bk+1;
 //   finish     per wire: pairs whose closest state is farther than the far radius get e^2 = cutoff^2,
 //              (chunk, wire) items with a near lane go to the work list of k_fine_ck.
 //
@@ -32,7 +36,7 @@
 namespace comet {
 
 #ifndef COMET_FUSED_TR
-#define COMET_FUSED_TR 32          // rows per tile (level-0 block)
+#define COMET_FUSED_TR 16          // rows per tile
 #endif
 #ifndef COMET_FUSED_CK
 #define COMET_FUSED_CK 4           // rows between checkpoints
@@ -40,7 +44,24 @@ namespace comet {
 #ifndef COMET_FUSED_WARPS
 #define COMET_FUSED_WARPS 1        // warps (chunks) per CTA
 #endif
+#ifndef COMET_FUSED_MINB
+#define COMET_FUSED_MINB 12        // resident CTAs per SM the register allocation aims at (<= 168 registers)
+#endif
 #define COMET_FUSED_QMAX 3         // wires per lane and round in level 0
+
+// Packed shortlist key of a (seed, wire) pair: the bit pattern of the non-negative squared distance
+// (monotone as an unsigned integer) with its 13 low mantissa bits replaced by the row (<= 4096).
+#define COMET_KEY_NONE 0xffffffffffffffffull
+#define COMET_KEY_KBITS 13
+__device__ __forceinline__ unsigned long long pack_key(double d2, int k)
+{
+    return ((unsigned long long)__double_as_longlong(d2) & ~((1ull << COMET_KEY_KBITS) - 1ull)) | (unsigned long long)k;
+}
+__device__ __forceinline__ double key_d2(unsigned long long key)
+{
+    return __longlong_as_double((long long)(key & ~((1ull << COMET_KEY_KBITS) - 1ull)));
+}
+__device__ __forceinline__ int key_row(unsigned long long key) { return (int)(key & ((1ull << COMET_KEY_KBITS) - 1ull)); }
 
 struct FusedArgs {
     const double* seeds;
@@ -58,8 +79,7 @@ struct FusedArgs {
     int64_t SP;              // 32 * chunks of this slab: stride of bd / kb
     int32_t n_ck;            // checkpoint rows per chunk: n_steps / CK + 1
     double* ck;              // [chunks][n_ck][6][32]
-    double* bd;              // [W][SP] best squared distance of the pair so far; e^2 afterwards
-    int32_t* kb;             // [W][SP] its row, -1 = none / far
+    double* bd;              // [W][SP] packed (d^2, row) key of the pair's closest state so far; e^2 afterwards
     int32_t* n_pts;          // [n_seeds]
     unsigned long long* items;
     unsigned int* n_items;
@@ -67,12 +87,11 @@ struct FusedArgs {
 };
 
 template <int Q>
-__global__ void __launch_bounds__(32 * COMET_FUSED_WARPS) k_scan_fused(const FusedArgs a)
+__global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
 {
     constexpr int TR = COMET_FUSED_TR, CK = COMET_FUSED_CK, ROW = 3 * COMET_LANES;
     constexpr int NSUB = TR / COMET_M1;
     constexpr unsigned FULL = 0xffffffffu;
-    constexpr int IMAX = 0x7fffffff;
     static_assert(TR % COMET_M1 == 0 && TR % CK == 0, "tile rows");
     extern __shared__ __align__(16) double fsm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -85,7 +104,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS) k_scan_fused(const Fus
     const double h = a.hk.h;
     const double INF = 1.7976931348623157e308;
     const double L = COMET_LIP * h;
-    const double half0 = (TR / 2) * L + COMET_SLACK, half1 = (COMET_M1 / 2) * L + COMET_SLACK;
+    const double half1 = (COMET_M1 / 2) * L + COMET_SLACK;
     const double lam2 = xmul(a.lambda, a.lambda);
 
     State st;
@@ -103,15 +122,14 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS) k_scan_fused(const Fus
     const bool use_stop = a.r_stop2 > 0.0;
 
     // pair workspace of this chunk: nothing found yet
-    for (int i = 0; i < W; ++i) {
-        a.bd[(size_t)i * a.SP + s] = INF;
-        a.kb[(size_t)i * a.SP + s] = -1;
-    }
+    unsigned long long* const keys = reinterpret_cast<unsigned long long*>(a.bd);
+    for (int i = 0; i < W; ++i) keys[(size_t)i * a.SP + s] = COMET_KEY_NONE;
 
-    // level-0 constants of this lane's wires (lane = wire): wire i = (r * Q + q) * 32 + lane
+    // shortlist constants of this lane's wires (lane = wire): wire i = (r * Q + q) * 32 + lane.  They stay
+    // in registers for the whole chunk; a visit of wire i (lane = seed) gets them by warp shuffles.
     const int n_rounds = (W + 32 * Q - 1) / (32 * Q);
     EvalC ec[Q];
-    int thi[Q];
+    double capq[Q];                                         // far radius; < 0: no entries / past the end
     auto load_round = [&](int r) {
 #pragma unroll
         for (int q = 0; q < Q; ++q) {
@@ -119,16 +137,24 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS) k_scan_fused(const Fus
             const int ii = min(i, W - 1);
             load_evalc(ec[q], a.wt, W, ii);
             const double cap = __ldg(a.wt + 14 * W + ii);
-            const double t0 = cap + half0;
-            thi[q] = (i < W && cap >= 0.0) ? __double2hiint(t0 * t0) : -1;
+            capq[q] = (i < W) ? cap : -1.0;
         }
     };
     if (n_rounds == 1) load_round(0);
 
     double* ckc = a.ck + (size_t)chunk * a.n_ck * (6 * COMET_LANES) + lane;
     const int n_tiles = (a.n_steps + TR) / TR;              // rows 0 .. n_steps
+#ifdef COMET_FUSED_PROF
+    long long pc_gen = 0, pc_l0 = 0, pc_l1 = 0, pc_visits = 0, pc_sweeps = 0, pc_mark;
+#define PC_MARK() (pc_mark = clock64())
+#define PC_ADD(v) do { const long long pc_now = clock64(); v += pc_now - pc_mark; pc_mark = pc_now; } while (0)
+#else
+#define PC_MARK()
+#define PC_ADD(v)
+#endif
     for (int t = 0; t < n_tiles; ++t) {
         const int r0 = t * TR;
+        PC_MARK();
         // ---- generate rows r0 .. r0 + TR - 1 (Algorithm 1; finished lanes hold their last state) ------
 #pragma unroll 2
         for (int rr = 0; rr < TR; ++rr) {
@@ -146,60 +172,76 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS) k_scan_fused(const Fus
             }
         }
         __syncwarp();
+        PC_ADD(pc_gen);
         const unsigned live = __ballot_sync(FULL, np > r0);  // lanes with a real row in this tile
-        // ---- level 0 (lane = wire) and, per wire with candidates, level 1 + sweeps (lane = seed) ------
+        if (!live) break;
+        // ---- level 0 (lane = wire): one evaluation per (wire, sub-block) --------------------------------
+        // The sample (row M1/2) of sub-block j of every live seed lies within `spread` of the sample of
+        // a representative seed -- measured perpendicular to the wire: at most rho_xy + rho_z sqrt(1 - w_z^2)
+        // for offsets of at most rho_xy in (x, y) and rho_z in z -- and the distance to a line is
+        // 1-Lipschitz, so no row of the sub-block of any seed is closer to the wire than
+        // d(representative sample) - spread - (M1/2) L.  Sub-blocks that cannot hold a state within the
+        // wire's far radius are skipped for the whole chunk; a chunk of unrelated seeds only loses pruning.
+        const int rep = __ffs(live) - 1;
+        const bool is_live = (live >> lane) & 1u;
+        double rx[NSUB][3];
+        float rxy[NSUB], rz[NSUB];
+#pragma unroll
+        for (int j = 0; j < NSUB; ++j) {
+            const double* ps = tile + (j * COMET_M1 + COMET_M1 / 2) * ROW + lane;
+            const double s0 = ps[0], s1 = ps[32], s2 = ps[64];
+            rx[j][0] = __shfl_sync(FULL, s0, rep); rx[j][1] = __shfl_sync(FULL, s1, rep); rx[j][2] = __shfl_sync(FULL, s2, rep);
+            const double e0 = s0 - rx[j][0], e1 = s1 - rx[j][1], e2 = s2 - rx[j][2];
+            const float fxy = is_live ? __fsqrt_ru(__double2float_ru(fma(e0, e0, e1 * e1))) : 0.f;
+            const float fz = is_live ? __double2float_ru(fabs(e2)) : 0.f;
+            // non-negative floats order like their bit patterns
+            rxy[j] = __uint_as_float(__reduce_max_sync(FULL, __float_as_uint(fxy)));
+            rz[j] = __uint_as_float(__reduce_max_sync(FULL, __float_as_uint(fz)));
+        }
+        const bool any_nolip = (nolip_mask & live) != 0u;
         for (int r = 0; r < n_rounds; ++r) {
             if (n_rounds > 1) load_round(r);
-            unsigned m[Q];
-#pragma unroll
-            for (int q = 0; q < Q; ++q) m[q] = 0u;
-            const double* sp = tile + (TR / 2) * ROW;
-#pragma unroll 4
-            for (int ss = 0; ss < 32; ++ss) {
-                const double x0 = sp[ss], x1 = sp[32 + ss], x2 = sp[64 + ss];
-#pragma unroll
-                for (int q = 0; q < Q; ++q)
-                    m[q] |= (unsigned)(__double2hiint(d2_fma(ec[q], x0, x1, x2)) <= thi[q]) << ss;
-            }
+            unsigned sm[Q];                                 // bit j: sub-block j of this tile may matter to wire q
 #pragma unroll
             for (int q = 0; q < Q; ++q) {
-                if (thi[q] >= 0) m[q] |= nolip_mask;
-                m[q] &= live;
-                unsigned any = __ballot_sync(FULL, m[q] != 0u);
+                sm[q] = 0u;
+                // sqrt(1 - w_z^2) = sqrt(e1z^2 + e2z^2) for the orthonormal basis {e1, e2, w}
+                const double swz = (double)__fsqrt_ru(__double2float_ru(fma(ec[q].e1z, ec[q].e1z, ec[q].e2z * ec[q].e2z)));
+#pragma unroll
+                for (int j = 0; j < NSUB; ++j) {
+                    const double spread = ((double)rxy[j] + (double)rz[j] * swz) * 1.000001;
+                    const double t0 = capq[q] + half1 + spread;
+                    if (d2_fma(ec[q], rx[j][0], rx[j][1], rx[j][2]) <= t0 * t0) sm[q] |= 1u << j;
+                }
+                if (any_nolip) sm[q] = (1u << NSUB) - 1u;
+                if (capq[q] < 0.0) sm[q] = 0u;
+            }
+            PC_ADD(pc_l0);
+#pragma unroll
+            for (int q = 0; q < Q; ++q) {
+                unsigned any = __ballot_sync(FULL, sm[q] != 0u);
                 while (any) {
                     const int wl = __ffs(any) - 1;
                     any &= any - 1;
-                    const unsigned mask = __shfl_sync(FULL, m[q], wl);
+                    unsigned wsub = __shfl_sync(FULL, sm[q], wl);
                     const int i = (r * Q + q) * 32 + wl;
-                    // ---- wire i, lane = seed ------------------------------------------------------
-                    const bool mine = (mask >> lane) & 1u;
-                    const size_t pidx = (size_t)i * a.SP + s;
-                    const double old = __ldcg(a.bd + pidx);           // used after the sweeps
+                    // ---- wire i, lane = seed: sweep the candidate sub-blocks row by row ------------------
+#ifdef COMET_FUSED_PROF
+                    pc_visits += 1;
+#endif
                     EvalC w;
-                    load_evalc(w, a.wt, W, i);                        // warp-uniform, L1-resident
-                    const double cap = __ldg(a.wt + 14 * W + i);
-                    int d1h[NSUB];
-                    int m1 = IMAX;
-#pragma unroll
-                    for (int j = 0; j < NSUB; ++j) {
-                        const double* ps = tile + (j * COMET_M1 + COMET_M1 / 2) * ROW + lane;
-                        d1h[j] = __double2hiint(d2_fma(w, ps[0], ps[32], ps[64]));
-                        m1 = min(m1, d1h[j]);
-                    }
-                    const double ub = fmin(cap, sqrt(__hiloint2double(m1 + 1, 0)));
-                    const double t1 = ub + half1;
-                    const int t1h = lip_ok ? __double2hiint(t1 * t1) : IMAX;
-                    unsigned sub = 0u;
-#pragma unroll
-                    for (int j = 0; j < NSUB; ++j)
-                        if (mine && d1h[j] <= t1h) sub |= 1u << j;
-                    unsigned wsub = __reduce_or_sync(FULL, sub);
-                    if (!wsub) continue;
-                    double best = old;
+                    w.e1x = __shfl_sync(FULL, ec[q].e1x, wl); w.e1y = __shfl_sync(FULL, ec[q].e1y, wl);
+                    w.e1z = __shfl_sync(FULL, ec[q].e1z, wl); w.c1 = __shfl_sync(FULL, ec[q].c1, wl);
+                    w.e2x = __shfl_sync(FULL, ec[q].e2x, wl); w.e2y = __shfl_sync(FULL, ec[q].e2y, wl);
+                    w.e2z = __shfl_sync(FULL, ec[q].e2z, wl); w.c2 = __shfl_sync(FULL, ec[q].c2, wl);
+                    double best = INF;
                     int bk = -1;
                     while (wsub) {
                         const int j = __ffs(wsub) - 1;
                         wsub &= wsub - 1;
+#ifdef COMET_FUSED_PROF
+                        pc_sweeps += 1;
+#endif
                         const double* pr = tile + (j * COMET_M1) * ROW + lane;
 #pragma unroll
                         for (int kk = 0; kk < COMET_M1; ++kk) {
@@ -209,28 +251,71 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS) k_scan_fused(const Fus
                             if (d2 < best && k < np) { best = d2; bk = k; }
                         }
                     }
-                    if (bk >= 0) { a.bd[pidx] = best; a.kb[pidx] = bk; }
+                    if (bk >= 0) atomicMin(keys + (size_t)i * a.SP + s, pack_key(best, bk));
                 }
             }
+            PC_ADD(pc_l1);
         }
         __syncwarp();
         if (!__any_sync(FULL, active)) break;
     }
+#ifdef COMET_FUSED_PROF
+    if (lane == 0 && a.stats) {
+        atomicAdd(a.stats + 0, (unsigned long long)pc_gen); atomicAdd(a.stats + 1, (unsigned long long)pc_l0);
+        atomicAdd(a.stats + 2, (unsigned long long)pc_l1); atomicAdd(a.stats + 3, (unsigned long long)pc_visits);
+        atomicAdd(a.stats + 4, (unsigned long long)pc_sweeps);
+    }
+    PC_MARK();
+#endif
     if (valid) a.n_pts[s] = np;
     // ---- finish: far pairs take the cutoff, (chunk, wire) items with a near lane go to k_fine_ck -------
-    for (int i = 0; i < W; ++i) {
-        const size_t pidx = (size_t)i * a.SP + s;
-        const double bdv = __ldcg(a.bd + pidx);
-        const int kbv = __ldcg(a.kb + pidx);
-        const double cap = __ldg(a.wt + 14 * W + i);
-        const bool near = valid && kbv >= 0 && (sqrt(bdv) <= cap || !lip_ok);
-        if (__any_sync(FULL, near)) {
-            if (!near && kbv >= 0) a.kb[pidx] = -1;
-            if (lane == 0) a.items[atomicAdd(a.n_items, 1u)] = ((unsigned long long)chunk << 16) | (unsigned)i;
-        } else {
-            a.bd[pidx] = lam2;
+    // Keys come from L2: FB wires in flight at a time.  The items are collected in the (now free) tile
+    // and appended to the work list with one reservation per LCAP items.
+    constexpr int FB = 8, LCAP = 1024;
+    static_assert(LCAP * (int)sizeof(unsigned short) <= TR * ROW * (int)sizeof(double), "item list fits the tile");
+    unsigned short* lst = reinterpret_cast<unsigned short*>(tile);
+    int cnt = 0;                                            // warp-uniform
+    auto flush = [&]() {
+        __syncwarp();
+        unsigned base = 0;
+        if (lane == 0) base = atomicAdd(a.n_items, (unsigned)cnt);
+        base = __shfl_sync(FULL, base, 0);
+        for (int j = lane; j < cnt; j += 32) a.items[base + j] = ((unsigned long long)chunk << 16) | (unsigned)lst[j];
+        cnt = 0;
+        __syncwarp();
+    };
+    for (int i0 = 0; i0 < W; i0 += FB) {
+        unsigned long long kv[FB];
+        double cap2[FB];
+#pragma unroll
+        for (int j = 0; j < FB; ++j) {
+            const int i = min(i0 + j, W - 1);
+            kv[j] = __ldcg(keys + (size_t)i * a.SP + s);
+            const double cap = __ldg(a.wt + 14 * W + i);
+            cap2[j] = cap * cap;
+        }
+#pragma unroll
+        for (int j = 0; j < FB; ++j) {
+            const int i = i0 + j;
+            if (i < W) {
+                const size_t pidx = (size_t)i * a.SP + s;
+                const bool found = kv[j] != COMET_KEY_NONE;
+                // key_d2 <= d^2 of the closest recorded state: "far" is decided on the safe side
+                const bool near = valid && found && (key_d2(kv[j]) <= cap2[j] || !lip_ok);
+                if (__any_sync(FULL, near)) {
+                    if (!near && found) keys[pidx] = COMET_KEY_NONE;
+                    if (lane == 0) lst[cnt] = (unsigned short)i;
+                    if (++cnt == LCAP) flush();
+                } else {
+                    a.bd[pidx] = lam2;
+                }
+            }
         }
     }
+    if (cnt) flush();
+#ifdef COMET_FUSED_PROF
+    if (lane == 0 && a.stats) atomicAdd(a.stats + 5, (unsigned long long)(clock64() - pc_mark));
+#endif
 }
 
 // Persistent warps over the work list: exact decision between bk-1, bk, bk+1 on states regenerated
@@ -249,9 +334,10 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, COMET_FINE_MINB) k_fine_ck
         const int i = (int)(item & 0xffffu);
         const int64_t s = chunk * COMET_LANES + lane;
         const size_t pidx = (size_t)i * a.SP + s;
-        const int bk = a.kb[pidx];
+        const unsigned long long key = reinterpret_cast<const unsigned long long*>(a.bd)[pidx];
+        const int bk = key_row(key);
         double e2 = lam2;
-        if (s < a.n_seeds && bk >= 0) {
+        if (s < a.n_seeds && key != COMET_KEY_NONE) {
             const int np = a.n_pts[s];
             const double px = a.seeds[3 * a.stride + s], py = a.seeds[4 * a.stride + s], pz = a.seeds[5 * a.stride + s];
             const double c = xdiv(a.qkb, xsqrt(xdot3(px, py, pz, px, py, pz)));
