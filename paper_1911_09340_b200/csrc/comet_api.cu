@@ -47,6 +47,8 @@ struct comet_ctx {
     size_t ck_max;               // growth limit of the checkpoint workspace
     int32_t* npw;
     size_t npw_cap;
+    double* cw;                  // [slab seeds] curvature constant c of every seed (fused path)
+    size_t cw_bytes;
     int fused_smem;
     // device workspace
     double* wt;            // wire table [14][wt_cap]
@@ -148,7 +150,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items);
     for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
-    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw);
+    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw);
     delete ctx;
     return COMET_OK;
 }
@@ -491,6 +493,8 @@ extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_
     if (rc) return rc;
     rc = grow_dev(ctx, (void**)&ctx->ck, &ctx->ck_bytes, (size_t)slab_chunks * ck_chunk);
     if (rc) return rc;
+    rc = grow_dev(ctx, (void**)&ctx->cw, &ctx->cw_bytes, (size_t)slab_chunks * COMET_LANES * sizeof(double));
+    if (rc) return rc;
     if (!n_pts) {
         size_t have = ctx->npw_cap * sizeof(int32_t);
         rc = grow_dev(ctx, (void**)&ctx->npw, &have, (size_t)slab_chunks * COMET_LANES * sizeof(int32_t));
@@ -519,6 +523,7 @@ extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_
         a.ck = ctx->ck;
         a.bd = ctx->e2;
         a.n_pts = n_pts ? n_pts + s0 : ctx->npw;
+        a.cw = ctx->cw;
         a.items = ctx->items;
         a.n_items = ctx->n_items;
         a.stats = ctx->opt_stats ? ctx->stats : nullptr;

@@ -26,10 +26,14 @@ namespace comet {
 #define COMET_DCA_WARPS 8
 
 // B1: wire prep, one thread per fired wire (once per event).
-// Field 14 is the wire's "far radius" R_i = max_j |rho_ij| + lambda + 1.01 h + 1e-6 cm (-1 for a
-// wire without entries): a track whose every recorded state is farther than R_i from the wire ends
-// the virtual-plane iteration (at most h of arc away from k*, R10) with |D| - |rho_ij| > lambda for
-// every entry, so its bounded residual is exactly lambda (pruned mode).
+// Field 14 is the wire's "far radius" R_i = max_j |rho_ij| + lambda + 0.51 h + 1e-6 cm (-1 for a
+// wire without entries).  The virtual-plane iteration ends on the arc between the recorded states
+// k*-1 and k*+1 (R10), at an offset sigma from k* with |sigma| <= h; that point is at most |sigma| of
+// arc from state k* and at most h - |sigma| from its neighbour on that side, and both are at least
+// d_k* from the wire (k* is the closest recorded state), so |D| >= d_k* - h/2 (1-Lipschitz; the
+// 0.01 h + 1e-6 cover the step-length excess 1.001 and the RKN error of the sub-steps).  A track whose
+// every recorded state is farther than R_i therefore has |D| - |rho_ij| > lambda for every entry and
+// its bounded residual is exactly lambda (pruned mode).
 __global__ void k_wire_prep(const double* __restrict__ wire_a, const double* __restrict__ wire_b,
                             int32_t n_wires, const int32_t* __restrict__ fired_wire, int32_t W,
                             const int32_t* __restrict__ hit_off, const double* __restrict__ rho,
@@ -62,7 +66,7 @@ __global__ void k_wire_prep(const double* __restrict__ wire_a, const double* __r
     wt[13 * W + i] = -(m0 * q0 + m1 * q1 + m2 * q2);
     double rmax = -1.0;
     for (int j = hit_off[i]; j < hit_off[i + 1]; ++j) rmax = fmax(rmax, fabs(rho[j]));
-    wt[14 * W + i] = (rmax < 0.0) ? -1.0 : rmax + lambda + 1.01 * h + 1e-6;
+    wt[14 * W + i] = (rmax < 0.0) ? -1.0 : rmax + lambda + 0.51 * h + 1e-6;
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)

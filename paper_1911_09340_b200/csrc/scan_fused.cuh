@@ -47,6 +47,9 @@ namespace comet {
 #ifndef COMET_FUSED_MINB
 #define COMET_FUSED_MINB 12        // resident CTAs per SM the register allocation aims at (<= 168 registers)
 #endif
+#ifndef COMET_FUSED_M1
+#define COMET_FUSED_M1 8           // rows per sub-block
+#endif
 #define COMET_FUSED_QMAX 3         // wires per lane and round in level 0
 
 // Packed shortlist key of a (seed, wire) pair: the bit pattern of the non-negative squared distance
@@ -81,6 +84,7 @@ struct FusedArgs {
     double* ck;              // [chunks][n_ck][6][32]
     double* bd;              // [W][SP] packed (d^2, row) key of the pair's closest state so far; e^2 afterwards
     int32_t* n_pts;          // [n_seeds]
+    double* cw;              // [SP] curvature constant c = kappa q B_z / |p| of every seed, for k_fine_ck
     unsigned long long* items;
     unsigned int* n_items;
     unsigned long long* stats;
@@ -90,9 +94,10 @@ template <int Q>
 __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
 {
     constexpr int TR = COMET_FUSED_TR, CK = COMET_FUSED_CK, ROW = 3 * COMET_LANES;
-    constexpr int NSUB = TR / COMET_M1;
+    constexpr int FM1 = COMET_FUSED_M1;
+    constexpr int NSUB = TR / FM1;
     constexpr unsigned FULL = 0xffffffffu;
-    static_assert(TR % COMET_M1 == 0 && TR % CK == 0, "tile rows");
+    static_assert(TR % FM1 == 0 && TR % CK == 0, "tile rows");
     extern __shared__ __align__(16) double fsm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* tile = fsm + warp * (TR * ROW);
@@ -104,7 +109,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
     const double h = a.hk.h;
     const double INF = 1.7976931348623157e308;
     const double L = COMET_LIP * h;
-    const double half1 = (COMET_M1 / 2) * L + COMET_SLACK;
+    const double half1 = (FM1 / 2) * L + COMET_SLACK;
     const double lam2 = xmul(a.lambda, a.lambda);
 
     State st;
@@ -188,7 +193,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
         float rxy[NSUB], rz[NSUB];
 #pragma unroll
         for (int j = 0; j < NSUB; ++j) {
-            const double* ps = tile + (j * COMET_M1 + COMET_M1 / 2) * ROW + lane;
+            const double* ps = tile + (j * FM1 + FM1 / 2) * ROW + lane;
             const double s0 = ps[0], s1 = ps[32], s2 = ps[64];
             rx[j][0] = __shfl_sync(FULL, s0, rep); rx[j][1] = __shfl_sync(FULL, s1, rep); rx[j][2] = __shfl_sync(FULL, s2, rep);
             const double e0 = s0 - rx[j][0], e1 = s1 - rx[j][1], e2 = s2 - rx[j][2];
@@ -242,11 +247,11 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
 #ifdef COMET_FUSED_PROF
                         pc_sweeps += 1;
 #endif
-                        const double* pr = tile + (j * COMET_M1) * ROW + lane;
+                        const double* pr = tile + (j * FM1) * ROW + lane;
 #pragma unroll
-                        for (int kk = 0; kk < COMET_M1; ++kk) {
+                        for (int kk = 0; kk < FM1; ++kk) {
                             const double d2 = d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
-                            const int k = r0 + j * COMET_M1 + kk;
+                            const int k = r0 + j * FM1 + kk;
                             // rows at or past n_pts repeat the last state: not recorded, never taken
                             if (d2 < best && k < np) { best = d2; bk = k; }
                         }
@@ -267,7 +272,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
     }
     PC_MARK();
 #endif
-    if (valid) a.n_pts[s] = np;
+    if (valid) { a.n_pts[s] = np; a.cw[s] = c; }
     // ---- finish: far pairs take the cutoff, (chunk, wire) items with a near lane go to k_fine_ck -------
     // Keys come from L2: FB wires in flight at a time.  The items are collected in the (now free) tile
     // and appended to the work list with one reservation per LCAP items.
@@ -339,8 +344,7 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, COMET_FINE_MINB) k_fine_ck
         double e2 = lam2;
         if (s < a.n_seeds && key != COMET_KEY_NONE) {
             const int np = a.n_pts[s];
-            const double px = a.seeds[3 * a.stride + s], py = a.seeds[4 * a.stride + s], pz = a.seeds[5 * a.stride + s];
-            const double c = xdiv(a.qkb, xsqrt(xdot3(px, py, pz, px, py, pz)));
+            const double c = a.cw[s];
             WireLine wl;
             wl.m0 = __ldg(a.wt + i); wl.m1 = __ldg(a.wt + W + i); wl.m2 = __ldg(a.wt + 2 * W + i);
             wl.w0 = __ldg(a.wt + 3 * W + i); wl.w1 = __ldg(a.wt + 4 * W + i); wl.w2 = __ldg(a.wt + 5 * W + i);
