@@ -1,15 +1,16 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the seed x hit scan on BASELINE.json configs[1], one JSON line.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1] [--path fused|materialised]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 
-A step is one pass of the whole hot path (comet_seed_extrapolate, comet_dca_rss,
-comet_select_and_classify) over one synthetic event whose inputs are resident in HBM.  `value` is
+A step is one pass of the whole hot path over one synthetic event whose inputs are resident in HBM:
+comet_scan_rss (kernels A + B fused, track on chip; default) or comet_seed_extrapolate + comet_dca_rss
+(--path materialised), then comet_select_and_classify.  `value` is
 seed x fired-wire DCA evaluations per second over all ranks (each rank scans its own replica of the
 event: weak scaling, no data-path collective).  `e2e` is the same metric through
 comet_scan_event_host with pinned HOST buffers (H2D of the inputs and D2H of the results inside the
-timed region).  `roofline` is for comet_dca_rss' kernel, timed live with CUDA events on its stream.
+timed region).  `roofline` is for the longest kernel of the step, timed live with CUDA events on its stream.
 `--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample.
 """
 import argparse
@@ -36,8 +37,11 @@ SHORTLIST_INSTR = 9
 FINE_INSTR = 600
 # 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz)
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum of k_dca_rss per launch (profiles/, ncu --set full); None = not captured
-DCA_TRAFFIC_BYTES = {}
+# FP64-pipe instructions per recorded state in kernel A: the RKN4 step of reading R1 is 48 IEEE operations
+# (44 issued: the two exact doublings ride on FMAs) + 4 for the target-region test of R3
+GEN_INSTR = 48
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1c_*, ncu --set full)
+TRAFFIC_BYTES = {}
 
 
 def _event(cfg):
@@ -168,6 +172,17 @@ class ClockSampler:
 # --------------------------------------------------------------------------------------------------
 # CUDA legs
 # --------------------------------------------------------------------------------------------------
+def _time_steps(fn, n, stream):
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(n):
+        out = fn()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / n, out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -187,97 +202,90 @@ def run_ours(args):
     torch.cuda.set_device(local)
     ev, seeds, part_off = _event(args.config)
     S, W, H, P = seeds.shape[1], ev.n_fired, ev.n_hits, len(part_off) - 1
+    fused = args.path == "fused"
     c = Comet(local)
-    c.set_option(OPT_COARSE_SEARCH, COARSE_PRUNED if args.coarse == "pruned" else COARSE_EXHAUSTIVE)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     d_seeds, d_wa, d_wb = dev(seeds), dev(ev.geom.wire_a), dev(ev.geom.wire_b)
     d_fw, d_ho, d_rho = dev(ev.fired_wire), dev(ev.hit_off), dev(ev.rho)
-    track = torch.empty(c.track_bytes(S, ev.n_steps), dtype=torch.uint8, device="cuda")
     n_pts = torch.empty(S, dtype=torch.int32, device="cuda")
     rss = torch.empty(S, dtype=torch.float64, device="cuda")
     phys = (ev.charge, ev.bz, ev.step, ev.n_steps)
     hits = (d_wa, d_wb, d_fw, d_ho, d_rho)
     stream = torch.cuda.current_stream()
-    b_events = []
+    track = None
 
-    def step(timed):
-        c.seed_extrapolate(d_seeds, *phys, ev.r_stop, track=track, n_pts=n_pts)
-        if timed:
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-        c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss)
-        if timed:
-            e1.record(stream)
-            b_events.append((e0, e1))
+    def step_fused():
+        c.scan_rss(d_seeds, *phys, ev.r_stop, *hits, ev.cutoff, rss=rss, n_pts=n_pts)
         return c.select_and_classify(d_seeds, *phys, ev.r_stop, *hits, ev.cutoff, rss, part_off)
 
+    def step_mat():
+        c.seed_extrapolate(d_seeds, *phys, ev.r_stop, track=track, n_pts=n_pts)
+        c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss)
+        return c.select_and_classify(d_seeds, *phys, ev.r_stop, *hits, ev.cutoff, rss, part_off)
+
+    if not fused:
+        track = torch.empty(c.track_bytes(S, ev.n_steps), dtype=torch.uint8, device="cuda")
+    step = step_fused if fused else step_mat
+    knames = ("k_scan_fused", "k_fine_ck", "k_rss_sum") if fused else ("k_coarse_pruned", "k_fine", "k_rss_sum")
+
     for _ in range(args.warmup):
-        step(False)
+        step()
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     sampler = ClockSampler(local) if rank == 0 else None
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    if args.coarse == "pruned":
-        c.set_option(OPT_TIMING, 1)          # the library brackets its kernels with CUDA events on the stream
+    c.set_option(OPT_TIMING, 1)          # the library brackets its kernels with CUDA events on its stream
     torch.cuda.synchronize()
-    t0.record(stream)
-    for _ in range(args.steps):
-        out = step(True)
-    t1.record(stream)
-    torch.cuda.synchronize()
-    ktimes_live = None
-    if args.coarse == "pruned":
-        ktimes_live = c.read_timing()        # mean over the last <= 64 timed steps
-        c.set_option(OPT_TIMING, 0)
+    ms_per_step, out = _time_steps(step, args.steps, stream)
+    ktimes = c.read_timing(knames)       # mean over the last <= 64 timed steps
+    c.set_option(OPT_TIMING, 0)
     if world > 1:
         dist.barrier()
     clocks = sampler.stop() if sampler else None
-    ms = t0.elapsed_time(t1)
-    ms_b = float(np.mean([a.elapsed_time(b) for a, b in b_events]))
     if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        t = torch.tensor([ms_per_step], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    ms_per_step = ms / args.steps
+        ms_per_step = float(t.item())
     pairs = float(S) * W
     value = world * pairs / (ms_per_step * 1e-3)
     n_states = float(n_pts.sum().item())
     best = out["best_seed"].cpu().numpy().tolist()
     n_cls = int(out["cls"].sum().item())
+    rss_main = rss.clone()
 
-    # ---- work counters and per-kernel device times of the pruned search (untimed extra launches) ---
-    stats, ktimes = None, None
-    if args.coarse == "pruned":
-        c.set_option(OPT_STATS, 1)
-        c.read_stats(reset=True)
+    # ---- work counters (one untimed extra pass) -------------------------------------------------
+    c.set_option(OPT_STATS, 1)
+    c.read_stats(reset=True)
+    if fused:
+        c.scan_rss(d_seeds, *phys, ev.r_stop, *hits, ev.cutoff, rss=rss, n_pts=n_pts)
+    else:
         c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss)
-        stats = c.read_stats(reset=True)
-        c.set_option(OPT_STATS, 0)
-        ktimes = ktimes_live
-    other = "exhaustive" if args.coarse == "pruned" else "pruned"
-    c.set_option(OPT_COARSE_SEARCH, COARSE_EXHAUSTIVE if other == "exhaustive" else COARSE_PRUNED)
-    rss2 = torch.empty_like(rss)
-    o_ev = []
-    for i in range(1 + min(args.steps, 5)):
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record(stream)
-        c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss2)
-        e1.record(stream)
-        if i:
-            o_ev.append((e0, e1))
-    torch.cuda.synchronize()
-    ms_other = float(np.mean([a.elapsed_time(b) for a, b in o_ev]))
-    modes_agree = bool(torch.equal(rss, rss2))
-    c.set_option(OPT_COARSE_SEARCH, COARSE_PRUNED if args.coarse == "pruned" else COARSE_EXHAUSTIVE)
+    stats = c.read_stats(reset=True)
+    c.set_option(OPT_STATS, 0)
+
+    # ---- the other path and the exhaustive closest-state search, for comparison (untimed region) ----
+    n_cmp = 1 + min(args.steps, 5)
+    if track is None:
+        track = torch.empty(c.track_bytes(S, ev.n_steps), dtype=torch.uint8, device="cuda")
+    other_step = step_mat if fused else step_fused
+    other_step()
+    ms_other, _ = _time_steps(other_step, n_cmp, stream)
+    paths_agree = bool(torch.equal(rss, rss_main))
+    c.seed_extrapolate(d_seeds, *phys, ev.r_stop, track=track, n_pts=n_pts)
+    c.set_option(OPT_COARSE_SEARCH, COARSE_EXHAUSTIVE)
+    exh = lambda: c.dca_rss(track, n_pts, d_seeds, *phys, *hits, ev.cutoff, rss=rss)
+    exh()
+    ms_exh, _ = _time_steps(exh, n_cmp, stream)
+    exh_agree = bool(torch.equal(rss, rss_main))
+    c.set_option(OPT_COARSE_SEARCH, COARSE_PRUNED)
+    del track
+    torch.cuda.empty_cache()
 
     # ---- e2e: host buffers through comet_scan_event_host -------------------------------------
     pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
     h = dict(seeds=pin(seeds, torch.float64), wa=pin(ev.geom.wire_a, torch.float64), wb=pin(ev.geom.wire_b, torch.float64),
              fw=pin(ev.fired_wire, torch.int32), ho=pin(ev.hit_off, torch.int32), rho=pin(ev.rho, torch.float64))
-    del track
-    torch.cuda.empty_cache()
-    budget = 8 << 30
+    budget = 0 if fused else 8 << 30
     hout = None
 
     def e2e_step():
@@ -316,64 +324,58 @@ def run_ours(args):
         torch.cuda.synchronize()
         best_ms = min(best_ms, pe0.elapsed_time(pe1))
     peak_measured = 2 * n_fma / (best_ms * 1e-3) / 1e12
-    flops_exh = 2.0 * (SHORTLIST_INSTR * n_states * W + FINE_INSTR * pairs)
     peak = FP64_PEAK_NOMINAL_TFLOPS
-    if stats is not None:
-        fl = {"k_coarse_pruned": 2.0 * SHORTLIST_INSTR * (stats["samples"] + stats["rows_needed"]),
-              "k_fine": 2.0 * FINE_INSTR * stats["fine_needed"]}
-        fl_exec = {"k_coarse_pruned": 2.0 * SHORTLIST_INSTR * (stats["samples"] + stats["rows_executed"]),
-                   "k_fine": 2.0 * FINE_INSTR * stats["fine_executed"]}
-        kernels = {"timed_over": "last %d steps of the timed region (CUDA events recorded by the library on its stream)" % ktimes["n_calls"]}
-        kernels.update({k: {"ms_per_launch": ktimes[k], "achieved": fl[k] / (ktimes[k] * 1e-3) / 1e12,
-                       "frac": fl[k] / (ktimes[k] * 1e-3) / 1e12 / peak,
-                       "achieved_executed": fl_exec[k] / (ktimes[k] * 1e-3) / 1e12,
-                       "share_of_step": ktimes[k] / ms_per_step} for k in fl})
-        kernels["k_rss_sum"] = {"ms_per_launch": ktimes["k_rss_sum"], "bound": "hbm",
-                                "achieved_gbs": (pairs * 8 + S * 8) / (ktimes["k_rss_sum"] * 1e-3) / 1e9}
-        kernel = max(fl, key=lambda k: ktimes[k])
-        ms_k, achieved = ktimes[kernel], kernels[kernel]["achieved"]
-        model = ("FP64-pipe slots x 2 of the work the pruned search needs (thread-level counters, comet_read_stats): "
-                 "k_coarse_pruned %d per block/sub-block sample or row evaluation; k_fine %d per (seed, wire) pair "
-                 "that runs the plane iteration" % (SHORTLIST_INSTR, FINE_INSTR))
-        ms_exh = ms_other
-    else:
-        kernels, kernel, ms_k = None, "k_dca_rss", ms_b
-        achieved = flops_exh / (ms_b * 1e-3) / 1e12
-        model = ("FP64-pipe slots x 2: %d per (seed, wire, recorded state) + %d per (seed, wire)"
-                 % (SHORTLIST_INSTR, FINE_INSTR))
-        ms_exh = ms_b
+    ev_needed = stats["samples"] + stats["rows_needed"]
+    ev_exec = stats["samples"] + stats["rows_executed"]
+    gen = GEN_INSTR * n_states if fused else 0.0
+    fl = {knames[0]: 2.0 * (gen + SHORTLIST_INSTR * ev_needed), knames[1]: 2.0 * FINE_INSTR * stats["fine_needed"]}
+    fl_exec = {knames[0]: 2.0 * (gen + SHORTLIST_INSTR * ev_exec), knames[1]: 2.0 * FINE_INSTR * stats["fine_executed"]}
+    kernels = {"timed_over": "last %d steps of the timed region (CUDA events recorded by the library on its stream)" % ktimes["n_calls"]}
+    kernels.update({k: {"ms_per_launch": ktimes[k], "achieved": fl[k] / (ktimes[k] * 1e-3) / 1e12,
+                        "frac": fl[k] / (ktimes[k] * 1e-3) / 1e12 / peak,
+                        "achieved_executed": fl_exec[k] / (ktimes[k] * 1e-3) / 1e12,
+                        "share_of_step": ktimes[k] / ms_per_step} for k in fl})
+    kernels["k_rss_sum"] = {"ms_per_launch": ktimes["k_rss_sum"], "bound": "hbm",
+                            "achieved_gbs": (pairs * 8 + S * 8) / (ktimes["k_rss_sum"] * 1e-3) / 1e9}
+    kernel = max(fl, key=lambda k: ktimes[k])
+    model = ("FP64-pipe slots x 2 of the work the path needs (thread-level counters, comet_read_stats): "
+             + ("%d per recorded state (RKN4 step + target-region test, Alg. 1), " % GEN_INSTR if fused else "")
+             + "%d per shortlist evaluation (sub-block sample or swept row); %s: %d per (seed, wire) pair that runs "
+               "the virtual-plane iteration" % (SHORTLIST_INSTR, knames[1], FINE_INSTR))
+    flops_exh = 2.0 * (SHORTLIST_INSTR * n_states * W + FINE_INSTR * pairs)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": _workload_name(args.config, ev, seeds, part_off),
-                   "coarse_search": args.coarse,
-                   "l2": "inputs larger than L2 (126 MB): every step rewrites the recorded part of the track buffer "
-                         "(%.1f GB of the %.1f GB allocation) and kernel B rereads it"
-                         % (n_states * 48 / 1e9, c.track_bytes(S, ev.n_steps) / 1e9),
+                   "path": ("fused: comet_scan_rss (track on chip) + comet_select_and_classify" if fused else
+                            "materialised: comet_seed_extrapolate + comet_dca_rss + comet_select_and_classify"),
+                   "l2": ("working set larger than L2 (126 MB): every step rewrites %.1f GB of checkpoints and %.2f GB of "
+                          "(seed, wire) pair keys and rereads them" % (n_states * 12 / 1e9, pairs * 8 / 1e9)) if fused else
+                         ("inputs larger than L2 (126 MB): every step rewrites the recorded part of the track buffer "
+                          "(%.1f GB) and kernel B rereads it" % (n_states * 48 / 1e9)),
                    "parallelism": "one replica of the event per GPU (event-level sharding, no collective)"},
         "events_per_s": world / (ms_per_step * 1e-3),
         "result": {"best_seed": best, "classified_entries": n_cls, "recorded_states_per_seed": n_states / S},
         "e2e": {"value": world * pairs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "ms_per_step": e2e_s * 1e3, "api": "comet_scan_event_host, pinned host buffers, %d GiB track slab" % (budget >> 30)},
-        "gpu_launches": (8 if args.coarse == "pruned" else 6) * args.steps,
+                "ms_per_step": e2e_s * 1e3,
+                "api": "comet_scan_event_host, pinned host buffers" + ("" if fused else ", %d GiB track slab" % (budget >> 30))},
+        "gpu_launches": (7 if fused else 8) * args.steps,
         "clocks": clocks,
-        "roofline": {"kernel": kernel, "bound": "alu", "achieved": achieved, "peak": peak,
-                     "unit": "TFLOP/s", "frac": achieved / peak, "traffic": DCA_TRAFFIC_BYTES.get(kernel),
+        "roofline": {"kernel": kernel, "bound": "alu", "achieved": kernels[kernel]["achieved"], "peak": peak,
+                     "unit": "TFLOP/s", "frac": kernels[kernel]["frac"], "traffic": TRAFFIC_BYTES.get(kernel),
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 figure)",
-                     "peak_measured_dfma_probe": peak_measured, "frac_of_measured": achieved / peak_measured,
-                     "ms_per_launch": ms_k, "share_of_step": ms_k / ms_per_step,
-                     "model": model,
-                     "comet_dca_rss_ms": ms_b, "comet_dca_rss_share_of_step": ms_b / ms_per_step,
-                     "kernels": kernels,
-                     "work_counters": stats,
-                     "exhaustive_kernel": {"kernel": "k_dca_rss", "ms_per_launch": ms_exh,
+                     "peak_measured_dfma_probe": peak_measured,
+                     "frac_of_measured": kernels[kernel]["achieved"] / peak_measured,
+                     "ms_per_launch": ktimes[kernel], "share_of_step": ktimes[kernel] / ms_per_step,
+                     "model": model, "kernels": kernels, "work_counters": stats,
+                     "other_path": {"path": "materialised" if fused else "fused", "ms_per_step": ms_other,
+                                    "rss_bit_identical": paths_agree},
+                     "exhaustive_search": {"kernel": "k_dca_rss", "ms_per_launch": ms_exh, "rss_bit_identical": exh_agree,
                                            "achieved": flops_exh / (ms_exh * 1e-3) / 1e12,
                                            "frac": flops_exh / (ms_exh * 1e-3) / 1e12 / peak,
                                            "model": "%d per (seed, wire, recorded state) + %d per (seed, wire)"
-                                                    % (SHORTLIST_INSTR, FINE_INSTR)},
-                     "other_mode": {"coarse_search": other, "ms_per_launch": ms_other, "rss_bit_identical": modes_agree},
-                     "track_bytes_read_once": n_states * 24},
+                                                    % (SHORTLIST_INSTR, FINE_INSTR)}},
     }
     if args.cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(ev, seeds, part_off)
@@ -390,7 +392,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--coarse", choices=["exhaustive", "pruned"], default="pruned")
+    ap.add_argument("--path", choices=["fused", "materialised"], default="fused")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     args = ap.parse_args()
     if args.impl == "reference":

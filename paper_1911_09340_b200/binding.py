@@ -143,14 +143,16 @@ class Comet:
         """Pre-allocates the pruned search's (seed, wire) pair workspace (12 bytes per pair)."""
         self._check(self._L.comet_reserve(self._h, int(max_pairs_per_launch)))
 
-    def read_timing(self) -> dict:
-        """Mean device milliseconds per kernel of the latest (<= 64) pruned comet_dca_rss slabs made with
-        OPT_TIMING = 1 (waits for them)."""
+    def read_timing(self, names=("k_coarse_pruned", "k_fine", "k_rss_sum")) -> dict:
+        """Mean device milliseconds per kernel of the latest (<= 64) seed slabs of comet_dca_rss (pruned:
+        k_coarse_pruned, k_fine, k_rss_sum) or comet_scan_rss (k_scan_fused, k_fine_ck, k_rss_sum) made
+        with OPT_TIMING = 1 (waits for them).  `names` labels the three slots."""
         buf = (ctypes.c_float * 3)()
         n = ctypes.c_int32()
         self._check(self._L.comet_read_timing(self._h, buf, 3, ctypes.byref(n)))
-        return {"k_coarse_pruned": float(buf[0]), "k_fine": float(buf[1]), "k_rss_sum": float(buf[2]),
-                "n_calls": int(n.value)}
+        out = {k: float(v) for k, v in zip(names, buf)}
+        out["n_calls"] = int(n.value)
+        return out
 
     def read_stats(self, reset: bool = True, stream=None) -> dict:
         """Work counters of the pruned comet_dca_rss calls made with OPT_STATS = 1 (synchronises)."""

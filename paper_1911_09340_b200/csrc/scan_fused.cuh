@@ -90,7 +90,7 @@ struct FusedArgs {
     unsigned long long* stats;
 };
 
-template <int Q>
+template <int Q, bool STATS>
 __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
 {
     constexpr int TR = COMET_FUSED_TR, CK = COMET_FUSED_CK, ROW = 3 * COMET_LANES;
@@ -149,6 +149,12 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
 
     double* ckc = a.ck + (size_t)chunk * a.n_ck * (6 * COMET_LANES) + lane;
     const int n_tiles = (a.n_steps + TR) / TR;              // rows 0 .. n_steps
+    unsigned long long st_cnt[ST_N];                        // work counters (COMET_OPT_STATS), thread-level
+    if (STATS) {
+#pragma unroll
+        for (int j = 0; j < ST_N; ++j) st_cnt[j] = 0;
+        if (valid) st_cnt[ST_PAIRS] = (unsigned long long)W;
+    }
 #ifdef COMET_FUSED_PROF
     long long pc_gen = 0, pc_l0 = 0, pc_l1 = 0, pc_visits = 0, pc_sweeps = 0, pc_mark;
 #define PC_MARK() (pc_mark = clock64())
@@ -220,6 +226,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
                 }
                 if (any_nolip) sm[q] = (1u << NSUB) - 1u;
                 if (capq[q] < 0.0) sm[q] = 0u;
+                if (STATS && capq[q] >= 0.0) st_cnt[ST_SAMPLES] += NSUB;
             }
             PC_ADD(pc_l0);
 #pragma unroll
@@ -248,6 +255,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
                         pc_sweeps += 1;
 #endif
                         const double* pr = tile + (j * FM1) * ROW + lane;
+                        if (STATS) { st_cnt[ST_ROWS_EXEC] += FM1; if (is_live) st_cnt[ST_ROWS_NEEDED] += FM1; }
 #pragma unroll
                         for (int kk = 0; kk < FM1; ++kk) {
                             const double d2 = d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
@@ -307,7 +315,9 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
                 const bool found = kv[j] != COMET_KEY_NONE;
                 // key_d2 <= d^2 of the closest recorded state: "far" is decided on the safe side
                 const bool near = valid && found && (key_d2(kv[j]) <= cap2[j] || !lip_ok);
+                if (STATS && near) st_cnt[ST_FINE_NEEDED] += 1;
                 if (__any_sync(FULL, near)) {
+                    if (STATS) st_cnt[ST_FINE_EXEC] += 1;
                     if (!near && found) keys[pidx] = COMET_KEY_NONE;
                     if (lane == 0) lst[cnt] = (unsigned short)i;
                     if (++cnt == LCAP) flush();
@@ -318,6 +328,16 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
         }
     }
     if (cnt) flush();
+#ifndef COMET_FUSED_PROF
+    if (STATS) {
+#pragma unroll
+        for (int j = 0; j < ST_N; ++j) {
+            unsigned long long v = st_cnt[j];
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(FULL, v, o);
+            if (lane == 0 && a.stats && v) atomicAdd(a.stats + j, v);
+        }
+    }
+#endif
 #ifdef COMET_FUSED_PROF
     if (lane == 0 && a.stats) atomicAdd(a.stats + 5, (unsigned long long)(clock64() - pc_mark));
 #endif
