@@ -111,13 +111,11 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaMemset(ctx->stats, 0, sizeof(unsigned long long) * ST_N);
     ctx->pair_max = (size_t)1 << 26;
     ctx->ck_max = (size_t)8 << 30;
-    ctx->fused_smem = COMET_FUSED_WARPS * COMET_FUSED_TR * 3 * COMET_LANES * (int)sizeof(double);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
+    ctx->fused_smem = ((COMET_FUSED_WFIELDS + 1) * COMET_FUSED_WCAP + COMET_FUSED_WARPS * COMET_FUSED_TR * 3 * COMET_LANES) * (int)sizeof(double);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int));
     if (e == cudaSuccess) {
         int per_sm = 0;
@@ -504,7 +502,6 @@ extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_
         if (rc) return rc;
         ctx->npw_cap = have / sizeof(int32_t);
     }
-    const int q = n_fired <= 32 ? 1 : (n_fired <= 64 ? 2 : 3);
     for (int64_t c0 = 0; c0 < total_chunks; c0 += slab_chunks) {
         const int64_t nc = (total_chunks - c0 < slab_chunks) ? (total_chunks - c0) : slab_chunks;
         const int64_t s0 = c0 * COMET_LANES;
@@ -540,15 +537,8 @@ extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_
         cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
         if (tm) CU(ctx, cudaEventRecord(tev[0], st));
         const int thr = 32 * COMET_FUSED_WARPS;
-        if (a.stats) {
-            if (q == 1) k_scan_fused<1, true><<<b1, thr, ctx->fused_smem, st>>>(a);
-            else if (q == 2) k_scan_fused<2, true><<<b1, thr, ctx->fused_smem, st>>>(a);
-            else k_scan_fused<3, true><<<b1, thr, ctx->fused_smem, st>>>(a);
-        } else {
-            if (q == 1) k_scan_fused<1, false><<<b1, thr, ctx->fused_smem, st>>>(a);
-            else if (q == 2) k_scan_fused<2, false><<<b1, thr, ctx->fused_smem, st>>>(a);
-            else k_scan_fused<3, false><<<b1, thr, ctx->fused_smem, st>>>(a);
-        }
+        if (a.stats) k_scan_fused<true><<<b1, thr, ctx->fused_smem, st>>>(a);
+        else k_scan_fused<false><<<b1, thr, ctx->fused_smem, st>>>(a);
         if (tm) CU(ctx, cudaEventRecord(tev[1], st));
         if (n_fired > 0) k_fine_ck<<<b2, COMET_FINE_THREADS, 0, st>>>(a);
         if (tm) CU(ctx, cudaEventRecord(tev[2], st));

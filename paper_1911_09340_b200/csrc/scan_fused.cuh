@@ -7,14 +7,14 @@
 //   generate   TR RKN4 steps per lane (the definition's operations, common.cuh), the positions of the
 //              TR rows go to a warp-private shared-memory tile [TR][3][32] fp64 (conflict-free, never
 //              to HBM); every CK-th recorded state (x, T) is written to a small checkpoint buffer;
-//   level 0    one evaluation per (8-row sub-block, wire) with lane = WIRE: the wire's shortlist
-//              constants stay in registers for the whole chunk; the sub-block sample of one
-//              representative seed and the largest offset of the other seeds' samples from it bound
-//              every seed's distance from below (Lipschitz bound of dca.cuh with the wire's far radius
-//              as the upper bound), so a sub-block is opened for a wire only if some seed may have its
-//              closest state there;
-//   sweeps     per wire with candidate sub-blocks (lane = seed again, the wire's constants arrive by
-//              warp shuffles): their rows are evaluated from the tile; the tile's
+//   level 0    one evaluation per (8-row sub-block, wire) with lane = WIRE, the wires' shortlist
+//              constants coming from a table in shared memory (one copy per CTA): the sub-block sample
+//              of one representative seed and the largest offset of the other seeds' samples from it
+//              bound every seed's distance from below (Lipschitz bound of dca.cuh with the wire's far
+//              radius as the upper bound), so a sub-block is opened for a wire only if some seed may
+//              have its closest state there;
+//   sweeps     per wire with open sub-blocks (lane = seed again, the wire's constants are broadcast
+//              from the table): their rows are evaluated from the tile; the tile's
 //              best (squared distance, row) of the pair is merged into the pair workspace with one
 //              fire-and-forget 64-bit atomic min on a packed key (no read-modify-write round trip to
 //              L2): key = bits(d^2) with the low 13 bits replaced by the row, so keys order by d^2
@@ -42,15 +42,19 @@ namespace comet {
 #define COMET_FUSED_CK 4           // rows between checkpoints
 #endif
 #ifndef COMET_FUSED_WARPS
-#define COMET_FUSED_WARPS 1        // warps (chunks) per CTA
+#define COMET_FUSED_WARPS 4        // warps (chunks) per CTA; they share the wire table
 #endif
 #ifndef COMET_FUSED_MINB
-#define COMET_FUSED_MINB 12        // resident CTAs per SM the register allocation aims at (<= 168 registers)
+#define COMET_FUSED_MINB 4         // resident CTAs per SM the register allocation aims at
 #endif
 #ifndef COMET_FUSED_M1
 #define COMET_FUSED_M1 8           // rows per sub-block
 #endif
-#define COMET_FUSED_QMAX 3         // wires per lane and round in level 0
+#ifndef COMET_FUSED_WCAP
+#define COMET_FUSED_WCAP 96        // wires whose constants the shared-memory table holds (the others: L1/L2)
+#endif
+#define COMET_FUSED_WFIELDS 9      // e1[3] -m.e1 | e2[3] -m.e2 | far radius  (fields 6..14 of the wire table)
+// the CTA's table has one more row: sqrt(1 - w_z^2) rounded up, the wire's slope against the z axis
 
 // Packed shortlist key of a (seed, wire) pair: the bit pattern of the non-negative squared distance
 // (monotone as an unsigned integer) with its 13 low mantissa bits replaced by the row (<= 4096).
@@ -79,7 +83,7 @@ struct FusedArgs {
     const int32_t* hit_off;
     const double* rho;
     double lambda;
-    int64_t SP;              // 32 * chunks of this slab: stride of bd / kb
+    int64_t SP;              // 32 * chunks of this slab: stride of bd
     int32_t n_ck;            // checkpoint rows per chunk: n_steps / CK + 1
     double* ck;              // [chunks][n_ck][6][32]
     double* bd;              // [W][SP] packed (d^2, row) key of the pair's closest state so far; e^2 afterwards
@@ -90,22 +94,51 @@ struct FusedArgs {
     unsigned long long* stats;
 };
 
-template <int Q, bool STATS>
+// shortlist constants of wire i: from the CTA's table when it holds the wire, else from the wire table
+// in global memory (warp-uniform or lane-contiguous addresses either way)
+__device__ __forceinline__ double wconst(const double* wtab, const double* __restrict__ wt, int W, int f, int i)
+{
+    return (i < COMET_FUSED_WCAP) ? wtab[f * COMET_FUSED_WCAP + i] : __ldg(wt + (size_t)(6 + f) * W + i);
+}
+__device__ __forceinline__ void wconst_evalc(EvalC& w, const double* wtab, const double* __restrict__ wt, int W, int i)
+{
+    w.e1x = wconst(wtab, wt, W, 0, i); w.e1y = wconst(wtab, wt, W, 1, i); w.e1z = wconst(wtab, wt, W, 2, i);
+    w.c1 = wconst(wtab, wt, W, 3, i);
+    w.e2x = wconst(wtab, wt, W, 4, i); w.e2y = wconst(wtab, wt, W, 5, i); w.e2z = wconst(wtab, wt, W, 6, i);
+    w.c2 = wconst(wtab, wt, W, 7, i);
+}
+
+// sqrt(1 - w_z^2) = sqrt(e1z^2 + e2z^2) for the orthonormal basis {e1, e2, w}, rounded up
+__device__ __forceinline__ double wire_slope(double e1z, double e2z)
+{
+    return (double)__fsqrt_ru(__double2float_ru(fma(e1z, e1z, e2z * e2z)));
+}
+
+template <bool STATS>
 __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
 {
     constexpr int TR = COMET_FUSED_TR, CK = COMET_FUSED_CK, ROW = 3 * COMET_LANES;
     constexpr int FM1 = COMET_FUSED_M1;
     constexpr int NSUB = TR / FM1;
+    constexpr int WCAP = COMET_FUSED_WCAP;
     constexpr unsigned FULL = 0xffffffffu;
     static_assert(TR % FM1 == 0 && TR % CK == 0, "tile rows");
     extern __shared__ __align__(16) double fsm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double* tile = fsm + warp * (TR * ROW);
+    double* wtab = fsm;                                     // [WFIELDS + 1][WCAP]
+    double* tile = fsm + (COMET_FUSED_WFIELDS + 1) * WCAP + warp * (TR * ROW);
+    const int W = a.W;
+    for (int v = threadIdx.x; v < COMET_FUSED_WFIELDS * WCAP; v += 32 * COMET_FUSED_WARPS) {
+        const int f = v / WCAP, i = v - f * WCAP;
+        wtab[v] = (i < W) ? __ldg(a.wt + (size_t)(6 + f) * W + i) : -1.0;
+    }
+    for (int i = threadIdx.x; i < WCAP; i += 32 * COMET_FUSED_WARPS)
+        wtab[COMET_FUSED_WFIELDS * WCAP + i] = (i < W) ? wire_slope(__ldg(a.wt + (size_t)8 * W + i), __ldg(a.wt + (size_t)12 * W + i)) : 0.0;
+    __syncthreads();
     const int64_t chunk = (int64_t)blockIdx.x * COMET_FUSED_WARPS + warp;
     if (chunk * COMET_LANES >= a.n_seeds) return;
     const int64_t s = chunk * COMET_LANES + lane;
     const bool valid = s < a.n_seeds;
-    const int W = a.W;
     const double h = a.hk.h;
     const double INF = 1.7976931348623157e308;
     const double L = COMET_LIP * h;
@@ -130,23 +163,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
     unsigned long long* const keys = reinterpret_cast<unsigned long long*>(a.bd);
     for (int i = 0; i < W; ++i) keys[(size_t)i * a.SP + s] = COMET_KEY_NONE;
 
-    // shortlist constants of this lane's wires (lane = wire): wire i = (r * Q + q) * 32 + lane.  They stay
-    // in registers for the whole chunk; a visit of wire i (lane = seed) gets them by warp shuffles.
-    const int n_rounds = (W + 32 * Q - 1) / (32 * Q);
-    EvalC ec[Q];
-    double capq[Q];                                         // far radius; < 0: no entries / past the end
-    auto load_round = [&](int r) {
-#pragma unroll
-        for (int q = 0; q < Q; ++q) {
-            const int i = (r * Q + q) * 32 + lane;
-            const int ii = min(i, W - 1);
-            load_evalc(ec[q], a.wt, W, ii);
-            const double cap = __ldg(a.wt + 14 * W + ii);
-            capq[q] = (i < W) ? cap : -1.0;
-        }
-    };
-    if (n_rounds == 1) load_round(0);
-
+    const int n_rounds = (W + 31) / 32;                     // level 0: wire i = r * 32 + lane
     double* ckc = a.ck + (size_t)chunk * a.n_ck * (6 * COMET_LANES) + lane;
     const int n_tiles = (a.n_steps + TR) / TR;              // rows 0 .. n_steps
     unsigned long long st_cnt[ST_N];                        // work counters (COMET_OPT_STATS), thread-level
@@ -211,61 +228,56 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
         }
         const bool any_nolip = (nolip_mask & live) != 0u;
         for (int r = 0; r < n_rounds; ++r) {
-            if (n_rounds > 1) load_round(r);
-            unsigned sm[Q];                                 // bit j: sub-block j of this tile may matter to wire q
-#pragma unroll
-            for (int q = 0; q < Q; ++q) {
-                sm[q] = 0u;
-                // sqrt(1 - w_z^2) = sqrt(e1z^2 + e2z^2) for the orthonormal basis {e1, e2, w}
-                const double swz = (double)__fsqrt_ru(__double2float_ru(fma(ec[q].e1z, ec[q].e1z, ec[q].e2z * ec[q].e2z)));
+            unsigned sm = 0u;                               // bit j: sub-block j of this tile may matter to the lane's wire
+            {
+                const int i = r * 32 + lane;
+                const int ii = min(i, W - 1);
+                EvalC ec;
+                wconst_evalc(ec, wtab, a.wt, W, ii);
+                const double cap = (i < W) ? wconst(wtab, a.wt, W, 8, ii) : -1.0;   // far radius; < 0: no entries
+                const double swz = (ii < WCAP) ? wtab[COMET_FUSED_WFIELDS * WCAP + ii] : wire_slope(ec.e1z, ec.e2z);
 #pragma unroll
                 for (int j = 0; j < NSUB; ++j) {
                     const double spread = ((double)rxy[j] + (double)rz[j] * swz) * 1.000001;
-                    const double t0 = capq[q] + half1 + spread;
-                    if (d2_fma(ec[q], rx[j][0], rx[j][1], rx[j][2]) <= t0 * t0) sm[q] |= 1u << j;
+                    const double t0 = cap + half1 + spread;
+                    if (d2_fma(ec, rx[j][0], rx[j][1], rx[j][2]) <= t0 * t0) sm |= 1u << j;
                 }
-                if (any_nolip) sm[q] = (1u << NSUB) - 1u;
-                if (capq[q] < 0.0) sm[q] = 0u;
-                if (STATS && capq[q] >= 0.0) st_cnt[ST_SAMPLES] += NSUB;
+                if (any_nolip) sm = (1u << NSUB) - 1u;
+                if (cap < 0.0) sm = 0u;
+                if (STATS && cap >= 0.0) st_cnt[ST_SAMPLES] += NSUB;
             }
             PC_ADD(pc_l0);
-#pragma unroll
-            for (int q = 0; q < Q; ++q) {
-                unsigned any = __ballot_sync(FULL, sm[q] != 0u);
-                while (any) {
-                    const int wl = __ffs(any) - 1;
-                    any &= any - 1;
-                    unsigned wsub = __shfl_sync(FULL, sm[q], wl);
-                    const int i = (r * Q + q) * 32 + wl;
-                    // ---- wire i, lane = seed: sweep the candidate sub-blocks row by row ------------------
+            unsigned any = __ballot_sync(FULL, sm != 0u);
+            while (any) {
+                const int wl = __ffs(any) - 1;
+                any &= any - 1;
+                unsigned wsub = __shfl_sync(FULL, sm, wl);
+                const int i = r * 32 + wl;
+                // ---- wire i, lane = seed: sweep the open sub-blocks row by row --------------------------
 #ifdef COMET_FUSED_PROF
-                    pc_visits += 1;
+                pc_visits += 1;
 #endif
-                    EvalC w;
-                    w.e1x = __shfl_sync(FULL, ec[q].e1x, wl); w.e1y = __shfl_sync(FULL, ec[q].e1y, wl);
-                    w.e1z = __shfl_sync(FULL, ec[q].e1z, wl); w.c1 = __shfl_sync(FULL, ec[q].c1, wl);
-                    w.e2x = __shfl_sync(FULL, ec[q].e2x, wl); w.e2y = __shfl_sync(FULL, ec[q].e2y, wl);
-                    w.e2z = __shfl_sync(FULL, ec[q].e2z, wl); w.c2 = __shfl_sync(FULL, ec[q].c2, wl);
-                    double best = INF;
-                    int bk = -1;
-                    while (wsub) {
-                        const int j = __ffs(wsub) - 1;
-                        wsub &= wsub - 1;
+                EvalC w;
+                wconst_evalc(w, wtab, a.wt, W, i);          // broadcast
+                double best = INF;
+                int bk = -1;
+                while (wsub) {
+                    const int j = __ffs(wsub) - 1;
+                    wsub &= wsub - 1;
 #ifdef COMET_FUSED_PROF
-                        pc_sweeps += 1;
+                    pc_sweeps += 1;
 #endif
-                        const double* pr = tile + (j * FM1) * ROW + lane;
-                        if (STATS) { st_cnt[ST_ROWS_EXEC] += FM1; if (is_live) st_cnt[ST_ROWS_NEEDED] += FM1; }
+                    const double* pr = tile + (j * FM1) * ROW + lane;
+                    if (STATS) { st_cnt[ST_ROWS_EXEC] += FM1; if (is_live) st_cnt[ST_ROWS_NEEDED] += FM1; }
 #pragma unroll
-                        for (int kk = 0; kk < FM1; ++kk) {
-                            const double d2 = d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
-                            const int k = r0 + j * FM1 + kk;
-                            // rows at or past n_pts repeat the last state: not recorded, never taken
-                            if (d2 < best && k < np) { best = d2; bk = k; }
-                        }
+                    for (int kk = 0; kk < FM1; ++kk) {
+                        const double d2 = d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
+                        const int k = r0 + j * FM1 + kk;
+                        // rows at or past n_pts repeat the last state: not recorded, never taken
+                        if (d2 < best && k < np) { best = d2; bk = k; }
                     }
-                    if (bk >= 0) atomicMin(keys + (size_t)i * a.SP + s, pack_key(best, bk));
                 }
+                if (bk >= 0) atomicMin(keys + (size_t)i * a.SP + s, pack_key(best, bk));
             }
             PC_ADD(pc_l1);
         }
@@ -304,7 +316,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
         for (int j = 0; j < FB; ++j) {
             const int i = min(i0 + j, W - 1);
             kv[j] = __ldcg(keys + (size_t)i * a.SP + s);
-            const double cap = __ldg(a.wt + 14 * W + i);
+            const double cap = wconst(wtab, a.wt, W, 8, i);
             cap2[j] = cap * cap;
         }
 #pragma unroll
