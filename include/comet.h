@@ -49,6 +49,7 @@ typedef enum comet_status {
                                        *   the closest one, and (when neither dca nor kstar is requested) pairs
                                        *   whose residual is provably the cutoff; k*, D and rss are identical   */
 #define COMET_OPT_TIMING 3            /* 1: comet_dca_rss (pruned) times its kernels, see comet_read_timing      */
+#define COMET_OPT_LANES 4             /* 1..8 (default 6): sub-slabs comet_scan_rss runs concurrently on internal streams */
 #define COMET_OPT_STATS 2             /* 1: comet_dca_rss (pruned) adds its work counters, see comet_read_stats  */
 
 /* ---- context ---------------------------------------------------------------------------- */

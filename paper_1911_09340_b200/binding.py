@@ -26,6 +26,7 @@ COARSE_EXHAUSTIVE = 0
 COARSE_PRUNED = 1
 OPT_STATS = 2
 OPT_TIMING = 3
+OPT_LANES = 4
 STATS_FIELDS = ("samples", "rows_needed", "rows_executed", "fine_needed", "fine_executed", "pairs")
 
 

@@ -19,6 +19,10 @@
 #define COMET_PRUNED_WT 3
 #endif
 #define COMET_TEV_RING 64
+#define COMET_MAX_LANES 8
+#ifndef COMET_DEFAULT_LANES
+#define COMET_DEFAULT_LANES 6
+#endif
 #define COMET_PR_CAP_S 96      // sub-block samples staged in shared memory per chunk (72 KB)
 
 using namespace comet;
@@ -37,7 +41,12 @@ struct comet_ctx {
     int32_t* kb;
     double* e2;
     unsigned long long* items;   // [pair_cap / 32] work list of k_fine
-    unsigned int* n_items;
+    unsigned int* n_items;       // [COMET_MAX_LANES] (one counter per internal stream lane)
+    // comet_scan_rss runs the sub-slabs of a slab concurrently: scan kernels on ls[], the fine stage on
+    // the high-priority lf[] so that its CTAs take the slots retiring scan CTAs free
+    int opt_lanes;
+    cudaStream_t ls[COMET_MAX_LANES], lf[COMET_MAX_LANES];
+    cudaEvent_t ev_fork, ev_scan[COMET_MAX_LANES], ev_join[COMET_MAX_LANES];
     int fine_blocks;             // persistent grid of k_fine
     size_t pair_cap;             // pairs the two buffers hold
     size_t pair_max;             // growth limit (larger problems are processed in seed slabs)
@@ -116,7 +125,19 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int) * COMET_MAX_LANES);
+    ctx->opt_lanes = COMET_DEFAULT_LANES;
+    {
+        int prio_lo = 0, prio_hi = 0;
+        if (e == cudaSuccess) e = cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+        for (int l = 0; l < COMET_MAX_LANES && e == cudaSuccess; ++l) {
+            e = cudaStreamCreateWithPriority(&ctx->ls[l], cudaStreamNonBlocking, prio_lo);
+            if (e == cudaSuccess) e = cudaStreamCreateWithPriority(&ctx->lf[l], cudaStreamNonBlocking, prio_hi);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_scan[l], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_join[l], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming);
+    }
     if (e == cudaSuccess) {
         int per_sm = 0;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_fine<false>, COMET_FINE_THREADS, 0);
@@ -152,6 +173,13 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items);
     for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw);
+    for (int l = 0; l < COMET_MAX_LANES; ++l) {
+        if (ctx->ls[l]) cudaStreamDestroy(ctx->ls[l]);
+        if (ctx->lf[l]) cudaStreamDestroy(ctx->lf[l]);
+        if (ctx->ev_scan[l]) cudaEventDestroy(ctx->ev_scan[l]);
+        if (ctx->ev_join[l]) cudaEventDestroy(ctx->ev_join[l]);
+    }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
     delete ctx;
     return COMET_OK;
 }
@@ -167,6 +195,10 @@ extern "C" int comet_set_option(comet_ctx* ctx, int option, int value)
         ctx->opt_stats = value;
         return COMET_OK;
     }
+    if (option == COMET_OPT_LANES && value >= 1 && value <= COMET_MAX_LANES) {
+        ctx->opt_lanes = value;
+        return COMET_OK;
+    }
     if (option == COMET_OPT_TIMING && (value == 0 || value == 1)) {
         ctx->opt_timing = value;
         ctx->tev_count = 0;
@@ -180,6 +212,7 @@ extern "C" int comet_get_option(const comet_ctx* ctx, int option, int* value)
     if (!ctx || !value) return COMET_EINVAL;
     if (option == COMET_OPT_COARSE_SEARCH) { *value = ctx->opt_coarse; return COMET_OK; }
     if (option == COMET_OPT_STATS) { *value = ctx->opt_stats; return COMET_OK; }
+    if (option == COMET_OPT_LANES) { *value = ctx->opt_lanes; return COMET_OK; }
     if (option == COMET_OPT_TIMING) { *value = ctx->opt_timing; return COMET_OK; }
     return COMET_EINVAL;
 }
@@ -502,49 +535,79 @@ extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_
         if (rc) return rc;
         ctx->npw_cap = have / sizeof(int32_t);
     }
+    // A slab (what the workspace holds) is cut into up to opt_lanes sub-slabs that run concurrently on the
+    // ctx's internal streams: k_scan_fused of sub-slab l on ls[l], its fine stage on the high-priority
+    // lf[l], so that k_fine_ck of one sub-slab shares the SMs with k_scan_fused of the next ones (the two
+    // kernels leave different parts of the FP64 pipe idle).  The caller's stream forks into the lanes and
+    // joins them again with events: the call stays asynchronous and capturable.  Per-kernel timing
+    // (COMET_OPT_TIMING) and the work counters run one lane on the caller's stream.
+    const bool tm = ctx->opt_timing != 0;
+    const int lanes_opt = (tm || ctx->opt_stats) ? 1 : ctx->opt_lanes;
     for (int64_t c0 = 0; c0 < total_chunks; c0 += slab_chunks) {
-        const int64_t nc = (total_chunks - c0 < slab_chunks) ? (total_chunks - c0) : slab_chunks;
-        const int64_t s0 = c0 * COMET_LANES;
-        FusedArgs a;
-        a.seeds = seeds + s0;
-        a.stride = seed_stride;
-        a.n_seeds = (n_seeds - s0 < nc * COMET_LANES) ? (n_seeds - s0) : nc * COMET_LANES;
-        a.qkb = COMET_KAPPA * (double)charge * bz_tesla;
-        a.hk = make_stepk_host(step_cm);
-        a.n_steps = n_steps;
-        a.r_stop2 = r_stop_cm * r_stop_cm;
-        a.wt = ctx->wt;
-        a.W = n_fired;
-        a.hit_off = hit_off;
-        a.rho = rho;
-        a.lambda = cutoff_cm;
-        a.SP = nc * COMET_LANES;
-        a.n_ck = n_ck;
-        a.ck = ctx->ck;
-        a.bd = ctx->e2;
-        a.n_pts = n_pts ? n_pts + s0 : ctx->npw;
-        a.cw = ctx->cw;
-        a.items = ctx->items;
-        a.n_items = ctx->n_items;
-        a.stats = ctx->opt_stats ? ctx->stats : nullptr;
-        CU(ctx, cudaMemsetAsync(ctx->n_items, 0, sizeof(unsigned int), st));
-        const unsigned b1 = (unsigned)((nc + COMET_FUSED_WARPS - 1) / COMET_FUSED_WARPS);
-        const int64_t w2 = nc * (int64_t)n_fired;
-        const int64_t b2_all = (w2 + COMET_FINE_THREADS / 32 - 1) / (COMET_FINE_THREADS / 32);
-        unsigned b2 = (unsigned)(b2_all < ctx->fine_blocks ? b2_all : ctx->fine_blocks);
-        if (b2 < 1) b2 = 1;
-        const bool tm = ctx->opt_timing != 0;
-        cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
-        if (tm) CU(ctx, cudaEventRecord(tev[0], st));
-        const int thr = 32 * COMET_FUSED_WARPS;
-        if (a.stats) k_scan_fused<true><<<b1, thr, ctx->fused_smem, st>>>(a);
-        else k_scan_fused<false><<<b1, thr, ctx->fused_smem, st>>>(a);
-        if (tm) CU(ctx, cudaEventRecord(tev[1], st));
-        if (n_fired > 0) k_fine_ck<<<b2, COMET_FINE_THREADS, 0, st>>>(a);
-        if (tm) CU(ctx, cudaEventRecord(tev[2], st));
-        k_rss_sum<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, st>>>(a.bd, a.SP, n_fired, a.n_seeds, rss + s0);
-        if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }
-        CU(ctx, cudaGetLastError());
+        const int64_t nc_slab = (total_chunks - c0 < slab_chunks) ? (total_chunks - c0) : slab_chunks;
+        // sub-slabs of whole CTAs, at least two CTAs per SM each
+        const int64_t min_sub = (int64_t)COMET_FUSED_WARPS * ctx->n_sm * 2;
+        int lanes = lanes_opt;
+        while (lanes > 1 && nc_slab / lanes < min_sub) --lanes;
+        int64_t sub = (nc_slab + lanes - 1) / lanes;
+        sub = (sub + COMET_FUSED_WARPS - 1) / COMET_FUSED_WARPS * COMET_FUSED_WARPS;
+        if (lanes > 1) CU(ctx, cudaEventRecord(ctx->ev_fork, st));
+        int used = 0;
+        for (int l = 0; l < lanes; ++l) {
+            const int64_t cl = (int64_t)l * sub;             // first chunk of the sub-slab within the slab
+            if (cl >= nc_slab) break;
+            const int64_t nc = (nc_slab - cl < sub) ? (nc_slab - cl) : sub;
+            const int64_t s0 = (c0 + cl) * COMET_LANES;
+            cudaStream_t s_scan = lanes > 1 ? ctx->ls[l] : st, s_fine = lanes > 1 ? ctx->lf[l] : st;
+            FusedArgs a;
+            a.seeds = seeds + s0;
+            a.stride = seed_stride;
+            a.n_seeds = (n_seeds - s0 < nc * COMET_LANES) ? (n_seeds - s0) : nc * COMET_LANES;
+            a.qkb = COMET_KAPPA * (double)charge * bz_tesla;
+            a.hk = make_stepk_host(step_cm);
+            a.n_steps = n_steps;
+            a.r_stop2 = r_stop_cm * r_stop_cm;
+            a.wt = ctx->wt;
+            a.W = n_fired;
+            a.hit_off = hit_off;
+            a.rho = rho;
+            a.lambda = cutoff_cm;
+            a.SP = nc * COMET_LANES;
+            a.n_ck = n_ck;
+            a.ck = ctx->ck + (size_t)cl * (ck_chunk / sizeof(double));
+            a.bd = ctx->e2 + (size_t)cl * COMET_LANES * (size_t)n_fired;
+            a.n_pts = n_pts ? n_pts + s0 : ctx->npw + cl * COMET_LANES;
+            a.cw = ctx->cw + cl * COMET_LANES;
+            a.items = ctx->items + (size_t)cl * (size_t)n_fired;
+            a.n_items = ctx->n_items + l;
+            a.stats = ctx->opt_stats ? ctx->stats : nullptr;
+            if (lanes > 1) CU(ctx, cudaStreamWaitEvent(s_scan, ctx->ev_fork, 0));
+            CU(ctx, cudaMemsetAsync(a.n_items, 0, sizeof(unsigned int), s_scan));
+            const unsigned b1 = (unsigned)((nc + COMET_FUSED_WARPS - 1) / COMET_FUSED_WARPS);
+            const int64_t w2 = nc * (int64_t)n_fired;
+            const int64_t b2_all = (w2 + COMET_FINE_THREADS / 32 - 1) / (COMET_FINE_THREADS / 32);
+            unsigned b2 = (unsigned)(b2_all < ctx->fine_blocks ? b2_all : ctx->fine_blocks);
+            if (b2 < 1) b2 = 1;
+            cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
+            if (tm) CU(ctx, cudaEventRecord(tev[0], st));
+            const int thr = 32 * COMET_FUSED_WARPS;
+            if (a.stats) k_scan_fused<true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+            else k_scan_fused<false><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+            if (tm) CU(ctx, cudaEventRecord(tev[1], st));
+            if (lanes > 1) {
+                CU(ctx, cudaEventRecord(ctx->ev_scan[l], s_scan));
+                CU(ctx, cudaStreamWaitEvent(s_fine, ctx->ev_scan[l], 0));
+            }
+            if (n_fired > 0) k_fine_ck<<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
+            if (tm) CU(ctx, cudaEventRecord(tev[2], st));
+            k_rss_sum<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_fine>>>(a.bd, a.SP, n_fired, a.n_seeds, rss + s0);
+            if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }
+            if (lanes > 1) CU(ctx, cudaEventRecord(ctx->ev_join[l], s_fine));
+            CU(ctx, cudaGetLastError());
+            used = l + 1;
+        }
+        if (lanes > 1)
+            for (int l = 0; l < used; ++l) CU(ctx, cudaStreamWaitEvent(st, ctx->ev_join[l], 0));
     }
     return COMET_OK;
 }

@@ -280,6 +280,49 @@ def test_fused_high_occupancy_cutoffs_and_odd_steps(comet):
     assert np.array_equal(rss, ref["rss"])
 
 
+@pytest.mark.parametrize("lanes", [1, 3, 8])
+def test_fused_internal_stream_lanes(comet, cfg1_event, lanes):
+    """comet_scan_rss cuts a slab into sub-slabs on internal streams (COMET_OPT_LANES): same numbers."""
+    from paper_1911_09340_b200.binding import OPT_LANES
+    ev = cfg1_event
+    seeds, _ = event_seeds(ev)
+    seeds = np.ascontiguousarray(seeds[:, :3 * 4 * 148 * 32 + 77])      # several sub-slabs and a ragged tail
+    d = DevEvent(ev, seeds)
+    old = comet.get_option(OPT_LANES)
+    try:
+        comet.set_option(OPT_LANES, lanes)
+        rss, n_pts = _run_fused(comet, d)
+        rss2, _ = _run_fused(comet, d)                                  # back to back on the same workspace
+    finally:
+        comet.set_option(OPT_LANES, old)
+    sample = np.arange(0, seeds.shape[1], 37)
+    ref = _oracle_scan(ev, np.ascontiguousarray(seeds[:, sample]), want_npts=True)
+    np.testing.assert_array_equal(n_pts[sample], ref["n_pts"])
+    assert np.array_equal(rss[sample], ref["rss"])
+    assert np.array_equal(rss, rss2)
+    comet.set_option(OPT_LANES, 1)
+    try:
+        rss1, _ = _run_fused(comet, d)
+    finally:
+        comet.set_option(OPT_LANES, old)
+    assert np.array_equal(rss, rss1)
+
+
+def test_fused_unrelated_seeds_in_a_chunk(comet, cfg1_event):
+    """The sub-block test bounds a chunk's seeds by a representative one: shuffled seeds (a chunk then
+    mixes partitions and far-apart grid points) only lose pruning, never correctness."""
+    ev = cfg1_event
+    seeds, _ = event_seeds(ev)
+    rng = np.random.default_rng(5)
+    pick = rng.permutation(seeds.shape[1])[:2048 + 13]
+    seeds = np.ascontiguousarray(seeds[:, pick])
+    d = DevEvent(ev, seeds)
+    rss, n_pts = _run_fused(comet, d)
+    ref = _oracle_scan(ev, seeds, want_npts=True)
+    np.testing.assert_array_equal(n_pts, ref["n_pts"])
+    assert np.array_equal(rss, ref["rss"])
+
+
 def test_fused_no_wires(comet, cfg0_event):
     ev = cfg0_event
     seeds, _ = event_seeds(ev, shape=(2, 2, 2, 5))
