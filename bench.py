@@ -40,8 +40,8 @@ FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # FP64-pipe instructions per recorded state in kernel A: the RKN4 step of reading R1 is 48 IEEE operations
 # (44 issued: the two exact doublings ride on FMAs) + 4 for the target-region test of R3
 GEN_INSTR = 48
-# dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1c_*, ncu --set full)
-TRAFFIC_BYTES = {}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1c_full_scan_fused_fine_ck.txt)
+TRAFFIC_BYTES = {"k_scan_fused": 318474496 + 2222977000, "k_fine_ck": 680873984 + 80947000}
 
 
 def _event(cfg):
@@ -187,7 +187,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_1911_09340_b200 import Comet
-    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH, OPT_STATS, OPT_TIMING
+    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH, OPT_LANES, OPT_STATS, OPT_TIMING
     from paper_1911_09340_b200.build import build
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -214,8 +214,14 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     track = None
 
+    call_events = []                     # CUDA events on the stream around the A + B call of every timed step
+
     def step_fused():
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
         c.scan_rss(d_seeds, *phys, ev.r_stop, *hits, ev.cutoff, rss=rss, n_pts=n_pts)
+        e1.record(stream)
+        call_events.append((e0, e1))
         return c.select_and_classify(d_seeds, *phys, ev.r_stop, *hits, ev.cutoff, rss, part_off)
 
     def step_mat():
@@ -234,14 +240,19 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     sampler = ClockSampler(local) if rank == 0 else None
-    c.set_option(OPT_TIMING, 1)          # the library brackets its kernels with CUDA events on its stream
     torch.cuda.synchronize()
+    del call_events[:]
     ms_per_step, out = _time_steps(step, args.steps, stream)
-    ktimes = c.read_timing(knames)       # mean over the last <= 64 timed steps
-    c.set_option(OPT_TIMING, 0)
     if world > 1:
         dist.barrier()
     clocks = sampler.stop() if sampler else None
+    ms_call = float(np.mean([a.elapsed_time(b) for a, b in call_events])) if call_events else None
+    # per-kernel device times: the library brackets its kernels with CUDA events; with this option
+    # comet_scan_rss runs its sub-slabs one after the other on the caller's stream (kernels in isolation)
+    c.set_option(OPT_TIMING, 1)
+    _time_steps(step, min(args.steps, 32), stream)
+    ktimes = c.read_timing(knames)
+    c.set_option(OPT_TIMING, 0)
     if world > 1:
         t = torch.tensor([ms_per_step], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -330,7 +341,8 @@ def run_ours(args):
     gen = GEN_INSTR * n_states if fused else 0.0
     fl = {knames[0]: 2.0 * (gen + SHORTLIST_INSTR * ev_needed), knames[1]: 2.0 * FINE_INSTR * stats["fine_needed"]}
     fl_exec = {knames[0]: 2.0 * (gen + SHORTLIST_INSTR * ev_exec), knames[1]: 2.0 * FINE_INSTR * stats["fine_executed"]}
-    kernels = {"timed_over": "last %d steps of the timed region (CUDA events recorded by the library on its stream)" % ktimes["n_calls"]}
+    kernels = {"timed_over": "%d steps after the timed region with COMET_OPT_TIMING (CUDA events recorded by the library "
+                             "on its stream; kernels run one after the other)" % ktimes["n_calls"]}
     kernels.update({k: {"ms_per_launch": ktimes[k], "achieved": fl[k] / (ktimes[k] * 1e-3) / 1e12,
                         "frac": fl[k] / (ktimes[k] * 1e-3) / 1e12 / peak,
                         "achieved_executed": fl_exec[k] / (ktimes[k] * 1e-3) / 1e12,
@@ -338,11 +350,31 @@ def run_ours(args):
     kernels["k_rss_sum"] = {"ms_per_launch": ktimes["k_rss_sum"], "bound": "hbm",
                             "achieved_gbs": (pairs * 8 + S * 8) / (ktimes["k_rss_sum"] * 1e-3) / 1e9}
     kernel = max(fl, key=lambda k: ktimes[k])
+    if fused and ms_call is not None:
+        # the timed region runs k_scan_fused and k_fine_ck of different sub-slabs concurrently: the roofline entry
+        # is the A + B call as launched there (both kernels' algorithmic work over the call's device time)
+        lanes = c.get_option(OPT_LANES)
+        top = {"kernel": "k_scan_fused + k_fine_ck (comet_scan_rss: sub-slabs on %d internal streams)" % lanes,
+               "achieved": (fl[knames[0]] + fl[knames[1]]) / (ms_call * 1e-3) / 1e12, "ms_per_launch": ms_call,
+               "timed": "CUDA events on the caller's stream around every comet_scan_rss of the timed region"}
+    else:
+        top = {"kernel": kernel, "achieved": kernels[kernel]["achieved"], "ms_per_launch": ktimes[kernel],
+               "timed": kernels["timed_over"]}
     model = ("FP64-pipe slots x 2 of the work the path needs (thread-level counters, comet_read_stats): "
              + ("%d per recorded state (RKN4 step + target-region test, Alg. 1), " % GEN_INSTR if fused else "")
              + "%d per shortlist evaluation (sub-block sample or swept row); %s: %d per (seed, wire) pair that runs "
                "the virtual-plane iteration" % (SHORTLIST_INSTR, knames[1], FINE_INSTR))
     flops_exh = 2.0 * (SHORTLIST_INSTR * n_states * W + FINE_INSTR * pairs)
+    if fused:
+        # k_wire_prep, then k_scan_fused + k_fine_ck + k_rss_sum per sub-slab (the library's rule: up to
+        # COMET_OPT_LANES sub-slabs of at least 2 CTAs of 4 chunks per SM), then k_wire_prep, k_argmin_stage1, k_select_classify
+        n_sub, chunks = c.get_option(OPT_LANES), (S + 31) // 32
+        n_sm = torch.cuda.get_device_properties(local).multi_processor_count
+        while n_sub > 1 and chunks // n_sub < 4 * n_sm * 2:
+            n_sub -= 1
+        launches_per_step = 1 + 3 * n_sub + 3
+    else:
+        launches_per_step = 8
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -360,14 +392,15 @@ def run_ours(args):
         "e2e": {"value": world * pairs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "ms_per_step": e2e_s * 1e3,
                 "api": "comet_scan_event_host, pinned host buffers" + ("" if fused else ", %d GiB track slab" % (budget >> 30))},
-        "gpu_launches": (7 if fused else 8) * args.steps,
+        "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
-        "roofline": {"kernel": kernel, "bound": "alu", "achieved": kernels[kernel]["achieved"], "peak": peak,
-                     "unit": "TFLOP/s", "frac": kernels[kernel]["frac"], "traffic": TRAFFIC_BYTES.get(kernel),
+        "roofline": {"kernel": top["kernel"], "bound": "alu", "achieved": top["achieved"], "peak": peak,
+                     "unit": "TFLOP/s", "frac": top["achieved"] / peak, "traffic": TRAFFIC_BYTES.get(kernel),
+                     "timed": top["timed"],
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 figure)",
                      "peak_measured_dfma_probe": peak_measured,
-                     "frac_of_measured": kernels[kernel]["achieved"] / peak_measured,
-                     "ms_per_launch": ktimes[kernel], "share_of_step": ktimes[kernel] / ms_per_step,
+                     "frac_of_measured": top["achieved"] / peak_measured,
+                     "ms_per_launch": top["ms_per_launch"], "share_of_step": top["ms_per_launch"] / ms_per_step,
                      "model": model, "kernels": kernels, "work_counters": stats,
                      "other_path": {"path": "materialised" if fused else "fused", "ms_per_step": ms_other,
                                     "rss_bit_identical": paths_agree},
