@@ -152,10 +152,18 @@ int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64
  * checkpoint workspace from which the virtual-plane iteration restarts.
  * Arguments as in the two calls above;
  *   n_pts   dev [n_seeds], written; NULL to skip.
- * Workspace (pair buffers and checkpoints, 12 bytes per recorded state + 12 per (seed, wire) pair)
- * lives in the ctx and grows on the first call that needs it (that call synchronises the device);
- * larger problems are processed in seed slabs bounded by comet_reserve's pair limit and by 8 GiB of
- * checkpoints.  COMET_OPT_TIMING applies (k_scan_fused, k_fine_ck, k_rss_sum). */
+ * Workspace (checkpoints: 12 bytes per recorded state of capacity; 8 bytes per (seed, wire) pair;
+ * 8 bytes per seed) lives in the ctx and grows on the first call that needs it (that call
+ * synchronises the device); larger problems are processed in seed slabs bounded by comet_reserve's
+ * pair limit and by 8 GiB of checkpoints.  A slab is cut into up to COMET_OPT_LANES sub-slabs that
+ * run concurrently on streams owned by the ctx; `cuda_stream` forks into them and joins them again
+ * with events, so the call is asynchronous with respect to the host and ordered on `cuda_stream`
+ * like any other work (and can be captured into a CUDA graph).  COMET_OPT_TIMING (k_scan_fused,
+ * k_fine_ck, k_rss_sum) and COMET_OPT_STATS run the sub-slabs one after the other on `cuda_stream`.
+ * With COMET_OPT_STATS the counters of comet_read_stats mean: [0] sub-block samples evaluated
+ * (one per wire, sub-block and chunk), [1] rows swept for a lane whose tile holds recorded states,
+ * [2] rows swept, [3] pairs that needed the virtual-plane iteration, [4] 32 x (chunk, wire) items
+ * for which a warp executed it, [5] all pairs. */
 int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
                    int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                    const double* wire_a, const double* wire_b, int32_t n_wires,
