@@ -358,3 +358,98 @@ void oracle_rkn4_step(double* state6, double h, double c)
 }
 
 double oracle_kappa(void) { return ORACLE_KAPPA; }
+
+/* ------------------------------------------------------------------------------------------
+ * Iterative seed refinement (readings R24-R27 of DESIGN.md).
+ *
+ * "several seeds with the lowest RSS are selected as reference points for the next seed
+ * scanning, where new seeds are fetched in their vicinity and with a finer granularity. [...]
+ * the selected seeds are ensured to be sparse enough to avoid overlaps between new seed sets
+ * from each reference point."
+ *
+ * The scanned seed components are the paper's (z, p_x, p_y, p_z) at fixed (x, y), i.e. fixed
+ * azimuth on the R = 50 cm cylinder: dimension d = 0..3 is seed component 2 + d.
+ * The new seed set of a reference point is the box ref_d +- half_width_d; two boxes overlap iff
+ * |ref_a,d - ref_b,d| < 2 half_width_d in every dimension (strict).
+ * ------------------------------------------------------------------------------------------ */
+
+/* 1 iff the refinement boxes around seeds a and b overlap (R25). */
+static int boxes_overlap(const double* seeds, int64_t n_seeds, int64_t a, int64_t b, const double* half_width)
+{
+    int d;
+    for (d = 0; d < 4; ++d) {
+        const double* comp = seeds + (size_t)(2 + d) * (size_t)n_seeds;
+        const double two_hw = 2.0 * half_width[d];
+        if (!(fabs(comp[a] - comp[b]) < two_hw)) return 0;
+    }
+    return 1;
+}
+
+/* O12: per partition, up to k_ref reference points: repeatedly the seed of lowest RSS (ties ->
+ * lowest index; NaN never) among those that are not selected yet and whose box overlaps no
+ * selected box.  ref_seed [n_part][k_ref], -1 where no seed is left. */
+void oracle_select_references(const double* seeds, int64_t n_seeds, const double* rss,
+                              const int64_t* part_off, int n_part, const double* half_width,
+                              int k_ref, int64_t* ref_seed)
+{
+    int p, r, q;
+    for (p = 0; p < n_part; ++p) {
+        int64_t* sel = ref_seed + (size_t)p * (size_t)k_ref;
+        for (r = 0; r < k_ref; ++r) sel[r] = -1;
+        for (r = 0; r < k_ref; ++r) {
+            int64_t s, best = -1;
+            for (s = part_off[p]; s < part_off[p + 1]; ++s) {
+                int blocked = 0;
+                if (rss[s] != rss[s]) continue;
+                for (q = 0; q < r && !blocked; ++q)
+                    if (sel[q] == s || boxes_overlap(seeds, n_seeds, s, sel[q], half_width)) blocked = 1;
+                if (blocked) continue;
+                if (best < 0 || rss[s] < rss[best]) best = s;
+            }
+            if (best < 0) break;
+            sel[r] = best;
+        }
+    }
+}
+
+/* O13: the new seed set.  Slot (p, r) holds G = n_grid[0] n_grid[1] n_grid[2] n_grid[3] seeds
+ * around reference ref_seed[p][r] (an empty slot repeats the partition's first reference, R27):
+ * component 2 + d takes the n_grid[d] values lo + j step, lo = ref_d - half_width_d,
+ * step = (2 half_width_d) / (n_grid[d] - 1)   (n_grid[d] = 1: the reference's own value);
+ * (x, y) are the reference's.  Seed index within the slot: ((j0 n1 + j1) n2 + j2) n3 + j3.
+ * new_seeds is SoA [6][n_part k_ref G]. */
+void oracle_refine_seeds(const double* seeds, int64_t n_seeds, const int64_t* ref_seed, int n_part,
+                         int k_ref, const double* half_width, const int32_t* n_grid,
+                         double* new_seeds)
+{
+    const int64_t G = (int64_t)n_grid[0] * n_grid[1] * n_grid[2] * n_grid[3];
+    const int64_t S_new = (int64_t)n_part * k_ref * G;
+    int p, r, d;
+    for (p = 0; p < n_part; ++p) {
+        for (r = 0; r < k_ref; ++r) {
+            int64_t ref = ref_seed[(size_t)p * k_ref + r];
+            int64_t g, base = ((int64_t)p * k_ref + r) * G;
+            double lo[4], stp[4];
+            if (ref < 0) ref = ref_seed[(size_t)p * k_ref];
+            for (d = 0; d < 4; ++d) {
+                const double v = seeds[(size_t)(2 + d) * (size_t)n_seeds + ref];
+                if (n_grid[d] > 1) {
+                    lo[d] = v - half_width[d];
+                    stp[d] = (2.0 * half_width[d]) / (double)(n_grid[d] - 1);
+                } else {
+                    lo[d] = v;
+                    stp[d] = 0.0;
+                }
+            }
+            for (g = 0; g < G; ++g) {
+                int64_t rem = g;
+                int j[4];
+                for (d = 3; d >= 0; --d) { j[d] = (int)(rem % n_grid[d]); rem /= n_grid[d]; }
+                new_seeds[0 * S_new + base + g] = seeds[0 * (size_t)n_seeds + ref];
+                new_seeds[1 * S_new + base + g] = seeds[1 * (size_t)n_seeds + ref];
+                for (d = 0; d < 4; ++d)
+                    new_seeds[(size_t)(2 + d) * S_new + base + g] = lo[d] + (double)j[d] * stp[d];
+            }
+        }
+    }
+}

@@ -46,6 +46,8 @@ def lib():
         L.oracle_select_classify.argtypes = [_F64, c_i64, c_int, c_dbl, c_dbl, c_int, c_dbl,
                                              _F64, _F64, c_int, _I32, _I32, _F64, c_int, c_int, c_dbl,
                                              _F64, _I64, c_int, _I64, _F64, _F64, _U8]
+        L.oracle_select_references.argtypes = [_F64, c_i64, _F64, _I64, c_int, _F64, c_int, _I64]
+        L.oracle_refine_seeds.argtypes = [_F64, c_i64, _I64, c_int, c_int, _F64, _I32, _F64]
         _lib = L
     return _lib
 
@@ -124,3 +126,74 @@ def select_classify(seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fi
                                  rho, W, H, float(cutoff), rss, part_off, P,
                                  best_seed, best_rss, best_dca, cls)
     return {"best_seed": best_seed, "best_rss": best_rss, "best_dca": best_dca, "cls": cls}
+
+
+def select_references(seeds, rss, part_off, half_width, k_ref):
+    """O12: sparse lowest-RSS reference points -> int64 [P][k_ref], -1 = none."""
+    seeds, rss, part_off = _c(seeds, np.float64), _c(rss, np.float64), _c(part_off, np.int64)
+    hw = _c(half_width, np.float64)
+    P = part_off.shape[0] - 1
+    ref = np.empty((P, int(k_ref)), dtype=np.int64)
+    lib().oracle_select_references(seeds, seeds.shape[1], rss, part_off, P, hw, int(k_ref), ref)
+    return ref
+
+
+def refine_seeds(seeds, ref_seed, half_width, n_grid):
+    """O13: the finer seed set around every reference -> (seeds [6][P k G], part_off)."""
+    seeds, ref_seed = _c(seeds, np.float64), _c(ref_seed, np.int64)
+    hw, ng = _c(half_width, np.float64), _c(n_grid, np.int32)
+    P, K = ref_seed.shape
+    G = int(np.prod(ng.astype(np.int64)))
+    new = np.empty((6, P * K * G))
+    lib().oracle_refine_seeds(seeds, seeds.shape[1], ref_seed, P, K, hw, ng, new)
+    return new, np.arange(P + 1, dtype=np.int64) * (K * G)
+
+
+def classify_seeds(seeds, idx, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
+                   cutoff):
+    """O11 for the listed seeds -> dict(dca [n][W], cls [n][H]); idx < 0 -> NaN / zeros.
+    Each listed seed is scored as a partition of its own by select_classify."""
+    seeds = _c(seeds, np.float64)
+    idx = np.asarray(idx, dtype=np.int64).ravel()
+    W, H = len(fired_wire), len(rho)
+    dca = np.full((idx.size, W), np.nan)
+    cls = np.zeros((idx.size, H), dtype=np.uint8)
+    ok = np.flatnonzero(idx >= 0)
+    if ok.size:
+        sub = np.ascontiguousarray(seeds[:, idx[ok]])
+        r = select_classify(sub, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
+                            cutoff, np.zeros(ok.size), np.arange(ok.size + 1, dtype=np.int64))
+        dca[ok], cls[ok] = r["best_dca"], r["cls"]
+    return {"dca": dca, "cls": cls}
+
+
+def scan_stage(seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
+               cutoff, half_width, n_grid, n_iter, shrink, k_ref, k_final):
+    """One *stage* (the seed scanning of a turn, several *iterations*), every turn
+    partition at once (R14).  Iteration 0 scans the given seeds; each of the n_iter further iterations
+    picks k_ref sparse reference points (box half_width), scans the finer sets around them, and
+    multiplies half_width by `shrink`.  The k_final finally selected seeds ("finally
+    selected 10 seeds") are picked by the same rule with the last half_width and classified.
+    -> dict(final_seed [P][k_final][6] (NaN = none), final_rss, final_dca, cls, history)."""
+    seeds = _c(seeds, np.float64)
+    part_off = _c(part_off, np.int64)
+    hw = np.array(half_width, dtype=np.float64)
+    args = (charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho, cutoff)
+    history = []
+    rss = scan(seeds, *args)["rss"]
+    for _ in range(int(n_iter)):
+        ref = select_references(seeds, rss, part_off, hw, k_ref)
+        history.append({"ref_rss": np.where(ref >= 0, rss[np.maximum(ref, 0)], np.nan), "half_width": hw.copy()})
+        seeds, part_off = refine_seeds(seeds, ref, hw, n_grid)
+        rss = scan(seeds, *args)["rss"]
+        hw = hw * float(shrink)
+    fin = select_references(seeds, rss, part_off, hw, k_final)
+    P = fin.shape[0]
+    final_seed = np.full((P, int(k_final), 6), np.nan)
+    ok = fin >= 0
+    final_seed[ok] = seeds[:, fin[ok]].T
+    final_rss = np.where(ok, rss[np.maximum(fin, 0)], np.nan)
+    c = classify_seeds(seeds, fin, *args)
+    W, H = len(fired_wire), len(rho)
+    return {"final_seed": final_seed, "final_rss": final_rss, "final_dca": c["dca"].reshape(P, int(k_final), W),
+            "cls": c["cls"].reshape(P, int(k_final), H), "history": history}
