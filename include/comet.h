@@ -191,6 +191,76 @@ int comet_select_and_classify(comet_ctx* ctx, const double* seeds, int64_t seed_
                               int64_t* best_seed, double* best_rss, double* best_dca, uint8_t* cls,
                               void* cuda_stream);
 
+/* ---- iterative seed refinement (readings R24-R28 of DESIGN.md) ------ */
+
+#define COMET_MAX_REFS 64             /* limit of k_ref and k_final */
+
+/* "several seeds with the lowest RSS are selected as reference points for the next seed scanning
+ * [...] sparse enough to avoid overlaps between new seed sets from each reference point"
+ * (PAPER.md:81).  The refined components are (z, p_x, p_y, p_z) = seed components 2..5 at the
+ * reference's (x, y) (R24).  Per partition p, ref_seed[p][0..k_ref) are taken one by
+ * one: the seed of lowest rss (ties -> lowest index, NaN never) that is not selected yet and whose
+ * box ref_d +- half_width[d] overlaps no selected box; two boxes overlap iff
+ * |ref_a,d - ref_b,d| < 2 half_width[d] in every dimension d (R25).  -1 where no seed is left.
+ *   rss         dev [n_seeds];  part_off  HOST [n_part+1];  half_width  HOST [4], >= 0
+ *   ref_seed    dev [n_part][k_ref], written (global seed indices) */
+int comet_select_references(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                            const double* rss, const int64_t* part_off, int32_t n_part,
+                            const double* half_width, int32_t k_ref, int64_t* ref_seed,
+                            void* cuda_stream);
+
+/* "new seeds are fetched in their vicinity and with a finer granularity": slot
+ * (p, r) of new_seeds holds G = n_grid[0] n_grid[1] n_grid[2] n_grid[3] seeds around reference
+ * ref_seed[p][r] (an empty slot repeats ref_seed[p][0], R27): component 2+d takes the values
+ * (ref_d - half_width[d]) + j (2 half_width[d] / (n_grid[d] - 1)), j = 0..n_grid[d]-1 (the
+ * reference's own value when n_grid[d] = 1), (x, y) are the reference's; the seed of (j0..j3) is at
+ * index ((j0 n1 + j1) n2 + j2) n3 + j3 of the slot, slot (p, r) starts at (p k_ref + r) G (R26).
+ *   new_seeds   dev SoA [6][new_stride], new_stride >= n_part k_ref G, written
+ *   n_grid      HOST [4], each 1..4096 */
+int comet_refine_seeds(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                       const int64_t* ref_seed, int32_t n_part, int32_t k_ref,
+                       const double* half_width, const int32_t* n_grid,
+                       double* new_seeds, int64_t new_stride, void* cuda_stream);
+
+/* The classification rule of PAPER.md:83 (as in comet_select_and_classify) for the listed seeds:
+ * dca[n][i] = signed D of seed seed_idx[n] on fired wire i, cls[n][j] = 1 for the classified hit
+ * entries.  seed_idx[n] < 0 gives NaN / zeros.
+ *   seed_idx  dev [n_sel];  dca  dev [n_sel][n_fired];  cls  dev [n_sel][n_hits] */
+int comet_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                         int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                         double r_stop_cm,
+                         const double* wire_a, const double* wire_b, int32_t n_wires,
+                         const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                         int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                         const int64_t* seed_idx, int32_t n_sel, double* dca, uint8_t* cls,
+                         void* cuda_stream);
+
+/* Bytes of the device work buffer of comet_scan_stage (0 for invalid arguments). */
+size_t comet_stage_work_bytes(int64_t n_seeds, int32_t n_part, int32_t k_ref, int32_t k_final,
+                              const int32_t* n_grid);
+
+/* One *stage* (the seed scanning of a turn, several *iterations*) for all turn
+ * partitions at once, entirely on the device (the paper crosses the PCIe bus four times per
+ * iteration).  Iteration 0: comet_scan_rss of the given seeds.  Each
+ * of the n_iter further iterations: comet_select_references (k_ref, half_width), comet_refine_seeds,
+ * comet_scan_rss of the new set, half_width *= shrink.  Then the k_final finally selected seeds
+ * by the same rule with the last half_width, each classified (R28):
+ *   final_seed  dev [n_part][k_final][6] (x,y,z,px,py,pz; NaN where none), final_rss dev [n_part][k_final],
+ *   final_dca   dev [n_part][k_final][n_fired], cls dev [n_part][k_final][n_hits]
+ *   part_off    HOST [n_part+1], part_off[0] = 0, part_off[n_part] = n_seeds, no empty partition
+ *   work        dev, comet_stage_work_bytes(...) bytes
+ * Only enqueues work on cuda_stream (plus the ctx's internal streams, see comet_scan_rss). */
+int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                     int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                     const double* wire_a, const double* wire_b, int32_t n_wires,
+                     const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                     int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                     const int64_t* part_off, int32_t n_part,
+                     const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                     int32_t k_ref, int32_t k_final, void* work,
+                     double* final_seed, double* final_rss, double* final_dca, uint8_t* cls,
+                     void* cuda_stream);
+
 /* ---- whole event from host buffers ------------------------------------------------------- */
 
 /* Runs A, B and C for one event whose inputs and outputs live in HOST memory (pinned memory makes

@@ -18,6 +18,8 @@ EXPORTED_SYMBOLS = [
     "comet_set_option", "comet_get_option", "comet_track_bytes", "comet_seed_extrapolate",
     "comet_track_export", "comet_dca_rss", "comet_select_and_classify", "comet_scan_event_host",
     "comet_fp64_peak_probe", "comet_read_stats", "comet_reserve", "comet_read_timing", "comet_scan_rss",
+    "comet_select_references", "comet_refine_seeds", "comet_classify_seeds", "comet_stage_work_bytes",
+    "comet_scan_stage",
 ]
 
 COMET_CHUNK = 32
@@ -77,8 +79,17 @@ def load_library():
     L.comet_reserve.argtypes = [vp, i64]
     L.comet_read_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32, ctypes.POINTER(i32)]
     L.comet_read_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), i32, i32, vp]
+    L.comet_select_references.argtypes = [vp, vp, i64, i64, vp, vp, i32, vp, i32, vp, vp]
+    L.comet_refine_seeds.argtypes = [vp, vp, i64, i64, vp, i32, i32, vp, vp, vp, i64, vp]
+    L.comet_classify_seeds.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
+                                       vp, vp, i32, vp, vp, vp, i32, i32, dbl, vp, i32, vp, vp, vp]
+    L.comet_stage_work_bytes.argtypes = [i64, i32, i32, i32, vp]
+    L.comet_stage_work_bytes.restype = sz
+    L.comet_scan_stage.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
+                                   vp, vp, i32, vp, vp, vp, i32, i32, dbl,
+                                   vp, i32, vp, vp, i32, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
-        if name not in ("comet_status_string", "comet_track_bytes"):
+        if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes"):
             getattr(L, name).restype = ctypes.c_int
     _lib = L
     return L
@@ -266,6 +277,81 @@ class Comet:
             int(best_seed.data_ptr()), int(best_rss.data_ptr()), int(best_dca.data_ptr()), int(cls.data_ptr()),
             _stream_ptr(stream)))
         return {"best_seed": best_seed, "best_rss": best_rss, "best_dca": best_dca, "cls": cls}
+
+    # -- iterative seed refinement ------------------------------------------------------------
+    def select_references(self, seeds, rss, part_off, half_width, k_ref, stream=None):
+        """comet_select_references -> int64 [P][k_ref] (device), -1 = none."""
+        S = seeds.shape[1]
+        po = np.ascontiguousarray(np.asarray(part_off, dtype=np.int64))
+        hw = np.ascontiguousarray(np.asarray(half_width, dtype=np.float64))
+        P, d = po.shape[0] - 1, self.device
+        ref = torch.empty((P, int(k_ref)), dtype=torch.int64, device=self._tdev())
+        self._check(self._L.comet_select_references(
+            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, _dev(rss, torch.float64, "rss", d),
+            po.ctypes.data, P, hw.ctypes.data, int(k_ref), int(ref.data_ptr()), _stream_ptr(stream)))
+        return ref
+
+    def refine_seeds(self, seeds, ref_seed, half_width, n_grid, stream=None):
+        """comet_refine_seeds -> (new seeds [6][P k G] (device), part_off of the new set)."""
+        S = seeds.shape[1]
+        hw = np.ascontiguousarray(np.asarray(half_width, dtype=np.float64))
+        ng = np.ascontiguousarray(np.asarray(n_grid, dtype=np.int32))
+        P, K = int(ref_seed.shape[0]), int(ref_seed.shape[1])
+        G, d = int(np.prod(ng.astype(np.int64))), self.device
+        new = torch.empty((6, P * K * G), dtype=torch.float64, device=self._tdev())
+        self._check(self._L.comet_refine_seeds(
+            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, _dev(ref_seed, torch.int64, "ref_seed", d), P, K,
+            hw.ctypes.data, ng.ctypes.data, int(new.data_ptr()), P * K * G, _stream_ptr(stream)))
+        return new, np.arange(P + 1, dtype=np.int64) * (K * G)
+
+    def classify_seeds(self, seeds, seed_idx, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
+                       hit_off, rho, cutoff, stream=None):
+        S, n = seeds.shape[1], int(seed_idx.numel())
+        W, H, d, td = int(fired_wire.shape[0]), int(rho.shape[0]), self.device, self._tdev()
+        dca = torch.empty((n, W), dtype=torch.float64, device=td)
+        cls = torch.empty((n, H), dtype=torch.uint8, device=td)
+        self._check(self._L.comet_classify_seeds(
+            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, int(charge), float(bz), float(step),
+            int(n_steps), float(r_stop),
+            _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
+            int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d),
+            _dev(hit_off, torch.int32, "hit_off", d), _dev(rho, torch.float64, "rho", d), W, H, float(cutoff),
+            _dev(seed_idx, torch.int64, "seed_idx", d), n, int(dca.data_ptr()), int(cls.data_ptr()),
+            _stream_ptr(stream)))
+        return {"dca": dca, "cls": cls}
+
+    def stage_work_bytes(self, n_seeds, n_part, k_ref, k_final, n_grid) -> int:
+        ng = np.ascontiguousarray(np.asarray(n_grid, dtype=np.int32))
+        return int(self._L.comet_stage_work_bytes(int(n_seeds), int(n_part), int(k_ref), int(k_final), ng.ctypes.data))
+
+    def scan_stage(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off,
+                   rho, cutoff, half_width, n_grid, n_iter, shrink, k_ref, k_final, work=None, stream=None):
+        """comet_scan_stage: a whole stage (scan, n_iter refinements, final selection, classification)."""
+        S = seeds.shape[1]
+        po = np.ascontiguousarray(np.asarray(part_off, dtype=np.int64))
+        hw = np.ascontiguousarray(np.asarray(half_width, dtype=np.float64))
+        ng = np.ascontiguousarray(np.asarray(n_grid, dtype=np.int32))
+        P, W, H = po.shape[0] - 1, int(fired_wire.shape[0]), int(rho.shape[0])
+        d, td = self.device, self._tdev()
+        if work is None:
+            nb = self.stage_work_bytes(S, P, k_ref, k_final, ng)
+            if nb == 0:
+                raise CometError("comet_stage_work_bytes: invalid arguments")
+            work = torch.empty(nb, dtype=torch.uint8, device=td)
+        out = {"final_seed": torch.empty((P, int(k_final), 6), dtype=torch.float64, device=td),
+               "final_rss": torch.empty((P, int(k_final)), dtype=torch.float64, device=td),
+               "final_dca": torch.empty((P, int(k_final), W), dtype=torch.float64, device=td),
+               "cls": torch.empty((P, int(k_final), H), dtype=torch.uint8, device=td), "work": work}
+        self._check(self._L.comet_scan_stage(
+            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, int(charge), float(bz), float(step),
+            int(n_steps), float(r_stop),
+            _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
+            int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d),
+            _dev(hit_off, torch.int32, "hit_off", d), _dev(rho, torch.float64, "rho", d), W, H, float(cutoff),
+            po.ctypes.data, P, hw.ctypes.data, ng.ctypes.data, int(n_iter), float(shrink), int(k_ref), int(k_final),
+            int(work.data_ptr()), int(out["final_seed"].data_ptr()), int(out["final_rss"].data_ptr()),
+            int(out["final_dca"].data_ptr()), int(out["cls"].data_ptr()), _stream_ptr(stream)))
+        return out
 
     # -- whole event, device-resident inputs --------------------------------------------------
     def scan_event(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,

@@ -14,6 +14,7 @@
 #include "extrapolate.cuh"
 #include "select.cuh"
 #include "scan_fused.cuh"
+#include "refine.cuh"
 
 #ifndef COMET_PRUNED_WT
 #define COMET_PRUNED_WT 3
@@ -155,6 +156,9 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_select_classify, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_classify_seeds, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
     if (e != cudaSuccess) {
         cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats); cudaFree(ctx->n_items);
@@ -666,6 +670,222 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     k_select_classify<<<n_part, 256, smem, st>>>(a);
     CU(ctx, cudaGetLastError());
     return COMET_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// iterative seed refinement (readings R24-R28)
+// ---------------------------------------------------------------------------------------------
+static int fill_partoff(PartOff* po, const int64_t* part_off, int32_t n_part, int64_t n_seeds, bool non_empty)
+{
+    memset(po, 0, sizeof(*po));
+    for (int p = 0; p <= n_part; ++p) {
+        po->off[p] = part_off[p];
+        if (part_off[p] < 0 || part_off[p] > n_seeds || (p > 0 && part_off[p] < part_off[p - 1])) return COMET_EINVAL;
+        if (non_empty && p > 0 && part_off[p] == part_off[p - 1]) return COMET_EINVAL;
+    }
+    return COMET_OK;
+}
+
+static bool bad_box(const double* half_width)
+{
+    if (!half_width) return true;
+    for (int d = 0; d < 4; ++d)
+        if (!(half_width[d] >= 0.0) || !isfinite(half_width[d])) return true;
+    return false;
+}
+
+extern "C" int comet_select_references(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                                       const double* rss, const int64_t* part_off, int32_t n_part,
+                                       const double* half_width, int32_t k_ref, int64_t* ref_seed,
+                                       void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || seed_stride < n_seeds || n_part < 0 || n_part > COMET_MAX_PARTITIONS ||
+        k_ref < 1 || k_ref > COMET_MAX_REFS || bad_box(half_width))
+        return COMET_EINVAL;
+    if (n_part == 0) return COMET_OK;
+    if (!part_off || !ref_seed) return COMET_EINVAL;
+    PartOff po;
+    if (fill_partoff(&po, part_off, n_part, n_seeds, false)) return COMET_EINVAL;
+    if (po.off[n_part] > 0 && (!seeds || !rss)) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    RefBox box;
+    for (int d = 0; d < 4; ++d) box.two_hw[d] = 2.0 * half_width[d];
+    k_select_refs<<<n_part, COMET_REF_THREADS, 0, (cudaStream_t)cuda_stream>>>(seeds, seed_stride, rss, po, box, k_ref, ref_seed);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+static int make_grid(RefineGrid* g, int64_t* G, const double* half_width, const int32_t* n_grid)
+{
+    if (bad_box(half_width) || !n_grid) return COMET_EINVAL;
+    *G = 1;
+    for (int d = 0; d < 4; ++d) {
+        if (n_grid[d] < 1 || n_grid[d] > 4096) return COMET_EINVAL;
+        g->n[d] = n_grid[d];
+        g->hw[d] = half_width[d];
+        g->step[d] = n_grid[d] > 1 ? (2.0 * half_width[d]) / (double)(n_grid[d] - 1) : 0.0;
+        *G *= n_grid[d];
+        if (*G > ((int64_t)1 << 31)) return COMET_EINVAL;
+    }
+    return COMET_OK;
+}
+
+extern "C" int comet_refine_seeds(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                                  const int64_t* ref_seed, int32_t n_part, int32_t k_ref,
+                                  const double* half_width, const int32_t* n_grid,
+                                  double* new_seeds, int64_t new_stride, void* cuda_stream)
+{
+    RefineGrid g;
+    int64_t G = 0;
+    if (!ctx || n_seeds < 0 || seed_stride < n_seeds || n_part < 0 || n_part > COMET_MAX_PARTITIONS ||
+        k_ref < 1 || k_ref > COMET_MAX_REFS || make_grid(&g, &G, half_width, n_grid))
+        return COMET_EINVAL;
+    if (n_part == 0) return COMET_OK;
+    if (!seeds || !ref_seed || !new_seeds || new_stride < (int64_t)n_part * k_ref * G) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    const dim3 grid((unsigned)((G + 255) / 256), (unsigned)(n_part * k_ref));
+    k_refine_seeds<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(seeds, seed_stride, ref_seed, k_ref, g, G, new_seeds, new_stride);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+static int launch_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int32_t charge,
+                                 double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                                 const int32_t* hit_off, const double* rho, int32_t n_fired, int32_t n_hits,
+                                 double cutoff_cm, const int64_t* seed_idx, int32_t n_sel, const double* rss,
+                                 double* dca, uint8_t* cls, double* seed_out, double* rss_out, cudaStream_t st)
+{
+    ClassifyArgs a;
+    memset(&a, 0, sizeof(a));
+    a.seeds = seeds;
+    a.stride = seed_stride;
+    a.qkb = COMET_KAPPA * (double)charge * bz_tesla;
+    a.hk = make_stepk_host(step_cm);
+    a.n_steps = n_steps;
+    a.r_stop2 = r_stop_cm * r_stop_cm;
+    a.wt = ctx->wt;
+    a.W = n_fired;
+    a.hit_off = hit_off;
+    a.rho = rho;
+    a.n_hits = n_hits;
+    a.lambda = cutoff_cm;
+    const size_t smem = (size_t)(n_steps + 1) * 6 * sizeof(double);
+    k_classify_seeds<<<n_sel, 256, smem, st>>>(a, seed_idx, rss, dca, cls, seed_out, rss_out);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+extern "C" int comet_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                                    int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                                    double r_stop_cm,
+                                    const double* wire_a, const double* wire_b, int32_t n_wires,
+                                    const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                    int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                    const int64_t* seed_idx, int32_t n_sel, double* dca, uint8_t* cls,
+                                    void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
+        !(r_stop_cm >= 0.0) || n_sel < 0 ||
+        bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm))
+        return COMET_EINVAL;
+    if (n_sel == 0) return COMET_OK;
+    if (!seeds || !seed_idx || (n_fired > 0 && !dca) || (n_hits > 0 && !cls)) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
+    if (rc) return rc;
+    return launch_classify_seeds(ctx, seeds, seed_stride, charge, bz_tesla, step_cm, n_steps, r_stop_cm, hit_off, rho,
+                                 n_fired, n_hits, cutoff_cm, seed_idx, n_sel, nullptr, dca, cls, nullptr, nullptr, st);
+}
+
+// work buffer of comet_scan_stage: two seed sets [6][S_max], rss [S_max], references [P][max(k_ref, k_final)]
+static size_t stage_layout(int64_t n_seeds, int32_t n_part, int32_t k_ref, int32_t k_final, int64_t G,
+                           int64_t* s_max, size_t* off_rss, size_t* off_ref)
+{
+    const int64_t s_new = (int64_t)n_part * k_ref * G;
+    *s_max = ((n_seeds > s_new ? n_seeds : s_new) + 31) / 32 * 32;
+    size_t o = 2 * 6 * sizeof(double) * (size_t)*s_max;
+    *off_rss = o;
+    o += sizeof(double) * (size_t)*s_max;
+    *off_ref = o;
+    o += sizeof(int64_t) * (size_t)n_part * (size_t)(k_ref > k_final ? k_ref : k_final);
+    return (o + 255) / 256 * 256;
+}
+
+extern "C" size_t comet_stage_work_bytes(int64_t n_seeds, int32_t n_part, int32_t k_ref, int32_t k_final,
+                                         const int32_t* n_grid)
+{
+    RefineGrid g;
+    int64_t G = 0, s_max;
+    size_t o1, o2;
+    const double hw0[4] = {0.0, 0.0, 0.0, 0.0};
+    if (n_seeds < 0 || n_part < 0 || n_part > COMET_MAX_PARTITIONS || k_ref < 1 || k_ref > COMET_MAX_REFS ||
+        k_final < 1 || k_final > COMET_MAX_REFS || make_grid(&g, &G, hw0, n_grid))
+        return 0;
+    return stage_layout(n_seeds, n_part, k_ref, k_final, G, &s_max, &o1, &o2);
+}
+
+extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                                int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                                const double* wire_a, const double* wire_b, int32_t n_wires,
+                                const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                const int64_t* part_off, int32_t n_part,
+                                const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                                int32_t k_ref, int32_t k_final, void* work,
+                                double* final_seed, double* final_rss, double* final_dca, uint8_t* cls,
+                                void* cuda_stream)
+{
+    RefineGrid g;
+    int64_t G = 0;
+    if (!ctx || n_seeds < 1 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
+        !(r_stop_cm >= 0.0) ||
+        bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm) ||
+        n_part < 1 || n_part > COMET_MAX_PARTITIONS || !part_off || n_iter < 0 || !(shrink > 0.0) || !isfinite(shrink) ||
+        k_ref < 1 || k_ref > COMET_MAX_REFS || k_final < 1 || k_final > COMET_MAX_REFS ||
+        make_grid(&g, &G, half_width, n_grid) || !seeds || !work || !final_seed || !final_rss ||
+        (n_fired > 0 && !final_dca) || (n_hits > 0 && !cls))
+        return COMET_EINVAL;
+    PartOff po;
+    if (fill_partoff(&po, part_off, n_part, n_seeds, true) || po.off[0] != 0 || po.off[n_part] != n_seeds) return COMET_EINVAL;
+    int64_t s_max;
+    size_t off_rss, off_ref;
+    stage_layout(n_seeds, n_part, k_ref, k_final, G, &s_max, &off_rss, &off_ref);
+    double* set[2] = {(double*)work, (double*)work + 6 * s_max};
+    double* rss = (double*)((char*)work + off_rss);
+    int64_t* ref = (int64_t*)((char*)work + off_ref);
+    // iteration 0 scans the caller's seeds; iteration i > 0 the set written by the refinement before it
+    const double* cur = seeds;
+    int64_t cur_stride = seed_stride, cur_n = n_seeds;
+    int64_t po_cur[COMET_MAX_PARTITIONS + 1];
+    for (int p = 0; p <= n_part; ++p) po_cur[p] = part_off[p];
+    double hw[4] = {half_width[0], half_width[1], half_width[2], half_width[3]};
+    int rc;
+    for (int it = 0; ; ++it) {
+        rc = comet_scan_rss(ctx, cur, cur_stride, cur_n, charge, bz_tesla, step_cm, n_steps, r_stop_cm, wire_a, wire_b,
+                            n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm, rss, nullptr, cuda_stream);
+        if (rc) return rc;
+        if (it == n_iter) break;
+        rc = comet_select_references(ctx, cur, cur_stride, cur_n, rss, po_cur, n_part, hw, k_ref, ref, cuda_stream);
+        if (rc) return rc;
+        double* nxt = set[it & 1];
+        rc = comet_refine_seeds(ctx, cur, cur_stride, cur_n, ref, n_part, k_ref, hw, n_grid, nxt, s_max, cuda_stream);
+        if (rc) return rc;
+        cur = nxt;
+        cur_stride = s_max;
+        cur_n = (int64_t)n_part * k_ref * G;
+        for (int p = 0; p <= n_part; ++p) po_cur[p] = (int64_t)p * k_ref * G;
+        for (int d = 0; d < 4; ++d) hw[d] = hw[d] * shrink;
+    }
+    rc = comet_select_references(ctx, cur, cur_stride, cur_n, rss, po_cur, n_part, hw, k_final, ref, cuda_stream);
+    if (rc) return rc;
+    // the wire table is the one comet_scan_rss has just written on this stream
+    return launch_classify_seeds(ctx, cur, cur_stride, charge, bz_tesla, step_cm, n_steps, r_stop_cm, hit_off, rho,
+                                 n_fired, n_hits, cutoff_cm, ref, n_part * k_final, rss, final_dca, cls, final_seed,
+                                 final_rss, (cudaStream_t)cuda_stream);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -1,0 +1,128 @@
+// refine.cuh -- iterative seed refinement (readings R24-R28 of DESIGN.md), sm_100a.
+//
+//   k_select_refs     per turn partition, up to k sparse reference points: repeatedly the seed of lowest RSS
+//                     (ties -> lowest index, NaN never) that is not selected yet and whose refinement box
+//                     ref_d +- hw_d overlaps no selected box (|delta_d| < 2 hw_d in every dimension, strict);
+//   k_refine_seeds    the finer seed set around every reference point, linear in (z, p_x, p_y, p_z);
+//   k_classify_seeds  hit classification for a list of seeds (select.cuh's classify_cta).
+//
+// Everything stays on the device between the iterations of a stage (the paper copies seeds, tracks and RSS
+// across the PCIe bus four times per iteration).  Each comparison and each grid
+// value is one IEEE operation per operation of the definition, so references and seeds do not depend
+// on the kernel variant or on compiler flags.
+#pragma once
+#include "common.cuh"
+#include "select.cuh"
+
+namespace comet {
+
+#define COMET_REF_THREADS 1024
+// COMET_MAX_REFS (comet.h): limit of k_ref and k_final
+
+struct RefBox {
+    double two_hw[4];           // 2 * half width of dimension d (seed component 2 + d)
+};
+
+// One CTA per partition.  Round r: every thread walks its seeds in increasing index and keeps the first one
+// of strictly lowest RSS that is not blocked by the r references selected so far (the overlap test runs
+// only for a seed that would become the thread's candidate); the CTA merges the candidates (ties -> lower
+// index) and appends the winner.
+__global__ void __launch_bounds__(COMET_REF_THREADS)
+k_select_refs(const double* __restrict__ seeds, int64_t stride, const double* __restrict__ rss, PartOff po,
+              RefBox box, int32_t k_ref, int64_t* __restrict__ ref_seed)
+{
+    __shared__ int64_t sel_idx[COMET_MAX_REFS];
+    __shared__ double sel_c[COMET_MAX_REFS][4];
+    __shared__ double sv[COMET_REF_THREADS / 32];
+    __shared__ int64_t si[COMET_REF_THREADS / 32];
+    __shared__ int64_t s_win;
+    const int p = blockIdx.x;
+    const int64_t lo = po.off[p], hi = po.off[p + 1];
+    int64_t* out = ref_seed + (size_t)p * k_ref;
+    for (int r = threadIdx.x; r < k_ref; r += blockDim.x) out[r] = -1;
+    for (int r = 0; r < k_ref; ++r) {
+        double v = 0.0;
+        int64_t idx = -1;
+        for (int64_t s = lo + threadIdx.x; s < hi; s += blockDim.x) {
+            const double rs = rss[s];
+            if (rs != rs) continue;
+            if (idx >= 0 && !(rs < v)) continue;
+            bool blocked = false;
+            if (r > 0) {
+                const double c0 = seeds[2 * stride + s], c1 = seeds[3 * stride + s];
+                const double c2 = seeds[4 * stride + s], c3 = seeds[5 * stride + s];
+                for (int q = 0; q < r && !blocked; ++q) {
+                    const bool ov = fabs(xsub(c0, sel_c[q][0])) < box.two_hw[0] && fabs(xsub(c1, sel_c[q][1])) < box.two_hw[1] &&
+                                    fabs(xsub(c2, sel_c[q][2])) < box.two_hw[2] && fabs(xsub(c3, sel_c[q][3])) < box.two_hw[3];
+                    blocked = ov || sel_idx[q] == s;
+                }
+            }
+            if (!blocked) { v = rs; idx = s; }
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            const double v2 = __shfl_down_sync(0xffffffffu, v, o);
+            const int64_t i2 = __shfl_down_sync(0xffffffffu, idx, o);
+            argmin_merge(v, idx, v2, i2);
+        }
+        if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = v; si[threadIdx.x >> 5] = idx; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < COMET_REF_THREADS / 32; ++w) argmin_merge(v, idx, sv[w], si[w]);
+            s_win = idx;
+            if (idx >= 0) {
+                sel_idx[r] = idx;
+                for (int d = 0; d < 4; ++d) sel_c[r][d] = seeds[(size_t)(2 + d) * stride + idx];
+                out[r] = idx;
+            }
+        }
+        __syncthreads();
+        if (s_win < 0) break;
+    }
+}
+
+struct RefineGrid {
+    double hw[4];
+    double step[4];             // (2 hw) / (n - 1), 0 for n = 1
+    int32_t n[4];
+};
+
+// One thread per new seed.  Slot (p, r) = blockIdx.y holds G seeds around reference ref_seed[p][r]; an
+// empty slot repeats the partition's first reference (R27).
+__global__ void __launch_bounds__(256)
+k_refine_seeds(const double* __restrict__ seeds, int64_t stride, const int64_t* __restrict__ ref_seed,
+               int32_t k_ref, RefineGrid g, int64_t G, double* __restrict__ out, int64_t out_stride)
+{
+    const int64_t slot = blockIdx.y;
+    const int64_t gi = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gi >= G) return;
+    int64_t ref = ref_seed[slot];
+    if (ref < 0) ref = ref_seed[slot / k_ref * k_ref];
+    if (ref < 0) return;                                  // empty partition: nothing to write
+    const int64_t o = slot * G + gi;
+    out[o] = seeds[ref];
+    out[out_stride + o] = seeds[stride + ref];
+    int64_t rem = gi;
+#pragma unroll
+    for (int d = 3; d >= 0; --d) {
+        const int j = (int)(rem % g.n[d]);
+        rem /= g.n[d];
+        const double v = seeds[(size_t)(2 + d) * stride + ref];
+        out[(size_t)(2 + d) * out_stride + o] = (g.n[d] > 1) ? xadd(xsub(v, g.hw[d]), xmul((double)j, g.step[d])) : v;
+    }
+}
+
+// One CTA per listed seed: classification of PAPER.md:83 (classify_cta), the seed itself and its RSS.
+__global__ void __launch_bounds__(256)
+k_classify_seeds(const ClassifyArgs a, const int64_t* __restrict__ seed_idx, const double* __restrict__ rss,
+                 double* __restrict__ dca, uint8_t* __restrict__ cls, double* __restrict__ seed_out,
+                 double* __restrict__ rss_out)
+{
+    extern __shared__ __align__(16) double sm[];
+    const int64_t idx = seed_idx[blockIdx.x];
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+    if (threadIdx.x < 6 && seed_out) seed_out[(size_t)blockIdx.x * 6 + threadIdx.x] = (idx >= 0) ? a.seeds[threadIdx.x * a.stride + idx] : qnan;
+    if (threadIdx.x == 0 && rss_out) rss_out[blockIdx.x] = (idx >= 0 && rss) ? rss[idx] : qnan;
+    classify_cta(a, idx, dca + (size_t)blockIdx.x * a.W, cls + (size_t)blockIdx.x * a.n_hits, sm);
+}
+
+}  // namespace comet

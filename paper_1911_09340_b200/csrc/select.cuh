@@ -74,48 +74,35 @@ struct ClassifyArgs {
     uint8_t* cls;
 };
 
-// One CTA per partition: finish the argmin, re-extrapolate the winning seed into shared memory
-// (state k at sm[k*6..]), then one thread per fired wire does O5..O8 + O11 in exact arithmetic.
-__global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
+// CTA-wide: re-extrapolate seed `idx` into shared memory (state k at sm[k*6..]), then one thread per fired
+// wire does O5..O8 + O11 in exact arithmetic: dca[i] = signed D, cls[j] = 1 for the classified entries
+// (all other entries 0).  idx < 0: NaN / zeros.
+__device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx, double* __restrict__ dca,
+                                             uint8_t* __restrict__ cls, double* sm)
 {
-    extern __shared__ __align__(16) double sm[];       // [(n_steps+1)][6]
-    __shared__ int64_t s_best;
     __shared__ int32_t s_np;
     __shared__ double s_c;
-    const int p = blockIdx.x;
-    uint8_t* cls = a.cls + (size_t)p * a.n_hits;
     for (int j = threadIdx.x; j < a.n_hits; j += blockDim.x) cls[j] = 0;
-    if (threadIdx.x == 0) {
-        double v = 0.0;
-        int64_t idx = -1;
-        for (int b = 0; b < COMET_ARGMIN_SPLIT; ++b)
-            argmin_merge(v, idx, a.pv[p * COMET_ARGMIN_SPLIT + b], a.pi[p * COMET_ARGMIN_SPLIT + b]);
-        s_best = idx;
-        a.best_seed[p] = idx;
-        a.best_rss[p] = (idx >= 0) ? v : __longlong_as_double(0x7ff8000000000000LL);
-        if (idx >= 0) {
-            State st;
-            const double c = seed_init(a.seeds, a.stride, idx, a.qkb, st);
-            s_c = c;
-            int32_t np = a.n_steps + 1;
-            sm[0] = st.x0; sm[1] = st.x1; sm[2] = st.x2; sm[3] = st.t0; sm[4] = st.t1; sm[5] = st.t2;
-            for (int32_t k = 1; k <= a.n_steps; ++k) {
-                rkn4_step(st, a.hk, c);
-                double* o = sm + (size_t)k * 6;
-                o[0] = st.x0; o[1] = st.x1; o[2] = st.x2; o[3] = st.t0; o[4] = st.t1; o[5] = st.t2;
-                if (a.r_stop2 > 0.0 && in_target_region(st, a.r_stop2)) { np = k + 1; break; }
-            }
-            s_np = np;
-        }
-    }
-    __syncthreads();
-    const int64_t best = s_best;
     const int W = a.W;
-    if (best < 0) {
-        for (int i = threadIdx.x; i < W; i += blockDim.x)
-            a.best_dca[(size_t)p * W + i] = __longlong_as_double(0x7ff8000000000000LL);
+    if (idx < 0) {
+        for (int i = threadIdx.x; i < W; i += blockDim.x) dca[i] = __longlong_as_double(0x7ff8000000000000LL);
         return;
     }
+    if (threadIdx.x == 0) {
+        State st;
+        const double c = seed_init(a.seeds, a.stride, idx, a.qkb, st);
+        s_c = c;
+        int32_t np = a.n_steps + 1;
+        sm[0] = st.x0; sm[1] = st.x1; sm[2] = st.x2; sm[3] = st.t0; sm[4] = st.t1; sm[5] = st.t2;
+        for (int32_t k = 1; k <= a.n_steps; ++k) {
+            rkn4_step(st, a.hk, c);
+            double* o = sm + (size_t)k * 6;
+            o[0] = st.x0; o[1] = st.x1; o[2] = st.x2; o[3] = st.t0; o[4] = st.t1; o[5] = st.t2;
+            if (a.r_stop2 > 0.0 && in_target_region(st, a.r_stop2)) { np = k + 1; break; }
+        }
+        s_np = np;
+    }
+    __syncthreads();                                    // also orders the cls zeroing before the marks below
     const int32_t np = s_np;
     const double c = s_c;
     for (int i = threadIdx.x; i < W; i += blockDim.x) {
@@ -133,12 +120,31 @@ __global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
         st.x0 = sm[ks * 6]; st.x1 = sm[ks * 6 + 1]; st.x2 = sm[ks * 6 + 2];
         st.t0 = sm[ks * 6 + 3]; st.t1 = sm[ks * 6 + 4]; st.t2 = sm[ks * 6 + 5];
         const double D = fine_dca(st, ks, np, a.hk.h, c, wl);
-        a.best_dca[(size_t)p * W + i] = D;
+        dca[i] = D;
         int js;
         double rmin;
         (void)wire_residual(D, a.rho, a.hit_off[i], a.hit_off[i + 1], a.lambda, &js, &rmin);
         if (js >= 0 && rmin < a.lambda) cls[js] = 1;
     }
+}
+
+// One CTA per partition: finish the argmin, then classify the winning seed.
+__global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
+{
+    extern __shared__ __align__(16) double sm[];       // [(n_steps+1)][6]
+    __shared__ int64_t s_best;
+    const int p = blockIdx.x;
+    if (threadIdx.x == 0) {
+        double v = 0.0;
+        int64_t idx = -1;
+        for (int b = 0; b < COMET_ARGMIN_SPLIT; ++b)
+            argmin_merge(v, idx, a.pv[p * COMET_ARGMIN_SPLIT + b], a.pi[p * COMET_ARGMIN_SPLIT + b]);
+        s_best = idx;
+        a.best_seed[p] = idx;
+        a.best_rss[p] = (idx >= 0) ? v : __longlong_as_double(0x7ff8000000000000LL);
+    }
+    __syncthreads();
+    classify_cta(a, s_best, a.best_dca + (size_t)p * a.W, a.cls + (size_t)p * a.n_hits, sm);
 }
 
 }  // namespace comet

@@ -633,3 +633,112 @@ def test_seed_sharded_scan_two_ranks_emulated(comet, cfg1_event):
     sel = comet.select_and_classify(winners, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, gv.contiguous(),
                                     np.arange(P + 1, dtype=np.int64))
     assert torch.equal(sel["cls"], one["cls"]) and torch.equal(sel["best_dca"], one["best_dca"])
+
+
+# ------------------------------------------------------------------------------------------------
+# iterative seed refinement (comet_select_references, comet_refine_seeds, comet_classify_seeds,
+# comet_scan_stage): bit-identical references, seeds, RSS and classification
+# ------------------------------------------------------------------------------------------------
+def _ev_args(ev):
+    return (ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire,
+            ev.hit_off, ev.rho, ev.cutoff)
+
+
+@pytest.mark.parametrize("k_ref", [1, 5, 64])
+def test_select_references_matches_oracle(comet, k_ref):
+    rng = np.random.default_rng(11)
+    n = 5000
+    s = np.zeros((6, n))
+    s[2:] = rng.integers(0, 9, size=(4, n)) * np.array([[0.5], [1.0], [1.0], [2.0]])     # exact |d| = 2 hw ties
+    rss = rng.integers(0, 300, size=n).astype(float) * 0.01                               # many RSS ties
+    rss[rng.integers(0, n, 20)] = np.nan
+    po = np.array([0, 1, 1, 1900, 5000])                                                  # a 1-seed and an empty partition
+    hw = np.array([0.5, 1.0, 1.5, 2.0])
+    ref = comet.select_references(_dev(s), _dev(rss), po, hw, k_ref)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(ref.cpu().numpy(), O.select_references(s, rss, po, hw, k_ref))
+
+
+def test_select_references_cfg1_rss(comet, cfg1_event):
+    ev = cfg1_event
+    seeds, po = event_seeds(ev)
+    d = DevEvent(ev, seeds)
+    rss, _ = _run_fused(comet, d)
+    hw = np.array([0.6, 0.5, 0.5, 1.5])
+    ref = comet.select_references(d.seeds, _dev(rss), po, hw, 10)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(ref.cpu().numpy(), O.select_references(seeds, rss, po, hw, 10))
+
+
+def test_refine_seeds_matches_oracle(comet):
+    rng = np.random.default_rng(12)
+    seeds = rng.normal(size=(6, 300)) * 20
+    ref = np.array([[7, 11, -1, 5], [250, -1, -1, -1], [3, 4, 5, 6]], dtype=np.int64)
+    hw = np.array([1.5, 0.25, 2.0, 0.0])
+    for ng in ([4, 3, 2, 1], [1, 1, 1, 1], [5, 7, 3, 9]):
+        new, po = comet.refine_seeds(_dev(seeds), _dev(ref), hw, ng)
+        torch.cuda.synchronize()
+        exp, epo = O.refine_seeds(seeds, ref, hw, ng)
+        assert np.array_equal(new.cpu().numpy(), exp)
+        np.testing.assert_array_equal(po, epo)
+
+
+def test_classify_seeds_matches_oracle(comet, cfg0_event):
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev)
+    d = DevEvent(ev, seeds)
+    idx = np.array([5, -1, 8191, 670, 670], dtype=np.int64)
+    out = comet.classify_seeds(d.seeds, _dev(idx), *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    torch.cuda.synchronize()
+    ref = O.classify_seeds(seeds, idx, *_ev_args(ev))
+    np.testing.assert_array_equal(out["cls"].cpu().numpy(), ref["cls"])
+    np.testing.assert_array_equal(out["dca"].cpu().numpy(), ref["dca"])               # bit-identical, NaN rows included
+
+
+@pytest.mark.parametrize("n_iter", [0, 3])
+def test_scan_stage_matches_oracle_cfg0(comet, cfg0_event, n_iter):
+    ev = cfg0_event
+    seeds, po = event_seeds(ev)
+    d = DevEvent(ev, seeds)
+    kw = dict(half_width=[1.2, 1.0, 1.0, 4.0], n_grid=[3, 5, 5, 5], n_iter=n_iter, shrink=0.5, k_ref=4, k_final=10)
+    out = comet.scan_stage(d.seeds, po, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, **kw)
+    torch.cuda.synchronize()
+    ref = O.scan_stage(seeds, po, *_ev_args(ev), **kw)
+    np.testing.assert_array_equal(out["final_seed"].cpu().numpy(), ref["final_seed"])
+    np.testing.assert_array_equal(out["final_rss"].cpu().numpy(), ref["final_rss"])
+    np.testing.assert_array_equal(out["cls"].cpu().numpy(), ref["cls"])
+    _check_dca(np.nan_to_num(out["final_dca"].cpu().numpy()), np.nan_to_num(ref["final_dca"]))
+
+
+def test_scan_stage_cfg1_three_partitions(comet, cfg1_event):
+    """Three turn partitions at once, a coarse first set (every 8th seed of the configs[1] grid), two refinements."""
+    ev = cfg1_event
+    seeds, po = event_seeds(ev)
+    n_per = seeds.shape[1] // 3
+    seeds = np.ascontiguousarray(np.concatenate([seeds[:, p * n_per:(p + 1) * n_per:8] for p in range(3)], axis=1))
+    po = np.arange(4, dtype=np.int64) * (n_per // 8)
+    d = DevEvent(ev, seeds)
+    kw = dict(half_width=[0.6, 0.5, 0.5, 1.0], n_grid=[3, 4, 4, 3], n_iter=2, shrink=0.5, k_ref=6, k_final=10)
+    out = comet.scan_stage(d.seeds, po, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, **kw)
+    torch.cuda.synchronize()
+    ref = O.scan_stage(seeds, po, *_ev_args(ev), **kw)
+    np.testing.assert_array_equal(out["final_seed"].cpu().numpy(), ref["final_seed"])
+    np.testing.assert_array_equal(out["final_rss"].cpu().numpy(), ref["final_rss"])
+    np.testing.assert_array_equal(out["cls"].cpu().numpy(), ref["cls"])
+
+
+def test_refinement_argument_errors(comet, cfg0_event):
+    from paper_1911_09340_b200 import CometError
+    ev = cfg0_event
+    seeds, po = event_seeds(ev, shape=(2, 2, 2, 2))
+    d = DevEvent(ev, seeds)
+    rss = torch.zeros(seeds.shape[1], dtype=torch.float64, device="cuda")
+    with pytest.raises(CometError):
+        comet.select_references(d.seeds, rss, po, [1, 1, 1, 1], 65)
+    with pytest.raises(CometError):
+        comet.select_references(d.seeds, rss, po, [1, -1, 1, 1], 2)
+    with pytest.raises(CometError):
+        comet.refine_seeds(d.seeds, torch.zeros((1, 2), dtype=torch.int64, device="cuda"), [1, 1, 1, 1], [2, 0, 2, 2])
+    with pytest.raises(CometError):          # an empty partition
+        comet.scan_stage(d.seeds, [0, 0, seeds.shape[1]], *d.phys(), ev.r_stop, *d.hits(), ev.cutoff,
+                         half_width=[1, 1, 1, 1], n_grid=[2, 2, 2, 2], n_iter=1, shrink=0.5, k_ref=2, k_final=2)
