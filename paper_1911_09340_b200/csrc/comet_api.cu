@@ -158,6 +158,9 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
         e = cudaFuncSetAttribute(k_select_classify, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
     if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_select_refs_cluster<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 COMET_REF_SMEM_MAX * (int)sizeof(double));
+    if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_classify_seeds, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
     if (e != cudaSuccess) {
@@ -711,7 +714,21 @@ extern "C" int comet_select_references(comet_ctx* ctx, const double* seeds, int6
     if (rc) return rc;
     RefBox box;
     for (int d = 0; d < 4; ++d) box.two_hw[d] = 2.0 * half_width[d];
-    k_select_refs<<<n_part, COMET_REF_THREADS, 0, (cudaStream_t)cuda_stream>>>(seeds, seed_stride, rss, po, box, k_ref, ref_seed);
+    // small partitions: one CTA each; large ones: a cluster of CTAs each (RSS staged in shared memory when it fits)
+    int64_t n_max = 0;
+    for (int p = 0; p < n_part; ++p)
+        if (po.off[p + 1] - po.off[p] > n_max) n_max = po.off[p + 1] - po.off[p];
+    const int64_t per = (n_max + COMET_REF_CLUSTER - 1) / COMET_REF_CLUSTER;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (n_max <= 16 * COMET_REF_THREADS) {
+        k_select_refs<<<n_part, COMET_REF_THREADS, 0, st>>>(seeds, seed_stride, rss, po, box, k_ref, ref_seed);
+    } else if (per <= COMET_REF_SMEM_MAX) {
+        k_select_refs_cluster<true><<<dim3(COMET_REF_CLUSTER, n_part), COMET_REF_THREADS, (size_t)per * sizeof(double), st>>>(
+            seeds, seed_stride, rss, po, box, k_ref, ref_seed);
+    } else {
+        k_select_refs_cluster<false><<<dim3(COMET_REF_CLUSTER, n_part), COMET_REF_THREADS, 0, st>>>(
+            seeds, seed_stride, rss, po, box, k_ref, ref_seed);
+    }
     CU(ctx, cudaGetLastError());
     return COMET_OK;
 }

@@ -659,6 +659,21 @@ def test_select_references_matches_oracle(comet, k_ref):
     np.testing.assert_array_equal(ref.cpu().numpy(), O.select_references(s, rss, po, hw, k_ref))
 
 
+@pytest.mark.parametrize("n", [20000, 150000, 300000])
+def test_select_references_large_partitions(comet, n):
+    """One CTA (<= 16384 seeds), a cluster with RSS staged in shared memory, a cluster reading global memory."""
+    rng = np.random.default_rng(n)
+    s = np.zeros((6, n + 700))
+    s[2:] = rng.integers(0, 12, size=(4, n + 700)) * np.array([[0.5], [1.0], [1.0], [2.0]])
+    rss = rng.integers(0, 2000, size=n + 700).astype(float) * 0.001
+    rss[rng.integers(0, n, 50)] = np.nan
+    po = np.array([0, n, n + 700])
+    hw = np.array([0.5, 1.0, 1.0, 2.0])
+    ref = comet.select_references(_dev(s), _dev(rss), po, hw, 12)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(ref.cpu().numpy(), O.select_references(s, rss, po, hw, 12))
+
+
 def test_select_references_cfg1_rss(comet, cfg1_event):
     ev = cfg1_event
     seeds, po = event_seeds(ev)
