@@ -40,6 +40,9 @@ FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # FP64-pipe instructions per recorded state in kernel A: the RKN4 step of reading R1 is 48 IEEE operations
 # (44 issued: the two exact doublings ride on FMAs) + 4 for the target-region test of R3
 GEN_INSTR = 48
+# refinement recipe of the `stage` entry (R26): box half widths about one step of the configs[1] grid
+STAGE_HALF_WIDTH = [0.6, 0.5, 0.5, 1.0]
+STAGE_GRID = [5, 5, 5, 5]
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1c_full_scan_fused_fine_ck.txt)
 TRAFFIC_BYTES = {"k_scan_fused": 318474496 + 2222977000, "k_fine_ck": 680873984 + 80947000}
 
@@ -292,6 +295,24 @@ def run_ours(args):
     del track
     torch.cuda.empty_cache()
 
+    # ---- a whole stage: scan + 3 on-device refinements + final selection + classification ----
+    stage = None
+    if fused:
+        skw = dict(half_width=STAGE_HALF_WIDTH, n_grid=STAGE_GRID, n_iter=3, shrink=0.5, k_ref=10, k_final=10)
+        so = c.scan_stage(d_seeds, part_off, *phys, ev.r_stop, *hits, ev.cutoff, **skw)
+        swork = so["work"]
+        ms_stage, so = _time_steps(lambda: c.scan_stage(d_seeds, part_off, *phys, ev.r_stop, *hits, ev.cutoff, work=swork, **skw),
+                                   n_cmp, stream)
+        g = int(np.prod(STAGE_GRID))
+        stage = {"ms_per_stage": ms_stage, "iterations": 4,
+                 "seeds_per_iteration": [S] + [P * 10 * g] * 3,
+                 "dca_evals_per_s": (S + 3 * P * 10 * g) * W / (ms_stage * 1e-3),
+                 "best_rss_first_iteration": out["best_rss"].cpu().numpy().tolist(),
+                 "best_rss_final": so["final_rss"][:, 0].cpu().numpy().tolist(),
+                 "recipe": "comet_scan_stage: k_ref 10, half widths %s (z cm, px, py, pz MeV/c) halved per iteration, "
+                           "grid %s per reference, 10 finally selected seeds per partition classified" % (STAGE_HALF_WIDTH, STAGE_GRID)}
+        del swork, so
+
     # ---- e2e: host buffers through comet_scan_event_host -------------------------------------
     pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
     h = dict(seeds=pin(seeds, torch.float64), wa=pin(ev.geom.wire_a, torch.float64), wb=pin(ev.geom.wire_b, torch.float64),
@@ -394,6 +415,7 @@ def run_ours(args):
                 "api": "comet_scan_event_host, pinned host buffers" + ("" if fused else ", %d GiB track slab" % (budget >> 30))},
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
+        "stage": stage,
         "roofline": {"kernel": top["kernel"], "bound": "alu", "achieved": top["achieved"], "peak": peak,
                      "unit": "TFLOP/s", "frac": top["achieved"] / peak, "traffic": TRAFFIC_BYTES.get(kernel),
                      "timed": top["timed"],
