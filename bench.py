@@ -43,8 +43,8 @@ GEN_INSTR = 48
 # refinement recipe of the `stage` entry (R26): box half widths about one step of the configs[1] grid
 STAGE_HALF_WIDTH = [0.6, 0.5, 0.5, 1.0]
 STAGE_GRID = [5, 5, 5, 5]
-# dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1c_full_scan_fused_fine_ck.txt)
-TRAFFIC_BYTES = {"k_scan_fused": 318474496 + 2222977000, "k_fine_ck": 680873984 + 80947000}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1d_full_scan_fused_fine_ck.txt)
+TRAFFIC_BYTES = {"k_scan_fused": 347658496 + 2243479000, "k_fine_ck": 681160960 + 80465000}
 
 
 def _event(cfg):
@@ -377,10 +377,11 @@ def run_ours(args):
         lanes = c.get_option(OPT_LANES)
         top = {"kernel": "k_scan_fused + k_fine_ck (comet_scan_rss: sub-slabs on %d internal streams)" % lanes,
                "achieved": (fl[knames[0]] + fl[knames[1]]) / (ms_call * 1e-3) / 1e12, "ms_per_launch": ms_call,
-               "timed": "CUDA events on the caller's stream around every comet_scan_rss of the timed region"}
+               "timed": "CUDA events on the caller's stream around every comet_scan_rss of the timed region",
+               "traffic": (TRAFFIC_BYTES["k_scan_fused"] + TRAFFIC_BYTES["k_fine_ck"]) if args.config == 1 else None}
     else:
         top = {"kernel": kernel, "achieved": kernels[kernel]["achieved"], "ms_per_launch": ktimes[kernel],
-               "timed": kernels["timed_over"]}
+               "timed": kernels["timed_over"], "traffic": None}
     model = ("FP64-pipe slots x 2 of the work the path needs (thread-level counters, comet_read_stats): "
              + ("%d per recorded state (RKN4 step + target-region test, Alg. 1), " % GEN_INSTR if fused else "")
              + "%d per shortlist evaluation (sub-block sample or swept row); %s: %d per (seed, wire) pair that runs "
@@ -417,7 +418,7 @@ def run_ours(args):
         "clocks": clocks,
         "stage": stage,
         "roofline": {"kernel": top["kernel"], "bound": "alu", "achieved": top["achieved"], "peak": peak,
-                     "unit": "TFLOP/s", "frac": top["achieved"] / peak, "traffic": TRAFFIC_BYTES.get(kernel),
+                     "unit": "TFLOP/s", "frac": top["achieved"] / peak, "traffic": top["traffic"],
                      "timed": top["timed"],
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 figure)",
                      "peak_measured_dfma_probe": peak_measured,
