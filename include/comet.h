@@ -265,7 +265,8 @@ int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, i
 
 /* Runs A, B and C for one event whose inputs and outputs live in HOST memory (pinned memory makes
  * the copies asynchronous): copies the inputs to the device, runs comet_scan_rss (track on chip) when
- * track_budget_bytes == 0, else comet_seed_extrapolate + comet_dca_rss over slabs of seeds that fit
+ * track_budget_bytes == 0 -- the seeds are then uploaded sub-slab by sub-slab on the ctx's internal
+ * streams, so the upload overlaps the kernels of the sub-slabs already on the device --, else comet_seed_extrapolate + comet_dca_rss over slabs of seeds that fit
  * `track_budget_bytes` of track workspace (grown inside the ctx when needed), copies
  * best_seed/best_rss/best_dca/cls (and rss if rss_host != NULL) back and synchronises the stream.
  * All array arguments have the shapes of the device-buffer calls above. */

@@ -500,12 +500,15 @@ static int grow_dev(comet_ctx* ctx, void** buf, size_t* have, size_t need)
     return COMET_OK;
 }
 
-extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
-                              int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
-                              const double* wire_a, const double* wire_b, int32_t n_wires,
-                              const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
-                              int32_t n_fired, int32_t n_hits, double cutoff_cm,
-                              double* rss, int32_t* n_pts, void* cuda_stream)
+// comet_scan_rss; with seeds_host != NULL (HOST SoA [6][n_seeds]) every sub-slab first copies its seeds to
+// `seeds` on its own stream, so the upload of one sub-slab overlaps the kernels of the others
+static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_host,
+                         const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                         int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                         const double* wire_a, const double* wire_b, int32_t n_wires,
+                         const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                         int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                         double* rss, int32_t* n_pts, void* cuda_stream)
 {
     if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
         !(r_stop_cm >= 0.0) ||
@@ -589,6 +592,10 @@ extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_
             a.n_items = ctx->n_items + l;
             a.stats = ctx->opt_stats ? ctx->stats : nullptr;
             if (lanes > 1) CU(ctx, cudaStreamWaitEvent(s_scan, ctx->ev_fork, 0));
+            if (seeds_host)
+                for (int j = 0; j < 6; ++j)
+                    CU(ctx, cudaMemcpyAsync(seeds_w + (size_t)j * seed_stride + s0, seeds_host + (size_t)j * n_seeds + s0,
+                                            sizeof(double) * (size_t)a.n_seeds, cudaMemcpyHostToDevice, s_scan));
             CU(ctx, cudaMemsetAsync(a.n_items, 0, sizeof(unsigned int), s_scan));
             const unsigned b1 = (unsigned)((nc + COMET_FUSED_WARPS - 1) / COMET_FUSED_WARPS);
             const int64_t w2 = nc * (int64_t)n_fired;
@@ -617,6 +624,18 @@ extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_
             for (int l = 0; l < used; ++l) CU(ctx, cudaStreamWaitEvent(st, ctx->ev_join[l], 0));
     }
     return COMET_OK;
+}
+
+extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                              int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                              const double* wire_a, const double* wire_b, int32_t n_wires,
+                              const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                              int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                              double* rss, int32_t* n_pts, void* cuda_stream)
+{
+    return scan_rss_impl(ctx, nullptr, nullptr, seeds, seed_stride, n_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+                         wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm, rss, n_pts,
+                         cuda_stream);
 }
 
 extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
@@ -982,7 +1001,8 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
         if (rc) return rc;
     }
     // ---- H2D ---------------------------------------------------------------------------------
-    if (n_seeds) CU(ctx, cudaMemcpyAsync(d_seeds, seeds_host, sizeof(double) * 6 * (size_t)n_seeds, cudaMemcpyHostToDevice, st));
+    // (fused mode uploads the seeds per sub-slab inside scan_rss_impl, overlapped with the kernels)
+    if (n_seeds && !fused) CU(ctx, cudaMemcpyAsync(d_seeds, seeds_host, sizeof(double) * 6 * (size_t)n_seeds, cudaMemcpyHostToDevice, st));
     if (n_fired) {
         CU(ctx, cudaMemcpyAsync(d_wa, wire_a_host, sizeof(double) * 3 * (size_t)n_wires, cudaMemcpyHostToDevice, st));
         CU(ctx, cudaMemcpyAsync(d_wb, wire_b_host, sizeof(double) * 3 * (size_t)n_wires, cudaMemcpyHostToDevice, st));
@@ -992,8 +1012,8 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
     if (n_hits) CU(ctx, cudaMemcpyAsync(d_rho, rho_host, sizeof(double) * (size_t)n_hits, cudaMemcpyHostToDevice, st));
     // ---- A + B per slab, then C --------------------------------------------------------------
     if (fused && n_seeds > 0) {
-        rc = comet_scan_rss(ctx, d_seeds, n_seeds, n_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm, d_wa, d_wb,
-                            n_wires, d_fw, d_ho, d_rho, n_fired, n_hits, cutoff_cm, d_rss, d_npts, st);
+        rc = scan_rss_impl(ctx, d_seeds, seeds_host, d_seeds, n_seeds, n_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+                           d_wa, d_wb, n_wires, d_fw, d_ho, d_rho, n_fired, n_hits, cutoff_cm, d_rss, d_npts, st);
         if (rc) return rc;
     }
     const int64_t slab_seeds = slab_chunks * COMET_LANES;
