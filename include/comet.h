@@ -66,7 +66,7 @@ int comet_set_option(comet_ctx* ctx, int option, int value);
 int comet_get_option(const comet_ctx* ctx, int option, int* value);
 
 /* Sets the size of the (seed, wire) pair workspace of the pruned search to max_pairs_per_launch
- * pairs (12 bytes each; default limit 2^26) and allocates it now, so that later comet_dca_rss calls
+ * pairs (8 bytes each, 12 on the materialised path; default limit 2^28) and allocates it now, so that later comet_dca_rss calls
  * never allocate.  comet_dca_rss processes larger problems in seed slabs that fit; without this
  * call the workspace grows on the first comet_dca_rss that needs it (that call synchronises the
  * device). */

@@ -49,7 +49,8 @@ struct comet_ctx {
     cudaStream_t ls[COMET_MAX_LANES], lf[COMET_MAX_LANES];
     cudaEvent_t ev_fork, ev_scan[COMET_MAX_LANES], ev_join[COMET_MAX_LANES];
     int fine_blocks;             // persistent grid of k_fine
-    size_t pair_cap;             // pairs the two buffers hold
+    size_t pair_cap;             // pairs e2 / items hold
+    size_t kb_cap;               // pairs kb holds (allocated on the first pruned comet_dca_rss)
     size_t pair_max;             // growth limit (larger problems are processed in seed slabs)
     // fused path: checkpoints [chunks][n_ck][6][32] and n_pts when the caller does not want them
     double* ck;
@@ -119,7 +120,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaMalloc(&ctx->pi, sizeof(int64_t) * COMET_MAX_PARTITIONS * COMET_ARGMIN_SPLIT);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->stats, sizeof(unsigned long long) * ST_N);
     if (e == cudaSuccess) e = cudaMemset(ctx->stats, 0, sizeof(unsigned long long) * ST_N);
-    ctx->pair_max = (size_t)1 << 26;
+    ctx->pair_max = (size_t)1 << 28;
     ctx->ck_max = (size_t)8 << 30;
     ctx->fused_smem = ((COMET_FUSED_WFIELDS + 1) * COMET_FUSED_WCAP + COMET_FUSED_WARPS * COMET_FUSED_TR * 3 * COMET_LANES) * (int)sizeof(double);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
@@ -262,23 +263,32 @@ extern "C" int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, i
 static inline int64_t n_chunks_of(int64_t n_seeds) { return (n_seeds + COMET_LANES - 1) / COMET_LANES; }
 
 // grows the pair workspace to hold `pairs` (seed, wire) pairs (synchronises when it reallocates)
-static int ensure_pairs(comet_ctx* ctx, size_t pairs)
+static int ensure_pairs(comet_ctx* ctx, size_t pairs, bool need_kb)
 {
-    if (pairs <= ctx->pair_cap) return COMET_OK;
-    CU(ctx, cudaDeviceSynchronize());
-    cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items);
-    ctx->kb = nullptr; ctx->e2 = nullptr; ctx->items = nullptr; ctx->pair_cap = 0;
-    cudaError_t e = cudaMalloc(&ctx->kb, sizeof(int32_t) * pairs);
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->e2, sizeof(double) * pairs);
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->items, sizeof(unsigned long long) * (pairs / COMET_LANES + 1));
-    if (e != cudaSuccess) {
-        ctx->last_cuda = (int)e;
-        cudaFree(ctx->kb); ctx->kb = nullptr;
-        cudaFree(ctx->e2); ctx->e2 = nullptr;
-        cudaGetLastError();
-        return COMET_ENOMEM;
+    if (pairs > ctx->pair_cap) {
+        CU(ctx, cudaDeviceSynchronize());
+        cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items);
+        ctx->kb = nullptr; ctx->e2 = nullptr; ctx->items = nullptr; ctx->pair_cap = 0; ctx->kb_cap = 0;
+        cudaError_t e = cudaMalloc(&ctx->e2, sizeof(double) * pairs);
+        if (e == cudaSuccess) e = cudaMalloc(&ctx->items, sizeof(unsigned long long) * (pairs / COMET_LANES + 1));
+        if (e != cudaSuccess) {
+            ctx->last_cuda = (int)e;
+            cudaFree(ctx->e2); ctx->e2 = nullptr;
+            cudaFree(ctx->items); ctx->items = nullptr;
+            cudaGetLastError();
+            return COMET_ENOMEM;
+        }
+        ctx->pair_cap = pairs;
     }
-    ctx->pair_cap = pairs;
+    // the shortlisted-state buffer is used by the materialised pruned path only
+    if (need_kb && ctx->kb_cap < ctx->pair_cap) {
+        CU(ctx, cudaDeviceSynchronize());
+        cudaFree(ctx->kb);
+        ctx->kb = nullptr; ctx->kb_cap = 0;
+        cudaError_t e = cudaMalloc(&ctx->kb, sizeof(int32_t) * ctx->pair_cap);
+        if (e != cudaSuccess) { ctx->last_cuda = (int)e; cudaGetLastError(); return COMET_ENOMEM; }
+        ctx->kb_cap = ctx->pair_cap;
+    }
     return COMET_OK;
 }
 
@@ -288,7 +298,7 @@ extern "C" int comet_reserve(comet_ctx* ctx, int64_t max_pairs_per_launch)
     int rc = set_device(ctx);
     if (rc) return rc;
     ctx->pair_max = (size_t)max_pairs_per_launch;
-    return ensure_pairs(ctx, ctx->pair_max);
+    return ensure_pairs(ctx, ctx->pair_max, false);
 }
 
 extern "C" size_t comet_track_bytes(int64_t n_seeds, int32_t n_steps)
@@ -423,7 +433,7 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
         int64_t slab_chunks = (int64_t)(ctx->pair_max / ((size_t)COMET_LANES * (size_t)n_fired));
         if (slab_chunks < 1) slab_chunks = 1;
         if (slab_chunks > total_chunks) slab_chunks = total_chunks;
-        rc = ensure_pairs(ctx, (size_t)slab_chunks * COMET_LANES * (size_t)n_fired);
+        rc = ensure_pairs(ctx, (size_t)slab_chunks * COMET_LANES * (size_t)n_fired, true);
         if (rc) return rc;
         const int32_t n_rows = track_rows(n_steps);
         for (int64_t c0 = 0; c0 < total_chunks; c0 += slab_chunks) {
@@ -533,7 +543,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
     const int64_t by_ck = (int64_t)(ctx->ck_max / ck_chunk);
     if (by_ck < slab_chunks) slab_chunks = by_ck;
     if (slab_chunks < 1) slab_chunks = 1;
-    rc = ensure_pairs(ctx, (size_t)slab_chunks * COMET_LANES * (size_t)(n_fired > 0 ? n_fired : 1));
+    rc = ensure_pairs(ctx, (size_t)slab_chunks * COMET_LANES * (size_t)(n_fired > 0 ? n_fired : 1), false);
     if (rc) return rc;
     rc = grow_dev(ctx, (void**)&ctx->ck, &ctx->ck_bytes, (size_t)slab_chunks * ck_chunk);
     if (rc) return rc;
