@@ -453,3 +453,292 @@ void oracle_refine_seeds(const double* seeds, int64_t n_seeds, const int64_t* re
         }
     }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Inhomogeneous field map and adaptive step ("RKN method [7] with an adaptive step
+ * size that adjusts to the roughness of the magnetic field", :99 "BFields in the grid format",
+ * :135-136; readings R29-R32 of DESIGN.md).  Separate functions: the uniform-field ones above
+ * stay as pinned.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+    const double* B;     /* [nx][ny][nz][3] Tesla, node (i,j,k) at o + (i dx, j dy, k dz) */
+    int n[3];
+    double o[3], d[3];
+} ofield;
+
+static double lerp1(double a, double b, double f) { return a + f * (b - a); }
+
+/* R29: trilinear interpolation, z then y then x; outside the grid the edge value (clamped). */
+static void field_at(const ofield* F, const double x[3], double B[3])
+{
+    int idx[3], a, c;
+    double f[3];
+    for (a = 0; a < 3; ++a) {
+        double t = (x[a] - F->o[a]) / F->d[a];
+        double fl = floor(t);
+        if (fl < 0.0) fl = 0.0;
+        if (fl > (double)(F->n[a] - 2)) fl = (double)(F->n[a] - 2);
+        idx[a] = (int)fl;
+        f[a] = t - fl;
+        if (f[a] < 0.0) f[a] = 0.0;
+        if (f[a] > 1.0) f[a] = 1.0;
+    }
+    for (c = 0; c < 3; ++c) {
+        double v[2][2];
+        int di, dj;
+        for (di = 0; di < 2; ++di)
+            for (dj = 0; dj < 2; ++dj) {
+                size_t base = (((size_t)(idx[0] + di) * F->n[1] + (size_t)(idx[1] + dj)) * F->n[2] + (size_t)idx[2]) * 3 + c;
+                v[di][dj] = lerp1(F->B[base], F->B[base + 3], f[2]);
+            }
+        B[c] = lerp1(lerp1(v[0][0], v[0][1], f[1]), lerp1(v[1][0], v[1][1], f[1]), f[0]);
+    }
+}
+
+/* k = cq (T x B), cq = kappa q / |p|. */
+static void lorentz_rhs(const double T[3], const double B[3], double cq, double k[3])
+{
+    k[0] = cq * (T[1] * B[2] - T[2] * B[1]);
+    k[1] = cq * (T[2] * B[0] - T[0] * B[2]);
+    k[2] = cq * (T[0] * B[1] - T[1] * B[0]);
+}
+
+/* R30: one Nystrom RK4 step of signed length h in the field map: field at x, at the midpoint
+ * x + h/2 T + h^2/8 k1 (used for k2 and k3) and at the end point x + h T + h^2/2 k3.  Returns the
+ * error estimate EST = h^2 (|k1-k2-k3+k4|_x + |.|_y + |.|_z) of the method of ref [7]. */
+static double rkn4_field_step(ostate* s, double h, double cq, const ofield* F)
+{
+    double B[3], k1[3], k2[3], k3[3], k4[3], t[3], xm[3], est = 0.0;
+    int i;
+    field_at(F, s->x, B);
+    lorentz_rhs(s->T, B, cq, k1);
+    for (i = 0; i < 3; ++i) xm[i] = s->x[i] + (h / 2.0) * s->T[i] + ((h * h) / 8.0) * k1[i];
+    field_at(F, xm, B);
+    for (i = 0; i < 3; ++i) t[i] = s->T[i] + (h / 2.0) * k1[i];
+    lorentz_rhs(t, B, cq, k2);
+    for (i = 0; i < 3; ++i) t[i] = s->T[i] + (h / 2.0) * k2[i];
+    lorentz_rhs(t, B, cq, k3);
+    for (i = 0; i < 3; ++i) xm[i] = s->x[i] + h * s->T[i] + ((h * h) / 2.0) * k3[i];
+    field_at(F, xm, B);
+    for (i = 0; i < 3; ++i) t[i] = s->T[i] + h * k3[i];
+    lorentz_rhs(t, B, cq, k4);
+    for (i = 0; i < 3; ++i) est = est + fabs(((k1[i] - k2[i]) - k3[i]) + k4[i]);
+    est = (h * h) * est;
+    for (i = 0; i < 3; ++i) s->x[i] = s->x[i] + h * s->T[i] + ((h * h) / 6.0) * (k1[i] + k2[i] + k3[i]);
+    for (i = 0; i < 3; ++i) s->T[i] = s->T[i] + (h / 6.0) * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+    return est;
+}
+
+/* R31: Algorithm 1 with the adaptive step.  The trial step starts at h_max; a step whose EST
+ * exceeds tol is retried with half the length (not below h_max/64); after an accepted step with
+ * EST < tol/32 the trial step doubles (not above h_max).  hs[k] = length of the step from state
+ * k to state k+1.  Stop rule R3 as in record_track. */
+static int record_track_field(const double seed[6], int charge, const ofield* F, double h_max, int n_steps,
+                              double r_stop, double tol, ostate* pts, double* hs)
+{
+    double P = sqrt(seed[3] * seed[3] + seed[4] * seed[4] + seed[5] * seed[5]);
+    double cq = ORACLE_KAPPA * (double)charge / P;
+    double h = h_max, h_min = h_max / 64.0;
+    int k, n_pts = n_steps + 1;
+    pts[0].x[0] = seed[0]; pts[0].x[1] = seed[1]; pts[0].x[2] = seed[2];
+    pts[0].T[0] = seed[3] / P; pts[0].T[1] = seed[4] / P; pts[0].T[2] = seed[5] / P;
+    for (k = 1; k <= n_steps; ++k) {
+        double est;
+        for (;;) {
+            pts[k] = pts[k - 1];
+            est = rkn4_field_step(&pts[k], h, cq, F);
+            if (est > tol && h > h_min) { h = h / 2.0; continue; }
+            break;
+        }
+        hs[k - 1] = h;
+        if (est < tol / 32.0 && h < h_max) h = 2.0 * h;
+        if (r_stop > 0.0) {
+            double r2 = pts[k].x[0] * pts[k].x[0] + pts[k].x[1] * pts[k].x[1];
+            double rad = pts[k].x[0] * pts[k].T[0] + pts[k].x[1] * pts[k].T[1];
+            if (r2 < r_stop * r_stop && rad < 0.0) { n_pts = k + 1; break; }
+        }
+    }
+    return n_pts;
+}
+
+/* O5..O7 in the field map: as wire_dca, the sub-steps are field steps (PAPER.md:180
+ * "RKN(state, distance, BFields)") and the bracket is the two recorded steps around k* (R32). */
+static double wire_dca_field(const ostate* pts, const double* hs, int n_pts, double cq, const ofield* F,
+                             const double m[3], const double w[3], int* kstar_out)
+{
+    int k, kstar = 0, it;
+    double best = 0.0, u[3], sigma = 0.0, lo, hi, cross[3], side, dist;
+    ostate s;
+    for (k = 0; k < n_pts; ++k) {
+        double d2;
+        perp_to_wire(pts[k].x, m, w, u);
+        d2 = dot3(u, u);
+        if (k == 0 || d2 < best) { best = d2; kstar = k; }
+    }
+    s = pts[kstar];
+    lo = (kstar > 0) ? -hs[kstar - 1] : 0.0;
+    hi = (kstar < n_pts - 1) ? hs[kstar] : 0.0;
+    for (it = 0; it < ORACLE_MAX_ITER; ++it) {
+        double nv[3], tw, den, mx[3], delta, target;
+        int i;
+        tw = dot3(s.T, w);
+        for (i = 0; i < 3; ++i) nv[i] = s.T[i] - tw * w[i];
+        den = dot3(s.T, nv);
+        if (den < 1e-12) break;
+        for (i = 0; i < 3; ++i) mx[i] = m[i] - s.x[i];
+        delta = dot3(mx, nv) / den;
+        target = sigma + delta;
+        if (target < lo) target = lo;
+        if (target > hi) target = hi;
+        delta = target - sigma;
+        if (fabs(delta) < ORACLE_TOL_CM) break;
+        (void)rkn4_field_step(&s, delta, cq, F);
+        sigma = sigma + delta;
+    }
+    perp_to_wire(s.x, m, w, u);
+    cross[0] = s.T[1] * w[2] - s.T[2] * w[1];
+    cross[1] = s.T[2] * w[0] - s.T[0] * w[2];
+    cross[2] = s.T[0] * w[1] - s.T[1] * w[0];
+    side = dot3(u, cross);
+    dist = sqrt(dot3(u, u));
+    if (kstar_out) *kstar_out = kstar;
+    return (side >= 0.0) ? dist : -dist;
+}
+
+static ofield make_field(const double* B, const int32_t* n, const double* o, const double* d)
+{
+    ofield F;
+    int a;
+    F.B = B;
+    for (a = 0; a < 3; ++a) { F.n[a] = n[a]; F.o[a] = o[a]; F.d[a] = d[a]; }
+    return F;
+}
+
+/* pins */
+void oracle_field_at(const double* B, const int32_t* n, const double* o, const double* d,
+                     const double* x3, double* out3)
+{
+    ofield F = make_field(B, n, o, d);
+    field_at(&F, x3, out3);
+}
+
+double oracle_rkn4_field_step(const double* B, const int32_t* n, const double* o, const double* d,
+                              double* state6, double h, double cq)
+{
+    ofield F = make_field(B, n, o, d);
+    ostate s;
+    double est;
+    int i;
+    for (i = 0; i < 3; ++i) { s.x[i] = state6[i]; s.T[i] = state6[3 + i]; }
+    est = rkn4_field_step(&s, h, cq, &F);
+    for (i = 0; i < 3; ++i) { state6[i] = s.x[i]; state6[3 + i] = s.T[i]; }
+    return est;
+}
+
+/* Algorithm 1 in the field map: track [n_seeds][n_steps+1][6] (NaN beyond n_pts), n_pts [n_seeds],
+ * hs [n_seeds][n_steps] step lengths (NaN beyond n_pts-1). */
+void oracle_extrapolate_field(const double* seeds, int64_t n_seeds, int charge,
+                              const double* B, const int32_t* n, const double* o, const double* d,
+                              double h_max, int n_steps, double r_stop, double tol,
+                              double* track, int32_t* n_pts, double* hs_out)
+{
+    ofield F = make_field(B, n, o, d);
+    int64_t s;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (s = 0; s < n_seeds; ++s) {
+        ostate* pts = (ostate*)malloc(sizeof(ostate) * (size_t)(n_steps + 1));
+        double* hs = (double*)malloc(sizeof(double) * (size_t)n_steps);
+        double seed[6];
+        int i, k, np;
+        for (i = 0; i < 6; ++i) seed[i] = seeds[(size_t)i * n_seeds + s];
+        np = record_track_field(seed, charge, &F, h_max, n_steps, r_stop, tol, pts, hs);
+        n_pts[s] = np;
+        for (k = 0; k <= n_steps; ++k) {
+            double* row = track + ((size_t)s * (size_t)(n_steps + 1) + (size_t)k) * 6;
+            for (i = 0; i < 3; ++i) {
+                row[i] = (k < np) ? pts[k].x[i] : NAN;
+                row[3 + i] = (k < np) ? pts[k].T[i] : NAN;
+            }
+            if (k < n_steps) hs_out[(size_t)s * n_steps + k] = (k < np - 1) ? hs[k] : NAN;
+        }
+        free(pts);
+        free(hs);
+    }
+}
+
+/* Algorithm 3 in the field map (as oracle_scan). */
+void oracle_scan_field(const double* seeds, int64_t n_seeds, int charge,
+                       const double* B, const int32_t* n, const double* o, const double* d,
+                       double h_max, int n_steps, double r_stop, double tol,
+                       const double* wire_a, const double* wire_b, int n_wires,
+                       const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                       int n_fired, double cutoff, double* rss, double* dca, int32_t* kstar, int32_t* n_pts)
+{
+    ofield F = make_field(B, n, o, d);
+    int64_t s;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (s = 0; s < n_seeds; ++s) {
+        ostate* pts = (ostate*)malloc(sizeof(ostate) * (size_t)(n_steps + 1));
+        double* hs = (double*)malloc(sizeof(double) * (size_t)n_steps);
+        double seed[6], P, cq, acc = 0.0;
+        int i, np;
+        for (i = 0; i < 6; ++i) seed[i] = seeds[(size_t)i * n_seeds + s];
+        P = sqrt(seed[3] * seed[3] + seed[4] * seed[4] + seed[5] * seed[5]);
+        cq = ORACLE_KAPPA * (double)charge / P;
+        np = record_track_field(seed, charge, &F, h_max, n_steps, r_stop, tol, pts, hs);
+        if (n_pts) n_pts[s] = np;
+        for (i = 0; i < n_fired; ++i) {
+            double m[3], w[3], D, e;
+            int ks;
+            wire_line(wire_a, wire_b, n_wires, fired_wire[i], m, w);
+            D = wire_dca_field(pts, hs, np, cq, &F, m, w, &ks);
+            e = wire_residual(D, rho, hit_off[i], hit_off[i + 1], cutoff, NULL, NULL);
+            acc = acc + e * e;
+            if (dca) dca[(size_t)s * n_fired + i] = D;
+            if (kstar) kstar[(size_t)s * n_fired + i] = ks;
+        }
+        rss[s] = acc;
+        free(pts);
+        free(hs);
+    }
+}
+
+/* O11 in the field map for the listed seeds: dca [n_sel][n_fired], cls [n_sel][n_hits]. */
+void oracle_classify_seeds_field(const double* seeds, int64_t n_seeds, int charge,
+                                 const double* B, const int32_t* n, const double* o, const double* d,
+                                 double h_max, int n_steps, double r_stop, double tol,
+                                 const double* wire_a, const double* wire_b, int n_wires,
+                                 const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                 int n_fired, int n_hits, double cutoff,
+                                 const int64_t* seed_idx, int n_sel, double* dca, uint8_t* cls)
+{
+    ofield F = make_field(B, n, o, d);
+    ostate* pts = (ostate*)malloc(sizeof(ostate) * (size_t)(n_steps + 1));
+    double* hs = (double*)malloc(sizeof(double) * (size_t)n_steps);
+    int q;
+    for (q = 0; q < n_sel; ++q) {
+        int64_t s = seed_idx[q];
+        double seed[6], P, cq;
+        int i, np;
+        memset(cls + (size_t)q * (size_t)n_hits, 0, (size_t)n_hits);
+        if (s < 0) {
+            for (i = 0; i < n_fired; ++i) dca[(size_t)q * n_fired + i] = NAN;
+            continue;
+        }
+        for (i = 0; i < 6; ++i) seed[i] = seeds[(size_t)i * n_seeds + s];
+        P = sqrt(seed[3] * seed[3] + seed[4] * seed[4] + seed[5] * seed[5]);
+        cq = ORACLE_KAPPA * (double)charge / P;
+        np = record_track_field(seed, charge, &F, h_max, n_steps, r_stop, tol, pts, hs);
+        for (i = 0; i < n_fired; ++i) {
+            double m[3], w[3], D, rmin;
+            int js;
+            wire_line(wire_a, wire_b, n_wires, fired_wire[i], m, w);
+            D = wire_dca_field(pts, hs, np, cq, &F, m, w, NULL);
+            dca[(size_t)q * n_fired + i] = D;
+            (void)wire_residual(D, rho, hit_off[i], hit_off[i + 1], cutoff, &js, &rmin);
+            if (js >= 0 && rmin < cutoff) cls[(size_t)q * (size_t)n_hits + js] = 1;
+        }
+    }
+    free(pts);
+    free(hs);
+}

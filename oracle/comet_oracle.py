@@ -46,6 +46,16 @@ def lib():
         L.oracle_select_classify.argtypes = [_F64, c_i64, c_int, c_dbl, c_dbl, c_int, c_dbl,
                                              _F64, _F64, c_int, _I32, _I32, _F64, c_int, c_int, c_dbl,
                                              _F64, _I64, c_int, _I64, _F64, _F64, _U8]
+        fld = [_F64, _I32, _F64, _F64]
+        L.oracle_field_at.argtypes = fld + [_F64, _F64]
+        L.oracle_rkn4_field_step.argtypes = fld + [_F64, c_dbl, c_dbl]
+        L.oracle_rkn4_field_step.restype = c_dbl
+        L.oracle_extrapolate_field.argtypes = [_F64, c_i64, c_int] + fld + [c_dbl, c_int, c_dbl, c_dbl, _F64, _I32, _F64]
+        L.oracle_scan_field.argtypes = [_F64, c_i64, c_int] + fld + [c_dbl, c_int, c_dbl, c_dbl,
+                                        _F64, _F64, c_int, _I32, _I32, _F64, c_int, c_dbl, _F64, vp, vp, vp]
+        L.oracle_classify_seeds_field.argtypes = [_F64, c_i64, c_int] + fld + [c_dbl, c_int, c_dbl, c_dbl,
+                                                  _F64, _F64, c_int, _I32, _I32, _F64, c_int, c_int, c_dbl,
+                                                  _I64, c_int, _F64, _U8]
         L.oracle_select_references.argtypes = [_F64, c_i64, _F64, _I64, c_int, _F64, c_int, _I64]
         L.oracle_refine_seeds.argtypes = [_F64, c_i64, _I64, c_int, c_int, _F64, _I32, _F64]
         _lib = L
@@ -197,3 +207,73 @@ def scan_stage(seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_
     W, H = len(fired_wire), len(rho)
     return {"final_seed": final_seed, "final_rss": final_rss, "final_dca": c["dca"].reshape(P, int(k_final), W),
             "cls": c["cls"].reshape(P, int(k_final), H), "history": history}
+
+
+# ---- inhomogeneous field map + adaptive step (readings R29-R32) -------------------
+def _fld(field):
+    """field = (B [nx][ny][nz][3], origin [3], spacing [3]) -> ctypes arguments."""
+    B, o, d = field
+    B = _c(B, np.float64)
+    return B, np.array(B.shape[:3], dtype=np.int32), _c(o, np.float64), _c(d, np.float64)
+
+
+def field_at(field, x):
+    out = np.empty(3)
+    lib().oracle_field_at(*_fld(field), _c(x, np.float64), out)
+    return out
+
+
+def rkn4_field_step(field, state6, h, cq):
+    """One Nystrom RK4 step in the field map -> (new state, EST)."""
+    s = np.array(state6, dtype=np.float64)
+    est = lib().oracle_rkn4_field_step(*_fld(field), s, float(h), float(cq))
+    return s, float(est)
+
+
+def extrapolate_field(seeds, charge, field, h_max, n_steps, r_stop, tol):
+    seeds = _c(seeds, np.float64)
+    S = seeds.shape[1]
+    track = np.empty((S, n_steps + 1, 6))
+    n_pts = np.empty(S, dtype=np.int32)
+    hs = np.empty((S, n_steps))
+    lib().oracle_extrapolate_field(seeds, S, int(charge), *_fld(field), float(h_max), int(n_steps), float(r_stop),
+                                   float(tol), track, n_pts, hs)
+    return track, n_pts, hs
+
+
+def scan_field(seeds, charge, field, h_max, n_steps, r_stop, tol, wire_a, wire_b, fired_wire, hit_off, rho,
+               cutoff, want_dca=False, want_kstar=False, want_npts=False):
+    seeds = _c(seeds, np.float64)
+    wire_a, wire_b = _c(wire_a, np.float64), _c(wire_b, np.float64)
+    fired_wire, hit_off, rho = _c(fired_wire, np.int32), _c(hit_off, np.int32), _c(rho, np.float64)
+    S, W = seeds.shape[1], fired_wire.shape[0]
+    out = {"rss": np.empty(S)}
+    dca = np.empty((S, W)) if want_dca else None
+    ks = np.empty((S, W), dtype=np.int32) if want_kstar else None
+    npt = np.empty(S, dtype=np.int32) if want_npts else None
+    ptr = lambda a: a.ctypes.data_as(ctypes.c_void_p) if a is not None else None
+    lib().oracle_scan_field(seeds, S, int(charge), *_fld(field), float(h_max), int(n_steps), float(r_stop), float(tol),
+                            wire_a, wire_b, wire_a.shape[1], fired_wire, hit_off, rho, W, float(cutoff),
+                            out["rss"], ptr(dca), ptr(ks), ptr(npt))
+    if want_dca:
+        out["dca"] = dca
+    if want_kstar:
+        out["kstar"] = ks
+    if want_npts:
+        out["n_pts"] = npt
+    return out
+
+
+def classify_seeds_field(seeds, idx, charge, field, h_max, n_steps, r_stop, tol, wire_a, wire_b, fired_wire,
+                         hit_off, rho, cutoff):
+    seeds = _c(seeds, np.float64)
+    wire_a, wire_b = _c(wire_a, np.float64), _c(wire_b, np.float64)
+    fired_wire, hit_off, rho = _c(fired_wire, np.int32), _c(hit_off, np.int32), _c(rho, np.float64)
+    idx = _c(np.asarray(idx, dtype=np.int64).ravel(), np.int64)
+    W, H = fired_wire.shape[0], rho.shape[0]
+    dca = np.empty((idx.size, W))
+    cls = np.zeros((idx.size, H), dtype=np.uint8)
+    lib().oracle_classify_seeds_field(seeds, seeds.shape[1], int(charge), *_fld(field), float(h_max), int(n_steps),
+                                      float(r_stop), float(tol), wire_a, wire_b, wire_a.shape[1], fired_wire,
+                                      hit_off, rho, W, H, float(cutoff), idx, idx.size, dca, cls)
+    return {"dca": dca, "cls": cls}
