@@ -87,6 +87,27 @@ int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n, int32_t* n_call
  * executed it, [5] all pairs. */
 int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, int32_t reset, void* cuda_stream);
 
+/* ---- inhomogeneous field map and adaptive step (R29-R32) ------- */
+
+#define COMET_MAX_STEPS_FIELD 4000    /* n_steps limit while a field map is set */
+
+/* "BFields in the grid format": field_dev is a regular grid [nx][ny][nz][3] of
+ * (Bx, By, Bz) in Tesla (dev, caller-owned, must stay valid while it is set), node (i,j,k) at
+ * origin_cm + (i dx, j dy, k dz); n_nodes, origin_cm, spacing_cm are HOST [3].  The field at a point
+ * is the trilinear interpolation, the edge value outside the grid (R29).  While a map is set,
+ * comet_scan_rss, comet_select_and_classify, comet_classify_seeds, comet_scan_stage and
+ * comet_scan_event_host (fused) extrapolate in it -- their bz_tesla argument is ignored -- with the
+ * Nystrom RK4 step of R30 and the adaptive step of R31 ("an adaptive step size that adjusts to the
+ * roughness of the magnetic field"): step_cm is the longest step h_max, a step whose
+ * error estimate exceeds rkn_tol_cm is retried with half the length (not below h_max/64), after a
+ * step with an estimate below rkn_tol_cm/32 the next trial step doubles; n_steps stays the capacity
+ * in recorded states (<= COMET_MAX_STEPS_FIELD).  comet_seed_extrapolate and comet_dca_rss (the
+ * materialised track) are uniform-field paths and return COMET_EINVAL.  field_dev = NULL returns
+ * to the uniform field.  Enqueues one small kernel on cuda_stream (the map's largest |B|). */
+int comet_set_field(comet_ctx* ctx, const double* field_dev, const int32_t* n_nodes,
+                    const double* origin_cm, const double* spacing_cm, double rkn_tol_cm,
+                    void* cuda_stream);
+
 /* ---- kernel A: track recording (Algorithm 1) ---------------------------- */
 
 /* Bytes of the opaque track buffer for n_seeds seeds and n_steps steps.

@@ -178,7 +178,7 @@ def classify_seeds(seeds, idx, charge, bz, step, n_steps, r_stop, wire_a, wire_b
 
 
 def scan_stage(seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
-               cutoff, half_width, n_grid, n_iter, shrink, k_ref, k_final):
+               cutoff, half_width, n_grid, n_iter, shrink, k_ref, k_final, field=None, rkn_tol=None):
     """One *stage* (the seed scanning of a turn, several *iterations*), every turn
     partition at once (R14).  Iteration 0 scans the given seeds; each of the n_iter further iterations
     picks k_ref sparse reference points (box half_width), scans the finer sets around them, and
@@ -189,13 +189,20 @@ def scan_stage(seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_
     part_off = _c(part_off, np.int64)
     hw = np.array(half_width, dtype=np.float64)
     args = (charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho, cutoff)
+    if field is not None:        # the same stage in a field map (R29-R32): bz is not used
+        fargs = (charge, field, step, n_steps, r_stop, rkn_tol, wire_a, wire_b, fired_wire, hit_off, rho, cutoff)
+        scan_ = lambda sd: scan_field(sd, *fargs)
+        classify_ = lambda sd, idx: classify_seeds_field(sd, idx, *fargs)
+    else:
+        scan_ = lambda sd: scan(sd, *args)
+        classify_ = lambda sd, idx: classify_seeds(sd, idx, *args)
     history = []
-    rss = scan(seeds, *args)["rss"]
+    rss = scan_(seeds)["rss"]
     for _ in range(int(n_iter)):
         ref = select_references(seeds, rss, part_off, hw, k_ref)
         history.append({"ref_rss": np.where(ref >= 0, rss[np.maximum(ref, 0)], np.nan), "half_width": hw.copy()})
         seeds, part_off = refine_seeds(seeds, ref, hw, n_grid)
-        rss = scan(seeds, *args)["rss"]
+        rss = scan_(seeds)["rss"]
         hw = hw * float(shrink)
     fin = select_references(seeds, rss, part_off, hw, k_final)
     P = fin.shape[0]
@@ -203,7 +210,7 @@ def scan_stage(seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_
     ok = fin >= 0
     final_seed[ok] = seeds[:, fin[ok]].T
     final_rss = np.where(ok, rss[np.maximum(fin, 0)], np.nan)
-    c = classify_seeds(seeds, fin, *args)
+    c = classify_(seeds, fin)
     W, H = len(fired_wire), len(rho)
     return {"final_seed": final_seed, "final_rss": final_rss, "final_dca": c["dca"].reshape(P, int(k_final), W),
             "cls": c["cls"].reshape(P, int(k_final), H), "history": history}

@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = [
     "comet_track_export", "comet_dca_rss", "comet_select_and_classify", "comet_scan_event_host",
     "comet_fp64_peak_probe", "comet_read_stats", "comet_reserve", "comet_read_timing", "comet_scan_rss",
     "comet_select_references", "comet_refine_seeds", "comet_classify_seeds", "comet_stage_work_bytes",
-    "comet_scan_stage",
+    "comet_scan_stage", "comet_set_field",
 ]
 
 COMET_CHUNK = 32
@@ -79,6 +79,7 @@ def load_library():
     L.comet_reserve.argtypes = [vp, i64]
     L.comet_read_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32, ctypes.POINTER(i32)]
     L.comet_read_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), i32, i32, vp]
+    L.comet_set_field.argtypes = [vp, vp, vp, vp, vp, dbl, vp]
     L.comet_select_references.argtypes = [vp, vp, i64, i64, vp, vp, i32, vp, i32, vp, vp]
     L.comet_refine_seeds.argtypes = [vp, vp, i64, i64, vp, i32, i32, vp, vp, vp, i64, vp]
     L.comet_classify_seeds.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
@@ -150,6 +151,22 @@ class Comet:
         v = ctypes.c_int()
         self._check(self._L.comet_get_option(self._h, int(option), ctypes.byref(v)))
         return v.value
+
+    def set_field(self, field=None, origin=None, spacing=None, rkn_tol=1e-7, stream=None):
+        """comet_set_field: `field` is a CUDA tensor [nx][ny][nz][3] (Tesla) that must stay alive while it
+        is set; None returns to the uniform field."""
+        if field is None:
+            self._field = None
+            self._check(self._L.comet_set_field(self._h, 0, 0, 0, 0, 0.0, 0))
+            return
+        n = np.ascontiguousarray(np.asarray(field.shape[:3], dtype=np.int32))
+        o = np.ascontiguousarray(np.asarray(origin, dtype=np.float64))
+        d = np.ascontiguousarray(np.asarray(spacing, dtype=np.float64))
+        if field.dim() != 4 or field.shape[3] != 3:
+            raise CometError("field must be [nx][ny][nz][3]")
+        self._check(self._L.comet_set_field(self._h, _dev(field, torch.float64, "field", self.device), n.ctypes.data,
+                                            o.ctypes.data, d.ctypes.data, float(rkn_tol), _stream_ptr(stream)))
+        self._field = field
 
     def reserve(self, max_pairs_per_launch: int):
         """Pre-allocates the pruned search's (seed, wire) pair workspace (12 bytes per pair)."""

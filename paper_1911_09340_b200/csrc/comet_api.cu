@@ -61,6 +61,8 @@ struct comet_ctx {
     double* cw;                  // [slab seeds] curvature constant c of every seed (fused path)
     size_t cw_bytes;
     int fused_smem;
+    FieldMap field;              // field.B == nullptr: uniform field (the bz_tesla arguments)
+    double* bmax;                // device scalar: largest |B| of the map
     // device workspace
     double* wt;            // wire table [14][wt_cap]
     int32_t wt_cap;
@@ -123,10 +125,15 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     ctx->pair_max = (size_t)1 << 28;
     ctx->ck_max = (size_t)8 << 30;
     ctx->fused_smem = ((COMET_FUSED_WFIELDS + 1) * COMET_FUSED_WCAP + COMET_FUSED_WARPS * COMET_FUSED_TR * 3 * COMET_LANES) * (int)sizeof(double);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<false>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_fused<true>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+    {
+        const void* fk[4] = {(const void*)k_scan_fused<false, false>, (const void*)k_scan_fused<true, false>,
+                             (const void*)k_scan_fused<false, true>, (const void*)k_scan_fused<true, true>};
+        for (int j = 0; j < 4 && e == cudaSuccess; ++j) {
+            e = cudaFuncSetAttribute(fk[j], cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(fk[j], cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        }
+    }
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->bmax, sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int) * COMET_MAX_LANES);
     ctx->opt_lanes = COMET_DEFAULT_LANES;
     {
@@ -156,13 +163,19 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_select_classify, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        e = cudaFuncSetAttribute(k_select_classify<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_select_classify<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (COMET_MAX_STEPS_FIELD + 1) * 7 * (int)sizeof(double));
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_classify_seeds<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (COMET_MAX_STEPS_FIELD + 1) * 7 * (int)sizeof(double));
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(k_select_refs_cluster<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  COMET_REF_SMEM_MAX * (int)sizeof(double));
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_classify_seeds, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        e = cudaFuncSetAttribute(k_classify_seeds<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
     if (e != cudaSuccess) {
         cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats); cudaFree(ctx->n_items);
@@ -180,7 +193,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items);
     for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
-    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw);
+    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->bmax);
     for (int l = 0; l < COMET_MAX_LANES; ++l) {
         if (ctx->ls[l]) cudaStreamDestroy(ctx->ls[l]);
         if (ctx->lf[l]) cudaStreamDestroy(ctx->lf[l]);
@@ -313,6 +326,52 @@ static inline double* plane_T(void* track, int64_t n_seeds, int32_t n_steps)
     return (double*)track + track_row(n_chunks_of(n_seeds), track_rows(n_steps), 0);
 }
 
+// COMET_MAX_STEPS_FIELD (comet.h): the classification kernels hold 7 doubles per state in shared memory
+
+// |B| maximum of a field map -> *out (one CTA; runs once per comet_set_field)
+__global__ void __launch_bounds__(1024) k_field_bmax(const double* __restrict__ B, int64_t n_nodes, double* out)
+{
+    __shared__ double sm[32];
+    double m = 0.0;
+    for (int64_t i = threadIdx.x; i < n_nodes; i += blockDim.x) {
+        const double b0 = B[3 * i], b1 = B[3 * i + 1], b2 = B[3 * i + 2];
+        m = fmax(m, sqrt(b0 * b0 + b1 * b1 + b2 * b2));
+    }
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_down_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 32; ++w) m = fmax(m, sm[w]);
+        *out = m * 1.000001;
+    }
+}
+
+extern "C" int comet_set_field(comet_ctx* ctx, const double* field_dev, const int32_t* n_nodes, const double* origin_cm,
+                               const double* spacing_cm, double rkn_tol_cm, void* cuda_stream)
+{
+    if (!ctx) return COMET_EINVAL;
+    if (!field_dev) { ctx->field.B = nullptr; return COMET_OK; }
+    if (!n_nodes || !origin_cm || !spacing_cm || !(rkn_tol_cm > 0.0)) return COMET_EINVAL;
+    int64_t nodes = 1;
+    for (int a = 0; a < 3; ++a) {
+        if (n_nodes[a] < 2 || n_nodes[a] > 4096 || !(spacing_cm[a] > 0.0) || !isfinite(spacing_cm[a]) || !isfinite(origin_cm[a]))
+            return COMET_EINVAL;
+        nodes *= n_nodes[a];
+    }
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    FieldMap F;
+    F.B = field_dev;
+    for (int a = 0; a < 3; ++a) { F.n[a] = n_nodes[a]; F.o[a] = origin_cm[a]; F.d[a] = spacing_cm[a]; }
+    F.tol = rkn_tol_cm;
+    F.tol32 = rkn_tol_cm / 32.0;
+    F.bmax = ctx->bmax;
+    k_field_bmax<<<1, 1024, 0, (cudaStream_t)cuda_stream>>>(field_dev, nodes, ctx->bmax);
+    CU(ctx, cudaGetLastError());
+    ctx->field = F;
+    return COMET_OK;
+}
+
 static bool bad_physics(int32_t charge, double bz, double step, int32_t n_steps)
 {
     return (charge != 1 && charge != -1) || !isfinite(bz) || !(step > 0.0) || !isfinite(step) ||
@@ -326,6 +385,7 @@ extern "C" int comet_seed_extrapolate(comet_ctx* ctx, const double* seeds, int64
     if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
         !(r_stop_cm >= 0.0))
         return COMET_EINVAL;
+    if (ctx->field.B) return COMET_EINVAL;      // the materialised track is a uniform-field path (comet_set_field)
     if (n_seeds == 0) return COMET_OK;
     if (!seeds || !track || !n_pts) return COMET_EINVAL;
     int rc = set_device(ctx);
@@ -395,6 +455,7 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
         bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm))
         return COMET_EINVAL;
     if (n_seeds == 0) return COMET_OK;
+    if (ctx->field.B) return COMET_EINVAL;      // uniform-field path only (comet_set_field)
     if (!track || !n_pts || !seeds || !rss) return COMET_EINVAL;
     int rc = set_device(ctx);
     if (rc) return rc;
@@ -524,6 +585,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
         !(r_stop_cm >= 0.0) ||
         bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm))
         return COMET_EINVAL;
+    if (ctx->field.B && n_steps > COMET_MAX_STEPS_FIELD) return COMET_EINVAL;
     if (n_seeds == 0) return COMET_OK;
     if (!seeds || !rss) return COMET_EINVAL;
     int rc = set_device(ctx);
@@ -533,7 +595,8 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
     if (rc) return rc;
     const int64_t total_chunks = n_chunks_of(n_seeds);
     const int32_t n_ck = n_steps / COMET_FUSED_CK + 1;
-    const size_t ck_chunk = (size_t)n_ck * 6 * COMET_LANES * sizeof(double);
+    const bool field = ctx->field.B != nullptr;
+    const size_t ck_chunk = (size_t)n_ck * COMET_CK_FIELDS(field) * COMET_LANES * sizeof(double);
     // seed slabs bounded by the pair workspace and by the checkpoint workspace
     int64_t slab_chunks = total_chunks;
     if (n_fired > 0) {
@@ -583,7 +646,9 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             a.seeds = seeds + s0;
             a.stride = seed_stride;
             a.n_seeds = (n_seeds - s0 < nc * COMET_LANES) ? (n_seeds - s0) : nc * COMET_LANES;
-            a.qkb = COMET_KAPPA * (double)charge * bz_tesla;
+            a.qkb = field ? COMET_KAPPA * (double)charge : COMET_KAPPA * (double)charge * bz_tesla;
+            a.F = ctx->field;
+            a.h_min = step_cm / 64.0;
             a.hk = make_stepk_host(step_cm);
             a.n_steps = n_steps;
             a.r_stop2 = r_stop_cm * r_stop_cm;
@@ -615,14 +680,22 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
             if (tm) CU(ctx, cudaEventRecord(tev[0], st));
             const int thr = 32 * COMET_FUSED_WARPS;
-            if (a.stats) k_scan_fused<true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
-            else k_scan_fused<false><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+            if (field) {
+                if (a.stats) k_scan_fused<true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                else k_scan_fused<false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+            } else {
+                if (a.stats) k_scan_fused<true, false><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                else k_scan_fused<false, false><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+            }
             if (tm) CU(ctx, cudaEventRecord(tev[1], st));
             if (lanes > 1) {
                 CU(ctx, cudaEventRecord(ctx->ev_scan[l], s_scan));
                 CU(ctx, cudaStreamWaitEvent(s_fine, ctx->ev_scan[l], 0));
             }
-            if (n_fired > 0) k_fine_ck<<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
+            if (n_fired > 0) {
+                if (field) k_fine_ck<true><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
+                else k_fine_ck<false><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
+            }
             if (tm) CU(ctx, cudaEventRecord(tev[2], st));
             k_rss_sum<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_fine>>>(a.bd, a.SP, n_fired, a.n_seeds, rss + s0);
             if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }
@@ -663,6 +736,7 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
         bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm) ||
         n_part < 0 || n_part > COMET_MAX_PARTITIONS)
         return COMET_EINVAL;
+    if (ctx->field.B && n_steps > COMET_MAX_STEPS_FIELD) return COMET_EINVAL;
     if (n_part == 0) return COMET_OK;
     if (!part_off || !best_seed || !best_rss || (n_fired > 0 && !best_dca) || (n_hits > 0 && !cls)) return COMET_EINVAL;
     PartOff po;
@@ -698,8 +772,13 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     a.best_rss = best_rss;
     a.best_dca = best_dca;
     a.cls = cls;
-    const size_t smem = (size_t)(n_steps + 1) * 6 * sizeof(double);
-    k_select_classify<<<n_part, 256, smem, st>>>(a);
+    const bool field = ctx->field.B != nullptr;
+    if (field) a.qkb = COMET_KAPPA * (double)charge;
+    a.F = ctx->field;
+    a.h_min = step_cm / 64.0;
+    const size_t smem = (size_t)(n_steps + 1) * (field ? 7 : 6) * sizeof(double);
+    if (field) k_select_classify<true><<<n_part, 256, smem, st>>>(a);
+    else k_select_classify<false><<<n_part, 256, smem, st>>>(a);
     CU(ctx, cudaGetLastError());
     return COMET_OK;
 }
@@ -817,8 +896,13 @@ static int launch_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t se
     a.rho = rho;
     a.n_hits = n_hits;
     a.lambda = cutoff_cm;
-    const size_t smem = (size_t)(n_steps + 1) * 6 * sizeof(double);
-    k_classify_seeds<<<n_sel, 256, smem, st>>>(a, seed_idx, rss, dca, cls, seed_out, rss_out);
+    const bool field = ctx->field.B != nullptr;
+    if (field) a.qkb = COMET_KAPPA * (double)charge;
+    a.F = ctx->field;
+    a.h_min = step_cm / 64.0;
+    const size_t smem = (size_t)(n_steps + 1) * (field ? 7 : 6) * sizeof(double);
+    if (field) k_classify_seeds<true><<<n_sel, 256, smem, st>>>(a, seed_idx, rss, dca, cls, seed_out, rss_out);
+    else k_classify_seeds<false><<<n_sel, 256, smem, st>>>(a, seed_idx, rss, dca, cls, seed_out, rss_out);
     CU(ctx, cudaGetLastError());
     return COMET_OK;
 }
@@ -836,6 +920,7 @@ extern "C" int comet_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t
         !(r_stop_cm >= 0.0) || n_sel < 0 ||
         bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm))
         return COMET_EINVAL;
+    if (ctx->field.B && n_steps > COMET_MAX_STEPS_FIELD) return COMET_EINVAL;
     if (n_sel == 0) return COMET_OK;
     if (!seeds || !seed_idx || (n_fired > 0 && !dca) || (n_hits > 0 && !cls)) return COMET_EINVAL;
     int rc = set_device(ctx);

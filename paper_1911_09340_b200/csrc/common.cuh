@@ -180,6 +180,146 @@ __device__ __forceinline__ double fine_dca(State s, int kstar, int n_pts, double
     return (side >= 0.0) ? dist : -dist;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Inhomogeneous field map + adaptive step (readings R29-R32).
+// ---------------------------------------------------------------------------------------------
+struct FieldMap {
+    const double* B;        // [nx][ny][nz][3] Tesla, node (i,j,k) at o + (i dx, j dy, k dz); nullptr = uniform field
+    int32_t n[3];
+    double o[3], d[3];
+    double tol, tol32;      // step tolerance of R31 and tol / 32
+    const double* bmax;     // device scalar: largest |B| of the map (for the step-length bound of the pruning)
+};
+
+__device__ __forceinline__ double lerp1(double a, double b, double f) { return xadd(a, xmul(f, xsub(b, a))); }
+
+// R29: trilinear interpolation, z then y then x; outside the grid the edge value.
+__device__ __forceinline__ void field_at(const FieldMap& F, double x0, double x1, double x2,
+                                         double& b0, double& b1, double& b2)
+{
+    const double xs[3] = {x0, x1, x2};
+    int idx[3];
+    double f[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double t = xdiv(xsub(xs[a], F.o[a]), F.d[a]);
+        double fl = floor(t);
+        if (fl < 0.0) fl = 0.0;
+        if (fl > (double)(F.n[a] - 2)) fl = (double)(F.n[a] - 2);
+        idx[a] = (int)fl;
+        double fr = xsub(t, fl);
+        if (fr < 0.0) fr = 0.0;
+        if (fr > 1.0) fr = 1.0;
+        f[a] = fr;
+    }
+    double out[3];
+    const size_t sy = (size_t)F.n[2] * 3, sx = (size_t)F.n[1] * sy;
+    const double* p = F.B + (size_t)idx[0] * sx + (size_t)idx[1] * sy + (size_t)idx[2] * 3;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const double v00 = lerp1(__ldg(p + c), __ldg(p + c + 3), f[2]);
+        const double v01 = lerp1(__ldg(p + sy + c), __ldg(p + sy + c + 3), f[2]);
+        const double v10 = lerp1(__ldg(p + sx + c), __ldg(p + sx + c + 3), f[2]);
+        const double v11 = lerp1(__ldg(p + sx + sy + c), __ldg(p + sx + sy + c + 3), f[2]);
+        out[c] = lerp1(lerp1(v00, v01, f[1]), lerp1(v10, v11, f[1]), f[0]);
+    }
+    b0 = out[0]; b1 = out[1]; b2 = out[2];
+}
+
+// k = cq (T x B)
+__device__ __forceinline__ void lorentz_rhs(double t0, double t1, double t2, double b0, double b1, double b2,
+                                            double cq, double& k0, double& k1, double& k2)
+{
+    k0 = xmul(cq, xsub(xmul(t1, b2), xmul(t2, b1)));
+    k1 = xmul(cq, xsub(xmul(t2, b0), xmul(t0, b2)));
+    k2 = xmul(cq, xsub(xmul(t0, b1), xmul(t1, b0)));
+}
+
+// R30: one Nystrom RK4 step of signed length h in the field map; returns the error estimate EST.
+__device__ __forceinline__ double rkn4_field_step(State& s, double h, double cq, const FieldMap& F)
+{
+    const double hh = xmul(h, 0.5), h2 = xmul(h, h);
+    const double hh8 = xmul(h2, 0.125), hh2 = xmul(h2, 0.5), hh6 = div6(h2), h6 = div6(h);
+    const double x[3] = {s.x0, s.x1, s.x2}, T[3] = {s.t0, s.t1, s.t2};
+    double b0, b1, b2, k1[3], k2[3], k3[3], k4[3];
+    field_at(F, x[0], x[1], x[2], b0, b1, b2);
+    lorentz_rhs(T[0], T[1], T[2], b0, b1, b2, cq, k1[0], k1[1], k1[2]);
+    field_at(F, xadd(xadd(x[0], xmul(hh, T[0])), xmul(hh8, k1[0])), xadd(xadd(x[1], xmul(hh, T[1])), xmul(hh8, k1[1])),
+             xadd(xadd(x[2], xmul(hh, T[2])), xmul(hh8, k1[2])), b0, b1, b2);
+    lorentz_rhs(xadd(T[0], xmul(hh, k1[0])), xadd(T[1], xmul(hh, k1[1])), xadd(T[2], xmul(hh, k1[2])), b0, b1, b2, cq,
+                k2[0], k2[1], k2[2]);
+    lorentz_rhs(xadd(T[0], xmul(hh, k2[0])), xadd(T[1], xmul(hh, k2[1])), xadd(T[2], xmul(hh, k2[2])), b0, b1, b2, cq,
+                k3[0], k3[1], k3[2]);
+    field_at(F, xadd(xadd(x[0], xmul(h, T[0])), xmul(hh2, k3[0])), xadd(xadd(x[1], xmul(h, T[1])), xmul(hh2, k3[1])),
+             xadd(xadd(x[2], xmul(h, T[2])), xmul(hh2, k3[2])), b0, b1, b2);
+    lorentz_rhs(xadd(T[0], xmul(h, k3[0])), xadd(T[1], xmul(h, k3[1])), xadd(T[2], xmul(h, k3[2])), b0, b1, b2, cq,
+                k4[0], k4[1], k4[2]);
+    double est = 0.0, xn[3], tn[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) est = xadd(est, fabs(xadd(xsub(xsub(k1[i], k2[i]), k3[i]), k4[i])));
+    est = xmul(h2, est);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        xn[i] = xadd(xadd(x[i], xmul(h, T[i])), xmul(hh6, xadd(xadd(k1[i], k2[i]), k3[i])));
+        tn[i] = xadd(T[i], xmul(h6, xadd(fma(2.0, k3[i], fma(2.0, k2[i], k1[i])), k4[i])));
+    }
+    s.x0 = xn[0]; s.x1 = xn[1]; s.x2 = xn[2];
+    s.t0 = tn[0]; s.t1 = tn[1]; s.t2 = tn[2];
+    return est;
+}
+
+// R31: one recorded step with the adaptive step control.  `h` is the trial step on entry and the next trial
+// step on exit; returns the length of the step taken.
+__device__ __forceinline__ double adaptive_field_step(State& s, double& h, double h_max, double h_min, double cq,
+                                                      const FieldMap& F)
+{
+    State t;
+    double est;
+    for (;;) {
+        t = s;
+        est = rkn4_field_step(t, h, cq, F);
+        if (est > F.tol && h > h_min) { h = xmul(h, 0.5); continue; }
+        break;
+    }
+    s = t;
+    const double used = h;
+    if (est < F.tol32 && h < h_max) h = xmul(2.0, h);
+    return used;
+}
+
+// O6 + O7 in the field map: the bracket [lo, hi] is given by the recorded steps around k* (R32).
+__device__ __forceinline__ double fine_dca_field(State s, double lo, double hi, double cq, const FieldMap& F,
+                                                 const WireLine& wl)
+{
+    double sigma = 0.0;
+#pragma unroll 1
+    for (int it = 0; it < COMET_MAX_ITER; ++it) {
+        const double tw = xdot3(s.t0, s.t1, s.t2, wl.w0, wl.w1, wl.w2);
+        const double n0 = xsub(s.t0, xmul(tw, wl.w0));
+        const double n1 = xsub(s.t1, xmul(tw, wl.w1));
+        const double n2 = xsub(s.t2, xmul(tw, wl.w2));
+        const double den = xdot3(s.t0, s.t1, s.t2, n0, n1, n2);
+        if (den < COMET_DEN_MIN) break;
+        const double mx0 = xsub(wl.m0, s.x0), mx1 = xsub(wl.m1, s.x1), mx2 = xsub(wl.m2, s.x2);
+        double delta = xdiv(xdot3(mx0, mx1, mx2, n0, n1, n2), den);
+        double target = xadd(sigma, delta);
+        if (target < lo) target = lo;
+        if (target > hi) target = hi;
+        delta = xsub(target, sigma);
+        if (fabs(delta) < COMET_TOL_CM) break;
+        (void)rkn4_field_step(s, delta, cq, F);
+        sigma = xadd(sigma, delta);
+    }
+    double u0, u1, u2;
+    const double d2 = perp2_exact(s.x0, s.x1, s.x2, wl, u0, u1, u2);
+    const double c0 = xsub(xmul(s.t1, wl.w2), xmul(s.t2, wl.w1));
+    const double c1 = xsub(xmul(s.t2, wl.w0), xmul(s.t0, wl.w2));
+    const double c2 = xsub(xmul(s.t0, wl.w1), xmul(s.t1, wl.w0));
+    const double side = xdot3(u0, u1, u2, c0, c1, c2);
+    const double dist = xsqrt(d2);
+    return (side >= 0.0) ? dist : -dist;
+}
+
 // O8: bounded residual of one wire; *jstar = lowest entry index attaining the minimum (-1: none).
 __device__ __forceinline__ double wire_residual(double D, const double* __restrict__ rho, int j0, int j1,
                                                 double lambda, int* jstar, double* rmin_out)

@@ -196,6 +196,7 @@ k_refine_seeds(const double* __restrict__ seeds, int64_t stride, const int64_t* 
 }
 
 // One CTA per listed seed: classification of PAPER.md:83 (classify_cta), the seed itself and its RSS.
+template <bool FIELD>
 __global__ void __launch_bounds__(256)
 k_classify_seeds(const ClassifyArgs a, const int64_t* __restrict__ seed_idx, const double* __restrict__ rss,
                  double* __restrict__ dca, uint8_t* __restrict__ cls, double* __restrict__ seed_out,
@@ -206,7 +207,7 @@ k_classify_seeds(const ClassifyArgs a, const int64_t* __restrict__ seed_idx, con
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
     if (threadIdx.x < 6 && seed_out) seed_out[(size_t)blockIdx.x * 6 + threadIdx.x] = (idx >= 0) ? a.seeds[threadIdx.x * a.stride + idx] : qnan;
     if (threadIdx.x == 0 && rss_out) rss_out[blockIdx.x] = (idx >= 0 && rss) ? rss[idx] : qnan;
-    classify_cta(a, idx, dca + (size_t)blockIdx.x * a.W, cls + (size_t)blockIdx.x * a.n_hits, sm);
+    classify_cta<FIELD>(a, idx, dca + (size_t)blockIdx.x * a.W, cls + (size_t)blockIdx.x * a.n_hits, sm);
 }
 
 }  // namespace comet

@@ -92,7 +92,10 @@ struct FusedArgs {
     unsigned long long* items;
     unsigned int* n_items;
     unsigned long long* stats;
+    FieldMap F;              // field-map variants (FIELD = true): the map, and qkb = kappa q, hk.h = h_max
+    double h_min;            // h_max / 64 (R31)
 };
+#define COMET_CK_FIELDS(FIELD) ((FIELD) ? 7 : 6)    // checkpoint row: x, T and, in a field map, the trial step
 
 // shortlist constants of wire i: from the CTA's table when it holds the wire, else from the wire table
 // in global memory (warp-uniform or lane-contiguous addresses either way)
@@ -114,9 +117,10 @@ __device__ __forceinline__ double wire_slope(double e1z, double e2z)
     return (double)__fsqrt_ru(__double2float_ru(fma(e1z, e1z, e2z * e2z)));
 }
 
-template <bool STATS>
+template <bool STATS, bool FIELD>
 __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
 {
+    constexpr int CKF = COMET_CK_FIELDS(FIELD);
     constexpr int TR = COMET_FUSED_TR, CK = COMET_FUSED_CK, ROW = 3 * COMET_LANES;
     constexpr int FM1 = COMET_FUSED_M1;
     constexpr int NSUB = TR / FM1;
@@ -153,8 +157,10 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
         st.x0 = st.x1 = st.x2 = 0.0;
         st.t0 = st.t1 = st.t2 = 0.0;
     }
-    const bool lip_ok = fabs(c) * h <= COMET_CH_MAX;
+    // states are at most 1.001 h apart when |curvature| h <= 0.05 (in a map: with its largest |B| and h = h_max)
+    const bool lip_ok = (FIELD ? fabs(c) * __ldg(a.F.bmax) * h : fabs(c) * h) <= COMET_CH_MAX;
     const unsigned nolip_mask = __ballot_sync(FULL, valid && !lip_ok);
+    double htry = h;                                        // FIELD: trial step of the adaptive control (R31)
     bool active = valid;
     int32_t np = valid ? a.n_steps + 1 : 0;
     const bool use_stop = a.r_stop2 > 0.0;
@@ -164,7 +170,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
     for (int i = 0; i < W; ++i) keys[(size_t)i * a.SP + s] = COMET_KEY_NONE;
 
     const int n_rounds = (W + 31) / 32;                     // level 0: wire i = r * 32 + lane
-    double* ckc = a.ck + (size_t)chunk * a.n_ck * (6 * COMET_LANES) + lane;
+    double* ckc = a.ck + (size_t)chunk * a.n_ck * (CKF * COMET_LANES) + lane;
     const int n_tiles = (a.n_steps + TR) / TR;              // rows 0 .. n_steps
     unsigned long long st_cnt[ST_N];                        // work counters (COMET_OPT_STATS), thread-level
     if (STATS) {
@@ -188,15 +194,17 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
         for (int rr = 0; rr < TR; ++rr) {
             const int k = r0 + rr;
             if (k > 0 && active) {
-                rkn4_step(st, a.hk, c);
+                if (FIELD) (void)adaptive_field_step(st, htry, h, a.h_min, c, a.F);
+                else rkn4_step(st, a.hk, c);
                 if (use_stop && in_target_region(st, a.r_stop2)) { np = k + 1; active = false; }
             }
             if (k >= a.n_steps) active = false;
             double* tr = tile + rr * ROW + lane;
             tr[0] = st.x0; tr[32] = st.x1; tr[64] = st.x2;
             if ((rr & (CK - 1)) == 0 && k <= a.n_steps) {
-                double* o = ckc + (size_t)(k / CK) * (6 * COMET_LANES);
+                double* o = ckc + (size_t)(k / CK) * (CKF * COMET_LANES);
                 o[0] = st.x0; o[32] = st.x1; o[64] = st.x2; o[96] = st.t0; o[128] = st.t1; o[160] = st.t2;
+                if (FIELD) o[192] = htry;
             }
         }
         __syncwarp();
@@ -357,9 +365,11 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
 
 // Persistent warps over the work list: exact decision between bk-1, bk, bk+1 on states regenerated
 // from the nearest checkpoint at or before bk-1, then O6..O8 (common.cuh).
+template <bool FIELD>
 __global__ void __launch_bounds__(COMET_FINE_THREADS, COMET_FINE_MINB) k_fine_ck(const FusedArgs a)
 {
     constexpr int CK = COMET_FUSED_CK;
+    constexpr int CKF = COMET_CK_FIELDS(FIELD);
     const int lane = threadIdx.x & 31;
     const unsigned n_items = *a.n_items;
     const unsigned n_warps = gridDim.x * (COMET_FINE_THREADS / 32);
@@ -381,21 +391,47 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, COMET_FINE_MINB) k_fine_ck
             wl.m0 = __ldg(a.wt + i); wl.m1 = __ldg(a.wt + W + i); wl.m2 = __ldg(a.wt + 2 * W + i);
             wl.w0 = __ldg(a.wt + 3 * W + i); wl.w1 = __ldg(a.wt + 4 * W + i); wl.w2 = __ldg(a.wt + 5 * W + i);
             const int ka = max(bk - 1, 0), kz = min(bk + 1, np - 1);
-            const int kc = ka & ~(CK - 1);
-            const double* o = a.ck + ((size_t)chunk * a.n_ck + (size_t)(kc / CK)) * (6 * COMET_LANES) + lane;
-            State st;
-            st.x0 = o[0]; st.x1 = o[32]; st.x2 = o[64]; st.t0 = o[96]; st.t1 = o[128]; st.t2 = o[160];
-            for (int k = kc; k < ka; ++k) rkn4_step(st, a.hk, c);
-            State bs = st;
-            int ks = ka;
-            double bd = 0.0;
-            for (int k = ka; k <= kz; ++k) {
-                double u0, u1, u2;
-                const double d2 = perp2_exact(st.x0, st.x1, st.x2, wl, u0, u1, u2);
-                if (k == ka || d2 < bd) { bd = d2; ks = k; bs = st; }
-                if (k < kz) rkn4_step(st, a.hk, c);
+            double D;
+            if (FIELD) {
+                // replay the adaptive recording from the checkpoint at or before ka - 1 up to kz + 1: the
+                // candidates ka..kz with the lengths of the recorded steps into and out of them (R32)
+                const int kc = max(ka - 1, 0) & ~(CK - 1);
+                const double* o = a.ck + ((size_t)chunk * a.n_ck + (size_t)(kc / CK)) * (CKF * COMET_LANES) + lane;
+                State st;
+                st.x0 = o[0]; st.x1 = o[32]; st.x2 = o[64]; st.t0 = o[96]; st.t1 = o[128]; st.t2 = o[160];
+                double h = o[192], h_in = 0.0, bs_in = 0.0, bs_out = 0.0, bd = 0.0;
+                State bs = st;
+                int ks = ka;
+                for (int k = kc;; ++k) {
+                    if (k >= ka && k <= kz) {
+                        double u0, u1, u2;
+                        const double d2 = perp2_exact(st.x0, st.x1, st.x2, wl, u0, u1, u2);
+                        if (k == ka || d2 < bd) { bd = d2; ks = k; bs = st; bs_in = h_in; }
+                    }
+                    if (k > kz || k >= np - 1) break;
+                    const double used = adaptive_field_step(st, h, a.hk.h, a.h_min, c, a.F);
+                    if (ks == k && k >= ka) bs_out = used;
+                    h_in = used;
+                }
+                const double lo = (ks > 0) ? -bs_in : 0.0, hi = (ks < np - 1) ? bs_out : 0.0;
+                D = fine_dca_field(bs, lo, hi, c, a.F, wl);
+            } else {
+                const int kc = ka & ~(CK - 1);
+                const double* o = a.ck + ((size_t)chunk * a.n_ck + (size_t)(kc / CK)) * (CKF * COMET_LANES) + lane;
+                State st;
+                st.x0 = o[0]; st.x1 = o[32]; st.x2 = o[64]; st.t0 = o[96]; st.t1 = o[128]; st.t2 = o[160];
+                for (int k = kc; k < ka; ++k) rkn4_step(st, a.hk, c);
+                State bs = st;
+                int ks = ka;
+                double bd = 0.0;
+                for (int k = ka; k <= kz; ++k) {
+                    double u0, u1, u2;
+                    const double d2 = perp2_exact(st.x0, st.x1, st.x2, wl, u0, u1, u2);
+                    if (k == ka || d2 < bd) { bd = d2; ks = k; bs = st; }
+                    if (k < kz) rkn4_step(st, a.hk, c);
+                }
+                D = fine_dca(bs, ks, np, a.hk.h, c, wl);
             }
-            const double D = fine_dca(bs, ks, np, a.hk.h, c, wl);
             const double e = wire_residual(D, a.rho, __ldg(a.hit_off + i), __ldg(a.hit_off + i + 1), a.lambda,
                                            nullptr, nullptr);
             e2 = xmul(e, e);

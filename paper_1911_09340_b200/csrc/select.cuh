@@ -72,14 +72,18 @@ struct ClassifyArgs {
     double* best_rss;
     double* best_dca;
     uint8_t* cls;
+    FieldMap F;                // field-map variants: the map; qkb = kappa q, hk.h = h_max
+    double h_min;
 };
 
 // CTA-wide: re-extrapolate seed `idx` into shared memory (state k at sm[k*6..]), then one thread per fired
 // wire does O5..O8 + O11 in exact arithmetic: dca[i] = signed D, cls[j] = 1 for the classified entries
 // (all other entries 0).  idx < 0: NaN / zeros.
+template <bool FIELD>
 __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx, double* __restrict__ dca,
                                              uint8_t* __restrict__ cls, double* sm)
 {
+    constexpr int RS = FIELD ? 7 : 6;                   // row: x, T and, in a field map, the step leaving the state
     __shared__ int32_t s_np;
     __shared__ double s_c;
     for (int j = threadIdx.x; j < a.n_hits; j += blockDim.x) cls[j] = 0;
@@ -94,9 +98,11 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
         s_c = c;
         int32_t np = a.n_steps + 1;
         sm[0] = st.x0; sm[1] = st.x1; sm[2] = st.x2; sm[3] = st.t0; sm[4] = st.t1; sm[5] = st.t2;
+        double htry = a.hk.h;
         for (int32_t k = 1; k <= a.n_steps; ++k) {
-            rkn4_step(st, a.hk, c);
-            double* o = sm + (size_t)k * 6;
+            if (FIELD) sm[(size_t)(k - 1) * RS + 6] = adaptive_field_step(st, htry, a.hk.h, a.h_min, c, a.F);
+            else rkn4_step(st, a.hk, c);
+            double* o = sm + (size_t)k * RS;
             o[0] = st.x0; o[1] = st.x1; o[2] = st.x2; o[3] = st.t0; o[4] = st.t1; o[5] = st.t2;
             if (a.r_stop2 > 0.0 && in_target_region(st, a.r_stop2)) { np = k + 1; break; }
         }
@@ -113,13 +119,19 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
         double bd = 0.0;
         for (int k = 0; k < np; ++k) {
             double u0, u1, u2;
-            const double d2 = perp2_exact(sm[k * 6], sm[k * 6 + 1], sm[k * 6 + 2], wl, u0, u1, u2);
+            const double d2 = perp2_exact(sm[k * RS], sm[k * RS + 1], sm[k * RS + 2], wl, u0, u1, u2);
             if (k == 0 || d2 < bd) { bd = d2; ks = k; }
         }
         State st;
-        st.x0 = sm[ks * 6]; st.x1 = sm[ks * 6 + 1]; st.x2 = sm[ks * 6 + 2];
-        st.t0 = sm[ks * 6 + 3]; st.t1 = sm[ks * 6 + 4]; st.t2 = sm[ks * 6 + 5];
-        const double D = fine_dca(st, ks, np, a.hk.h, c, wl);
+        st.x0 = sm[ks * RS]; st.x1 = sm[ks * RS + 1]; st.x2 = sm[ks * RS + 2];
+        st.t0 = sm[ks * RS + 3]; st.t1 = sm[ks * RS + 4]; st.t2 = sm[ks * RS + 5];
+        double D;
+        if (FIELD) {
+            const double lo = (ks > 0) ? -sm[(ks - 1) * RS + 6] : 0.0, hi = (ks < np - 1) ? sm[ks * RS + 6] : 0.0;
+            D = fine_dca_field(st, lo, hi, c, a.F, wl);
+        } else {
+            D = fine_dca(st, ks, np, a.hk.h, c, wl);
+        }
         dca[i] = D;
         int js;
         double rmin;
@@ -129,6 +141,7 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
 }
 
 // One CTA per partition: finish the argmin, then classify the winning seed.
+template <bool FIELD>
 __global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
 {
     extern __shared__ __align__(16) double sm[];       // [(n_steps+1)][6]
@@ -144,7 +157,7 @@ __global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
         a.best_rss[p] = (idx >= 0) ? v : __longlong_as_double(0x7ff8000000000000LL);
     }
     __syncthreads();
-    classify_cta(a, s_best, a.best_dca + (size_t)p * a.W, a.cls + (size_t)p * a.n_hits, sm);
+    classify_cta<FIELD>(a, s_best, a.best_dca + (size_t)p * a.W, a.cls + (size_t)p * a.n_hits, sm);
 }
 
 }  // namespace comet

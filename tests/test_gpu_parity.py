@@ -757,3 +757,114 @@ def test_refinement_argument_errors(comet, cfg0_event):
     with pytest.raises(CometError):          # an empty partition
         comet.scan_stage(d.seeds, [0, 0, seeds.shape[1]], *d.phys(), ev.r_stop, *d.hits(), ev.cutoff,
                          half_width=[1, 1, 1, 1], n_grid=[2, 2, 2, 2], n_iter=1, shrink=0.5, k_ref=2, k_final=2)
+
+
+# ------------------------------------------------------------------------------------------------
+# inhomogeneous field map + adaptive step (comet_set_field): bit-identical to the oracle's field path
+# ------------------------------------------------------------------------------------------------
+@pytest.fixture()
+def field_comet():
+    from paper_1911_09340_b200 import Comet
+    c = Comet(0)
+    yield c
+    c.close()
+
+
+def _set_map(c, F, tol):
+    B, o, d = F
+    t = _dev(B)
+    c.set_field(t, o, d, tol)
+    return t
+
+
+@pytest.mark.parametrize("tol", [1e-5, 1e-7, 1e-9])
+def test_field_scan_matches_oracle_cfg0(field_comet, cfg0_event, tol):
+    from comet_synth import solenoid_map
+    c, ev = field_comet, cfg0_event
+    seeds, po = event_seeds(ev)
+    seeds = np.ascontiguousarray(seeds[:, :2048 + 19])
+    seeds[2, 1000:] += 40.0                       # part of the seeds start near the end plate, where the steps halve
+    d = DevEvent(ev, seeds)
+    F = solenoid_map()
+    _set_map(c, F, tol)
+    out = c.scan_rss(d.seeds, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    torch.cuda.synchronize()
+    ref = O.scan_field(seeds, ev.charge, F, ev.step, ev.n_steps, ev.r_stop, tol, ev.geom.wire_a, ev.geom.wire_b,
+                       ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, want_npts=True)
+    np.testing.assert_array_equal(out["n_pts"].cpu().numpy(), ref["n_pts"])
+    assert np.array_equal(out["rss"].cpu().numpy(), ref["rss"])
+    tr, npt, hs = O.extrapolate_field(seeds[:, 1500:1600], ev.charge, F, ev.step, ev.n_steps, ev.r_stop, tol)
+    if tol < 1e-6:
+        assert np.nanmin(hs) < ev.step            # the case does exercise the step control
+
+
+def test_field_uniform_map_equals_uniform_path(field_comet, cfg0_event):
+    from comet_synth import uniform_map
+    c, ev = field_comet, cfg0_event
+    seeds, po = event_seeds(ev, shape=(4, 4, 4, 4))
+    d = DevEvent(ev, seeds)
+    a = c.scan_rss(d.seeds, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    rss_u, np_u = a["rss"].clone(), a["n_pts"].clone()
+    keep = _set_map(c, uniform_map(ev.bz), 1e-3)
+    b = c.scan_rss(d.seeds, ev.charge, 123.0, ev.step, ev.n_steps, ev.r_stop, *d.hits(), ev.cutoff)   # bz ignored
+    torch.cuda.synchronize()
+    assert torch.equal(np_u, b["n_pts"])
+    np.testing.assert_allclose(b["rss"].cpu().numpy(), rss_u.cpu().numpy(), rtol=1e-9)
+    # the materialised track is a uniform-field path
+    from paper_1911_09340_b200 import CometError
+    with pytest.raises(CometError):
+        c.seed_extrapolate(d.seeds, *d.phys(), ev.r_stop)
+    c.set_field(None)
+    c.seed_extrapolate(d.seeds, *d.phys(), ev.r_stop)
+    del keep
+
+
+def test_field_classify_and_stage_match_oracle(field_comet, cfg0_event):
+    from comet_synth import solenoid_map
+    c, ev = field_comet, cfg0_event
+    seeds, po = event_seeds(ev, shape=(6, 4, 4, 4))
+    d = DevEvent(ev, seeds)
+    F, tol = solenoid_map(), 1e-7
+    keep = _set_map(c, F, tol)
+    fargs = (ev.charge, F, ev.step, ev.n_steps, ev.r_stop, tol, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire,
+             ev.hit_off, ev.rho, ev.cutoff)
+    idx = np.array([0, 17, -1, seeds.shape[1] - 1], dtype=np.int64)
+    got = c.classify_seeds(d.seeds, _dev(idx), *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    ref = O.classify_seeds_field(seeds, idx, *fargs)
+    ref["dca"][2] = np.nan
+    np.testing.assert_array_equal(got["dca"].cpu().numpy(), ref["dca"])
+    np.testing.assert_array_equal(got["cls"].cpu().numpy(), ref["cls"])
+    # whole path A + B + C
+    out = c.scan_event(d.seeds, po, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    rs = O.scan_field(seeds, *fargs)["rss"]
+    best = int(np.argmin(rs))
+    assert np.array_equal(out["rss"].cpu().numpy(), rs)
+    assert out["best_seed"].cpu().tolist() == [best]
+    np.testing.assert_array_equal(out["cls"].cpu().numpy()[0], O.classify_seeds_field(seeds, [best], *fargs)["cls"][0])
+    # a stage with two refinements
+    kw = dict(half_width=[1.2, 1.0, 1.0, 4.0], n_grid=[3, 3, 3, 3], n_iter=2, shrink=0.5, k_ref=3, k_final=4)
+    so = c.scan_stage(d.seeds, po, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, **kw)
+    torch.cuda.synchronize()
+    sr = O.scan_stage(seeds, po, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a, ev.geom.wire_b,
+                      ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, field=F, rkn_tol=tol, **kw)
+    np.testing.assert_array_equal(so["final_seed"].cpu().numpy(), sr["final_seed"])
+    np.testing.assert_array_equal(so["final_rss"].cpu().numpy(), sr["final_rss"])
+    np.testing.assert_array_equal(so["cls"].cpu().numpy(), sr["cls"])
+    del keep
+
+
+def test_field_scan_cfg1_ragged_three_partitions(field_comet, cfg1_event):
+    from comet_synth import solenoid_map
+    c, ev = field_comet, cfg1_event
+    seeds, _ = event_seeds(ev)
+    seeds = np.ascontiguousarray(seeds[:, ::97])
+    d = DevEvent(ev, seeds)
+    F, tol = solenoid_map(), 1e-8
+    keep = _set_map(c, F, tol)
+    out = c.scan_rss(d.seeds, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    torch.cuda.synchronize()
+    ref = O.scan_field(seeds, ev.charge, F, ev.step, ev.n_steps, ev.r_stop, tol, ev.geom.wire_a, ev.geom.wire_b,
+                       ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, want_npts=True)
+    np.testing.assert_array_equal(out["n_pts"].cpu().numpy(), ref["n_pts"])
+    assert np.array_equal(out["rss"].cpu().numpy(), ref["rss"])
+    del keep
