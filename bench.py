@@ -43,6 +43,9 @@ GEN_INSTR = 48
 # refinement recipe of the `stage` entry (R26): box half widths about one step of the configs[1] grid
 STAGE_HALF_WIDTH = [0.6, 0.5, 0.5, 1.0]
 STAGE_GRID = [5, 5, 5, 5]
+# `field` entry: step tolerance of R31 and the FP64-pipe instructions of one attempted Nystrom step in the map
+FIELD_TOL = 1e-7
+FIELD_STEP_INSTR = 420
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1d_full_scan_fused_fine_ck.txt)
 TRAFFIC_BYTES = {"k_scan_fused": 347658496 + 2243479000, "k_fine_ck": 681160960 + 80465000}
 
@@ -316,6 +319,31 @@ def run_ours(args):
                            "grid %s per reference, 10 finally selected seeds per partition classified" % (STAGE_HALF_WIDTH, STAGE_GRID)}
         del swork, so
 
+    # ---- the same event in an inhomogeneous field map with the adaptive step (R29-R32) ----
+    field = None
+    if fused and args.field:
+        from comet_synth import solenoid_map
+        fB, fo, fd = solenoid_map()
+        d_map = dev(fB)
+        c.set_field(d_map, fo, fd, FIELD_TOL)
+        step_fused()
+        ms_field, fo_out = _time_steps(step_fused, max(2, n_cmp // 2), stream)
+        st_field = float(n_pts.sum().item())
+        c.set_option(OPT_TIMING, 1)
+        _time_steps(step_fused, 2, stream)
+        kt_field = c.read_timing(knames)
+        c.set_option(OPT_TIMING, 0)
+        c.set_field(None)
+        field = {"ms_per_step": ms_field, "dca_evals_per_s": pairs / (ms_field * 1e-3), "rkn_tol_cm": FIELD_TOL,
+                 "recorded_states_per_seed": st_field / S, "kernels_serial_ms": kt_field,
+                 "best_seed": fo_out["best_seed"].cpu().numpy().tolist(),
+                 "map": "comet_synth.solenoid_map(): %s nodes, %.0f cm spacing, B_z falling off towards the end plates"
+                        % ("x".join(str(v) for v in fB.shape[:3]), fd[0]),
+                 "fp64_model": "about %d FP64-pipe instructions per attempted step (3 trilinear look-ups of 3 components, "
+                               "4 cross products, error estimate)" % FIELD_STEP_INSTR,
+                 "k_scan_fused_tflops_model": 2.0 * FIELD_STEP_INSTR * st_field / (kt_field["k_scan_fused"] * 1e-3) / 1e12}
+        del d_map
+
     # ---- e2e: host buffers through comet_scan_event_host -------------------------------------
     pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
     h = dict(seeds=pin(seeds, torch.float64), wa=pin(ev.geom.wire_a, torch.float64), wb=pin(ev.geom.wire_b, torch.float64),
@@ -420,6 +448,7 @@ def run_ours(args):
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
         "stage": stage,
+        "field": field,
         "roofline": {"kernel": top["kernel"], "bound": "alu", "achieved": top["achieved"], "peak": peak,
                      "unit": "TFLOP/s", "frac": top["achieved"] / peak, "traffic": top["traffic"],
                      "timed": top["timed"],
@@ -454,6 +483,7 @@ def main():
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--path", choices=["fused", "materialised"], default="fused")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    ap.add_argument("--no-field", dest="field", action="store_false", help="skip the field-map leg")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -365,8 +365,11 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
 
 // Persistent warps over the work list: exact decision between bk-1, bk, bk+1 on states regenerated
 // from the nearest checkpoint at or before bk-1, then O6..O8 (common.cuh).
+#ifndef COMET_FINE_MINB_FIELD
+#define COMET_FINE_MINB_FIELD 2    // the field-map variant needs ~2x the registers (three field look-ups per step)
+#endif
 template <bool FIELD>
-__global__ void __launch_bounds__(COMET_FINE_THREADS, COMET_FINE_MINB) k_fine_ck(const FusedArgs a)
+__global__ void __launch_bounds__(COMET_FINE_THREADS, FIELD ? COMET_FINE_MINB_FIELD : COMET_FINE_MINB) k_fine_ck(const FusedArgs a)
 {
     constexpr int CK = COMET_FUSED_CK;
     constexpr int CKF = COMET_CK_FIELDS(FIELD);
