@@ -868,3 +868,33 @@ def test_field_scan_cfg1_ragged_three_partitions(field_comet, cfg1_event):
     np.testing.assert_array_equal(out["n_pts"].cpu().numpy(), ref["n_pts"])
     assert np.array_equal(out["rss"].cpu().numpy(), ref["rss"])
     del keep
+
+
+def test_scan_path_is_capturable_in_a_cuda_graph(comet, cfg1_event):
+    """comet_scan_rss forks into the ctx's internal streams and joins them with events, and nothing on the hot
+    path allocates or synchronises: the whole A + B + C sequence can be captured once and replayed."""
+    ev = cfg1_event
+    seeds, po = event_seeds(ev)
+    seeds = np.ascontiguousarray(seeds[:, :4 * 4 * 148 * 32])
+    po = [0, seeds.shape[1]]
+    d = DevEvent(ev, seeds)
+    S = seeds.shape[1]
+    rss = torch.empty(S, dtype=torch.float64, device="cuda")
+    n_pts = torch.empty(S, dtype=torch.int32, device="cuda")
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        comet.scan_rss(d.seeds, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, rss=rss, n_pts=n_pts, stream=st)   # grows the workspace
+        ref = comet.select_and_classify(d.seeds, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, rss, po, stream=st)
+    st.synchronize()
+    rss_ref, best_ref, cls_ref = rss.clone(), ref["best_seed"].clone(), ref["cls"].clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=st):
+        comet.scan_rss(d.seeds, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, rss=rss, n_pts=n_pts, stream=st)
+        out = comet.select_and_classify(d.seeds, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, rss, po, stream=st)
+    for _ in range(2):
+        rss.zero_()
+        out["cls"].zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(rss, rss_ref)
+        assert torch.equal(out["best_seed"], best_ref) and torch.equal(out["cls"], cls_ref)
