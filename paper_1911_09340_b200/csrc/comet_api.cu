@@ -594,7 +594,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
     rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
     if (rc) return rc;
     const int64_t total_chunks = n_chunks_of(n_seeds);
-    const int32_t n_ck = n_steps / COMET_FUSED_CK + 1;
+    const int32_t n_ck = n_steps / COMET_CK_ROWS(ctx->field.B != nullptr) + 1;
     const bool field = ctx->field.B != nullptr;
     const size_t ck_chunk = (size_t)n_ck * COMET_CK_FIELDS(field) * COMET_LANES * sizeof(double);
     // seed slabs bounded by the pair workspace and by the checkpoint workspace
@@ -625,7 +625,8 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
     // joins them again with events: the call stays asynchronous and capturable.  Per-kernel timing
     // (COMET_OPT_TIMING) and the work counters run one lane on the caller's stream.
     const bool tm = ctx->opt_timing != 0;
-    const int lanes_opt = (tm || ctx->opt_stats) ? 1 : ctx->opt_lanes;
+    // (in a field map the sub-slab kernels gain nothing from sharing the SMs: one lane)
+    const int lanes_opt = (tm || ctx->opt_stats || field) ? 1 : ctx->opt_lanes;
     for (int64_t c0 = 0; c0 < total_chunks; c0 += slab_chunks) {
         const int64_t nc_slab = (total_chunks - c0 < slab_chunks) ? (total_chunks - c0) : slab_chunks;
         // sub-slabs of whole CTAs, at least two CTAs per SM each

@@ -96,6 +96,10 @@ struct FusedArgs {
     double h_min;            // h_max / 64 (R31)
 };
 #define COMET_CK_FIELDS(FIELD) ((FIELD) ? 7 : 6)    // checkpoint row: x, T and, in a field map, the trial step
+#ifndef COMET_FUSED_CK_FIELD
+#define COMET_FUSED_CK_FIELD 4     // rows between checkpoints in a field map (1 and 2 were measured: the extra checkpoint traffic costs what the shorter replay saves)
+#endif
+#define COMET_CK_ROWS(FIELD) ((FIELD) ? COMET_FUSED_CK_FIELD : COMET_FUSED_CK)
 
 // shortlist constants of wire i: from the CTA's table when it holds the wire, else from the wire table
 // in global memory (warp-uniform or lane-contiguous addresses either way)
@@ -121,7 +125,7 @@ template <bool STATS, bool FIELD>
 __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
 {
     constexpr int CKF = COMET_CK_FIELDS(FIELD);
-    constexpr int TR = COMET_FUSED_TR, CK = COMET_FUSED_CK, ROW = 3 * COMET_LANES;
+    constexpr int TR = COMET_FUSED_TR, CK = COMET_CK_ROWS(FIELD), ROW = 3 * COMET_LANES;
     constexpr int FM1 = COMET_FUSED_M1;
     constexpr int NSUB = TR / FM1;
     constexpr int WCAP = COMET_FUSED_WCAP;
@@ -371,7 +375,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
 template <bool FIELD>
 __global__ void __launch_bounds__(COMET_FINE_THREADS, FIELD ? COMET_FINE_MINB_FIELD : COMET_FINE_MINB) k_fine_ck(const FusedArgs a)
 {
-    constexpr int CK = COMET_FUSED_CK;
+    constexpr int CK = COMET_CK_ROWS(FIELD);
     constexpr int CKF = COMET_CK_FIELDS(FIELD);
     const int lane = threadIdx.x & 31;
     const unsigned n_items = *a.n_items;
