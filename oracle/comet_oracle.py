@@ -284,3 +284,61 @@ def classify_seeds_field(seeds, idx, charge, field, h_max, n_steps, r_stop, tol,
                                       float(r_stop), float(tol), wire_a, wire_b, wire_a.shape[1], fired_wire,
                                       hit_off, rho, W, H, float(cutoff), idx, idx.size, dca, cls)
     return {"dca": dca, "cls": cls}
+
+
+# ---- sequential stages with hit removal (readings R33-R34) ---------------------------
+def remove_hits(fired_wire, hit_off, rho, cls):
+    """"The hits classified previously were excluded in the seed scanning; therefore, the number of wires
+    gets reduced whenever a track is fitted".  A measured hit is the adjacent pair of ghost
+    entries (2m, 2m+1) (R12, R33): an entry goes when it or its partner is classified; a wire left without
+    entries goes too.  -> (fired_wire, hit_off, rho, src) with src[j'] = old index of kept entry j'."""
+    fired_wire, hit_off, rho = np.asarray(fired_wire), np.asarray(hit_off), np.asarray(rho)
+    cls = np.asarray(cls).astype(bool)
+    H = rho.shape[0]
+    assert H % 2 == 0 and np.all(hit_off % 2 == 0)
+    new_fw, new_off, new_rho, src = [], [0], [], []
+    for i in range(fired_wire.shape[0]):                 # plain loops: wire by wire, entry by entry
+        kept = []
+        for j in range(hit_off[i], hit_off[i + 1]):
+            if not (cls[j] or cls[j ^ 1]):
+                kept.append(j)
+        if kept:
+            new_fw.append(fired_wire[i])
+            new_rho.extend(rho[j] for j in kept)
+            src.extend(kept)
+            new_off.append(new_off[-1] + len(kept))
+    return (np.array(new_fw, dtype=np.int32), np.array(new_off, dtype=np.int32),
+            np.array(new_rho, dtype=np.float64), np.array(src, dtype=np.int32))
+
+
+def scan_turns(seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
+               cutoff, half_width, n_grid, n_iter, shrink, k_ref, min_wires=30, max_tracks=5):
+    """The stage loop of PAPER.md:256 without the fit: the last turn partition first; each stage scans its
+    partition's seeds against the hits that are left (scan_stage with one finally selected seed), classifies
+    the hits of its best seed, removes them (remove_hits) and moves to the previous turn; it stops when fewer
+    than min_wires fired wires are left or max_tracks stages are done (R34).
+    -> dict(turn_seed [P][6], turn_rss [P], turn_cls [P][H] in the ORIGINAL entry numbering, done [P] bool,
+            wires_before [P])."""
+    seeds = _c(seeds, np.float64)
+    part_off = np.asarray(part_off, dtype=np.int64)
+    P, H = part_off.shape[0] - 1, len(rho)
+    fw, ho, rh = np.asarray(fired_wire, np.int32), np.asarray(hit_off, np.int32), np.asarray(rho, np.float64)
+    orig = np.arange(H, dtype=np.int32)
+    out = {"turn_seed": np.full((P, 6), np.nan), "turn_rss": np.full(P, np.nan),
+           "turn_cls": np.zeros((P, H), dtype=np.uint8), "done": np.zeros(P, dtype=bool),
+           "wires_before": np.zeros(P, dtype=np.int32)}
+    n_done = 0
+    for p in range(P - 1, -1, -1):
+        if fw.shape[0] < min_wires or n_done >= max_tracks:
+            break
+        sub = np.ascontiguousarray(seeds[:, part_off[p]:part_off[p + 1]])
+        st = scan_stage(sub, np.array([0, sub.shape[1]], dtype=np.int64), charge, bz, step, n_steps, r_stop,
+                        wire_a, wire_b, fw, ho, rh, cutoff, half_width, n_grid, n_iter, shrink, k_ref, 1)
+        out["turn_seed"][p], out["turn_rss"][p] = st["final_seed"][0, 0], st["final_rss"][0, 0]
+        out["wires_before"][p], out["done"][p] = fw.shape[0], True
+        cls = st["cls"][0, 0]
+        out["turn_cls"][p, orig[cls.astype(bool)]] = 1
+        fw, ho, rh, src = remove_hits(fw, ho, rh, cls)
+        orig = orig[src]
+        n_done += 1
+    return out
