@@ -282,6 +282,48 @@ int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, i
                      double* final_seed, double* final_rss, double* final_dca, uint8_t* cls,
                      void* cuda_stream);
 
+/* ---- sequential stages with hit removal (readings R33-R34) -------------------- */
+
+/* "The hits classified previously were excluded in the seed scanning; therefore, the number of
+ * wires gets reduced whenever a track is fitted".  Input convention (R33): a measured
+ * hit is the adjacent pair of ghost entries (2m, 2m+1), so n_hits and every hit_off[i] are even.
+ * Entry j is removed when cls[j] or cls[j ^ 1] is set; a wire left without entries leaves the fired
+ * list; the order of wires and entries is kept.
+ *   cls          dev [n_hits] 0/1 (e.g. one row of comet_scan_stage's cls)
+ *   orig_in      dev [n_hits] entry numbers carried along (NULL = 0, 1, 2, ...), orig_out dev [n_hits] or NULL
+ *   fired_out    dev [n_fired], hit_off_out dev [n_fired+1], rho_out dev [n_hits]: the reduced list
+ *   counts       dev [2]: its number of fired wires and of entries */
+int comet_remove_hits(comet_ctx* ctx, const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                      int32_t n_fired, int32_t n_hits, const uint8_t* cls, const int32_t* orig_in,
+                      int32_t* fired_out, int32_t* hit_off_out, double* rho_out, int32_t* orig_out,
+                      int32_t* counts, void* cuda_stream);
+
+/* Bytes of the device work buffer of comet_scan_turns (0 for invalid arguments). */
+size_t comet_turns_work_bytes(int64_t max_partition_seeds, int32_t n_fired, int32_t n_hits, int32_t k_ref,
+                              const int32_t* n_grid);
+
+/* The stage loop of PAPER.md:256 without the fit between the stages (GENFIT2, out of scope): the
+ * last turn partition first (descending partition index); each stage is comet_scan_stage on that
+ * partition's seeds (k_final = 1) against the hits that are left, the hits its best seed classifies
+ * are removed (comet_remove_hits) before the previous turn is scanned; the loop stops when fewer
+ * than min_wires fired wires are left or max_tracks stages are done (paper: 30 and 5) (R34).
+ *   turn_seed   dev [n_part][6], turn_rss dev [n_part]: the stage's best seed (NaN where no stage ran)
+ *   turn_cls    dev [n_part][n_hits]: the hits given to each turn, in the event's own entry numbering
+ *   done_host, wires_before_host  HOST [n_part]: 1 where a stage ran; fired wires it started with
+ *   work        dev, comet_turns_work_bytes(largest partition, n_fired, n_hits, k_ref, n_grid)
+ * Synchronises cuda_stream once per stage (the size of the reduced hit list sets the next launches),
+ * as the paper's host loop does. */
+int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                     int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                     const double* wire_a, const double* wire_b, int32_t n_wires,
+                     const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                     int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                     const int64_t* part_off, int32_t n_part,
+                     const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                     int32_t k_ref, int32_t min_wires, int32_t max_tracks, void* work,
+                     double* turn_seed, double* turn_rss, uint8_t* turn_cls,
+                     int32_t* done_host, int32_t* wires_before_host, void* cuda_stream);
+
 /* ---- whole event from host buffers ------------------------------------------------------- */
 
 /* Runs A, B and C for one event whose inputs and outputs live in HOST memory (pinned memory makes

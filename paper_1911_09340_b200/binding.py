@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = [
     "comet_track_export", "comet_dca_rss", "comet_select_and_classify", "comet_scan_event_host",
     "comet_fp64_peak_probe", "comet_read_stats", "comet_reserve", "comet_read_timing", "comet_scan_rss",
     "comet_select_references", "comet_refine_seeds", "comet_classify_seeds", "comet_stage_work_bytes",
-    "comet_scan_stage", "comet_set_field",
+    "comet_scan_stage", "comet_set_field", "comet_remove_hits", "comet_turns_work_bytes", "comet_scan_turns",
 ]
 
 COMET_CHUNK = 32
@@ -79,6 +79,12 @@ def load_library():
     L.comet_reserve.argtypes = [vp, i64]
     L.comet_read_timing.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32, ctypes.POINTER(i32)]
     L.comet_read_stats.argtypes = [vp, ctypes.POINTER(ctypes.c_uint64), i32, i32, vp]
+    L.comet_remove_hits.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.comet_turns_work_bytes.argtypes = [i64, i32, i32, i32, vp]
+    L.comet_turns_work_bytes.restype = sz
+    L.comet_scan_turns.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
+                                   vp, vp, i32, vp, vp, vp, i32, i32, dbl,
+                                   vp, i32, vp, vp, i32, dbl, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     L.comet_set_field.argtypes = [vp, vp, vp, vp, vp, dbl, vp]
     L.comet_select_references.argtypes = [vp, vp, i64, i64, vp, vp, i32, vp, i32, vp, vp]
     L.comet_refine_seeds.argtypes = [vp, vp, i64, i64, vp, i32, i32, vp, vp, vp, i64, vp]
@@ -90,7 +96,7 @@ def load_library():
                                    vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                    vp, i32, vp, vp, i32, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
-        if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes"):
+        if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes", "comet_turns_work_bytes"):
             getattr(L, name).restype = ctypes.c_int
     _lib = L
     return L
@@ -368,6 +374,55 @@ class Comet:
             po.ctypes.data, P, hw.ctypes.data, ng.ctypes.data, int(n_iter), float(shrink), int(k_ref), int(k_final),
             int(work.data_ptr()), int(out["final_seed"].data_ptr()), int(out["final_rss"].data_ptr()),
             int(out["final_dca"].data_ptr()), int(out["cls"].data_ptr()), _stream_ptr(stream)))
+        return out
+
+    # -- sequential stages with hit removal -------------------------------------------------------
+    def remove_hits(self, fired_wire, hit_off, rho, cls, orig=None, stream=None):
+        """comet_remove_hits -> dict(fired_wire, hit_off, rho, orig, counts) (device; sliced to the new sizes,
+        which costs one synchronisation)."""
+        W, H, d, td = int(fired_wire.shape[0]), int(rho.shape[0]), self.device, self._tdev()
+        fo = torch.empty(W, dtype=torch.int32, device=td)
+        ho = torch.empty(W + 1, dtype=torch.int32, device=td)
+        ro = torch.empty(H, dtype=torch.float64, device=td)
+        oo = torch.empty(H, dtype=torch.int32, device=td)
+        cnt = torch.empty(2, dtype=torch.int32, device=td)
+        self._check(self._L.comet_remove_hits(
+            self._h, _dev(fired_wire, torch.int32, "fired_wire", d), _dev(hit_off, torch.int32, "hit_off", d),
+            _dev(rho, torch.float64, "rho", d), W, H, _dev(cls, torch.uint8, "cls", d), _dev(orig, torch.int32, "orig", d),
+            int(fo.data_ptr()), int(ho.data_ptr()), int(ro.data_ptr()), int(oo.data_ptr()), int(cnt.data_ptr()),
+            _stream_ptr(stream)))
+        nw, nh = (int(v) for v in cnt.cpu().tolist())
+        return {"fired_wire": fo[:nw], "hit_off": ho[:nw + 1], "rho": ro[:nh], "orig": oo[:nh], "counts": (nw, nh)}
+
+    def scan_turns(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off,
+                   rho, cutoff, half_width, n_grid, n_iter, shrink, k_ref, min_wires=30, max_tracks=5, stream=None):
+        """comet_scan_turns: the last turn first, hits of a stage's best seed removed before the previous turn."""
+        S = seeds.shape[1]
+        po = np.ascontiguousarray(np.asarray(part_off, dtype=np.int64))
+        hw = np.ascontiguousarray(np.asarray(half_width, dtype=np.float64))
+        ng = np.ascontiguousarray(np.asarray(n_grid, dtype=np.int32))
+        P, W, H = po.shape[0] - 1, int(fired_wire.shape[0]), int(rho.shape[0])
+        d, td = self.device, self._tdev()
+        nb = int(self._L.comet_turns_work_bytes(int(np.diff(po).max()), W, H, int(k_ref), ng.ctypes.data))
+        if nb == 0:
+            raise CometError("comet_turns_work_bytes: invalid arguments")
+        work = torch.empty(nb, dtype=torch.uint8, device=td)
+        out = {"turn_seed": torch.empty((P, 6), dtype=torch.float64, device=td),
+               "turn_rss": torch.empty(P, dtype=torch.float64, device=td),
+               "turn_cls": torch.empty((P, H), dtype=torch.uint8, device=td)}
+        done = np.zeros(P, dtype=np.int32)
+        wb = np.zeros(P, dtype=np.int32)
+        self._check(self._L.comet_scan_turns(
+            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, int(charge), float(bz), float(step),
+            int(n_steps), float(r_stop),
+            _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
+            int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d),
+            _dev(hit_off, torch.int32, "hit_off", d), _dev(rho, torch.float64, "rho", d), W, H, float(cutoff),
+            po.ctypes.data, P, hw.ctypes.data, ng.ctypes.data, int(n_iter), float(shrink), int(k_ref),
+            int(min_wires), int(max_tracks), int(work.data_ptr()), int(out["turn_seed"].data_ptr()),
+            int(out["turn_rss"].data_ptr()), int(out["turn_cls"].data_ptr()), done.ctypes.data, wb.ctypes.data,
+            _stream_ptr(stream)))
+        out["done"], out["wires_before"] = done.astype(bool), wb
         return out
 
     # -- whole event, device-resident inputs --------------------------------------------------

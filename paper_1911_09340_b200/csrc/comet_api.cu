@@ -15,6 +15,7 @@
 #include "select.cuh"
 #include "scan_fused.cuh"
 #include "refine.cuh"
+#include "turns.cuh"
 
 #ifndef COMET_PRUNED_WT
 #define COMET_PRUNED_WT 3
@@ -1018,6 +1019,132 @@ extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t see
     return launch_classify_seeds(ctx, cur, cur_stride, charge, bz_tesla, step_cm, n_steps, r_stop_cm, hit_off, rho,
                                  n_fired, n_hits, cutoff_cm, ref, n_part * k_final, rss, final_dca, cls, final_seed,
                                  final_rss, (cudaStream_t)cuda_stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// sequential stages with hit removal (readings R33-R34)
+// ---------------------------------------------------------------------------------------------
+extern "C" int comet_remove_hits(comet_ctx* ctx, const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                 int32_t n_fired, int32_t n_hits, const uint8_t* cls, const int32_t* orig_in,
+                                 int32_t* fired_out, int32_t* hit_off_out, double* rho_out, int32_t* orig_out,
+                                 int32_t* counts, void* cuda_stream)
+{
+    if (!ctx || n_fired < 0 || n_hits < 0 || (n_hits & 1) || !hit_off || !hit_off_out || !counts ||
+        (n_fired > 0 && (!fired_wire || !fired_out)) || (n_hits > 0 && (!rho || !cls || !rho_out)))
+        return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    k_remove_hits<<<1, COMET_RM_THREADS, 0, (cudaStream_t)cuda_stream>>>(fired_wire, hit_off, rho, n_fired, cls, orig_in,
+                                                                        fired_out, hit_off_out, rho_out, orig_out, counts);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+// work buffer of comet_scan_turns: the stage work, two reduced hit lists (fired, hit_off, rho, orig), the
+// stage's classification and DCAs, the two counters
+struct TurnsLayout {
+    size_t stage, list[2], cls, dca, counts, total;
+    size_t o_fired, o_off, o_rho, o_orig;     // within a list
+};
+static TurnsLayout turns_layout(size_t stage_bytes, int32_t n_fired, int32_t n_hits)
+{
+    TurnsLayout L;
+    auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+    L.o_fired = 0;
+    L.o_off = up(sizeof(int32_t) * (size_t)n_fired);
+    L.o_rho = L.o_off + up(sizeof(int32_t) * ((size_t)n_fired + 1));
+    L.o_orig = L.o_rho + up(sizeof(double) * (size_t)n_hits);
+    const size_t list_bytes = L.o_orig + up(sizeof(int32_t) * (size_t)n_hits);
+    size_t o = up(stage_bytes);
+    L.stage = 0;
+    L.list[0] = o; o += list_bytes;
+    L.list[1] = o; o += list_bytes;
+    L.cls = o; o += up((size_t)n_hits);
+    L.dca = o; o += up(sizeof(double) * (size_t)n_fired);
+    L.counts = o; o += 256;
+    L.total = o;
+    return L;
+}
+
+extern "C" size_t comet_turns_work_bytes(int64_t max_partition_seeds, int32_t n_fired, int32_t n_hits, int32_t k_ref,
+                                         const int32_t* n_grid)
+{
+    if (n_fired < 0 || n_hits < 0) return 0;
+    const size_t sb = comet_stage_work_bytes(max_partition_seeds, 1, k_ref, 1, n_grid);
+    if (!sb) return 0;
+    return turns_layout(sb, n_fired, n_hits).total;
+}
+
+extern "C" int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                                int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                                const double* wire_a, const double* wire_b, int32_t n_wires,
+                                const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                const int64_t* part_off, int32_t n_part,
+                                const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                                int32_t k_ref, int32_t min_wires, int32_t max_tracks, void* work,
+                                double* turn_seed, double* turn_rss, uint8_t* turn_cls,
+                                int32_t* done_host, int32_t* wires_before_host, void* cuda_stream)
+{
+    if (!ctx || n_part < 1 || n_part > COMET_MAX_PARTITIONS || !part_off || !work || !turn_seed || !turn_rss ||
+        (n_hits > 0 && !turn_cls) || !done_host || !wires_before_host || (n_hits & 1) || min_wires < 0 || max_tracks < 0 ||
+        n_seeds < 1 || seed_stride < n_seeds)
+        return COMET_EINVAL;
+    PartOff po;
+    if (fill_partoff(&po, part_off, n_part, n_seeds, true)) return COMET_EINVAL;
+    int64_t max_part = 0;
+    for (int p = 0; p < n_part; ++p)
+        if (po.off[p + 1] - po.off[p] > max_part) max_part = po.off[p + 1] - po.off[p];
+    const size_t sb = comet_stage_work_bytes(max_part, 1, k_ref, 1, n_grid);
+    if (!sb) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const TurnsLayout L = turns_layout(sb, n_fired, n_hits);
+    char* Wk = (char*)work;
+    uint8_t* cls_stage = (uint8_t*)(Wk + L.cls);
+    double* dca_stage = (double*)(Wk + L.dca);
+    int32_t* counts = (int32_t*)(Wk + L.counts);
+    // nothing done yet: NaN seeds / RSS (all-ones is a NaN), empty classification
+    CU(ctx, cudaMemsetAsync(turn_seed, 0xff, sizeof(double) * 6 * (size_t)n_part, st));
+    CU(ctx, cudaMemsetAsync(turn_rss, 0xff, sizeof(double) * (size_t)n_part, st));
+    if (n_hits) CU(ctx, cudaMemsetAsync(turn_cls, 0, (size_t)n_part * (size_t)n_hits, st));
+    for (int p = 0; p < n_part; ++p) { done_host[p] = 0; wires_before_host[p] = 0; }
+    const int32_t* cur_fw = fired_wire;
+    const int32_t* cur_ho = hit_off;
+    const double* cur_rho = rho;
+    const int32_t* cur_orig = nullptr;                   // identity
+    int32_t cur_w = n_fired, cur_h = n_hits, n_done = 0, flip = 0;
+    for (int p = n_part - 1; p >= 0; --p) {              // the last turn first
+        if (cur_w < min_wires || n_done >= max_tracks) break;
+        const int64_t np_seeds = po.off[p + 1] - po.off[p];
+        const int64_t one[2] = {0, np_seeds};
+        rc = comet_scan_stage(ctx, seeds + po.off[p], seed_stride, np_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+                              wire_a, wire_b, n_wires, cur_fw, cur_ho, cur_rho, cur_w, cur_h, cutoff_cm, one, 1,
+                              half_width, n_grid, n_iter, shrink, k_ref, 1, Wk + L.stage,
+                              turn_seed + 6 * (size_t)p, turn_rss + p, dca_stage, cls_stage, st);
+        if (rc) return rc;
+        done_host[p] = 1;
+        wires_before_host[p] = cur_w;
+        n_done += 1;
+        if (cur_h) k_scatter_cls<<<(cur_h + 255) / 256, 256, 0, st>>>(cls_stage, cur_orig, cur_h, turn_cls + (size_t)p * n_hits);
+        char* Lb = Wk + L.list[flip];
+        int32_t* n_fw = (int32_t*)(Lb + L.o_fired);
+        int32_t* n_ho = (int32_t*)(Lb + L.o_off);
+        double* n_rho = (double*)(Lb + L.o_rho);
+        int32_t* n_orig = (int32_t*)(Lb + L.o_orig);
+        k_remove_hits<<<1, COMET_RM_THREADS, 0, st>>>(cur_fw, cur_ho, cur_rho, cur_w, cls_stage, cur_orig, n_fw, n_ho, n_rho,
+                                                      n_orig, counts);
+        CU(ctx, cudaGetLastError());
+        // the next stage's launch sizes: one synchronisation per stage, as in the paper's host loop
+        int32_t hc[2];
+        CU(ctx, cudaMemcpyAsync(hc, counts, sizeof(hc), cudaMemcpyDeviceToHost, st));
+        CU(ctx, cudaStreamSynchronize(st));
+        cur_fw = n_fw; cur_ho = n_ho; cur_rho = n_rho; cur_orig = n_orig;
+        cur_w = hc[0]; cur_h = hc[1];
+        flip ^= 1;
+    }
+    return COMET_OK;
 }
 
 // ---------------------------------------------------------------------------------------------

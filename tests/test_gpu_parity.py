@@ -898,3 +898,43 @@ def test_scan_path_is_capturable_in_a_cuda_graph(comet, cfg1_event):
         torch.cuda.synchronize()
         assert torch.equal(rss, rss_ref)
         assert torch.equal(out["best_seed"], best_ref) and torch.equal(out["cls"], cls_ref)
+
+
+# ------------------------------------------------------------------------------------------------
+# sequential stages with hit removal (comet_remove_hits, comet_scan_turns)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_wires_case", [0, 1, 300, 5000])
+def test_remove_hits_matches_oracle(comet, n_wires_case):
+    rng = np.random.default_rng(21 + n_wires_case)
+    W = n_wires_case
+    counts = rng.integers(0, 4, size=W) * 2
+    hit_off = np.concatenate([[0], np.cumsum(counts)]).astype(np.int32)
+    H = int(hit_off[-1])
+    rho = rng.normal(size=H)
+    cls = (rng.uniform(size=H) < 0.25).astype(np.uint8)
+    fired = rng.permutation(20000)[:W].astype(np.int32)
+    orig = rng.permutation(H).astype(np.int32)
+    for og in (None, orig):
+        got = comet.remove_hits(_dev(fired), _dev(hit_off), _dev(rho), _dev(cls), None if og is None else _dev(og))
+        fw, ho, rh, src = O.remove_hits(fired, hit_off, rho, cls)
+        np.testing.assert_array_equal(got["fired_wire"].cpu().numpy(), fw)
+        np.testing.assert_array_equal(got["hit_off"].cpu().numpy(), ho)
+        np.testing.assert_array_equal(got["rho"].cpu().numpy(), rh)
+        np.testing.assert_array_equal(got["orig"].cpu().numpy(), src if og is None else og[src])
+        assert got["counts"] == (fw.size, rh.size)
+
+
+def test_scan_turns_matches_oracle_cfg1(comet, cfg1_event):
+    ev = cfg1_event
+    seeds, po = event_seeds(ev, shape=(6, 6, 6, 6))
+    d = DevEvent(ev, seeds)
+    kw = dict(half_width=[1.2, 1.0, 1.0, 2.0], n_grid=[3, 3, 3, 3], n_iter=2, shrink=0.5, k_ref=4)
+    for extra in ({}, {"max_tracks": 2}, {"min_wires": 50}):
+        out = comet.scan_turns(d.seeds, po, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff, **kw, **extra)
+        torch.cuda.synchronize()
+        ref = O.scan_turns(seeds, po, *_ev_args(ev), **kw, **extra)
+        np.testing.assert_array_equal(out["done"], ref["done"])
+        np.testing.assert_array_equal(out["wires_before"], ref["wires_before"])
+        np.testing.assert_array_equal(out["turn_seed"].cpu().numpy(), ref["turn_seed"])
+        np.testing.assert_array_equal(out["turn_rss"].cpu().numpy(), ref["turn_rss"])
+        np.testing.assert_array_equal(out["turn_cls"].cpu().numpy(), ref["turn_cls"])
