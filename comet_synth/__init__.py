@@ -13,10 +13,10 @@ from .geometry import cdc_geometry, CDCGeometry
 from .helix import Helix, KAPPA
 from .events import (Event, Partition, make_event, make_config, config_spec,
                      seed_grid, event_seeds, truth_seed, CONFIG_SPECS)
-from .fieldmap import solenoid_map, uniform_map
+from .fieldmap import solenoid_map, uniform_map, hough_tables
 
 __all__ = [
     "cdc_geometry", "CDCGeometry", "Helix", "KAPPA", "Event", "Partition",
     "make_event", "make_config", "config_spec", "seed_grid", "event_seeds",
-    "truth_seed", "CONFIG_SPECS", "solenoid_map", "uniform_map",
+    "truth_seed", "CONFIG_SPECS", "solenoid_map", "uniform_map", "hough_tables",
 ]

@@ -34,3 +34,10 @@ def uniform_map(bz=1.0, half=100.0, spacing=(25.0, 25.0, 25.0)):
     B = np.zeros((n, n, n, 3))
     B[..., 2] = bz
     return B, np.array([-half, -half, -half]), d
+
+
+def hough_tables(n_phi=256):
+    """cos / sin of the Hough directions phi_j = 2 pi j / n_phi (inputs of the transverse seeding: both the
+    oracle and the CUDA path read these tables, neither evaluates a trigonometric function)."""
+    phi = 2.0 * np.pi * np.arange(n_phi) / n_phi
+    return np.cos(phi), np.sin(phi)

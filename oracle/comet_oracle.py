@@ -342,3 +342,65 @@ def scan_turns(seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_
         orig = orig[src]
         n_done += 1
     return out
+
+
+# ---- Hough-transform transverse seeding (Fig. 10; readings R35-R37) -----------------
+def hough_seeds(wire_a, wire_b, fired_wire, cos_tab, sin_tab, rho_min, inv_drho, n_rho, charge, bz, r_seed):
+    """"The transverse components (theta, p_x, p_y) were extracted by finding a circle that is the transverse
+    projection of a helical trajectory [...] the Hough transform was applied to the set of transverse positions
+    of the fired wires".  R35: a wire's transverse position is the (x, y) of its midpoint.
+    R36: the circle passes through the origin (the stopping target on the axis), so u = x/(x^2+y^2),
+    v = y/(x^2+y^2) maps it to the line u cos(phi) + v sin(phi) = rho with rho = 1/(2R) and phi the azimuth of
+    the circle's centre; every fired wire votes once per direction phi_j (tables given) in the bin
+    floor((rho - rho_min) inv_drho) if that lies in [0, n_rho); the peak is the bin of most votes, ties -> the
+    lowest j n_rho + k.  R37: R = 1/(2 rho*) with rho* the bin centre, centre R (cos, sin); the seed points are
+    the two intersections with the cylinder r = r_seed, p_T = kappa |B_z| R along the tangent in the sense of
+    rotation of the particle; the entrance is the one where the track moves outwards.
+    -> dict(acc [n_phi][n_rho] int32, peak (votes, j, k), R, centre [2], entrance [4] (x, y, px, py), exit [4])."""
+    wire_a, wire_b = np.asarray(wire_a, np.float64), np.asarray(wire_b, np.float64)
+    cos_tab, sin_tab = np.asarray(cos_tab, np.float64), np.asarray(sin_tab, np.float64)
+    n_phi = cos_tab.shape[0]
+    acc = np.zeros((n_phi, int(n_rho)), dtype=np.int32)
+    for wi in np.asarray(fired_wire):
+        x = (wire_a[0, wi] + wire_b[0, wi]) / 2.0
+        y = (wire_a[1, wi] + wire_b[1, wi]) / 2.0
+        r2 = x * x + y * y
+        u, v = x / r2, y / r2
+        for j in range(n_phi):
+            rho = u * cos_tab[j] + v * sin_tab[j]
+            k = np.floor((rho - rho_min) * inv_drho)
+            if 0.0 <= k < n_rho:
+                acc[j, int(k)] += 1
+    flat = acc.ravel()
+    best = int(np.argmax(flat))                            # first maximum = lowest j n_rho + k
+    j, k = divmod(best, int(n_rho))
+    out = {"acc": acc, "peak": (int(flat[best]), j, k)}
+    nan4 = np.full(4, np.nan)
+    if flat[best] == 0:
+        out.update(R=np.nan, centre=np.full(2, np.nan), entrance=nan4, exit=nan4.copy())
+        return out
+    rho_s = rho_min + (k + 0.5) / inv_drho
+    R = 1.0 / (2.0 * rho_s)
+    cx, cy = R * cos_tab[j], R * sin_tab[j]
+    out.update(R=R, centre=np.array([cx, cy]))
+    t = (r_seed * r_seed) / (2.0 * R)                      # component of the seed point along the centre direction
+    n2 = r_seed * r_seed - t * t
+    if not (n2 > 0.0):
+        out.update(entrance=nan4, exit=nan4.copy())         # the circle does not reach the seed cylinder
+        return out
+    n = np.sqrt(n2)
+    sense = -1.0 if (charge * bz) > 0.0 else 1.0            # +1: counter-clockwise (electron in B_z > 0)
+    pT = KAPPA_ * abs(bz) * R
+    pts = []
+    for sgn in (1.0, -1.0):
+        px_ = t * cos_tab[j] - sgn * n * sin_tab[j]
+        py_ = t * sin_tab[j] + sgn * n * cos_tab[j]
+        tx, ty = -(py_ - cy) / R, (px_ - cx) / R            # counter-clockwise tangent
+        tx, ty = sense * tx, sense * ty
+        pts.append((px_, py_, pT * tx, pT * ty, px_ * tx + py_ * ty))
+    ent, ext = (pts[0], pts[1]) if pts[0][4] > 0.0 else (pts[1], pts[0])
+    out.update(entrance=np.array(ent[:4]), exit=np.array(ext[:4]))
+    return out
+
+
+KAPPA_ = 2.99792458     # R4
