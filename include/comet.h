@@ -324,6 +324,40 @@ int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t seed_stride, i
                      double* turn_seed, double* turn_rss, uint8_t* turn_cls,
                      int32_t* done_host, int32_t* wires_before_host, void* cuda_stream);
 
+/* ---- Hough-transform transverse seeding (Fig. 10; readings R35-R37) ------------ */
+
+/* Bytes of the device work buffer of comet_hough_seeds (0 for n_events < 0). */
+size_t comet_hough_work_bytes(int32_t n_events);
+
+/* "The transverse components of (theta, p_x, p_y) were extracted by finding a circle that is the
+ * transverse projection of a helical trajectory [...] the Hough transform was applied to the set of
+ * transverse positions of the fired wires", for a batch of events in one launch.
+ * R35: a wire's transverse position is the (x, y) of its midpoint.  R36: the circle passes through
+ * the origin, so u = x/(x^2+y^2), v = y/(x^2+y^2) lie on the line u cos(phi) + v sin(phi) = rho with
+ * rho = 1/(2R) and phi the azimuth of the circle's centre; every fired wire votes once per direction
+ * phi_j in the bin floor((rho - rho_min) inv_drho) if that lies in [0, n_rho) (fp64, one IEEE
+ * operation per operation written here; no trigonometric function is evaluated: the tables are
+ * inputs); the peak is the bin of most votes, ties -> the lowest j n_rho + k.  R37: R = 1/(2 rho*)
+ * with rho* = rho_min + (k + 0.5)/inv_drho, centre R (cos, sin); the seed points are the two
+ * intersections with the cylinder r = r_seed_cm, p_T = kappa |B_z| R along the tangent in the
+ * particle's sense of rotation; the entrance is the one where the track moves outwards.
+ *   wire_a, wire_b   dev SoA [3][n_wires] endpoints (cm)
+ *   fired_wire       dev [ev_off[n_events]] wire indices in [0, n_wires), the events one after the other
+ *   ev_off           dev [n_events+1] non-decreasing offsets into fired_wire, ev_off[0] = 0; n_events <= 65535
+ *   cos_tab, sin_tab dev [n_phi]; n_phi >= 1, 1 <= n_rho <= 32768, n_phi n_rho < 2^31, inv_drho > 0
+ *   acc              dev [n_events][n_phi][n_rho] int32 votes, or NULL to skip writing them
+ *   peak             dev [n_events][3] int32: votes, j, k of the peak ((0, 0, 0) without votes)
+ *   circle           dev [n_events][11]: R, centre x, y, entrance (x, y, p_x, p_y), exit (x, y, p_x, p_y);
+ *                    NaN without votes; entrance/exit NaN when the circle does not reach r_seed_cm
+ *   work             dev, comet_hough_work_bytes(n_events)
+ * Indices in fired_wire are not checked on the device.  No host synchronisation. */
+int comet_hough_seeds(comet_ctx* ctx, const double* wire_a, const double* wire_b, int32_t n_wires,
+                      const int32_t* fired_wire, const int32_t* ev_off, int32_t n_events,
+                      const double* cos_tab, const double* sin_tab, int32_t n_phi,
+                      double rho_min, double inv_drho, int32_t n_rho,
+                      int32_t charge, double bz_tesla, double r_seed_cm, void* work,
+                      int32_t* acc, int32_t* peak, double* circle, void* cuda_stream);
+
 /* ---- whole event from host buffers ------------------------------------------------------- */
 
 /* Runs A, B and C for one event whose inputs and outputs live in HOST memory (pinned memory makes

@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = [
     "comet_fp64_peak_probe", "comet_read_stats", "comet_reserve", "comet_read_timing", "comet_scan_rss",
     "comet_select_references", "comet_refine_seeds", "comet_classify_seeds", "comet_stage_work_bytes",
     "comet_scan_stage", "comet_set_field", "comet_remove_hits", "comet_turns_work_bytes", "comet_scan_turns",
+    "comet_hough_work_bytes", "comet_hough_seeds",
 ]
 
 COMET_CHUNK = 32
@@ -85,6 +86,10 @@ def load_library():
     L.comet_scan_turns.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
                                    vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                    vp, i32, vp, vp, i32, dbl, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
+    L.comet_hough_work_bytes.argtypes = [i32]
+    L.comet_hough_work_bytes.restype = sz
+    L.comet_hough_seeds.argtypes = [vp, vp, vp, i32, vp, vp, i32, vp, vp, i32, dbl, dbl, i32, i32, dbl, dbl,
+                                    vp, vp, vp, vp, vp]
     L.comet_set_field.argtypes = [vp, vp, vp, vp, vp, dbl, vp]
     L.comet_select_references.argtypes = [vp, vp, i64, i64, vp, vp, i32, vp, i32, vp, vp]
     L.comet_refine_seeds.argtypes = [vp, vp, i64, i64, vp, i32, i32, vp, vp, vp, i64, vp]
@@ -96,7 +101,8 @@ def load_library():
                                    vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                    vp, i32, vp, vp, i32, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
-        if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes", "comet_turns_work_bytes"):
+        if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes", "comet_turns_work_bytes",
+                        "comet_hough_work_bytes"):
             getattr(L, name).restype = ctypes.c_int
     _lib = L
     return L
@@ -423,6 +429,27 @@ class Comet:
             int(out["turn_rss"].data_ptr()), int(out["turn_cls"].data_ptr()), done.ctypes.data, wb.ctypes.data,
             _stream_ptr(stream)))
         out["done"], out["wires_before"] = done.astype(bool), wb
+        return out
+
+    # -- Hough-transform transverse seeding --------------------------------------------------------
+    def hough_seeds(self, wire_a, wire_b, fired_wire, ev_off, cos_tab, sin_tab, rho_min, inv_drho, n_rho,
+                    charge, bz, r_seed, want_acc=True, stream=None):
+        """comet_hough_seeds for a batch of events (fired_wire concatenated, ev_off [n_events+1]) ->
+        dict(acc [E][n_phi][n_rho] or None, peak [E][3], circle [E][11]) (device)."""
+        d, td = self.device, self._tdev()
+        E, n_phi = int(ev_off.shape[0]) - 1, int(cos_tab.shape[0])
+        work = torch.empty(int(self._L.comet_hough_work_bytes(E)), dtype=torch.uint8, device=td)
+        out = {"acc": torch.empty((E, n_phi, int(n_rho)), dtype=torch.int32, device=td) if want_acc else None,
+               "peak": torch.empty((E, 3), dtype=torch.int32, device=td),
+               "circle": torch.empty((E, 11), dtype=torch.float64, device=td)}
+        self._check(self._L.comet_hough_seeds(
+            self._h, _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
+            int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d), _dev(ev_off, torch.int32, "ev_off", d),
+            E, _dev(cos_tab, torch.float64, "cos_tab", d), _dev(sin_tab, torch.float64, "sin_tab", d), n_phi,
+            float(rho_min), float(inv_drho), int(n_rho), int(charge), float(bz), float(r_seed),
+            int(work.data_ptr()), _dev(out["acc"], torch.int32, "acc", d), int(out["peak"].data_ptr()),
+            int(out["circle"].data_ptr()), _stream_ptr(stream)))
+        out["_work"] = work          # keeps the buffer alive until the caller drops the result
         return out
 
     # -- whole event, device-resident inputs --------------------------------------------------

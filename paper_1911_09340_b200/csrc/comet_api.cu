@@ -16,6 +16,7 @@
 #include "scan_fused.cuh"
 #include "refine.cuh"
 #include "turns.cuh"
+#include "hough.cuh"
 
 #ifndef COMET_PRUNED_WT
 #define COMET_PRUNED_WT 3
@@ -1144,6 +1145,48 @@ extern "C" int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t see
         cur_w = hc[0]; cur_h = hc[1];
         flip ^= 1;
     }
+    return COMET_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Hough-transform transverse seeding (readings R35-R37)
+// ---------------------------------------------------------------------------------------------
+extern "C" size_t comet_hough_work_bytes(int32_t n_events)
+{
+    return n_events < 0 ? 0 : sizeof(HoughWork) * (size_t)(n_events > 0 ? n_events : 1);
+}
+
+extern "C" int comet_hough_seeds(comet_ctx* ctx, const double* wire_a, const double* wire_b, int32_t n_wires,
+                                 const int32_t* fired_wire, const int32_t* ev_off, int32_t n_events,
+                                 const double* cos_tab, const double* sin_tab, int32_t n_phi,
+                                 double rho_min, double inv_drho, int32_t n_rho,
+                                 int32_t charge, double bz_tesla, double r_seed_cm, void* work,
+                                 int32_t* acc, int32_t* peak, double* circle, void* cuda_stream)
+{
+    if (!ctx || n_events < 0 || n_events > 65535 || n_wires < 0 || n_phi < 1 || n_rho < 1 || n_rho > 32768 ||
+        (int64_t)n_phi * n_rho >= ((int64_t)1 << 31) || !(inv_drho > 0.0) || !isfinite(inv_drho) || !isfinite(rho_min) ||
+        !(r_seed_cm > 0.0) || (charge != 1 && charge != -1) || !isfinite(bz_tesla) || bz_tesla == 0.0 ||
+        !cos_tab || !sin_tab || !ev_off || !work || (n_events > 0 && (!peak || !circle)) ||
+        (n_wires > 0 && (!wire_a || !wire_b)))
+        return COMET_EINVAL;
+    if (n_events == 0) return COMET_OK;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // directions per CTA: about one CTA per SM and event batch, rows of the CTA in shared memory (<= 64 KB)
+    int64_t ctas_per_event = (ctx->n_sm + n_events - 1) / n_events;
+    int D = (int)((n_phi + ctas_per_event - 1) / ctas_per_event);
+    const int d_max = 65536 / (4 * n_rho) > 0 ? 65536 / (4 * n_rho) : 1;
+    if (D > d_max) D = d_max;
+    if (D < 1) D = 1;
+    const size_t smem = (size_t)D * n_rho * sizeof(int) + 2 * COMET_HT_THREADS * sizeof(double);
+    if (smem > 48 * 1024) CU(ctx, cudaFuncSetAttribute(k_hough, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    CU(ctx, cudaMemsetAsync(work, 0, sizeof(HoughWork) * (size_t)n_events, st));
+    const dim3 grid((unsigned)((n_phi + D - 1) / D), (unsigned)n_events);
+    k_hough<<<grid, COMET_HT_THREADS, smem, st>>>(wire_a, wire_b, n_wires, fired_wire, ev_off, cos_tab, sin_tab, n_phi, D,
+                                                  rho_min, inv_drho, n_rho, charge, bz_tesla, r_seed_cm, acc, peak,
+                                                  circle, (HoughWork*)work);
+    CU(ctx, cudaGetLastError());
     return COMET_OK;
 }
 
