@@ -403,4 +403,120 @@ def hough_seeds(wire_a, wire_b, fired_wire, cos_tab, sin_tab, rho_min, inv_drho,
     return out
 
 
+# ---- half tracks (readings R38-R42) --------------------------------------------
+def flip_seeds(seeds):
+    """"The track extrapolation was done in the forward direction from the entrance and the backward direction
+    from the exit by flipping the charge and momentum".  R38: the backward seed of an exit-side
+    seed (x, p) is (x, -p), extrapolated with the charge -q (the caller passes -charge).  The signed DCA of a
+    wire is measured against the track's direction of travel, so on the way back it has the opposite sign:
+    the backward scan is run against -rho (scan_half_tracks does that)."""
+    out = np.array(seeds, dtype=np.float64, copy=True)
+    out[3:6] = -out[3:6]
+    return out
+
+
+def half_hit_masks(wire_a, wire_b, fired_wire, hit_off, n_hits, circle, overlap):
+    """"The hits of the event were also grouped into two sets for each half track" (PAPER.md:230).  R39: the
+    two half tracks meet at the apex of the transverse circle found by the Hough transform (circle = R, centre
+    x, y, entrance x, y, ...: hough_seeds' output), which lies on the line from the origin through the centre.
+    With m the (x, y) of a wire's midpoint, d = (cx m_y - cy m_x) / R is its signed distance from that line and
+    s = +1 if cx e_y - cy e_x > 0 else -1 the side of the entrance point e: the wire's entries belong to the
+    entrance half iff s d > -overlap and to the exit half iff s d <= overlap.
+    -> (in_ent [n_hits] uint8, in_exit [n_hits] uint8)."""
+    wire_a, wire_b = np.asarray(wire_a, np.float64), np.asarray(wire_b, np.float64)
+    circle = np.asarray(circle, np.float64)
+    R, cx, cy, ex, ey = circle[0], circle[1], circle[2], circle[3], circle[4]
+    s = 1.0 if (cx * ey - cy * ex) > 0.0 else -1.0
+    in_e = np.zeros(int(n_hits), dtype=np.uint8)
+    in_x = np.zeros(int(n_hits), dtype=np.uint8)
+    for i, wi in enumerate(np.asarray(fired_wire)):
+        mx = (wire_a[0, wi] + wire_b[0, wi]) / 2.0
+        my = (wire_a[1, wi] + wire_b[1, wi]) / 2.0
+        d = s * ((cx * my - cy * mx) / R)
+        for j in range(hit_off[i], hit_off[i + 1]):
+            in_e[j] = 1 if d > -overlap else 0
+            in_x[j] = 1 if d <= overlap else 0
+    return in_e, in_x
+
+
+def layer_veto(cls, fired_wire, hit_off, wire_layer, min_layers):
+    """"the seeds which have any missing layer without the hits were excluded".  R40: a half
+    track starts in front of the first layer, so it crosses the layers 0 .. l_max, l_max the highest layer
+    with a classified hit of this seed: the seed is kept iff every one of those layers has a classified hit
+    and there are at least min_layers of them.  cls [K][H] -> ok [K] uint8."""
+    cls = np.atleast_2d(np.asarray(cls)).astype(bool)
+    wire_layer = np.asarray(wire_layer)
+    ok = np.zeros(cls.shape[0], dtype=np.uint8)
+    for a in range(cls.shape[0]):
+        layers = set()
+        for i, wi in enumerate(np.asarray(fired_wire)):
+            for j in range(hit_off[i], hit_off[i + 1]):
+                if cls[a, j]:
+                    layers.add(int(wire_layer[wi]))
+        if layers:
+            l_max = max(layers)
+            ok[a] = 1 if (all(l in layers for l in range(l_max + 1)) and l_max + 1 >= min_layers) else 0
+    return ok
+
+
+def merge_half_sets(cls_e, orig_e, ok_e, cls_x, orig_x, ok_x, n_hits):
+    """"The complete sets of classified hits were formed by combinatorially merging two half sets, one of which
+    is from each direction".  R41: pair (a, b) of an entrance-side seed a and an exit-side seed
+    b is valid iff both passed the layer veto; its complete set is the union of the two half sets in the
+    event's own entry numbering (orig_* map the entries of the half lists back).
+    -> dict(valid [Ke][Kx] uint8, cls [Ke][Kx][n_hits] uint8 (zeros where not valid), n_cls [Ke][Kx] int32)."""
+    cls_e, cls_x = np.atleast_2d(np.asarray(cls_e)), np.atleast_2d(np.asarray(cls_x))
+    Ke, Kx = cls_e.shape[0], cls_x.shape[0]
+    valid = np.zeros((Ke, Kx), dtype=np.uint8)
+    cls = np.zeros((Ke, Kx, int(n_hits)), dtype=np.uint8)
+    n_cls = np.zeros((Ke, Kx), dtype=np.int32)
+    for a in range(Ke):
+        for b in range(Kx):
+            if not (ok_e[a] and ok_x[b]):
+                continue
+            valid[a, b] = 1
+            for j in range(cls_e.shape[1]):
+                if cls_e[a, j]:
+                    cls[a, b, orig_e[j]] = 1
+            for j in range(cls_x.shape[1]):
+                if cls_x[b, j]:
+                    cls[a, b, orig_x[j]] = 1
+            n_cls[a, b] = int(cls[a, b].sum())
+    return {"valid": valid, "cls": cls, "n_cls": n_cls}
+
+
+def scan_half_tracks(seeds_e, seeds_x, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
+                     cutoff, wire_layer, circle, overlap, min_layers, half_width, n_grid, n_iter, shrink, k_ref,
+                     k_final):
+    """One turn partition as two half tracks (R38-R42): the hits are grouped by
+    half_hit_masks; the entrance-side seeds are scanned forwards against the entrance set, the exit-side
+    seeds backwards (flip_seeds, -charge) against the exit set, each by scan_stage with k_final finally
+    selected seeds (paper: 10 per side); seeds with a missing layer are vetoed; the half sets are merged
+    combinatorially.  R42: a half track ends at the apex, the first recorded state that moves inwards --
+    this is the target region of R3 with r_stop beyond the chamber (the caller passes e.g. 1e3 cm).
+    The exit-side final seeds are returned in the physical (forward) convention.
+    -> dict(ent / ext: dict(final_seed [K][6], final_rss [K], cls [K][H_half], ok [K], orig [H_half],
+            fired_wire, hit_off), valid, cls, n_cls)."""
+    H = len(rho)
+    in_e, in_x = half_hit_masks(wire_a, wire_b, fired_wire, hit_off, H, circle, overlap)
+    out = {}
+    for key, keep, sd, q in (("ent", in_e, np.asarray(seeds_e, np.float64), charge),
+                             ("ext", in_x, flip_seeds(seeds_x), -charge)):
+        fw, ho, rh, src = remove_hits(fired_wire, hit_off, rho, 1 - keep)
+        if key == "ext":
+            rh = -rh            # R38: the reversed tangent swaps left and right, so the signed drift changes sign
+        st = scan_stage(np.ascontiguousarray(sd), np.array([0, sd.shape[1]], dtype=np.int64), q, bz, step, n_steps,
+                        r_stop, wire_a, wire_b, fw, ho, rh, cutoff, half_width, n_grid, n_iter, shrink, k_ref, k_final)
+        fs = st["final_seed"][0]
+        if key == "ext":
+            fs = flip_seeds(fs.T).T
+        cls = st["cls"][0]
+        out[key] = {"final_seed": fs, "final_rss": st["final_rss"][0], "cls": cls, "orig": src, "fired_wire": fw,
+                    "hit_off": ho, "ok": layer_veto(cls, fw, ho, wire_layer, min_layers)}
+    m = merge_half_sets(out["ent"]["cls"], out["ent"]["orig"], out["ent"]["ok"],
+                        out["ext"]["cls"], out["ext"]["orig"], out["ext"]["ok"], H)
+    out.update(m)
+    return out
+
+
 KAPPA_ = 2.99792458     # R4
