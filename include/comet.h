@@ -358,6 +358,81 @@ int comet_hough_seeds(comet_ctx* ctx, const double* wire_a, const double* wire_b
                       int32_t charge, double bz_tesla, double r_seed_cm, void* work,
                       int32_t* acc, int32_t* peak, double* circle, void* cuda_stream);
 
+/* ---- half tracks (readings R38-R42) ------------------------------------- */
+
+/* "The hits of the event were also grouped into two sets for each half track".
+ * R39: the half tracks meet at the apex of the Hough circle, on the line from the origin through
+ * its centre c.  With m the (x, y) of a wire's midpoint, d = (c_x m_y - c_y m_x)/R and s = +1 if
+ * c_x e_y - c_y e_x > 0 else -1 (e the entrance point): the wire's entries belong to the entrance
+ * half iff s d > -overlap_cm and to the exit half iff s d <= overlap_cm (fp64, one IEEE operation
+ * per operation written here).  A NaN circle puts nothing in either set.
+ *   circle   dev [11]: one row of comet_hough_seeds' output (R, centre, entrance, exit)
+ *   in_ent, in_exit  dev [n_hits] 0/1 */
+int comet_half_hit_masks(comet_ctx* ctx, const double* wire_a, const double* wire_b, int32_t n_wires,
+                         const int32_t* fired_wire, const int32_t* hit_off, int32_t n_fired, int32_t n_hits,
+                         const double* circle, double overlap_cm, uint8_t* in_ent, uint8_t* in_exit,
+                         void* cuda_stream);
+
+/* "by flipping the charge and momentum" (R38): out = (x, -p) of seeds SoA
+ * [6][seed_stride] -> SoA [6][out_stride] (out may be seeds itself); the caller passes -charge to
+ * the scan and scans against -rho (the reversed tangent swaps left and right). */
+int comet_flip_seeds(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                     double* out, int64_t out_stride, void* cuda_stream);
+
+/* "the seeds which have any missing layer without the hits were excluded".  R40:
+ * with l_max the highest layer holding a classified hit of the seed, ok = 1 iff every layer
+ * 0..l_max holds one and l_max + 1 >= min_layers; nothing classified gives 0.
+ *   cls         dev [n_sel][n_hits] (e.g. comet_scan_stage's cls);  ok  dev [n_sel] 0/1
+ *   wire_layer  dev [n_wires], values in [0, 64) (not checked on the device) */
+int comet_layer_veto(comet_ctx* ctx, const uint8_t* cls, int32_t n_sel,
+                     const int32_t* fired_wire, const int32_t* hit_off, int32_t n_fired, int32_t n_hits,
+                     const int32_t* wire_layer, int32_t n_wires, int32_t min_layers, uint8_t* ok,
+                     void* cuda_stream);
+
+/* "The complete sets of classified hits were formed by combinatorially merging two half sets, one
+ * of which is from each direction".  R41: pair (a, b) is valid iff ok_e[a] and
+ * ok_x[b]; its complete set is the union of the two half sets in the event's entry numbering.
+ *   cls_e  dev [k_e][h_e], orig_e dev [h_e] (entry of the half list -> entry of the event, < n_hits),
+ *   ok_e   dev [k_e]; the same for the exit side (k_x, h_x); 1 <= k_e, k_x <= 65535
+ *   valid  dev [k_e][k_x] 0/1, cls dev [k_e][k_x][n_hits] (zeros where not valid), n_cls dev [k_e][k_x] */
+int comet_merge_half_sets(comet_ctx* ctx, const uint8_t* cls_e, const int32_t* orig_e, const uint8_t* ok_e,
+                          int32_t k_e, int32_t h_e, const uint8_t* cls_x, const int32_t* orig_x,
+                          const uint8_t* ok_x, int32_t k_x, int32_t h_x, int32_t n_hits,
+                          uint8_t* valid, uint8_t* cls, int32_t* n_cls, void* cuda_stream);
+
+/* Bytes of the device work buffer of comet_scan_half_tracks (0 for invalid arguments). */
+size_t comet_half_work_bytes(int64_t n_seeds_ent, int64_t n_seeds_exit, int32_t n_fired, int32_t n_hits,
+                             int32_t k_ref, int32_t k_final, const int32_t* n_grid);
+
+/* One turn partition as two half tracks (R38-R42): comet_half_hit_masks +
+ * comet_remove_hits give the two hit lists; the entrance-side seeds are scanned forwards against
+ * the entrance list and the exit-side seeds backwards (comet_flip_seeds, -charge, -rho) against
+ * the exit list, each by comet_scan_stage with one partition and k_final finally selected seeds
+ * (paper: 10 per side); comet_layer_veto; comet_merge_half_sets.  A half track ends at the apex:
+ * pass r_stop_cm beyond the chamber (e.g. 1e3; R42).
+ *   seeds_ent  dev SoA [6][n_ent], seeds_exit dev SoA [6][n_exit] (physical momenta), n_* >= 1
+ *   circle     dev [11] (comet_hough_seeds); wire_layer dev [n_wires]; n_hits and every hit_off even (R33)
+ *   half_seed  dev [2][k_final][6]: the finally selected seeds, entrance side then exit side (physical
+ *              momenta; NaN where none); half_rss dev [2][k_final]; half_ok dev [2][k_final]
+ *   half_cls   dev [2][k_final * n_hits]: side h's rows are [k_final][counts_host[2 h + 1]] (dense), entries
+ *              in the numbering of its half list; half_orig dev [2][n_hits]: half-list entry -> event entry
+ *   counts_host  HOST [4]: fired wires and entries of the entrance list, then of the exit list
+ *   valid dev [k_final][k_final], cls dev [k_final][k_final][n_hits], n_cls dev [k_final][k_final]
+ *   work       dev, comet_half_work_bytes(n_ent, n_exit, n_fired, n_hits, k_ref, k_final, n_grid)
+ * Synchronises cuda_stream once (the sizes of the two hit lists set the launches of the scans). */
+int comet_scan_half_tracks(comet_ctx* ctx, const double* seeds_ent, int64_t n_ent,
+                           const double* seeds_exit, int64_t n_exit,
+                           int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                           const double* wire_a, const double* wire_b, int32_t n_wires,
+                           const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                           int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                           const int32_t* wire_layer, const double* circle, double overlap_cm, int32_t min_layers,
+                           const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                           int32_t k_ref, int32_t k_final, void* work,
+                           double* half_seed, double* half_rss, uint8_t* half_ok, uint8_t* half_cls,
+                           int32_t* half_orig, int32_t* counts_host,
+                           uint8_t* valid, uint8_t* cls, int32_t* n_cls, void* cuda_stream);
+
 /* ---- whole event from host buffers ------------------------------------------------------- */
 
 /* Runs A, B and C for one event whose inputs and outputs live in HOST memory (pinned memory makes

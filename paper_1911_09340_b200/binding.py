@@ -20,7 +20,8 @@ EXPORTED_SYMBOLS = [
     "comet_fp64_peak_probe", "comet_read_stats", "comet_reserve", "comet_read_timing", "comet_scan_rss",
     "comet_select_references", "comet_refine_seeds", "comet_classify_seeds", "comet_stage_work_bytes",
     "comet_scan_stage", "comet_set_field", "comet_remove_hits", "comet_turns_work_bytes", "comet_scan_turns",
-    "comet_hough_work_bytes", "comet_hough_seeds",
+    "comet_hough_work_bytes", "comet_hough_seeds", "comet_half_hit_masks", "comet_flip_seeds", "comet_layer_veto",
+    "comet_merge_half_sets", "comet_half_work_bytes", "comet_scan_half_tracks",
 ]
 
 COMET_CHUNK = 32
@@ -90,6 +91,16 @@ def load_library():
     L.comet_hough_work_bytes.restype = sz
     L.comet_hough_seeds.argtypes = [vp, vp, vp, i32, vp, vp, i32, vp, vp, i32, dbl, dbl, i32, i32, dbl, dbl,
                                     vp, vp, vp, vp, vp]
+    L.comet_half_hit_masks.argtypes = [vp, vp, vp, i32, vp, vp, i32, i32, vp, dbl, vp, vp, vp]
+    L.comet_flip_seeds.argtypes = [vp, vp, i64, i64, vp, i64, vp]
+    L.comet_layer_veto.argtypes = [vp, vp, i32, vp, vp, i32, i32, vp, i32, i32, vp, vp]
+    L.comet_merge_half_sets.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, vp, i32, i32, i32, vp, vp, vp, vp]
+    L.comet_half_work_bytes.argtypes = [i64, i64, i32, i32, i32, i32, vp]
+    L.comet_half_work_bytes.restype = sz
+    L.comet_scan_half_tracks.argtypes = [vp, vp, i64, vp, i64, i32, dbl, dbl, i32, dbl,
+                                         vp, vp, i32, vp, vp, vp, i32, i32, dbl,
+                                         vp, vp, dbl, i32, vp, vp, i32, dbl, i32, i32, vp,
+                                         vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.comet_set_field.argtypes = [vp, vp, vp, vp, vp, dbl, vp]
     L.comet_select_references.argtypes = [vp, vp, i64, i64, vp, vp, i32, vp, i32, vp, vp]
     L.comet_refine_seeds.argtypes = [vp, vp, i64, i64, vp, i32, i32, vp, vp, vp, i64, vp]
@@ -102,7 +113,7 @@ def load_library():
                                    vp, i32, vp, vp, i32, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes", "comet_turns_work_bytes",
-                        "comet_hough_work_bytes"):
+                        "comet_hough_work_bytes", "comet_half_work_bytes"):
             getattr(L, name).restype = ctypes.c_int
     _lib = L
     return L
@@ -450,6 +461,93 @@ class Comet:
             int(work.data_ptr()), _dev(out["acc"], torch.int32, "acc", d), int(out["peak"].data_ptr()),
             int(out["circle"].data_ptr()), _stream_ptr(stream)))
         out["_work"] = work          # keeps the buffer alive until the caller drops the result
+        return out
+
+    # -- half tracks -----------------------------------------------------------------------------
+    def half_hit_masks(self, wire_a, wire_b, fired_wire, hit_off, n_hits, circle, overlap, stream=None):
+        """comet_half_hit_masks -> (in_ent, in_exit) uint8 [n_hits] (device)."""
+        d, td = self.device, self._tdev()
+        ie = torch.zeros(int(n_hits), dtype=torch.uint8, device=td)
+        ix = torch.zeros(int(n_hits), dtype=torch.uint8, device=td)
+        self._check(self._L.comet_half_hit_masks(
+            self._h, _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
+            int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d), _dev(hit_off, torch.int32, "hit_off", d),
+            int(fired_wire.shape[0]), int(n_hits), _dev(circle, torch.float64, "circle", d), float(overlap),
+            int(ie.data_ptr()), int(ix.data_ptr()), _stream_ptr(stream)))
+        return ie, ix
+
+    def flip_seeds(self, seeds, stream=None):
+        """comet_flip_seeds -> new SoA [6][S] tensor with the momentum negated."""
+        S = int(seeds.shape[1])
+        out = torch.empty_like(seeds)
+        self._check(self._L.comet_flip_seeds(self._h, _dev(seeds, torch.float64, "seeds", self.device), S, S,
+                                             int(out.data_ptr()), S, _stream_ptr(stream)))
+        return out
+
+    def layer_veto(self, cls, fired_wire, hit_off, wire_layer, min_layers, stream=None):
+        """comet_layer_veto: cls [n_sel][n_hits] -> ok uint8 [n_sel] (device)."""
+        d = self.device
+        n_sel, H = int(cls.shape[0]), int(cls.shape[1])
+        ok = torch.empty(n_sel, dtype=torch.uint8, device=self._tdev())
+        self._check(self._L.comet_layer_veto(
+            self._h, _dev(cls, torch.uint8, "cls", d), n_sel, _dev(fired_wire, torch.int32, "fired_wire", d),
+            _dev(hit_off, torch.int32, "hit_off", d), int(fired_wire.shape[0]), H,
+            _dev(wire_layer, torch.int32, "wire_layer", d), int(wire_layer.shape[0]), int(min_layers),
+            int(ok.data_ptr()), _stream_ptr(stream)))
+        return ok
+
+    def merge_half_sets(self, cls_e, orig_e, ok_e, cls_x, orig_x, ok_x, n_hits, stream=None):
+        """comet_merge_half_sets -> dict(valid [Ke][Kx], cls [Ke][Kx][n_hits], n_cls [Ke][Kx]) (device)."""
+        d, td = self.device, self._tdev()
+        Ke, He, Kx, Hx = int(cls_e.shape[0]), int(cls_e.shape[1]), int(cls_x.shape[0]), int(cls_x.shape[1])
+        out = {"valid": torch.empty((Ke, Kx), dtype=torch.uint8, device=td),
+               "cls": torch.empty((Ke, Kx, int(n_hits)), dtype=torch.uint8, device=td),
+               "n_cls": torch.empty((Ke, Kx), dtype=torch.int32, device=td)}
+        self._check(self._L.comet_merge_half_sets(
+            self._h, _dev(cls_e, torch.uint8, "cls_e", d), _dev(orig_e, torch.int32, "orig_e", d),
+            _dev(ok_e, torch.uint8, "ok_e", d), Ke, He, _dev(cls_x, torch.uint8, "cls_x", d),
+            _dev(orig_x, torch.int32, "orig_x", d), _dev(ok_x, torch.uint8, "ok_x", d), Kx, Hx, int(n_hits),
+            int(out["valid"].data_ptr()), int(out["cls"].data_ptr()), int(out["n_cls"].data_ptr()), _stream_ptr(stream)))
+        return out
+
+    def scan_half_tracks(self, seeds_e, seeds_x, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
+                         hit_off, rho, cutoff, wire_layer, circle, overlap, min_layers, half_width, n_grid, n_iter,
+                         shrink, k_ref, k_final, stream=None):
+        """comet_scan_half_tracks -> dict(ent / ext: dict(final_seed [K][6], final_rss [K], ok [K], cls [K][H_half],
+        orig [H_half], n_fired), valid, cls, n_cls) (device tensors)."""
+        d, td = self.device, self._tdev()
+        hw = np.ascontiguousarray(np.asarray(half_width, dtype=np.float64))
+        ng = np.ascontiguousarray(np.asarray(n_grid, dtype=np.int32))
+        Se, Sx, W, H, K = int(seeds_e.shape[1]), int(seeds_x.shape[1]), int(fired_wire.shape[0]), int(rho.shape[0]), int(k_final)
+        nb = int(self._L.comet_half_work_bytes(Se, Sx, W, H, int(k_ref), K, ng.ctypes.data))
+        if nb == 0:
+            raise CometError("comet_half_work_bytes: invalid arguments")
+        work = torch.empty(nb, dtype=torch.uint8, device=td)
+        hs = torch.empty((2, K, 6), dtype=torch.float64, device=td)
+        hr = torch.empty((2, K), dtype=torch.float64, device=td)
+        hok = torch.empty((2, K), dtype=torch.uint8, device=td)
+        hcls = torch.empty((2, K * H), dtype=torch.uint8, device=td)
+        horig = torch.empty((2, H), dtype=torch.int32, device=td)
+        counts = np.zeros(4, dtype=np.int32)
+        out = {"valid": torch.empty((K, K), dtype=torch.uint8, device=td),
+               "cls": torch.empty((K, K, H), dtype=torch.uint8, device=td),
+               "n_cls": torch.empty((K, K), dtype=torch.int32, device=td)}
+        self._check(self._L.comet_scan_half_tracks(
+            self._h, _dev(seeds_e, torch.float64, "seeds_e", d), Se, _dev(seeds_x, torch.float64, "seeds_x", d), Sx,
+            int(charge), float(bz), float(step), int(n_steps), float(r_stop),
+            _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d), int(wire_a.shape[1]),
+            _dev(fired_wire, torch.int32, "fired_wire", d), _dev(hit_off, torch.int32, "hit_off", d),
+            _dev(rho, torch.float64, "rho", d), W, H, float(cutoff),
+            _dev(wire_layer, torch.int32, "wire_layer", d), _dev(circle, torch.float64, "circle", d), float(overlap),
+            int(min_layers), hw.ctypes.data, ng.ctypes.data, int(n_iter), float(shrink), int(k_ref), K,
+            int(work.data_ptr()), int(hs.data_ptr()), int(hr.data_ptr()), int(hok.data_ptr()), int(hcls.data_ptr()),
+            int(horig.data_ptr()), counts.ctypes.data, int(out["valid"].data_ptr()), int(out["cls"].data_ptr()),
+            int(out["n_cls"].data_ptr()), _stream_ptr(stream)))
+        for h, key in enumerate(("ent", "ext")):
+            w, hh = int(counts[2 * h]), int(counts[2 * h + 1])
+            out[key] = {"final_seed": hs[h], "final_rss": hr[h], "ok": hok[h], "cls": hcls[h, :K * hh].view(K, hh),
+                        "orig": horig[h, :hh], "n_fired": w}
+        out["_work"] = work
         return out
 
     # -- whole event, device-resident inputs --------------------------------------------------

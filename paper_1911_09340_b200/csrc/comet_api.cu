@@ -17,6 +17,7 @@
 #include "refine.cuh"
 #include "turns.cuh"
 #include "hough.cuh"
+#include "half.cuh"
 
 #ifndef COMET_PRUNED_WT
 #define COMET_PRUNED_WT 3
@@ -1186,6 +1187,175 @@ extern "C" int comet_hough_seeds(comet_ctx* ctx, const double* wire_a, const dou
     k_hough<<<grid, COMET_HT_THREADS, smem, st>>>(wire_a, wire_b, n_wires, fired_wire, ev_off, cos_tab, sin_tab, n_phi, D,
                                                   rho_min, inv_drho, n_rho, charge, bz_tesla, r_seed_cm, acc, peak,
                                                   circle, (HoughWork*)work);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// half tracks (readings R38-R42)
+// ---------------------------------------------------------------------------------------------
+extern "C" int comet_half_hit_masks(comet_ctx* ctx, const double* wire_a, const double* wire_b, int32_t n_wires,
+                                    const int32_t* fired_wire, const int32_t* hit_off, int32_t n_fired, int32_t n_hits,
+                                    const double* circle, double overlap_cm, uint8_t* in_ent, uint8_t* in_exit,
+                                    void* cuda_stream)
+{
+    if (!ctx || n_wires < 0 || n_fired < 0 || n_hits < 0 || !circle || !(overlap_cm >= 0.0) ||
+        (n_fired > 0 && (!wire_a || !wire_b || !fired_wire || !hit_off)) || (n_hits > 0 && (!in_ent || !in_exit)))
+        return COMET_EINVAL;
+    if (n_fired == 0) return COMET_OK;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    k_half_masks<<<(n_fired + 255) / 256, 256, 0, (cudaStream_t)cuda_stream>>>(wire_a, wire_b, n_wires, fired_wire, hit_off,
+                                                                               n_fired, circle, overlap_cm, in_ent, in_exit,
+                                                                               nullptr, nullptr);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+extern "C" int comet_flip_seeds(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                                double* out, int64_t out_stride, void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || seed_stride < n_seeds || out_stride < n_seeds || (n_seeds > 0 && (!seeds || !out)))
+        return COMET_EINVAL;
+    if (n_seeds == 0) return COMET_OK;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    k_flip_seeds<<<(unsigned)((6 * n_seeds + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(seeds, seed_stride, n_seeds, out,
+                                                                                              out_stride, 0);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+extern "C" int comet_layer_veto(comet_ctx* ctx, const uint8_t* cls, int32_t n_sel,
+                                const int32_t* fired_wire, const int32_t* hit_off, int32_t n_fired, int32_t n_hits,
+                                const int32_t* wire_layer, int32_t n_wires, int32_t min_layers, uint8_t* ok,
+                                void* cuda_stream)
+{
+    if (!ctx || n_sel < 0 || n_fired < 0 || n_hits < 0 || n_wires < 0 || (n_sel > 0 && !ok) ||
+        (n_sel > 0 && n_hits > 0 && !cls) || (n_fired > 0 && (!fired_wire || !hit_off || !wire_layer)))
+        return COMET_EINVAL;
+    if (n_sel == 0) return COMET_OK;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    k_layer_veto<<<(n_sel + 7) / 8, 256, 0, (cudaStream_t)cuda_stream>>>(cls, n_sel, n_hits, fired_wire, hit_off, n_fired,
+                                                                        wire_layer, min_layers, ok);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+extern "C" int comet_merge_half_sets(comet_ctx* ctx, const uint8_t* cls_e, const int32_t* orig_e, const uint8_t* ok_e,
+                                     int32_t k_e, int32_t h_e, const uint8_t* cls_x, const int32_t* orig_x,
+                                     const uint8_t* ok_x, int32_t k_x, int32_t h_x, int32_t n_hits,
+                                     uint8_t* valid, uint8_t* cls, int32_t* n_cls, void* cuda_stream)
+{
+    if (!ctx || k_e < 1 || k_x < 1 || k_e > 65535 || k_x > 65535 || h_e < 0 || h_x < 0 || n_hits < 0 || h_e > n_hits ||
+        h_x > n_hits || !ok_e || !ok_x || !valid || !n_cls || (n_hits > 0 && !cls) || (h_e > 0 && (!cls_e || !orig_e)) ||
+        (h_x > 0 && (!cls_x || !orig_x)))
+        return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    k_merge_half<<<dim3((unsigned)k_x, (unsigned)k_e), 256, 0, (cudaStream_t)cuda_stream>>>(cls_e, orig_e, ok_e, h_e, cls_x, orig_x,
+                                                                                           ok_x, h_x, n_hits, valid, cls, n_cls);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+// work buffer of comet_scan_half_tracks: the stage work, the flipped exit-side seeds, the two remove masks, the
+// two half lists (fired, hit_off, rho; orig goes to the caller), the stage's DCAs, the four counters
+struct HalfLayout {
+    size_t stage, flip, rm[2], fw[2], ho[2], rho[2], dca, counts, total;
+};
+static HalfLayout half_layout(size_t stage_bytes, int64_t n_exit, int32_t n_fired, int32_t n_hits, int32_t k_final)
+{
+    HalfLayout L;
+    auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+    size_t o = 0;
+    L.stage = o; o += up(stage_bytes);
+    L.flip = o; o += up(sizeof(double) * 6 * (size_t)n_exit);
+    for (int h = 0; h < 2; ++h) {
+        L.rm[h] = o; o += up((size_t)n_hits);
+        L.fw[h] = o; o += up(sizeof(int32_t) * (size_t)n_fired);
+        L.ho[h] = o; o += up(sizeof(int32_t) * ((size_t)n_fired + 1));
+        L.rho[h] = o; o += up(sizeof(double) * (size_t)n_hits);
+    }
+    L.dca = o; o += up(sizeof(double) * (size_t)k_final * (size_t)n_fired);
+    L.counts = o; o += 256;
+    L.total = o;
+    return L;
+}
+
+extern "C" size_t comet_half_work_bytes(int64_t n_seeds_ent, int64_t n_seeds_exit, int32_t n_fired, int32_t n_hits,
+                                        int32_t k_ref, int32_t k_final, const int32_t* n_grid)
+{
+    if (n_seeds_ent < 1 || n_seeds_exit < 1 || n_fired < 0 || n_hits < 0) return 0;
+    const size_t sb = comet_stage_work_bytes(n_seeds_ent > n_seeds_exit ? n_seeds_ent : n_seeds_exit, 1, k_ref, k_final, n_grid);
+    if (!sb) return 0;
+    return half_layout(sb, n_seeds_exit, n_fired, n_hits, k_final).total;
+}
+
+extern "C" int comet_scan_half_tracks(comet_ctx* ctx, const double* seeds_ent, int64_t n_ent,
+                                      const double* seeds_exit, int64_t n_exit,
+                                      int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                                      const double* wire_a, const double* wire_b, int32_t n_wires,
+                                      const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                      int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                      const int32_t* wire_layer, const double* circle, double overlap_cm, int32_t min_layers,
+                                      const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                                      int32_t k_ref, int32_t k_final, void* work,
+                                      double* half_seed, double* half_rss, uint8_t* half_ok, uint8_t* half_cls,
+                                      int32_t* half_orig, int32_t* counts_host,
+                                      uint8_t* valid, uint8_t* cls, int32_t* n_cls, void* cuda_stream)
+{
+    if (!ctx || n_ent < 1 || n_exit < 1 || !seeds_ent || !seeds_exit || n_fired < 0 || n_hits < 0 || (n_hits & 1) ||
+        !circle || !(overlap_cm >= 0.0) || !work || !half_seed || !half_rss || !half_ok || !counts_host || !valid || !n_cls ||
+        !hit_off || (n_fired > 0 && (!wire_layer || !fired_wire)) || (n_hits > 0 && (!rho || !half_cls || !half_orig || !cls)))
+        return COMET_EINVAL;
+    const size_t sb = comet_stage_work_bytes(n_ent > n_exit ? n_ent : n_exit, 1, k_ref, k_final, n_grid);
+    if (!sb) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const HalfLayout L = half_layout(sb, n_exit, n_fired, n_hits, k_final);
+    char* Wk = (char*)work;
+    int32_t* counts = (int32_t*)(Wk + L.counts);
+    double* flipped = (double*)(Wk + L.flip);
+    double* dca_stage = (double*)(Wk + L.dca);
+    // the two hit lists (R39) and the backward seeds (R38)
+    if (n_fired)
+        k_half_masks<<<(n_fired + 255) / 256, 256, 0, st>>>(wire_a, wire_b, n_wires, fired_wire, hit_off, n_fired, circle,
+                                                            overlap_cm, nullptr, nullptr, (uint8_t*)(Wk + L.rm[0]),
+                                                            (uint8_t*)(Wk + L.rm[1]));
+    for (int h = 0; h < 2; ++h)
+        k_remove_hits<<<1, COMET_RM_THREADS, 0, st>>>(fired_wire, hit_off, rho, n_fired, (const uint8_t*)(Wk + L.rm[h]), nullptr,
+                                                      (int32_t*)(Wk + L.fw[h]), (int32_t*)(Wk + L.ho[h]),
+                                                      (double*)(Wk + L.rho[h]), half_orig ? half_orig + (size_t)h * n_hits : nullptr,
+                                                      counts + 2 * h);
+    k_flip_seeds<<<(unsigned)((6 * n_exit + 255) / 256), 256, 0, st>>>(seeds_exit, n_exit, n_exit, flipped, n_exit, 0);
+    CU(ctx, cudaGetLastError());
+    CU(ctx, cudaMemcpyAsync(counts_host, counts, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    CU(ctx, cudaStreamSynchronize(st));              // the sizes of the two lists set the launches of the scans
+    const size_t side_cls = (size_t)k_final * (size_t)n_hits;
+    for (int h = 0; h < 2; ++h) {
+        const int32_t w = counts_host[2 * h], hh = counts_host[2 * h + 1];
+        double* rho_h = (double*)(Wk + L.rho[h]);
+        if (h == 1 && hh) k_negate<<<(hh + 255) / 256, 256, 0, st>>>(rho_h, hh);     // R38: left and right swap
+        const int64_t ns = h == 0 ? n_ent : n_exit;
+        const int64_t one[2] = {0, ns};
+        double* fs = half_seed + (size_t)h * k_final * 6;
+        uint8_t* cls_h = half_cls ? half_cls + (size_t)h * side_cls : nullptr;
+        rc = comet_scan_stage(ctx, h == 0 ? seeds_ent : flipped, ns, ns, h == 0 ? charge : -charge, bz_tesla, step_cm, n_steps,
+                              r_stop_cm, wire_a, wire_b, n_wires, (const int32_t*)(Wk + L.fw[h]), (const int32_t*)(Wk + L.ho[h]),
+                              rho_h, w, hh, cutoff_cm, one, 1, half_width, n_grid, n_iter, shrink, k_ref, k_final,
+                              Wk + L.stage, fs, half_rss + (size_t)h * k_final, dca_stage, cls_h, st);
+        if (rc) return rc;
+        if (h == 1) k_flip_seeds<<<(6 * k_final + 255) / 256, 256, 0, st>>>(fs, 0, k_final, fs, 0, 1);
+        k_layer_veto<<<(k_final + 7) / 8, 256, 0, st>>>(cls_h, k_final, hh, (const int32_t*)(Wk + L.fw[h]),
+                                                        (const int32_t*)(Wk + L.ho[h]), w, wire_layer, min_layers,
+                                                        half_ok + (size_t)h * k_final);
+    }
+    k_merge_half<<<dim3((unsigned)k_final, (unsigned)k_final), 256, 0, st>>>(
+        half_cls, half_orig, half_ok, counts_host[1], half_cls ? half_cls + side_cls : nullptr,
+        half_orig ? half_orig + n_hits : nullptr, half_ok + k_final, counts_host[3], n_hits, valid, cls, n_cls);
     CU(ctx, cudaGetLastError());
     return COMET_OK;
 }
