@@ -46,6 +46,8 @@ STAGE_GRID = [5, 5, 5, 5]
 # `field` entry: step tolerance of R31 and the FP64-pipe instructions of one attempted Nystrom step in the map
 FIELD_TOL = 1e-7
 FIELD_STEP_INSTR = 420
+# `seeding` entry: Hough accumulator (R36): directions, rho bins, rho window in 1/cm (R from 15 to 75 cm)
+HOUGH_N_PHI, HOUGH_N_RHO, HOUGH_RHO = 256, 128, (1.0 / 150.0, 1.0 / 30.0)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1d_full_scan_fused_fine_ck.txt)
 TRAFFIC_BYTES = {"k_scan_fused": 347658496 + 2243479000, "k_fine_ck": 681160960 + 80465000}
 
@@ -344,6 +346,55 @@ def run_ours(args):
                  "k_scan_fused_tflops_model": 2.0 * FIELD_STEP_INSTR * st_field / (kt_field["k_scan_fused"] * 1e-3) / 1e12}
         del d_map
 
+    # ---- seeding workloads of SURVEY 8(f): Hough transform (NEXT #4) and one turn as two half tracks (NEXT #3) ----
+    seeding = None
+    if fused and args.seeding:
+        from comet_synth import hough_tables, make_config
+        evs = make_config(2, n_events=32)
+        lists = [e.fired_wire for e in evs] * 8                      # 256 events: the first 32 of configs[2], 8 times
+        ev_off = np.zeros(len(lists) + 1, dtype=np.int32)
+        ev_off[1:] = np.cumsum([f.size for f in lists])
+        ct, stb = hough_tables(HOUGH_N_PHI)
+        inv = HOUGH_N_RHO / (HOUGH_RHO[1] - HOUGH_RHO[0])
+        hargs = (d_wa, d_wb, dev(np.concatenate(lists)), dev(ev_off), dev(ct), dev(stb), HOUGH_RHO[0], inv, HOUGH_N_RHO,
+                 -1, 1.0, 50.0)
+        c.hough_seeds(*hargs, want_acc=False)
+        ms_h, _ = _time_steps(lambda: c.hough_seeds(*hargs, want_acc=False), 20, stream)
+        votes = float(ev_off[-1]) * HOUGH_N_PHI
+        # one turn of this event as two half tracks: Hough circle of the event, grids at the entrance and exit points
+        one = dev(np.array([0, ev.n_fired], dtype=np.int32))
+        ho1 = c.hough_seeds(d_wa, d_wb, d_fw, one, dev(ct), dev(stb), HOUGH_RHO[0], inv, HOUGH_N_RHO, ev.charge, ev.bz, 50.0,
+                            want_acc=False)
+        n0 = int(part_off[1])
+        se = d_seeds[:, :n0].contiguous()
+        hx, pt = ev.helix(), ev.partitions[0]
+        x_out = hx.position(np.asarray(pt.s_out))
+        t_out = hx.tangent(np.asarray(pt.s_out))
+        sx_h = seeds[:, :n0].copy()                                  # the same grid shape, moved to the exit state
+        sx_h[0], sx_h[1] = x_out[0], x_out[1]
+        sx_h[2] += x_out[2] - pt.z
+        rot = np.arctan2(t_out[1], t_out[0]) - pt.phi
+        px, py = sx_h[3].copy(), sx_h[4].copy()
+        sx_h[3], sx_h[4] = px * np.cos(rot) - py * np.sin(rot), px * np.sin(rot) + py * np.cos(rot)
+        sx = dev(sx_h)
+        hkw = dict(half_width=STAGE_HALF_WIDTH, n_grid=STAGE_GRID, n_iter=3, shrink=0.5, k_ref=10, k_final=10)
+        hfn = lambda: c.scan_half_tracks(se, sx, *phys, 1.0e3, *hits, ev.cutoff, dev(ev.geom.layer), ho1["circle"][0].contiguous(),
+                                         3.0, 3, **hkw)
+        hfn()
+        ms_half, hout_ = _time_steps(hfn, max(2, n_cmp // 2), stream)
+        seeding = {"hough": {"ms_per_launch": ms_h, "events": len(lists), "fired_wires": int(ev_off[-1]),
+                             "votes_per_s": votes / (ms_h * 1e-3), "events_per_s": len(lists) / (ms_h * 1e-3),
+                             "accumulator": "%d directions x %d rho bins per event, kept in shared memory (not written out)"
+                                            % (HOUGH_N_PHI, HOUGH_N_RHO),
+                             "workload": "256 events in one launch: the first 32 events of configs[2], 8 times"},
+                   "half_tracks": {"ms_per_turn": ms_half, "seeds_per_side": n0, "k_final": 10,
+                                   "valid_pairs": int(hout_["valid"].sum().item()),
+                                   "best_pair_hits": int(hout_["n_cls"][0, 0].item()),
+                                   "recipe": "comet_scan_half_tracks on turn 0 of the event: Hough circle -> two hit lists "
+                                             "(3 cm overlap), the partition's grid at the entrance and the same grid moved to "
+                                             "the truth exit state, 3 refinements per side, layer veto (>= 3 layers), 10 x 10 merge"}}
+        del hout_, se, sx
+
     # ---- e2e: host buffers through comet_scan_event_host -------------------------------------
     pin = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a)).to(dt).pin_memory()
     h = dict(seeds=pin(seeds, torch.float64), wa=pin(ev.geom.wire_a, torch.float64), wb=pin(ev.geom.wire_b, torch.float64),
@@ -449,6 +500,7 @@ def run_ours(args):
         "clocks": clocks,
         "stage": stage,
         "field": field,
+        "seeding": seeding,
         "roofline": {"kernel": top["kernel"], "bound": "alu", "achieved": top["achieved"], "peak": peak,
                      "unit": "TFLOP/s", "frac": top["achieved"] / peak, "traffic": top["traffic"],
                      "timed": top["timed"],
@@ -484,6 +536,7 @@ def main():
     ap.add_argument("--path", choices=["fused", "materialised"], default="fused")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     ap.add_argument("--no-field", dest="field", action="store_false", help="skip the field-map leg")
+    ap.add_argument("--no-seeding", dest="seeding", action="store_false", help="skip the Hough / half-track legs")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
