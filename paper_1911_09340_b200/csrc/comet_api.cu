@@ -1174,12 +1174,18 @@ extern "C" int comet_hough_seeds(comet_ctx* ctx, const double* wire_a, const dou
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    // directions per CTA: about one CTA per SM and event batch, rows of the CTA in shared memory (<= 64 KB)
+    // directions per CTA: at least one CTA per SM, and small CTAs (about COMET_HT_BINS bins in shared memory) so
+    // that a batch of events runs as many short CTAs per SM rather than one or two long waves
     int64_t ctas_per_event = (ctx->n_sm + n_events - 1) / n_events;
     int D = (int)((n_phi + ctas_per_event - 1) / ctas_per_event);
-    const int d_max = 65536 / (4 * n_rho) > 0 ? 65536 / (4 * n_rho) : 1;
+    const int d_max = COMET_HT_BINS / n_rho > 0 ? COMET_HT_BINS / n_rho : 1;
     if (D > d_max) D = d_max;
     if (D < 1) D = 1;
+    if (D < COMET_HT_THREADS) {                            // a divisor of the CTA size: threads keep their direction
+        int p2 = 1;
+        while (2 * p2 <= D) p2 *= 2;
+        D = p2;
+    }
     const size_t smem = (size_t)D * n_rho * sizeof(int) + 2 * COMET_HT_THREADS * sizeof(double);
     if (smem > 48 * 1024) CU(ctx, cudaFuncSetAttribute(k_hough, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     CU(ctx, cudaMemsetAsync(work, 0, sizeof(HoughWork) * (size_t)n_events, st));

@@ -7,7 +7,7 @@
 // per direction phi_j in the bin floor((rho - rho_min) inv_drho).  Integer/histogram work: the votes of a
 // CTA's directions are counted with shared-memory atomics (integer adds: the counts do not depend on the
 // order), the peak is a packed-key maximum (votes high word, inverted flat index low word: most votes,
-// ties -> the lowest j n_rho + k), and the last CTA of an event to finish turns the peak into the circle and
+// ties -> the lowest j n_rho + k) taken over the votes themselves (no pass over the bins), and the last CTA of an event to finish turns the peak into the circle and
 // the entrance/exit seed points (R37).  The bin of a vote is decided in fp64 with one IEEE operation per
 // operation of the definition (common.cuh's arithmetic policy).
 #pragma once
@@ -16,6 +16,9 @@
 namespace comet {
 
 #define COMET_HT_THREADS 256
+#ifndef COMET_HT_BINS
+#define COMET_HT_BINS 8192          // vote bins per CTA the launch aims at (more, smaller CTAs: a short tail)
+#endif
 
 struct HoughWork {                 // per event, zeroed by the API before the launch
     unsigned long long key;        // max over the CTAs of (votes << 32) | ~flat
@@ -84,8 +87,19 @@ k_hough(const double* __restrict__ wire_a, const double* __restrict__ wire_b, in
     const int j0 = blockIdx.x * D, nd = min(D, n_phi - j0);
     const int w0 = ev_off[ev], W = ev_off[ev + 1] - w0;
     const int n_bins = nd * n_rho;
-    for (int i = t; i < n_bins; i += COMET_HT_THREADS) s_acc[i] = 0;
+    {   // zero the rows, 16 bytes per store (s_acc is 16-byte aligned, the tail goes word by word)
+        int4* z4 = reinterpret_cast<int4*>(s_acc);
+        const int n4 = n_bins >> 2;
+        for (int i = t; i < n4; i += COMET_HT_THREADS) z4[i] = make_int4(0, 0, 0, 0);
+        for (int i = (n4 << 2) + t; i < n_bins; i += COMET_HT_THREADS) s_acc[i] = 0;
+    }
     const double n_rho_d = (double)n_rho;
+    // The peak is found while voting: the thread whose vote completes a bin's final count sees that count, so
+    // the maximum over all votes of (count after the vote, inverted flat index) is the peak with the rule of R36.
+    unsigned long long key = 0;
+    const bool fixed_d = (COMET_HT_THREADS % nd) == 0;      // CTA-uniform
+    const int d_fix = t % nd, w_first = t / nd, w_step = COMET_HT_THREADS / nd;
+    const double c_fix = cos_tab[j0 + d_fix], s_fix = sin_tab[j0 + d_fix];
     for (int base = 0; base < W; base += COMET_HT_THREADS) {
         __syncthreads();                                   // zeroing done / previous tile consumed
         const int nt = min(COMET_HT_THREADS, W - base);
@@ -98,23 +112,30 @@ k_hough(const double* __restrict__ wire_a, const double* __restrict__ wire_b, in
             s_v[t] = xdiv(y, r2);
         }
         __syncthreads();
-        for (int i = t; i < nt * nd; i += COMET_HT_THREADS) {
-            const int w = i / nd, d = i - w * nd;
-            const double rho = xadd(xmul(s_u[w], cos_tab[j0 + d]), xmul(s_v[w], sin_tab[j0 + d]));
+        auto vote = [&](int w, int d, double cd, double sd) {
+            const double rho = xadd(xmul(s_u[w], cd), xmul(s_v[w], sd));
             const double k = floor(xmul(xsub(rho, rho_min), inv_drho));
-            if (k >= 0.0 && k < n_rho_d) atomicAdd(&s_acc[d * n_rho + (int)k], 1);
+            if (k >= 0.0 && k < n_rho_d) {
+                const int bin = d * n_rho + (int)k;
+                const unsigned int c = (unsigned int)atomicAdd(&s_acc[bin], 1) + 1u;
+                const unsigned int flat = (unsigned int)(j0 * n_rho + bin);
+                const unsigned long long kk = ((unsigned long long)c << 32) | (unsigned long long)(~flat);
+                key = kk > key ? kk : key;
+            }
+        };
+        if (fixed_d) {                                     // the thread keeps its direction: tables in registers
+            for (int w = w_first; w < nt; w += w_step) vote(w, d_fix, c_fix, s_fix);
+        } else {
+            for (int i = t; i < nt * nd; i += COMET_HT_THREADS) {
+                const int w = i / nd, d = i - w * nd;
+                vote(w, d, cos_tab[j0 + d], sin_tab[j0 + d]);
+            }
         }
     }
-    __syncthreads();
-    // rows out (optional) and the CTA's peak
-    unsigned long long key = 0;
-    int32_t* acc_e = acc ? acc + ((size_t)ev * n_phi + j0) * n_rho : nullptr;
-    for (int i = t; i < n_bins; i += COMET_HT_THREADS) {
-        const int c = s_acc[i];
-        if (acc_e) acc_e[i] = c;
-        const unsigned int flat = (unsigned int)(j0 * n_rho + i);
-        const unsigned long long kk = ((unsigned long long)(unsigned int)c << 32) | (unsigned long long)(~flat);
-        key = kk > key ? kk : key;
+    if (acc) {                                             // rows out (optional)
+        __syncthreads();
+        int32_t* acc_e = acc + ((size_t)ev * n_phi + j0) * n_rho;
+        for (int i = t; i < n_bins; i += COMET_HT_THREADS) acc_e[i] = s_acc[i];
     }
     for (int o = 16; o > 0; o >>= 1) {
         const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
@@ -124,7 +145,7 @@ k_hough(const double* __restrict__ wire_a, const double* __restrict__ wire_b, in
     __syncthreads();
     if (t == 0) {
         for (int i = 1; i < COMET_HT_THREADS / 32; ++i) key = s_key[i] > key ? s_key[i] : key;
-        atomicMax(&work[ev].key, key);
+        if (key) atomicMax(&work[ev].key, key);
         __threadfence();
         s_last = atomicAdd(&work[ev].done, 1u) == gridDim.x - 1;
     }
@@ -133,7 +154,7 @@ k_hough(const double* __restrict__ wire_a, const double* __restrict__ wire_b, in
     __threadfence();
     const unsigned long long best = atomicMax(&work[ev].key, 0ull);   // atomic read of the final key
     const int votes = (int)(best >> 32);
-    const unsigned int flat = ~(unsigned int)(best & 0xffffffffu);
+    const unsigned int flat = best ? ~(unsigned int)(best & 0xffffffffu) : 0u;   // no votes: peak (0, 0, 0)
     const int j = (int)(flat / (unsigned int)n_rho), k = (int)(flat - (unsigned int)j * (unsigned int)n_rho);
     peak[3 * ev] = votes;
     peak[3 * ev + 1] = j;
