@@ -181,3 +181,31 @@ def test_scan_half_tracks_without_a_circle(comet, cfg0_event):
     torch.cuda.synchronize()
     _compare_half_tracks(got, ref, ev.n_hits)
     assert got["ent"]["n_fired"] == 0 and not got["valid"].any().item() and not got["cls"].any().item()
+
+
+def test_scan_half_tracks_full_size_as_benchmarked(comet, cfg1_event):
+    """configs[1], turn 0, in the configuration bench.py's `seeding.half_tracks` leg times: the full 131072-seed grid
+    per side (the partition's grid at the entrance, the same grid moved to the truth exit state), 3 refinements of
+    10 references x 5^4 seeds per side, 10 finally selected seeds per side, 10 x 10 merge -- identical to the oracle."""
+    ev = cfg1_event
+    circ = _circle(ev)
+    sp = ev.spec
+    se = seed_grid(ev, 0, sp["grid"], tuple(sp["p_range"]), ct_range=sp.get("ct_range"), ct_hw=sp.get("ct_hw", 0.15))
+    assert se.shape[1] == 131072
+    x_out, t_out = _exit_state(ev, 0)
+    pt = ev.partitions[0]
+    sx = se.copy()
+    sx[0], sx[1] = x_out[0], x_out[1]
+    sx[2] += x_out[2] - pt.z
+    rot = np.arctan2(t_out[1], t_out[0]) - pt.phi
+    px, py = sx[3].copy(), sx[4].copy()
+    sx[3], sx[4] = px * np.cos(rot) - py * np.sin(rot), px * np.sin(rot) + py * np.cos(rot)
+    kw = dict(half_width=[0.6, 0.5, 0.5, 1.0], n_grid=[5, 5, 5, 5], n_iter=3, shrink=0.5, k_ref=10, k_final=10)
+    got = comet.scan_half_tracks(_dev(se), _dev(sx), ev.charge, ev.bz, ev.step, ev.n_steps, R_HALF,
+                                 _dev(ev.geom.wire_a), _dev(ev.geom.wire_b), _dev(ev.fired_wire), _dev(ev.hit_off),
+                                 _dev(ev.rho), ev.cutoff, _dev(ev.geom.layer), _dev(circ), 3.0, 3, **kw)
+    torch.cuda.synchronize()
+    ref = O.scan_half_tracks(se, sx, ev.charge, ev.bz, ev.step, ev.n_steps, R_HALF, ev.geom.wire_a, ev.geom.wire_b,
+                             ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, ev.geom.layer, circ, 3.0, 3, **kw)
+    _compare_half_tracks(got, ref, ev.n_hits)
+    assert ref["valid"].sum() >= 50 and ref["n_cls"].max() >= 40
