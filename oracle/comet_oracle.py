@@ -519,4 +519,58 @@ def scan_half_tracks(seeds_e, seeds_x, charge, bz, step, n_steps, r_stop, wire_a
     return out
 
 
+def best_pair(valid, n_cls):
+    """R43: the complete set that goes on -- the paper keeps the one whose fit has the highest NDF (PAPER.md:250);
+    without the fit, the valid pair with the most classified entries, ties -> the lowest a K_x + b; -1 = none."""
+    valid, n_cls = np.asarray(valid), np.asarray(n_cls)
+    best, arg = -1, -1
+    for a in range(valid.shape[0]):
+        for b in range(valid.shape[1]):
+            if valid[a, b] and n_cls[a, b] > best:
+                best, arg = int(n_cls[a, b]), a * valid.shape[1] + b
+    return arg
+
+
+def scan_turns_half(seeds_e, off_e, seeds_x, off_x, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
+                    hit_off, rho, cutoff, wire_layer, circle, overlap, min_layers, half_width, n_grid, n_iter, shrink,
+                    k_ref, k_final, min_wires=30, max_tracks=5):
+    """The event loop of Fig. 13 with half tracks and without the fits: the last turn partition
+    first; scan_half_tracks of the turn's entrance- and exit-side seed sets against the hits that are left; the
+    complete set of best_pair (R43) is the turn's, its hits are removed (remove_hits) before the previous turn;
+    the loop stops when fewer than min_wires fired wires are left, max_tracks turns are done (R34) or a turn has
+    no valid pair (":244 If the fitting results were not converged for any of the complete sets, the event
+    reconstruction process was stopped").  The transverse seed (the circle) is the same for every turn (:256).
+    -> dict(turn_pair [P][2] (-1 = none), turn_n [P], turn_cls [P][H] in the event's own numbering,
+            turn_seed [P][2][6] (entrance, exit), done [P], wires_before [P])."""
+    seeds_e, seeds_x = _c(seeds_e, np.float64), _c(seeds_x, np.float64)
+    off_e, off_x = np.asarray(off_e, np.int64), np.asarray(off_x, np.int64)
+    P, H, K = off_e.shape[0] - 1, len(rho), int(k_final)
+    fw, ho, rh = np.asarray(fired_wire, np.int32), np.asarray(hit_off, np.int32), np.asarray(rho, np.float64)
+    orig = np.arange(H, dtype=np.int32)
+    out = {"turn_pair": np.full((P, 2), -1, dtype=np.int32), "turn_n": np.zeros(P, dtype=np.int32),
+           "turn_cls": np.zeros((P, H), dtype=np.uint8), "turn_seed": np.full((P, 2, 6), np.nan),
+           "done": np.zeros(P, dtype=bool), "wires_before": np.zeros(P, dtype=np.int32)}
+    n_done = 0
+    for p in range(P - 1, -1, -1):
+        if fw.shape[0] < min_wires or n_done >= max_tracks:
+            break
+        se = np.ascontiguousarray(seeds_e[:, off_e[p]:off_e[p + 1]])
+        sx = np.ascontiguousarray(seeds_x[:, off_x[p]:off_x[p + 1]])
+        ht = scan_half_tracks(se, sx, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fw, ho, rh, cutoff, wire_layer,
+                              circle, overlap, min_layers, half_width, n_grid, n_iter, shrink, k_ref, k_final)
+        out["wires_before"][p] = fw.shape[0]
+        arg = best_pair(ht["valid"], ht["n_cls"])
+        if arg < 0:
+            break
+        a, b = divmod(arg, K)
+        cls = ht["cls"][a, b]
+        out["turn_pair"][p], out["turn_n"][p], out["done"][p] = (a, b), ht["n_cls"][a, b], True
+        out["turn_seed"][p, 0], out["turn_seed"][p, 1] = ht["ent"]["final_seed"][a], ht["ext"]["final_seed"][b]
+        out["turn_cls"][p, orig[cls.astype(bool)]] = 1
+        fw, ho, rh, src = remove_hits(fw, ho, rh, cls)
+        orig = orig[src]
+        n_done += 1
+    return out
+
+
 KAPPA_ = 2.99792458     # R4

@@ -209,3 +209,26 @@ def test_scan_half_tracks_full_size_as_benchmarked(comet, cfg1_event):
                              ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, ev.geom.layer, circ, 3.0, 3, **kw)
     _compare_half_tracks(got, ref, ev.n_hits)
     assert ref["valid"].sum() >= 50 and ref["n_cls"].max() >= 40
+
+
+def test_half_track_argument_errors(comet, cfg0_event):
+    from paper_1911_09340_b200 import CometError
+    ev = cfg0_event
+    wa, wb, fw, ho, rho = (_dev(ev.geom.wire_a), _dev(ev.geom.wire_b), _dev(ev.fired_wire), _dev(ev.hit_off), _dev(ev.rho))
+    circ, lay = _dev(_circle(ev)), _dev(ev.geom.layer)
+    se = _dev(truth_seed(ev, 0).reshape(6, 1))
+    good = dict(half_width=[1.0, 1.0, 1.0, 1.0], n_grid=[2, 2, 2, 2], n_iter=1, shrink=0.5, k_ref=2, k_final=2)
+    with pytest.raises(CometError):                                  # negative overlap
+        comet.half_hit_masks(wa, wb, fw, ho, ev.n_hits, circ, -1.0)
+    with pytest.raises(CometError):                                  # negative overlap in the whole call
+        comet.scan_half_tracks(se, se, ev.charge, ev.bz, ev.step, ev.n_steps, R_HALF, wa, wb, fw, ho, rho, ev.cutoff,
+                               lay, circ, -0.5, 3, **good)
+    with pytest.raises(CometError):                                  # an odd number of entries breaks the ghost pairs (R33)
+        comet.scan_half_tracks(se, se, ev.charge, ev.bz, ev.step, ev.n_steps, R_HALF, wa, wb, fw, ho, rho[:-1].contiguous(),
+                               ev.cutoff, lay, circ, 1.0, 3, **good)
+    with pytest.raises(CometError):                                  # grid sizes out of range
+        comet.scan_half_tracks(se, se, ev.charge, ev.bz, ev.step, ev.n_steps, R_HALF, wa, wb, fw, ho, rho, ev.cutoff,
+                               lay, circ, 1.0, 3, **dict(good, n_grid=[0, 2, 2, 2]))
+    with pytest.raises(CometError):                                  # half lists longer than the event
+        comet.merge_half_sets(_dev(np.zeros((1, 8), np.uint8)), _dev(np.arange(8, dtype=np.int32)), _dev(np.ones(1, np.uint8)),
+                              _dev(np.zeros((1, 2), np.uint8)), _dev(np.arange(2, dtype=np.int32)), _dev(np.ones(1, np.uint8)), 4)

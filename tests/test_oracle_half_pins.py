@@ -195,3 +195,75 @@ def test_two_truth_half_tracks_cover_the_turn():
                        ev.geom.wire_b, ex["fired_wire"], ex["hit_off"], ev.rho[ex["orig"]], ev.cutoff, **kw)
     picked = ex["orig"][bad["cls"][0, 0].astype(bool)]
     assert picked.size >= 5 and np.mean(ev.hit_real[picked]) < 0.5
+
+
+def test_best_pair_hand_cases():
+    valid = np.array([[1, 0, 1], [1, 1, 0]], dtype=np.uint8)
+    n = np.array([[5, 99, 7], [7, 6, 50]], dtype=np.int32)
+    assert O.best_pair(valid, n) == 2                     # 7 at (0, 2) and (1, 0): the lower flat index; 99 and 50 are not valid
+    assert O.best_pair(np.zeros((2, 3), np.uint8), n) == -1
+    assert O.best_pair(np.ones((2, 3), np.uint8), n) == 1
+    assert O.best_pair(np.ones((1, 1), np.uint8), np.zeros((1, 1), np.int32)) == 0       # a valid empty set still counts
+    rng = np.random.default_rng(4)
+    for _ in range(50):
+        v, m = (rng.uniform(size=(4, 5)) < 0.5).astype(np.uint8), rng.integers(0, 6, size=(4, 5)).astype(np.int32)
+        key = np.where(v.ravel() > 0, m.ravel(), -1)
+        want = int(np.argmax(key)) if key.max() >= 0 else -1                             # first maximum
+        assert O.best_pair(v, m) == want
+
+
+def _turn_seed_sets(ev, shape_e=(5, 5, 5, 4), shape_x=(5, 5, 4, 5)):
+    from comet_synth import seed_grid
+    pr = tuple(ev.spec["p_range"])
+    se, sx = [], []
+    for p in range(len(ev.partitions)):
+        se.append(seed_grid(ev, p, shape_e, pr, ct_hw=0.15))
+        x, T = _exit_seed(ev, p)[:3], _exit_seed(ev, p)[3:] / ev.pmag
+        g = seed_grid(ev, p, shape_x, pr, ct_hw=0.15)                # the partition's grid moved to the exit state
+        pt = ev.partitions[p]
+        rot = np.arctan2(T[1], T[0]) - pt.phi
+        px, py = g[3].copy(), g[4].copy()
+        g[0], g[1], g[2] = x[0], x[1], g[2] + (x[2] - pt.z)
+        g[3], g[4] = px * np.cos(rot) - py * np.sin(rot), px * np.sin(rot) + py * np.cos(rot)
+        sx.append(g)
+    off = lambda blocks: np.concatenate([[0], np.cumsum([b.shape[1] for b in blocks])]).astype(np.int64)
+    return np.concatenate(se, axis=1), off(se), np.concatenate(sx, axis=1), off(sx)
+
+
+def test_event_loop_with_half_tracks_takes_turns_apart():
+    ev = make_config(1)[0]
+    c, s = hough_tables(256)
+    hs = O.hough_seeds(ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, c, s, 1 / 120.0, 128 / (1 / 40.0 - 1 / 120.0), 128,
+                       ev.charge, ev.bz, 50.0)
+    circ = np.concatenate([[hs["R"]], hs["centre"], hs["entrance"], hs["exit"]])
+    se, oe, sx, ox = _turn_seed_sets(ev)
+    args = (ev.charge, ev.bz, ev.step, ev.n_steps, R_HALF, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, ev.hit_off,
+            ev.rho, ev.cutoff, ev.geom.layer, circ, 3.0, 3)
+    kw = dict(half_width=[1.0, 1.2, 1.2, 1.5], n_grid=[3, 3, 3, 3], n_iter=2, shrink=0.5, k_ref=3, k_final=3)
+    out = O.scan_turns_half(se, oe, sx, ox, *args, min_wires=10, **kw)
+    P = len(oe) - 1
+    assert out["done"].all() and (out["turn_pair"] >= 0).all()
+    wb = out["wires_before"]
+    assert wb[P - 1] == ev.n_fired and np.all(np.diff(wb[::-1]) < 0)       # fewer wires for every earlier turn
+    cls = out["turn_cls"].astype(int)
+    assert cls.sum(axis=0).max() == 1                                      # a hit entry goes to one turn only
+    assert cls.sum(axis=0).reshape(-1, 2).sum(axis=1).max() == 1           # never both ghosts of a hit
+    turn = np.asarray(ev.hit_turn)
+    for p in range(P):
+        got = turn[cls[p].astype(bool)]
+        assert got.size == out["turn_n"][p] >= 30 and np.mean(got == p) > 0.75
+    # the first stage is scan_half_tracks on the full list with best_pair's choice
+    ht = O.scan_half_tracks(se[:, oe[P - 1]:oe[P]], sx[:, ox[P - 1]:ox[P]], *args, **kw)
+    a, b = divmod(O.best_pair(ht["valid"], ht["n_cls"]), 3)
+    assert tuple(out["turn_pair"][P - 1]) == (a, b)
+    np.testing.assert_array_equal(out["turn_cls"][P - 1], ht["cls"][a, b])
+    np.testing.assert_array_equal(out["turn_seed"][P - 1, 0], ht["ent"]["final_seed"][a])
+    np.testing.assert_array_equal(out["turn_seed"][P - 1, 1], ht["ext"]["final_seed"][b])
+    # stopping rules: max_tracks, min_wires, and a turn without a valid pair (a veto nothing passes)
+    one = O.scan_turns_half(se, oe, sx, ox, *args, min_wires=10, max_tracks=1, **kw)
+    assert one["done"].tolist() == [False] * (P - 1) + [True]
+    none = O.scan_turns_half(se, oe, sx, ox, *args, min_wires=ev.n_fired + 1, **kw)
+    assert not none["done"].any() and not none["wires_before"].any()
+    veto = O.scan_turns_half(se, oe, sx, ox, *args[:-1], 21, min_wires=10, **kw)
+    assert not veto["done"].any() and veto["wires_before"].tolist() == [0] * (P - 1) + [ev.n_fired]
+    assert not veto["turn_cls"].any() and np.isnan(veto["turn_seed"]).all()
