@@ -433,6 +433,37 @@ int comet_scan_half_tracks(comet_ctx* ctx, const double* seeds_ent, int64_t n_en
                            int32_t* half_orig, int32_t* counts_host,
                            uint8_t* valid, uint8_t* cls, int32_t* n_cls, void* cuda_stream);
 
+/* Bytes of the device work buffer of comet_scan_turns_half (0 for invalid arguments). */
+size_t comet_turns_half_work_bytes(int64_t max_seeds_ent, int64_t max_seeds_exit, int32_t n_fired, int32_t n_hits,
+                                   int32_t k_ref, int32_t k_final, const int32_t* n_grid);
+
+/* The event loop of Fig. 13 with half tracks and without the fits (GENFIT2, out of
+ * scope): the last turn partition first; comet_scan_half_tracks of the turn's entrance- and
+ * exit-side seed sets against the hits that are left; the complete set that goes on is the valid
+ * pair with the most classified entries, ties -> the lowest a k_final + b (R43: stands in for the
+ * highest NDF of the fits); its hits are removed (comet_remove_hits) before the
+ * previous turn.  Stops when fewer than min_wires fired wires are left, max_tracks turns are done
+ * (R34) or a turn has no valid pair.  The circle is the same for every turn (:256).
+ *   seeds_ent   dev SoA [6][n_ent], off_ent HOST [n_part+1] (off[0] = 0, off[n_part] = n_ent, no empty
+ *               partition); the same for the exit side
+ *   turn_pair   dev [n_part][2] int32 (a, b), -1 where no turn was taken; turn_n dev [n_part] its entries
+ *   turn_seed   dev [n_part][2][6]: the pair's entrance- and exit-side seeds (NaN where none)
+ *   turn_cls    dev [n_part][n_hits]: the turn's complete set in the event's own entry numbering
+ *   done_host, wires_before_host  HOST [n_part]: 1 where a turn was taken; fired wires its scan started with
+ *   work        dev, comet_turns_half_work_bytes(largest entrance set, largest exit set, n_fired, n_hits, ...)
+ * Synchronises cuda_stream twice per turn (the sizes of the hit lists set the launches). */
+int comet_scan_turns_half(comet_ctx* ctx, const double* seeds_ent, const int64_t* off_ent, int64_t n_ent,
+                          const double* seeds_exit, const int64_t* off_exit, int64_t n_exit, int32_t n_part,
+                          int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                          const double* wire_a, const double* wire_b, int32_t n_wires,
+                          const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                          int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                          const int32_t* wire_layer, const double* circle, double overlap_cm, int32_t min_layers,
+                          const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                          int32_t k_ref, int32_t k_final, int32_t min_wires, int32_t max_tracks, void* work,
+                          int32_t* turn_pair, int32_t* turn_n, double* turn_seed, uint8_t* turn_cls,
+                          int32_t* done_host, int32_t* wires_before_host, void* cuda_stream);
+
 /* ---- whole event from host buffers ------------------------------------------------------- */
 
 /* Runs A, B and C for one event whose inputs and outputs live in HOST memory (pinned memory makes

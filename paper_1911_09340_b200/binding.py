@@ -22,6 +22,7 @@ EXPORTED_SYMBOLS = [
     "comet_scan_stage", "comet_set_field", "comet_remove_hits", "comet_turns_work_bytes", "comet_scan_turns",
     "comet_hough_work_bytes", "comet_hough_seeds", "comet_half_hit_masks", "comet_flip_seeds", "comet_layer_veto",
     "comet_merge_half_sets", "comet_half_work_bytes", "comet_scan_half_tracks",
+    "comet_turns_half_work_bytes", "comet_scan_turns_half",
 ]
 
 COMET_CHUNK = 32
@@ -101,6 +102,12 @@ def load_library():
                                          vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                          vp, vp, dbl, i32, vp, vp, i32, dbl, i32, i32, vp,
                                          vp, vp, vp, vp, vp, vp, vp, vp, vp, vp]
+    L.comet_turns_half_work_bytes.argtypes = [i64, i64, i32, i32, i32, i32, vp]
+    L.comet_turns_half_work_bytes.restype = sz
+    L.comet_scan_turns_half.argtypes = [vp, vp, vp, i64, vp, vp, i64, i32, i32, dbl, dbl, i32, dbl,
+                                        vp, vp, i32, vp, vp, vp, i32, i32, dbl,
+                                        vp, vp, dbl, i32, vp, vp, i32, dbl, i32, i32, i32, i32, vp,
+                                        vp, vp, vp, vp, vp, vp, vp]
     L.comet_set_field.argtypes = [vp, vp, vp, vp, vp, dbl, vp]
     L.comet_select_references.argtypes = [vp, vp, i64, i64, vp, vp, i32, vp, i32, vp, vp]
     L.comet_refine_seeds.argtypes = [vp, vp, i64, i64, vp, i32, i32, vp, vp, vp, i64, vp]
@@ -113,7 +120,8 @@ def load_library():
                                    vp, i32, vp, vp, i32, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes", "comet_turns_work_bytes",
-                        "comet_hough_work_bytes", "comet_half_work_bytes"):
+                        "comet_hough_work_bytes", "comet_half_work_bytes",
+                        "comet_turns_half_work_bytes"):
             getattr(L, name).restype = ctypes.c_int
     _lib = L
     return L
@@ -548,6 +556,44 @@ class Comet:
             out[key] = {"final_seed": hs[h], "final_rss": hr[h], "ok": hok[h], "cls": hcls[h, :K * hh].view(K, hh),
                         "orig": horig[h, :hh], "n_fired": w}
         out["_work"] = work
+        return out
+
+    def scan_turns_half(self, seeds_e, off_e, seeds_x, off_x, charge, bz, step, n_steps, r_stop, wire_a, wire_b,
+                        fired_wire, hit_off, rho, cutoff, wire_layer, circle, overlap, min_layers, half_width, n_grid,
+                        n_iter, shrink, k_ref, k_final, min_wires=30, max_tracks=5, stream=None):
+        """comet_scan_turns_half: the event loop of Fig. 13 with half tracks (last turn first, the best complete set's
+        hits removed before the previous turn)."""
+        d, td = self.device, self._tdev()
+        oe = np.ascontiguousarray(np.asarray(off_e, dtype=np.int64))
+        ox = np.ascontiguousarray(np.asarray(off_x, dtype=np.int64))
+        hw = np.ascontiguousarray(np.asarray(half_width, dtype=np.float64))
+        ng = np.ascontiguousarray(np.asarray(n_grid, dtype=np.int32))
+        P, W, H = oe.shape[0] - 1, int(fired_wire.shape[0]), int(rho.shape[0])
+        Se, Sx = int(seeds_e.shape[1]), int(seeds_x.shape[1])
+        nb = int(self._L.comet_turns_half_work_bytes(int(np.diff(oe).max()), int(np.diff(ox).max()), W, H, int(k_ref),
+                                                     int(k_final), ng.ctypes.data))
+        if nb == 0:
+            raise CometError("comet_turns_half_work_bytes: invalid arguments")
+        work = torch.empty(nb, dtype=torch.uint8, device=td)
+        out = {"turn_pair": torch.empty((P, 2), dtype=torch.int32, device=td),
+               "turn_n": torch.empty(P, dtype=torch.int32, device=td),
+               "turn_seed": torch.empty((P, 2, 6), dtype=torch.float64, device=td),
+               "turn_cls": torch.empty((P, H), dtype=torch.uint8, device=td)}
+        done = np.zeros(P, dtype=np.int32)
+        wb = np.zeros(P, dtype=np.int32)
+        self._check(self._L.comet_scan_turns_half(
+            self._h, _dev(seeds_e, torch.float64, "seeds_e", d), oe.ctypes.data, Se,
+            _dev(seeds_x, torch.float64, "seeds_x", d), ox.ctypes.data, Sx, P,
+            int(charge), float(bz), float(step), int(n_steps), float(r_stop),
+            _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d), int(wire_a.shape[1]),
+            _dev(fired_wire, torch.int32, "fired_wire", d), _dev(hit_off, torch.int32, "hit_off", d),
+            _dev(rho, torch.float64, "rho", d), W, H, float(cutoff),
+            _dev(wire_layer, torch.int32, "wire_layer", d), _dev(circle, torch.float64, "circle", d), float(overlap),
+            int(min_layers), hw.ctypes.data, ng.ctypes.data, int(n_iter), float(shrink), int(k_ref), int(k_final),
+            int(min_wires), int(max_tracks), int(work.data_ptr()), int(out["turn_pair"].data_ptr()),
+            int(out["turn_n"].data_ptr()), int(out["turn_seed"].data_ptr()), int(out["turn_cls"].data_ptr()),
+            done.ctypes.data, wb.ctypes.data, _stream_ptr(stream)))
+        out["done"], out["wires_before"] = done.astype(bool), wb
         return out
 
     # -- whole event, device-resident inputs --------------------------------------------------

@@ -1299,9 +1299,9 @@ extern "C" size_t comet_half_work_bytes(int64_t n_seeds_ent, int64_t n_seeds_exi
     return half_layout(sb, n_seeds_exit, n_fired, n_hits, k_final).total;
 }
 
-extern "C" int comet_scan_half_tracks(comet_ctx* ctx, const double* seeds_ent, int64_t n_ent,
-                                      const double* seeds_exit, int64_t n_exit,
-                                      int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+static int half_tracks_impl(comet_ctx* ctx, const double* seeds_ent, int64_t stride_ent, int64_t n_ent,
+                            const double* seeds_exit, int64_t stride_exit, int64_t n_exit,
+                            int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                                       const double* wire_a, const double* wire_b, int32_t n_wires,
                                       const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
                                       int32_t n_fired, int32_t n_hits, double cutoff_cm,
@@ -1312,7 +1312,8 @@ extern "C" int comet_scan_half_tracks(comet_ctx* ctx, const double* seeds_ent, i
                                       int32_t* half_orig, int32_t* counts_host,
                                       uint8_t* valid, uint8_t* cls, int32_t* n_cls, void* cuda_stream)
 {
-    if (!ctx || n_ent < 1 || n_exit < 1 || !seeds_ent || !seeds_exit || n_fired < 0 || n_hits < 0 || (n_hits & 1) ||
+    if (!ctx || n_ent < 1 || n_exit < 1 || stride_ent < n_ent || stride_exit < n_exit || !seeds_ent || !seeds_exit ||
+        n_fired < 0 || n_hits < 0 || (n_hits & 1) ||
         !circle || !(overlap_cm >= 0.0) || !work || !half_seed || !half_rss || !half_ok || !counts_host || !valid || !n_cls ||
         !hit_off || (n_fired > 0 && (!wire_layer || !fired_wire)) || (n_hits > 0 && (!rho || !half_cls || !half_orig || !cls)))
         return COMET_EINVAL;
@@ -1336,7 +1337,7 @@ extern "C" int comet_scan_half_tracks(comet_ctx* ctx, const double* seeds_ent, i
                                                       (int32_t*)(Wk + L.fw[h]), (int32_t*)(Wk + L.ho[h]),
                                                       (double*)(Wk + L.rho[h]), half_orig ? half_orig + (size_t)h * n_hits : nullptr,
                                                       counts + 2 * h);
-    k_flip_seeds<<<(unsigned)((6 * n_exit + 255) / 256), 256, 0, st>>>(seeds_exit, n_exit, n_exit, flipped, n_exit, 0);
+    k_flip_seeds<<<(unsigned)((6 * n_exit + 255) / 256), 256, 0, st>>>(seeds_exit, stride_exit, n_exit, flipped, n_exit, 0);
     CU(ctx, cudaGetLastError());
     CU(ctx, cudaMemcpyAsync(counts_host, counts, 4 * sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     CU(ctx, cudaStreamSynchronize(st));              // the sizes of the two lists set the launches of the scans
@@ -1349,7 +1350,7 @@ extern "C" int comet_scan_half_tracks(comet_ctx* ctx, const double* seeds_ent, i
         const int64_t one[2] = {0, ns};
         double* fs = half_seed + (size_t)h * k_final * 6;
         uint8_t* cls_h = half_cls ? half_cls + (size_t)h * side_cls : nullptr;
-        rc = comet_scan_stage(ctx, h == 0 ? seeds_ent : flipped, ns, ns, h == 0 ? charge : -charge, bz_tesla, step_cm, n_steps,
+        rc = comet_scan_stage(ctx, h == 0 ? seeds_ent : flipped, h == 0 ? stride_ent : ns, ns, h == 0 ? charge : -charge, bz_tesla, step_cm, n_steps,
                               r_stop_cm, wire_a, wire_b, n_wires, (const int32_t*)(Wk + L.fw[h]), (const int32_t*)(Wk + L.ho[h]),
                               rho_h, w, hh, cutoff_cm, one, 1, half_width, n_grid, n_iter, shrink, k_ref, k_final,
                               Wk + L.stage, fs, half_rss + (size_t)h * k_final, dca_stage, cls_h, st);
@@ -1363,6 +1364,149 @@ extern "C" int comet_scan_half_tracks(comet_ctx* ctx, const double* seeds_ent, i
         half_cls, half_orig, half_ok, counts_host[1], half_cls ? half_cls + side_cls : nullptr,
         half_orig ? half_orig + n_hits : nullptr, half_ok + k_final, counts_host[3], n_hits, valid, cls, n_cls);
     CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+extern "C" int comet_scan_half_tracks(comet_ctx* ctx, const double* seeds_ent, int64_t n_ent,
+                                      const double* seeds_exit, int64_t n_exit,
+                                      int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                                      const double* wire_a, const double* wire_b, int32_t n_wires,
+                                      const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                      int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                      const int32_t* wire_layer, const double* circle, double overlap_cm, int32_t min_layers,
+                                      const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                                      int32_t k_ref, int32_t k_final, void* work,
+                                      double* half_seed, double* half_rss, uint8_t* half_ok, uint8_t* half_cls,
+                                      int32_t* half_orig, int32_t* counts_host,
+                                      uint8_t* valid, uint8_t* cls, int32_t* n_cls, void* cuda_stream)
+{
+    return half_tracks_impl(ctx, seeds_ent, n_ent, n_ent, seeds_exit, n_exit, n_exit, charge, bz_tesla, step_cm, n_steps,
+                            r_stop_cm, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm,
+                            wire_layer, circle, overlap_cm, min_layers, half_width, n_grid, n_iter, shrink, k_ref, k_final,
+                            work, half_seed, half_rss, half_ok, half_cls, half_orig, counts_host, valid, cls, n_cls,
+                            cuda_stream);
+}
+
+// work buffer of comet_scan_turns_half: the half-track work, the half-track outputs of a turn, the chosen set,
+// two reduced hit lists (fired, hit_off, rho, orig), the counters
+struct TurnsHalfLayout {
+    size_t half, hseed, hrss, hok, hcls, horig, valid, cls, ncls, best, pick, list[2], o_fired, o_off, o_rho, o_orig, total;
+};
+static TurnsHalfLayout turns_half_layout(size_t half_bytes, int32_t n_fired, int32_t n_hits, int32_t K)
+{
+    TurnsHalfLayout L;
+    auto up = [](size_t v) { return (v + 255) / 256 * 256; };
+    size_t o = 0;
+    L.half = o; o += up(half_bytes);
+    L.hseed = o; o += up(sizeof(double) * 2 * 6 * (size_t)K);
+    L.hrss = o; o += up(sizeof(double) * 2 * (size_t)K);
+    L.hok = o; o += up(2 * (size_t)K);
+    L.hcls = o; o += up(2 * (size_t)K * (size_t)n_hits);
+    L.horig = o; o += up(sizeof(int32_t) * 2 * (size_t)n_hits);
+    L.valid = o; o += up((size_t)K * K);
+    L.cls = o; o += up((size_t)K * K * (size_t)n_hits);
+    L.ncls = o; o += up(sizeof(int32_t) * (size_t)K * K);
+    L.best = o; o += up((size_t)n_hits);
+    L.pick = o; o += 256;                                   // counts [2] then pick [3], read back together
+    L.o_fired = 0;
+    L.o_off = up(sizeof(int32_t) * (size_t)n_fired);
+    L.o_rho = L.o_off + up(sizeof(int32_t) * ((size_t)n_fired + 1));
+    L.o_orig = L.o_rho + up(sizeof(double) * (size_t)n_hits);
+    const size_t list_bytes = L.o_orig + up(sizeof(int32_t) * (size_t)n_hits);
+    L.list[0] = o; o += list_bytes;
+    L.list[1] = o; o += list_bytes;
+    L.total = o;
+    return L;
+}
+
+extern "C" size_t comet_turns_half_work_bytes(int64_t max_seeds_ent, int64_t max_seeds_exit, int32_t n_fired, int32_t n_hits,
+                                              int32_t k_ref, int32_t k_final, const int32_t* n_grid)
+{
+    const size_t hb = comet_half_work_bytes(max_seeds_ent, max_seeds_exit, n_fired, n_hits, k_ref, k_final, n_grid);
+    if (!hb) return 0;
+    return turns_half_layout(hb, n_fired, n_hits, k_final).total;
+}
+
+extern "C" int comet_scan_turns_half(comet_ctx* ctx, const double* seeds_ent, const int64_t* off_ent, int64_t n_ent,
+                                     const double* seeds_exit, const int64_t* off_exit, int64_t n_exit, int32_t n_part,
+                                     int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                                     const double* wire_a, const double* wire_b, int32_t n_wires,
+                                     const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                     int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                     const int32_t* wire_layer, const double* circle, double overlap_cm, int32_t min_layers,
+                                     const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                                     int32_t k_ref, int32_t k_final, int32_t min_wires, int32_t max_tracks, void* work,
+                                     int32_t* turn_pair, int32_t* turn_n, double* turn_seed, uint8_t* turn_cls,
+                                     int32_t* done_host, int32_t* wires_before_host, void* cuda_stream)
+{
+    if (!ctx || n_part < 1 || n_part > COMET_MAX_PARTITIONS || !off_ent || !off_exit || !work || !turn_pair || !turn_n ||
+        !turn_seed || (n_hits > 0 && !turn_cls) || !done_host || !wires_before_host || (n_hits & 1) || n_hits < 0 ||
+        n_fired < 0 || min_wires < 0 || max_tracks < 0 || n_ent < 1 || n_exit < 1)
+        return COMET_EINVAL;
+    PartOff pe, px;
+    if (fill_partoff(&pe, off_ent, n_part, n_ent, true) || fill_partoff(&px, off_exit, n_part, n_exit, true)) return COMET_EINVAL;
+    int64_t max_e = 0, max_x = 0;
+    for (int p = 0; p < n_part; ++p) {
+        if (pe.off[p + 1] - pe.off[p] > max_e) max_e = pe.off[p + 1] - pe.off[p];
+        if (px.off[p + 1] - px.off[p] > max_x) max_x = px.off[p + 1] - px.off[p];
+    }
+    const size_t hb = comet_half_work_bytes(max_e, max_x, n_fired, n_hits, k_ref, k_final, n_grid);
+    if (!hb) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int K = k_final;
+    const TurnsHalfLayout L = turns_half_layout(hb, n_fired, n_hits, K);
+    char* Wk = (char*)work;
+    double* hseed = (double*)(Wk + L.hseed);
+    uint8_t* v_valid = (uint8_t*)(Wk + L.valid);
+    uint8_t* v_cls = (uint8_t*)(Wk + L.cls);
+    int32_t* v_ncls = (int32_t*)(Wk + L.ncls);
+    uint8_t* cls_best = (uint8_t*)(Wk + L.best);
+    int32_t* counts = (int32_t*)(Wk + L.pick);              // counts [0..1], pick [2..4]
+    // nothing done yet: pairs -1, sizes 0, NaN seeds (all-ones is a NaN), empty classification
+    CU(ctx, cudaMemsetAsync(turn_pair, 0xff, sizeof(int32_t) * 2 * (size_t)n_part, st));
+    CU(ctx, cudaMemsetAsync(turn_n, 0, sizeof(int32_t) * (size_t)n_part, st));
+    CU(ctx, cudaMemsetAsync(turn_seed, 0xff, sizeof(double) * 12 * (size_t)n_part, st));
+    if (n_hits) CU(ctx, cudaMemsetAsync(turn_cls, 0, (size_t)n_part * (size_t)n_hits, st));
+    for (int p = 0; p < n_part; ++p) { done_host[p] = 0; wires_before_host[p] = 0; }
+    const int32_t* cur_fw = fired_wire;
+    const int32_t* cur_ho = hit_off;
+    const double* cur_rho = rho;
+    const int32_t* cur_orig = nullptr;                      // identity
+    int32_t cur_w = n_fired, cur_h = n_hits, n_done = 0, flip = 0;
+    for (int p = n_part - 1; p >= 0; --p) {                 // the last turn first
+        if (cur_w < min_wires || n_done >= max_tracks) break;
+        int32_t hc4[4];
+        rc = half_tracks_impl(ctx, seeds_ent + pe.off[p], n_ent, pe.off[p + 1] - pe.off[p],
+                              seeds_exit + px.off[p], n_exit, px.off[p + 1] - px.off[p], charge, bz_tesla, step_cm, n_steps,
+                              r_stop_cm, wire_a, wire_b, n_wires, cur_fw, cur_ho, cur_rho, cur_w, cur_h, cutoff_cm, wire_layer,
+                              circle, overlap_cm, min_layers, half_width, n_grid, n_iter, shrink, k_ref, K, Wk + L.half,
+                              hseed, (double*)(Wk + L.hrss), (uint8_t*)(Wk + L.hok), (uint8_t*)(Wk + L.hcls),
+                              (int32_t*)(Wk + L.horig), hc4, v_valid, v_cls, v_ncls, st);
+        if (rc) return rc;
+        wires_before_host[p] = cur_w;
+        k_best_pair<<<1, 256, 0, st>>>(v_valid, v_ncls, v_cls, K, K, cur_h, hseed, K, cls_best, counts + 2,
+                                       turn_pair + 2 * (size_t)p, turn_n + p, turn_seed + 12 * (size_t)p);
+        if (cur_h) k_scatter_cls<<<(cur_h + 255) / 256, 256, 0, st>>>(cls_best, cur_orig, cur_h, turn_cls + (size_t)p * n_hits);
+        char* Lb = Wk + L.list[flip];
+        int32_t* n_fw = (int32_t*)(Lb + L.o_fired);
+        int32_t* n_ho = (int32_t*)(Lb + L.o_off);
+        double* n_rho = (double*)(Lb + L.o_rho);
+        int32_t* n_orig = (int32_t*)(Lb + L.o_orig);
+        k_remove_hits<<<1, COMET_RM_THREADS, 0, st>>>(cur_fw, cur_ho, cur_rho, cur_w, cls_best, cur_orig, n_fw, n_ho, n_rho,
+                                                      n_orig, counts);
+        CU(ctx, cudaGetLastError());
+        int32_t hc[5];
+        CU(ctx, cudaMemcpyAsync(hc, counts, sizeof(hc), cudaMemcpyDeviceToHost, st));
+        CU(ctx, cudaStreamSynchronize(st));
+        if (hc[2] < 0) break;                               // no valid pair: the reconstruction stops
+        done_host[p] = 1;
+        n_done += 1;
+        cur_fw = n_fw; cur_ho = n_ho; cur_rho = n_rho; cur_orig = n_orig;
+        cur_w = hc[0]; cur_h = hc[1];
+        flip ^= 1;
+    }
     return COMET_OK;
 }
 

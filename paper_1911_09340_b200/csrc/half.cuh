@@ -112,4 +112,41 @@ k_merge_half(const uint8_t* __restrict__ cls_e, const int32_t* __restrict__ orig
     }
 }
 
+// R43.  One CTA: the valid pair with the most classified entries (ties -> the lowest a Kx + b) by a packed-key
+// maximum ((n_cls + 1) in the high word, inverted flat index in the low word; 0 = no valid pair); its complete
+// set goes to cls_best [H] (zeros without a pair), its two seeds, (a, b) and its size to the turn's outputs.
+// pick [3]: a, b (-1 = none), n_cls -- the host reads it with the counters of the next hit list.
+__global__ void __launch_bounds__(256)
+k_best_pair(const uint8_t* __restrict__ valid, const int32_t* __restrict__ n_cls, const uint8_t* __restrict__ cls,
+            int32_t Ke, int32_t Kx, int32_t H, const double* __restrict__ half_seed, int32_t K,
+            uint8_t* __restrict__ cls_best, int32_t* __restrict__ pick, int32_t* __restrict__ turn_pair,
+            int32_t* __restrict__ turn_n, double* __restrict__ turn_seed)
+{
+    __shared__ unsigned long long s_key[8];
+    const int t = threadIdx.x;
+    unsigned long long key = 0;
+    for (int i = t; i < Ke * Kx; i += 256)
+        if (valid[i]) {
+            const unsigned long long kk = ((unsigned long long)(unsigned int)(n_cls[i] + 1) << 32) |
+                                          (unsigned long long)(~(unsigned int)i);
+            key = kk > key ? kk : key;
+        }
+    for (int o = 16; o > 0; o >>= 1) {
+        const unsigned long long other = __shfl_xor_sync(0xffffffffu, key, o);
+        key = other > key ? other : key;
+    }
+    if ((t & 31) == 0) s_key[t >> 5] = key;
+    __syncthreads();
+    key = s_key[0];
+    for (int i = 1; i < 8; ++i) key = s_key[i] > key ? s_key[i] : key;
+    const int flat = key ? (int)(~(unsigned int)(key & 0xffffffffu)) : -1;
+    const int a = flat >= 0 ? flat / Kx : -1, b = flat >= 0 ? flat - a * Kx : -1;
+    for (int j = t; j < H; j += 256) cls_best[j] = flat >= 0 ? cls[(size_t)flat * H + j] : 0;
+    if (t == 0) {
+        pick[0] = a; pick[1] = b; pick[2] = flat >= 0 ? n_cls[flat] : 0;
+        if (flat >= 0) { turn_pair[0] = a; turn_pair[1] = b; turn_n[0] = n_cls[flat]; }
+    }
+    if (flat >= 0 && t < 12) turn_seed[t] = t < 6 ? half_seed[(size_t)a * 6 + t] : half_seed[((size_t)K + b) * 6 + (t - 6)];
+}
+
 }  // namespace comet

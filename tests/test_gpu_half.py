@@ -232,3 +232,47 @@ def test_half_track_argument_errors(comet, cfg0_event):
     with pytest.raises(CometError):                                  # half lists longer than the event
         comet.merge_half_sets(_dev(np.zeros((1, 8), np.uint8)), _dev(np.arange(8, dtype=np.int32)), _dev(np.ones(1, np.uint8)),
                               _dev(np.zeros((1, 2), np.uint8)), _dev(np.arange(2, dtype=np.int32)), _dev(np.ones(1, np.uint8)), 4)
+
+
+def _turn_seed_sets(ev, shape_e=(5, 5, 5, 4), shape_x=(5, 5, 4, 5)):
+    pr = tuple(ev.spec["p_range"])
+    se = [seed_grid(ev, p, shape_e, pr, ct_hw=0.15) for p in range(len(ev.partitions))]
+    sx = [_exit_grid(ev, p, shape_x, pr) for p in range(len(ev.partitions))]
+    off = lambda blocks: np.concatenate([[0], np.cumsum([b.shape[1] for b in blocks])]).astype(np.int64)
+    return (np.ascontiguousarray(np.concatenate(se, axis=1)), off(se),
+            np.ascontiguousarray(np.concatenate(sx, axis=1)), off(sx))
+
+
+def _compare_turns_half(got, ref):
+    assert got["done"].tolist() == ref["done"].tolist()
+    assert got["wires_before"].tolist() == ref["wires_before"].tolist()
+    assert np.array_equal(got["turn_pair"].cpu().numpy(), ref["turn_pair"])
+    assert np.array_equal(got["turn_n"].cpu().numpy(), ref["turn_n"])
+    assert np.array_equal(got["turn_cls"].cpu().numpy(), ref["turn_cls"])
+    assert _same_f64(got["turn_seed"].cpu().numpy(), ref["turn_seed"])
+
+
+@pytest.mark.parametrize("cfg", [1, 4])
+def test_event_loop_with_half_tracks_identical(comet, cfg):
+    """Fig. 13 with half tracks: three turns, last first, the chosen complete set's hits removed in between; pairs,
+    sets, seeds, wire counts and stopping decisions identical to the oracle (configs[4]: 1000 noise wires)."""
+    ev = make_config(cfg)[0]
+    circ = _circle(ev)
+    se, oe, sx, ox = _turn_seed_sets(ev)
+    phys = (ev.charge, ev.bz, ev.step, ev.n_steps, R_HALF)
+    kw = dict(half_width=[1.0, 1.2, 1.2, 1.5], n_grid=[3, 3, 3, 3], n_iter=2, shrink=0.5, k_ref=3, k_final=3)
+    dargs = (_dev(ev.geom.wire_a), _dev(ev.geom.wire_b), _dev(ev.fired_wire), _dev(ev.hit_off), _dev(ev.rho), ev.cutoff,
+             _dev(ev.geom.layer), _dev(circ))
+    hargs = (ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, ev.geom.layer, circ)
+    for extra in (dict(min_wires=10), dict(min_wires=10, max_tracks=2), dict(min_wires=ev.n_fired + 1)):
+        ref = O.scan_turns_half(se, oe, sx, ox, *phys, *hargs, 3.0, 3, **kw, **extra)
+        got = comet.scan_turns_half(_dev(se), oe, _dev(sx), ox, *phys, *dargs, 3.0, 3, **kw, **extra)
+        torch.cuda.synchronize()
+        _compare_turns_half(got, ref)
+    assert ref["done"].sum() == 0
+    # a veto nothing passes: the first turn has no valid pair and the loop stops there
+    ref = O.scan_turns_half(se, oe, sx, ox, *phys, *hargs, 3.0, 21, min_wires=10, **kw)
+    got = comet.scan_turns_half(_dev(se), oe, _dev(sx), ox, *phys, *dargs, 3.0, 21, min_wires=10, **kw)
+    torch.cuda.synchronize()
+    _compare_turns_half(got, ref)
+    assert not ref["done"].any() and ref["wires_before"][-1] == ev.n_fired
