@@ -32,7 +32,8 @@ COARSE_PRUNED = 1
 OPT_STATS = 2
 OPT_TIMING = 3
 OPT_LANES = 4
-STATS_FIELDS = ("samples", "rows_needed", "rows_executed", "fine_needed", "fine_executed", "pairs")
+OPT_ZGROUP = 5
+STATS_FIELDS = ("samples", "rows_needed", "rows_executed", "fine_needed", "fine_executed", "pairs", "unique_states")
 
 
 class CometError(RuntimeError):

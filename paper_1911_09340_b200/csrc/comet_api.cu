@@ -14,6 +14,7 @@
 #include "extrapolate.cuh"
 #include "select.cuh"
 #include "scan_fused.cuh"
+#include "scan_zgroup.cuh"
 #include "refine.cuh"
 #include "turns.cuh"
 #include "hough.cuh"
@@ -49,6 +50,13 @@ struct comet_ctx {
     // comet_scan_rss runs the sub-slabs of a slab concurrently: scan kernels on ls[], the fine stage on
     // the high-priority lf[] so that its CTAs take the slots retiring scan CTAs free
     int opt_lanes;
+    int opt_zgroup;              // 1 (default): seeds in z-runs go through k_scan_zg
+    unsigned int* zg_flag;       // [COMET_MAX_LANES] run length found by k_zgroup_check
+    int zg_smem;                 // dynamic shared memory of k_scan_fused<.., ZG>
+    double* ub;                  // distinct transverse tracks of a slab (k_gen_unique)
+    size_t ub_bytes;
+    int32_t* npu;
+    size_t npu_bytes;
     cudaStream_t ls[COMET_MAX_LANES], lf[COMET_MAX_LANES];
     cudaEvent_t ev_fork, ev_scan[COMET_MAX_LANES], ev_join[COMET_MAX_LANES];
     int fine_blocks;             // persistent grid of k_fine
@@ -139,6 +147,16 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaMalloc(&ctx->bmax, sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int) * COMET_MAX_LANES);
     ctx->opt_lanes = COMET_DEFAULT_LANES;
+    ctx->opt_zgroup = 1;
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->zg_flag, sizeof(unsigned int) * COMET_MAX_LANES);
+    {
+        ctx->zg_smem = ((COMET_FUSED_WFIELDS + 1) * COMET_FUSED_WCAP + COMET_FUSED_WARPS * COMET_ZG_WTILE) * (int)sizeof(double);
+        const void* zk[2] = {(const void*)k_scan_fused<false, false, true>, (const void*)k_scan_fused<true, false, true>};
+        for (int j = 0; j < 2 && e == cudaSuccess; ++j) {
+            e = cudaFuncSetAttribute(zk[j], cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->zg_smem);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(zk[j], cudaFuncAttributePreferredSharedMemoryCarveout, 100);
+        }
+    }
     {
         int prio_lo = 0, prio_hi = 0;
         if (e == cudaSuccess) e = cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
@@ -194,7 +212,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     if (!ctx) return COMET_EINVAL;
     cudaSetDevice(ctx->device);
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
-    cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items);
+    cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ub); cudaFree(ctx->npu);
     for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->bmax);
     for (int l = 0; l < COMET_MAX_LANES; ++l) {
@@ -219,6 +237,10 @@ extern "C" int comet_set_option(comet_ctx* ctx, int option, int value)
         ctx->opt_stats = value;
         return COMET_OK;
     }
+    if (option == COMET_OPT_ZGROUP && (value == 0 || value == 1)) {
+        ctx->opt_zgroup = value;
+        return COMET_OK;
+    }
     if (option == COMET_OPT_LANES && value >= 1 && value <= COMET_MAX_LANES) {
         ctx->opt_lanes = value;
         return COMET_OK;
@@ -237,6 +259,7 @@ extern "C" int comet_get_option(const comet_ctx* ctx, int option, int* value)
     if (option == COMET_OPT_COARSE_SEARCH) { *value = ctx->opt_coarse; return COMET_OK; }
     if (option == COMET_OPT_STATS) { *value = ctx->opt_stats; return COMET_OK; }
     if (option == COMET_OPT_LANES) { *value = ctx->opt_lanes; return COMET_OK; }
+    if (option == COMET_OPT_ZGROUP) { *value = ctx->opt_zgroup; return COMET_OK; }
     if (option == COMET_OPT_TIMING) { *value = ctx->opt_timing; return COMET_OK; }
     return COMET_EINVAL;
 }
@@ -615,6 +638,17 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
     if (rc) return rc;
     rc = grow_dev(ctx, (void**)&ctx->cw, &ctx->cw_bytes, (size_t)slab_chunks * COMET_LANES * sizeof(double));
     if (rc) return rc;
+    const bool zgroup = !field && ctx->opt_zgroup != 0;
+    // distinct transverse tracks (scan_zgroup.cuh): at most 4 per chunk (runs of >= 8 seeds), blocks of 32 tracks of
+    // n_steps + 1 rows of 4 doubles; every sub-slab starts on a block of its own
+    const size_t ub_block = (size_t)(n_steps + 1) * 128 * sizeof(double);
+    if (zgroup) {
+        const size_t blocks = (size_t)slab_chunks / 8 + 2 * COMET_MAX_LANES + 2;
+        rc = grow_dev(ctx, (void**)&ctx->ub, &ctx->ub_bytes, blocks * ub_block);
+        if (rc) return rc;
+        rc = grow_dev(ctx, (void**)&ctx->npu, &ctx->npu_bytes, blocks * 32 * sizeof(int32_t));
+        if (rc) return rc;
+    }
     if (!n_pts) {
         size_t have = ctx->npw_cap * sizeof(int32_t);
         rc = grow_dev(ctx, (void**)&ctx->npw, &have, (size_t)slab_chunks * COMET_LANES * sizeof(int32_t));
@@ -684,6 +718,29 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
             if (tm) CU(ctx, cudaEventRecord(tev[0], st));
             const int thr = 32 * COMET_FUSED_WARPS;
+            a.zg = nullptr;
+            a.ub = nullptr;
+            a.np_u = nullptr;
+            a.u_rows = n_steps + 1;
+            if (zgroup) {
+                // seeds in runs that differ only in z: every distinct transverse track is stepped once (k_gen_unique),
+                // k_scan_fused<.., ZG> copies its tile rows from there; the run length is found on the device and the
+                // kernels that are not needed exit at once
+                const size_t blk0 = (size_t)cl / 8 + 2 * (size_t)l;
+                a.zg = ctx->zg_flag + l;
+                a.ub = ctx->ub + blk0 * (ub_block / sizeof(double));
+                a.np_u = ctx->npu + blk0 * 32;
+                CU(ctx, cudaMemsetAsync(ctx->zg_flag + l, 0xff, sizeof(unsigned int), s_scan));
+                k_zgroup_check<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_scan>>>(a.seeds, a.stride, a.n_seeds, ctx->zg_flag + l);
+                const unsigned bu = (unsigned)((a.n_seeds / COMET_ZG_MIN + 1 + 31) / 32);      // one warp per CTA: a latency-bound chain
+                if (a.stats) {
+                    k_gen_unique<true><<<bu, 32, 0, s_scan>>>(a);
+                    k_scan_fused<true, false, true><<<b1, thr, ctx->zg_smem, s_scan>>>(a);
+                } else {
+                    k_gen_unique<false><<<bu, 32, 0, s_scan>>>(a);
+                    k_scan_fused<false, false, true><<<b1, thr, ctx->zg_smem, s_scan>>>(a);
+                }
+            }
             if (field) {
                 if (a.stats) k_scan_fused<true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
                 else k_scan_fused<false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);

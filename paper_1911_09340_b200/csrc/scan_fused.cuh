@@ -53,6 +53,12 @@ namespace comet {
 #ifndef COMET_FUSED_WCAP
 #define COMET_FUSED_WCAP 96        // wires whose constants the shared-memory table holds (the others: L1/L2)
 #endif
+#ifndef COMET_FUSED_MINB_ZG
+#define COMET_FUSED_MINB_ZG 5      // the ZG variant keeps no track state and a smaller tile: one more CTA per SM
+#endif
+#define COMET_ZG_RING 4            // compact tiles fetched ahead (scan_zgroup.cuh)
+#define COMET_ZG_SLOT 160          // doubles per compact tile: [20][2][4 distinct tracks]
+#define COMET_ZG_WTILE (COMET_FUSED_TR * 32 + COMET_ZG_RING * COMET_ZG_SLOT)   // doubles per warp in the ZG variant
 #define COMET_FUSED_WFIELDS 9      // e1[3] -m.e1 | e2[3] -m.e2 | far radius  (fields 6..14 of the wire table)
 // the CTA's table has one more row: sqrt(1 - w_z^2) rounded up, the wire's slope against the z axis
 
@@ -94,7 +100,17 @@ struct FusedArgs {
     unsigned long long* stats;
     FieldMap F;              // field-map variants (FIELD = true): the map, and qkb = kappa q, hk.h = h_max
     double h_min;            // h_max / 64 (R31)
+    const unsigned int* zg;  // scan_zgroup.cuh: run length of the launch's seeds (device); nullptr = not checked
+    double* ub;              // scan_zgroup.cuh: (x_0, x_1, T_0, T_1) of the distinct transverse tracks [u / 32][u_rows][4][32]
+    int32_t* np_u;           //   and their numbers of recorded states
+    int32_t u_rows;          //   rows per track in ub: n_steps + 1
 };
+#define COMET_ZG_MIN 8             // smallest run length served by the ZG kernels (scan_zgroup.cuh)
+__device__ __forceinline__ unsigned int zgroup_of(const unsigned int* flag)
+{
+    const unsigned int f = *flag;
+    return f > 32u ? 32u : f;
+}
 #define COMET_CK_FIELDS(FIELD) ((FIELD) ? 7 : 6)    // checkpoint row: x, T and, in a field map, the trial step
 #ifndef COMET_FUSED_CK_FIELD
 #define COMET_FUSED_CK_FIELD 4     // rows between checkpoints in a field map (1 and 2 were measured: the extra checkpoint traffic costs what the shorter replay saves)
@@ -121,9 +137,12 @@ __device__ __forceinline__ double wire_slope(double e1z, double e2z)
     return (double)__fsqrt_ru(__double2float_ru(fma(e1z, e1z, e2z * e2z)));
 }
 
-template <bool STATS, bool FIELD>
-__global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
+// ZG = true: the rows of a tile are not generated here: (x, y) come from the distinct transverse tracks of
+// k_gen_unique and z is accumulated per seed (scan_zgroup.cuh); everything after the tile is the same code.
+template <bool STATS, bool FIELD, bool ZG = false>
+__global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_ZG : COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
 {
+    static_assert(!(FIELD && ZG), "the transverse motion depends on z in a field map");
     constexpr int CKF = COMET_CK_FIELDS(FIELD);
     constexpr int TR = COMET_FUSED_TR, CK = COMET_CK_ROWS(FIELD), ROW = 3 * COMET_LANES;
     constexpr int FM1 = COMET_FUSED_M1;
@@ -131,10 +150,15 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
     constexpr int WCAP = COMET_FUSED_WCAP;
     constexpr unsigned FULL = 0xffffffffu;
     static_assert(TR % FM1 == 0 && TR % CK == 0, "tile rows");
+    if (ZG) {
+        if (zgroup_of(a.zg) < COMET_ZG_MIN) return;         // the plain kernel serves this launch
+    } else if (!FIELD && a.zg && zgroup_of(a.zg) >= COMET_ZG_MIN) {
+        return;                                             // the ZG kernels serve this launch (scan_zgroup.cuh)
+    }
     extern __shared__ __align__(16) double fsm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* wtab = fsm;                                     // [WFIELDS + 1][WCAP]
-    double* tile = fsm + (COMET_FUSED_WFIELDS + 1) * WCAP + warp * (TR * ROW);
+    double* tile = fsm + (COMET_FUSED_WFIELDS + 1) * WCAP + warp * (ZG ? COMET_ZG_WTILE : TR * ROW);
     const int W = a.W;
     for (int v = threadIdx.x; v < COMET_FUSED_WFIELDS * WCAP; v += 32 * COMET_FUSED_WARPS) {
         const int f = v / WCAP, i = v - f * WCAP;
@@ -165,10 +189,55 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
     const bool lip_ok = (FIELD ? fabs(c) * __ldg(a.F.bmax) * h : fabs(c) * h) <= COMET_CH_MAX;
     const unsigned nolip_mask = __ballot_sync(FULL, valid && !lip_ok);
     double htry = h;                                        // FIELD: trial step of the adaptive control (R31)
-    bool active = valid;
+    bool active = valid && !ZG;
     int32_t np = valid ? a.n_steps + 1 : 0;
     const bool use_stop = a.r_stop2 > 0.0;
-
+    // ZG: the chunk's NU = 32 / ZG distinct transverse tracks, the seed's (final) number of recorded states and
+    // the z advance of a step.  The warp's shared memory holds the z column of the tile [TR][32] and a ring of
+    // ZRING compact tiles [20][2][NU]: (x, y) of the 16 rows and (T_0, T_1) of the 4 checkpoint rows of every
+    // distinct track, fetched ZRING - 1 tiles ahead with cp.async from k_gen_unique's buffer.
+    constexpr int ZRING = COMET_ZG_RING, ZSLOT = COMET_ZG_SLOT;
+    const int n_tiles_zg = (a.n_steps + TR) / TR;
+    static_assert(TR == 16 && CK == 4 || !ZG, "compact tile layout");
+    double hz = 0.0;
+    int zshift = 5, nshift = 0, ul = 0;
+    int64_t ug0 = 0;
+    double* const zt = tile;                                // ZG: z column
+    double* const xr = tile + TR * 32;                      // ZG: ring of compact tiles
+    if (ZG) {
+        zshift = 31 - __clz((int)zgroup_of(a.zg));
+        nshift = 5 - zshift;
+        ul = lane >> zshift;                                // the seed's distinct track within the chunk
+        ug0 = (chunk * COMET_LANES) >> zshift;              // the chunk's first distinct track
+        if (valid) {
+            np = a.np_u[ug0 + ul];
+            hz = xmul(h, st.t2);                            // x_2' = x_2 + h T_2, T_2 constant
+        }
+    }
+    // ZG: fetch the compact tile t (one cp.async group per call, possibly empty)
+    auto fetch_tile = [&](int t) {
+        const int r0f = t * TR;
+        const int n_el = 40 << nshift;
+        for (int e0 = 0; e0 < n_el; e0 += 32) {
+            const int e = e0 + lane;
+            const int eu = e & ((1 << nshift) - 1);         // distinct track
+            const int sc = e >> nshift, slot = sc >> 1, comp = sc & 1;
+            const int32_t np_e = __shfl_sync(FULL, np, eu << zshift);
+            if (e < n_el && t < n_tiles_zg) {
+                const int k = slot < 16 ? r0f + slot : r0f + (slot - 16) * CK;
+                double* dst = xr + (t % ZRING) * ZSLOT + e;
+                if (np_e > 0) {                             // rows past n_pts - 1 repeat the last state
+                    const int64_t ug = ug0 + eu;
+                    const double* src = a.ub + ((size_t)(ug >> 5) * (size_t)a.u_rows + (size_t)min(k, np_e - 1)) * 128 +
+                                        (slot < 16 ? comp : 2 + comp) * 32 + (ug & 31);
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src));
+                } else {
+                    *dst = 0.0;
+                }
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
     // pair workspace of this chunk: nothing found yet
     unsigned long long* const keys = reinterpret_cast<unsigned long long*>(a.bd);
     for (int i = 0; i < W; ++i) keys[(size_t)i * a.SP + s] = COMET_KEY_NONE;
@@ -193,9 +262,34 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
     for (int t = 0; t < n_tiles; ++t) {
         const int r0 = t * TR;
         PC_MARK();
+        const double* xc = xr + (t % ZRING) * ZSLOT + ul;     // ZG: compact tile t, this seed's distinct track
+        if (ZG) {
+            if (!__any_sync(FULL, np > r0)) break;
+            if (t == 0)
+                for (int q = 0; q < ZRING - 1; ++q) fetch_tile(q);
+            fetch_tile(t + ZRING - 1);
+            // ---- rows r0 .. r0 + TR - 1: the seed's own z column; (x, y) wait in the ring -------------------
+#pragma unroll
+            for (int rr = 0; rr < TR; ++rr) {
+                const int k = r0 + rr;
+                if (k > 0 && k < np) st.x2 = xadd(st.x2, hz);
+                zt[rr * 32 + lane] = st.x2;
+            }
+            asm volatile("cp.async.wait_group %0;" ::"n"(ZRING - 1) : "memory");
+            __syncwarp();
+#pragma unroll
+            for (int rr = 0; rr < TR; rr += CK) {
+                const int k = r0 + rr;
+                if (k < np) {                               // k_fine_ck starts from checkpoints at or before n_pts - 1 only
+                    double* o = ckc + (size_t)(k / CK) * (CKF * COMET_LANES);
+                    o[0] = xc[(rr * 2) << nshift]; o[32] = xc[(rr * 2 + 1) << nshift]; o[64] = zt[rr * 32 + lane];
+                    o[96] = xc[((16 + rr / CK) * 2) << nshift]; o[128] = xc[((16 + rr / CK) * 2 + 1) << nshift]; o[160] = st.t2;
+                }
+            }
+        }
         // ---- generate rows r0 .. r0 + TR - 1 (Algorithm 1; finished lanes hold their last state) ------
 #pragma unroll 2
-        for (int rr = 0; rr < TR; ++rr) {
+        for (int rr = 0; !ZG && rr < TR; ++rr) {
             const int k = r0 + rr;
             if (k > 0 && active) {
                 if (FIELD) (void)adaptive_field_step(st, htry, h, a.h_min, c, a.F);
@@ -228,8 +322,10 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
         float rxy[NSUB], rz[NSUB];
 #pragma unroll
         for (int j = 0; j < NSUB; ++j) {
-            const double* ps = tile + (j * FM1 + FM1 / 2) * ROW + lane;
-            const double s0 = ps[0], s1 = ps[32], s2 = ps[64];
+            const int srow = j * FM1 + FM1 / 2;
+            const double* ps = tile + srow * ROW + lane;
+            const double s0 = ZG ? xc[(srow * 2) << nshift] : ps[0], s1 = ZG ? xc[(srow * 2 + 1) << nshift] : ps[32];
+            const double s2 = ZG ? zt[srow * 32 + lane] : ps[64];
             rx[j][0] = __shfl_sync(FULL, s0, rep); rx[j][1] = __shfl_sync(FULL, s1, rep); rx[j][2] = __shfl_sync(FULL, s2, rep);
             const double e0 = s0 - rx[j][0], e1 = s1 - rx[j][1], e2 = s2 - rx[j][2];
             const float fxy = is_live ? __fsqrt_ru(__double2float_ru(fma(e0, e0, e1 * e1))) : 0.f;
@@ -283,7 +379,9 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
                     if (STATS) { st_cnt[ST_ROWS_EXEC] += FM1; if (is_live) st_cnt[ST_ROWS_NEEDED] += FM1; }
 #pragma unroll
                     for (int kk = 0; kk < FM1; ++kk) {
-                        const double d2 = d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
+                        const int row = j * FM1 + kk;
+                        const double d2 = ZG ? d2_fma(w, xc[(row * 2) << nshift], xc[(row * 2 + 1) << nshift], zt[row * 32 + lane])
+                                             : d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
                         const int k = r0 + j * FM1 + kk;
                         // rows at or past n_pts repeat the last state: not recorded, never taken
                         if (d2 < best && k < np) { best = d2; bk = k; }
@@ -294,7 +392,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
             PC_ADD(pc_l1);
         }
         __syncwarp();
-        if (!__any_sync(FULL, active)) break;
+        if (!ZG && !__any_sync(FULL, active)) break;
     }
 #ifdef COMET_FUSED_PROF
     if (lane == 0 && a.stats) {
@@ -304,6 +402,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
     }
     PC_MARK();
 #endif
+    if (ZG) { asm volatile("cp.async.wait_all;" ::: "memory"); __syncwarp(); }
     if (valid) { a.n_pts[s] = np; a.cw[s] = c; }
     // ---- finish: far pairs take the cutoff, (chunk, wire) items with a near lane go to k_fine_ck -------
     // Keys come from L2: FB wires in flight at a time.  The items are collected in the (now free) tile
