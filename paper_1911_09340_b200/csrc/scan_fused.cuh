@@ -225,7 +225,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
             const int32_t np_e = __shfl_sync(FULL, np, eu << zshift);
             if (e < n_el && t < n_tiles_zg) {
                 const int k = slot < 16 ? r0f + slot : r0f + (slot - 16) * CK;
-                double* dst = xr + (t % ZRING) * ZSLOT + e;
+                double* dst = xr + (t % ZRING) * ZSLOT + sc * 4 + eu;   // [slot][comp][4]: constant strides for the readers
                 if (np_e > 0) {                             // rows past n_pts - 1 repeat the last state
                     const int64_t ug = ug0 + eu;
                     const double* src = a.ub + ((size_t)(ug >> 5) * (size_t)a.u_rows + (size_t)min(k, np_e - 1)) * 128 +
@@ -282,8 +282,8 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
                 const int k = r0 + rr;
                 if (k < np) {                               // k_fine_ck starts from checkpoints at or before n_pts - 1 only
                     double* o = ckc + (size_t)(k / CK) * (CKF * COMET_LANES);
-                    o[0] = xc[(rr * 2) << nshift]; o[32] = xc[(rr * 2 + 1) << nshift]; o[64] = zt[rr * 32 + lane];
-                    o[96] = xc[((16 + rr / CK) * 2) << nshift]; o[128] = xc[((16 + rr / CK) * 2 + 1) << nshift]; o[160] = st.t2;
+                    o[0] = xc[(rr * 2) * 4]; o[32] = xc[(rr * 2 + 1) * 4]; o[64] = zt[rr * 32 + lane];
+                    o[96] = xc[((16 + rr / CK) * 2) * 4]; o[128] = xc[((16 + rr / CK) * 2 + 1) * 4]; o[160] = st.t2;
                 }
             }
         }
@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
         for (int j = 0; j < NSUB; ++j) {
             const int srow = j * FM1 + FM1 / 2;
             const double* ps = tile + srow * ROW + lane;
-            const double s0 = ZG ? xc[(srow * 2) << nshift] : ps[0], s1 = ZG ? xc[(srow * 2 + 1) << nshift] : ps[32];
+            const double s0 = ZG ? xc[(srow * 2) * 4] : ps[0], s1 = ZG ? xc[(srow * 2 + 1) * 4] : ps[32];
             const double s2 = ZG ? zt[srow * 32 + lane] : ps[64];
             rx[j][0] = __shfl_sync(FULL, s0, rep); rx[j][1] = __shfl_sync(FULL, s1, rep); rx[j][2] = __shfl_sync(FULL, s2, rep);
             const double e0 = s0 - rx[j][0], e1 = s1 - rx[j][1], e2 = s2 - rx[j][2];
@@ -380,7 +380,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
 #pragma unroll
                     for (int kk = 0; kk < FM1; ++kk) {
                         const int row = j * FM1 + kk;
-                        const double d2 = ZG ? d2_fma(w, xc[(row * 2) << nshift], xc[(row * 2 + 1) << nshift], zt[row * 32 + lane])
+                        const double d2 = ZG ? d2_fma(w, xc[(row * 2) * 4], xc[(row * 2 + 1) * 4], zt[row * 32 + lane])
                                              : d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
                         const int k = r0 + j * FM1 + kk;
                         // rows at or past n_pts repeat the last state: not recorded, never taken
