@@ -195,7 +195,7 @@ def run_ours(args):
     import torch
     import torch.distributed as dist
     from paper_1911_09340_b200 import Comet
-    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH, OPT_LANES, OPT_STATS, OPT_TIMING
+    from paper_1911_09340_b200.binding import COARSE_EXHAUSTIVE, COARSE_PRUNED, OPT_COARSE_SEARCH, OPT_LANES, OPT_STATS, OPT_TIMING, OPT_ZGROUP
     from paper_1911_09340_b200.build import build
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -212,6 +212,7 @@ def run_ours(args):
     S, W, H, P = seeds.shape[1], ev.n_fired, ev.n_hits, len(part_off) - 1
     fused = args.path == "fused"
     c = Comet(local)
+    c.set_option(OPT_ZGROUP, 1 if args.zgroup else 0)
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     d_seeds, d_wa, d_wb = dev(seeds), dev(ev.geom.wire_a), dev(ev.geom.wire_b)
     d_fw, d_ho, d_rho = dev(ev.fired_wire), dev(ev.hit_off), dev(ev.rho)
@@ -384,10 +385,11 @@ def run_ours(args):
         sx_h[3], sx_h[4] = px * np.cos(rot) - py * np.sin(rot), px * np.sin(rot) + py * np.cos(rot)
         sx = dev(sx_h)
         hkw = dict(half_width=STAGE_HALF_WIDTH, n_grid=STAGE_GRID, n_iter=3, shrink=0.5, k_ref=10, k_final=10)
-        hfn = lambda: c.scan_half_tracks(se, sx, *phys, 1.0e3, *hits, ev.cutoff, dev(ev.geom.layer), ho1["circle"][0].contiguous(),
-                                         3.0, 3, **hkw)
+        d_layer, d_circ = dev(ev.geom.layer), ho1["circle"][0].contiguous()
+        hfn = lambda: c.scan_half_tracks(se, sx, *phys, 1.0e3, *hits, ev.cutoff, d_layer, d_circ, 3.0, 3, **hkw)
         hfn()
-        ms_half, hout_ = _time_steps(hfn, max(2, n_cmp // 2), stream)
+        hfn()
+        ms_half, hout_ = _time_steps(hfn, 10, stream)
         seeding = {"hough": {"ms_per_launch": ms_h, "events": len(lists), "fired_wires": int(ev_off[-1]),
                              "ms_per_graph_replay": ms_hg, "votes_per_s": votes / (ms_hg * 1e-3),
                              "events_per_s": len(lists) / (ms_hg * 1e-3),
@@ -409,6 +411,8 @@ def run_ours(args):
         bevs = make_config(2, n_events=args.batch)
         n_str = 2
         bctx = [Comet(local) for _ in range(n_str)]
+        for q in bctx:
+            q.set_option(OPT_ZGROUP, 1 if args.zgroup else 0)
         bstr = [torch.cuda.Stream() for _ in range(n_str)]
         items = []
         for bev in bevs:
@@ -428,8 +432,9 @@ def run_ours(args):
                 stream.wait_stream(q)
             return res
         run_batch()
+        run_batch()
         torch.cuda.synchronize()
-        ms_batch, _ = _time_steps(run_batch, 3, stream)
+        ms_batch, _ = _time_steps(run_batch, 6, stream)
         b_parts = sum(len(it[2]) - 1 for it in items)
         b_pairs = sum(float(it[1].shape[1]) * it[0].n_fired for it in items)
         batch = {"events": len(items), "partitions": b_parts, "ms_per_batch": ms_batch,
@@ -487,8 +492,11 @@ def run_ours(args):
     ev_needed = stats["samples"] + stats["rows_needed"]
     ev_exec = stats["samples"] + stats["rows_executed"]
     gen = GEN_INSTR * n_states if fused else 0.0
+    # z-runs (scan_zgroup.cuh): the RKN4 step is executed once per distinct transverse track and every seed adds its z
+    uniq = float(stats.get("unique_states", 0))
+    gen_exec = (GEN_INSTR * uniq + n_states) if (fused and uniq > 0) else gen
     fl = {knames[0]: 2.0 * (gen + SHORTLIST_INSTR * ev_needed), knames[1]: 2.0 * FINE_INSTR * stats["fine_needed"]}
-    fl_exec = {knames[0]: 2.0 * (gen + SHORTLIST_INSTR * ev_exec), knames[1]: 2.0 * FINE_INSTR * stats["fine_executed"]}
+    fl_exec = {knames[0]: 2.0 * (gen_exec + SHORTLIST_INSTR * ev_exec), knames[1]: 2.0 * FINE_INSTR * stats["fine_executed"]}
     kernels = {"timed_over": "%d steps after the timed region with COMET_OPT_TIMING (CUDA events recorded by the library "
                              "on its stream; kernels run one after the other)" % ktimes["n_calls"]}
     kernels.update({k: {"ms_per_launch": ktimes[k], "achieved": fl[k] / (ktimes[k] * 1e-3) / 1e12,
@@ -504,6 +512,7 @@ def run_ours(args):
         lanes = c.get_option(OPT_LANES)
         top = {"kernel": "k_scan_fused + k_fine_ck (comet_scan_rss: sub-slabs on %d internal streams)" % lanes,
                "achieved": (fl[knames[0]] + fl[knames[1]]) / (ms_call * 1e-3) / 1e12, "ms_per_launch": ms_call,
+               "achieved_executed": (fl_exec[knames[0]] + fl_exec[knames[1]]) / (ms_call * 1e-3) / 1e12,
                "timed": "CUDA events on the caller's stream around every comet_scan_rss of the timed region",
                "traffic": (TRAFFIC_BYTES["k_scan_fused"] + TRAFFIC_BYTES["k_fine_ck"]) if args.config == 1 else None}
     else:
@@ -512,7 +521,10 @@ def run_ours(args):
     model = ("FP64-pipe slots x 2 of the work the path needs (thread-level counters, comet_read_stats): "
              + ("%d per recorded state (RKN4 step + target-region test, Alg. 1), " % GEN_INSTR if fused else "")
              + "%d per shortlist evaluation (sub-block sample or swept row); %s: %d per (seed, wire) pair that runs "
-               "the virtual-plane iteration" % (SHORTLIST_INSTR, knames[1], FINE_INSTR))
+               "the virtual-plane iteration" % (SHORTLIST_INSTR, knames[1], FINE_INSTR)
+             + ("; `achieved` counts the RKN4 step once per (seed, recorded state) -- SURVEY 8(d)'s unit -- although with "
+                "COMET_OPT_ZGROUP the library executes it once per distinct transverse track (%.0f of %.0f states) plus one "
+                "z addition per (seed, state): `achieved_executed` counts what is executed" % (uniq, n_states) if uniq > 0 else ""))
     flops_exh = 2.0 * (SHORTLIST_INSTR * n_states * W + FINE_INSTR * pairs)
     if fused:
         # k_wire_prep, then k_scan_fused + k_fine_ck + k_rss_sum per sub-slab (the library's rule: up to
@@ -521,7 +533,7 @@ def run_ours(args):
         n_sm = torch.cuda.get_device_properties(local).multi_processor_count
         while n_sub > 1 and chunks // n_sub < 4 * n_sm * 2:
             n_sub -= 1
-        launches_per_step = 1 + 3 * n_sub + 3
+        launches_per_step = 1 + (6 if uniq > 0 or c.get_option(OPT_ZGROUP) else 3) * n_sub + 3   # ZGROUP: + k_zgroup_check, k_gen_unique, k_scan_fused<ZG>
     else:
         launches_per_step = 8
     line = {
@@ -553,6 +565,8 @@ def run_ours(args):
                      "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no FP64 figure)",
                      "peak_measured_dfma_probe": peak_measured,
                      "frac_of_measured": top["achieved"] / peak_measured,
+                     "achieved_executed": top.get("achieved_executed"),
+                     "frac_executed": (top["achieved_executed"] / peak) if top.get("achieved_executed") else None,
                      "ms_per_launch": top["ms_per_launch"], "share_of_step": top["ms_per_launch"] / ms_per_step,
                      "model": model, "kernels": kernels, "work_counters": stats,
                      "other_path": {"path": "materialised" if fused else "fused", "ms_per_step": ms_other,
@@ -583,6 +597,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     ap.add_argument("--no-field", dest="field", action="store_false", help="skip the field-map leg")
     ap.add_argument("--batch", type=int, default=16, help="events of configs[2] in the batch leg (0 = skip)")
+    ap.add_argument("--no-zgroup", dest="zgroup", action="store_false",
+                    help="COMET_OPT_ZGROUP = 0: every seed runs its own RKN4 steps even where runs of seeds differ only in z")
     ap.add_argument("--no-seeding", dest="seeding", action="store_false", help="skip the Hough / half-track legs")
     args = ap.parse_args()
     if args.impl == "reference":

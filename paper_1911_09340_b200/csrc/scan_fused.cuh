@@ -54,7 +54,7 @@ namespace comet {
 #define COMET_FUSED_WCAP 96        // wires whose constants the shared-memory table holds (the others: L1/L2)
 #endif
 #ifndef COMET_FUSED_MINB_ZG
-#define COMET_FUSED_MINB_ZG 5      // the ZG variant keeps no track state and a smaller tile: one more CTA per SM
+#define COMET_FUSED_MINB_ZG 4      // (5 CTAs per SM fit the smaller tile of the ZG variant but 96 registers cost more than they gain)
 #endif
 #define COMET_ZG_RING 4            // compact tiles fetched ahead (scan_zgroup.cuh)
 #define COMET_ZG_SLOT 160          // doubles per compact tile: [20][2][4 distinct tracks]
@@ -214,25 +214,29 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
             hz = xmul(h, st.t2);                            // x_2' = x_2 + h T_2, T_2 constant
         }
     }
-    // ZG: fetch the compact tile t (one cp.async group per call, possibly empty)
+    // ZG: fetch the compact tile t (one cp.async group per call, possibly empty).  A lane always serves the same
+    // (component, distinct track) and walks the 20 row slots in steps of 32 / (2 NU), so everything but the row is
+    // fixed per lane: lane = (slot_low, comp, track).
+    const int f_eu = lane & ((1 << nshift) - 1), f_comp = (lane >> nshift) & 1, f_slot0 = lane >> (1 + nshift);
+    const int f_spi = 32 >> (1 + nshift);                   // slots per pass: 16, 8, 4
+    const int32_t f_np = ZG ? __shfl_sync(FULL, np, f_eu << zshift) : 0;
+    const double* f_src = nullptr;
+    if (ZG && f_np > 0) {
+        const int64_t ug = ug0 + f_eu;
+        f_src = a.ub + (size_t)(ug >> 5) * (size_t)a.u_rows * 128 + f_comp * 32 + (ug & 31);
+    }
+    const unsigned f_dst = (unsigned)__cvta_generic_to_shared(xr + f_comp * 4 + f_eu);
     auto fetch_tile = [&](int t) {
-        const int r0f = t * TR;
-        const int n_el = 40 << nshift;
-        for (int e0 = 0; e0 < n_el; e0 += 32) {
-            const int e = e0 + lane;
-            const int eu = e & ((1 << nshift) - 1);         // distinct track
-            const int sc = e >> nshift, slot = sc >> 1, comp = sc & 1;
-            const int32_t np_e = __shfl_sync(FULL, np, eu << zshift);
-            if (e < n_el && t < n_tiles_zg) {
+        if (t < n_tiles_zg) {
+            const int r0f = t * TR;
+            const unsigned dst_t = f_dst + (unsigned)((t % ZRING) * ZSLOT * 8);
+            for (int slot = f_slot0; slot < 20; slot += f_spi) {
                 const int k = slot < 16 ? r0f + slot : r0f + (slot - 16) * CK;
-                double* dst = xr + (t % ZRING) * ZSLOT + sc * 4 + eu;   // [slot][comp][4]: constant strides for the readers
-                if (np_e > 0) {                             // rows past n_pts - 1 repeat the last state
-                    const int64_t ug = ug0 + eu;
-                    const double* src = a.ub + ((size_t)(ug >> 5) * (size_t)a.u_rows + (size_t)min(k, np_e - 1)) * 128 +
-                                        (slot < 16 ? comp : 2 + comp) * 32 + (ug & 31);
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src));
+                if (f_np > 0) {                             // rows past n_pts - 1 repeat the last state
+                    const double* src = f_src + (size_t)min(k, f_np - 1) * 128 + (slot < 16 ? 0 : 64);
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst_t + (unsigned)(slot * 64)), "l"(src));
                 } else {
-                    *dst = 0.0;
+                    xr[(t % ZRING) * ZSLOT + slot * 8 + f_comp * 4 + f_eu] = 0.0;
                 }
             }
         }
