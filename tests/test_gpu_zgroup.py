@@ -1,0 +1,114 @@
+"""COMET_OPT_ZGROUP (scan_zgroup.cuh): seeds in runs that differ only in z share their transverse track.
+
+k_zgroup_check finds the run length on the device, k_gen_unique steps every distinct transverse track once and
+k_scan_fused<.., ZG> adds the z column.  The results must not depend on which path ran: n_pts and RSS are compared
+with the oracle bit for bit, for run lengths 8, 16 and 32, ragged seed counts, a seed set without runs (the plain
+kernel must take over) and with the option switched off; the work counter `unique_states` shows which path ran.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from comet_synth import event_seeds, make_config, seed_grid  # noqa: E402
+from oracle import comet_oracle as O  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def comet():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device")
+    from paper_1911_09340_b200 import Comet
+    from paper_1911_09340_b200.build import build
+    build()
+    c = Comet(0)
+    yield c
+    c.close()
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _scan(comet, ev, seeds, zgroup, r_stop=None):
+    from paper_1911_09340_b200.binding import OPT_STATS, OPT_ZGROUP
+    S = seeds.shape[1]
+    rss = torch.empty(S, dtype=torch.float64, device="cuda")
+    n_pts = torch.empty(S, dtype=torch.int32, device="cuda")
+    comet.set_option(OPT_ZGROUP, zgroup)
+    comet.set_option(OPT_STATS, 1)
+    comet.read_stats(reset=True)
+    try:
+        comet.scan_rss(_dev(seeds), ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop if r_stop is None else r_stop,
+                       _dev(ev.geom.wire_a), _dev(ev.geom.wire_b), _dev(ev.fired_wire), _dev(ev.hit_off), _dev(ev.rho),
+                       ev.cutoff, rss=rss, n_pts=n_pts)
+        st = comet.read_stats(reset=True)
+    finally:
+        comet.set_option(OPT_STATS, 0)
+        comet.set_option(OPT_ZGROUP, 1)
+    return rss.cpu().numpy(), n_pts.cpu().numpy(), st
+
+
+def _oracle(ev, seeds, r_stop=None):
+    return O.scan(seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop if r_stop is None else r_stop, ev.geom.wire_a,
+                  ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, want_npts=True)
+
+
+@pytest.mark.parametrize("n_z,n_seeds", [(8, 8 * 8 * 8 * 4), (16, 2048), (16, 2048 - 5), (32, 1024 + 32 + 7), (64, 1024)])
+def test_z_runs_identical_to_the_oracle(comet, cfg1_event, n_z, n_seeds):
+    """Grids with z as the fastest axis (run length n_z); seed counts that end inside a run and inside a chunk."""
+    ev = cfg1_event
+    sp = ev.spec
+    seeds = seed_grid(ev, 1, (8, 4, 4, n_z), tuple(sp["p_range"]), ct_hw=sp.get("ct_hw", 0.15))[:, :n_seeds]
+    seeds = np.ascontiguousarray(seeds)
+    ref = _oracle(ev, seeds)
+    rss, n_pts, st = _scan(comet, ev, seeds, 1)
+    assert np.array_equal(n_pts, ref["n_pts"]) and np.array_equal(rss, ref["rss"])
+    run = min(n_z, 32)
+    # the z-run kernels served the call: one RKN4 step per recorded state of every run's first seed
+    assert st["unique_states"] == int((ref["n_pts"][::run].astype(np.int64) - 1).sum())
+    rss0, n_pts0, st0 = _scan(comet, ev, seeds, 0)
+    assert st0["unique_states"] == 0
+    assert np.array_equal(rss0, rss) and np.array_equal(n_pts0, n_pts)
+    for k in ("samples", "rows_needed", "fine_needed", "pairs"):      # the same search, whoever generated the rows
+        assert st[k] == st0[k], k
+
+
+@pytest.mark.parametrize("case", ["runs_of_4", "one_odd_seed", "shuffled", "apex_stop"])
+def test_fallback_and_mixed_sets(comet, cfg1_event, case):
+    ev = cfg1_event
+    sp = ev.spec
+    pr = tuple(sp["p_range"])
+    r_stop = None
+    if case == "runs_of_4":
+        seeds = seed_grid(ev, 0, (8, 4, 8, 4), pr, ct_hw=0.15)       # z-runs shorter than 8: the plain kernel
+        expect_zg = False
+    elif case == "one_odd_seed":
+        seeds = seed_grid(ev, 0, (4, 4, 4, 16), pr, ct_hw=0.15).copy()
+        seeds[3, 777] *= 1.0000001                                    # one seed breaks its run
+        expect_zg = False
+    elif case == "shuffled":
+        seeds = seed_grid(ev, 0, (4, 4, 4, 16), pr, ct_hw=0.15)
+        seeds = seeds[:, np.random.default_rng(3).permutation(seeds.shape[1])]
+        expect_zg = False
+    else:
+        seeds = seed_grid(ev, 2, (4, 4, 4, 16), pr, ct_hw=0.15)      # half tracks: the target region beyond the chamber
+        r_stop = 1.0e3
+        expect_zg = True
+    seeds = np.ascontiguousarray(seeds)
+    ref = _oracle(ev, seeds, r_stop)
+    rss, n_pts, st = _scan(comet, ev, seeds, 1, r_stop)
+    assert np.array_equal(n_pts, ref["n_pts"]) and np.array_equal(rss, ref["rss"])
+    assert (st["unique_states"] > 0) == expect_zg
+
+
+def test_full_cfg1_both_paths_agree(comet, cfg1_event):
+    """The benchmarked event (3 x 131072 seeds, runs of 16): the z-run path against the plain path, every seed."""
+    ev = cfg1_event
+    seeds, _ = event_seeds(ev)
+    rss1, n1, st1 = _scan(comet, ev, seeds, 1)
+    rss0, n0, st0 = _scan(comet, ev, seeds, 0)
+    assert np.array_equal(rss1, rss0) and np.array_equal(n1, n0)
+    assert st1["unique_states"] * 16 == int(n1.astype(np.int64).sum()) - seeds.shape[1] and st0["unique_states"] == 0
