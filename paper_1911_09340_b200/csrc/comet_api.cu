@@ -71,6 +71,8 @@ struct comet_ctx {
     size_t npw_cap;
     double* cw;                  // [slab seeds] curvature constant c of every seed (fused path)
     size_t cw_bytes;
+    double* tw;                  // T_z per seed of a slab (ZG variants)
+    size_t tw_bytes;
     int fused_smem;
     FieldMap field;              // field.B == nullptr: uniform field (the bz_tesla arguments)
     double* bmax;                // device scalar: largest |B| of the map
@@ -214,7 +216,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ub); cudaFree(ctx->npu);
     for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
-    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->bmax);
+    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->tw); cudaFree(ctx->bmax);
     for (int l = 0; l < COMET_MAX_LANES; ++l) {
         if (ctx->ls[l]) cudaStreamDestroy(ctx->ls[l]);
         if (ctx->lf[l]) cudaStreamDestroy(ctx->lf[l]);
@@ -648,6 +650,8 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
         if (rc) return rc;
         rc = grow_dev(ctx, (void**)&ctx->npu, &ctx->npu_bytes, blocks * 32 * sizeof(int32_t));
         if (rc) return rc;
+        rc = grow_dev(ctx, (void**)&ctx->tw, &ctx->tw_bytes, (size_t)slab_chunks * COMET_LANES * sizeof(double));
+        if (rc) return rc;
     }
     if (!n_pts) {
         size_t have = ctx->npw_cap * sizeof(int32_t);
@@ -701,6 +705,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             a.bd = ctx->e2 + (size_t)cl * COMET_LANES * (size_t)n_fired;
             a.n_pts = n_pts ? n_pts + s0 : ctx->npw + cl * COMET_LANES;
             a.cw = ctx->cw + cl * COMET_LANES;
+            a.tw = zgroup ? ctx->tw + cl * COMET_LANES : nullptr;
             a.items = ctx->items + (size_t)cl * (size_t)n_fired;
             a.n_items = ctx->n_items + l;
             a.stats = ctx->opt_stats ? ctx->stats : nullptr;
@@ -755,7 +760,10 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             }
             if (n_fired > 0) {
                 if (field) k_fine_ck<true><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
-                else k_fine_ck<false><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
+                else {
+                    if (zgroup) k_fine_ck<false, true><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
+                    k_fine_ck<false><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
+                }
             }
             if (tm) CU(ctx, cudaEventRecord(tev[2], st));
             k_rss_sum<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_fine>>>(a.bd, a.SP, n_fired, a.n_seeds, rss + s0);

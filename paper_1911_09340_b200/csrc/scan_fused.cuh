@@ -95,6 +95,7 @@ struct FusedArgs {
     double* bd;              // [W][SP] packed (d^2, row) key of the pair's closest state so far; e^2 afterwards
     int32_t* n_pts;          // [n_seeds]
     double* cw;              // [SP] curvature constant c = kappa q B_z / |p| of every seed, for k_fine_ck
+    double* tw;              // [SP] ZG: T_z of every seed, for k_fine_ck
     unsigned long long* items;
     unsigned int* n_items;
     unsigned long long* stats;
@@ -230,10 +231,10 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
         if (t < n_tiles_zg) {
             const int r0f = t * TR;
             const unsigned dst_t = f_dst + (unsigned)((t % ZRING) * ZSLOT * 8);
-            for (int slot = f_slot0; slot < 20; slot += f_spi) {
-                const int k = slot < 16 ? r0f + slot : r0f + (slot - 16) * CK;
+            for (int slot = f_slot0; slot < 16; slot += f_spi) {
+                const int k = r0f + slot;
                 if (f_np > 0) {                             // rows past n_pts - 1 repeat the last state
-                    const double* src = f_src + (size_t)min(k, f_np - 1) * 128 + (slot < 16 ? 0 : 64);
+                    const double* src = f_src + (size_t)min(k, f_np - 1) * 128;
                     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst_t + (unsigned)(slot * 64)), "l"(src));
                 } else {
                     xr[(t % ZRING) * ZSLOT + slot * 8 + f_comp * 4 + f_eu] = 0.0;
@@ -281,14 +282,12 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
             }
             asm volatile("cp.async.wait_group %0;" ::"n"(ZRING - 1) : "memory");
             __syncwarp();
+            // checkpoints: z only -- k_fine_ck<.., ZG> takes (x, y, T_0, T_1) of the recorded states from the distinct
+            // tracks themselves (row stride 32 instead of 6 x 32 in the chunk's checkpoint block)
 #pragma unroll
             for (int rr = 0; rr < TR; rr += CK) {
                 const int k = r0 + rr;
-                if (k < np) {                               // k_fine_ck starts from checkpoints at or before n_pts - 1 only
-                    double* o = ckc + (size_t)(k / CK) * (CKF * COMET_LANES);
-                    o[0] = xc[(rr * 2) * 4]; o[32] = xc[(rr * 2 + 1) * 4]; o[64] = zt[rr * 32 + lane];
-                    o[96] = xc[((16 + rr / CK) * 2) * 4]; o[128] = xc[((16 + rr / CK) * 2 + 1) * 4]; o[160] = st.t2;
-                }
+                if (k < np) ckc[(size_t)(k / CK) * COMET_LANES] = zt[rr * 32 + lane];
             }
         }
         // ---- generate rows r0 .. r0 + TR - 1 (Algorithm 1; finished lanes hold their last state) ------
@@ -407,7 +406,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     PC_MARK();
 #endif
     if (ZG) { asm volatile("cp.async.wait_all;" ::: "memory"); __syncwarp(); }
-    if (valid) { a.n_pts[s] = np; a.cw[s] = c; }
+    if (valid) { a.n_pts[s] = np; a.cw[s] = c; if (ZG) a.tw[s] = st.t2; }
     // ---- finish: far pairs take the cutoff, (chunk, wire) items with a near lane go to k_fine_ck -------
     // Keys come from L2: FB wires in flight at a time.  The items are collected in the (now free) tile
     // and appended to the work list with one reservation per LCAP items.
@@ -475,9 +474,19 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
 #ifndef COMET_FINE_MINB_FIELD
 #define COMET_FINE_MINB_FIELD 2    // the field-map variant needs ~2x the registers (three field look-ups per step)
 #endif
-template <bool FIELD>
+// ZG = true (scan_zgroup.cuh): the candidates bk-1, bk, bk+1 are not regenerated: their (x, y, T_0, T_1) are the
+// recorded states of the seed's distinct transverse track (the same numbers), z comes from the z checkpoint at or
+// before bk-1 plus one addition per step.
+template <bool FIELD, bool ZG = false>
 __global__ void __launch_bounds__(COMET_FINE_THREADS, FIELD ? COMET_FINE_MINB_FIELD : COMET_FINE_MINB) k_fine_ck(const FusedArgs a)
 {
+    static_assert(!(FIELD && ZG), "the transverse motion depends on z in a field map");
+    if (ZG) {
+        if (zgroup_of(a.zg) < COMET_ZG_MIN) return;
+    } else if (!FIELD && a.zg && zgroup_of(a.zg) >= COMET_ZG_MIN) {
+        return;
+    }
+    const int zshift = ZG ? 31 - __clz((int)zgroup_of(a.zg)) : 0;
     constexpr int CK = COMET_CK_ROWS(FIELD);
     constexpr int CKF = COMET_CK_FIELDS(FIELD);
     const int lane = threadIdx.x & 31;
@@ -525,6 +534,34 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, FIELD ? COMET_FINE_MINB_FI
                 }
                 const double lo = (ks > 0) ? -bs_in : 0.0, hi = (ks < np - 1) ? bs_out : 0.0;
                 D = fine_dca_field(bs, lo, hi, c, a.F, wl);
+            } else if (ZG) {
+                const int kc = ka & ~(CK - 1);
+                const int64_t u = s >> zshift;
+                const double* g = a.ub + ((size_t)(u >> 5) * (size_t)a.u_rows + (size_t)ka) * 128 + (u & 31);
+                const double t2 = a.tw[s], hz = xmul(a.hk.h, t2);
+                double z = a.ck[(size_t)chunk * a.n_ck * (CKF * COMET_LANES) + (size_t)(kc / CK) * COMET_LANES + lane];
+                for (int k = kc; k < ka; ++k) z = xadd(z, hz);
+                State cand[3];
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {                // rows ka, ka + 1, ka + 2 (clamped: read, not used, past kz)
+                    const double* r = g + (size_t)min(j, kz - ka) * 128;
+                    cand[j].x0 = __ldg(r); cand[j].x1 = __ldg(r + 32); cand[j].t0 = __ldg(r + 64); cand[j].t1 = __ldg(r + 96);
+                    cand[j].t2 = t2;
+                }
+                State bs = cand[0];
+                int ks = ka;
+                double bd = 0.0;
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    if (ka + j <= kz) {
+                        cand[j].x2 = z;
+                        double u0, u1, u2;
+                        const double d2 = perp2_exact(cand[j].x0, cand[j].x1, z, wl, u0, u1, u2);
+                        if (j == 0 || d2 < bd) { bd = d2; ks = ka + j; bs = cand[j]; }
+                        z = xadd(z, hz);
+                    }
+                }
+                D = fine_dca(bs, ks, np, a.hk.h, c, wl);
             } else {
                 const int kc = ka & ~(CK - 1);
                 const double* o = a.ck + ((size_t)chunk * a.n_ck + (size_t)(kc / CK)) * (CKF * COMET_LANES) + lane;
