@@ -511,7 +511,7 @@ def run_ours(args):
     if fused and ms_call is not None:
         # the timed region runs k_scan_fused and k_fine_ck of different sub-slabs concurrently: the roofline entry
         # is the A + B call as launched there (both kernels' algorithmic work over the call's device time)
-        lanes = c.get_option(OPT_LANES)
+        lanes = 4 if c.get_option(OPT_ZGROUP) else c.get_option(OPT_LANES)
         top = {"kernel": "k_scan_fused + k_fine_ck (comet_scan_rss: sub-slabs on %d internal streams)" % lanes,
                "achieved": (fl[knames[0]] + fl[knames[1]]) / (ms_call * 1e-3) / 1e12, "ms_per_launch": ms_call,
                "achieved_executed": (fl_exec[knames[0]] + fl_exec[knames[1]]) / (ms_call * 1e-3) / 1e12,
@@ -531,11 +531,14 @@ def run_ours(args):
     if fused:
         # k_wire_prep, then k_scan_fused + k_fine_ck + k_rss_sum per sub-slab (the library's rule: up to
         # COMET_OPT_LANES sub-slabs of at least 2 CTAs of 4 chunks per SM), then k_wire_prep, k_argmin_stage1, k_select_classify
-        n_sub, chunks = c.get_option(OPT_LANES), (S + 31) // 32
+        zg_on = bool(c.get_option(OPT_ZGROUP))
+        n_sub, chunks = (4 if zg_on else c.get_option(OPT_LANES)), (S + 31) // 32
         n_sm = torch.cuda.get_device_properties(local).multi_processor_count
         while n_sub > 1 and chunks // n_sub < 4 * n_sm * 2:
             n_sub -= 1
-        launches_per_step = 1 + (6 if uniq > 0 or c.get_option(OPT_ZGROUP) else 3) * n_sub + 3   # ZGROUP: + k_zgroup_check, k_gen_unique, k_scan_fused<ZG>
+        # per sub-slab: k_scan_fused, k_fine_ck, k_rss_sum; with COMET_OPT_ZGROUP also k_zgroup_check, k_gen_unique and the ZG
+        # variants of the first two (the variants that do not serve the launch exit at once)
+        launches_per_step = 1 + (7 if zg_on else 3) * n_sub + 3
     else:
         launches_per_step = 8
     line = {

@@ -49,7 +49,7 @@ typedef enum comet_status {
                                        *   the closest one, and (when neither dca nor kstar is requested) pairs
                                        *   whose residual is provably the cutoff; k*, D and rss are identical   */
 #define COMET_OPT_TIMING 3            /* 1: comet_dca_rss (pruned) times its kernels, see comet_read_timing      */
-#define COMET_OPT_LANES 4             /* 1..8 (default 6): sub-slabs comet_scan_rss runs concurrently on internal streams */
+#define COMET_OPT_LANES 4             /* 1..8 (default 6, 4 with COMET_OPT_ZGROUP): sub-slabs comet_scan_rss runs concurrently on internal streams */
 #define COMET_OPT_ZGROUP 5            /* 1 (default): comet_scan_rss steps every distinct transverse track once when runs of >= 8
                                        *   consecutive seeds differ only in z (found on the device; results are identical) */
 #define COMET_OPT_STATS 2             /* 1: comet_dca_rss (pruned) adds its work counters, see comet_read_stats  */

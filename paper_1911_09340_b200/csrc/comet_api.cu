@@ -50,7 +50,8 @@ struct comet_ctx {
     // comet_scan_rss runs the sub-slabs of a slab concurrently: scan kernels on ls[], the fine stage on
     // the high-priority lf[] so that its CTAs take the slots retiring scan CTAs free
     int opt_lanes;
-    int opt_zgroup;              // 1 (default): seeds in z-runs go through k_scan_zg
+    int opt_zgroup;              // 1 (default): seeds in z-runs go through the ZG kernels (scan_zgroup.cuh)
+    int lanes_set;               // COMET_OPT_LANES was set by the caller
     unsigned int* zg_flag;       // [COMET_MAX_LANES] run length found by k_zgroup_check
     int zg_smem;                 // dynamic shared memory of k_scan_fused<.., ZG>
     double* ub;                  // distinct transverse tracks of a slab (k_gen_unique)
@@ -245,6 +246,7 @@ extern "C" int comet_set_option(comet_ctx* ctx, int option, int value)
     }
     if (option == COMET_OPT_LANES && value >= 1 && value <= COMET_MAX_LANES) {
         ctx->opt_lanes = value;
+        ctx->lanes_set = 1;
         return COMET_OK;
     }
     if (option == COMET_OPT_TIMING && (value == 0 || value == 1)) {
@@ -667,7 +669,11 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
     // (COMET_OPT_TIMING) and the work counters run one lane on the caller's stream.
     const bool tm = ctx->opt_timing != 0;
     // (in a field map the sub-slab kernels gain nothing from sharing the SMs: one lane)
-    const int lanes_opt = (tm || ctx->opt_stats || field) ? 1 : ctx->opt_lanes;
+    // (measured on configs[1]: 6 lanes suit the plain kernels, 4 the z-run kernels, whose sub-slabs start with a
+    // latency-bound k_gen_unique; a value set with COMET_OPT_LANES is taken as it is)
+    // (with seeds coming from the host the sub-slabs also pipeline the upload: finer sub-slabs)
+    const int lanes_auto = ctx->lanes_set ? ctx->opt_lanes : (seeds_host ? COMET_MAX_LANES : (zgroup ? 4 : ctx->opt_lanes));
+    const int lanes_opt = (tm || ctx->opt_stats || field) ? 1 : lanes_auto;
     for (int64_t c0 = 0; c0 < total_chunks; c0 += slab_chunks) {
         const int64_t nc_slab = (total_chunks - c0 < slab_chunks) ? (total_chunks - c0) : slab_chunks;
         // sub-slabs of whole CTAs, at least two CTAs per SM each
