@@ -48,8 +48,10 @@ FIELD_TOL = 1e-7
 FIELD_STEP_INSTR = 420
 # `seeding` entry: Hough accumulator (R36): directions, rho bins, rho window in 1/cm (R from 15 to 75 cm)
 HOUGH_N_PHI, HOUGH_N_RHO, HOUGH_RHO = 256, 128, (1.0 / 150.0, 1.0 / 30.0)
-# dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1d_full_scan_fused_fine_ck.txt)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1d_full_scan_fused_fine_ck.txt: plain kernels)
 TRAFFIC_BYTES = {"k_scan_fused": 347658496 + 2243479000, "k_fine_ck": 681160960 + 80465000}
+# the same with COMET_OPT_ZGROUP (profiles/r1g_full_zgroup.txt): k_gen_unique + k_scan_fused<ZG>, k_fine_ck<ZG>
+TRAFFIC_BYTES_ZG = {"k_scan_fused": 16869376 + 234161920 + 339810560 + 656851200, "k_fine_ck": 526513920 + 82170368}
 
 
 def _event(cfg):
@@ -516,7 +518,7 @@ def run_ours(args):
                "achieved": (fl[knames[0]] + fl[knames[1]]) / (ms_call * 1e-3) / 1e12, "ms_per_launch": ms_call,
                "achieved_executed": (fl_exec[knames[0]] + fl_exec[knames[1]]) / (ms_call * 1e-3) / 1e12,
                "timed": "CUDA events on the caller's stream around every comet_scan_rss of the timed region",
-               "traffic": (TRAFFIC_BYTES["k_scan_fused"] + TRAFFIC_BYTES["k_fine_ck"]) if args.config == 1 else None}
+               "traffic": (sum((TRAFFIC_BYTES_ZG if uniq > 0 else TRAFFIC_BYTES).values())) if args.config == 1 else None}
     else:
         top = {"kernel": kernel, "achieved": kernels[kernel]["achieved"], "ms_per_launch": ktimes[kernel],
                "timed": kernels["timed_over"], "traffic": None}
@@ -548,8 +550,11 @@ def run_ours(args):
         "config": {"workload": _workload_name(args.config, ev, seeds, part_off),
                    "path": ("fused: comet_scan_rss (track on chip) + comet_select_and_classify" if fused else
                             "materialised: comet_seed_extrapolate + comet_dca_rss + comet_select_and_classify"),
-                   "l2": ("working set larger than L2 (126 MB): every step rewrites %.1f GB of checkpoints and %.2f GB of "
-                          "(seed, wire) pair keys and rereads them" % (n_states * 12 / 1e9, pairs * 8 / 1e9)) if fused else
+                   "l2": (("working set larger than L2 (126 MB): every step rewrites %.2f GB of distinct-track rows, %.2f GB of z "
+                           "checkpoints and %.2f GB of (seed, wire) pair keys and rereads them"
+                           % (uniq * 32 / 1e9, n_states * 2 / 1e9, pairs * 8 / 1e9)) if uniq > 0 else
+                          ("working set larger than L2 (126 MB): every step rewrites %.1f GB of checkpoints and %.2f GB of "
+                           "(seed, wire) pair keys and rereads them" % (n_states * 12 / 1e9, pairs * 8 / 1e9))) if fused else
                          ("inputs larger than L2 (126 MB): every step rewrites the recorded part of the track buffer "
                           "(%.1f GB) and kernel B rereads it" % (n_states * 48 / 1e9)),
                    "parallelism": "one replica of the event per GPU (event-level sharding, no collective)"},
