@@ -186,7 +186,14 @@ int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64
  * With COMET_OPT_STATS the counters of comet_read_stats mean: [0] sub-block samples evaluated
  * (one per wire, sub-block and chunk), [1] rows swept for a lane whose tile holds recorded states,
  * [2] rows swept, [3] pairs that needed the virtual-plane iteration, [4] 32 x (chunk, wire) items
- * for which a warp executed it, [5] all pairs. */
+ * for which a warp executed it, [5] all pairs, [6] RKN4 steps taken for distinct transverse tracks
+ * by the z-run kernels (0 when the plain kernels served the call).
+ * COMET_OPT_ZGROUP (default 1, uniform field only): in B = (0, 0, B_z) the transverse motion does
+ * not depend on z, so seeds with bit-identical (x, y, p_x, p_y, p_z) share their (x, y, T_x, T_y)
+ * sequence and their stop.  When every aligned run of ZG >= 8 consecutive seeds of the call is
+ * uniform in those components (found on the device; the seed grids of the method with z as the
+ * fastest axis are), the RKN4 steps are taken once per distinct transverse track and every seed
+ * adds its own z column; rss and n_pts are the same numbers either way. */
 int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
                    int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                    const double* wire_a, const double* wire_b, int32_t n_wires,
