@@ -11,7 +11,7 @@
 // distinct track) and leaves (x_0, x_1, T_0, T_1) of every recorded state in a buffer that stays in L2;
 // k_scan_fused<.., ZG = true> (lane = seed) copies its tile rows from there, adds its own z column (one addition
 // per recorded state instead of the 48 operations of the RKN4 step) and goes on as before.  Every number is
-// produced by the same IEEE operations as in the plain k_scan_fused (and the oracle), so n_pts, checkpoints, keys
+// produced by the same IEEE operations as in the plain k_scan_fused (and the definition), so n_pts, checkpoints, keys
 // and RSS are bit-identical.
 //
 // Which seeds qualify is decided on the device (k_zgroup_check: the largest power of two ZG <= 32 such that every
