@@ -381,16 +381,20 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
                     const double* pr = tile + (j * FM1) * ROW + lane;
                     if (STATS) { st_cnt[ST_ROWS_EXEC] += FM1; if (is_live) st_cnt[ST_ROWS_NEEDED] += FM1; }
 #pragma unroll
+                    const double* pxz = xc + (j * FM1) * 8;  // ZG: (x, y) of the sub-block's rows
+                    const double* pzz = zt + (j * FM1) * 32 + lane;
+                    const int k0 = r0 + j * FM1;
                     for (int kk = 0; kk < FM1; ++kk) {
-                        const int row = j * FM1 + kk;
-                        const double d2 = ZG ? d2_fma(w, xc[(row * 2) * 4], xc[(row * 2 + 1) * 4], zt[row * 32 + lane])
+                        const double d2 = ZG ? d2_fma(w, pxz[kk * 8], pxz[kk * 8 + 4], pzz[kk * 32])
                                              : d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
-                        const int k = r0 + j * FM1 + kk;
-                        // rows at or past n_pts repeat the last state: not recorded, never taken
-                        if (d2 < best && k < np) { best = d2; bk = k; }
+                        if (d2 < best) { best = d2; bk = k0 + kk; }
                     }
                 }
-                if (bk >= 0) atomicMin(keys + (size_t)i * a.SP + s, pack_key(best, bk));
+                // Rows at or past n_pts repeat the last recorded state, so one of them can only tie with it (and then
+                // loses to the strict <) or stand in for it from a later sub-block: the row index is clamped, the distance
+                // is that state's own.  Lanes without a recorded row in this tile keep out.
+                bk = min(bk, np - 1);
+                if (bk >= 0 && np > r0) atomicMin(keys + (size_t)i * a.SP + s, pack_key(best, bk));
             }
             PC_ADD(pc_l1);
         }
