@@ -513,7 +513,7 @@ def run_ours(args):
     if fused and ms_call is not None:
         # the timed region runs k_scan_fused and k_fine_ck of different sub-slabs concurrently: the roofline entry
         # is the A + B call as launched there (both kernels' algorithmic work over the call's device time)
-        lanes = 4 if c.get_option(OPT_ZGROUP) else c.get_option(OPT_LANES)
+        lanes = 4 if (c.get_option(OPT_ZGROUP) and (S + 31) // 32 >= 1024) else c.get_option(OPT_LANES)
         top = {"kernel": "k_scan_fused + k_fine_ck (comet_scan_rss: sub-slabs on %d internal streams)" % lanes,
                "achieved": (fl[knames[0]] + fl[knames[1]]) / (ms_call * 1e-3) / 1e12, "ms_per_launch": ms_call,
                "achieved_executed": (fl_exec[knames[0]] + fl_exec[knames[1]]) / (ms_call * 1e-3) / 1e12,
@@ -533,8 +533,9 @@ def run_ours(args):
     if fused:
         # k_wire_prep, then k_scan_fused + k_fine_ck + k_rss_sum per sub-slab (the library's rule: up to
         # COMET_OPT_LANES sub-slabs of at least 2 CTAs of 4 chunks per SM), then k_wire_prep, k_argmin_stage1, k_select_classify
-        zg_on = bool(c.get_option(OPT_ZGROUP))
-        n_sub, chunks = (4 if zg_on else c.get_option(OPT_LANES)), (S + 31) // 32
+        chunks = (S + 31) // 32
+        zg_on = bool(c.get_option(OPT_ZGROUP)) and chunks >= 1024        # the library's size threshold for the z-run kernels
+        n_sub = 4 if zg_on else c.get_option(OPT_LANES)
         n_sm = torch.cuda.get_device_properties(local).multi_processor_count
         while n_sub > 1 and chunks // n_sub < 4 * n_sm * 2:
             n_sub -= 1

@@ -51,7 +51,8 @@ typedef enum comet_status {
 #define COMET_OPT_TIMING 3            /* 1: comet_dca_rss (pruned) times its kernels, see comet_read_timing      */
 #define COMET_OPT_LANES 4             /* 1..8 (default 6, 4 with COMET_OPT_ZGROUP): sub-slabs comet_scan_rss runs concurrently on internal streams */
 #define COMET_OPT_ZGROUP 5            /* 1 (default): comet_scan_rss steps every distinct transverse track once when runs of >= 8
-                                       *   consecutive seeds differ only in z (found on the device; results are identical) */
+                                       *   consecutive seeds differ only in z (found on the device; results are identical) and the
+                                       *   call has at least 1024 chunks; 2: whatever the size of the call; 0: never */
 #define COMET_OPT_STATS 2             /* 1: comet_dca_rss (pruned) adds its work counters, see comet_read_stats  */
 
 /* ---- context ---------------------------------------------------------------------------- */
@@ -193,7 +194,8 @@ int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64
  * sequence and their stop.  When every aligned run of ZG >= 8 consecutive seeds of the call is
  * uniform in those components (found on the device; the seed grids of the method with z as the
  * fastest axis are), the RKN4 steps are taken once per distinct transverse track and every seed
- * adds its own z column; rss and n_pts are the same numbers either way. */
+ * adds its own z column; rss and n_pts are the same numbers either way.  Calls of fewer than 1024
+ * chunks (32768 seeds) always take the plain kernels. */
 int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
                    int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                    const double* wire_a, const double* wire_b, int32_t n_wires,

@@ -28,6 +28,9 @@
 #ifndef COMET_DEFAULT_LANES
 #define COMET_DEFAULT_LANES 6
 #endif
+#ifndef COMET_ZG_MIN_CHUNKS
+#define COMET_ZG_MIN_CHUNKS 1024
+#endif
 #define COMET_PR_CAP_S 96      // sub-block samples staged in shared memory per chunk (72 KB)
 
 using namespace comet;
@@ -240,7 +243,7 @@ extern "C" int comet_set_option(comet_ctx* ctx, int option, int value)
         ctx->opt_stats = value;
         return COMET_OK;
     }
-    if (option == COMET_OPT_ZGROUP && (value == 0 || value == 1)) {
+    if (option == COMET_OPT_ZGROUP && value >= 0 && value <= 2) {
         ctx->opt_zgroup = value;
         return COMET_OK;
     }
@@ -642,7 +645,9 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
     if (rc) return rc;
     rc = grow_dev(ctx, (void**)&ctx->cw, &ctx->cw_bytes, (size_t)slab_chunks * COMET_LANES * sizeof(double));
     if (rc) return rc;
-    const bool zgroup = !field && ctx->opt_zgroup != 0;
+    // (small calls are launch- and latency-bound: the run-length check and the chain of k_gen_unique in front of the
+    // scan cost more than they save below about a thousand chunks -- configs[0], the refined sets of a stage)
+    const bool zgroup = !field && ctx->opt_zgroup != 0 && (ctx->opt_zgroup == 2 || total_chunks >= COMET_ZG_MIN_CHUNKS);
     // distinct transverse tracks (scan_zgroup.cuh): at most 4 per chunk (runs of >= 8 seeds), blocks of 32 tracks of
     // n_steps + 1 rows of 4 doubles; every sub-slab starts on a block of its own
     const size_t ub_block = (size_t)(n_steps + 1) * 128 * sizeof(double);

@@ -37,7 +37,7 @@ def _scan(comet, ev, seeds, zgroup, r_stop=None):
     S = seeds.shape[1]
     rss = torch.empty(S, dtype=torch.float64, device="cuda")
     n_pts = torch.empty(S, dtype=torch.int32, device="cuda")
-    comet.set_option(OPT_ZGROUP, zgroup)
+    comet.set_option(OPT_ZGROUP, 2 if zgroup else 0)        # 2: also for calls below the size threshold of the default
     comet.set_option(OPT_STATS, 1)
     comet.read_stats(reset=True)
     try:
@@ -112,3 +112,19 @@ def test_full_cfg1_both_paths_agree(comet, cfg1_event):
     rss0, n0, st0 = _scan(comet, ev, seeds, 0)
     assert np.array_equal(rss1, rss0) and np.array_equal(n1, n0)
     assert st1["unique_states"] * 16 == int(n1.astype(np.int64).sum()) - seeds.shape[1] and st0["unique_states"] == 0
+
+
+def test_small_calls_take_the_plain_kernels_by_default(comet, cfg0_event):
+    """configs[0] (8192 seeds in runs of 8) is below the size threshold of COMET_OPT_ZGROUP = 1."""
+    from paper_1911_09340_b200.binding import OPT_STATS
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev)
+    comet.set_option(OPT_STATS, 1)
+    comet.read_stats(reset=True)
+    try:
+        comet.scan_rss(_dev(seeds), ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, _dev(ev.geom.wire_a), _dev(ev.geom.wire_b),
+                       _dev(ev.fired_wire), _dev(ev.hit_off), _dev(ev.rho), ev.cutoff)
+        st = comet.read_stats(reset=True)
+    finally:
+        comet.set_option(OPT_STATS, 0)
+    assert st["unique_states"] == 0 and st["pairs"] == seeds.shape[1] * ev.n_fired
