@@ -74,7 +74,11 @@ __global__ void __launch_bounds__(128) k_gen_unique(const FusedArgs a)
             rkn4_step(st, a.hk, c);
             double* r = o + (size_t)(k + j) * 128;
             r[0] = st.x0; r[32] = st.x1; r[64] = st.t0; r[96] = st.t1;
-            if (use_stop && first == 4 && in_target_region(st, a.r_stop2)) first = j;
+            // in_target_region without its early exit: no branch waits for this step's position
+            const double r2 = xadd(xmul(st.x0, st.x0), xmul(st.x1, st.x1));
+            const double rad = xadd(xmul(st.x0, st.t0), xmul(st.x1, st.t1));
+            const bool stop = (r2 < a.r_stop2) & (rad < 0.0) & use_stop;
+            first = (stop & (first == 4)) ? j : first;
         }
         if (first < 4) { np = k + first + 1; break; }
     }
