@@ -726,7 +726,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                     CU(ctx, cudaMemcpyAsync(seeds_w + (size_t)j * seed_stride + s0, seeds_host + (size_t)j * n_seeds + s0,
                                             sizeof(double) * (size_t)a.n_seeds, cudaMemcpyHostToDevice, s_scan));
             CU(ctx, cudaMemsetAsync(a.n_items, 0, sizeof(unsigned int), s_scan));
-            const unsigned b1 = (unsigned)((nc + COMET_FUSED_WARPS - 1) / COMET_FUSED_WARPS);
+            const unsigned b1_packed = (unsigned)((nc + COMET_FUSED_WARPS - 1) / COMET_FUSED_WARPS);
             const int64_t w2 = nc * (int64_t)n_fired;
             const int64_t b2_all = (w2 + COMET_FINE_THREADS / 32 - 1) / (COMET_FINE_THREADS / 32);
             unsigned b2 = (unsigned)(b2_all < ctx->fine_blocks ? b2_all : ctx->fine_blocks);
@@ -734,6 +734,9 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
             if (tm) CU(ctx, cudaEventRecord(tev[0], st));
             const int thr = 32 * COMET_FUSED_WARPS;
+            // a launch that cannot give every SM two CTAs of four chunks: the CTA's warps share one chunk's wires
+            a.split = (!zgroup && n_fired > 32 && nc < (int64_t)COMET_FUSED_WARPS * ctx->n_sm * 2) ? 1 : 0;
+            const unsigned b1 = a.split ? (unsigned)nc : b1_packed;
             a.zg = nullptr;
             a.ub = nullptr;
             a.np_u = nullptr;

@@ -101,6 +101,7 @@ struct FusedArgs {
     unsigned long long* stats;
     FieldMap F;              // field-map variants (FIELD = true): the map, and qkb = kappa q, hk.h = h_max
     double h_min;            // h_max / 64 (R31)
+    int32_t split;           // 1: the warps of a CTA share one chunk and split its wires (small launches)
     const unsigned int* zg;  // scan_zgroup.cuh: run length of the launch's seeds (device); nullptr = not checked
     double* ub;              // scan_zgroup.cuh: (x_0, x_1, T_0, T_1) of the distinct transverse tracks [u / 32][u_rows][4][32]
     int32_t* np_u;           //   and their numbers of recorded states
@@ -168,7 +169,11 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     for (int i = threadIdx.x; i < WCAP; i += 32 * COMET_FUSED_WARPS)
         wtab[COMET_FUSED_WFIELDS * WCAP + i] = (i < W) ? wire_slope(__ldg(a.wt + (size_t)8 * W + i), __ldg(a.wt + (size_t)12 * W + i)) : 0.0;
     __syncthreads();
-    const int64_t chunk = (int64_t)blockIdx.x * COMET_FUSED_WARPS + warp;
+    // a.split (small launches that cannot fill the GPU: the refined seed sets of a stage): the CTA's warps all take
+    // the SAME chunk -- each generates the track for itself -- and share its wires: warp w takes the level-0 rounds
+    // and the finish groups w, w + 4, ...; one chunk is then a quarter of the serial work per warp
+    const int wpart = a.split ? warp : 0, nparts = a.split ? COMET_FUSED_WARPS : 1;
+    const int64_t chunk = a.split ? (int64_t)blockIdx.x : (int64_t)blockIdx.x * COMET_FUSED_WARPS + warp;
     if (chunk * COMET_LANES >= a.n_seeds) return;
     const int64_t s = chunk * COMET_LANES + lane;
     const bool valid = s < a.n_seeds;
@@ -245,7 +250,8 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     };
     // pair workspace of this chunk: nothing found yet
     unsigned long long* const keys = reinterpret_cast<unsigned long long*>(a.bd);
-    for (int i = 0; i < W; ++i) keys[(size_t)i * a.SP + s] = COMET_KEY_NONE;
+    for (int i = 32 * wpart; i < W; i += 32 * nparts)      // (the wires of this warp's rounds)
+        for (int q = i; q < min(i + 32, W); ++q) keys[(size_t)q * a.SP + s] = COMET_KEY_NONE;
 
     const int n_rounds = (W + 31) / 32;                     // level 0: wire i = r * 32 + lane
     double* ckc = a.ck + (size_t)chunk * a.n_ck * (CKF * COMET_LANES) + lane;
@@ -254,7 +260,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     if (STATS) {
 #pragma unroll
         for (int j = 0; j < ST_N; ++j) st_cnt[j] = 0;
-        if (valid) st_cnt[ST_PAIRS] = (unsigned long long)W;
+        if (valid && wpart == 0) st_cnt[ST_PAIRS] = (unsigned long long)W;
     }
 #ifdef COMET_FUSED_PROF
     long long pc_gen = 0, pc_l0 = 0, pc_l1 = 0, pc_visits = 0, pc_sweeps = 0, pc_mark;
@@ -302,7 +308,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
             if (k >= a.n_steps) active = false;
             double* tr = tile + rr * ROW + lane;
             tr[0] = st.x0; tr[32] = st.x1; tr[64] = st.x2;
-            if ((rr & (CK - 1)) == 0 && k <= a.n_steps) {
+            if ((rr & (CK - 1)) == 0 && k <= a.n_steps && wpart == 0) {
                 double* o = ckc + (size_t)(k / CK) * (CKF * COMET_LANES);
                 o[0] = st.x0; o[32] = st.x1; o[64] = st.x2; o[96] = st.t0; o[128] = st.t1; o[160] = st.t2;
                 if (FIELD) o[192] = htry;
@@ -338,7 +344,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
             rz[j] = __uint_as_float(__reduce_max_sync(FULL, __float_as_uint(fz)));
         }
         const bool any_nolip = (nolip_mask & live) != 0u;
-        for (int r = 0; r < n_rounds; ++r) {
+        for (int r = wpart; r < n_rounds; r += nparts) {
             unsigned sm = 0u;                               // bit j: sub-block j of this tile may matter to the lane's wire
             {
                 const int i = r * 32 + lane;
@@ -410,7 +416,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     PC_MARK();
 #endif
     if (ZG) { asm volatile("cp.async.wait_all;" ::: "memory"); __syncwarp(); }
-    if (valid) { a.n_pts[s] = np; a.cw[s] = c; if (ZG) a.tw[s] = st.t2; }
+    if (valid && wpart == 0) { a.n_pts[s] = np; a.cw[s] = c; if (ZG) a.tw[s] = st.t2; }
     // ---- finish: far pairs take the cutoff, (chunk, wire) items with a near lane go to k_fine_ck -------
     // Keys come from L2: FB wires in flight at a time.  The items are collected in the (now free) tile
     // and appended to the work list with one reservation per LCAP items.
@@ -427,7 +433,9 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
         cnt = 0;
         __syncwarp();
     };
+    // (a.split: the groups of the wires of this warp's rounds: FB divides 32)
     for (int i0 = 0; i0 < W; i0 += FB) {
+        if (((i0 >> 5) % nparts) != wpart) continue;
         unsigned long long kv[FB];
         double cap2[FB];
 #pragma unroll
