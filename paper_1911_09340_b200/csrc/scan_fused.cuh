@@ -172,8 +172,9 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     // a.split (small launches that cannot fill the GPU: the refined seed sets of a stage): the CTA's warps all take
     // the SAME chunk -- each generates the track for itself -- and share its wires: warp w takes the level-0 rounds
     // and the finish groups w, w + 4, ...; one chunk is then a quarter of the serial work per warp
-    const int wpart = a.split ? warp : 0, nparts = a.split ? COMET_FUSED_WARPS : 1;
-    const int64_t chunk = a.split ? (int64_t)blockIdx.x : (int64_t)blockIdx.x * COMET_FUSED_WARPS + warp;
+    const bool split = !ZG && a.split;                      // (the z-run variant serves large launches only)
+    const int wpart = split ? warp : 0, nparts = split ? COMET_FUSED_WARPS : 1;
+    const int64_t chunk = split ? (int64_t)blockIdx.x : (int64_t)blockIdx.x * COMET_FUSED_WARPS + warp;
     if (chunk * COMET_LANES >= a.n_seeds) return;
     const int64_t s = chunk * COMET_LANES + lane;
     const bool valid = s < a.n_seeds;
