@@ -143,9 +143,11 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     ctx->ck_max = (size_t)8 << 30;
     ctx->fused_smem = ((COMET_FUSED_WFIELDS + 1) * COMET_FUSED_WCAP + COMET_FUSED_WARPS * COMET_FUSED_TR * 3 * COMET_LANES) * (int)sizeof(double);
     {
-        const void* fk[4] = {(const void*)k_scan_fused<false, false>, (const void*)k_scan_fused<true, false>,
-                             (const void*)k_scan_fused<false, true>, (const void*)k_scan_fused<true, true>};
-        for (int j = 0; j < 4 && e == cudaSuccess; ++j) {
+        const void* fk[8] = {(const void*)k_scan_fused<false, false>, (const void*)k_scan_fused<true, false>,
+                             (const void*)k_scan_fused<false, true>, (const void*)k_scan_fused<true, true>,
+                             (const void*)k_scan_fused<false, false, false, true>, (const void*)k_scan_fused<true, false, false, true>,
+                             (const void*)k_scan_fused<false, true, false, true>, (const void*)k_scan_fused<true, true, false, true>};
+        for (int j = 0; j < 8 && e == cudaSuccess; ++j) {
             e = cudaFuncSetAttribute(fk[j], cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(fk[j], cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         }
@@ -735,8 +737,8 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             if (tm) CU(ctx, cudaEventRecord(tev[0], st));
             const int thr = 32 * COMET_FUSED_WARPS;
             // a launch that cannot give every SM two CTAs of four chunks: the CTA's warps share one chunk's wires
-            a.split = (!zgroup && n_fired > 32 && nc < (int64_t)COMET_FUSED_WARPS * ctx->n_sm * 2) ? 1 : 0;
-            const unsigned b1 = a.split ? (unsigned)nc : b1_packed;
+            const bool split = !zgroup && n_fired > 32 && nc < (int64_t)COMET_FUSED_WARPS * ctx->n_sm * 2;
+            const unsigned b1 = split ? (unsigned)nc : b1_packed;
             a.zg = nullptr;
             a.ub = nullptr;
             a.np_u = nullptr;
@@ -760,7 +762,15 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                     k_scan_fused<false, false, true><<<b1, thr, ctx->zg_smem, s_scan>>>(a);
                 }
             }
-            if (field) {
+            if (split) {
+                if (field) {
+                    if (a.stats) k_scan_fused<true, true, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                    else k_scan_fused<false, true, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                } else {
+                    if (a.stats) k_scan_fused<true, false, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                    else k_scan_fused<false, false, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                }
+            } else if (field) {
                 if (a.stats) k_scan_fused<true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
                 else k_scan_fused<false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
             } else {

@@ -101,7 +101,6 @@ struct FusedArgs {
     unsigned long long* stats;
     FieldMap F;              // field-map variants (FIELD = true): the map, and qkb = kappa q, hk.h = h_max
     double h_min;            // h_max / 64 (R31)
-    int32_t split;           // 1: the warps of a CTA share one chunk and split its wires (small launches)
     const unsigned int* zg;  // scan_zgroup.cuh: run length of the launch's seeds (device); nullptr = not checked
     double* ub;              // scan_zgroup.cuh: (x_0, x_1, T_0, T_1) of the distinct transverse tracks [u / 32][u_rows][4][32]
     int32_t* np_u;           //   and their numbers of recorded states
@@ -141,7 +140,7 @@ __device__ __forceinline__ double wire_slope(double e1z, double e2z)
 
 // ZG = true: the rows of a tile are not generated here: (x, y) come from the distinct transverse tracks of
 // k_gen_unique and z is accumulated per seed (scan_zgroup.cuh); everything after the tile is the same code.
-template <bool STATS, bool FIELD, bool ZG = false>
+template <bool STATS, bool FIELD, bool ZG = false, bool SPLIT = false>
 __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_ZG : COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
 {
     static_assert(!(FIELD && ZG), "the transverse motion depends on z in a field map");
@@ -169,10 +168,11 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     for (int i = threadIdx.x; i < WCAP; i += 32 * COMET_FUSED_WARPS)
         wtab[COMET_FUSED_WFIELDS * WCAP + i] = (i < W) ? wire_slope(__ldg(a.wt + (size_t)8 * W + i), __ldg(a.wt + (size_t)12 * W + i)) : 0.0;
     __syncthreads();
-    // a.split (small launches that cannot fill the GPU: the refined seed sets of a stage): the CTA's warps all take
+    // SPLIT (small launches that cannot fill the GPU: the refined seed sets of a stage): the CTA's warps all take
     // the SAME chunk -- each generates the track for itself -- and share its wires: warp w takes the level-0 rounds
     // and the finish groups w, w + 4, ...; one chunk is then a quarter of the serial work per warp
-    const bool split = !ZG && a.split;                      // (the z-run variant serves large launches only)
+    static_assert(!(ZG && SPLIT), "the z-run variant serves large launches only");
+    constexpr bool split = SPLIT;
     const int wpart = split ? warp : 0, nparts = split ? COMET_FUSED_WARPS : 1;
     const int64_t chunk = split ? (int64_t)blockIdx.x : (int64_t)blockIdx.x * COMET_FUSED_WARPS + warp;
     if (chunk * COMET_LANES >= a.n_seeds) return;
@@ -434,7 +434,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
         cnt = 0;
         __syncwarp();
     };
-    // (a.split: the groups of the wires of this warp's rounds: FB divides 32)
+    // (SPLIT: the groups of the wires of this warp's rounds: FB divides 32)
     for (int i0 = 0; i0 < W; i0 += FB) {
         if (((i0 >> 5) % nparts) != wpart) continue;
         unsigned long long kv[FB];
