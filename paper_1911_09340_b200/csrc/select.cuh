@@ -99,7 +99,27 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
         int32_t np = a.n_steps + 1;
         sm[0] = st.x0; sm[1] = st.x1; sm[2] = st.x2; sm[3] = st.t0; sm[4] = st.t1; sm[5] = st.t2;
         double htry = a.hk.h;
-        for (int32_t k = 1; k <= a.n_steps; ++k) {
+        int32_t k = 1;
+        if (!FIELD) {
+            // one thread, one chain of dependent operations: blocks of four steps are recorded unconditionally (rows
+            // past the stop are never read) and the stop test stays off the chain, as in k_gen_unique
+            const bool use_stop = a.r_stop2 > 0.0;
+            for (; k + 3 <= a.n_steps; k += 4) {
+                int first = 4;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    rkn4_step(st, a.hk, c);
+                    double* o = sm + (size_t)(k + j) * RS;
+                    o[0] = st.x0; o[1] = st.x1; o[2] = st.x2; o[3] = st.t0; o[4] = st.t1; o[5] = st.t2;
+                    const double r2 = xadd(xmul(st.x0, st.x0), xmul(st.x1, st.x1));
+                    const double rad = xadd(xmul(st.x0, st.t0), xmul(st.x1, st.t1));
+                    const bool stop = (r2 < a.r_stop2) & (rad < 0.0) & use_stop;
+                    first = (stop & (first == 4)) ? j : first;
+                }
+                if (first < 4) { np = k + first + 1; break; }
+            }
+        }
+        for (; np == a.n_steps + 1 && k <= a.n_steps; ++k) {
             if (FIELD) sm[(size_t)(k - 1) * RS + 6] = adaptive_field_step(st, htry, a.hk.h, a.h_min, c, a.F);
             else rkn4_step(st, a.hk, c);
             double* o = sm + (size_t)k * RS;
