@@ -57,7 +57,7 @@ namespace comet {
 #define COMET_FUSED_MINB_ZG 4      // (5 CTAs per SM fit the smaller tile of the ZG variant but 96 registers cost more than they gain)
 #endif
 #define COMET_ZG_RING 4            // compact tiles fetched ahead (scan_zgroup.cuh)
-#define COMET_ZG_SLOT 160          // doubles per compact tile: [20][2][4 distinct tracks]
+#define COMET_ZG_SLOT 128          // doubles per compact tile: [16 rows][x, y][4 distinct tracks]
 #define COMET_ZG_WTILE (COMET_FUSED_TR * 32 + COMET_ZG_RING * COMET_ZG_SLOT)   // doubles per warp in the ZG variant
 #define COMET_FUSED_WFIELDS 9      // e1[3] -m.e1 | e2[3] -m.e2 | far radius  (fields 6..14 of the wire table)
 // the CTA's table has one more row: sqrt(1 - w_z^2) rounded up, the wire's slope against the z axis
@@ -201,8 +201,8 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     const bool use_stop = a.r_stop2 > 0.0;
     // ZG: the chunk's NU = 32 / ZG distinct transverse tracks, the seed's (final) number of recorded states and
     // the z advance of a step.  The warp's shared memory holds the z column of the tile [TR][32] and a ring of
-    // ZRING compact tiles [20][2][NU]: (x, y) of the 16 rows and (T_0, T_1) of the 4 checkpoint rows of every
-    // distinct track, fetched ZRING - 1 tiles ahead with cp.async from k_gen_unique's buffer.
+    // ZRING compact tiles [16][2][4]: (x, y) of the 16 rows of every distinct track, fetched ZRING - 1 tiles ahead
+    // with cp.async from k_gen_unique's buffer.
     constexpr int ZRING = COMET_ZG_RING, ZSLOT = COMET_ZG_SLOT;
     const int n_tiles_zg = (a.n_steps + TR) / TR;
     static_assert(TR == 16 && CK == 4 || !ZG, "compact tile layout");
