@@ -463,7 +463,7 @@ static int launch_wire_prep(comet_ctx* ctx, const double* wire_a, const double* 
     if (n_fired > ctx->wt_cap) return COMET_EINVAL;
     if (n_fired == 0) return COMET_OK;
     k_wire_prep<<<(n_fired + 127) / 128, 128, 0, st>>>(wire_a, wire_b, n_wires, fired_wire, n_fired, hit_off, rho,
-                                                       cutoff_cm, step_cm, ctx->wt);
+                                                       cutoff_cm, step_cm, ctx->field.B == nullptr ? 1 : 0, ctx->wt);
     CU(ctx, cudaGetLastError());
     return COMET_OK;
 }

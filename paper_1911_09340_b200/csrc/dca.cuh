@@ -34,10 +34,23 @@ namespace comet {
 // 0.01 h + 1e-6 cover the step-length excess 1.001 and the RKN error of the sub-steps).  A track whose
 // every recorded state is farther than R_i therefore has |D| - |rho_ij| > lambda for every entry and
 // its bounded residual is exactly lambda (pruned mode).
+//
+// `tight` (uniform field: recorded states exactly h of arc apart): a sharper radius from the shape of the
+// distance along the track.  Let s* be the arc position of k*, d* = d_k*, and u = s - s* in the bracket of the
+// iteration (|u| <= 1.001 h).  On the tangent line at k* the squared distance to the wire is the quadratic
+// g(u)^2 = d*^2 + a u (u + 2 v), 0 <= a <= 1, with its minimum at u = -v; the track leaves that line by at most
+// eps = |c| (1.001 h)^2 / 2 <= 0.0251 h (|c| h <= COMET_CH_MAX = 0.05; lanes beyond that take no shortcut), and the
+// distance to a line is 1-Lipschitz, so the neighbours' d_k*+-1 >= d* give g(+-h) >= d* - eps, i.e.
+// a h (2|v| - h) <= 2 d* eps.  Minimising g^2 over the bracket under that constraint (|v| <= h: -a v^2 with
+// a v^2 <= a h^2/4 + 1.5 d* eps; |v| > h: the bracket end, -a h (2|v| - h) >= -2 d* eps) leaves
+// g^2 >= d*^2 - 0.2505 h^2 - 2 d* eps everywhere in the bracket -- at a track end the missing neighbour's side is
+// not in the bracket --, hence |D| >= sqrt(d*^2 - 0.2505 h^2 - 2 d* eps) - eps - 1e-6 for whatever point the
+// iteration ends on.  |D| - max|rho| > lambda then follows from d* > eps + sqrt((max|rho| + lambda + eps + 1e-6)^2
+// + 0.2505 h^2 + eps^2); the smaller of the two radii is used.
 __global__ void k_wire_prep(const double* __restrict__ wire_a, const double* __restrict__ wire_b,
                             int32_t n_wires, const int32_t* __restrict__ fired_wire, int32_t W,
                             const int32_t* __restrict__ hit_off, const double* __restrict__ rho,
-                            double lambda, double h, double* __restrict__ wt)
+                            double lambda, double h, int tight, double* __restrict__ wt)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= W) return;
@@ -66,7 +79,12 @@ __global__ void k_wire_prep(const double* __restrict__ wire_a, const double* __r
     wt[13 * W + i] = -(m0 * q0 + m1 * q1 + m2 * q2);
     double rmax = -1.0;
     for (int j = hit_off[i]; j < hit_off[i + 1]; ++j) rmax = fmax(rmax, fabs(rho[j]));
-    wt[14 * W + i] = (rmax < 0.0) ? -1.0 : rmax + lambda + 0.51 * h + 1e-6;
+    double cap = rmax + lambda + 0.51 * h + 1e-6;
+    if (tight) {
+        const double eps = 0.0251 * h, b = rmax + lambda + eps + 1e-6;
+        cap = fmin(cap, eps + sqrt(b * b + 0.2505 * h * h + eps * eps));
+    }
+    wt[14 * W + i] = (rmax < 0.0) ? -1.0 : cap;
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)
