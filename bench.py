@@ -50,8 +50,8 @@ FIELD_STEP_INSTR = 420
 HOUGH_N_PHI, HOUGH_N_RHO, HOUGH_RHO = 256, 128, (1.0 / 150.0, 1.0 / 30.0)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1] (profiles/r1d_full_scan_fused_fine_ck.txt: plain kernels)
 TRAFFIC_BYTES = {"k_scan_fused": 347658496 + 2243479000, "k_fine_ck": 681160960 + 80465000}
-# the same with COMET_OPT_ZGROUP (profiles/r1g_full_zgroup.txt): k_gen_unique + k_scan_fused<ZG>, k_fine_ck<ZG>
-TRAFFIC_BYTES_ZG = {"k_scan_fused": 16869376 + 234161920 + 339810560 + 656851200, "k_fine_ck": 526513920 + 82170368}
+# the same with COMET_OPT_ZGROUP (profiles/r1h_full_zgroup.txt): k_gen_unique + k_scan_fused<ZG>, k_fine_ck<ZG>
+TRAFFIC_BYTES_ZG = {"k_scan_fused": 17152768 + 235757056 + 338066432 + 661437952, "k_fine_ck": 471857920 + 72980736}
 
 
 def _event(cfg):
