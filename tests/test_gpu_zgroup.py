@@ -128,3 +128,22 @@ def test_small_calls_take_the_plain_kernels_by_default(comet, cfg0_event):
     finally:
         comet.set_option(OPT_STATS, 0)
     assert st["unique_states"] == 0 and st["pairs"] == seeds.shape[1] * ev.n_fired
+
+
+def test_turn_loop_at_full_size_runs_partitions_through_the_z_run_kernels(comet, cfg1_event):
+    """comet_scan_turns on the full configs[1] grids: every stage scans ONE partition of the caller's seed array
+    (a pointer offset with the whole array's stride, 4096 chunks: above the size threshold), against a hit list that
+    shrinks from stage to stage -- turn seeds, RSS and classified sets identical to the oracle's loop."""
+    ev = cfg1_event
+    seeds, po = event_seeds(ev)
+    kw = dict(half_width=[0.6, 0.5, 0.5, 1.0], n_grid=[3, 3, 3, 3], n_iter=1, shrink=0.5, k_ref=4)
+    args = (ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop)
+    ref = O.scan_turns(seeds, po, *args, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, **kw)
+    got = comet.scan_turns(_dev(seeds), po, *args, _dev(ev.geom.wire_a), _dev(ev.geom.wire_b), _dev(ev.fired_wire),
+                           _dev(ev.hit_off), _dev(ev.rho), ev.cutoff, **kw)
+    torch.cuda.synchronize()
+    assert got["done"].tolist() == ref["done"].tolist() and ref["done"].all()
+    assert got["wires_before"].tolist() == ref["wires_before"].tolist()
+    assert np.array_equal(got["turn_seed"].cpu().numpy(), ref["turn_seed"])
+    assert np.array_equal(got["turn_rss"].cpu().numpy(), ref["turn_rss"])
+    assert np.array_equal(got["turn_cls"].cpu().numpy(), ref["turn_cls"])
