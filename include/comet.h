@@ -83,11 +83,12 @@ int comet_reserve(comet_ctx* ctx, int64_t max_pairs_per_launch);
 int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n, int32_t* n_calls);
 
 /* Copies the work counters accumulated by comet_dca_rss calls made with COMET_OPT_STATS = 1 to
- * out_host[0..n) (HOST, n <= 6) and synchronises the stream; reset != 0 zeroes them afterwards.
+ * out_host[0..n) (HOST, n <= 7) and synchronises the stream; reset != 0 zeroes them afterwards.
  * Counters are thread-level: [0] block/sub-block sample evaluations, [1] row evaluations a lane
  * needed, [2] row evaluations executed (a warp opens a sub-block when any lane needs it),
  * [3] (seed, wire) pairs that needed the virtual-plane iteration, [4] pairs for which a warp
- * executed it, [5] all pairs. */
+ * executed it, [5] all pairs, [6] RKN4 steps of distinct transverse tracks (comet_scan_rss with
+ * COMET_OPT_ZGROUP; 0 otherwise). */
 int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, int32_t reset, void* cuda_stream);
 
 /* ---- inhomogeneous field map and adaptive step (R29-R32) ------- */
