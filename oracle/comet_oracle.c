@@ -20,7 +20,7 @@
  * contraction: every operation below is one IEEE-754 double operation in the
  * order written).
  *
- * Parity pins (tests/test_oracle_pins.py): closed-form helix radius / angular
+ * Parity pins (tests/test_oracle_*_pins.py, tests/test_oracle_golden.py): closed-form helix radius / angular
  * advance / pitch, |T| conservation, straight-line limit, reversibility, axial
  * wire closed form, brute-force dense sampling, rotation / translation / endpoint
  * swap symmetries, truth-seed RSS = injected smearing, RSS bounds, brute-force

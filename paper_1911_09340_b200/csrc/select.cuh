@@ -19,10 +19,11 @@ __device__ __forceinline__ void argmin_merge(double& v, int64_t& i, double v2, i
     if (i2 >= 0 && (i < 0 || v2 < v || (v2 == v && i2 < i))) { v = v2; i = i2; }
 }
 
-// A serial scan keeps the first index whose value is strictly smaller than every earlier one.
-// With NaNs: "rss[s] < rss[b]" is false when either is NaN, so a NaN at the first position stays
-// the winner.  We reproduce that by treating the first element of the partition as the initial
-// winner and merging only strictly smaller values; ties resolve to the lower index.
+// A serial scan "b = lo; for s > lo: if (rss[s] < rss[b]) b = s" keeps the first index whose value is strictly
+// smaller than every earlier one.  With NaNs the comparison is false when either side is NaN: a NaN at the first
+// position of the partition stays the winner whatever follows, a NaN anywhere else never wins.  Reproduced here by
+// skipping NaNs at s > lo and giving a NaN at lo the value -infinity (RSS is a sum of squares: no number is that
+// small); k_select_classify turns it back into the NaN it stands for.
 __global__ void __launch_bounds__(COMET_ARGMIN_THREADS)
 k_argmin_stage1(const double* __restrict__ rss, PartOff po, double* __restrict__ pv, int64_t* __restrict__ pi)
 {
@@ -34,7 +35,11 @@ k_argmin_stage1(const double* __restrict__ rss, PartOff po, double* __restrict__
     double v = 0.0;
     int64_t idx = -1;
     for (int64_t s = b + threadIdx.x; s < e; s += blockDim.x) {
-        const double r = rss[s];
+        double r = rss[s];
+        if (r != r) {
+            if (s != lo) continue;
+            r = -INFINITY;
+        }
         if (idx < 0 || r < v) { v = r; idx = s; }       // increasing s per thread: ties keep lower s
     }
     for (int o = 16; o > 0; o >>= 1) {
@@ -174,7 +179,7 @@ __global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
             argmin_merge(v, idx, a.pv[p * COMET_ARGMIN_SPLIT + b], a.pi[p * COMET_ARGMIN_SPLIT + b]);
         s_best = idx;
         a.best_seed[p] = idx;
-        a.best_rss[p] = (idx >= 0) ? v : __longlong_as_double(0x7ff8000000000000LL);
+        a.best_rss[p] = (idx >= 0 && v != -INFINITY) ? v : __longlong_as_double(0x7ff8000000000000LL);
     }
     __syncthreads();
     classify_cta<FIELD>(a, s_best, a.best_dca + (size_t)p * a.W, a.cls + (size_t)p * a.n_hits, sm);

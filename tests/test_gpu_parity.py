@@ -430,6 +430,38 @@ def test_select_ties_and_empty_partition(comet, cfg0_event):
     assert int(one["best_seed"][0]) == int(bs[0])              # tie between the copies -> lower index
 
 
+def test_select_with_nan_rss_follows_the_serial_rule(comet, cfg0_event):
+    """NaN in RSS (a degenerate seed with |p| = 0): the serial argmin "rss[s] < rss[b]" keeps a NaN at the first
+    position of a partition and never takes one anywhere else.  Positions chosen to hit the first element of a
+    CTA's range, of a thread's stride and interior ones, in partitions long enough for all 64 CTAs of stage 1."""
+    ev = cfg0_event
+    seeds, _ = event_seeds(ev, shape=(16, 8, 8, 8))
+    S = seeds.shape[1]
+    d = DevEvent(ev, seeds)
+    rng = np.random.default_rng(11)
+    rss = rng.uniform(0.1, 1.0, S)
+    part_off = np.array([0, 3000, 3001, S], dtype=np.int64)
+    per = (S - 3001 + 63) // 64
+    for s in (1, 2, 255, 256, 257, 2999, 3001 + per, 3001 + per + 256, 3001 + 5 * per + 3, S - 1):
+        rss[s] = np.nan
+    rss[300] = 0.01                                         # the winner of partition 0 sits behind NaNs of its thread
+    rss[3001 + per + 512] = 0.02                            # and so does the winner of partition 2 (same thread as two NaNs)
+    cases = [rss.copy()]
+    first_nan = rss.copy()
+    first_nan[0] = np.nan                                   # NaN at a partition's first position wins it
+    first_nan[3000] = np.nan                                # one-seed partition holding a NaN
+    cases.append(first_nan)
+    for r in cases:
+        out = comet.select_and_classify(d.seeds, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff,
+                                        torch.from_numpy(r).cuda(), part_off)
+        rs = O.select_classify(seeds, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a,
+                               ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff, r, part_off)
+        np.testing.assert_array_equal(out["best_seed"].cpu().numpy(), rs["best_seed"])
+        np.testing.assert_array_equal(out["best_rss"].cpu().numpy(), rs["best_rss"])
+        np.testing.assert_array_equal(out["cls"].cpu().numpy(), rs["cls"])
+        np.testing.assert_array_equal(out["best_dca"].cpu().numpy(), rs["best_dca"])
+
+
 def test_whole_path_host_buffers(comet, cfg0_event):
     ev = cfg0_event
     seeds, part_off = event_seeds(ev)

@@ -124,6 +124,68 @@ def test_adaptive_step_control(cfg0):
     assert np.all(hs2[~np.isnan(hs2)] == h_max)
 
 
+def test_step_error_estimate_closed_forms():
+    """R31's error estimate EST = h^2 sum_xyz |k1 - k2 - k3 + k4| pinned against numbers that do not come from the
+    oracle's own step: (a) in a uniform field the four slopes of R30 are powers of the rotation generator
+    J T = (T_y, -T_x, 0) applied to T -- k1 = w J T, k2 = k1 + (h/2) w^2 J^2 T, k3 = k2 + (h^2/4) w^3 J^3 T,
+    k4 = k1 + h w^2 J^2 T + (h^2/2) w^3 J^3 T + (h^3/4) w^4 J^4 T, w = cq B_z -- so k1 - k2 - k3 + k4 =
+    (h^2/4) w^3 J^3 T + (h^3/4) w^4 J^4 T with J^2 = -1 in the transverse plane: a closed form in which any other
+    sign pattern of the four slopes leaves a term of order h w^2, four orders of magnitude larger;  (b) in the
+    field B = (0, 0, b0 + g x), which the trilinear map holds exactly, k1..k4 are written out with numpy cross
+    products at the three positions of R30 (start, midpoint with k1, end point with k3)."""
+    # (a) uniform field
+    for (bz, P, q, h, T) in [(1.0, 104.0, -1, 0.5, [0.6, 0.3, 0.2]), (0.8, 60.0, 1, 0.25, [-0.1, 0.9, 0.3]),
+                             (1.2, 95.0, -1, 0.125, [0.7, -0.7, 0.1])]:
+        T = np.array(T) / np.linalg.norm(T)
+        cq = KAPPA * q / P
+        w = cq * bz
+        _, est = O.rkn4_field_step(uniform_map(bz), np.concatenate([[3.0, -2.0, 5.0], T]), h, cq)
+        a, b = h * h * w ** 3 / 4.0, h ** 3 * w ** 4 / 4.0
+        expect = h * h * (abs(-a * T[1] + b * T[0]) + abs(a * T[0] + b * T[1]))
+        assert expect > 0.0
+        np.testing.assert_allclose(est, expect, rtol=1e-7)
+        for signs in [(1, 1, -1, -1), (1, -1, 1, -1), (1, 1, 1, 1), (1, -1, -1, -1), (-1, 1, 1, 1)]:
+            # what a mis-signed combination would give (k's from the closed forms above): far from EST
+            JT = np.array([T[1], -T[0], 0.0]); Tp = np.array([T[0], T[1], 0.0])
+            k1 = w * JT
+            k2 = k1 - (h / 2) * w ** 2 * Tp
+            k3 = k2 - (h * h / 4) * w ** 3 * JT
+            k4 = k1 - h * w ** 2 * Tp - (h * h / 2) * w ** 3 * JT + (h ** 3 / 4) * w ** 4 * Tp
+            wrong = h * h * np.abs(signs[0] * k1 + signs[1] * k2 + signs[2] * k3 + signs[3] * k4).sum()
+            assert abs(wrong - est) > 100.0 * est
+    # (b) linear gradient along x: B_z = b0 + g x (exact under trilinear interpolation)
+    b0, g = 0.9, 0.004
+    d = np.array([8.0, 8.0, 8.0]); o = np.array([-96.0, -96.0, -96.0]); n = 25
+    B = np.zeros((n, n, n, 3))
+    B[..., 2] = (b0 + g * (o[0] + d[0] * np.arange(n)))[:, None, None]
+    F = (B, o, d)
+    bfield = lambda x: np.array([0.0, 0.0, b0 + g * x[0]])
+    rng = np.random.default_rng(5)
+    for _ in range(6):
+        x = rng.uniform(-60.0, 60.0, 3)
+        T = rng.normal(size=3); T /= np.linalg.norm(T)
+        h = float(rng.choice([0.5, 0.25, -0.3]))
+        cq = KAPPA * float(rng.choice([-1, 1])) / rng.uniform(60.0, 110.0)
+        k1 = cq * np.cross(T, bfield(x))
+        bm = bfield(x + h / 2 * T + h * h / 8 * k1)
+        k2 = cq * np.cross(T + h / 2 * k1, bm)
+        k3 = cq * np.cross(T + h / 2 * k2, bm)
+        k4 = cq * np.cross(T + h * k3, bfield(x + h * T + h * h / 2 * k3))
+        s1, est = O.rkn4_field_step(F, np.concatenate([x, T]), h, cq)
+        np.testing.assert_allclose(est, h * h * np.abs(k1 - k2 - k3 + k4).sum(), rtol=1e-6)
+        np.testing.assert_allclose(s1[:3], x + h * T + h * h / 6 * (k1 + k2 + k3), rtol=0, atol=1e-13)
+        np.testing.assert_allclose(s1[3:], T + h / 6 * (k1 + 2 * k2 + 2 * k3 + k4), rtol=0, atol=1e-14)
+    # the gradient shows up in EST at the order the closed form predicts: with T along x and a weak field the
+    # second difference of the acceleration along the step is k1 - 2 k(h/2) + k(h) ~ 0 for a linear B(x), so EST
+    # stays at the uniform-field size, while a kink of the map (a cell face crossed by the step) raises it
+    Bk = B.copy()
+    Bk[n // 2:, :, :, 2] += 0.05 * (d[0] * np.arange(n - n // 2))[:, None, None] / d[0]
+    x0 = np.array([o[0] + d[0] * (n // 2) - 0.2, 1.0, 2.0]); T0 = np.array([1.0, 0.0, 0.0])
+    _, e_lin = O.rkn4_field_step(F, np.concatenate([x0, T0]), 0.5, KAPPA / 100.0)
+    _, e_kink = O.rkn4_field_step((Bk, o, d), np.concatenate([x0, T0]), 0.5, KAPPA / 100.0)
+    assert e_kink > 20.0 * e_lin
+
+
 def test_field_dca_against_dense_sampling(cfg0):
     ev, seeds = cfg0
     F = solenoid_map()
