@@ -12,11 +12,12 @@ Units: cm, MeV/c, Tesla, charge in units of e.
 from .geometry import cdc_geometry, CDCGeometry
 from .helix import Helix, KAPPA
 from .events import (Event, Partition, make_event, make_config, config_spec,
-                     seed_grid, event_seeds, truth_seed, CONFIG_SPECS)
+                     seed_grid, event_seeds, truth_seed, CONFIG_SPECS,
+                     seed_axes, pack_axes, grid_from_axes, event_axes)
 from .fieldmap import solenoid_map, uniform_map, hough_tables
 
 __all__ = [
     "cdc_geometry", "CDCGeometry", "Helix", "KAPPA", "Event", "Partition",
-    "make_event", "make_config", "config_spec", "seed_grid", "event_seeds",
+    "make_event", "make_config", "config_spec", "seed_grid", "event_seeds", "seed_axes", "pack_axes", "grid_from_axes", "event_axes",
     "truth_seed", "CONFIG_SPECS", "solenoid_map", "uniform_map", "hough_tables",
 ]

@@ -290,33 +290,70 @@ def truth_seed(ev: Event, part: int) -> np.ndarray:
     return np.concatenate([pt.x_in, ev.pmag * pt.T_in])
 
 
-def seed_grid(ev: Event, part: int, shape: Sequence[int], p_range: Tuple[float, float],
+def seed_axes(ev: Event, part: int, shape: Sequence[int], p_range: Tuple[float, float],
               ct_range: Optional[Tuple[float, float]] = None, ct_hw: float = 0.15,
-              phi_hw: float = 0.04, z_hw: float = 4.0) -> np.ndarray:
-    """SoA seeds [6][S] for one partition (reading R17).
-
-    Axes are inclusive linspaces: |p| over p_range; cos theta over ct_range or
-    truth +- ct_hw; phi0 over truth +- phi_hw; z0 over truth +- z_hw.
-    """
+              phi_hw: float = 0.04, z_hw: float = 4.0) -> dict:
+    """The axis tables of one partition's seed grid (readings R17, R44): inclusive linspaces of
+    |p| over p_range, cos theta over ct_range or truth +- ct_hw, phi0 over truth +- phi_hw, z0 over truth +- z_hw,
+    with the tables derived from them (sin theta, cos phi0, sin phi0) and the seed point (x, y) on r = 50 cm."""
     pt = ev.partitions[part]
     n_p, n_ct, n_phi, n_z = (int(v) for v in shape)
-    pa = np.linspace(p_range[0], p_range[1], n_p)
     if ct_range is None:
         ct_range = (pt.cos_theta - ct_hw, pt.cos_theta + ct_hw)
     ca = np.linspace(ct_range[0], ct_range[1], n_ct)
     fa = np.linspace(pt.phi - phi_hw, pt.phi + phi_hw, n_phi)
-    za = np.linspace(pt.z - z_hw, pt.z + z_hw, n_z)
-    P, C, F, Z = np.meshgrid(pa, ca, fa, za, indexing="ij")
-    P, C, F, Z = P.ravel(), C.ravel(), F.ravel(), Z.ravel()
-    S = np.sqrt(1.0 - C * C)
+    return {"xy": np.array([R_SEED * np.cos(pt.theta_e), R_SEED * np.sin(pt.theta_e)]),
+            "p": np.linspace(p_range[0], p_range[1], n_p),
+            "sin_theta": np.sqrt(1.0 - ca * ca), "cos_theta": ca,
+            "cos_phi": np.cos(fa), "sin_phi": np.sin(fa),
+            "z": np.linspace(pt.z - z_hw, pt.z + z_hw, n_z)}
+
+
+def pack_axes(ax: dict) -> np.ndarray:
+    """The layout of comet_seed_grid's `axes` argument (include/comet.h):
+    x, y | p | sin theta | cos theta | cos phi0 | sin phi0 | z0."""
+    return np.concatenate([ax["xy"], ax["p"], ax["sin_theta"], ax["cos_theta"], ax["cos_phi"], ax["sin_phi"], ax["z"]])
+
+
+def grid_from_axes(ax: dict) -> np.ndarray:
+    """SoA seeds [6][S] from the axis tables: index ((i_p n_ct + i_ct) n_phi + i_phi) n_z + i_z (z fastest),
+    p_x = (|p| sin theta) cos phi0, p_y = (|p| sin theta) sin phi0, p_z = |p| cos theta (one multiplication each,
+    in this order)."""
+    ip, ic, jf, iz = np.meshgrid(np.arange(ax["p"].size), np.arange(ax["cos_theta"].size),
+                                 np.arange(ax["cos_phi"].size), np.arange(ax["z"].size), indexing="ij")
+    ip, ic, jf, iz = ip.ravel(), ic.ravel(), jf.ravel(), iz.ravel()
+    P = ax["p"][ip]
+    PS = P * ax["sin_theta"][ic]
     seeds = np.empty((6, P.size))
-    seeds[0] = R_SEED * np.cos(pt.theta_e)
-    seeds[1] = R_SEED * np.sin(pt.theta_e)
-    seeds[2] = Z
-    seeds[3] = P * S * np.cos(F)
-    seeds[4] = P * S * np.sin(F)
-    seeds[5] = P * C
+    seeds[0] = ax["xy"][0]
+    seeds[1] = ax["xy"][1]
+    seeds[2] = ax["z"][iz]
+    seeds[3] = PS * ax["cos_phi"][jf]
+    seeds[4] = PS * ax["sin_phi"][jf]
+    seeds[5] = P * ax["cos_theta"][ic]
     return seeds
+
+
+def seed_grid(ev: Event, part: int, shape: Sequence[int], p_range: Tuple[float, float],
+              ct_range: Optional[Tuple[float, float]] = None, ct_hw: float = 0.15,
+              phi_hw: float = 0.04, z_hw: float = 4.0) -> np.ndarray:
+    """SoA seeds [6][S] for one partition (reading R17): the grid of seed_axes."""
+    return grid_from_axes(seed_axes(ev, part, shape, p_range, ct_range, ct_hw, phi_hw, z_hw))
+
+
+def _grid_args(ev: Event, shape):
+    sp = ev.spec
+    shape = tuple(shape or sp["grid"])
+    p_range = tuple(sp["p_range"]) if "p_range" in sp else (ev.pmag - sp["p_hw"], ev.pmag + sp["p_hw"])
+    return shape, p_range, sp.get("ct_range"), sp.get("ct_hw", 0.15)
+
+
+def event_axes(ev: Event, shape: Optional[Sequence[int]] = None):
+    """The axes of all partitions' grids: (axes [P][A] as comet_seed_grid takes them, shape, part_off [P+1])."""
+    shape, p_range, ct_range, ct_hw = _grid_args(ev, shape)
+    rows = [pack_axes(seed_axes(ev, i, shape, p_range, ct_range=ct_range, ct_hw=ct_hw)) for i in range(len(ev.partitions))]
+    G = int(np.prod(shape))
+    return np.ascontiguousarray(np.stack(rows)), shape, np.arange(len(rows) + 1, dtype=np.int64) * G
 
 
 def event_seeds(ev: Event, shape: Optional[Sequence[int]] = None):

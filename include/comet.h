@@ -11,7 +11,11 @@
  *     the work enqueued on `cuda_stream` has completed.  "host" pointers are ordinary host
  *     memory read or written before the call returns unless stated otherwise.
  *   - `cuda_stream` is a cudaStream_t cast to void* (NULL = the legacy default stream).
- *     The device-buffer calls only enqueue work: no host synchronisation, no allocation.
+ *     The device-buffer calls only enqueue work: no host synchronisation, and no allocation once the
+ *     ctx's workspace has been sized (comet_reserve_scan / comet_reserve; a call that finds it too small
+ *     grows it -- that call synchronises the device -- unless the stream is being captured into a CUDA
+ *     graph, where it returns COMET_ENOMEM instead).  The entry points that say so (the turn loops, the
+ *     host-buffer calls, comet_seed_runs) synchronise the stream.
  *   - A comet_ctx owns a small device workspace; use one ctx per stream.  Calls on different
  *     ctx objects / streams are independent.
  *   - There is no CPU implementation behind this interface.
@@ -74,6 +78,15 @@ int comet_get_option(const comet_ctx* ctx, int option, int* value);
  * call the workspace grows on the first comet_dca_rss that needs it (that call synchronises the
  * device). */
 int comet_reserve(comet_ctx* ctx, int64_t max_pairs_per_launch);
+
+/* Sizes every workspace comet_scan_rss (and the calls built on it: comet_scan_stage, comet_scan_turns, the
+ * half-track calls) needs for seed sets of up to n_seeds seeds, n_steps steps and n_fired fired wires --
+ * (seed, wire) pair keys, checkpoints, per-seed constants, the distinct-track rows of the z-run kernels --
+ * under the current options and field mode, so that those calls never allocate or synchronise afterwards
+ * (they can then be captured into a CUDA graph from the first call on).  Larger problems than comet_reserve's
+ * pair limit or 8 GiB of checkpoints allow are processed in seed slabs of that size.  Synchronises the device
+ * when it reallocates. */
+int comet_reserve_scan(comet_ctx* ctx, int64_t n_seeds, int32_t n_steps, int32_t n_fired);
 
 /* With COMET_OPT_TIMING = 1 the pruned comet_dca_rss records CUDA events on its stream around its
  * three kernels (once per seed slab).  Waits for the timed slabs and writes the mean device time in
@@ -178,8 +191,8 @@ int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64
  * Arguments as in the two calls above;
  *   n_pts   dev [n_seeds], written; NULL to skip.
  * Workspace (checkpoints: 12 bytes per recorded state of capacity; 8 bytes per (seed, wire) pair;
- * 8 bytes per seed) lives in the ctx and grows on the first call that needs it (that call
- * synchronises the device); larger problems are processed in seed slabs bounded by comet_reserve's
+ * 8 bytes per seed) lives in the ctx: sized by comet_reserve_scan, else grown on the first call that
+ * needs it (that call synchronises the device; COMET_ENOMEM while the stream is being captured); larger problems are processed in seed slabs bounded by comet_reserve's
  * pair limit and by 8 GiB of checkpoints.  A slab is cut into up to COMET_OPT_LANES sub-slabs that
  * run concurrently on streams owned by the ctx; `cuda_stream` forks into them and joins them again
  * with events, so the call is asynchronous with respect to the host and ordered on `cuda_stream`
@@ -196,8 +209,15 @@ int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n_pts, int64
  * uniform in those components (found on the device; the seed grids of the method with z as the
  * fastest axis are), the RKN4 steps are taken once per distinct transverse track and every seed
  * adds its own z column; rss and n_pts are the same numbers either way.  Calls of fewer than 1024
- * chunks (32768 seeds) always take the plain kernels. */
-int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+ * chunks (32768 seeds) always take the plain kernels.
+ *   z_run   what the caller knows about the seeds: 0 = nothing (the run length is found on the device: one
+ *           small kernel per sub-slab, and both kernel variants are enqueued, the one that does not serve
+ *           the launch returns at once); 8, 16, 32, ... (a power of two) = a promise that every aligned run
+ *           of min(z_run, 32) consecutive seeds, counted from seeds[0], is bit-identical in (x, y, p_x, p_y,
+ *           p_z) -- comet_seed_grid's output with z_run = comet_grid_z_run(n_z), or what comet_seed_runs
+ *           found; a false promise gives wrong results, it is not checked; 1 = no runs: plain kernels.
+ * Workspace: see comet_reserve_scan. */
+int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
                    int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                    const double* wire_a, const double* wire_b, int32_t n_wires,
                    const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
@@ -282,8 +302,9 @@ size_t comet_stage_work_bytes(int64_t n_seeds, int32_t n_part, int32_t k_ref, in
  *   final_dca   dev [n_part][k_final][n_fired], cls dev [n_part][k_final][n_hits]
  *   part_off    HOST [n_part+1], part_off[0] = 0, part_off[n_part] = n_seeds, no empty partition
  *   work        dev, comet_stage_work_bytes(...) bytes
+ *   z_run       the caller's knowledge about `seeds` as in comet_scan_rss (iteration 0 only)
  * Only enqueues work on cuda_stream (plus the ctx's internal streams, see comet_scan_rss). */
-int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
                      int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                      const double* wire_a, const double* wire_b, int32_t n_wires,
                      const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
@@ -323,9 +344,10 @@ size_t comet_turns_work_bytes(int64_t max_partition_seeds, int32_t n_fired, int3
  *   turn_cls    dev [n_part][n_hits]: the hits given to each turn, in the event's own entry numbering
  *   done_host, wires_before_host  HOST [n_part]: 1 where a stage ran; fired wires it started with
  *   work        dev, comet_turns_work_bytes(largest partition, n_fired, n_hits, k_ref, n_grid)
+ *   z_run       as in comet_scan_rss, used for the partitions that start on a run
  * Synchronises cuda_stream once per stage (the size of the reduced hit list sets the next launches),
  * as the paper's host loop does. */
-int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
                      int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                      const double* wire_a, const double* wire_b, int32_t n_wires,
                      const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
@@ -476,6 +498,39 @@ int comet_scan_turns_half(comet_ctx* ctx, const double* seeds_ent, const int64_t
                           int32_t* turn_pair, int32_t* turn_n, double* turn_seed, uint8_t* turn_cls,
                           int32_t* done_host, int32_t* wires_before_host, void* cuda_stream);
 
+/* ---- seed grids as inputs (readings R17, R44) --------------------------------- */
+
+/* "A seed set was prepared by combining each component from the grids of the ranges":
+ * the first-iteration seed set of n_part turn partitions built on the device from its axes instead of
+ * 6 x S doubles crossing the bus.  axes is [n_part][A] doubles, A = comet_grid_axes_len(...) =
+ * 2 + n_p + 2 n_ct + 2 n_phi + n_z, per partition:
+ *   x, y (the seed point on the r = 50 cm cylinder) | |p| [n_p] | sin(theta) [n_ct] |
+ *   cos(theta) [n_ct] | cos(phi0) [n_phi] | sin(phi0) [n_phi] | z0 [n_z]
+ * (tables: no transcendental function is evaluated by the library).  Seed ((i_p n_ct + i_ct) n_phi +
+ * i_phi) n_z + i_z of partition q, at index q G + that, G = n_p n_ct n_phi n_z (R17), is
+ *   (x, y, z0[i_z], (|p| sin) cos(phi0), (|p| sin) sin(phi0), |p| cos(theta))
+ * each product one IEEE multiplication in the order written (R44).
+ *   axes    dev [n_part][A];  seeds  dev SoA [6][seed_stride], seed_stride >= n_part G, written
+ * z is the fastest index, so comet_grid_z_run(n_z) -- the largest power of two <= 32 dividing n_z -- is a
+ * valid z_run promise for scans of this set (and of any partition of it). */
+int comet_seed_grid(comet_ctx* ctx, const double* axes, int32_t n_part, int32_t n_p, int32_t n_ct,
+                    int32_t n_phi, int32_t n_z, double* seeds, int64_t seed_stride, void* cuda_stream);
+size_t comet_grid_axes_len(int32_t n_p, int32_t n_ct, int32_t n_phi, int32_t n_z);   /* 0 for invalid shapes */
+int32_t comet_grid_z_run(int32_t n_z);
+
+/* The z_run of an arbitrary seed set: the largest power of two r <= 32 such that every aligned run of r
+ * consecutive seeds is bit-identical in (x, y, p_x, p_y, p_z), written to *z_run_host (HOST).  One small
+ * kernel; synchronises cuda_stream (a query made once per seed set, not in the hot loop). */
+int comet_seed_runs(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                    int32_t* z_run_host, void* cuda_stream);
+
+/* Keeps a copy of the detector's wire endpoints (HOST SoA [3][n_wires] each) on the device for the host-buffer
+ * entry points below (the geometry is a constant of the detector, not an input of an event).  Synchronises
+ * cuda_stream; n_wires = 0 frees the copy.  comet_get_geometry returns the device pointers (NULL when none). */
+int comet_set_geometry(comet_ctx* ctx, const double* wire_a_host, const double* wire_b_host, int32_t n_wires,
+                       void* cuda_stream);
+int comet_get_geometry(const comet_ctx* ctx, const double** wire_a_dev, const double** wire_b_dev, int32_t* n_wires);
+
 /* ---- whole event from host buffers ------------------------------------------------------- */
 
 /* Runs A, B and C for one event whose inputs and outputs live in HOST memory (pinned memory makes
@@ -484,7 +539,8 @@ int comet_scan_turns_half(comet_ctx* ctx, const double* seeds_ent, const int64_t
  * streams, so the upload overlaps the kernels of the sub-slabs already on the device --, else comet_seed_extrapolate + comet_dca_rss over slabs of seeds that fit
  * `track_budget_bytes` of track workspace (grown inside the ctx when needed), copies
  * best_seed/best_rss/best_dca/cls (and rss if rss_host != NULL) back and synchronises the stream.
- * All array arguments have the shapes of the device-buffer calls above. */
+ * All array arguments have the shapes of the device-buffer calls above.  wire_a_host = wire_b_host = NULL
+ * uses the geometry of comet_set_geometry (n_wires is then ignored). */
 int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, int64_t n_seeds,
                           int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
                           double r_stop_cm,
@@ -494,6 +550,20 @@ int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, int64_t n_se
                           const int64_t* part_off_host, int32_t n_part, size_t track_budget_bytes,
                           int64_t* best_seed_host, double* best_rss_host, double* best_dca_host,
                           uint8_t* cls_host, double* rss_host, void* cuda_stream);
+
+/* The same event with its seed sets given as grid axes (comet_seed_grid; HOST [n_part][A]) and the geometry
+ * of comet_set_geometry: per event only the axes, the fired wires and the hit entries cross the bus (a few
+ * KB).  Copies them in, builds the seeds on the device, runs comet_scan_rss with z_run =
+ * comet_grid_z_run(n_z) and comet_select_and_classify with part_off[q] = q G, copies best_seed / best_rss /
+ * best_dca / cls (and rss [n_part G] if rss_host != NULL) back and synchronises the stream. */
+int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_host, int32_t n_part, int32_t n_p,
+                               int32_t n_ct, int32_t n_phi, int32_t n_z,
+                               int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                               double r_stop_cm,
+                               const int32_t* fired_wire_host, const int32_t* hit_off_host,
+                               const double* rho_host, int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                               int64_t* best_seed_host, double* best_rss_host, double* best_dca_host,
+                               uint8_t* cls_host, double* rss_host, void* cuda_stream);
 
 /* ---- measurement helper ------------------------------------------------------------------ */
 

@@ -23,6 +23,8 @@ EXPORTED_SYMBOLS = [
     "comet_hough_work_bytes", "comet_hough_seeds", "comet_half_hit_masks", "comet_flip_seeds", "comet_layer_veto",
     "comet_merge_half_sets", "comet_half_work_bytes", "comet_scan_half_tracks",
     "comet_turns_half_work_bytes", "comet_scan_turns_half",
+    "comet_reserve_scan", "comet_seed_grid", "comet_grid_axes_len", "comet_grid_z_run", "comet_seed_runs",
+    "comet_set_geometry", "comet_get_geometry", "comet_scan_event_grid_host",
 ]
 
 COMET_CHUNK = 32
@@ -71,7 +73,7 @@ def load_library():
     L.comet_track_export.argtypes = [vp, vp, vp, i64, i32, i64, i64, vp, vp]
     L.comet_dca_rss.argtypes = [vp, vp, vp, i64, i32, i32, dbl, dbl, vp, i64,
                                 vp, vp, i32, vp, vp, vp, i32, i32, dbl, vp, vp, vp, vp]
-    L.comet_scan_rss.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
+    L.comet_scan_rss.argtypes = [vp, vp, i64, i64, i32, i32, dbl, dbl, i32, dbl,
                                  vp, vp, i32, vp, vp, vp, i32, i32, dbl, vp, vp, vp]
     L.comet_select_and_classify.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
                                             vp, vp, i32, vp, vp, vp, i32, i32, dbl,
@@ -86,7 +88,7 @@ def load_library():
     L.comet_remove_hits.argtypes = [vp, vp, vp, vp, i32, i32, vp, vp, vp, vp, vp, vp, vp, vp]
     L.comet_turns_work_bytes.argtypes = [i64, i32, i32, i32, vp]
     L.comet_turns_work_bytes.restype = sz
-    L.comet_scan_turns.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
+    L.comet_scan_turns.argtypes = [vp, vp, i64, i64, i32, i32, dbl, dbl, i32, dbl,
                                    vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                    vp, i32, vp, vp, i32, dbl, i32, i32, i32, vp, vp, vp, vp, vp, vp, vp]
     L.comet_hough_work_bytes.argtypes = [i32]
@@ -116,12 +118,23 @@ def load_library():
                                        vp, vp, i32, vp, vp, vp, i32, i32, dbl, vp, i32, vp, vp, vp]
     L.comet_stage_work_bytes.argtypes = [i64, i32, i32, i32, vp]
     L.comet_stage_work_bytes.restype = sz
-    L.comet_scan_stage.argtypes = [vp, vp, i64, i64, i32, dbl, dbl, i32, dbl,
+    L.comet_scan_stage.argtypes = [vp, vp, i64, i64, i32, i32, dbl, dbl, i32, dbl,
                                    vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                    vp, i32, vp, vp, i32, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
+    L.comet_reserve_scan.argtypes = [vp, i64, i32, i32]
+    L.comet_seed_grid.argtypes = [vp, vp, i32, i32, i32, i32, i32, vp, i64, vp]
+    L.comet_grid_axes_len.argtypes = [i32, i32, i32, i32]
+    L.comet_grid_axes_len.restype = sz
+    L.comet_grid_z_run.argtypes = [i32]
+    L.comet_grid_z_run.restype = i32
+    L.comet_seed_runs.argtypes = [vp, vp, i64, i64, ctypes.POINTER(i32), vp]
+    L.comet_set_geometry.argtypes = [vp, vp, vp, i32, vp]
+    L.comet_get_geometry.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i32)]
+    L.comet_scan_event_grid_host.argtypes = [vp, vp, i32, i32, i32, i32, i32, i32, dbl, dbl, i32, dbl,
+                                             vp, vp, vp, i32, i32, dbl, vp, vp, vp, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes", "comet_turns_work_bytes",
-                        "comet_hough_work_bytes", "comet_half_work_bytes",
+                        "comet_hough_work_bytes", "comet_half_work_bytes", "comet_grid_axes_len", "comet_grid_z_run",
                         "comet_turns_half_work_bytes"):
             getattr(L, name).restype = ctypes.c_int
     _lib = L
@@ -204,6 +217,10 @@ class Comet:
         """Pre-allocates the pruned search's (seed, wire) pair workspace (12 bytes per pair)."""
         self._check(self._L.comet_reserve(self._h, int(max_pairs_per_launch)))
 
+    def reserve_scan(self, n_seeds: int, n_steps: int, n_fired: int):
+        """comet_reserve_scan: sizes every workspace of comet_scan_rss & co.; later calls do not allocate."""
+        self._check(self._L.comet_reserve_scan(self._h, int(n_seeds), int(n_steps), int(n_fired)))
+
     def read_timing(self, names=("k_coarse_pruned", "k_fine", "k_rss_sum")) -> dict:
         """Mean device milliseconds per kernel of the latest (<= 64) seed slabs of comet_dca_rss (pruned:
         k_coarse_pruned, k_fine, k_rss_sum) or comet_scan_rss (k_scan_fused, k_fine_ck, k_rss_sum) made
@@ -284,7 +301,7 @@ class Comet:
 
     # -- kernels A + B fused, track on chip ---------------------------------------------------
     def scan_rss(self, seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
-                 cutoff, rss=None, n_pts=None, want_npts=True, seed_range=None, stream=None):
+                 cutoff, rss=None, n_pts=None, want_npts=True, seed_range=None, stream=None, z_run=0):
         """comet_scan_rss: RSS (and n_pts) of seeds[:, b:e] without a track buffer."""
         S = seeds.shape[1]
         b, e = (0, S) if seed_range is None else seed_range
@@ -296,7 +313,7 @@ class Comet:
         if n_pts is None and want_npts:
             n_pts = torch.empty(n, dtype=torch.int32, device=self._tdev())
         self._check(self._L.comet_scan_rss(
-            self._h, _dev(seeds, torch.float64, "seeds", d) + 8 * b, S, n, int(charge), float(bz), float(step),
+            self._h, _dev(seeds, torch.float64, "seeds", d) + 8 * b, S, n, int(z_run), int(charge), float(bz), float(step),
             int(n_steps), float(r_stop),
             _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
             int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d),
@@ -374,7 +391,7 @@ class Comet:
         return int(self._L.comet_stage_work_bytes(int(n_seeds), int(n_part), int(k_ref), int(k_final), ng.ctypes.data))
 
     def scan_stage(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off,
-                   rho, cutoff, half_width, n_grid, n_iter, shrink, k_ref, k_final, work=None, stream=None):
+                   rho, cutoff, half_width, n_grid, n_iter, shrink, k_ref, k_final, work=None, stream=None, z_run=0):
         """comet_scan_stage: a whole stage (scan, n_iter refinements, final selection, classification)."""
         S = seeds.shape[1]
         po = np.ascontiguousarray(np.asarray(part_off, dtype=np.int64))
@@ -392,7 +409,7 @@ class Comet:
                "final_dca": torch.empty((P, int(k_final), W), dtype=torch.float64, device=td),
                "cls": torch.empty((P, int(k_final), H), dtype=torch.uint8, device=td), "work": work}
         self._check(self._L.comet_scan_stage(
-            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, int(charge), float(bz), float(step),
+            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, int(z_run), int(charge), float(bz), float(step),
             int(n_steps), float(r_stop),
             _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
             int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d),
@@ -421,7 +438,8 @@ class Comet:
         return {"fired_wire": fo[:nw], "hit_off": ho[:nw + 1], "rho": ro[:nh], "orig": oo[:nh], "counts": (nw, nh)}
 
     def scan_turns(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off,
-                   rho, cutoff, half_width, n_grid, n_iter, shrink, k_ref, min_wires=30, max_tracks=5, stream=None):
+                   rho, cutoff, half_width, n_grid, n_iter, shrink, k_ref, min_wires=30, max_tracks=5, stream=None,
+                   z_run=0):
         """comet_scan_turns: the last turn first, hits of a stage's best seed removed before the previous turn."""
         S = seeds.shape[1]
         po = np.ascontiguousarray(np.asarray(part_off, dtype=np.int64))
@@ -439,7 +457,7 @@ class Comet:
         done = np.zeros(P, dtype=np.int32)
         wb = np.zeros(P, dtype=np.int32)
         self._check(self._L.comet_scan_turns(
-            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, int(charge), float(bz), float(step),
+            self._h, _dev(seeds, torch.float64, "seeds", d), S, S, int(z_run), int(charge), float(bz), float(step),
             int(n_steps), float(r_stop),
             _dev(wire_a, torch.float64, "wire_a", d), _dev(wire_b, torch.float64, "wire_b", d),
             int(wire_a.shape[1]), _dev(fired_wire, torch.int32, "fired_wire", d),
@@ -600,7 +618,7 @@ class Comet:
     # -- whole event, device-resident inputs --------------------------------------------------
     def scan_event(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
                    hit_off, rho, cutoff, track=None, n_pts=None, rss=None, slab_seeds=None, stream=None,
-                   fused=True):
+                   fused=True, z_run=0):
         """A, B and C.  fused=True (default): comet_scan_rss, the track stays on chip.  fused=False:
         comet_seed_extrapolate + comet_dca_rss through a track buffer in HBM (per slab of seeds when
         the buffer is smaller than the whole set)."""
@@ -611,7 +629,7 @@ class Comet:
             if n_pts is None:
                 n_pts = torch.empty(S, dtype=torch.int32, device=self._tdev())
             self.scan_rss(seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off, rho,
-                          cutoff, rss=rss, n_pts=n_pts, stream=stream)
+                          cutoff, rss=rss, n_pts=n_pts, stream=stream, z_run=z_run)
             out = self.select_and_classify(seeds, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire,
                                            hit_off, rho, cutoff, rss, part_off, stream=stream)
             out["rss"] = rss
@@ -647,7 +665,9 @@ class Comet:
             if t.is_cuda or t.dtype != dt or not t.is_contiguous():
                 raise CometError("host array must be a contiguous CPU tensor of dtype %s" % dt)
             return t
-        seeds, wire_a, wire_b = host(seeds, torch.float64), host(wire_a, torch.float64), host(wire_b, torch.float64)
+        seeds = host(seeds, torch.float64)
+        if wire_a is not None:                               # None: the geometry of set_geometry
+            wire_a, wire_b = host(wire_a, torch.float64), host(wire_b, torch.float64)
         fired_wire, hit_off, rho = host(fired_wire, torch.int32), host(hit_off, torch.int32), host(rho, torch.float64)
         po = host(np.asarray(part_off, dtype=np.int64) if not isinstance(part_off, torch.Tensor) else part_off,
                   torch.int64)
@@ -662,8 +682,69 @@ class Comet:
         rss_ptr = out["rss"].data_ptr() if "rss" in out else 0
         self._check(self._L.comet_scan_event_host(
             self._h, seeds.data_ptr(), S, int(charge), float(bz), float(step), int(n_steps), float(r_stop),
-            wire_a.data_ptr(), wire_b.data_ptr(), int(wire_a.shape[1]), fired_wire.data_ptr(), hit_off.data_ptr(),
+            wire_a.data_ptr() if wire_a is not None else 0, wire_b.data_ptr() if wire_a is not None else 0,
+            int(wire_a.shape[1]) if wire_a is not None else 0, fired_wire.data_ptr(), hit_off.data_ptr(),
             rho.data_ptr(), W, H, float(cutoff), po.data_ptr(), P, int(track_budget_bytes),
+            out["best_seed"].data_ptr(), out["best_rss"].data_ptr(), out["best_dca"].data_ptr(),
+            out["cls"].data_ptr(), rss_ptr, _stream_ptr(stream)))
+        return out
+
+    # -- seed grids as inputs -------------------------------------------------------------------
+    def grid_z_run(self, n_z: int) -> int:
+        return int(self._L.comet_grid_z_run(int(n_z)))
+
+    def seed_grid(self, axes, shape, seeds=None, stream=None):
+        """comet_seed_grid: axes CUDA float64 [P][A], shape = (n_p, n_ct, n_phi, n_z) -> seeds [6][P G] (device)."""
+        n_p, n_ct, n_phi, n_z = (int(v) for v in shape)
+        A = int(self._L.comet_grid_axes_len(n_p, n_ct, n_phi, n_z))
+        if A == 0 or axes.dim() != 2 or axes.shape[1] != A:
+            raise CometError("axes must be [n_part][%d] for this grid shape" % A)
+        P = int(axes.shape[0])
+        S = P * n_p * n_ct * n_phi * n_z
+        if seeds is None:
+            seeds = torch.empty((6, S), dtype=torch.float64, device=self._tdev())
+        self._check(self._L.comet_seed_grid(self._h, _dev(axes, torch.float64, "axes", self.device), P, n_p, n_ct, n_phi,
+                                            n_z, _dev(seeds, torch.float64, "seeds", self.device), int(seeds.shape[1]),
+                                            _stream_ptr(stream)))
+        return seeds
+
+    def seed_runs(self, seeds, stream=None) -> int:
+        """comet_seed_runs: the z_run of a seed set (synchronises)."""
+        v = ctypes.c_int32()
+        self._check(self._L.comet_seed_runs(self._h, _dev(seeds, torch.float64, "seeds", self.device), int(seeds.shape[1]),
+                                            int(seeds.shape[1]), ctypes.byref(v), _stream_ptr(stream)))
+        return int(v.value)
+
+    def set_geometry(self, wire_a, wire_b, stream=None):
+        """comet_set_geometry: HOST arrays [3][n_wires]; returns the device copies as CUDA tensors' addresses."""
+        wa = torch.from_numpy(np.ascontiguousarray(np.asarray(wire_a, dtype=np.float64)))
+        wb = torch.from_numpy(np.ascontiguousarray(np.asarray(wire_b, dtype=np.float64)))
+        self._check(self._L.comet_set_geometry(self._h, wa.data_ptr(), wb.data_ptr(), int(wa.shape[1]), _stream_ptr(stream)))
+
+    def scan_event_grid_host(self, axes, shape, charge, bz, step, n_steps, r_stop, fired_wire, hit_off, rho, cutoff,
+                             out=None, want_rss=False, stream=None):
+        """comet_scan_event_grid_host: axes HOST [P][A] (pinned for asynchronous copies), the event's hits HOST."""
+        def host(a, dt):
+            t = a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a))
+            if t.is_cuda or t.dtype != dt or not t.is_contiguous():
+                raise CometError("host array must be a contiguous CPU tensor of dtype %s" % dt)
+            return t
+        axes = host(axes, torch.float64)
+        fired_wire, hit_off, rho = host(fired_wire, torch.int32), host(hit_off, torch.int32), host(rho, torch.float64)
+        n_p, n_ct, n_phi, n_z = (int(v) for v in shape)
+        P, W, H = int(axes.shape[0]), int(fired_wire.shape[0]), int(rho.shape[0])
+        S = P * n_p * n_ct * n_phi * n_z
+        if out is None:
+            out = {"best_seed": torch.empty(P, dtype=torch.int64).pin_memory(),
+                   "best_rss": torch.empty(P, dtype=torch.float64).pin_memory(),
+                   "best_dca": torch.empty((P, W), dtype=torch.float64).pin_memory(),
+                   "cls": torch.empty((P, H), dtype=torch.uint8).pin_memory()}
+            if want_rss:
+                out["rss"] = torch.empty(S, dtype=torch.float64).pin_memory()
+        rss_ptr = out["rss"].data_ptr() if "rss" in out else 0
+        self._check(self._L.comet_scan_event_grid_host(
+            self._h, axes.data_ptr(), P, n_p, n_ct, n_phi, n_z, int(charge), float(bz), float(step), int(n_steps),
+            float(r_stop), fired_wire.data_ptr(), hit_off.data_ptr(), rho.data_ptr(), W, H, float(cutoff),
             out["best_seed"].data_ptr(), out["best_rss"].data_ptr(), out["best_dca"].data_ptr(),
             out["cls"].data_ptr(), rss_ptr, _stream_ptr(stream)))
         return out
@@ -678,41 +759,3 @@ class Comet:
         self._check(self._L.comet_fp64_peak_probe(self._h, int(iters), int(sink.data_ptr()), ctypes.byref(n),
                                                   _stream_ptr(stream)))
         return n.value
-
-
-_default = {}
-
-
-def _ctx(device=None) -> Comet:
-    device = torch.cuda.current_device() if device is None else int(device)
-    if device not in _default:
-        _default[device] = Comet(device)
-    return _default[device]
-
-
-def seed_extrapolate(seeds, *a, **k):
-    return _ctx(seeds.device.index).seed_extrapolate(seeds, *a, **k)
-
-
-def track_export(track, *a, **k):
-    return _ctx(track.device.index).track_export(track, *a, **k)
-
-
-def dca_rss(track, *a, **k):
-    return _ctx(track.device.index).dca_rss(track, *a, **k)
-
-
-def select_and_classify(seeds, *a, **k):
-    return _ctx(seeds.device.index).select_and_classify(seeds, *a, **k)
-
-
-def scan_rss(seeds, *a, **k):
-    return _ctx(seeds.device.index).scan_rss(seeds, *a, **k)
-
-
-def scan_event(seeds, *a, **k):
-    return _ctx(seeds.device.index).scan_event(seeds, *a, **k)
-
-
-def scan_event_host(*a, **k):
-    return _ctx().scan_event_host(*a, **k)

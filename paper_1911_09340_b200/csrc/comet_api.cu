@@ -19,6 +19,7 @@
 #include "turns.cuh"
 #include "hough.cuh"
 #include "half.cuh"
+#include "seedgrid.cuh"
 
 #ifndef COMET_PRUNED_WT
 #define COMET_PRUNED_WT 3
@@ -90,6 +91,10 @@ struct comet_ctx {
     size_t hbuf_bytes;
     void* tbuf;            // track slab
     size_t tbuf_bytes;
+    // detector geometry kept on the device for the host-buffer entry points (comet_set_geometry)
+    double* geom_a;
+    double* geom_b;
+    int32_t geom_n;
 };
 
 #define CU(ctx, call)                                  \
@@ -156,7 +161,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int) * COMET_MAX_LANES);
     ctx->opt_lanes = COMET_DEFAULT_LANES;
     ctx->opt_zgroup = 1;
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->zg_flag, sizeof(unsigned int) * COMET_MAX_LANES);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->zg_flag, sizeof(unsigned int) * (COMET_MAX_LANES + 1));
     {
         ctx->zg_smem = ((COMET_FUSED_WFIELDS + 1) * COMET_FUSED_WCAP + COMET_FUSED_WARPS * COMET_ZG_WTILE) * (int)sizeof(double);
         const void* zk[2] = {(const void*)k_scan_fused<false, false, true>, (const void*)k_scan_fused<true, false, true>};
@@ -222,6 +227,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ub); cudaFree(ctx->npu);
     for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
+    cudaFree(ctx->geom_a); cudaFree(ctx->geom_b);
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->tw); cudaFree(ctx->bmax);
     for (int l = 0; l < COMET_MAX_LANES; ++l) {
         if (ctx->ls[l]) cudaStreamDestroy(ctx->ls[l]);
@@ -595,6 +601,53 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
 // ---------------------------------------------------------------------------------------------
 // kernels A + B fused (scan_fused.cuh)
 // ---------------------------------------------------------------------------------------------
+// Workspace of comet_scan_rss for a call of `total_chunks` track chunks (sizes in bytes; slab_chunks = chunks a
+// slab holds: bounded by the pair workspace limit and by 8 GiB of checkpoints).
+struct ScanWs {
+    int64_t slab_chunks;
+    int32_t n_ck;
+    size_t ck_chunk, pairs, ck, cw, ub, npu, tw, npw, ub_block;
+    bool zgroup;
+};
+static ScanWs scan_ws(const comet_ctx* ctx, int64_t total_chunks, int32_t n_steps, int32_t n_fired, int32_t z_run)
+{
+    ScanWs w;
+    const bool field = ctx->field.B != nullptr;
+    w.n_ck = n_steps / COMET_CK_ROWS(field) + 1;
+    w.ck_chunk = (size_t)w.n_ck * COMET_CK_FIELDS(field) * COMET_LANES * sizeof(double);
+    int64_t slab_chunks = total_chunks;
+    if (n_fired > 0) {
+        const int64_t by_pairs = (int64_t)(ctx->pair_max / ((size_t)COMET_LANES * (size_t)n_fired));
+        if (by_pairs < slab_chunks) slab_chunks = by_pairs;
+    }
+    const int64_t by_ck = (int64_t)(ctx->ck_max / w.ck_chunk);
+    if (by_ck < slab_chunks) slab_chunks = by_ck;
+    if (slab_chunks < 1) slab_chunks = 1;
+    w.slab_chunks = slab_chunks;
+    w.pairs = (size_t)slab_chunks * COMET_LANES * (size_t)(n_fired > 0 ? n_fired : 1);
+    w.ck = (size_t)slab_chunks * w.ck_chunk;
+    w.cw = (size_t)slab_chunks * COMET_LANES * sizeof(double);
+    w.npw = (size_t)slab_chunks * COMET_LANES * sizeof(int32_t);
+    // (small calls are launch- and latency-bound: the run-length check and the chain of k_gen_unique in front of the
+    // scan cost more than they save below about a thousand chunks -- configs[0], the refined sets of a stage)
+    w.zgroup = !field && ctx->opt_zgroup != 0 && z_run != 1 &&
+               (ctx->opt_zgroup == 2 || total_chunks >= COMET_ZG_MIN_CHUNKS);
+    // distinct transverse tracks (scan_zgroup.cuh): at most 4 per chunk (runs of >= 8 seeds), blocks of 32 tracks of
+    // n_steps + 1 rows of 4 doubles; every sub-slab starts on a block of its own
+    w.ub_block = (size_t)(n_steps + 1) * 128 * sizeof(double);
+    const size_t blocks = (size_t)slab_chunks / 8 + 2 * COMET_MAX_LANES + 2;
+    w.ub = w.zgroup ? blocks * w.ub_block : 0;
+    w.npu = w.zgroup ? blocks * 32 * sizeof(int32_t) : 0;
+    w.tw = w.zgroup ? w.cw : 0;
+    return w;
+}
+
+static bool scan_ws_fits(const comet_ctx* ctx, const ScanWs& w)
+{
+    return w.pairs <= ctx->pair_cap && w.ck <= ctx->ck_bytes && w.cw <= ctx->cw_bytes && w.ub <= ctx->ub_bytes &&
+           w.npu <= ctx->npu_bytes && w.tw <= ctx->tw_bytes && w.npw <= ctx->npw_cap * sizeof(int32_t);
+}
+
 static int grow_dev(comet_ctx* ctx, void** buf, size_t* have, size_t need)
 {
     if (need <= *have) return COMET_OK;
@@ -606,10 +659,37 @@ static int grow_dev(comet_ctx* ctx, void** buf, size_t* have, size_t need)
     return COMET_OK;
 }
 
+// grows the ctx's workspace to `w` (synchronises the device when anything is reallocated)
+static int scan_ws_grow(comet_ctx* ctx, const ScanWs& w)
+{
+    int rc = ensure_pairs(ctx, w.pairs, false);
+    if (rc) return rc;
+    if ((rc = grow_dev(ctx, (void**)&ctx->ck, &ctx->ck_bytes, w.ck))) return rc;
+    if ((rc = grow_dev(ctx, (void**)&ctx->cw, &ctx->cw_bytes, w.cw))) return rc;
+    if ((rc = grow_dev(ctx, (void**)&ctx->ub, &ctx->ub_bytes, w.ub))) return rc;
+    if ((rc = grow_dev(ctx, (void**)&ctx->npu, &ctx->npu_bytes, w.npu))) return rc;
+    if ((rc = grow_dev(ctx, (void**)&ctx->tw, &ctx->tw_bytes, w.tw))) return rc;
+    size_t have = ctx->npw_cap * sizeof(int32_t);
+    if ((rc = grow_dev(ctx, (void**)&ctx->npw, &have, w.npw))) return rc;
+    ctx->npw_cap = have / sizeof(int32_t);
+    return COMET_OK;
+}
+
+extern "C" int comet_reserve_scan(comet_ctx* ctx, int64_t n_seeds, int32_t n_steps, int32_t n_fired)
+{
+    if (!ctx || n_seeds < 1 || n_steps < 1 || n_steps > COMET_MAX_STEPS || n_fired < 0 || n_fired > ctx->wt_cap)
+        return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    return scan_ws_grow(ctx, scan_ws(ctx, n_chunks_of(n_seeds), n_steps, n_fired, 0));
+}
+
+static bool bad_zrun(int32_t z_run) { return z_run < 0 || (z_run > 1 && (z_run < 8 || (z_run & (z_run - 1)) != 0)); }
+
 // comet_scan_rss; with seeds_host != NULL (HOST SoA [6][n_seeds]) every sub-slab first copies its seeds to
 // `seeds` on its own stream, so the upload of one sub-slab overlaps the kernels of the others
 static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_host,
-                         const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                         const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
                          int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                          const double* wire_a, const double* wire_b, int32_t n_wires,
                          const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
@@ -617,57 +697,35 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                          double* rss, int32_t* n_pts, void* cuda_stream)
 {
     if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
-        !(r_stop_cm >= 0.0) ||
+        !(r_stop_cm >= 0.0) || bad_zrun(z_run) ||
         bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm))
         return COMET_EINVAL;
     if (ctx->field.B && n_steps > COMET_MAX_STEPS_FIELD) return COMET_EINVAL;
+    if (n_fired > ctx->wt_cap) return COMET_EINVAL;
     if (n_seeds == 0) return COMET_OK;
     if (!seeds || !rss) return COMET_EINVAL;
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int64_t total_chunks = n_chunks_of(n_seeds);
+    const bool field = ctx->field.B != nullptr;
+    // workspace: sized by comet_reserve_scan, else grown here -- never while the stream is being captured
+    const ScanWs ws = scan_ws(ctx, total_chunks, n_steps, n_fired, z_run);
+    if (!scan_ws_fits(ctx, ws)) {
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        CU(ctx, cudaStreamIsCapturing(st, &cap));
+        if (cap != cudaStreamCaptureStatusNone) return COMET_ENOMEM;
+        rc = scan_ws_grow(ctx, ws);
+        if (rc) return rc;
+    }
     rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
     if (rc) return rc;
-    const int64_t total_chunks = n_chunks_of(n_seeds);
-    const int32_t n_ck = n_steps / COMET_CK_ROWS(ctx->field.B != nullptr) + 1;
-    const bool field = ctx->field.B != nullptr;
-    const size_t ck_chunk = (size_t)n_ck * COMET_CK_FIELDS(field) * COMET_LANES * sizeof(double);
-    // seed slabs bounded by the pair workspace and by the checkpoint workspace
-    int64_t slab_chunks = total_chunks;
-    if (n_fired > 0) {
-        const int64_t by_pairs = (int64_t)(ctx->pair_max / ((size_t)COMET_LANES * (size_t)n_fired));
-        if (by_pairs < slab_chunks) slab_chunks = by_pairs;
-    }
-    const int64_t by_ck = (int64_t)(ctx->ck_max / ck_chunk);
-    if (by_ck < slab_chunks) slab_chunks = by_ck;
-    if (slab_chunks < 1) slab_chunks = 1;
-    rc = ensure_pairs(ctx, (size_t)slab_chunks * COMET_LANES * (size_t)(n_fired > 0 ? n_fired : 1), false);
-    if (rc) return rc;
-    rc = grow_dev(ctx, (void**)&ctx->ck, &ctx->ck_bytes, (size_t)slab_chunks * ck_chunk);
-    if (rc) return rc;
-    rc = grow_dev(ctx, (void**)&ctx->cw, &ctx->cw_bytes, (size_t)slab_chunks * COMET_LANES * sizeof(double));
-    if (rc) return rc;
-    // (small calls are launch- and latency-bound: the run-length check and the chain of k_gen_unique in front of the
-    // scan cost more than they save below about a thousand chunks -- configs[0], the refined sets of a stage)
-    const bool zgroup = !field && ctx->opt_zgroup != 0 && (ctx->opt_zgroup == 2 || total_chunks >= COMET_ZG_MIN_CHUNKS);
-    // distinct transverse tracks (scan_zgroup.cuh): at most 4 per chunk (runs of >= 8 seeds), blocks of 32 tracks of
-    // n_steps + 1 rows of 4 doubles; every sub-slab starts on a block of its own
-    const size_t ub_block = (size_t)(n_steps + 1) * 128 * sizeof(double);
-    if (zgroup) {
-        const size_t blocks = (size_t)slab_chunks / 8 + 2 * COMET_MAX_LANES + 2;
-        rc = grow_dev(ctx, (void**)&ctx->ub, &ctx->ub_bytes, blocks * ub_block);
-        if (rc) return rc;
-        rc = grow_dev(ctx, (void**)&ctx->npu, &ctx->npu_bytes, blocks * 32 * sizeof(int32_t));
-        if (rc) return rc;
-        rc = grow_dev(ctx, (void**)&ctx->tw, &ctx->tw_bytes, (size_t)slab_chunks * COMET_LANES * sizeof(double));
-        if (rc) return rc;
-    }
-    if (!n_pts) {
-        size_t have = ctx->npw_cap * sizeof(int32_t);
-        rc = grow_dev(ctx, (void**)&ctx->npw, &have, (size_t)slab_chunks * COMET_LANES * sizeof(int32_t));
-        if (rc) return rc;
-        ctx->npw_cap = have / sizeof(int32_t);
-    }
+    const int32_t n_ck = ws.n_ck;
+    const size_t ck_chunk = ws.ck_chunk;
+    const int64_t slab_chunks = ws.slab_chunks;
+    const bool zgroup = ws.zgroup;
+    const size_t ub_block = ws.ub_block;
+    const int32_t zrun_host = (zgroup && z_run >= COMET_ZG_MIN) ? (z_run > 32 ? 32 : z_run) : 0;
     // A slab (what the workspace holds) is cut into up to opt_lanes sub-slabs that run concurrently on the
     // ctx's internal streams: k_scan_fused of sub-slab l on ls[l], its fine stage on the high-priority
     // lf[l], so that k_fine_ck of one sub-slab shares the SMs with k_scan_fused of the next ones (the two
@@ -740,6 +798,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             const bool split = !zgroup && n_fired > 32 && nc < (int64_t)COMET_FUSED_WARPS * ctx->n_sm * 2;
             const unsigned b1 = split ? (unsigned)nc : b1_packed;
             a.zg = nullptr;
+            a.zrun = zrun_host;
             a.ub = nullptr;
             a.np_u = nullptr;
             a.u_rows = n_steps + 1;
@@ -748,11 +807,13 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 // k_scan_fused<.., ZG> copies its tile rows from there; the run length is found on the device and the
                 // kernels that are not needed exit at once
                 const size_t blk0 = (size_t)cl / 8 + 2 * (size_t)l;
-                a.zg = ctx->zg_flag + l;
                 a.ub = ctx->ub + blk0 * (ub_block / sizeof(double));
                 a.np_u = ctx->npu + blk0 * 32;
-                CU(ctx, cudaMemsetAsync(ctx->zg_flag + l, 0xff, sizeof(unsigned int), s_scan));
-                k_zgroup_check<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_scan>>>(a.seeds, a.stride, a.n_seeds, ctx->zg_flag + l);
+                if (!zrun_host) {                              // run length not promised by the caller: found on the device
+                    a.zg = ctx->zg_flag + l;
+                    CU(ctx, cudaMemsetAsync(ctx->zg_flag + l, 0xff, sizeof(unsigned int), s_scan));
+                    k_zgroup_check<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_scan>>>(a.seeds, a.stride, a.n_seeds, ctx->zg_flag + l);
+                }
                 const unsigned bu = (unsigned)((a.n_seeds / COMET_ZG_MIN + 1 + 31) / 32);      // one warp per CTA: a latency-bound chain
                 if (a.stats) {
                     k_gen_unique<true><<<bu, 32, 0, s_scan>>>(a);
@@ -762,7 +823,9 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                     k_scan_fused<false, false, true><<<b1, thr, ctx->zg_smem, s_scan>>>(a);
                 }
             }
-            if (split) {
+            if (zrun_host) {
+                // (the ZG kernels serve the launch: the plain variants are not enqueued)
+            } else if (split) {
                 if (field) {
                     if (a.stats) k_scan_fused<true, true, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
                     else k_scan_fused<false, true, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
@@ -786,7 +849,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 if (field) k_fine_ck<true><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
                 else {
                     if (zgroup) k_fine_ck<false, true><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
-                    k_fine_ck<false><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
+                    if (!zrun_host) k_fine_ck<false><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
                 }
             }
             if (tm) CU(ctx, cudaEventRecord(tev[2], st));
@@ -802,14 +865,14 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
     return COMET_OK;
 }
 
-extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+extern "C" int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
                               int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                               const double* wire_a, const double* wire_b, int32_t n_wires,
                               const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
                               int32_t n_fired, int32_t n_hits, double cutoff_cm,
                               double* rss, int32_t* n_pts, void* cuda_stream)
 {
-    return scan_rss_impl(ctx, nullptr, nullptr, seeds, seed_stride, n_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+    return scan_rss_impl(ctx, nullptr, nullptr, seeds, seed_stride, n_seeds, z_run, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
                          wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm, rss, n_pts,
                          cuda_stream);
 }
@@ -1052,7 +1115,7 @@ extern "C" size_t comet_stage_work_bytes(int64_t n_seeds, int32_t n_part, int32_
     return stage_layout(n_seeds, n_part, k_ref, k_final, G, &s_max, &o1, &o2);
 }
 
-extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
                                 int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                                 const double* wire_a, const double* wire_b, int32_t n_wires,
                                 const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
@@ -1069,7 +1132,7 @@ extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t see
         !(r_stop_cm >= 0.0) ||
         bad_hits(wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm) ||
         n_part < 1 || n_part > COMET_MAX_PARTITIONS || !part_off || n_iter < 0 || !(shrink > 0.0) || !isfinite(shrink) ||
-        k_ref < 1 || k_ref > COMET_MAX_REFS || k_final < 1 || k_final > COMET_MAX_REFS ||
+        k_ref < 1 || k_ref > COMET_MAX_REFS || k_final < 1 || k_final > COMET_MAX_REFS || bad_zrun(z_run) ||
         make_grid(&g, &G, half_width, n_grid) || !seeds || !work || !final_seed || !final_rss ||
         (n_fired > 0 && !final_dca) || (n_hits > 0 && !cls))
         return COMET_EINVAL;
@@ -1089,7 +1152,8 @@ extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t see
     double hw[4] = {half_width[0], half_width[1], half_width[2], half_width[3]};
     int rc;
     for (int it = 0; ; ++it) {
-        rc = comet_scan_rss(ctx, cur, cur_stride, cur_n, charge, bz_tesla, step_cm, n_steps, r_stop_cm, wire_a, wire_b,
+        // (the caller's promise is about the seeds it passed: the refined sets are checked on the device)
+        rc = comet_scan_rss(ctx, cur, cur_stride, cur_n, it == 0 ? z_run : 0, charge, bz_tesla, step_cm, n_steps, r_stop_cm, wire_a, wire_b,
                             n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm, rss, nullptr, cuda_stream);
         if (rc) return rc;
         if (it == n_iter) break;
@@ -1166,7 +1230,7 @@ extern "C" size_t comet_turns_work_bytes(int64_t max_partition_seeds, int32_t n_
     return turns_layout(sb, n_fired, n_hits).total;
 }
 
-extern "C" int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+extern "C" int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
                                 int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                                 const double* wire_a, const double* wire_b, int32_t n_wires,
                                 const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
@@ -1179,7 +1243,7 @@ extern "C" int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t see
 {
     if (!ctx || n_part < 1 || n_part > COMET_MAX_PARTITIONS || !part_off || !work || !turn_seed || !turn_rss ||
         (n_hits > 0 && !turn_cls) || !done_host || !wires_before_host || (n_hits & 1) || min_wires < 0 || max_tracks < 0 ||
-        n_seeds < 1 || seed_stride < n_seeds)
+        n_seeds < 1 || seed_stride < n_seeds || bad_zrun(z_run))
         return COMET_EINVAL;
     PartOff po;
     if (fill_partoff(&po, part_off, n_part, n_seeds, true)) return COMET_EINVAL;
@@ -1210,7 +1274,8 @@ extern "C" int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t see
         if (cur_w < min_wires || n_done >= max_tracks) break;
         const int64_t np_seeds = po.off[p + 1] - po.off[p];
         const int64_t one[2] = {0, np_seeds};
-        rc = comet_scan_stage(ctx, seeds + po.off[p], seed_stride, np_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+        rc = comet_scan_stage(ctx, seeds + po.off[p], seed_stride, np_seeds, (z_run > 1 && po.off[p] % z_run == 0) ? z_run : 0,
+                              charge, bz_tesla, step_cm, n_steps, r_stop_cm,
                               wire_a, wire_b, n_wires, cur_fw, cur_ho, cur_rho, cur_w, cur_h, cutoff_cm, one, 1,
                               half_width, n_grid, n_iter, shrink, k_ref, 1, Wk + L.stage,
                               turn_seed + 6 * (size_t)p, turn_rss + p, dca_stage, cls_stage, st);
@@ -1439,7 +1504,7 @@ static int half_tracks_impl(comet_ctx* ctx, const double* seeds_ent, int64_t str
         const int64_t one[2] = {0, ns};
         double* fs = half_seed + (size_t)h * k_final * 6;
         uint8_t* cls_h = half_cls ? half_cls + (size_t)h * side_cls : nullptr;
-        rc = comet_scan_stage(ctx, h == 0 ? seeds_ent : flipped, h == 0 ? stride_ent : ns, ns, h == 0 ? charge : -charge, bz_tesla, step_cm, n_steps,
+        rc = comet_scan_stage(ctx, h == 0 ? seeds_ent : flipped, h == 0 ? stride_ent : ns, ns, 0, h == 0 ? charge : -charge, bz_tesla, step_cm, n_steps,
                               r_stop_cm, wire_a, wire_b, n_wires, (const int32_t*)(Wk + L.fw[h]), (const int32_t*)(Wk + L.ho[h]),
                               rho_h, w, hh, cutoff_cm, one, 1, half_width, n_grid, n_iter, shrink, k_ref, k_final,
                               Wk + L.stage, fs, half_rss + (size_t)h * k_final, dca_stage, cls_h, st);
@@ -1600,6 +1665,99 @@ extern "C" int comet_scan_turns_half(comet_ctx* ctx, const double* seeds_ent, co
 }
 
 // ---------------------------------------------------------------------------------------------
+// seed grids as inputs (readings R17, R44)
+// ---------------------------------------------------------------------------------------------
+extern "C" int32_t comet_grid_z_run(int32_t n_z)
+{
+    if (n_z < 1) return 0;
+    int32_t r = 1;
+    while (r < 32 && n_z % (2 * r) == 0) r *= 2;
+    return r;
+}
+
+static int make_shape(GridShape* g, int32_t n_part, int32_t n_p, int32_t n_ct, int32_t n_phi, int32_t n_z)
+{
+    if (n_part < 1 || n_part > COMET_MAX_PARTITIONS || n_p < 1 || n_ct < 1 || n_phi < 1 || n_z < 1 || n_p > 65536 ||
+        n_ct > 65536 || n_phi > 65536 || n_z > 65536)
+        return COMET_EINVAL;
+    g->n_p = n_p; g->n_ct = n_ct; g->n_phi = n_phi; g->n_z = n_z;
+    g->G = (int64_t)n_p * n_ct * n_phi * n_z;
+    if (g->G > ((int64_t)1 << 40)) return COMET_EINVAL;
+    g->A = 2 + n_p + 2 * n_ct + 2 * n_phi + n_z;
+    return COMET_OK;
+}
+
+extern "C" size_t comet_grid_axes_len(int32_t n_p, int32_t n_ct, int32_t n_phi, int32_t n_z)
+{
+    GridShape g;
+    return make_shape(&g, 1, n_p, n_ct, n_phi, n_z) ? 0 : (size_t)g.A;
+}
+
+extern "C" int comet_seed_grid(comet_ctx* ctx, const double* axes, int32_t n_part, int32_t n_p, int32_t n_ct,
+                               int32_t n_phi, int32_t n_z, double* seeds, int64_t seed_stride, void* cuda_stream)
+{
+    GridShape g;
+    if (!ctx || make_shape(&g, n_part, n_p, n_ct, n_phi, n_z) || !axes || !seeds || seed_stride < g.G * n_part)
+        return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    const int64_t total = g.G * n_part;
+    k_seed_grid<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(axes, g, total, seeds, seed_stride);
+    CU(ctx, cudaGetLastError());
+    return COMET_OK;
+}
+
+extern "C" int comet_seed_runs(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
+                               int32_t* z_run_host, void* cuda_stream)
+{
+    if (!ctx || n_seeds < 0 || seed_stride < n_seeds || !z_run_host || (n_seeds > 0 && !seeds)) return COMET_EINVAL;
+    *z_run_host = 32;
+    if (n_seeds < 2) return COMET_OK;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unsigned int* flag = ctx->zg_flag + COMET_MAX_LANES;      // a slot of its own (the lanes use [0, COMET_MAX_LANES))
+    CU(ctx, cudaMemsetAsync(flag, 0xff, sizeof(unsigned int), st));
+    k_zgroup_check<<<(unsigned)((n_seeds + 255) / 256), 256, 0, st>>>(seeds, seed_stride, n_seeds, flag);
+    CU(ctx, cudaGetLastError());
+    unsigned int f = 0;
+    CU(ctx, cudaMemcpyAsync(&f, flag, sizeof(f), cudaMemcpyDeviceToHost, st));
+    CU(ctx, cudaStreamSynchronize(st));
+    *z_run_host = f > 32u ? 32 : (int32_t)f;
+    return COMET_OK;
+}
+
+extern "C" int comet_set_geometry(comet_ctx* ctx, const double* wire_a_host, const double* wire_b_host, int32_t n_wires,
+                                  void* cuda_stream)
+{
+    if (!ctx || n_wires < 0 || (n_wires > 0 && (!wire_a_host || !wire_b_host))) return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(ctx, cudaStreamSynchronize(st));
+    if (ctx->geom_a) { cudaFree(ctx->geom_a); ctx->geom_a = nullptr; }
+    if (ctx->geom_b) { cudaFree(ctx->geom_b); ctx->geom_b = nullptr; }
+    ctx->geom_n = 0;
+    if (n_wires == 0) return COMET_OK;
+    const size_t bytes = sizeof(double) * 3 * (size_t)n_wires;
+    cudaError_t e = cudaMalloc(&ctx->geom_a, bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->geom_b, bytes);
+    if (e != cudaSuccess) { ctx->last_cuda = (int)e; cudaGetLastError(); return COMET_ENOMEM; }
+    CU(ctx, cudaMemcpyAsync(ctx->geom_a, wire_a_host, bytes, cudaMemcpyHostToDevice, st));
+    CU(ctx, cudaMemcpyAsync(ctx->geom_b, wire_b_host, bytes, cudaMemcpyHostToDevice, st));
+    CU(ctx, cudaStreamSynchronize(st));
+    ctx->geom_n = n_wires;
+    return COMET_OK;
+}
+
+extern "C" int comet_get_geometry(const comet_ctx* ctx, const double** wire_a_dev, const double** wire_b_dev, int32_t* n_wires)
+{
+    if (!ctx || !wire_a_dev || !wire_b_dev || !n_wires) return COMET_EINVAL;
+    *wire_a_dev = ctx->geom_a; *wire_b_dev = ctx->geom_b; *n_wires = ctx->geom_n;
+    return COMET_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
 // whole event from host buffers
 // ---------------------------------------------------------------------------------------------
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -1624,9 +1782,12 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
                                      int64_t* best_seed_host, double* best_rss_host, double* best_dca_host,
                                      uint8_t* cls_host, double* rss_host, void* cuda_stream)
 {
+    // wire_a_host == NULL: the geometry set with comet_set_geometry, already on the device
+    const bool resident = ctx && !wire_a_host && !wire_b_host && ctx->geom_n > 0;
+    if (resident) n_wires = ctx->geom_n;
     if (!ctx || n_seeds < 0 || bad_physics(charge, bz_tesla, step_cm, n_steps) || !(r_stop_cm >= 0.0) ||
-        bad_hits(wire_a_host, wire_b_host, n_wires, fired_wire_host, hit_off_host, rho_host, n_fired, n_hits,
-                 cutoff_cm) ||
+        bad_hits(resident ? ctx->geom_a : wire_a_host, resident ? ctx->geom_b : wire_b_host, n_wires, fired_wire_host,
+                 hit_off_host, rho_host, n_fired, n_hits, cutoff_cm) ||
         n_part < 0 || n_part > COMET_MAX_PARTITIONS || (n_seeds > 0 && !seeds_host) ||
         (n_part > 0 && (!part_off_host || !best_seed_host || !best_rss_host)) ||
         (n_part > 0 && n_fired > 0 && !best_dca_host) || (n_part > 0 && n_hits > 0 && !cls_host))
@@ -1638,8 +1799,8 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
     const size_t o_seeds = take(sizeof(double) * 6 * (size_t)n_seeds);
-    const size_t o_wa = take(sizeof(double) * 3 * (size_t)n_wires);
-    const size_t o_wb = take(sizeof(double) * 3 * (size_t)n_wires);
+    const size_t o_wa = take(resident ? 0 : sizeof(double) * 3 * (size_t)n_wires);
+    const size_t o_wb = take(resident ? 0 : sizeof(double) * 3 * (size_t)n_wires);
     const size_t o_fw = take(sizeof(int32_t) * (size_t)n_fired);
     const size_t o_ho = take(sizeof(int32_t) * ((size_t)n_fired + 1));
     const size_t o_rho = take(sizeof(double) * (size_t)n_hits);
@@ -1653,8 +1814,8 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
     if (rc) return rc;
     char* B = (char*)ctx->hbuf;
     double* d_seeds = (double*)(B + o_seeds);
-    double* d_wa = (double*)(B + o_wa);
-    double* d_wb = (double*)(B + o_wb);
+    double* d_wa = resident ? ctx->geom_a : (double*)(B + o_wa);
+    double* d_wb = resident ? ctx->geom_b : (double*)(B + o_wb);
     int32_t* d_fw = (int32_t*)(B + o_fw);
     int32_t* d_ho = (int32_t*)(B + o_ho);
     double* d_rho = (double*)(B + o_rho);
@@ -1679,15 +1840,17 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
     // (fused mode uploads the seeds per sub-slab inside scan_rss_impl, overlapped with the kernels)
     if (n_seeds && !fused) CU(ctx, cudaMemcpyAsync(d_seeds, seeds_host, sizeof(double) * 6 * (size_t)n_seeds, cudaMemcpyHostToDevice, st));
     if (n_fired) {
-        CU(ctx, cudaMemcpyAsync(d_wa, wire_a_host, sizeof(double) * 3 * (size_t)n_wires, cudaMemcpyHostToDevice, st));
-        CU(ctx, cudaMemcpyAsync(d_wb, wire_b_host, sizeof(double) * 3 * (size_t)n_wires, cudaMemcpyHostToDevice, st));
+        if (!resident) {
+            CU(ctx, cudaMemcpyAsync(d_wa, wire_a_host, sizeof(double) * 3 * (size_t)n_wires, cudaMemcpyHostToDevice, st));
+            CU(ctx, cudaMemcpyAsync(d_wb, wire_b_host, sizeof(double) * 3 * (size_t)n_wires, cudaMemcpyHostToDevice, st));
+        }
         CU(ctx, cudaMemcpyAsync(d_fw, fired_wire_host, sizeof(int32_t) * (size_t)n_fired, cudaMemcpyHostToDevice, st));
         CU(ctx, cudaMemcpyAsync(d_ho, hit_off_host, sizeof(int32_t) * ((size_t)n_fired + 1), cudaMemcpyHostToDevice, st));
     }
     if (n_hits) CU(ctx, cudaMemcpyAsync(d_rho, rho_host, sizeof(double) * (size_t)n_hits, cudaMemcpyHostToDevice, st));
     // ---- A + B per slab, then C --------------------------------------------------------------
     if (fused && n_seeds > 0) {
-        rc = scan_rss_impl(ctx, d_seeds, seeds_host, d_seeds, n_seeds, n_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+        rc = scan_rss_impl(ctx, d_seeds, seeds_host, d_seeds, n_seeds, n_seeds, 0, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
                            d_wa, d_wb, n_wires, d_fw, d_ho, d_rho, n_fired, n_hits, cutoff_cm, d_rss, d_npts, st);
         if (rc) return rc;
     }
@@ -1714,6 +1877,83 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
         if (n_hits) CU(ctx, cudaMemcpyAsync(cls_host, d_cls, (size_t)n_part * n_hits, cudaMemcpyDeviceToHost, st));
     }
     if (rss_host && n_seeds) CU(ctx, cudaMemcpyAsync(rss_host, d_rss, sizeof(double) * (size_t)n_seeds, cudaMemcpyDeviceToHost, st));
+    CU(ctx, cudaStreamSynchronize(st));
+    return COMET_OK;
+}
+
+// The event of comet_scan_event_host with the seed sets given as grid axes: a few KB cross the bus per event.
+extern "C" int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_host, int32_t n_part, int32_t n_p,
+                                          int32_t n_ct, int32_t n_phi, int32_t n_z,
+                                          int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                                          double r_stop_cm,
+                                          const int32_t* fired_wire_host, const int32_t* hit_off_host,
+                                          const double* rho_host, int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                          int64_t* best_seed_host, double* best_rss_host, double* best_dca_host,
+                                          uint8_t* cls_host, double* rss_host, void* cuda_stream)
+{
+    GridShape g;
+    if (!ctx || make_shape(&g, n_part, n_p, n_ct, n_phi, n_z) || !axes_host || ctx->geom_n <= 0 ||
+        bad_physics(charge, bz_tesla, step_cm, n_steps) || !(r_stop_cm >= 0.0) ||
+        bad_hits(ctx->geom_a, ctx->geom_b, ctx->geom_n, fired_wire_host, hit_off_host, rho_host, n_fired, n_hits, cutoff_cm) ||
+        !best_seed_host || !best_rss_host || (n_fired > 0 && !best_dca_host) || (n_hits > 0 && !cls_host))
+        return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int64_t n_seeds = g.G * n_part;
+    const int64_t stride = (n_seeds + 31) / 32 * 32;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+    const size_t o_axes = take(sizeof(double) * (size_t)g.A * n_part);
+    const size_t o_seeds = take(sizeof(double) * 6 * (size_t)stride);
+    const size_t o_fw = take(sizeof(int32_t) * (size_t)n_fired);
+    const size_t o_ho = take(sizeof(int32_t) * ((size_t)n_fired + 1));
+    const size_t o_rho = take(sizeof(double) * (size_t)n_hits);
+    const size_t o_rss = take(sizeof(double) * (size_t)n_seeds);
+    const size_t o_bs = take(sizeof(int64_t) * (size_t)n_part);
+    const size_t o_br = take(sizeof(double) * (size_t)n_part);
+    const size_t o_bd = take(sizeof(double) * (size_t)n_part * (size_t)n_fired);
+    const size_t o_cls = take((size_t)n_part * (size_t)n_hits);
+    if (off > ctx->hbuf_bytes) {
+        CU(ctx, cudaDeviceSynchronize());
+        rc = grow(ctx, &ctx->hbuf, &ctx->hbuf_bytes, off);
+        if (rc) return rc;
+    }
+    char* B = (char*)ctx->hbuf;
+    double* d_axes = (double*)(B + o_axes);
+    double* d_seeds = (double*)(B + o_seeds);
+    int32_t* d_fw = (int32_t*)(B + o_fw);
+    int32_t* d_ho = (int32_t*)(B + o_ho);
+    double* d_rho = (double*)(B + o_rho);
+    double* d_rss = (double*)(B + o_rss);
+    int64_t* d_bs = (int64_t*)(B + o_bs);
+    double* d_br = (double*)(B + o_br);
+    double* d_bd = (double*)(B + o_bd);
+    uint8_t* d_cls = (uint8_t*)(B + o_cls);
+    CU(ctx, cudaMemcpyAsync(d_axes, axes_host, sizeof(double) * (size_t)g.A * n_part, cudaMemcpyHostToDevice, st));
+    if (n_fired) {
+        CU(ctx, cudaMemcpyAsync(d_fw, fired_wire_host, sizeof(int32_t) * (size_t)n_fired, cudaMemcpyHostToDevice, st));
+        CU(ctx, cudaMemcpyAsync(d_ho, hit_off_host, sizeof(int32_t) * ((size_t)n_fired + 1), cudaMemcpyHostToDevice, st));
+    }
+    if (n_hits) CU(ctx, cudaMemcpyAsync(d_rho, rho_host, sizeof(double) * (size_t)n_hits, cudaMemcpyHostToDevice, st));
+    rc = comet_seed_grid(ctx, d_axes, n_part, n_p, n_ct, n_phi, n_z, d_seeds, stride, st);
+    if (rc) return rc;
+    // (a partition is a whole number of runs: G is a multiple of the run length)
+    rc = scan_rss_impl(ctx, nullptr, nullptr, d_seeds, stride, n_seeds, comet_grid_z_run(n_z), charge, bz_tesla, step_cm,
+                       n_steps, r_stop_cm, ctx->geom_a, ctx->geom_b, ctx->geom_n, d_fw, d_ho, d_rho, n_fired, n_hits,
+                       cutoff_cm, d_rss, nullptr, st);
+    if (rc) return rc;
+    int64_t po[COMET_MAX_PARTITIONS + 1];
+    for (int p = 0; p <= n_part; ++p) po[p] = (int64_t)p * g.G;
+    rc = comet_select_and_classify(ctx, d_seeds, stride, n_seeds, charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+                                   ctx->geom_a, ctx->geom_b, ctx->geom_n, d_fw, d_ho, d_rho, n_fired, n_hits, cutoff_cm,
+                                   d_rss, po, n_part, d_bs, d_br, d_bd, d_cls, st);
+    if (rc) return rc;
+    CU(ctx, cudaMemcpyAsync(best_seed_host, d_bs, sizeof(int64_t) * (size_t)n_part, cudaMemcpyDeviceToHost, st));
+    CU(ctx, cudaMemcpyAsync(best_rss_host, d_br, sizeof(double) * (size_t)n_part, cudaMemcpyDeviceToHost, st));
+    if (n_fired) CU(ctx, cudaMemcpyAsync(best_dca_host, d_bd, sizeof(double) * (size_t)n_part * n_fired, cudaMemcpyDeviceToHost, st));
+    if (n_hits) CU(ctx, cudaMemcpyAsync(cls_host, d_cls, (size_t)n_part * n_hits, cudaMemcpyDeviceToHost, st));
+    if (rss_host) CU(ctx, cudaMemcpyAsync(rss_host, d_rss, sizeof(double) * (size_t)n_seeds, cudaMemcpyDeviceToHost, st));
     CU(ctx, cudaStreamSynchronize(st));
     return COMET_OK;
 }

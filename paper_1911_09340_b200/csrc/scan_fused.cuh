@@ -102,6 +102,7 @@ struct FusedArgs {
     FieldMap F;              // field-map variants (FIELD = true): the map, and qkb = kappa q, hk.h = h_max
     double h_min;            // h_max / 64 (R31)
     const unsigned int* zg;  // scan_zgroup.cuh: run length of the launch's seeds (device); nullptr = not checked
+    int32_t zrun;            //   or the caller's promise (comet_scan_rss z_run >= 8): `zg` is then nullptr
     double* ub;              // scan_zgroup.cuh: (x_0, x_1, T_0, T_1) of the distinct transverse tracks [u / 32][u_rows][4][32]
     int32_t* np_u;           //   and their numbers of recorded states
     int32_t u_rows;          //   rows per track in ub: n_steps + 1
@@ -111,6 +112,11 @@ __device__ __forceinline__ unsigned int zgroup_of(const unsigned int* flag)
 {
     const unsigned int f = *flag;
     return f > 32u ? 32u : f;
+}
+// run length the ZG kernels work with: the caller's promise, else what k_zgroup_check found
+__device__ __forceinline__ unsigned int zrun_of(const int32_t zrun, const unsigned int* flag)
+{
+    return zrun > 0 ? (unsigned int)zrun : zgroup_of(flag);
 }
 #define COMET_CK_FIELDS(FIELD) ((FIELD) ? 7 : 6)    // checkpoint row: x, T and, in a field map, the trial step
 #ifndef COMET_FUSED_CK_FIELD
@@ -152,7 +158,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     constexpr unsigned FULL = 0xffffffffu;
     static_assert(TR % FM1 == 0 && TR % CK == 0, "tile rows");
     if (ZG) {
-        if (zgroup_of(a.zg) < COMET_ZG_MIN) return;         // the plain kernel serves this launch
+        if (zrun_of(a.zrun, a.zg) < COMET_ZG_MIN) return;   // the plain kernel serves this launch
     } else if (!FIELD && a.zg && zgroup_of(a.zg) >= COMET_ZG_MIN) {
         return;                                             // the ZG kernels serve this launch (scan_zgroup.cuh)
     }
@@ -212,7 +218,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     double* const zt = tile;                                // ZG: z column
     double* const xr = tile + TR * 32;                      // ZG: ring of compact tiles
     if (ZG) {
-        zshift = 31 - __clz((int)zgroup_of(a.zg));
+        zshift = 31 - __clz((int)zrun_of(a.zrun, a.zg));
         nshift = 5 - zshift;
         ul = lane >> zshift;                                // the seed's distinct track within the chunk
         ug0 = (chunk * COMET_LANES) >> zshift;              // the chunk's first distinct track
@@ -495,11 +501,11 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, FIELD ? COMET_FINE_MINB_FI
 {
     static_assert(!(FIELD && ZG), "the transverse motion depends on z in a field map");
     if (ZG) {
-        if (zgroup_of(a.zg) < COMET_ZG_MIN) return;
+        if (zrun_of(a.zrun, a.zg) < COMET_ZG_MIN) return;
     } else if (!FIELD && a.zg && zgroup_of(a.zg) >= COMET_ZG_MIN) {
         return;
     }
-    const int zshift = ZG ? 31 - __clz((int)zgroup_of(a.zg)) : 0;
+    const int zshift = ZG ? 31 - __clz((int)zrun_of(a.zrun, a.zg)) : 0;
     constexpr int CK = COMET_CK_ROWS(FIELD);
     constexpr int CKF = COMET_CK_FIELDS(FIELD);
     const int lane = threadIdx.x & 31;

@@ -49,7 +49,7 @@ k_zgroup_check(const double* __restrict__ seeds, int64_t stride, int64_t n, unsi
 template <bool STATS>
 __global__ void __launch_bounds__(128) k_gen_unique(const FusedArgs a)
 {
-    const unsigned int zg = zgroup_of(a.zg);
+    const unsigned int zg = zrun_of(a.zrun, a.zg);
     if (zg < COMET_ZG_MIN) return;                          // the plain k_scan_fused serves this launch
     const int zshift = 31 - __clz((int)zg);
     const int64_t ug = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;

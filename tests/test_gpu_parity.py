@@ -588,31 +588,18 @@ def test_cfg3_large_scan_in_slabs(comet):
 
 
 def _sampled_full_size_check(comet, ev, seeds, part_off, n_sample, cutoff=None, budget=8 << 30):
-    """Whole path at full size through the host-buffer entry point; RSS of a strided sample of seeds
-    against the oracle, the argmin recomputed from the device RSS, and the winners' D / classified
-    sets against the oracle (which needs only the winning seeds)."""
+    """Whole path at full size through the host-buffer entry point (run length found on the device); a sample of
+    RSS, the contenders for the best seed and the winners' D / classified sets against the oracle
+    (parity_checks.check_event_against_oracle)."""
     cutoff = ev.cutoff if cutoff is None else cutoff
     S = seeds.shape[1]
     out = comet.scan_event_host(torch.from_numpy(seeds).pin_memory(), part_off, ev.charge, ev.bz, ev.step,
                                 ev.n_steps, ev.r_stop, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire,
                                 ev.hit_off, ev.rho, cutoff, want_rss=True, track_budget_bytes=budget)
-    rss = out["rss"].numpy()
-    idx = np.unique(np.concatenate([np.arange(0, S, max(1, S // n_sample)), out["best_seed"].numpy()]))
-    sub = np.ascontiguousarray(seeds[:, idx])
-    ref = _oracle_scan(ev, sub, cutoff=cutoff)
-    assert np.array_equal(rss[idx], ref["rss"])
-    W = ev.n_fired
-    assert rss.min() >= 0.0 and rss.max() <= W * cutoff * cutoff * (1 + 1e-12)
-    for p in range(len(part_off) - 1):
-        lo, hi = int(part_off[p]), int(part_off[p + 1])
-        b = lo + int(np.argmin(rss[lo:hi]))                               # first minimum = lowest index
-        assert int(out["best_seed"][p]) == b
-        one = np.ascontiguousarray(seeds[:, b:b + 1])
-        r1 = _oracle_scan(ev, one, cutoff=cutoff)
-        rs = _oracle_select(ev, one, r1["rss"], np.array([0, 1], dtype=np.int64), cutoff=cutoff)
-        assert float(out["best_rss"][p]) == float(r1["rss"][0])
-        _check_dca(out["best_dca"][p].numpy(), rs["best_dca"][0])
-        np.testing.assert_array_equal(out["cls"][p].numpy(), rs["cls"][0])
+    from parity_checks import check_event_against_oracle
+    got = {k: out[k].numpy() for k in ("best_seed", "best_rss", "best_dca", "cls")}
+    check_event_against_oracle(ev, seeds, tuple(ev.spec["grid"]), part_off, out["rss"].numpy(), got, n_sample,
+                               np.random.default_rng(S % 1000 + int(budget > 0)), cutoff=cutoff)
     return out
 
 
