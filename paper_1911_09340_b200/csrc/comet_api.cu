@@ -15,6 +15,7 @@
 #include "select.cuh"
 #include "scan_fused.cuh"
 #include "scan_zgroup.cuh"
+#include "scan_zrun.cuh"
 #include "refine.cuh"
 #include "turns.cuh"
 #include "hough.cuh"
@@ -57,7 +58,6 @@ struct comet_ctx {
     int opt_zgroup;              // 1 (default): seeds in z-runs go through the ZG kernels (scan_zgroup.cuh)
     int lanes_set;               // COMET_OPT_LANES was set by the caller
     unsigned int* zg_flag;       // [COMET_MAX_LANES] run length found by k_zgroup_check
-    int zg_smem;                 // dynamic shared memory of k_scan_fused<.., ZG>
     double* ub;                  // distinct transverse tracks of a slab (k_gen_unique)
     size_t ub_bytes;
     int32_t* npu;
@@ -162,14 +162,6 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     ctx->opt_lanes = COMET_DEFAULT_LANES;
     ctx->opt_zgroup = 1;
     if (e == cudaSuccess) e = cudaMalloc(&ctx->zg_flag, sizeof(unsigned int) * (COMET_MAX_LANES + 1));
-    {
-        ctx->zg_smem = ((COMET_FUSED_WFIELDS + 1) * COMET_FUSED_WCAP + COMET_FUSED_WARPS * COMET_ZG_WTILE) * (int)sizeof(double);
-        const void* zk[2] = {(const void*)k_scan_fused<false, false, true>, (const void*)k_scan_fused<true, false, true>};
-        for (int j = 0; j < 2 && e == cudaSuccess; ++j) {
-            e = cudaFuncSetAttribute(zk[j], cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->zg_smem);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(zk[j], cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-        }
-    }
     {
         int prio_lo = 0, prio_hi = 0;
         if (e == cudaSuccess) e = cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
@@ -606,7 +598,8 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
 struct ScanWs {
     int64_t slab_chunks;
     int32_t n_ck;
-    size_t ck_chunk, pairs, ck, cw, ub, npu, tw, npw, ub_block;
+    size_t ck_chunk, pairs, ck, cw, ub, npu, tw, npw;
+    int32_t tpc, u_rows;      // distinct tracks per chunk the workspace is sized for, rows per track
     bool zgroup;
 };
 static ScanWs scan_ws(const comet_ctx* ctx, int64_t total_chunks, int32_t n_steps, int32_t n_fired, int32_t z_run)
@@ -632,12 +625,13 @@ static ScanWs scan_ws(const comet_ctx* ctx, int64_t total_chunks, int32_t n_step
     // scan cost more than they save below about a thousand chunks -- configs[0], the refined sets of a stage)
     w.zgroup = !field && ctx->opt_zgroup != 0 && z_run != 1 &&
                (ctx->opt_zgroup == 2 || total_chunks >= COMET_ZG_MIN_CHUNKS);
-    // distinct transverse tracks (scan_zgroup.cuh): at most 4 per chunk (runs of >= 8 seeds), blocks of 32 tracks of
-    // n_steps + 1 rows of 4 doubles; every sub-slab starts on a block of its own
-    w.ub_block = (size_t)(n_steps + 1) * 128 * sizeof(double);
-    const size_t blocks = (size_t)slab_chunks / 8 + 2 * COMET_MAX_LANES + 2;
-    w.ub = w.zgroup ? blocks * w.ub_block : 0;
-    w.npu = w.zgroup ? blocks * 32 * sizeof(int32_t) : 0;
+    // distinct transverse tracks (scan_zgroup.cuh): 32 / run length per chunk (at most 4: runs of >= 8 seeds), each
+    // u_rows = n_steps + 1 rounded up to whole 64-row blocks, 32 bytes per row
+    w.tpc = (z_run >= COMET_ZG_MIN) ? (z_run >= 32 ? 1 : 32 / z_run) : 4;
+    w.u_rows = (n_steps + 64) & ~63;
+    const size_t tracks = (size_t)slab_chunks * w.tpc + 64;
+    w.ub = w.zgroup ? tracks * (size_t)w.u_rows * 4 * sizeof(double) : 0;
+    w.npu = w.zgroup ? tracks * sizeof(int32_t) : 0;
     w.tw = w.zgroup ? w.cw : 0;
     return w;
 }
@@ -724,7 +718,6 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
     const size_t ck_chunk = ws.ck_chunk;
     const int64_t slab_chunks = ws.slab_chunks;
     const bool zgroup = ws.zgroup;
-    const size_t ub_block = ws.ub_block;
     const int32_t zrun_host = (zgroup && z_run >= COMET_ZG_MIN) ? (z_run > 32 ? 32 : z_run) : 0;
     // A slab (what the workspace holds) is cut into up to opt_lanes sub-slabs that run concurrently on the
     // ctx's internal streams: k_scan_fused of sub-slab l on ls[l], its fine stage on the high-priority
@@ -801,27 +794,39 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             a.zrun = zrun_host;
             a.ub = nullptr;
             a.np_u = nullptr;
-            a.u_rows = n_steps + 1;
+            a.u_rows = ws.u_rows;
+            FusedArgs az = a;                                   // the arguments of the z-run kernels
             if (zgroup) {
-                // seeds in runs that differ only in z: every distinct transverse track is stepped once (k_gen_unique),
-                // k_scan_fused<.., ZG> copies its tile rows from there; the run length is found on the device and the
-                // kernels that are not needed exit at once
-                const size_t blk0 = (size_t)cl / 8 + 2 * (size_t)l;
-                a.ub = ctx->ub + blk0 * (ub_block / sizeof(double));
-                a.np_u = ctx->npu + blk0 * 32;
-                if (!zrun_host) {                              // run length not promised by the caller: found on the device
-                    a.zg = ctx->zg_flag + l;
+                // seeds in runs that differ only in z: every distinct transverse track is stepped once (k_gen_unique) and
+                // k_scan_zrun works from those tracks (scan_zrun.cuh); the run length is the caller's promise, else it is
+                // found on the device and the kernels that are not needed exit at once
+                az.ub = ctx->ub + (size_t)cl * ws.tpc * (size_t)ws.u_rows * 4;
+                az.np_u = ctx->npu + (size_t)cl * ws.tpc;
+                az.n_ck = n_steps / COMET_ZR_CK + 1;             // z checkpoints only, inside the sub-slab's checkpoint region
+                if (!zrun_host) {
+                    az.zg = ctx->zg_flag + l;
+                    a.zg = az.zg;
                     CU(ctx, cudaMemsetAsync(ctx->zg_flag + l, 0xff, sizeof(unsigned int), s_scan));
                     k_zgroup_check<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_scan>>>(a.seeds, a.stride, a.n_seeds, ctx->zg_flag + l);
                 }
-                const unsigned bu = (unsigned)((a.n_seeds / COMET_ZG_MIN + 1 + 31) / 32);      // one warp per CTA: a latency-bound chain
-                if (a.stats) {
-                    k_gen_unique<true><<<bu, 32, 0, s_scan>>>(a);
-                    k_scan_fused<true, false, true><<<b1, thr, ctx->zg_smem, s_scan>>>(a);
-                } else {
-                    k_gen_unique<false><<<bu, 32, 0, s_scan>>>(a);
-                    k_scan_fused<false, false, true><<<b1, thr, ctx->zg_smem, s_scan>>>(a);
-                }
+                const int64_t zr_min = zrun_host ? zrun_host : COMET_ZG_MIN;
+                const unsigned bu = (unsigned)(((a.n_seeds + zr_min - 1) / zr_min + 31) / 32);  // one warp per CTA: a latency-bound chain
+                if (a.stats) k_gen_unique<true><<<bu, 32, 0, s_scan>>>(az);
+                else k_gen_unique<false><<<bu, 32, 0, s_scan>>>(az);
+                const bool bigw = n_fired > COMET_ZR_WCAP;
+                const unsigned bz = (unsigned)((nc + COMET_ZR_WARPS - 1) / COMET_ZR_WARPS);
+                const int zthr = 32 * COMET_ZR_WARPS;
+#define COMET_LAUNCH_ZRUN(NU)                                                                                         \
+                do {                                                                                                  \
+                    if (a.stats) { if (bigw) k_scan_zrun<true, NU, true><<<bz, zthr, COMET_ZR_SMEM, s_scan>>>(az);     \
+                                   else k_scan_zrun<true, NU, false><<<bz, zthr, COMET_ZR_SMEM, s_scan>>>(az); }       \
+                    else { if (bigw) k_scan_zrun<false, NU, true><<<bz, zthr, COMET_ZR_SMEM, s_scan>>>(az);            \
+                           else k_scan_zrun<false, NU, false><<<bz, zthr, COMET_ZR_SMEM, s_scan>>>(az); }              \
+                } while (0)
+                if (!zrun_host || zrun_host == 32) COMET_LAUNCH_ZRUN(1);
+                if (!zrun_host || zrun_host == 16) COMET_LAUNCH_ZRUN(2);
+                if (!zrun_host || zrun_host == 8) COMET_LAUNCH_ZRUN(4);
+#undef COMET_LAUNCH_ZRUN
             }
             if (zrun_host) {
                 // (the ZG kernels serve the launch: the plain variants are not enqueued)
@@ -848,7 +853,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             if (n_fired > 0) {
                 if (field) k_fine_ck<true><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
                 else {
-                    if (zgroup) k_fine_ck<false, true><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
+                    if (zgroup) k_fine_ck<false, true><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(az);
                     if (!zrun_host) k_fine_ck<false><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
                 }
             }

@@ -554,17 +554,21 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, FIELD ? COMET_FINE_MINB_FI
                 const double lo = (ks > 0) ? -bs_in : 0.0, hi = (ks < np - 1) ? bs_out : 0.0;
                 D = fine_dca_field(bs, lo, hi, c, a.F, wl);
             } else if (ZG) {
-                const int kc = ka & ~(CK - 1);
+                // the distinct track's rows [u][row] = (x, y, T_x, T_y) (scan_zgroup.cuh); z from the checkpoint at or
+                // before ka (one every COMET_ZR_CK rows, scan_zrun.cuh) plus one addition per step
+                constexpr int CKZ = 8;
+                const int kc = ka & ~(CKZ - 1);
                 const int64_t u = s >> zshift;
-                const double* g = a.ub + ((size_t)(u >> 5) * (size_t)a.u_rows + (size_t)ka) * 128 + (u & 31);
+                const double2* g = reinterpret_cast<const double2*>(a.ub + ((size_t)u * (size_t)a.u_rows + (size_t)ka) * 4);
                 const double t2 = a.tw[s], hz = xmul(a.hk.h, t2);
-                double z = a.ck[(size_t)chunk * a.n_ck * (CKF * COMET_LANES) + (size_t)(kc / CK) * COMET_LANES + lane];
+                double z = a.ck[(size_t)chunk * a.n_ck * COMET_LANES + (size_t)(kc / CKZ) * COMET_LANES + lane];
                 for (int k = kc; k < ka; ++k) z = xadd(z, hz);
                 State cand[3];
 #pragma unroll
                 for (int j = 0; j < 3; ++j) {                // rows ka, ka + 1, ka + 2 (clamped: read, not used, past kz)
-                    const double* r = g + (size_t)min(j, kz - ka) * 128;
-                    cand[j].x0 = __ldg(r); cand[j].x1 = __ldg(r + 32); cand[j].t0 = __ldg(r + 64); cand[j].t1 = __ldg(r + 96);
+                    const double2* r = g + (size_t)min(j, kz - ka) * 2;
+                    const double2 xy = __ldg(r), tt = __ldg(r + 1);
+                    cand[j].x0 = xy.x; cand[j].x1 = xy.y; cand[j].t0 = tt.x; cand[j].t1 = tt.y;
                     cand[j].t2 = t2;
                 }
                 State bs = cand[0];

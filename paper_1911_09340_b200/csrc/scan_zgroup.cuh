@@ -45,7 +45,9 @@ k_zgroup_check(const double* __restrict__ seeds, int64_t stride, int64_t n, unsi
 }
 
 // One thread per distinct transverse track of the launch (unique u = seeds [u ZG, (u + 1) ZG)): Algorithm 1 for
-// (x_0, x_1, T_0, T_1), every recorded state to ub [u / 32][row][4][32], the number of recorded states to np_u.
+// (x_0, x_1, T_0, T_1), every recorded state to ub [u][row] = (x_0, x_1, T_0, T_1) -- 32 bytes per state, the rows of a
+// track contiguous, so that k_scan_zrun reads a sub-block of a track as 8 x 32 bytes and a sample with its tangent as one
+// row --, the number of recorded states to np_u.  Rows between the last state and the end of its 64-row block repeat it.
 template <bool STATS>
 __global__ void __launch_bounds__(128) k_gen_unique(const FusedArgs a)
 {
@@ -59,36 +61,42 @@ __global__ void __launch_bounds__(128) k_gen_unique(const FusedArgs a)
     const double c = seed_init(a.seeds, a.stride, su, a.qkb, st);
     st.x2 = 0.0;                                            // z is the sweep kernel's business
     st.t2 = 0.0;
-    double* o = a.ub + (size_t)(ug >> 5) * (size_t)a.u_rows * 128 + (ug & 31);
+    double2* o = reinterpret_cast<double2*>(a.ub + (size_t)ug * (size_t)a.u_rows * 4);
     const bool use_stop = a.r_stop2 > 0.0;
     int32_t np = a.n_steps + 1;
-    o[0] = st.x0; o[32] = st.x1; o[64] = st.t0; o[96] = st.t1;
+    o[0] = make_double2(st.x0, st.x1); o[1] = make_double2(st.t0, st.t1);
     // The chain of dependent operations of a step is the whole cost here (one warp per CTA, nothing to overlap
     // with), so the stop test must not sit on it: blocks of 4 steps are taken and recorded unconditionally -- rows
-    // past the stop are never read -- and the first state in the target region, if any, ends the track afterwards.
+    // past the stop are overwritten by the padding below -- and the first state in the target region, if any, ends
+    // the track afterwards.
+    State last = st;
     int k = 1;
     for (; k + 3 <= a.n_steps; k += 4) {
         int first = 4;
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             rkn4_step(st, a.hk, c);
-            double* r = o + (size_t)(k + j) * 128;
-            r[0] = st.x0; r[32] = st.x1; r[64] = st.t0; r[96] = st.t1;
+            o[(size_t)(k + j) * 2] = make_double2(st.x0, st.x1); o[(size_t)(k + j) * 2 + 1] = make_double2(st.t0, st.t1);
             // in_target_region without its early exit: no branch waits for this step's position
             const double r2 = xadd(xmul(st.x0, st.x0), xmul(st.x1, st.x1));
             const double rad = xadd(xmul(st.x0, st.t0), xmul(st.x1, st.t1));
             const bool stop = (r2 < a.r_stop2) & (rad < 0.0) & use_stop;
-            first = (stop & (first == 4)) ? j : first;
+            if (stop & (first == 4)) { first = j; last = st; }
         }
         if (first < 4) { np = k + first + 1; break; }
+        last = st;
     }
     if (np == a.n_steps + 1)
         for (; k <= a.n_steps; ++k) {
             rkn4_step(st, a.hk, c);
-            double* r = o + (size_t)k * 128;
-            r[0] = st.x0; r[32] = st.x1; r[64] = st.t0; r[96] = st.t1;
+            o[(size_t)k * 2] = make_double2(st.x0, st.x1); o[(size_t)k * 2 + 1] = make_double2(st.t0, st.t1);
+            last = st;
             if (use_stop && in_target_region(st, a.r_stop2)) { np = k + 1; break; }
         }
+    // hold-last padding up to the end of the 64-row block (u_rows is a multiple of 64)
+    for (int q = np; q < ((np + 63) & ~63); ++q) {
+        o[(size_t)q * 2] = make_double2(last.x0, last.x1); o[(size_t)q * 2 + 1] = make_double2(last.t0, last.t1);
+    }
     a.np_u[ug] = np;
     if (STATS && a.stats) atomicAdd(a.stats + ST_UNIQUE, (unsigned long long)(np - 1));
 }

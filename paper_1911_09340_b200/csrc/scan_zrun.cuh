@@ -1,0 +1,367 @@
+// scan_zrun.cuh -- kernels A + B2 for seed sets in z-runs: the closest-state shortlist of every (seed, wire) pair
+// straight from the distinct transverse tracks, with a tangent-line bound per (track, sub-block) (sm_100a).
+//
+// Aligned runs of ZR = 32 / NU consecutive seeds share (x, y, p) and differ only in z (scan_zgroup.cuh), so a
+// track chunk of 32 seeds holds NU distinct transverse tracks.  k_gen_unique has stepped them once:
+// ub[track][row] = (x, y, T_x, T_y), 32 bytes per recorded state, rows past the last state of a track repeat it up
+// to the end of its 64-row block.  A warp owns a chunk from there to its shortlist keys (lane = seed in the
+// sweeps, lane = wire in the tests):
+//
+//   z chain    every seed's own z column, one addition per recorded state (the definition's x_2' = x_2 + h T_2),
+//              kept only as a checkpoint every 8th row for k_fine_ck; nothing else of the track is recomputed or
+//              staged: there is no tile;
+//   level A    per 64-row block and wire: the distance of ONE sample (row 36) of each distinct track, taken at
+//              the centre of the run's z range, against R_i + (z half range) sqrt(1 - w_z^2) + 36 L -- the
+//              1-Lipschitz bound of dca.cuh; the wires that pass are compacted into a list;
+//   level B    per listed wire, 8-row sub-block and distinct track: the sample (row 4 of the sub-block) WITH ITS
+//              TANGENT.  The rows of the sub-block lie within U = 4 h of arc of the sample, and a curve of
+//              curvature <= |c| leaves its tangent line by at most |c| U^2 / 2 over that arc, so no row of any seed
+//              of the run is closer to the wire than
+//                  sqrt( min_{|u| <= U} |a + u b|^2 ) - |c| U^2 / 2 - (z half range) sqrt(1 - w_z^2),
+//              a = the sample's offset from the wire and b = its tangent, both projected on the plane
+//              perpendicular to the wire.  The minimum of the quadratic is taken in closed form without a
+//              division.  A sub-block is opened for a wire only if that bound is within the far radius R_i: about
+//              1.2 opened sub-blocks per sub-block that holds a state within R_i, against 2.5 with the one-sample
+//              Lipschitz test of k_scan_fused (configs[1]);
+//   sweeps     lane = seed: the rows of the opened sub-blocks are read from ub (16 bytes per row, broadcast to the
+//              seeds of the run), z = z_0 + k h T_z, 9 FP64 instructions per row, best (d^2, row) merged into
+//              the pair key with one atomic min as in k_scan_fused;
+//   finish     as in k_scan_fused.
+//
+// Only shortlists are decided here (FMA-form distances, slack 1e-6 cm on every bound): k_fine_ck<ZG> re-decides
+// between rows k-1, k, k+1 with the definition's exact operations, so n_pts and RSS are the bit-identical numbers
+// of the plain path and of the oracle.  A chunk with a lane beyond |c| h <= 0.05 opens everything.
+#pragma once
+#include "scan_fused.cuh"
+
+namespace comet {
+
+#define COMET_ZR_WARPS 4
+#define COMET_ZR_WCAP 128          // wires whose constants the CTA's shared-memory table holds (the others: L1/L2)
+#define COMET_ZR_CK 8              // rows between z checkpoints
+#define COMET_ZR_LCAP 1024         // (chunk, wire) items collected per reservation in the finish
+#ifndef COMET_ZR_MINB
+#define COMET_ZR_MINB 5
+#endif
+#define COMET_ZR_NF (COMET_FUSED_WFIELDS + 1)
+// doubles of shared memory per warp: 32 samples of 6, the pass list (64 shorts), the item list (LCAP shorts)
+#define COMET_ZR_WSM (32 * 6 + 16 + COMET_ZR_LCAP / 4)
+#define COMET_ZR_SMEM ((COMET_ZR_NF * COMET_ZR_WCAP + COMET_ZR_WARPS * COMET_ZR_WSM) * (int)sizeof(double))
+#define COMET_ZR_MARGIN 1e-6       // cm, added to every pruning threshold (FMA rounding is ~1e-13)
+
+template <bool BIGW>
+__device__ __forceinline__ double zr_const(const double* wtab, const double* __restrict__ wt, int W, int f, int i)
+{
+    if (!BIGW) return wtab[f * COMET_ZR_WCAP + i];
+    return (i < COMET_ZR_WCAP) ? wtab[f * COMET_ZR_WCAP + i] : __ldg(wt + (size_t)(6 + f) * W + i);
+}
+template <bool BIGW>
+__device__ __forceinline__ void zr_evalc(EvalC& w, const double* wtab, const double* __restrict__ wt, int W, int i)
+{
+    w.e1x = zr_const<BIGW>(wtab, wt, W, 0, i); w.e1y = zr_const<BIGW>(wtab, wt, W, 1, i); w.e1z = zr_const<BIGW>(wtab, wt, W, 2, i);
+    w.c1 = zr_const<BIGW>(wtab, wt, W, 3, i);
+    w.e2x = zr_const<BIGW>(wtab, wt, W, 4, i); w.e2y = zr_const<BIGW>(wtab, wt, W, 5, i); w.e2z = zr_const<BIGW>(wtab, wt, W, 6, i);
+    w.c2 = zr_const<BIGW>(wtab, wt, W, 7, i);
+}
+template <bool BIGW>
+__device__ __forceinline__ double zr_slope(const double* wtab, const double* __restrict__ wt, int W, int i)
+{
+    if (!BIGW || i < COMET_ZR_WCAP) return wtab[COMET_FUSED_WFIELDS * COMET_ZR_WCAP + i];
+    return wire_slope(__ldg(wt + (size_t)8 * W + i), __ldg(wt + (size_t)12 * W + i));
+}
+
+template <bool STATS, int NU, bool BIGW>
+__global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zrun(const FusedArgs a)
+{
+    static_assert(NU == 1 || NU == 2 || NU == 4, "runs of 32, 16 or 8 seeds");
+    constexpr int ZR = 32 / NU, ZSH = (NU == 1 ? 5 : (NU == 2 ? 4 : 3));
+    constexpr int WCAP = COMET_ZR_WCAP, NF = COMET_ZR_NF;
+    constexpr int BLK = 64, SUB = 8, NSUB = BLK / SUB, NS = NU * NSUB, SROW = 36;
+    constexpr int CK = COMET_ZR_CK, LCAP = COMET_ZR_LCAP;
+    constexpr unsigned FULL = 0xffffffffu;
+    if (zrun_of(a.zrun, a.zg) != (unsigned)ZR) return;      // another variant serves this launch
+    extern __shared__ __align__(16) double zsm[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double* wtab = zsm;                                     // [NF][WCAP]
+    double* samp = zsm + NF * WCAP + warp * COMET_ZR_WSM;   // [NS][6]: x, y, T_x, T_y, z at the run's centre, live flag
+    unsigned short* plist = reinterpret_cast<unsigned short*>(samp + 32 * 6);      // [64] wires that passed level A
+    unsigned short* lst = reinterpret_cast<unsigned short*>(samp + 32 * 6 + 16);   // [LCAP] items of the finish
+    const int W = a.W;
+    for (int v = threadIdx.x; v < COMET_FUSED_WFIELDS * WCAP; v += 32 * COMET_ZR_WARPS) {
+        const int f = v / WCAP, i = v - f * WCAP;
+        wtab[v] = (i < W) ? __ldg(a.wt + (size_t)(6 + f) * W + i) : -1.0;
+    }
+    for (int i = threadIdx.x; i < WCAP; i += 32 * COMET_ZR_WARPS)
+        wtab[COMET_FUSED_WFIELDS * WCAP + i] = (i < W) ? wire_slope(__ldg(a.wt + (size_t)8 * W + i), __ldg(a.wt + (size_t)12 * W + i)) : 0.0;
+    __syncthreads();
+    const int64_t chunk = (int64_t)blockIdx.x * COMET_ZR_WARPS + warp;
+    if (chunk * COMET_LANES >= a.n_seeds) return;
+    const int64_t s = chunk * COMET_LANES + lane;
+    const bool valid = s < a.n_seeds;
+    const double h = a.hk.h;
+    const double INF = 1.7976931348623157e308;
+    const double L = COMET_LIP * h;
+    const double U = (SUB / 2) * h * 1.000001;              // arc between a sub-block's sample and its farthest row
+    const double lam2 = xmul(a.lambda, a.lambda);
+
+    State st;
+    double c = 0.0;
+    if (valid) {
+        c = seed_init(a.seeds, a.stride, s, a.qkb, st);
+    } else {
+        st.x0 = st.x1 = st.x2 = 0.0;
+        st.t0 = st.t1 = st.t2 = 0.0;
+    }
+    const bool lip_ok = fabs(c) * h <= COMET_CH_MAX;
+    const bool any_nolip = __any_sync(FULL, valid && !lip_ok);
+    const int tl = lane >> ZSH;                             // the seed's distinct track within the chunk
+    const int64_t ug = ((chunk * COMET_LANES) >> ZSH) + tl;
+    const int32_t np = valid ? __ldg(a.np_u + ug) : 0;      // recorded states of the seed = of its transverse track
+    const double hz = xmul(h, st.t2);                       // x_2' = x_2 + h T_2, T_2 constant
+    const double z0 = st.x2;
+    const double* const ubl = a.ub + (size_t)ug * (size_t)a.u_rows * 4;
+    // largest |c| of the chunk, rounded up: how far a track leaves its tangent line over the arc U
+    const float cf = valid ? __double2float_ru(fabs(c)) : 0.f;
+    const double cmax = (double)__uint_as_float(__reduce_max_sync(FULL, __float_as_uint(cf)));
+    const double dev = cmax * U * U * 0.5000005 + 1e-7;
+    // per run: centre and half range of the seeds' z_0 (an invalid lane of a ragged last run stands aside)
+    double zlo, zhi;
+    {
+        const double zfirst = __shfl_sync(FULL, z0, tl << ZSH);
+        const double zv = valid ? z0 : zfirst;
+        zlo = zv; zhi = zv;
+#pragma unroll
+        for (int o = 1; o < ZR; o <<= 1) {
+            zlo = fmin(zlo, __shfl_xor_sync(FULL, zlo, o));
+            zhi = fmax(zhi, __shfl_xor_sync(FULL, zhi, o));
+        }
+    }
+    const double zc0 = 0.5 * (zlo + zhi);
+    const double zh = 0.5 * (zhi - zlo) * 1.000001 + 1e-9; // |z_k(seed) - (zc0 + k hz)| <= zh for every seed of the run
+    double zh_t[NU], tz_t[NU];
+    int32_t np_t[NU];
+    int32_t npmax = 0;
+#pragma unroll
+    for (int t = 0; t < NU; ++t) {
+        zh_t[t] = __shfl_sync(FULL, zh, t << ZSH);
+        tz_t[t] = __shfl_sync(FULL, st.t2, t << ZSH);
+        np_t[t] = __shfl_sync(FULL, np, t << ZSH);
+        npmax = max(npmax, np_t[t]);
+    }
+    int32_t npmin = npmax;
+#pragma unroll
+    for (int t = 0; t < NU; ++t)
+        if (np_t[t] > 0) npmin = min(npmin, np_t[t]);
+
+    // pair keys of this chunk: nothing found yet
+    unsigned long long* const keys = reinterpret_cast<unsigned long long*>(a.bd);
+    for (int i = 0; i < W; ++i) keys[(size_t)i * a.SP + s] = COMET_KEY_NONE;
+    // the seed's z column (Algorithm 1 for x_2), a checkpoint every CK rows
+    {
+        double* ckc = a.ck + (size_t)chunk * a.n_ck * COMET_LANES + lane;
+        double z = z0;
+        if (np > 0) ckc[0] = z;
+        for (int k0 = 1; k0 < npmax; k0 += CK) {
+#pragma unroll
+            for (int q = 0; q < CK; ++q) {
+                const int k = k0 + q;
+                if (k < np) z = xadd(z, hz);
+                if (q == CK - 1 && k < np) ckc[(size_t)(k / CK) * COMET_LANES] = z;
+            }
+        }
+    }
+    if (valid) { a.n_pts[s] = np; a.cw[s] = c; a.tw[s] = st.t2; }
+
+    unsigned long long st_cnt[ST_N];
+    if (STATS) {
+#pragma unroll
+        for (int j = 0; j < ST_N; ++j) st_cnt[j] = 0;
+        if (valid) st_cnt[ST_PAIRS] = (unsigned long long)W;
+    }
+    const int n_rounds = (W + 31) / 32;
+    for (int r0 = 0; r0 < npmax; r0 += BLK) {
+        // ---- samples of the block: row 4 of every sub-block of every distinct track ------------------------
+        __syncwarp();
+#pragma unroll
+        for (int q0 = 0; q0 < NS; q0 += 16) {
+            const int q = q0 + (lane >> 1), half = lane & 1;
+            const int src = (q >> 3) << ZSH;                 // a lane of the sample's run
+            const int32_t npq = __shfl_sync(FULL, np, src);
+            const double zcq = __shfl_sync(FULL, zc0, src), hzq = __shfl_sync(FULL, hz, src);
+            const unsigned long long ubq = __shfl_sync(FULL, (unsigned long long)ubl, src);
+            if (q < NS) {
+                const bool live = npq > r0;
+                const int kz = min(r0 + (q & 7) * SUB + SUB / 2, npq - 1);
+                double2 v = make_double2(0.0, 0.0);
+                if (live) v = __ldg(reinterpret_cast<const double2*>(reinterpret_cast<const double*>(ubq) + (size_t)kz * 4 + half * 2));
+                *reinterpret_cast<double2*>(samp + q * 6 + half * 2) = v;
+                samp[q * 6 + 4 + half] = half ? (live ? 1.0 : 0.0) : fma((double)kz, hzq, zcq);
+            }
+        }
+        __syncwarp();
+        const bool tail = r0 + BLK > npmin;                   // some track of the chunk ends in this block
+        const double zb = fma((double)r0, hz, z0);           // the seed's z at row r0 (to rounding: shortlist only)
+        // ---- level A (lane = wire): one sample per distinct track and block ----------------------------------
+        int cnt = 0;
+        auto level_b = [&](const unsigned short* list, int n) {
+            // ---- level B (lane = listed wire): tangent-line bound per (distinct track, sub-block) ------------
+            const int i = lane < n ? (int)list[lane] : -1;
+            unsigned m8 = 0u;
+            if (i >= 0) {
+                EvalC ec;
+                zr_evalc<BIGW>(ec, wtab, a.wt, W, i);
+                const double cap = zr_const<BIGW>(wtab, a.wt, W, 8, i);
+                const double swz = zr_slope<BIGW>(wtab, a.wt, W, i);
+#pragma unroll
+                for (int t = 0; t < NU; ++t) {
+                    if (np_t[t] <= r0) continue;
+                    const double thr = cap + zh_t[t] * swz + dev + COMET_ZR_MARGIN;
+                    const double thr2 = thr * thr;
+                    const double bz1 = tz_t[t] * ec.e1z, bz2 = tz_t[t] * ec.e2z;
+#pragma unroll
+                    for (int j = 0; j < NSUB; ++j) {
+                        if (np_t[t] <= r0 + j * SUB) break;          // the track has no row in this sub-block
+                        const double* sp = samp + (t * NSUB + j) * 6;
+                        const double2 xy = *reinterpret_cast<const double2*>(sp), tt = *reinterpret_cast<const double2*>(sp + 2);
+                        const double z = sp[4];
+                        const double a1 = fma(xy.x, ec.e1x, fma(xy.y, ec.e1y, fma(z, ec.e1z, ec.c1)));
+                        const double a2 = fma(xy.x, ec.e2x, fma(xy.y, ec.e2y, fma(z, ec.e2z, ec.c2)));
+                        const double b1 = fma(tt.x, ec.e1x, fma(tt.y, ec.e1y, bz1));
+                        const double b2 = fma(tt.x, ec.e2x, fma(tt.y, ec.e2y, bz2));
+                        const double aa = fma(a1, a1, a2 * a2), bb = fma(b1, b1, b2 * b2);
+                        const double ab = fabs(fma(a1, b1, a2 * b2));
+                        // min over |u| <= U of |a + u b|^2 = aa - sv (2 ab - sv) / bb with sv = min(ab, U bb)
+                        const double sv = fmin(ab, U * bb);
+                        if (fma(aa - thr2, bb, -(sv * fma(2.0, ab, -sv))) <= 0.0) m8 |= 1u << j;
+                    }
+                    if (STATS) st_cnt[ST_SAMPLES] += NSUB;
+                }
+                if (any_nolip) m8 = (1u << NSUB) - 1u;
+            }
+            unsigned any = __ballot_sync(FULL, m8 != 0u);
+            while (any) {
+                const int wl = __ffs(any) - 1;
+                any &= any - 1;
+                unsigned msub = __shfl_sync(FULL, m8, wl);
+                const int iw = __shfl_sync(FULL, i, wl);
+                // ---- wire iw, lane = seed: sweep the opened sub-blocks row by row ------------------------------
+                EvalC w;
+                zr_evalc<BIGW>(w, wtab, a.wt, W, iw);      // broadcast
+                double best = INF;
+                int bk = -1;
+                while (msub) {
+                    const int j = __ffs(msub) - 1;
+                    msub &= msub - 1;
+                    const int k0 = r0 + j * SUB;
+                    const double zk = fma((double)(j * SUB), hz, zb);
+                    if (STATS) { st_cnt[ST_ROWS_EXEC] += SUB; if (np > k0) st_cnt[ST_ROWS_NEEDED] += min(SUB, np - k0); }
+                    if (!tail) {
+                        const double2* pr = reinterpret_cast<const double2*>(ubl + (size_t)k0 * 4);
+                        double2 xy[SUB];
+#pragma unroll
+                        for (int kk = 0; kk < SUB; ++kk) xy[kk] = __ldg(pr + kk * 2);
+#pragma unroll
+                        for (int kk = 0; kk < SUB; ++kk) {
+                            const double d2 = d2_fma(w, xy[kk].x, xy[kk].y, fma((double)kk, hz, zk));
+                            if (d2 < best) { best = d2; bk = k0 + kk; }
+                        }
+                    } else {
+                        // the block in which a track of the chunk ends: rows past the seed's last state stay out
+                        const int nr = np - k0;
+                        const double2* pr = reinterpret_cast<const double2*>(ubl + (size_t)min(k0, max(np - 1, 0)) * 4);
+#pragma unroll
+                        for (int kk = 0; kk < SUB; ++kk) {
+                            const double2 xy = __ldg(pr + (kk < nr ? kk * 2 : 0));
+                            const double d2 = d2_fma(w, xy.x, xy.y, fma((double)kk, hz, zk));
+                            if (kk < nr && d2 < best) { best = d2; bk = k0 + kk; }
+                        }
+                    }
+                }
+                if (bk >= 0) atomicMin(keys + (size_t)iw * a.SP + s, pack_key(best, bk));
+            }
+        };
+        for (int r = 0; r < n_rounds; ++r) {
+            const int i = r * 32 + lane;
+            const int ii = min(i, W - 1);
+            EvalC ec;
+            zr_evalc<BIGW>(ec, wtab, a.wt, W, ii);
+            const double cap = (i < W) ? zr_const<BIGW>(wtab, a.wt, W, 8, ii) : -1.0;    // far radius; < 0: no entries
+            const double swz = zr_slope<BIGW>(wtab, a.wt, W, ii);
+            bool pass = false;
+#pragma unroll
+            for (int t = 0; t < NU; ++t) {
+                if (np_t[t] <= r0) continue;
+                const double* sp = samp + (t * NSUB + SROW / SUB) * 6;
+                const double thr = cap + zh_t[t] * swz + SROW * L + COMET_ZR_MARGIN;
+                pass = pass || (d2_fma(ec, sp[0], sp[1], sp[4]) <= thr * thr);
+                if (STATS && cap >= 0.0) st_cnt[ST_SAMPLES] += 1;
+            }
+            if (any_nolip) pass = true;
+            if (cap < 0.0) pass = false;
+            const unsigned pm = __ballot_sync(FULL, pass);
+            if (pass) plist[cnt + __popc(pm & ((1u << lane) - 1u))] = (unsigned short)i;
+            cnt += __popc(pm);
+            __syncwarp();
+            if (cnt >= 32) {
+                cnt -= 32;
+                level_b(plist + cnt, 32);
+                __syncwarp();
+            }
+        }
+        if (cnt) level_b(plist, cnt);
+    }
+    __syncwarp();
+    // ---- finish: far pairs take the cutoff, (chunk, wire) items with a near lane go to k_fine_ck -------
+    constexpr int FB = 8;
+    int cnt = 0;                                            // warp-uniform
+    auto flush = [&]() {
+        __syncwarp();
+        unsigned base = 0;
+        if (lane == 0) base = atomicAdd(a.n_items, (unsigned)cnt);
+        base = __shfl_sync(FULL, base, 0);
+        for (int j = lane; j < cnt; j += 32) a.items[base + j] = ((unsigned long long)chunk << 16) | (unsigned)lst[j];
+        cnt = 0;
+        __syncwarp();
+    };
+    for (int i0 = 0; i0 < W; i0 += FB) {
+        unsigned long long kv[FB];
+        double cap2[FB];
+#pragma unroll
+        for (int j = 0; j < FB; ++j) {
+            const int i = min(i0 + j, W - 1);
+            kv[j] = __ldcg(keys + (size_t)i * a.SP + s);
+            const double cap = zr_const<BIGW>(wtab, a.wt, W, 8, i);
+            cap2[j] = cap * cap;
+        }
+#pragma unroll
+        for (int j = 0; j < FB; ++j) {
+            const int i = i0 + j;
+            if (i < W) {
+                const size_t pidx = (size_t)i * a.SP + s;
+                const bool found = kv[j] != COMET_KEY_NONE;
+                // key_d2 <= d^2 of the closest recorded state: "far" is decided on the safe side
+                const bool near = valid && found && (key_d2(kv[j]) <= cap2[j] || !lip_ok);
+                if (STATS && near) st_cnt[ST_FINE_NEEDED] += 1;
+                if (__any_sync(FULL, near)) {
+                    if (STATS) st_cnt[ST_FINE_EXEC] += 1;
+                    if (!near && found) keys[pidx] = COMET_KEY_NONE;
+                    if (lane == 0) lst[cnt] = (unsigned short)i;
+                    if (++cnt == LCAP) flush();
+                } else {
+                    a.bd[pidx] = lam2;
+                }
+            }
+        }
+    }
+    if (cnt) flush();
+    if (STATS) {
+#pragma unroll
+        for (int j = 0; j < ST_N; ++j) {
+            unsigned long long v = st_cnt[j];
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(FULL, v, o);
+            if (lane == 0 && a.stats && v) atomicAdd(a.stats + j, v);
+        }
+    }
+}
+
+}  // namespace comet

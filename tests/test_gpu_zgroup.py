@@ -72,8 +72,10 @@ def test_z_runs_identical_to_the_oracle(comet, cfg1_event, n_z, n_seeds):
     rss0, n_pts0, st0 = _scan(comet, ev, seeds, 0)
     assert st0["unique_states"] == 0
     assert np.array_equal(rss0, rss) and np.array_equal(n_pts0, n_pts)
-    for k in ("samples", "rows_needed", "fine_needed", "pairs"):      # the same search, whoever generated the rows
-        assert st[k] == st0[k], k
+    # the z-run kernel prunes with its own bound (tangent line per distinct track, scan_zrun.cuh): the same pairs reach
+    # the virtual-plane iteration -- a pair whose closest state sits on the far radius to 1e-12 could differ --, with fewer rows swept
+    assert st["pairs"] == st0["pairs"] and abs(st["fine_needed"] - st0["fine_needed"]) <= 2
+    assert st["rows_executed"] <= st0["rows_executed"]
 
 
 @pytest.mark.parametrize("case", ["runs_of_4", "one_odd_seed", "shuffled", "apex_stop"])
