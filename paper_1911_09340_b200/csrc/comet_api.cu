@@ -818,10 +818,10 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 const int zthr = 32 * COMET_ZR_WARPS;
 #define COMET_LAUNCH_ZRUN(NU)                                                                                         \
                 do {                                                                                                  \
-                    if (a.stats) { if (bigw) k_scan_zrun<true, NU, true><<<bz, zthr, COMET_ZR_SMEM, s_scan>>>(az);     \
-                                   else k_scan_zrun<true, NU, false><<<bz, zthr, COMET_ZR_SMEM, s_scan>>>(az); }       \
-                    else { if (bigw) k_scan_zrun<false, NU, true><<<bz, zthr, COMET_ZR_SMEM, s_scan>>>(az);            \
-                           else k_scan_zrun<false, NU, false><<<bz, zthr, COMET_ZR_SMEM, s_scan>>>(az); }              \
+                    if (a.stats) { if (bigw) k_scan_zrun<true, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU), s_scan>>>(az);     \
+                                   else k_scan_zrun<true, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU), s_scan>>>(az); }       \
+                    else { if (bigw) k_scan_zrun<false, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU), s_scan>>>(az);            \
+                           else k_scan_zrun<false, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU), s_scan>>>(az); }              \
                 } while (0)
                 if (!zrun_host || zrun_host == 32) COMET_LAUNCH_ZRUN(1);
                 if (!zrun_host || zrun_host == 16) COMET_LAUNCH_ZRUN(2);

@@ -8,8 +8,10 @@
 // sweeps, lane = wire in the tests):
 //
 //   z chain    every seed's own z column, one addition per recorded state (the definition's x_2' = x_2 + h T_2),
-//              kept only as a checkpoint every 8th row for k_fine_ck; nothing else of the track is recomputed or
-//              staged: there is no tile;
+//              kept only as a checkpoint every 8th row for k_fine_ck; nothing else of the track is recomputed;
+//   staging    per 64-row block the (x, y) rows of the chunk's NU tracks (2 KB for NU = 2) and the tangents of the 8
+//              sub-block samples go to the warp's shared memory with cp.async, one block ahead (double buffer), so
+//              the L2 latency of ub is off the path;
 //   level A    per 64-row block and wire: the distance of ONE sample (row 36) of each distinct track, taken at
 //              the centre of the run's z range, against R_i + (z half range) sqrt(1 - w_z^2) + 36 L -- the
 //              1-Lipschitz bound of dca.cuh; the wires that pass are compacted into a list;
@@ -23,9 +25,10 @@
 //              division.  A sub-block is opened for a wire only if that bound is within the far radius R_i: about
 //              1.2 opened sub-blocks per sub-block that holds a state within R_i, against 2.5 with the one-sample
 //              Lipschitz test of k_scan_fused (configs[1]);
-//   sweeps     lane = seed: the rows of the opened sub-blocks are read from ub (16 bytes per row, broadcast to the
-//              seeds of the run), z = z_0 + k h T_z, 9 FP64 instructions per row, best (d^2, row) merged into
-//              the pair key with one atomic min as in k_scan_fused;
+//   sweeps     lane = seed: the rows of the opened sub-blocks are read from the staged block (one 16-byte
+//              shared-memory load per row, broadcast to the seeds of the run), z = z_0 + k h T_z folded into the
+//              wire's constants, 8 FP64 instructions + compare per row, best (d^2, row) merged into the pair key
+//              with one atomic min as in k_scan_fused;
 //   finish     as in k_scan_fused.
 //
 // Only shortlists are decided here (FMA-form distances, slack 1e-6 cm on every bound): k_fine_ck<ZG> re-decides
@@ -44,9 +47,10 @@ namespace comet {
 #define COMET_ZR_MINB 5
 #endif
 #define COMET_ZR_NF (COMET_FUSED_WFIELDS + 1)
-// doubles of shared memory per warp: 32 samples of 6, the pass list (64 shorts), the item list (LCAP shorts)
-#define COMET_ZR_WSM (32 * 6 + 16 + COMET_ZR_LCAP / 4)
-#define COMET_ZR_SMEM ((COMET_ZR_NF * COMET_ZR_WCAP + COMET_ZR_WARPS * COMET_ZR_WSM) * (int)sizeof(double))
+// doubles of shared memory per warp: two staged blocks of (64 rows + 8 sample tangents) x NU tracks x 2, the pass
+// list (64 shorts); the item list of the finish (LCAP shorts = 256 doubles) reuses the staged blocks
+#define COMET_ZR_WSM(NU) (2 * (64 + 8) * (NU) * 2 + 16)
+#define COMET_ZR_SMEM(NU) ((COMET_ZR_NF * COMET_ZR_WCAP + COMET_ZR_WARPS * COMET_ZR_WSM(NU)) * (int)sizeof(double))
 #define COMET_ZR_MARGIN 1e-6       // cm, added to every pruning threshold (FMA rounding is ~1e-13)
 
 template <bool BIGW>
@@ -76,16 +80,19 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     static_assert(NU == 1 || NU == 2 || NU == 4, "runs of 32, 16 or 8 seeds");
     constexpr int ZR = 32 / NU, ZSH = (NU == 1 ? 5 : (NU == 2 ? 4 : 3));
     constexpr int WCAP = COMET_ZR_WCAP, NF = COMET_ZR_NF;
-    constexpr int BLK = 64, SUB = 8, NSUB = BLK / SUB, NS = NU * NSUB, SROW = 36;
+    constexpr int BLK = 64, SUB = 8, NSUB = BLK / SUB, SROW = 36;
     constexpr int CK = COMET_ZR_CK, LCAP = COMET_ZR_LCAP;
+    constexpr int BUFD = (BLK + NSUB) * NU * 2;             // doubles per staged block: rows [64][NU][x, y], tangents [8][NU][T_x, T_y]
     constexpr unsigned FULL = 0xffffffffu;
+    static_assert(LCAP * (int)sizeof(unsigned short) <= 2 * BUFD * (int)sizeof(double) || NU == 1, "item list fits the staged blocks");
     if (zrun_of(a.zrun, a.zg) != (unsigned)ZR) return;      // another variant serves this launch
     extern __shared__ __align__(16) double zsm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* wtab = zsm;                                     // [NF][WCAP]
-    double* samp = zsm + NF * WCAP + warp * COMET_ZR_WSM;   // [NS][6]: x, y, T_x, T_y, z at the run's centre, live flag
-    unsigned short* plist = reinterpret_cast<unsigned short*>(samp + 32 * 6);      // [64] wires that passed level A
-    unsigned short* lst = reinterpret_cast<unsigned short*>(samp + 32 * 6 + 16);   // [LCAP] items of the finish
+    double* stg = zsm + NF * WCAP + warp * COMET_ZR_WSM(NU);      // two staged blocks
+    unsigned short* plist = reinterpret_cast<unsigned short*>(stg + 2 * BUFD);     // [64] wires that passed level A
+    unsigned short* lst = reinterpret_cast<unsigned short*>(stg);                  // finish: [<= LCAP] items
+    constexpr int LCAPW = (NU == 1) ? (2 * BUFD * 4) : LCAP;                       // shorts the staged blocks hold
     const int W = a.W;
     for (int v = threadIdx.x; v < COMET_FUSED_WFIELDS * WCAP; v += 32 * COMET_ZR_WARPS) {
         const int f = v / WCAP, i = v - f * WCAP;
@@ -115,11 +122,10 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     const bool lip_ok = fabs(c) * h <= COMET_CH_MAX;
     const bool any_nolip = __any_sync(FULL, valid && !lip_ok);
     const int tl = lane >> ZSH;                             // the seed's distinct track within the chunk
-    const int64_t ug = ((chunk * COMET_LANES) >> ZSH) + tl;
-    const int32_t np = valid ? __ldg(a.np_u + ug) : 0;      // recorded states of the seed = of its transverse track
+    const int64_t ug0 = (chunk * COMET_LANES) >> ZSH;       // the chunk's first distinct track
+    const int32_t np = valid ? __ldg(a.np_u + ug0 + tl) : 0;       // recorded states of the seed = of its transverse track
     const double hz = xmul(h, st.t2);                       // x_2' = x_2 + h T_2, T_2 constant
     const double z0 = st.x2;
-    const double* const ubl = a.ub + (size_t)ug * (size_t)a.u_rows * 4;
     // largest |c| of the chunk, rounded up: how far a track leaves its tangent line over the arc U
     const float cf = valid ? __double2float_ru(fabs(c)) : 0.f;
     const double cmax = (double)__uint_as_float(__reduce_max_sync(FULL, __float_as_uint(cf)));
@@ -138,13 +144,15 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     }
     const double zc0 = 0.5 * (zlo + zhi);
     const double zh = 0.5 * (zhi - zlo) * 1.000001 + 1e-9; // |z_k(seed) - (zc0 + k hz)| <= zh for every seed of the run
-    double zh_t[NU], tz_t[NU];
+    double zh_t[NU], tz_t[NU], zc_t[NU], hz_t[NU];
     int32_t np_t[NU];
     int32_t npmax = 0;
 #pragma unroll
     for (int t = 0; t < NU; ++t) {
         zh_t[t] = __shfl_sync(FULL, zh, t << ZSH);
         tz_t[t] = __shfl_sync(FULL, st.t2, t << ZSH);
+        zc_t[t] = __shfl_sync(FULL, zc0, t << ZSH);
+        hz_t[t] = __shfl_sync(FULL, hz, t << ZSH);
         np_t[t] = __shfl_sync(FULL, np, t << ZSH);
         npmax = max(npmax, np_t[t]);
     }
@@ -152,6 +160,30 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
 #pragma unroll
     for (int t = 0; t < NU; ++t)
         if (np_t[t] > 0) npmin = min(npmin, np_t[t]);
+
+    // staging: lane l copies the pieces p = l, l + 32, ... of a block: always of track l % NU
+    const int ts = lane & (NU - 1);
+    const int32_t np_s = __shfl_sync(FULL, np, ts << ZSH);
+    const double* const ub_s = a.ub + (size_t)(ug0 + ts) * (size_t)a.u_rows * 4;
+    const unsigned stg_sh = (unsigned)__cvta_generic_to_shared(stg);
+    auto stage = [&](int r0s, int buf) {
+        if (r0s < npmax && np_s > r0s) {                    // (rows up to the end of a track's last 64-row block exist: hold-last)
+            const double* src = ub_s + (size_t)r0s * 4;
+            const unsigned dst = stg_sh + (unsigned)(buf * BUFD * 8);
+#pragma unroll
+            for (int m = 0; m < 2 * NU; ++m) {
+                const int row = (lane >> (5 - ZSH)) + m * ZR;         // p / NU with p = lane + 32 m
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + (unsigned)((row * NU + ts) * 16)), "l"(src + (size_t)row * 4));
+            }
+            if (lane < NSUB * NU) {
+                const int j = lane >> (5 - ZSH);
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + (unsigned)((BLK * NU + j * NU + ts) * 16)),
+                             "l"(src + (size_t)(j * SUB + SUB / 2) * 4 + 2));
+            }
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    stage(0, 0);
 
     // pair keys of this chunk: nothing found yet
     unsigned long long* const keys = reinterpret_cast<unsigned long long*>(a.bd);
@@ -161,7 +193,13 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
         double* ckc = a.ck + (size_t)chunk * a.n_ck * COMET_LANES + lane;
         double z = z0;
         if (np > 0) ckc[0] = z;
-        for (int k0 = 1; k0 < npmax; k0 += CK) {
+        int k0 = 1;
+        for (; k0 + CK <= npmin; k0 += CK) {                // rows every seed of the chunk has
+#pragma unroll
+            for (int q = 0; q < CK; ++q) z = xadd(z, hz);
+            ckc[(size_t)((k0 + CK - 1) / CK) * COMET_LANES] = z;
+        }
+        for (; k0 < npmax; k0 += CK) {
 #pragma unroll
             for (int q = 0; q < CK; ++q) {
                 const int k = k0 + q;
@@ -179,29 +217,25 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
         if (valid) st_cnt[ST_PAIRS] = (unsigned long long)W;
     }
     const int n_rounds = (W + 31) / 32;
-    for (int r0 = 0; r0 < npmax; r0 += BLK) {
-        // ---- samples of the block: row 4 of every sub-block of every distinct track ------------------------
+    int buf = 0;
+    for (int r0 = 0; r0 < npmax; r0 += BLK, buf ^= 1) {
+        __syncwarp();                                       // everyone is done with the block staged two blocks ago
+        stage(r0 + BLK, buf ^ 1);
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncwarp();
+        const double* rows = stg + buf * BUFD;              // [64][NU][x, y]
+        const double* tang = rows + BLK * NU * 2;           // [8][NU][T_x, T_y]
+        const bool tail = r0 + BLK > npmin;                 // some track of the chunk ends in this block
+        const double r0d = (double)r0;
+        const double zb = fma(r0d, hz, z0);                 // the seed's z at row r0 (to rounding: shortlist only)
+        double zcb[NU];                                     // the run centre's z at row r0
 #pragma unroll
-        for (int q0 = 0; q0 < NS; q0 += 16) {
-            const int q = q0 + (lane >> 1), half = lane & 1;
-            const int src = (q >> 3) << ZSH;                 // a lane of the sample's run
-            const int32_t npq = __shfl_sync(FULL, np, src);
-            const double zcq = __shfl_sync(FULL, zc0, src), hzq = __shfl_sync(FULL, hz, src);
-            const unsigned long long ubq = __shfl_sync(FULL, (unsigned long long)ubl, src);
-            if (q < NS) {
-                const bool live = npq > r0;
-                const int kz = min(r0 + (q & 7) * SUB + SUB / 2, npq - 1);
-                double2 v = make_double2(0.0, 0.0);
-                if (live) v = __ldg(reinterpret_cast<const double2*>(reinterpret_cast<const double*>(ubq) + (size_t)kz * 4 + half * 2));
-                *reinterpret_cast<double2*>(samp + q * 6 + half * 2) = v;
-                samp[q * 6 + 4 + half] = half ? (live ? 1.0 : 0.0) : fma((double)kz, hzq, zcq);
-            }
-        }
-        __syncwarp();
-        const bool tail = r0 + BLK > npmin;                   // some track of the chunk ends in this block
-        const double zb = fma((double)r0, hz, z0);           // the seed's z at row r0 (to rounding: shortlist only)
-        // ---- level A (lane = wire): one sample per distinct track and block ----------------------------------
+        for (int t = 0; t < NU; ++t) zcb[t] = fma(r0d, hz_t[t], zc_t[t]);
+        // z of a sample: row r0 + kr of track t at the run's centre (a sample past the last state repeats it)
+        auto samp_z = [&](int t, int kr) {
+            if (!tail) return fma((double)kr, hz_t[t], zcb[t]);
+            return fma((double)min(kr, np_t[t] - 1 - r0), hz_t[t], zcb[t]);
+        };
         int cnt = 0;
         auto level_b = [&](const unsigned short* list, int n) {
             // ---- level B (lane = listed wire): tangent-line bound per (distinct track, sub-block) ------------
@@ -221,9 +255,9 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
 #pragma unroll
                     for (int j = 0; j < NSUB; ++j) {
                         if (np_t[t] <= r0 + j * SUB) break;          // the track has no row in this sub-block
-                        const double* sp = samp + (t * NSUB + j) * 6;
-                        const double2 xy = *reinterpret_cast<const double2*>(sp), tt = *reinterpret_cast<const double2*>(sp + 2);
-                        const double z = sp[4];
+                        const double2 xy = *reinterpret_cast<const double2*>(rows + ((j * SUB + SUB / 2) * NU + t) * 2);
+                        const double2 tt = *reinterpret_cast<const double2*>(tang + (j * NU + t) * 2);
+                        const double z = samp_z(t, j * SUB + SUB / 2);
                         const double a1 = fma(xy.x, ec.e1x, fma(xy.y, ec.e1y, fma(z, ec.e1z, ec.c1)));
                         const double a2 = fma(xy.x, ec.e2x, fma(xy.y, ec.e2y, fma(z, ec.e2z, ec.c2)));
                         const double b1 = fma(tt.x, ec.e1x, fma(tt.y, ec.e1y, bz1));
@@ -247,32 +281,36 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
                 // ---- wire iw, lane = seed: sweep the opened sub-blocks row by row ------------------------------
                 EvalC w;
                 zr_evalc<BIGW>(w, wtab, a.wt, W, iw);      // broadcast
+                // u_c = x e_cx + y e_cy + (z e_cz + c_c) with z = zb + kr hz: the bracket is A_c + kr D_c
+                const double A1 = fma(zb, w.e1z, w.c1), A2 = fma(zb, w.e2z, w.c2), D1 = hz * w.e1z, D2 = hz * w.e2z;
                 double best = INF;
                 int bk = -1;
                 while (msub) {
                     const int j = __ffs(msub) - 1;
                     msub &= msub - 1;
                     const int k0 = r0 + j * SUB;
-                    const double zk = fma((double)(j * SUB), hz, zb);
+                    const double kd = (double)(j * SUB);
+                    const double A1j = fma(kd, D1, A1), A2j = fma(kd, D2, A2);
+                    const double* pr = rows + ((j * SUB) * NU + tl) * 2;
                     if (STATS) { st_cnt[ST_ROWS_EXEC] += SUB; if (np > k0) st_cnt[ST_ROWS_NEEDED] += min(SUB, np - k0); }
                     if (!tail) {
-                        const double2* pr = reinterpret_cast<const double2*>(ubl + (size_t)k0 * 4);
-                        double2 xy[SUB];
-#pragma unroll
-                        for (int kk = 0; kk < SUB; ++kk) xy[kk] = __ldg(pr + kk * 2);
 #pragma unroll
                         for (int kk = 0; kk < SUB; ++kk) {
-                            const double d2 = d2_fma(w, xy[kk].x, xy[kk].y, fma((double)kk, hz, zk));
+                            const double2 xy = *reinterpret_cast<const double2*>(pr + kk * NU * 2);
+                            const double u1 = fma(xy.x, w.e1x, fma(xy.y, w.e1y, fma((double)kk, D1, A1j)));
+                            const double u2 = fma(xy.x, w.e2x, fma(xy.y, w.e2y, fma((double)kk, D2, A2j)));
+                            const double d2 = fma(u1, u1, u2 * u2);
                             if (d2 < best) { best = d2; bk = k0 + kk; }
                         }
                     } else {
                         // the block in which a track of the chunk ends: rows past the seed's last state stay out
                         const int nr = np - k0;
-                        const double2* pr = reinterpret_cast<const double2*>(ubl + (size_t)min(k0, max(np - 1, 0)) * 4);
 #pragma unroll
                         for (int kk = 0; kk < SUB; ++kk) {
-                            const double2 xy = __ldg(pr + (kk < nr ? kk * 2 : 0));
-                            const double d2 = d2_fma(w, xy.x, xy.y, fma((double)kk, hz, zk));
+                            const double2 xy = *reinterpret_cast<const double2*>(pr + kk * NU * 2);
+                            const double u1 = fma(xy.x, w.e1x, fma(xy.y, w.e1y, fma((double)kk, D1, A1j)));
+                            const double u2 = fma(xy.x, w.e2x, fma(xy.y, w.e2y, fma((double)kk, D2, A2j)));
+                            const double d2 = fma(u1, u1, u2 * u2);
                             if (kk < nr && d2 < best) { best = d2; bk = k0 + kk; }
                         }
                     }
@@ -280,6 +318,10 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
                 if (bk >= 0) atomicMin(keys + (size_t)iw * a.SP + s, pack_key(best, bk));
             }
         };
+        // ---- level A (lane = wire): one sample per distinct track and block ----------------------------------
+        double zs_a[NU];
+#pragma unroll
+        for (int t = 0; t < NU; ++t) zs_a[t] = samp_z(t, SROW);
         for (int r = 0; r < n_rounds; ++r) {
             const int i = r * 32 + lane;
             const int ii = min(i, W - 1);
@@ -291,9 +333,9 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
 #pragma unroll
             for (int t = 0; t < NU; ++t) {
                 if (np_t[t] <= r0) continue;
-                const double* sp = samp + (t * NSUB + SROW / SUB) * 6;
+                const double2 xy = *reinterpret_cast<const double2*>(rows + (SROW * NU + t) * 2);
                 const double thr = cap + zh_t[t] * swz + SROW * L + COMET_ZR_MARGIN;
-                pass = pass || (d2_fma(ec, sp[0], sp[1], sp[4]) <= thr * thr);
+                pass = pass || (d2_fma(ec, xy.x, xy.y, zs_a[t]) <= thr * thr);
                 if (STATS && cap >= 0.0) st_cnt[ST_SAMPLES] += 1;
             }
             if (any_nolip) pass = true;
@@ -310,6 +352,7 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
         }
         if (cnt) level_b(plist, cnt);
     }
+    asm volatile("cp.async.wait_all;" ::: "memory");
     __syncwarp();
     // ---- finish: far pairs take the cutoff, (chunk, wire) items with a near lane go to k_fine_ck -------
     constexpr int FB = 8;
@@ -346,7 +389,7 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
                     if (STATS) st_cnt[ST_FINE_EXEC] += 1;
                     if (!near && found) keys[pidx] = COMET_KEY_NONE;
                     if (lane == 0) lst[cnt] = (unsigned short)i;
-                    if (++cnt == LCAP) flush();
+                    if (++cnt == LCAPW) flush();
                 } else {
                     a.bd[pidx] = lam2;
                 }
