@@ -78,6 +78,8 @@ struct comet_ctx {
     size_t cw_bytes;
     double* tw;                  // T_z per seed of a slab (ZG variants)
     size_t tw_bytes;
+    unsigned int* tmk;           // [chunks][ceil(W / 32)] rows of the pair workspace that exist (scan_zrun.cuh)
+    size_t tm_bytes;
     int fused_smem;
     FieldMap field;              // field.B == nullptr: uniform field (the bz_tesla arguments)
     double* bmax;                // device scalar: largest |B| of the map
@@ -220,7 +222,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ub); cudaFree(ctx->npu);
     for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
     cudaFree(ctx->geom_a); cudaFree(ctx->geom_b);
-    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->tw); cudaFree(ctx->bmax);
+    cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->tw); cudaFree(ctx->tmk); cudaFree(ctx->bmax);
     for (int l = 0; l < COMET_MAX_LANES; ++l) {
         if (ctx->ls[l]) cudaStreamDestroy(ctx->ls[l]);
         if (ctx->lf[l]) cudaStreamDestroy(ctx->lf[l]);
@@ -568,7 +570,7 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
             if (ctx->opt_stats) k_fine<true><<<b2, COMET_FINE_THREADS, 0, st>>>(pa);
             else k_fine<false><<<b2, COMET_FINE_THREADS, 0, st>>>(pa);
             if (tm) CU(ctx, cudaEventRecord(tev[2], st));
-            k_rss_sum<<<(unsigned)((pa.d.n_seeds + 255) / 256), 256, 0, st>>>(pa.e2, pa.SP, n_fired, pa.d.n_seeds, pa.d.rss);
+            k_rss_sum<<<(unsigned)((pa.d.n_seeds + 255) / 256), 256, 0, st>>>(pa.e2, pa.SP, n_fired, pa.d.n_seeds, pa.d.rss, nullptr, 0.0, nullptr);
             if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }
             CU(ctx, cudaGetLastError());
         }
@@ -598,7 +600,7 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
 struct ScanWs {
     int64_t slab_chunks;
     int32_t n_ck;
-    size_t ck_chunk, pairs, ck, cw, ub, npu, tw, npw;
+    size_t ck_chunk, pairs, ck, cw, ub, npu, tw, npw, tm;
     int32_t tpc, u_rows;      // distinct tracks per chunk the workspace is sized for, rows per track
     bool zgroup;
 };
@@ -633,13 +635,14 @@ static ScanWs scan_ws(const comet_ctx* ctx, int64_t total_chunks, int32_t n_step
     w.ub = w.zgroup ? tracks * (size_t)w.u_rows * 4 * sizeof(double) : 0;
     w.npu = w.zgroup ? tracks * sizeof(int32_t) : 0;
     w.tw = w.zgroup ? w.cw : 0;
+    w.tm = w.zgroup ? (size_t)slab_chunks * (size_t)((n_fired + 31) / 32 + 1) * sizeof(unsigned int) : 0;
     return w;
 }
 
 static bool scan_ws_fits(const comet_ctx* ctx, const ScanWs& w)
 {
     return w.pairs <= ctx->pair_cap && w.ck <= ctx->ck_bytes && w.cw <= ctx->cw_bytes && w.ub <= ctx->ub_bytes &&
-           w.npu <= ctx->npu_bytes && w.tw <= ctx->tw_bytes && w.npw <= ctx->npw_cap * sizeof(int32_t);
+           w.npu <= ctx->npu_bytes && w.tw <= ctx->tw_bytes && w.tm <= ctx->tm_bytes && w.npw <= ctx->npw_cap * sizeof(int32_t);
 }
 
 static int grow_dev(comet_ctx* ctx, void** buf, size_t* have, size_t need)
@@ -663,6 +666,7 @@ static int scan_ws_grow(comet_ctx* ctx, const ScanWs& w)
     if ((rc = grow_dev(ctx, (void**)&ctx->ub, &ctx->ub_bytes, w.ub))) return rc;
     if ((rc = grow_dev(ctx, (void**)&ctx->npu, &ctx->npu_bytes, w.npu))) return rc;
     if ((rc = grow_dev(ctx, (void**)&ctx->tw, &ctx->tw_bytes, w.tw))) return rc;
+    if ((rc = grow_dev(ctx, (void**)&ctx->tmk, &ctx->tm_bytes, w.tm))) return rc;
     size_t have = ctx->npw_cap * sizeof(int32_t);
     if ((rc = grow_dev(ctx, (void**)&ctx->npw, &have, w.npw))) return rc;
     ctx->npw_cap = have / sizeof(int32_t);
@@ -794,6 +798,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             a.zrun = zrun_host;
             a.ub = nullptr;
             a.np_u = nullptr;
+            a.tm = nullptr;
             a.u_rows = ws.u_rows;
             FusedArgs az = a;                                   // the arguments of the z-run kernels
             if (zgroup) {
@@ -802,6 +807,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 // found on the device and the kernels that are not needed exit at once
                 az.ub = ctx->ub + (size_t)cl * ws.tpc * (size_t)ws.u_rows * 4;
                 az.np_u = ctx->npu + (size_t)cl * ws.tpc;
+                az.tm = ctx->tmk + (size_t)cl * (size_t)((n_fired + 31) / 32);
                 az.n_ck = n_steps / COMET_ZR_CK + 1;             // z checkpoints only, inside the sub-slab's checkpoint region
                 if (!zrun_host) {
                     az.zg = ctx->zg_flag + l;
@@ -818,10 +824,10 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 const int zthr = 32 * COMET_ZR_WARPS;
 #define COMET_LAUNCH_ZRUN(NU)                                                                                         \
                 do {                                                                                                  \
-                    if (a.stats) { if (bigw) k_scan_zrun<true, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU), s_scan>>>(az);     \
-                                   else k_scan_zrun<true, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU), s_scan>>>(az); }       \
-                    else { if (bigw) k_scan_zrun<false, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU), s_scan>>>(az);            \
-                           else k_scan_zrun<false, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU), s_scan>>>(az); }              \
+                    if (a.stats) { if (bigw) k_scan_zrun<true, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired), s_scan>>>(az);     \
+                                   else k_scan_zrun<true, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired), s_scan>>>(az); }       \
+                    else { if (bigw) k_scan_zrun<false, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired), s_scan>>>(az);            \
+                           else k_scan_zrun<false, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired), s_scan>>>(az); }              \
                 } while (0)
                 if (!zrun_host || zrun_host == 32) COMET_LAUNCH_ZRUN(1);
                 if (!zrun_host || zrun_host == 16) COMET_LAUNCH_ZRUN(2);
@@ -858,7 +864,8 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 }
             }
             if (tm) CU(ctx, cudaEventRecord(tev[2], st));
-            k_rss_sum<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_fine>>>(a.bd, a.SP, n_fired, a.n_seeds, rss + s0);
+            k_rss_sum<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_fine>>>(a.bd, a.SP, n_fired, a.n_seeds, rss + s0,
+                                                                              zgroup ? az.tm : nullptr, cutoff_cm * cutoff_cm, az.zg);
             if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }
             if (lanes > 1) CU(ctx, cudaEventRecord(ctx->ev_join[l], s_fine));
             CU(ctx, cudaGetLastError());

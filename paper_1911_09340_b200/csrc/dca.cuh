@@ -573,15 +573,32 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, COMET_FINE_MINB) k_fine(co
     }
 }
 
-// B5: RSS_s = sum_i e^2_i in increasing wire order (Eq. (1); no atomics, cf. :374)
+// B5: RSS_s = sum_i e^2_i in increasing wire order (Eq. (1); no atomics, cf. :374).
+// tm != nullptr (scan_zrun.cuh): bit i of the chunk's mask says whether the row of wire i exists; every other pair is
+// beyond the far radius and contributes cutoff^2 = lam2 without a load.
 __global__ void __launch_bounds__(256) k_rss_sum(const double* __restrict__ e2, int64_t SP, int32_t W,
-                                                 int64_t n_seeds, double* __restrict__ rss)
+                                                 int64_t n_seeds, double* __restrict__ rss,
+                                                 const unsigned int* __restrict__ tm, double lam2,
+                                                 const unsigned int* __restrict__ zg)
 {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n_seeds) return;
     double acc = 0.0;
+    // (zg: the run length found on the device -- the mask exists only if the z-run kernel served the launch)
+    if (tm && (!zg || *zg >= 8u)) {
+        const int MW = (W + 31) / 32;
+        const unsigned int* m = tm + (size_t)(s >> 5) * MW;
+        for (int wd = 0; wd < MW; ++wd) {
+            const unsigned bits = __ldg(m + wd);
+            const int n = min(32, W - wd * 32);
 #pragma unroll 4
-    for (int i = 0; i < W; ++i) acc = xadd(acc, e2[(size_t)i * SP + s]);
+            for (int j = 0; j < n; ++j)
+                acc = xadd(acc, ((bits >> j) & 1u) ? e2[(size_t)(wd * 32 + j) * SP + s] : lam2);
+        }
+    } else {
+#pragma unroll 4
+        for (int i = 0; i < W; ++i) acc = xadd(acc, e2[(size_t)i * SP + s]);
+    }
     rss[s] = acc;
 }
 

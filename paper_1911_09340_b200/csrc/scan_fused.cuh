@@ -105,7 +105,8 @@ struct FusedArgs {
     int32_t zrun;            //   or the caller's promise (comet_scan_rss z_run >= 8): `zg` is then nullptr
     double* ub;              // scan_zgroup.cuh: (x_0, x_1, T_0, T_1) of the distinct transverse tracks [u / 32][u_rows][4][32]
     int32_t* np_u;           //   and their numbers of recorded states
-    int32_t u_rows;          //   rows per track in ub: n_steps + 1
+    int32_t u_rows;          //   rows per track in ub: n_steps + 1 rounded up to whole 64-row blocks
+    unsigned int* tm;        // scan_zrun.cuh: [chunks][ceil(W / 32)] bit i: k_fine_ck fills the e^2 row of wire i (else cutoff^2)
 };
 #define COMET_ZG_MIN 8             // smallest run length served by the ZG kernels (scan_zgroup.cuh)
 __device__ __forceinline__ unsigned int zgroup_of(const unsigned int* flag)

@@ -29,7 +29,12 @@
 //              shared-memory load per row, broadcast to the seeds of the run), z = z_0 + k h T_z folded into the
 //              wire's constants, 8 FP64 instructions + compare per row, best (d^2, row) merged into the pair key
 //              with one atomic min as in k_scan_fused;
-//   finish     as in k_scan_fused.
+//   keys       a warp owns the 32 keys of a (chunk, wire) pair row: the first sweep of a wire stores them, later
+//              ones (another block) merge with a fire-and-forget atomic min; a bit per wire in the warp's shared
+//              memory remembers which rows exist.  Nothing is written for the wires that never pass level B;
+//   finish     only the touched rows are read back: a row with a lane within the far radius becomes an item of
+//              k_fine_ck, the others are dropped; the chunk's mask of rows k_fine_ck will fill goes to memory and
+//              k_rss_sum adds cutoff^2 for every other wire without reading anything.
 //
 // Only shortlists are decided here (FMA-form distances, slack 1e-6 cm on every bound): k_fine_ck<ZG> re-decides
 // between rows k-1, k, k+1 with the definition's exact operations, so n_pts and RSS are the bit-identical numbers
@@ -50,7 +55,9 @@ namespace comet {
 // doubles of shared memory per warp: two staged blocks of (64 rows + 8 sample tangents) x NU tracks x 2, the pass
 // list (64 shorts); the item list of the finish (LCAP shorts = 256 doubles) reuses the staged blocks
 #define COMET_ZR_WSM(NU) (2 * (64 + 8) * (NU) * 2 + 16)
-#define COMET_ZR_SMEM(NU) ((COMET_ZR_NF * COMET_ZR_WCAP + COMET_ZR_WARPS * COMET_ZR_WSM(NU)) * (int)sizeof(double))
+// + the touched-wire mask: one bit per fired wire, rounded up to whole 16 bytes
+#define COMET_ZR_MWD(W) ((((W) + 31) / 32 + 3) / 4 * 2)
+#define COMET_ZR_SMEM(NU, W) ((COMET_ZR_NF * COMET_ZR_WCAP + COMET_ZR_WARPS * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W))) * (int)sizeof(double))
 #define COMET_ZR_MARGIN 1e-6       // cm, added to every pruning threshold (FMA rounding is ~1e-13)
 
 template <bool BIGW>
@@ -89,11 +96,13 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     extern __shared__ __align__(16) double zsm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* wtab = zsm;                                     // [NF][WCAP]
-    double* stg = zsm + NF * WCAP + warp * COMET_ZR_WSM(NU);      // two staged blocks
+    const int W = a.W;
+    const int MW = (W + 31) / 32;                           // words of the touched-wire mask
+    double* stg = zsm + NF * WCAP + warp * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W));   // two staged blocks
     unsigned short* plist = reinterpret_cast<unsigned short*>(stg + 2 * BUFD);     // [64] wires that passed level A
+    unsigned* tmask = reinterpret_cast<unsigned*>(stg + 2 * BUFD + 16);            // [MW] bit i: the key row of wire i exists
     unsigned short* lst = reinterpret_cast<unsigned short*>(stg);                  // finish: [<= LCAP] items
     constexpr int LCAPW = (NU == 1) ? (2 * BUFD * 4) : LCAP;                       // shorts the staged blocks hold
-    const int W = a.W;
     for (int v = threadIdx.x; v < COMET_FUSED_WFIELDS * WCAP; v += 32 * COMET_ZR_WARPS) {
         const int f = v / WCAP, i = v - f * WCAP;
         wtab[v] = (i < W) ? __ldg(a.wt + (size_t)(6 + f) * W + i) : -1.0;
@@ -185,9 +194,9 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     };
     stage(0, 0);
 
-    // pair keys of this chunk: nothing found yet
+    // pair keys of this chunk: no row exists yet
     unsigned long long* const keys = reinterpret_cast<unsigned long long*>(a.bd);
-    for (int i = 0; i < W; ++i) keys[(size_t)i * a.SP + s] = COMET_KEY_NONE;
+    for (int w = lane; w < MW; w += 32) tmask[w] = 0u;
     // the seed's z column (Algorithm 1 for x_2), a checkpoint every CK rows
     {
         double* ckc = a.ck + (size_t)chunk * a.n_ck * COMET_LANES + lane;
@@ -315,7 +324,16 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
                         }
                     }
                 }
-                if (bk >= 0) atomicMin(keys + (size_t)iw * a.SP + s, pack_key(best, bk));
+                // the row's first sweep stores the keys, later ones merge (the warp owns the row)
+                const unsigned tw_ = tmask[iw >> 5];
+                if (!((tw_ >> (iw & 31)) & 1u)) {
+                    keys[(size_t)iw * a.SP + s] = bk >= 0 ? pack_key(best, bk) : COMET_KEY_NONE;
+                    __syncwarp();
+                    if (lane == 0) tmask[iw >> 5] = tw_ | (1u << (iw & 31));
+                    __syncwarp();
+                } else if (bk >= 0) {
+                    atomicMin(keys + (size_t)iw * a.SP + s, pack_key(best, bk));
+                }
             }
         };
         // ---- level A (lane = wire): one sample per distinct track and block ----------------------------------
@@ -354,7 +372,7 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     }
     asm volatile("cp.async.wait_all;" ::: "memory");
     __syncwarp();
-    // ---- finish: far pairs take the cutoff, (chunk, wire) items with a near lane go to k_fine_ck -------
+    // ---- finish: the touched rows are read back; a row with a near lane is an item of k_fine_ck ---------
     constexpr int FB = 8;
     int cnt = 0;                                            // warp-uniform
     auto flush = [&]() {
@@ -366,35 +384,43 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
         cnt = 0;
         __syncwarp();
     };
-    for (int i0 = 0; i0 < W; i0 += FB) {
-        unsigned long long kv[FB];
-        double cap2[FB];
+    for (int wd = 0; wd < MW; ++wd) {
+        const unsigned bits = tmask[wd];
+        unsigned keep = bits;                               // rows k_fine_ck will fill
+        const int nt = __popc(bits);
+        __syncwarp();
+        if ((bits >> lane) & 1u) plist[__popc(bits & ((1u << lane) - 1u))] = (unsigned short)(wd * 32 + lane);
+        __syncwarp();
+        for (int b0 = 0; b0 < nt; b0 += FB) {
+            unsigned long long kv[FB];
+            double cap2[FB];
+            int iw[FB];
 #pragma unroll
-        for (int j = 0; j < FB; ++j) {
-            const int i = min(i0 + j, W - 1);
-            kv[j] = __ldcg(keys + (size_t)i * a.SP + s);
-            const double cap = zr_const<BIGW>(wtab, a.wt, W, 8, i);
-            cap2[j] = cap * cap;
-        }
+            for (int j = 0; j < FB; ++j) {
+                iw[j] = (int)plist[min(b0 + j, nt - 1)];
+                kv[j] = __ldcg(keys + (size_t)iw[j] * a.SP + s);
+                const double cap = zr_const<BIGW>(wtab, a.wt, W, 8, iw[j]);
+                cap2[j] = cap * cap;
+            }
 #pragma unroll
-        for (int j = 0; j < FB; ++j) {
-            const int i = i0 + j;
-            if (i < W) {
-                const size_t pidx = (size_t)i * a.SP + s;
-                const bool found = kv[j] != COMET_KEY_NONE;
-                // key_d2 <= d^2 of the closest recorded state: "far" is decided on the safe side
-                const bool near = valid && found && (key_d2(kv[j]) <= cap2[j] || !lip_ok);
-                if (STATS && near) st_cnt[ST_FINE_NEEDED] += 1;
-                if (__any_sync(FULL, near)) {
-                    if (STATS) st_cnt[ST_FINE_EXEC] += 1;
-                    if (!near && found) keys[pidx] = COMET_KEY_NONE;
-                    if (lane == 0) lst[cnt] = (unsigned short)i;
-                    if (++cnt == LCAPW) flush();
-                } else {
-                    a.bd[pidx] = lam2;
+            for (int j = 0; j < FB; ++j) {
+                if (b0 + j < nt) {
+                    const bool found = kv[j] != COMET_KEY_NONE;
+                    // key_d2 <= d^2 of the closest recorded state: "far" is decided on the safe side
+                    const bool near = valid && found && (key_d2(kv[j]) <= cap2[j] || !lip_ok);
+                    if (STATS && near) st_cnt[ST_FINE_NEEDED] += 1;
+                    if (__any_sync(FULL, near)) {
+                        if (STATS) st_cnt[ST_FINE_EXEC] += 1;
+                        if (!near && found) keys[(size_t)iw[j] * a.SP + s] = COMET_KEY_NONE;
+                        if (lane == 0) lst[cnt] = (unsigned short)iw[j];
+                        if (++cnt == LCAPW) flush();
+                    } else {
+                        keep &= ~(1u << (iw[j] & 31));      // every lane is far: cutoff^2, nothing to store
+                    }
                 }
             }
         }
+        if (lane == 0) a.tm[(size_t)chunk * MW + wd] = keep;
     }
     if (cnt) flush();
     if (STATS) {
