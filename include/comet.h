@@ -88,20 +88,23 @@ int comet_reserve(comet_ctx* ctx, int64_t max_pairs_per_launch);
  * when it reallocates. */
 int comet_reserve_scan(comet_ctx* ctx, int64_t n_seeds, int32_t n_steps, int32_t n_fired);
 
-/* With COMET_OPT_TIMING = 1 the pruned comet_dca_rss records CUDA events on its stream around its
- * three kernels (once per seed slab).  Waits for the timed slabs and writes the mean device time in
- * milliseconds of k_coarse_pruned, k_fine and k_rss_sum over the most recent ones (at most 64 since
- * the option was set or the last read) to ms_host[0..n), n <= 3, their number to *n_calls (may be
- * NULL), and restarts the count.  COMET_EINVAL if no timed call was made. */
+/* With COMET_OPT_TIMING = 1 the pruned comet_dca_rss and comet_scan_rss record CUDA events on the caller's
+ * stream around their kernels (once per seed slab; comet_scan_rss then runs its sub-slabs one after the other).
+ * Waits for the timed slabs and writes the mean device time in milliseconds over the most recent ones (at most
+ * 64 since the option was set or the last read) to ms_host[0..n), n <= 4 -- [0] the closest-state search
+ * (k_coarse_pruned / k_scan_fused / k_scan_zrun), [1] the fine stage (k_fine / k_fine_ck), [2] k_rss_sum,
+ * [3] k_gen_unique (0 when the z-run kernels did not serve the call) --, their number to *n_calls (may be NULL),
+ * and restarts the count.  COMET_EINVAL if no timed call was made. */
 int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n, int32_t* n_calls);
 
 /* Copies the work counters accumulated by comet_dca_rss calls made with COMET_OPT_STATS = 1 to
- * out_host[0..n) (HOST, n <= 7) and synchronises the stream; reset != 0 zeroes them afterwards.
+ * out_host[0..n) (HOST, n <= 9) and synchronises the stream; reset != 0 zeroes them afterwards.
  * Counters are thread-level: [0] block/sub-block sample evaluations, [1] row evaluations a lane
  * needed, [2] row evaluations executed (a warp opens a sub-block when any lane needs it),
  * [3] (seed, wire) pairs that needed the virtual-plane iteration, [4] pairs for which a warp
  * executed it, [5] all pairs, [6] RKN4 steps of distinct transverse tracks (comet_scan_rss with
- * COMET_OPT_ZGROUP; 0 otherwise). */
+ * COMET_OPT_ZGROUP; 0 otherwise), [7] tangent-line tests of k_scan_zrun's level B (per wire, sub-block and
+ * distinct track; [0] then counts its level-A samples), [8] 32 x (chunk, wire) key rows it created. */
 int comet_read_stats(comet_ctx* ctx, uint64_t* out_host, int32_t n, int32_t reset, void* cuda_stream);
 
 /* ---- inhomogeneous field map and adaptive step (R29-R32) ------- */

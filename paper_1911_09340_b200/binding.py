@@ -35,7 +35,8 @@ OPT_STATS = 2
 OPT_TIMING = 3
 OPT_LANES = 4
 OPT_ZGROUP = 5
-STATS_FIELDS = ("samples", "rows_needed", "rows_executed", "fine_needed", "fine_executed", "pairs", "unique_states")
+STATS_FIELDS = ("samples", "rows_needed", "rows_executed", "fine_needed", "fine_executed", "pairs", "unique_states",
+                "samples_b", "touched")
 
 
 class CometError(RuntimeError):
@@ -221,13 +222,13 @@ class Comet:
         """comet_reserve_scan: sizes every workspace of comet_scan_rss & co.; later calls do not allocate."""
         self._check(self._L.comet_reserve_scan(self._h, int(n_seeds), int(n_steps), int(n_fired)))
 
-    def read_timing(self, names=("k_coarse_pruned", "k_fine", "k_rss_sum")) -> dict:
+    def read_timing(self, names=("k_coarse_pruned", "k_fine", "k_rss_sum", "k_gen_unique")) -> dict:
         """Mean device milliseconds per kernel of the latest (<= 64) seed slabs of comet_dca_rss (pruned:
         k_coarse_pruned, k_fine, k_rss_sum) or comet_scan_rss (k_scan_fused, k_fine_ck, k_rss_sum) made
         with OPT_TIMING = 1 (waits for them).  `names` labels the three slots."""
-        buf = (ctypes.c_float * 3)()
+        buf = (ctypes.c_float * 4)()
         n = ctypes.c_int32()
-        self._check(self._L.comet_read_timing(self._h, buf, 3, ctypes.byref(n)))
+        self._check(self._L.comet_read_timing(self._h, buf, 4, ctypes.byref(n)))
         out = {k: float(v) for k, v in zip(names, buf)}
         out["n_calls"] = int(n.value)
         return out

@@ -44,7 +44,7 @@ struct comet_ctx {
     int opt_stats;
     int opt_timing;
     int n_sm;
-    cudaEvent_t tev[COMET_TEV_RING][4];   // COMET_OPT_TIMING: around k_coarse_pruned, k_fine, k_rss_sum
+    cudaEvent_t tev[COMET_TEV_RING][5];   // COMET_OPT_TIMING: around (k_gen_unique,) the coarse / scan kernel, the fine kernel, k_rss_sum
     long long tev_count;         // timed comet_dca_rss slabs since the option was set / last read
     unsigned long long* stats;   // device [ST_N] work counters of the pruned kernels
     // pair workspace of the pruned path: shortlisted state and e^2 per (wire, seed)
@@ -152,8 +152,8 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     {
         const void* fk[8] = {(const void*)k_scan_fused<false, false>, (const void*)k_scan_fused<true, false>,
                              (const void*)k_scan_fused<false, true>, (const void*)k_scan_fused<true, true>,
-                             (const void*)k_scan_fused<false, false, false, true>, (const void*)k_scan_fused<true, false, false, true>,
-                             (const void*)k_scan_fused<false, true, false, true>, (const void*)k_scan_fused<true, true, false, true>};
+                             (const void*)k_scan_fused<false, false, true>, (const void*)k_scan_fused<true, false, true>,
+                             (const void*)k_scan_fused<false, true, true>, (const void*)k_scan_fused<true, true, true>};
         for (int j = 0; j < 8 && e == cudaSuccess; ++j) {
             e = cudaFuncSetAttribute(fk[j], cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(fk[j], cudaFuncAttributePreferredSharedMemoryCarveout, 100);
@@ -183,7 +183,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     const int pr_smem = COMET_PR_CAP_S * 3 * COMET_LANES * (int)sizeof(double);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coarse_pruned<COMET_PRUNED_WT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coarse_pruned<COMET_PRUNED_WT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
-    for (int j = 0; j < COMET_TEV_RING * 4 && e == cudaSuccess; ++j) e = cudaEventCreate(&ctx->tev[j / 4][j % 4]);
+    for (int j = 0; j < COMET_TEV_RING * 5 && e == cudaSuccess; ++j) e = cudaEventCreate(&ctx->tev[j / 5][j % 5]);
     // shared-memory opt-ins (done once here, never on the hot path)
     const int dca_smem = (2 * COMET_KT * 3 * COMET_LANES + COMET_DCA_WARPS * 4 * 32) * (int)sizeof(double);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
@@ -220,7 +220,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaSetDevice(ctx->device);
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ub); cudaFree(ctx->npu);
-    for (int j = 0; j < COMET_TEV_RING * 4; ++j) if (ctx->tev[j / 4][j % 4]) cudaEventDestroy(ctx->tev[j / 4][j % 4]);
+    for (int j = 0; j < COMET_TEV_RING * 5; ++j) if (ctx->tev[j / 5][j % 5]) cudaEventDestroy(ctx->tev[j / 5][j % 5]);
     cudaFree(ctx->geom_a); cudaFree(ctx->geom_b);
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->tw); cudaFree(ctx->tmk); cudaFree(ctx->bmax);
     for (int l = 0; l < COMET_MAX_LANES; ++l) {
@@ -275,18 +275,20 @@ extern "C" int comet_get_option(const comet_ctx* ctx, int option, int* value)
 
 extern "C" int comet_read_timing(comet_ctx* ctx, float* ms_host, int32_t n, int32_t* n_calls)
 {
-    if (!ctx || !ms_host || n < 0 || n > 3) return COMET_EINVAL;
+    if (!ctx || !ms_host || n < 0 || n > 4) return COMET_EINVAL;
     if (ctx->tev_count <= 0) return COMET_EINVAL;
     int rc = set_device(ctx);
     if (rc) return rc;
     const long long have = ctx->tev_count < COMET_TEV_RING ? ctx->tev_count : COMET_TEV_RING;
-    double acc[3] = {0.0, 0.0, 0.0};
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
     for (long long r = ctx->tev_count - have; r < ctx->tev_count; ++r) {
         cudaEvent_t* ev = ctx->tev[r % COMET_TEV_RING];
-        CU(ctx, cudaEventSynchronize(ev[3]));
+        CU(ctx, cudaEventSynchronize(ev[4]));
+        // slots: coarse / scan kernel, fine kernel, k_rss_sum, then k_gen_unique (0 when it did not run)
+        const int a0[4] = {1, 2, 3, 0};
         for (int j = 0; j < n; ++j) {
             float ms = 0.f;
-            CU(ctx, cudaEventElapsedTime(&ms, ev[j], ev[j + 1]));
+            CU(ctx, cudaEventElapsedTime(&ms, ev[a0[j]], ev[a0[j] + 1]));
             acc[j] += ms;
         }
     }
@@ -563,15 +565,15 @@ extern "C" int comet_dca_rss(comet_ctx* ctx, const void* track, const int32_t* n
             const unsigned b2 = (unsigned)(b2_all < ctx->fine_blocks ? b2_all : ctx->fine_blocks);
             const bool tm = ctx->opt_timing != 0;
             cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
-            if (tm) CU(ctx, cudaEventRecord(tev[0], st));
+            if (tm) { CU(ctx, cudaEventRecord(tev[0], st)); CU(ctx, cudaEventRecord(tev[1], st)); }
             if (ctx->opt_stats) k_coarse_pruned<COMET_PRUNED_WT, true><<<b1, COMET_PR_WARPS * 32, sm1, st>>>(pa);
             else k_coarse_pruned<COMET_PRUNED_WT, false><<<b1, COMET_PR_WARPS * 32, sm1, st>>>(pa);
-            if (tm) CU(ctx, cudaEventRecord(tev[1], st));
+            if (tm) CU(ctx, cudaEventRecord(tev[2], st));
             if (ctx->opt_stats) k_fine<true><<<b2, COMET_FINE_THREADS, 0, st>>>(pa);
             else k_fine<false><<<b2, COMET_FINE_THREADS, 0, st>>>(pa);
-            if (tm) CU(ctx, cudaEventRecord(tev[2], st));
+            if (tm) CU(ctx, cudaEventRecord(tev[3], st));
             k_rss_sum<<<(unsigned)((pa.d.n_seeds + 255) / 256), 256, 0, st>>>(pa.e2, pa.SP, n_fired, pa.d.n_seeds, pa.d.rss, nullptr, 0.0, nullptr);
-            if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }
+            if (tm) { CU(ctx, cudaEventRecord(tev[4], st)); ctx->tev_count += 1; }
             CU(ctx, cudaGetLastError());
         }
         return COMET_OK;
@@ -790,6 +792,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             if (b2 < 1) b2 = 1;
             cudaEvent_t* tev = ctx->tev[ctx->tev_count % COMET_TEV_RING];
             if (tm) CU(ctx, cudaEventRecord(tev[0], st));
+            if (tm && !zgroup) CU(ctx, cudaEventRecord(tev[1], st));    // (no k_gen_unique: an empty slot)
             const int thr = 32 * COMET_FUSED_WARPS;
             // a launch that cannot give every SM two CTAs of four chunks: the CTA's warps share one chunk's wires
             const bool split = !zgroup && n_fired > 32 && nc < (int64_t)COMET_FUSED_WARPS * ctx->n_sm * 2;
@@ -819,6 +822,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 const unsigned bu = (unsigned)(((a.n_seeds + zr_min - 1) / zr_min + 31) / 32);  // one warp per CTA: a latency-bound chain
                 if (a.stats) k_gen_unique<true><<<bu, 32, 0, s_scan>>>(az);
                 else k_gen_unique<false><<<bu, 32, 0, s_scan>>>(az);
+                if (tm) CU(ctx, cudaEventRecord(tev[1], st));
                 const bool bigw = n_fired > COMET_ZR_WCAP;
                 const unsigned bz = (unsigned)((nc + COMET_ZR_WARPS - 1) / COMET_ZR_WARPS);
                 const int zthr = 32 * COMET_ZR_WARPS;
@@ -838,11 +842,11 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 // (the ZG kernels serve the launch: the plain variants are not enqueued)
             } else if (split) {
                 if (field) {
-                    if (a.stats) k_scan_fused<true, true, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
-                    else k_scan_fused<false, true, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                    if (a.stats) k_scan_fused<true, true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                    else k_scan_fused<false, true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
                 } else {
-                    if (a.stats) k_scan_fused<true, false, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
-                    else k_scan_fused<false, false, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                    if (a.stats) k_scan_fused<true, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                    else k_scan_fused<false, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
                 }
             } else if (field) {
                 if (a.stats) k_scan_fused<true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
@@ -851,7 +855,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 if (a.stats) k_scan_fused<true, false><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
                 else k_scan_fused<false, false><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
             }
-            if (tm) CU(ctx, cudaEventRecord(tev[1], st));
+            if (tm) CU(ctx, cudaEventRecord(tev[2], st));
             if (lanes > 1) {
                 CU(ctx, cudaEventRecord(ctx->ev_scan[l], s_scan));
                 CU(ctx, cudaStreamWaitEvent(s_fine, ctx->ev_scan[l], 0));
@@ -863,10 +867,10 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                     if (!zrun_host) k_fine_ck<false><<<b2, COMET_FINE_THREADS, 0, s_fine>>>(a);
                 }
             }
-            if (tm) CU(ctx, cudaEventRecord(tev[2], st));
+            if (tm) CU(ctx, cudaEventRecord(tev[3], st));
             k_rss_sum<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_fine>>>(a.bd, a.SP, n_fired, a.n_seeds, rss + s0,
                                                                               zgroup ? az.tm : nullptr, cutoff_cm * cutoff_cm, az.zg);
-            if (tm) { CU(ctx, cudaEventRecord(tev[3], st)); ctx->tev_count += 1; }
+            if (tm) { CU(ctx, cudaEventRecord(tev[4], st)); ctx->tev_count += 1; }
             if (lanes > 1) CU(ctx, cudaEventRecord(ctx->ev_join[l], s_fine));
             CU(ctx, cudaGetLastError());
             used = l + 1;

@@ -316,7 +316,7 @@ __device__ __forceinline__ double d2_fma(const EvalC& w, double x0, double x1, d
 }
 
 // optional work counters (COMET_OPT_STATS), thread-level
-enum { ST_SAMPLES = 0, ST_ROWS_NEEDED, ST_ROWS_EXEC, ST_FINE_NEEDED, ST_FINE_EXEC, ST_PAIRS, ST_UNIQUE, ST_N };
+enum { ST_SAMPLES = 0, ST_ROWS_NEEDED, ST_ROWS_EXEC, ST_FINE_NEEDED, ST_FINE_EXEC, ST_PAIRS, ST_UNIQUE, ST_SAMPLES_B, ST_TOUCHED, ST_N };
 
 struct PrunedArgs {
     DcaArgs d;

@@ -53,12 +53,6 @@ namespace comet {
 #ifndef COMET_FUSED_WCAP
 #define COMET_FUSED_WCAP 96        // wires whose constants the shared-memory table holds (the others: L1/L2)
 #endif
-#ifndef COMET_FUSED_MINB_ZG
-#define COMET_FUSED_MINB_ZG 4      // (5 CTAs per SM fit the smaller tile of the ZG variant but 96 registers cost more than they gain)
-#endif
-#define COMET_ZG_RING 4            // compact tiles fetched ahead (scan_zgroup.cuh)
-#define COMET_ZG_SLOT 128          // doubles per compact tile: [16 rows][x, y][4 distinct tracks]
-#define COMET_ZG_WTILE (COMET_FUSED_TR * 32 + COMET_ZG_RING * COMET_ZG_SLOT)   // doubles per warp in the ZG variant
 #define COMET_FUSED_WFIELDS 9      // e1[3] -m.e1 | e2[3] -m.e2 | far radius  (fields 6..14 of the wire table)
 // the CTA's table has one more row: sqrt(1 - w_z^2) rounded up, the wire's slope against the z axis
 
@@ -145,12 +139,11 @@ __device__ __forceinline__ double wire_slope(double e1z, double e2z)
     return (double)__fsqrt_ru(__double2float_ru(fma(e1z, e1z, e2z * e2z)));
 }
 
-// ZG = true: the rows of a tile are not generated here: (x, y) come from the distinct transverse tracks of
-// k_gen_unique and z is accumulated per seed (scan_zgroup.cuh); everything after the tile is the same code.
-template <bool STATS, bool FIELD, bool ZG = false, bool SPLIT = false>
-__global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_ZG : COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
+// (Seed sets in z-runs are served by k_scan_zrun, scan_zrun.cuh; with the run length found on the device both kernels
+// are enqueued and the one that does not serve the launch returns at once.)
+template <bool STATS, bool FIELD, bool SPLIT = false>
+__global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_scan_fused(const FusedArgs a)
 {
-    static_assert(!(FIELD && ZG), "the transverse motion depends on z in a field map");
     constexpr int CKF = COMET_CK_FIELDS(FIELD);
     constexpr int TR = COMET_FUSED_TR, CK = COMET_CK_ROWS(FIELD), ROW = 3 * COMET_LANES;
     constexpr int FM1 = COMET_FUSED_M1;
@@ -158,15 +151,11 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     constexpr int WCAP = COMET_FUSED_WCAP;
     constexpr unsigned FULL = 0xffffffffu;
     static_assert(TR % FM1 == 0 && TR % CK == 0, "tile rows");
-    if (ZG) {
-        if (zrun_of(a.zrun, a.zg) < COMET_ZG_MIN) return;   // the plain kernel serves this launch
-    } else if (!FIELD && a.zg && zgroup_of(a.zg) >= COMET_ZG_MIN) {
-        return;                                             // the ZG kernels serve this launch (scan_zgroup.cuh)
-    }
+    if (!FIELD && a.zg && zgroup_of(a.zg) >= COMET_ZG_MIN) return;     // the z-run kernels serve this launch (scan_zrun.cuh)
     extern __shared__ __align__(16) double fsm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* wtab = fsm;                                     // [WFIELDS + 1][WCAP]
-    double* tile = fsm + (COMET_FUSED_WFIELDS + 1) * WCAP + warp * (ZG ? COMET_ZG_WTILE : TR * ROW);
+    double* tile = fsm + (COMET_FUSED_WFIELDS + 1) * WCAP + warp * (TR * ROW);
     const int W = a.W;
     for (int v = threadIdx.x; v < COMET_FUSED_WFIELDS * WCAP; v += 32 * COMET_FUSED_WARPS) {
         const int f = v / WCAP, i = v - f * WCAP;
@@ -178,7 +167,6 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     // SPLIT (small launches that cannot fill the GPU: the refined seed sets of a stage): the CTA's warps all take
     // the SAME chunk -- each generates the track for itself -- and share its wires: warp w takes the level-0 rounds
     // and the finish groups w, w + 4, ...; one chunk is then a quarter of the serial work per warp
-    static_assert(!(ZG && SPLIT), "the z-run variant serves large launches only");
     constexpr bool split = SPLIT;
     const int wpart = split ? warp : 0, nparts = split ? COMET_FUSED_WARPS : 1;
     const int64_t chunk = split ? (int64_t)blockIdx.x : (int64_t)blockIdx.x * COMET_FUSED_WARPS + warp;
@@ -203,59 +191,9 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     const bool lip_ok = (FIELD ? fabs(c) * __ldg(a.F.bmax) * h : fabs(c) * h) <= COMET_CH_MAX;
     const unsigned nolip_mask = __ballot_sync(FULL, valid && !lip_ok);
     double htry = h;                                        // FIELD: trial step of the adaptive control (R31)
-    bool active = valid && !ZG;
+    bool active = valid;
     int32_t np = valid ? a.n_steps + 1 : 0;
     const bool use_stop = a.r_stop2 > 0.0;
-    // ZG: the chunk's NU = 32 / ZG distinct transverse tracks, the seed's (final) number of recorded states and
-    // the z advance of a step.  The warp's shared memory holds the z column of the tile [TR][32] and a ring of
-    // ZRING compact tiles [16][2][4]: (x, y) of the 16 rows of every distinct track, fetched ZRING - 1 tiles ahead
-    // with cp.async from k_gen_unique's buffer.
-    constexpr int ZRING = COMET_ZG_RING, ZSLOT = COMET_ZG_SLOT;
-    const int n_tiles_zg = (a.n_steps + TR) / TR;
-    static_assert(TR == 16 && CK == 4 || !ZG, "compact tile layout");
-    double hz = 0.0;
-    int zshift = 5, nshift = 0, ul = 0;
-    int64_t ug0 = 0;
-    double* const zt = tile;                                // ZG: z column
-    double* const xr = tile + TR * 32;                      // ZG: ring of compact tiles
-    if (ZG) {
-        zshift = 31 - __clz((int)zrun_of(a.zrun, a.zg));
-        nshift = 5 - zshift;
-        ul = lane >> zshift;                                // the seed's distinct track within the chunk
-        ug0 = (chunk * COMET_LANES) >> zshift;              // the chunk's first distinct track
-        if (valid) {
-            np = a.np_u[ug0 + ul];
-            hz = xmul(h, st.t2);                            // x_2' = x_2 + h T_2, T_2 constant
-        }
-    }
-    // ZG: fetch the compact tile t (one cp.async group per call, possibly empty).  A lane always serves the same
-    // (component, distinct track) and walks the 20 row slots in steps of 32 / (2 NU), so everything but the row is
-    // fixed per lane: lane = (slot_low, comp, track).
-    const int f_eu = lane & ((1 << nshift) - 1), f_comp = (lane >> nshift) & 1, f_slot0 = lane >> (1 + nshift);
-    const int f_spi = 32 >> (1 + nshift);                   // slots per pass: 16, 8, 4
-    const int32_t f_np = ZG ? __shfl_sync(FULL, np, f_eu << zshift) : 0;
-    const double* f_src = nullptr;
-    if (ZG && f_np > 0) {
-        const int64_t ug = ug0 + f_eu;
-        f_src = a.ub + (size_t)(ug >> 5) * (size_t)a.u_rows * 128 + f_comp * 32 + (ug & 31);
-    }
-    const unsigned f_dst = (unsigned)__cvta_generic_to_shared(xr + f_comp * 4 + f_eu);
-    auto fetch_tile = [&](int t) {
-        if (t < n_tiles_zg) {
-            const int r0f = t * TR;
-            const unsigned dst_t = f_dst + (unsigned)((t % ZRING) * ZSLOT * 8);
-            for (int slot = f_slot0; slot < 16; slot += f_spi) {
-                const int k = r0f + slot;
-                if (f_np > 0) {                             // rows past n_pts - 1 repeat the last state
-                    const double* src = f_src + (size_t)min(k, f_np - 1) * 128;
-                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst_t + (unsigned)(slot * 64)), "l"(src));
-                } else {
-                    xr[(t % ZRING) * ZSLOT + slot * 8 + f_comp * 4 + f_eu] = 0.0;
-                }
-            }
-        }
-        asm volatile("cp.async.commit_group;" ::: "memory");
-    };
     // pair workspace of this chunk: nothing found yet
     unsigned long long* const keys = reinterpret_cast<unsigned long long*>(a.bd);
     for (int i = 32 * wpart; i < W; i += 32 * nparts)      // (the wires of this warp's rounds)
@@ -281,32 +219,9 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     for (int t = 0; t < n_tiles; ++t) {
         const int r0 = t * TR;
         PC_MARK();
-        const double* xc = xr + (t % ZRING) * ZSLOT + ul;     // ZG: compact tile t, this seed's distinct track
-        if (ZG) {
-            if (!__any_sync(FULL, np > r0)) break;
-            if (t == 0)
-                for (int q = 0; q < ZRING - 1; ++q) fetch_tile(q);
-            fetch_tile(t + ZRING - 1);
-            // ---- rows r0 .. r0 + TR - 1: the seed's own z column; (x, y) wait in the ring -------------------
-#pragma unroll
-            for (int rr = 0; rr < TR; ++rr) {
-                const int k = r0 + rr;
-                if (k > 0 && k < np) st.x2 = xadd(st.x2, hz);
-                zt[rr * 32 + lane] = st.x2;
-            }
-            asm volatile("cp.async.wait_group %0;" ::"n"(ZRING - 1) : "memory");
-            __syncwarp();
-            // checkpoints: z only -- k_fine_ck<.., ZG> takes (x, y, T_0, T_1) of the recorded states from the distinct
-            // tracks themselves (row stride 32 instead of 6 x 32 in the chunk's checkpoint block)
-#pragma unroll
-            for (int rr = 0; rr < TR; rr += CK) {
-                const int k = r0 + rr;
-                if (k < np) ckc[(size_t)(k / CK) * COMET_LANES] = zt[rr * 32 + lane];
-            }
-        }
         // ---- generate rows r0 .. r0 + TR - 1 (Algorithm 1; finished lanes hold their last state) ------
 #pragma unroll 2
-        for (int rr = 0; !ZG && rr < TR; ++rr) {
+        for (int rr = 0; rr < TR; ++rr) {
             const int k = r0 + rr;
             if (k > 0 && active) {
                 if (FIELD) (void)adaptive_field_step(st, htry, h, a.h_min, c, a.F);
@@ -341,8 +256,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
         for (int j = 0; j < NSUB; ++j) {
             const int srow = j * FM1 + FM1 / 2;
             const double* ps = tile + srow * ROW + lane;
-            const double s0 = ZG ? xc[(srow * 2) * 4] : ps[0], s1 = ZG ? xc[(srow * 2 + 1) * 4] : ps[32];
-            const double s2 = ZG ? zt[srow * 32 + lane] : ps[64];
+            const double s0 = ps[0], s1 = ps[32], s2 = ps[64];
             rx[j][0] = __shfl_sync(FULL, s0, rep); rx[j][1] = __shfl_sync(FULL, s1, rep); rx[j][2] = __shfl_sync(FULL, s2, rep);
             const double e0 = s0 - rx[j][0], e1 = s1 - rx[j][1], e2 = s2 - rx[j][2];
             const float fxy = is_live ? __fsqrt_ru(__double2float_ru(fma(e0, e0, e1 * e1))) : 0.f;
@@ -394,13 +308,10 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
 #endif
                     const double* pr = tile + (j * FM1) * ROW + lane;
                     if (STATS) { st_cnt[ST_ROWS_EXEC] += FM1; if (is_live) st_cnt[ST_ROWS_NEEDED] += FM1; }
-#pragma unroll
-                    const double* pxz = xc + (j * FM1) * 8;  // ZG: (x, y) of the sub-block's rows
-                    const double* pzz = zt + (j * FM1) * 32 + lane;
                     const int k0 = r0 + j * FM1;
+#pragma unroll
                     for (int kk = 0; kk < FM1; ++kk) {
-                        const double d2 = ZG ? d2_fma(w, pxz[kk * 8], pxz[kk * 8 + 4], pzz[kk * 32])
-                                             : d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
+                        const double d2 = d2_fma(w, pr[kk * ROW], pr[kk * ROW + 32], pr[kk * ROW + 64]);
                         if (d2 < best) { best = d2; bk = k0 + kk; }
                     }
                 }
@@ -413,7 +324,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
             PC_ADD(pc_l1);
         }
         __syncwarp();
-        if (!ZG && !__any_sync(FULL, active)) break;
+        if (!__any_sync(FULL, active)) break;
     }
 #ifdef COMET_FUSED_PROF
     if (lane == 0 && a.stats) {
@@ -423,8 +334,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, ZG ? COMET_FUSED_MINB_
     }
     PC_MARK();
 #endif
-    if (ZG) { asm volatile("cp.async.wait_all;" ::: "memory"); __syncwarp(); }
-    if (valid && wpart == 0) { a.n_pts[s] = np; a.cw[s] = c; if (ZG) a.tw[s] = st.t2; }
+    if (valid && wpart == 0) { a.n_pts[s] = np; a.cw[s] = c; }
     // ---- finish: far pairs take the cutoff, (chunk, wire) items with a near lane go to k_fine_ck -------
     // Keys come from L2: FB wires in flight at a time.  The items are collected in the (now free) tile
     // and appended to the work list with one reservation per LCAP items.

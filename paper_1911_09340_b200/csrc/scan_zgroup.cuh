@@ -44,61 +44,100 @@ k_zgroup_check(const double* __restrict__ seeds, int64_t stride, int64_t n, unsi
     if ((threadIdx.x & 31) == 0 && cand < 32u && cand < *(volatile unsigned int*)flag) atomicMin(flag, cand);
 }
 
-// One thread per distinct transverse track of the launch (unique u = seeds [u ZG, (u + 1) ZG)): Algorithm 1 for
-// (x_0, x_1, T_0, T_1), every recorded state to ub [u][row] = (x_0, x_1, T_0, T_1) -- 32 bytes per state, the rows of a
-// track contiguous, so that k_scan_zrun reads a sub-block of a track as 8 x 32 bytes and a sample with its tangent as one
-// row --, the number of recorded states to np_u.  Rows between the last state and the end of its 64-row block repeat it.
+// One thread per distinct transverse track of the launch (unique u = seeds [u ZG, (u + 1) ZG)), one warp per CTA:
+// Algorithm 1 for (x_0, x_1, T_0, T_1), every recorded state to ub [u][row] = (x_0, x_1, T_0, T_1) -- 32 bytes per state,
+// the rows of a track contiguous, so that k_scan_zrun reads a sub-block of a track as 8 x 32 bytes and a sample with its
+// tangent as one row --, the number of recorded states to np_u.  Rows between the last state and the end of its 64-row
+// block repeat it.  A lane's rows are 32 bytes at a stride of a whole track, so the warp records 8 steps in shared memory
+// and writes them out together: 256 contiguous bytes per track and flush instead of 32 scattered 32-byte stores per step.
+#define COMET_GU_ROWS 8
+#define COMET_GU_STRIDE (32 * 4 + 4)       // doubles per staged row (padded against bank conflicts)
 template <bool STATS>
-__global__ void __launch_bounds__(128) k_gen_unique(const FusedArgs a)
+__global__ void __launch_bounds__(32) k_gen_unique(const FusedArgs a)
 {
+    constexpr int GR = COMET_GU_ROWS, RS = COMET_GU_STRIDE;
+    constexpr unsigned FULL = 0xffffffffu;
+    __shared__ __align__(16) double sm[GR * RS];
     const unsigned int zg = zrun_of(a.zrun, a.zg);
     if (zg < COMET_ZG_MIN) return;                          // the plain k_scan_fused serves this launch
     const int zshift = 31 - __clz((int)zg);
-    const int64_t ug = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x;
+    const int64_t ug0 = (int64_t)blockIdx.x * 32;
+    const int64_t ug = ug0 + lane;
     const int64_t su = ug << zshift;
-    if (su >= a.n_seeds) return;
+    if ((ug0 << zshift) >= a.n_seeds) return;               // (warp-uniform)
+    const bool valid = su < a.n_seeds;
     State st;
-    const double c = seed_init(a.seeds, a.stride, su, a.qkb, st);
+    double c = 0.0;
+    if (valid) {
+        c = seed_init(a.seeds, a.stride, su, a.qkb, st);
+    } else {
+        st.x0 = st.x1 = st.t0 = st.t1 = 0.0;
+    }
     st.x2 = 0.0;                                            // z is the sweep kernel's business
     st.t2 = 0.0;
-    double2* o = reinterpret_cast<double2*>(a.ub + (size_t)ug * (size_t)a.u_rows * 4);
     const bool use_stop = a.r_stop2 > 0.0;
-    int32_t np = a.n_steps + 1;
-    o[0] = make_double2(st.x0, st.x1); o[1] = make_double2(st.t0, st.t1);
-    // The chain of dependent operations of a step is the whole cost here (one warp per CTA, nothing to overlap
-    // with), so the stop test must not sit on it: blocks of 4 steps are taken and recorded unconditionally -- rows
-    // past the stop are overwritten by the padding below -- and the first state in the target region, if any, ends
-    // the track afterwards.
-    State last = st;
-    int k = 1;
-    for (; k + 3 <= a.n_steps; k += 4) {
-        int first = 4;
+    int32_t np = valid ? a.n_steps + 1 : 1;                 // recorded states (a lane without a track records nothing new)
+    bool active = valid;
+    // flush of the staged rows k0 .. k0 + GR - 1: lane l writes the pieces p = l, l + 32, ... of 16 bytes; 16 consecutive
+    // pieces are the 8 rows of one track (256 contiguous bytes)
+    auto flush = [&](int k0, int nrows) {
+        __syncwarp();
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            rkn4_step(st, a.hk, c);
-            o[(size_t)(k + j) * 2] = make_double2(st.x0, st.x1); o[(size_t)(k + j) * 2 + 1] = make_double2(st.t0, st.t1);
+        for (int i = 0; i < GR * 2; ++i) {
+            const int p = i * 32 + lane;
+            const int trk = p >> 4, row = (p >> 1) & 7, half = p & 1;
+            const int64_t u = ug0 + trk;
+            if (row < nrows && (u << zshift) < a.n_seeds) {
+                const double2 v = *reinterpret_cast<const double2*>(sm + row * RS + trk * 4 + half * 2);
+                *reinterpret_cast<double2*>(a.ub + ((size_t)u * (size_t)a.u_rows + (size_t)(k0 + row)) * 4 + half * 2) = v;
+            }
+        }
+        __syncwarp();
+    };
+    auto put = [&](int row) {
+        double* o = sm + row * RS + lane * 4;
+        *reinterpret_cast<double2*>(o) = make_double2(st.x0, st.x1);
+        *reinterpret_cast<double2*>(o + 2) = make_double2(st.t0, st.t1);
+    };
+    // Rows k .. k + GR - 1 per round (row 0 is the seed state).  The chain of dependent operations of a step is the whole
+    // cost here, so the stop test must not sit on it: the steps of a round are taken and staged unconditionally, the first
+    // state in the target region, if any, is remembered, and the rows after it are overwritten with it afterwards (a
+    // finished lane holds its last state: the hold-last padding).
+    int k = 0;                                              // first row of the round
+    const int n_rows = a.n_steps + 1;
+    while (true) {
+        State last = st;
+        int first = GR;                                     // row of this round at which the lane stops
+#pragma unroll
+        for (int j = 0; j < GR; ++j) {
+            const int kk = k + j;
+            const bool stepping = active && kk > 0 && kk < n_rows;
+            if (stepping) rkn4_step(st, a.hk, c);
+            put(j);
             // in_target_region without its early exit: no branch waits for this step's position
             const double r2 = xadd(xmul(st.x0, st.x0), xmul(st.x1, st.x1));
             const double rad = xadd(xmul(st.x0, st.t0), xmul(st.x1, st.t1));
-            const bool stop = (r2 < a.r_stop2) & (rad < 0.0) & use_stop;
-            if (stop & (first == 4)) { first = j; last = st; }
+            const bool stop = stepping & (r2 < a.r_stop2) & (rad < 0.0) & use_stop;
+            if (stop & (first == GR)) { first = j; last = st; }
         }
-        if (first < 4) { np = k + first + 1; break; }
-        last = st;
-    }
-    if (np == a.n_steps + 1)
-        for (; k <= a.n_steps; ++k) {
-            rkn4_step(st, a.hk, c);
-            o[(size_t)k * 2] = make_double2(st.x0, st.x1); o[(size_t)k * 2 + 1] = make_double2(st.t0, st.t1);
-            last = st;
-            if (use_stop && in_target_region(st, a.r_stop2)) { np = k + 1; break; }
+        if (active && first < GR) {
+            np = k + first + 1;
+            active = false;
+            st = last;
+            for (int j = first + 1; j < GR; ++j) put(j);
+        } else if (active && k + GR >= n_rows) {
+            active = false;                                 // capacity reached: np stays n_steps + 1
         }
-    // hold-last padding up to the end of the 64-row block (u_rows is a multiple of 64)
-    for (int q = np; q < ((np + 63) & ~63); ++q) {
-        o[(size_t)q * 2] = make_double2(last.x0, last.x1); o[(size_t)q * 2 + 1] = make_double2(last.t0, last.t1);
+        flush(k, min(GR, a.u_rows - k));                    // (u_rows is a multiple of 64: whole rounds)
+        k += GR;
+        // go on while a lane is still stepping, then to the end of the 64-row block of the warp's longest track
+        if ((!__any_sync(FULL, active) && (k & 63) == 0) || k >= a.u_rows) break;
     }
-    a.np_u[ug] = np;
-    if (STATS && a.stats) atomicAdd(a.stats + ST_UNIQUE, (unsigned long long)(np - 1));
+    if (valid) {
+        a.np_u[ug] = np;
+        if (STATS && a.stats) atomicAdd(a.stats + ST_UNIQUE, (unsigned long long)(np - 1));
+    }
 }
 
 }  // namespace comet

@@ -277,7 +277,7 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
                         const double sv = fmin(ab, U * bb);
                         if (fma(aa - thr2, bb, -(sv * fma(2.0, ab, -sv))) <= 0.0) m8 |= 1u << j;
                     }
-                    if (STATS) st_cnt[ST_SAMPLES] += NSUB;
+                    if (STATS) st_cnt[ST_SAMPLES_B] += NSUB;
                 }
                 if (any_nolip) m8 = (1u << NSUB) - 1u;
             }
@@ -328,6 +328,7 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
                 const unsigned tw_ = tmask[iw >> 5];
                 if (!((tw_ >> (iw & 31)) & 1u)) {
                     keys[(size_t)iw * a.SP + s] = bk >= 0 ? pack_key(best, bk) : COMET_KEY_NONE;
+                    if (STATS) st_cnt[ST_TOUCHED] += 1;
                     __syncwarp();
                     if (lane == 0) tmask[iw >> 5] = tw_ | (1u << (iw & 31));
                     __syncwarp();
