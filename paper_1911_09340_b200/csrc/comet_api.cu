@@ -93,6 +93,14 @@ struct comet_ctx {
     size_t hbuf_bytes;
     void* tbuf;            // track slab
     size_t tbuf_bytes;
+    // the comet_scan_rss call whose distinct transverse tracks are still in `ub`, one slab, run length promised: the
+    // classification of the winners copies their rows instead of stepping them again (select.cuh)
+    struct {
+        const double* seeds;
+        int64_t stride, n_seeds;
+        double qkb, step, r_stop;
+        int32_t n_steps, zshift, u_rows, valid;
+    } last;
     // detector geometry kept on the device for the host-buffer entry points (comet_set_geometry)
     double* geom_a;
     double* geom_b;
@@ -661,6 +669,7 @@ static int grow_dev(comet_ctx* ctx, void** buf, size_t* have, size_t need)
 // grows the ctx's workspace to `w` (synchronises the device when anything is reallocated)
 static int scan_ws_grow(comet_ctx* ctx, const ScanWs& w)
 {
+    ctx->last.valid = 0;                                    // (the distinct-track rows may move)
     int rc = ensure_pairs(ctx, w.pairs, false);
     if (rc) return rc;
     if ((rc = grow_dev(ctx, (void**)&ctx->ck, &ctx->ck_bytes, w.ck))) return rc;
@@ -878,6 +887,14 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
         if (lanes > 1)
             for (int l = 0; l < used; ++l) CU(ctx, cudaStreamWaitEvent(st, ctx->ev_join[l], 0));
     }
+    ctx->last.valid = 0;
+    if (zrun_host && slab_chunks >= total_chunks && !seeds_host) {
+        ctx->last.seeds = seeds; ctx->last.stride = seed_stride; ctx->last.n_seeds = n_seeds;
+        ctx->last.qkb = COMET_KAPPA * (double)charge * bz_tesla; ctx->last.step = step_cm; ctx->last.r_stop = r_stop_cm;
+        ctx->last.n_steps = n_steps; ctx->last.u_rows = ws.u_rows;
+        ctx->last.zshift = zrun_host == 32 ? 5 : (zrun_host == 16 ? 4 : 3);
+        ctx->last.valid = 1;
+    }
     return COMET_OK;
 }
 
@@ -948,6 +965,12 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     if (field) a.qkb = COMET_KAPPA * (double)charge;
     a.F = ctx->field;
     a.h_min = step_cm / 64.0;
+    // the tracks of the scan that produced rss, if this is that seed set (same buffer, same physics)
+    a.ub = nullptr; a.np_u = nullptr; a.zshift = 0; a.u_rows = 0;
+    if (!field && ctx->last.valid && ctx->last.seeds == seeds && ctx->last.stride == seed_stride && ctx->last.n_seeds == n_seeds &&
+        ctx->last.qkb == a.qkb && ctx->last.step == step_cm && ctx->last.r_stop == r_stop_cm && ctx->last.n_steps == n_steps) {
+        a.ub = ctx->ub; a.np_u = ctx->npu; a.zshift = ctx->last.zshift; a.u_rows = ctx->last.u_rows;
+    }
     const size_t smem = (size_t)(n_steps + 1) * (field ? 7 : 6) * sizeof(double);
     if (field) k_select_classify<true><<<n_part, 256, smem, st>>>(a);
     else k_select_classify<false><<<n_part, 256, smem, st>>>(a);

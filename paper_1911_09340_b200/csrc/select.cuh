@@ -79,6 +79,11 @@ struct ClassifyArgs {
     uint8_t* cls;
     FieldMap F;                // field-map variants: the map; qkb = kappa q, hk.h = h_max
     double h_min;
+    // the distinct transverse tracks of the comet_scan_rss call that produced rss (scan_zgroup.cuh), when the ctx knows
+    // they are still those of `seeds`: the winner's (x, y, T_x, T_y) rows are copied instead of stepped again
+    const double* ub;          // [track][u_rows][4], nullptr = record the track here
+    const int32_t* np_u;
+    int32_t zshift, u_rows;
 };
 
 // CTA-wide: re-extrapolate seed `idx` into shared memory (state k at sm[k*6..]), then one thread per fired
@@ -97,6 +102,28 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
         for (int i = threadIdx.x; i < W; i += blockDim.x) dca[i] = __longlong_as_double(0x7ff8000000000000LL);
         return;
     }
+    if (!FIELD && a.ub) {
+        // the same numbers without the chain of 400-odd dependent RKN4 steps: (x, y, T_x, T_y) of every recorded state are
+        // the rows of the seed's distinct transverse track, z is one addition per step (x_2' = x_2 + h T_2)
+        State st;
+        const double c = seed_init(a.seeds, a.stride, idx, a.qkb, st);
+        const int64_t u = idx >> a.zshift;
+        const int32_t np = __ldg(a.np_u + u);
+        const double2* g = reinterpret_cast<const double2*>(a.ub + (size_t)u * (size_t)a.u_rows * 4);
+        for (int k = threadIdx.x; k < np; k += blockDim.x) {
+            const double2 xy = __ldg(g + 2 * k), tt = __ldg(g + 2 * k + 1);
+            double* o = sm + (size_t)k * RS;
+            o[0] = xy.x; o[1] = xy.y; o[3] = tt.x; o[4] = tt.y; o[5] = st.t2;
+        }
+        if (threadIdx.x == 0) {
+            s_c = c;
+            s_np = np;
+            const double hz = xmul(a.hk.h, st.t2);
+            double z = st.x2;
+            sm[2] = z;
+            for (int k = 1; k < np; ++k) { z = xadd(z, hz); sm[(size_t)k * RS + 2] = z; }
+        }
+    } else
     if (threadIdx.x == 0) {
         State st;
         const double c = seed_init(a.seeds, a.stride, idx, a.qkb, st);
@@ -136,16 +163,41 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
     __syncthreads();                                    // also orders the cls zeroing before the marks below
     const int32_t np = s_np;
     const double c = s_c;
-    for (int i = threadIdx.x; i < W; i += blockDim.x) {
+    // O5 for every wire: the recorded states are cut into NSEG segments per wire (NSEG threads per wire), the segment
+    // minima are merged in increasing row order with a strict <, i.e. the lowest row wins ties as in the serial scan
+    __shared__ double s_bd[256];
+    __shared__ int s_ks[256];
+    const int nthr = blockDim.x;
+    const int Wp = min(W, nthr);
+    const int NSEG = Wp > 0 ? nthr / Wp : 1;
+    for (int i0 = 0; i0 < W; i0 += Wp) {
+        const int wi = i0 + (int)threadIdx.x % Wp, seg = (int)threadIdx.x / Wp;
+        const bool on = wi < W && seg < NSEG;
         WireLine wl;
-        wl.m0 = a.wt[i]; wl.m1 = a.wt[W + i]; wl.m2 = a.wt[2 * W + i];
-        wl.w0 = a.wt[3 * W + i]; wl.w1 = a.wt[4 * W + i]; wl.w2 = a.wt[5 * W + i];
         int ks = 0;
         double bd = 0.0;
-        for (int k = 0; k < np; ++k) {
-            double u0, u1, u2;
-            const double d2 = perp2_exact(sm[k * RS], sm[k * RS + 1], sm[k * RS + 2], wl, u0, u1, u2);
-            if (k == 0 || d2 < bd) { bd = d2; ks = k; }
+        if (on) {
+            wl.m0 = a.wt[wi]; wl.m1 = a.wt[W + wi]; wl.m2 = a.wt[2 * W + wi];
+            wl.w0 = a.wt[3 * W + wi]; wl.w1 = a.wt[4 * W + wi]; wl.w2 = a.wt[5 * W + wi];
+            const int len = (np + NSEG - 1) / NSEG;
+            const int kb = seg * len, ke = min(np, kb + len);
+            ks = -1;
+            for (int k = kb; k < ke; ++k) {
+                double u0, u1, u2;
+                const double d2 = perp2_exact(sm[k * RS], sm[k * RS + 1], sm[k * RS + 2], wl, u0, u1, u2);
+                if (ks < 0 || d2 < bd) { bd = d2; ks = k; }
+            }
+        }
+        __syncthreads();
+        s_bd[threadIdx.x] = bd;
+        s_ks[threadIdx.x] = on ? ks : -1;
+        __syncthreads();
+        const int i = wi;
+        if (!(on && seg == 0)) continue;
+        for (int g2 = 1; g2 < NSEG; ++g2) {
+            const int k2 = s_ks[g2 * Wp + (int)threadIdx.x];
+            const double d2 = s_bd[g2 * Wp + (int)threadIdx.x];
+            if (k2 >= 0 && (ks < 0 || d2 < bd)) { bd = d2; ks = k2; }
         }
         State st;
         st.x0 = sm[ks * RS]; st.x1 = sm[ks * RS + 1]; st.x2 = sm[ks * RS + 2];
