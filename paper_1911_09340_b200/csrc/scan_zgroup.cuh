@@ -80,56 +80,61 @@ __global__ void __launch_bounds__(32) k_gen_unique(const FusedArgs a)
     int32_t np = valid ? a.n_steps + 1 : 1;                 // recorded states (a lane without a track records nothing new)
     bool active = valid;
     // flush of the staged rows k0 .. k0 + GR - 1: lane l writes the pieces p = l, l + 32, ... of 16 bytes; 16 consecutive
-    // pieces are the 8 rows of one track (256 contiguous bytes)
-    auto flush = [&](int k0, int nrows) {
+    // pieces are the 8 rows of one track (256 contiguous bytes).  Everything but the round is fixed per lane.
+    const int f_row = (lane >> 1) & 7, f_half = lane & 1, f_trk = lane >> 4;
+    const int64_t n_trk = (a.n_seeds + ((int64_t)1 << zshift) - 1) >> zshift;
+    const int n_here = (int)min((int64_t)32, n_trk - ug0);  // tracks of this warp
+    double* const f_dst = a.ub + ((size_t)(ug0 + f_trk) * (size_t)a.u_rows + (size_t)f_row) * 4 + f_half * 2;
+    const double* const f_src = sm + f_row * RS + f_trk * 4 + f_half * 2;
+    const size_t f_step = (size_t)2 * (size_t)a.u_rows * 4;                     // two tracks per pass
+    auto flush = [&](int k0) {
         __syncwarp();
+        double* d = f_dst + (size_t)k0 * 4;
 #pragma unroll
         for (int i = 0; i < GR * 2; ++i) {
-            const int p = i * 32 + lane;
-            const int trk = p >> 4, row = (p >> 1) & 7, half = p & 1;
-            const int64_t u = ug0 + trk;
-            if (row < nrows && (u << zshift) < a.n_seeds) {
-                const double2 v = *reinterpret_cast<const double2*>(sm + row * RS + trk * 4 + half * 2);
-                *reinterpret_cast<double2*>(a.ub + ((size_t)u * (size_t)a.u_rows + (size_t)(k0 + row)) * 4 + half * 2) = v;
-            }
+            if (2 * i + f_trk < n_here) *reinterpret_cast<double2*>(d + i * f_step) = *reinterpret_cast<const double2*>(f_src + i * 8);
         }
         __syncwarp();
     };
+    double* const my = sm + lane * 4;
     auto put = [&](int row) {
-        double* o = sm + row * RS + lane * 4;
-        *reinterpret_cast<double2*>(o) = make_double2(st.x0, st.x1);
-        *reinterpret_cast<double2*>(o + 2) = make_double2(st.t0, st.t1);
+        *reinterpret_cast<double2*>(my + row * RS) = make_double2(st.x0, st.x1);
+        *reinterpret_cast<double2*>(my + row * RS + 2) = make_double2(st.t0, st.t1);
     };
     // Rows k .. k + GR - 1 per round (row 0 is the seed state).  The chain of dependent operations of a step is the whole
-    // cost here, so the stop test must not sit on it: the steps of a round are taken and staged unconditionally, the first
-    // state in the target region, if any, is remembered, and the rows after it are overwritten with it afterwards (a
-    // finished lane holds its last state: the hold-last padding).
-    int k = 0;                                              // first row of the round
+    // cost here (one warp per CTA, about one warp per scheduler), so nothing may sit on it: every lane takes the steps of a
+    // round unconditionally -- straight-line code, the tail of one step overlaps the chain of the next -- and stages them;
+    // the first state in the target region, if any, is only remembered.  Afterwards a lane that stopped (in this round or
+    // before) overwrites the rows after its last state with it: the hold-last padding.
     const int n_rows = a.n_steps + 1;
+    int k = 0;                                              // first row of the round
     while (true) {
-        State last = st;
+        const State hold = st;                              // (what a finished lane keeps)
         int first = GR;                                     // row of this round at which the lane stops
 #pragma unroll
         for (int j = 0; j < GR; ++j) {
-            const int kk = k + j;
-            const bool stepping = active && kk > 0 && kk < n_rows;
-            if (stepping) rkn4_step(st, a.hk, c);
+            if (k + j > 0) {                                // (row 0: the seed state itself; warp-uniform)
+                rkn4_step(st, a.hk, c);
+                // in_target_region without its early exit: no branch waits for this step's position
+                const double r2 = xadd(xmul(st.x0, st.x0), xmul(st.x1, st.x1));
+                const double rad = xadd(xmul(st.x0, st.t0), xmul(st.x1, st.t1));
+                const bool stop = ((r2 < a.r_stop2) & (rad < 0.0) & use_stop) | (k + j == n_rows - 1);
+                first = (stop & (first == GR)) ? j : first;
+            }
             put(j);
-            // in_target_region without its early exit: no branch waits for this step's position
-            const double r2 = xadd(xmul(st.x0, st.x0), xmul(st.x1, st.x1));
-            const double rad = xadd(xmul(st.x0, st.t0), xmul(st.x1, st.t1));
-            const bool stop = stepping & (r2 < a.r_stop2) & (rad < 0.0) & use_stop;
-            if (stop & (first == GR)) { first = j; last = st; }
         }
-        if (active && first < GR) {
+        if (!active) {
+            st = hold;
+            for (int j = 0; j < GR; ++j) put(j);
+        } else if (first < GR) {
+            // (the capacity counts as a stop at row n_steps: np = n_steps + 1 either way)
             np = k + first + 1;
             active = false;
-            st = last;
+            const double2 xy = *reinterpret_cast<const double2*>(my + first * RS), tt = *reinterpret_cast<const double2*>(my + first * RS + 2);
+            st.x0 = xy.x; st.x1 = xy.y; st.t0 = tt.x; st.t1 = tt.y;
             for (int j = first + 1; j < GR; ++j) put(j);
-        } else if (active && k + GR >= n_rows) {
-            active = false;                                 // capacity reached: np stays n_steps + 1
         }
-        flush(k, min(GR, a.u_rows - k));                    // (u_rows is a multiple of 64: whole rounds)
+        flush(k);                                           // (u_rows is a multiple of 64: whole rounds)
         k += GR;
         // go on while a lane is still stepping, then to the end of the 64-row block of the warp's longest track
         if ((!__any_sync(FULL, active) && (k & 63) == 0) || k >= a.u_rows) break;
