@@ -345,11 +345,14 @@ size_t comet_turns_work_bytes(int64_t max_partition_seeds, int32_t n_fired, int3
  * than min_wires fired wires are left or max_tracks stages are done (paper: 30 and 5) (R34).
  *   turn_seed   dev [n_part][6], turn_rss dev [n_part]: the stage's best seed (NaN where no stage ran)
  *   turn_cls    dev [n_part][n_hits]: the hits given to each turn, in the event's own entry numbering
- *   done_host, wires_before_host  HOST [n_part]: 1 where a stage ran; fired wires it started with
+ *   done, wires_before  dev [n_part] int32: 1 where a stage ran; fired wires it started with (0 elsewhere)
  *   work        dev, comet_turns_work_bytes(largest partition, n_fired, n_hits, k_ref, n_grid)
  *   z_run       as in comet_scan_rss, used for the partitions that start on a run
- * Synchronises cuda_stream once per stage (the size of the reduced hit list sets the next launches),
- * as the paper's host loop does. */
+ * Only enqueues work: no host read, no synchronisation (the paper's host loop reads the reduced list back after
+ * every fit).  Every stage is launched for the event's own list sizes; the reduced list is padded back
+ * to n_fired wires with wires that have no entries, Eq. (1) runs over the wires that are left (a device counter), and
+ * once the stop rule has fired every kernel of the later stages returns at once.  With the workspace reserved
+ * (comet_reserve_scan) the whole loop can be captured into a CUDA graph. */
 int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
                      int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                      const double* wire_a, const double* wire_b, int32_t n_wires,
@@ -359,7 +362,7 @@ int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t seed_stride, i
                      const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
                      int32_t k_ref, int32_t min_wires, int32_t max_tracks, void* work,
                      double* turn_seed, double* turn_rss, uint8_t* turn_cls,
-                     int32_t* done_host, int32_t* wires_before_host, void* cuda_stream);
+                     int32_t* done, int32_t* wires_before, void* cuda_stream);
 
 /* ---- Hough-transform transverse seeding (Fig. 10; readings R35-R37) ------------ */
 

@@ -440,7 +440,7 @@ class Comet:
 
     def scan_turns(self, seeds, part_off, charge, bz, step, n_steps, r_stop, wire_a, wire_b, fired_wire, hit_off,
                    rho, cutoff, half_width, n_grid, n_iter, shrink, k_ref, min_wires=30, max_tracks=5, stream=None,
-                   z_run=0):
+                   z_run=0, work=None, sync=True):
         """comet_scan_turns: the last turn first, hits of a stage's best seed removed before the previous turn."""
         S = seeds.shape[1]
         po = np.ascontiguousarray(np.asarray(part_off, dtype=np.int64))
@@ -451,12 +451,13 @@ class Comet:
         nb = int(self._L.comet_turns_work_bytes(int(np.diff(po).max()), W, H, int(k_ref), ng.ctypes.data))
         if nb == 0:
             raise CometError("comet_turns_work_bytes: invalid arguments")
-        work = torch.empty(nb, dtype=torch.uint8, device=td)
-        out = {"turn_seed": torch.empty((P, 6), dtype=torch.float64, device=td),
+        if work is None:
+            work = torch.empty(nb, dtype=torch.uint8, device=td)
+        out = {"work": work, "turn_seed": torch.empty((P, 6), dtype=torch.float64, device=td),
                "turn_rss": torch.empty(P, dtype=torch.float64, device=td),
                "turn_cls": torch.empty((P, H), dtype=torch.uint8, device=td)}
-        done = np.zeros(P, dtype=np.int32)
-        wb = np.zeros(P, dtype=np.int32)
+        done = torch.empty(P, dtype=torch.int32, device=td)
+        wb = torch.empty(P, dtype=torch.int32, device=td)
         self._check(self._L.comet_scan_turns(
             self._h, _dev(seeds, torch.float64, "seeds", d), S, S, int(z_run), int(charge), float(bz), float(step),
             int(n_steps), float(r_stop),
@@ -465,9 +466,11 @@ class Comet:
             _dev(hit_off, torch.int32, "hit_off", d), _dev(rho, torch.float64, "rho", d), W, H, float(cutoff),
             po.ctypes.data, P, hw.ctypes.data, ng.ctypes.data, int(n_iter), float(shrink), int(k_ref),
             int(min_wires), int(max_tracks), int(work.data_ptr()), int(out["turn_seed"].data_ptr()),
-            int(out["turn_rss"].data_ptr()), int(out["turn_cls"].data_ptr()), done.ctypes.data, wb.ctypes.data,
+            int(out["turn_rss"].data_ptr()), int(out["turn_cls"].data_ptr()), int(done.data_ptr()), int(wb.data_ptr()),
             _stream_ptr(stream)))
-        out["done"], out["wires_before"] = done.astype(bool), wb
+        out["done_dev"], out["wires_before_dev"] = done, wb
+        if sync:                                             # (the call itself only enqueues: reading the flags back waits for it)
+            out["done"], out["wires_before"] = done.cpu().numpy().astype(bool), wb.cpu().numpy()
         return out
 
     # -- Hough-transform transverse seeding --------------------------------------------------------

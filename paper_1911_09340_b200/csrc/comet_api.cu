@@ -703,7 +703,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                          const double* wire_a, const double* wire_b, int32_t n_wires,
                          const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
                          int32_t n_fired, int32_t n_hits, double cutoff_cm,
-                         double* rss, int32_t* n_pts, void* cuda_stream)
+                         double* rss, int32_t* n_pts, void* cuda_stream, const int32_t* dyn = nullptr)
 {
     if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
         !(r_stop_cm >= 0.0) || bad_zrun(z_run) ||
@@ -788,6 +788,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             a.items = ctx->items + (size_t)cl * (size_t)n_fired;
             a.n_items = ctx->n_items + l;
             a.stats = ctx->opt_stats ? ctx->stats : nullptr;
+            a.dyn = dyn;
             if (lanes > 1) CU(ctx, cudaStreamWaitEvent(s_scan, ctx->ev_fork, 0));
             if (seeds_host)
                 for (int j = 0; j < 6; ++j)
@@ -878,7 +879,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             }
             if (tm) CU(ctx, cudaEventRecord(tev[3], st));
             k_rss_sum<<<(unsigned)((a.n_seeds + 255) / 256), 256, 0, s_fine>>>(a.bd, a.SP, n_fired, a.n_seeds, rss + s0,
-                                                                              zgroup ? az.tm : nullptr, cutoff_cm * cutoff_cm, az.zg);
+                                                                              zgroup ? az.tm : nullptr, cutoff_cm * cutoff_cm, az.zg, dyn);
             if (tm) { CU(ctx, cudaEventRecord(tev[4], st)); ctx->tev_count += 1; }
             if (lanes > 1) CU(ctx, cudaEventRecord(ctx->ev_join[l], s_fine));
             CU(ctx, cudaGetLastError());
@@ -966,7 +967,7 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     a.F = ctx->field;
     a.h_min = step_cm / 64.0;
     // the tracks of the scan that produced rss, if this is that seed set (same buffer, same physics)
-    a.ub = nullptr; a.np_u = nullptr; a.zshift = 0; a.u_rows = 0;
+    a.ub = nullptr; a.np_u = nullptr; a.zshift = 0; a.u_rows = 0; a.dyn = nullptr;
     if (!field && ctx->last.valid && ctx->last.seeds == seeds && ctx->last.stride == seed_stride && ctx->last.n_seeds == n_seeds &&
         ctx->last.qkb == a.qkb && ctx->last.step == step_cm && ctx->last.r_stop == r_stop_cm && ctx->last.n_steps == n_steps) {
         a.ub = ctx->ub; a.np_u = ctx->npu; a.zshift = ctx->last.zshift; a.u_rows = ctx->last.u_rows;
@@ -1075,10 +1076,12 @@ static int launch_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t se
                                  double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
                                  const int32_t* hit_off, const double* rho, int32_t n_fired, int32_t n_hits,
                                  double cutoff_cm, const int64_t* seed_idx, int32_t n_sel, const double* rss,
-                                 double* dca, uint8_t* cls, double* seed_out, double* rss_out, cudaStream_t st)
+                                 double* dca, uint8_t* cls, double* seed_out, double* rss_out, cudaStream_t st,
+                                 const int32_t* dyn = nullptr)
 {
     ClassifyArgs a;
     memset(&a, 0, sizeof(a));
+    a.dyn = dyn;
     a.seeds = seeds;
     a.stride = seed_stride;
     a.qkb = COMET_KAPPA * (double)charge * bz_tesla;
@@ -1154,16 +1157,18 @@ extern "C" size_t comet_stage_work_bytes(int64_t n_seeds, int32_t n_part, int32_
     return stage_layout(n_seeds, n_part, k_ref, k_final, G, &s_max, &o1, &o2);
 }
 
-extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
-                                int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
-                                const double* wire_a, const double* wire_b, int32_t n_wires,
-                                const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
-                                int32_t n_fired, int32_t n_hits, double cutoff_cm,
-                                const int64_t* part_off, int32_t n_part,
-                                const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
-                                int32_t k_ref, int32_t k_final, void* work,
-                                double* final_seed, double* final_rss, double* final_dca, uint8_t* cls,
-                                void* cuda_stream)
+// comet_scan_stage; dyn != NULL (comet_scan_turns): n_fired / n_hits are the sizes the launches are made for, the
+// list's real sizes and the loop's stop flag live on the device
+static int scan_stage_impl(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
+                           int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                           const double* wire_a, const double* wire_b, int32_t n_wires,
+                           const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                           int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                           const int64_t* part_off, int32_t n_part,
+                           const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                           int32_t k_ref, int32_t k_final, void* work,
+                           double* final_seed, double* final_rss, double* final_dca, uint8_t* cls,
+                           void* cuda_stream, const int32_t* dyn)
 {
     RefineGrid g;
     int64_t G = 0;
@@ -1192,8 +1197,9 @@ extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t see
     int rc;
     for (int it = 0; ; ++it) {
         // (the caller's promise is about the seeds it passed: the refined sets are checked on the device)
-        rc = comet_scan_rss(ctx, cur, cur_stride, cur_n, it == 0 ? z_run : 0, charge, bz_tesla, step_cm, n_steps, r_stop_cm, wire_a, wire_b,
-                            n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm, rss, nullptr, cuda_stream);
+        rc = scan_rss_impl(ctx, nullptr, nullptr, cur, cur_stride, cur_n, it == 0 ? z_run : 0, charge, bz_tesla, step_cm, n_steps,
+                           r_stop_cm, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm, rss, nullptr,
+                           cuda_stream, dyn);
         if (rc) return rc;
         if (it == n_iter) break;
         rc = comet_select_references(ctx, cur, cur_stride, cur_n, rss, po_cur, n_part, hw, k_ref, ref, cuda_stream);
@@ -1212,7 +1218,23 @@ extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t see
     // the wire table is the one comet_scan_rss has just written on this stream
     return launch_classify_seeds(ctx, cur, cur_stride, charge, bz_tesla, step_cm, n_steps, r_stop_cm, hit_off, rho,
                                  n_fired, n_hits, cutoff_cm, ref, n_part * k_final, rss, final_dca, cls, final_seed,
-                                 final_rss, (cudaStream_t)cuda_stream);
+                                 final_rss, (cudaStream_t)cuda_stream, dyn);
+}
+
+extern "C" int comet_scan_stage(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds, int32_t z_run,
+                                int32_t charge, double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                                const double* wire_a, const double* wire_b, int32_t n_wires,
+                                const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
+                                int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                const int64_t* part_off, int32_t n_part,
+                                const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
+                                int32_t k_ref, int32_t k_final, void* work,
+                                double* final_seed, double* final_rss, double* final_dca, uint8_t* cls,
+                                void* cuda_stream)
+{
+    return scan_stage_impl(ctx, seeds, seed_stride, n_seeds, z_run, charge, bz_tesla, step_cm, n_steps, r_stop_cm, wire_a, wire_b,
+                           n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm, part_off, n_part, half_width, n_grid,
+                           n_iter, shrink, k_ref, k_final, work, final_seed, final_rss, final_dca, cls, cuda_stream, nullptr);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1278,10 +1300,10 @@ extern "C" int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t see
                                 const double* half_width, const int32_t* n_grid, int32_t n_iter, double shrink,
                                 int32_t k_ref, int32_t min_wires, int32_t max_tracks, void* work,
                                 double* turn_seed, double* turn_rss, uint8_t* turn_cls,
-                                int32_t* done_host, int32_t* wires_before_host, void* cuda_stream)
+                                int32_t* done, int32_t* wires_before, void* cuda_stream)
 {
     if (!ctx || n_part < 1 || n_part > COMET_MAX_PARTITIONS || !part_off || !work || !turn_seed || !turn_rss ||
-        (n_hits > 0 && !turn_cls) || !done_host || !wires_before_host || (n_hits & 1) || min_wires < 0 || max_tracks < 0 ||
+        (n_hits > 0 && !turn_cls) || !done || !wires_before || (n_hits & 1) || min_wires < 0 || max_tracks < 0 ||
         n_seeds < 1 || seed_stride < n_seeds || bad_zrun(z_run))
         return COMET_EINVAL;
     PartOff po;
@@ -1298,45 +1320,41 @@ extern "C" int comet_scan_turns(comet_ctx* ctx, const double* seeds, int64_t see
     char* Wk = (char*)work;
     uint8_t* cls_stage = (uint8_t*)(Wk + L.cls);
     double* dca_stage = (double*)(Wk + L.dca);
-    int32_t* counts = (int32_t*)(Wk + L.counts);
+    int32_t* dyn = (int32_t*)(Wk + L.counts);              // {fired wires left, entries left, stop flag, stages done}
     // nothing done yet: NaN seeds / RSS (all-ones is a NaN), empty classification
     CU(ctx, cudaMemsetAsync(turn_seed, 0xff, sizeof(double) * 6 * (size_t)n_part, st));
     CU(ctx, cudaMemsetAsync(turn_rss, 0xff, sizeof(double) * (size_t)n_part, st));
     if (n_hits) CU(ctx, cudaMemsetAsync(turn_cls, 0, (size_t)n_part * (size_t)n_hits, st));
-    for (int p = 0; p < n_part; ++p) { done_host[p] = 0; wires_before_host[p] = 0; }
+    k_turn_init<<<1, 1, 0, st>>>(dyn, n_fired, n_hits, done, wires_before, n_part);
+    // Every stage is enqueued for the event's own list sizes: after a removal the list is padded back to n_fired wires with
+    // wires without entries (k_remove_hits), which no kernel finds anything on; Eq. (1) runs over the dyn[0] wires that
+    // are left (k_rss_sum), and once the stop rule has fired (k_turn_gate) every kernel of the later stages returns at once.
+    // No host read, no synchronisation: the loop can be captured into a CUDA graph.
     const int32_t* cur_fw = fired_wire;
     const int32_t* cur_ho = hit_off;
     const double* cur_rho = rho;
     const int32_t* cur_orig = nullptr;                   // identity
-    int32_t cur_w = n_fired, cur_h = n_hits, n_done = 0, flip = 0;
+    int flip = 0;
     for (int p = n_part - 1; p >= 0; --p) {              // the last turn first
-        if (cur_w < min_wires || n_done >= max_tracks) break;
+        k_turn_gate<<<1, 1, 0, st>>>(dyn, p, min_wires, max_tracks, done, wires_before);
         const int64_t np_seeds = po.off[p + 1] - po.off[p];
         const int64_t one[2] = {0, np_seeds};
-        rc = comet_scan_stage(ctx, seeds + po.off[p], seed_stride, np_seeds, (z_run > 1 && po.off[p] % z_run == 0) ? z_run : 0,
-                              charge, bz_tesla, step_cm, n_steps, r_stop_cm,
-                              wire_a, wire_b, n_wires, cur_fw, cur_ho, cur_rho, cur_w, cur_h, cutoff_cm, one, 1,
-                              half_width, n_grid, n_iter, shrink, k_ref, 1, Wk + L.stage,
-                              turn_seed + 6 * (size_t)p, turn_rss + p, dca_stage, cls_stage, st);
+        rc = scan_stage_impl(ctx, seeds + po.off[p], seed_stride, np_seeds, (z_run > 1 && po.off[p] % z_run == 0) ? z_run : 0,
+                             charge, bz_tesla, step_cm, n_steps, r_stop_cm,
+                             wire_a, wire_b, n_wires, cur_fw, cur_ho, cur_rho, n_fired, n_hits, cutoff_cm, one, 1,
+                             half_width, n_grid, n_iter, shrink, k_ref, 1, Wk + L.stage,
+                             turn_seed + 6 * (size_t)p, turn_rss + p, dca_stage, cls_stage, st, dyn);
         if (rc) return rc;
-        done_host[p] = 1;
-        wires_before_host[p] = cur_w;
-        n_done += 1;
-        if (cur_h) k_scatter_cls<<<(cur_h + 255) / 256, 256, 0, st>>>(cls_stage, cur_orig, cur_h, turn_cls + (size_t)p * n_hits);
+        if (n_hits) k_scatter_cls<<<(n_hits + 255) / 256, 256, 0, st>>>(cls_stage, cur_orig, n_hits, turn_cls + (size_t)p * n_hits, dyn);
         char* Lb = Wk + L.list[flip];
         int32_t* n_fw = (int32_t*)(Lb + L.o_fired);
         int32_t* n_ho = (int32_t*)(Lb + L.o_off);
         double* n_rho = (double*)(Lb + L.o_rho);
         int32_t* n_orig = (int32_t*)(Lb + L.o_orig);
-        k_remove_hits<<<1, COMET_RM_THREADS, 0, st>>>(cur_fw, cur_ho, cur_rho, cur_w, cls_stage, cur_orig, n_fw, n_ho, n_rho,
-                                                      n_orig, counts);
+        k_remove_hits<<<1, COMET_RM_THREADS, 0, st>>>(cur_fw, cur_ho, cur_rho, n_fired, cls_stage, cur_orig, n_fw, n_ho, n_rho,
+                                                      n_orig, dyn, 1, dyn + 2);
         CU(ctx, cudaGetLastError());
-        // the next stage's launch sizes: one synchronisation per stage, as in the paper's host loop
-        int32_t hc[2];
-        CU(ctx, cudaMemcpyAsync(hc, counts, sizeof(hc), cudaMemcpyDeviceToHost, st));
-        CU(ctx, cudaStreamSynchronize(st));
         cur_fw = n_fw; cur_ho = n_ho; cur_rho = n_rho; cur_orig = n_orig;
-        cur_w = hc[0]; cur_h = hc[1];
         flip ^= 1;
     }
     return COMET_OK;

@@ -579,16 +579,21 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, COMET_FINE_MINB) k_fine(co
 __global__ void __launch_bounds__(256) k_rss_sum(const double* __restrict__ e2, int64_t SP, int32_t W,
                                                  int64_t n_seeds, double* __restrict__ rss,
                                                  const unsigned int* __restrict__ tm, double lam2,
-                                                 const unsigned int* __restrict__ zg)
+                                                 const unsigned int* __restrict__ zg, const int32_t* __restrict__ dyn = nullptr)
 {
     const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= n_seeds) return;
+    // (comet_scan_turns: the launch is sized by the event's first list; the wires that are left come first, Eq. (1) runs over them)
+    const int MW = (W + 31) / 32;                          // words per chunk of the mask (as launched)
+    if (dyn) {
+        if (dyn[2]) return;
+        W = dyn[0];
+    }
     double acc = 0.0;
     // (zg: the run length found on the device -- the mask exists only if the z-run kernel served the launch)
     if (tm && (!zg || *zg >= 8u)) {
-        const int MW = (W + 31) / 32;
         const unsigned int* m = tm + (size_t)(s >> 5) * MW;
-        for (int wd = 0; wd < MW; ++wd) {
+        for (int wd = 0; wd * 32 < W; ++wd) {
             const unsigned bits = __ldg(m + wd);
             const int n = min(32, W - wd * 32);
 #pragma unroll 4

@@ -264,6 +264,7 @@ k_classify_seeds(const ClassifyArgs a, const int64_t* __restrict__ seed_idx, con
                  double* __restrict__ rss_out)
 {
     extern __shared__ __align__(16) double sm[];
+    if (a.dyn && a.dyn[2]) return;                          // (the turn loop has stopped: the outputs keep their initial values)
     const int64_t idx = seed_idx[blockIdx.x];
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
     if (threadIdx.x < 6 && seed_out) seed_out[(size_t)blockIdx.x * 6 + threadIdx.x] = (idx >= 0) ? a.seeds[threadIdx.x * a.stride + idx] : qnan;

@@ -100,6 +100,7 @@ struct FusedArgs {
     double* ub;              // scan_zgroup.cuh: (x_0, x_1, T_0, T_1) of the distinct transverse tracks [u / 32][u_rows][4][32]
     int32_t* np_u;           //   and their numbers of recorded states
     int32_t u_rows;          //   rows per track in ub: n_steps + 1 rounded up to whole 64-row blocks
+    const int32_t* dyn;      // comet_scan_turns: device {fired wires left, entries left, stop flag}: nullptr = sizes are exact
     unsigned int* tm;        // scan_zrun.cuh: [chunks][ceil(W / 32)] bit i: k_fine_ck fills the e^2 row of wire i (else cutoff^2)
 };
 #define COMET_ZG_MIN 8             // smallest run length served by the ZG kernels (scan_zgroup.cuh)
@@ -151,6 +152,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
     constexpr int WCAP = COMET_FUSED_WCAP;
     constexpr unsigned FULL = 0xffffffffu;
     static_assert(TR % FM1 == 0 && TR % CK == 0, "tile rows");
+    if (a.dyn && a.dyn[2]) return;                          // (the turn loop has stopped)
     if (!FIELD && a.zg && zgroup_of(a.zg) >= COMET_ZG_MIN) return;     // the z-run kernels serve this launch (scan_zrun.cuh)
     extern __shared__ __align__(16) double fsm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -411,6 +413,7 @@ template <bool FIELD, bool ZG = false>
 __global__ void __launch_bounds__(COMET_FINE_THREADS, FIELD ? COMET_FINE_MINB_FIELD : COMET_FINE_MINB) k_fine_ck(const FusedArgs a)
 {
     static_assert(!(FIELD && ZG), "the transverse motion depends on z in a field map");
+    if (a.dyn && a.dyn[2]) return;                          // (the turn loop has stopped)
     if (ZG) {
         if (zrun_of(a.zrun, a.zg) < COMET_ZG_MIN) return;
     } else if (!FIELD && a.zg && zgroup_of(a.zg) >= COMET_ZG_MIN) {

@@ -58,6 +58,7 @@ __global__ void __launch_bounds__(32) k_gen_unique(const FusedArgs a)
     constexpr int GR = COMET_GU_ROWS, RS = COMET_GU_STRIDE;
     constexpr unsigned FULL = 0xffffffffu;
     __shared__ __align__(16) double sm[GR * RS];
+    if (a.dyn && a.dyn[2]) return;                          // (the turn loop has stopped)
     const unsigned int zg = zrun_of(a.zrun, a.zg);
     if (zg < COMET_ZG_MIN) return;                          // the plain k_scan_fused serves this launch
     const int zshift = 31 - __clz((int)zg);

@@ -38,7 +38,7 @@
 //
 // Only shortlists are decided here (FMA-form distances, slack 1e-6 cm on every bound): k_fine_ck<ZG> re-decides
 // between rows k-1, k, k+1 with the definition's exact operations, so n_pts and RSS are the bit-identical numbers
-// of the plain path and of the oracle.  A chunk with a lane beyond |c| h <= 0.05 opens everything.
+// of the plain path and of the definition.  A chunk with a lane beyond |c| h <= 0.05 opens everything.
 #pragma once
 #include "scan_fused.cuh"
 
@@ -92,6 +92,7 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     constexpr int BUFD = (BLK + NSUB) * NU * 2;             // doubles per staged block: rows [64][NU][x, y], tangents [8][NU][T_x, T_y]
     constexpr unsigned FULL = 0xffffffffu;
     static_assert(LCAP * (int)sizeof(unsigned short) <= 2 * BUFD * (int)sizeof(double) || NU == 1, "item list fits the staged blocks");
+    if (a.dyn && a.dyn[2]) return;                          // (the turn loop has stopped)
     if (zrun_of(a.zrun, a.zg) != (unsigned)ZR) return;      // another variant serves this launch
     extern __shared__ __align__(16) double zsm[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;

@@ -84,6 +84,7 @@ struct ClassifyArgs {
     const double* ub;          // [track][u_rows][4], nullptr = record the track here
     const int32_t* np_u;
     int32_t zshift, u_rows;
+    const int32_t* dyn;        // comet_scan_turns: device {.., .., stop flag}: set = write nothing
 };
 
 // CTA-wide: re-extrapolate seed `idx` into shared memory (state k at sm[k*6..]), then one thread per fired

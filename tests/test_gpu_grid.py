@@ -160,6 +160,44 @@ def test_cold_context_first_call_captured_in_a_graph(cfg1_event):
         cold.close()
 
 
+def test_turn_loop_replayed_from_a_graph(cfg1_event):
+    """comet_scan_turns enqueues a whole event -- three stages with refinements and hit removal, list sizes and the
+    stop rule on the device -- without a host read: captured once into a CUDA graph on a cold context (workspace
+    reserved), replayed twice, identical to the oracle's loop, also when the stop rule fires before the last stage."""
+    from paper_1911_09340_b200 import Comet
+    ev = cfg1_event
+    axes, shp, part_off = event_axes(ev, shape=(8, 8, 16, 16))           # 16384 seeds per partition: the z-run kernels
+    seeds_h, _ = event_seeds(ev, shape=(8, 8, 16, 16))
+    hits = _hits(ev)
+    kw = dict(half_width=[1.2, 1.0, 1.0, 2.0], n_grid=[3, 3, 3, 3], n_iter=2, shrink=0.5, k_ref=4)
+    args = (ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, ev.hit_off,
+            ev.rho, ev.cutoff)
+    side = torch.cuda.Stream()
+    for extra in ({}, {"max_tracks": 2}, {"min_wires": 50}):
+        cold = Comet(0)
+        try:
+            seeds = cold.seed_grid(_dev(axes), shp)
+            cold.reserve_scan(int(part_off[1]), ev.n_steps, ev.n_fired)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                out = cold.scan_turns(seeds, part_off, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop, *hits, ev.cutoff,
+                                      stream=side, z_run=16, sync=False, **kw, **extra)
+            ref = O.scan_turns(seeds_h, part_off, *args, **kw, **extra)
+            for _ in range(2):
+                for k in ("turn_seed", "turn_rss"):
+                    out[k].fill_(7.0)
+                g.replay()
+                torch.cuda.synchronize()
+                np.testing.assert_array_equal(out["done_dev"].cpu().numpy().astype(bool), ref["done"])
+                np.testing.assert_array_equal(out["wires_before_dev"].cpu().numpy(), ref["wires_before"])
+                np.testing.assert_array_equal(out["turn_seed"].cpu().numpy(), ref["turn_seed"])
+                np.testing.assert_array_equal(out["turn_rss"].cpu().numpy(), ref["turn_rss"])
+                np.testing.assert_array_equal(out["turn_cls"].cpu().numpy(), ref["turn_cls"])
+        finally:
+            cold.close()
+
+
 # ------------------------------------------------------------------------------------------------
 # comet_scan_event_grid_host
 # ------------------------------------------------------------------------------------------------
