@@ -559,9 +559,10 @@ int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, int64_t n_se
 
 /* The same event with its seed sets given as grid axes (comet_seed_grid; HOST [n_part][A]) and the geometry
  * of comet_set_geometry: per event only the axes, the fired wires and the hit entries cross the bus (a few
- * KB).  Copies them in, builds the seeds on the device, runs comet_scan_rss with z_run =
- * comet_grid_z_run(n_z) and comet_select_and_classify with part_off[q] = q G, copies best_seed / best_rss /
- * best_dca / cls (and rss [n_part G] if rss_host != NULL) back and synchronises the stream. */
+ * KB).  Copies them in (one transfer, through a pinned staging buffer of the ctx: the caller's arrays need not
+ * be pinned), builds the seeds on the device, runs comet_scan_rss with z_run = comet_grid_z_run(n_z) and
+ * comet_select_and_classify with part_off[q] = q G, copies best_seed / best_rss / best_dca / cls back (one
+ * transfer; rss [n_part G] too if rss_host != NULL) and synchronises the stream. */
 int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_host, int32_t n_part, int32_t n_p,
                                int32_t n_ct, int32_t n_phi, int32_t n_z,
                                int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,

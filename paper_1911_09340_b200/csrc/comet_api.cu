@@ -101,6 +101,8 @@ struct comet_ctx {
         double qkb, step, r_stop;
         int32_t n_steps, zshift, u_rows, valid;
     } last;
+    void* hstage;          // pinned host staging of comet_scan_event_grid_host: one copy in, one copy out per event
+    size_t hstage_bytes;
     // detector geometry kept on the device for the host-buffer entry points (comet_set_geometry)
     double* geom_a;
     double* geom_b;
@@ -230,6 +232,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ub); cudaFree(ctx->npu);
     for (int j = 0; j < COMET_TEV_RING * 5; ++j) if (ctx->tev[j / 5][j % 5]) cudaEventDestroy(ctx->tev[j / 5][j % 5]);
     cudaFree(ctx->geom_a); cudaFree(ctx->geom_b);
+    if (ctx->hstage) cudaFreeHost(ctx->hstage);
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->tw); cudaFree(ctx->tmk); cudaFree(ctx->bmax);
     for (int l = 0; l < COMET_MAX_LANES; ++l) {
         if (ctx->ls[l]) cudaStreamDestroy(ctx->ls[l]);
@@ -1959,24 +1962,37 @@ extern "C" int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_hos
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int64_t n_seeds = g.G * n_part;
     const int64_t stride = (n_seeds + 31) / 32 * 32;
+    // one device slab: [inputs: axes | fired | hit_off | rho] [seeds] [rss] [outputs: best_seed | best_rss | best_dca | cls];
+    // the inputs and the outputs each cross the bus as ONE copy through a pinned staging buffer of the same layout
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
     const size_t o_axes = take(sizeof(double) * (size_t)g.A * n_part);
-    const size_t o_seeds = take(sizeof(double) * 6 * (size_t)stride);
     const size_t o_fw = take(sizeof(int32_t) * (size_t)n_fired);
     const size_t o_ho = take(sizeof(int32_t) * ((size_t)n_fired + 1));
     const size_t o_rho = take(sizeof(double) * (size_t)n_hits);
+    const size_t in_bytes = off;
+    const size_t o_seeds = take(sizeof(double) * 6 * (size_t)stride);
     const size_t o_rss = take(sizeof(double) * (size_t)n_seeds);
+    const size_t o_out = off;
     const size_t o_bs = take(sizeof(int64_t) * (size_t)n_part);
     const size_t o_br = take(sizeof(double) * (size_t)n_part);
     const size_t o_bd = take(sizeof(double) * (size_t)n_part * (size_t)n_fired);
     const size_t o_cls = take((size_t)n_part * (size_t)n_hits);
+    const size_t out_bytes = off - o_out;
     if (off > ctx->hbuf_bytes) {
         CU(ctx, cudaDeviceSynchronize());
         rc = grow(ctx, &ctx->hbuf, &ctx->hbuf_bytes, off);
         if (rc) return rc;
     }
+    if (in_bytes + out_bytes > ctx->hstage_bytes) {
+        CU(ctx, cudaDeviceSynchronize());
+        if (ctx->hstage) { cudaFreeHost(ctx->hstage); ctx->hstage = nullptr; ctx->hstage_bytes = 0; }
+        cudaError_t e = cudaHostAlloc(&ctx->hstage, in_bytes + out_bytes, cudaHostAllocDefault);
+        if (e != cudaSuccess) { ctx->last_cuda = (int)e; ctx->hstage = nullptr; cudaGetLastError(); return COMET_ENOMEM; }
+        ctx->hstage_bytes = in_bytes + out_bytes;
+    }
     char* B = (char*)ctx->hbuf;
+    char* Hs = (char*)ctx->hstage;
     double* d_axes = (double*)(B + o_axes);
     double* d_seeds = (double*)(B + o_seeds);
     int32_t* d_fw = (int32_t*)(B + o_fw);
@@ -1987,12 +2003,13 @@ extern "C" int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_hos
     double* d_br = (double*)(B + o_br);
     double* d_bd = (double*)(B + o_bd);
     uint8_t* d_cls = (uint8_t*)(B + o_cls);
-    CU(ctx, cudaMemcpyAsync(d_axes, axes_host, sizeof(double) * (size_t)g.A * n_part, cudaMemcpyHostToDevice, st));
+    memcpy(Hs + o_axes, axes_host, sizeof(double) * (size_t)g.A * n_part);
     if (n_fired) {
-        CU(ctx, cudaMemcpyAsync(d_fw, fired_wire_host, sizeof(int32_t) * (size_t)n_fired, cudaMemcpyHostToDevice, st));
-        CU(ctx, cudaMemcpyAsync(d_ho, hit_off_host, sizeof(int32_t) * ((size_t)n_fired + 1), cudaMemcpyHostToDevice, st));
+        memcpy(Hs + o_fw, fired_wire_host, sizeof(int32_t) * (size_t)n_fired);
+        memcpy(Hs + o_ho, hit_off_host, sizeof(int32_t) * ((size_t)n_fired + 1));
     }
-    if (n_hits) CU(ctx, cudaMemcpyAsync(d_rho, rho_host, sizeof(double) * (size_t)n_hits, cudaMemcpyHostToDevice, st));
+    if (n_hits) memcpy(Hs + o_rho, rho_host, sizeof(double) * (size_t)n_hits);
+    CU(ctx, cudaMemcpyAsync(B, Hs, in_bytes, cudaMemcpyHostToDevice, st));
     rc = comet_seed_grid(ctx, d_axes, n_part, n_p, n_ct, n_phi, n_z, d_seeds, stride, st);
     if (rc) return rc;
     // (a partition is a whole number of runs: G is a multiple of the run length)
@@ -2006,12 +2023,14 @@ extern "C" int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_hos
                                    ctx->geom_a, ctx->geom_b, ctx->geom_n, d_fw, d_ho, d_rho, n_fired, n_hits, cutoff_cm,
                                    d_rss, po, n_part, d_bs, d_br, d_bd, d_cls, st);
     if (rc) return rc;
-    CU(ctx, cudaMemcpyAsync(best_seed_host, d_bs, sizeof(int64_t) * (size_t)n_part, cudaMemcpyDeviceToHost, st));
-    CU(ctx, cudaMemcpyAsync(best_rss_host, d_br, sizeof(double) * (size_t)n_part, cudaMemcpyDeviceToHost, st));
-    if (n_fired) CU(ctx, cudaMemcpyAsync(best_dca_host, d_bd, sizeof(double) * (size_t)n_part * n_fired, cudaMemcpyDeviceToHost, st));
-    if (n_hits) CU(ctx, cudaMemcpyAsync(cls_host, d_cls, (size_t)n_part * n_hits, cudaMemcpyDeviceToHost, st));
+    char* Ho = Hs + in_bytes;
+    CU(ctx, cudaMemcpyAsync(Ho, B + o_out, out_bytes, cudaMemcpyDeviceToHost, st));
     if (rss_host) CU(ctx, cudaMemcpyAsync(rss_host, d_rss, sizeof(double) * (size_t)n_seeds, cudaMemcpyDeviceToHost, st));
     CU(ctx, cudaStreamSynchronize(st));
+    memcpy(best_seed_host, Ho + (o_bs - o_out), sizeof(int64_t) * (size_t)n_part);
+    memcpy(best_rss_host, Ho + (o_br - o_out), sizeof(double) * (size_t)n_part);
+    if (n_fired) memcpy(best_dca_host, Ho + (o_bd - o_out), sizeof(double) * (size_t)n_part * n_fired);
+    if (n_hits) memcpy(cls_host, Ho + (o_cls - o_out), (size_t)n_part * n_hits);
     return COMET_OK;
 }
 
