@@ -54,8 +54,9 @@ FP64 = {
 DENSE = {"rkn_step": 52, "row": 9, "fine_pair": 600}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1], from the ncu --set full capture of THIS build
 # named beside them (profiles/): the bytes the live run moves are modelled from the library's own sizes below
-NCU_TRAFFIC = {"file": "profiles/r2_full_zrun.txt",
-               "k_gen_unique": None, "k_scan_zrun": None, "k_fine_ck": None}
+NCU_TRAFFIC = {"file": "profiles/r2_full_zrun.txt", "per": "launch = one sub-slab of 3072 chunks; a configs[1] step has four",
+               "k_gen_unique": 27.0e6, "k_scan_zrun": 121.1e6, "k_fine_ck": 62.9e6, "k_rss_sum": 17.7e6,
+               "per_step": 4 * (27.0e6 + 121.1e6 + 62.9e6 + 17.7e6)}
 STAGE_HALF_WIDTH = [0.6, 0.5, 0.5, 1.0]
 STAGE_GRID = [5, 5, 5, 5]
 FIELD_TOL = 1e-7
@@ -330,7 +331,8 @@ class Leg:
                 "z_checkpoints": 8.0 * n_states / 8,
                 "per_seed_constants": 20.0 * S + 28.0 * S,                       # n_pts, c, T_z written; read by the fine stage
                 "pair_keys": 8.0 * (st["touched"] + st["touched"]) + 8.0 * 2 * st["fine_executed"],   # written + read back; fine: read + e^2 written
-                "fine_candidates": (3 * 32.0 + 8.0) * st["fine_needed"],         # three rows of the distinct track + the z checkpoint
+                # per (chunk, wire) item three rows of each of the chunk's distinct tracks (shared by the seeds of a run), per pair the z checkpoint
+                "fine_candidates": 3 * 32.0 * (32 / self.z_run) * st["fine_executed"] / 32 + 8.0 * st["fine_needed"],
                 "rss_sum": 8.0 * st["fine_executed"] + 8.0 * S,
             }
         else:
