@@ -29,6 +29,9 @@
 // by the definition: n_pts and RSS are bit-identical.
 //
 // RSS-only (the hot path).  Calls that ask for D or k* of every pair use the materialised path.
+// Seed sets in z-runs (the first-iteration grids of the method) are served by k_gen_unique + k_scan_zrun
+// (scan_zgroup.cuh, scan_zrun.cuh) and share k_fine_ck<.., ZG = true> below; this kernel serves every other seed set
+// (refined sets, small calls) and the field map.
 #pragma once
 #include "common.cuh"
 #include "dca.cuh"

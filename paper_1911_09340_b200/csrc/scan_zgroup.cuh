@@ -7,16 +7,17 @@
 // differ only by the start value, one addition per step.  The seed grids of the method ("A seed set
 // was prepared by combining each component from the grids of the ranges") have z as one of the grid axes, so with z
 // as the fastest index a track chunk of 32 seeds holds only 32 / ZG distinct transverse tracks.  SIMT lanes cannot
-// skip duplicated work inside a warp, so the work is re-mapped: k_gen_unique steps the distinct tracks (lane =
-// distinct track) and leaves (x_0, x_1, T_0, T_1) of every recorded state in a buffer that stays in L2;
-// k_scan_fused<.., ZG = true> (lane = seed) copies its tile rows from there, adds its own z column (one addition
-// per recorded state instead of the 48 operations of the RKN4 step) and goes on as before.  Every number is
-// produced by the same IEEE operations as in the plain k_scan_fused (and the definition), so n_pts, checkpoints, keys
-// and RSS are bit-identical.
+// skip duplicated work inside a warp, so the work is re-mapped: k_gen_unique (this file) steps the distinct tracks
+// (lane = distinct track) and leaves (x_0, x_1, T_0, T_1) of every recorded state in ub[track][row];
+// k_scan_zrun (scan_zrun.cuh; lane = seed) works from those rows and adds its own z column (one addition per
+// recorded state instead of the 50 operations of the RKN4 step); k_fine_ck<.., ZG = true> (scan_fused.cuh) reads its
+// three candidate states from them.  Every number is produced by the same IEEE operations as in the plain
+// k_scan_fused (and the definition), so n_pts and RSS are bit-identical.
 //
-// Which seeds qualify is decided on the device (k_zgroup_check: the largest power of two ZG <= 32 such that every
-// aligned run of ZG seeds of the launch is uniform); the ZG kernels run when ZG >= 8 and the plain kernel
-// otherwise -- all are launched, the ones that are not needed exit at once, so the call stays asynchronous.
+// Which seeds qualify: the caller's promise (comet_scan_rss z_run), else decided on the device (k_zgroup_check: the
+// largest power of two ZG <= 32 such that every aligned run of ZG seeds of the launch is uniform); the z-run kernels
+// run when ZG >= 8 and the plain kernel otherwise -- without a promise all are launched, the ones that are not
+// needed exit at once, so the call stays asynchronous.
 #pragma once
 #include "scan_fused.cuh"
 
