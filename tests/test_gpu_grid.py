@@ -110,6 +110,64 @@ def test_z_run_promise_gives_the_same_numbers(comet, cfg1_event):
     comet.set_option(OPT_ZGROUP, 1)
 
 
+@pytest.mark.parametrize("n_z,cut,r_stop,n_steps", [(32, 0, 50.0, None), (8, 0, 50.0, None), (16, 5, 50.0, None), (8, 3, 0.0, 150),
+                                                    (16, 0, 1.0e3, None), (32, 31, 50.0, 40)])
+def test_z_run_kernel_variants_with_the_promise(comet, cfg1_event, n_z, cut, r_stop, n_steps):
+    """k_scan_zrun's three variants (1, 2 or 4 distinct tracks per chunk) with the run length PROMISED, on sets that
+    end inside a run and inside a chunk, without a stop (r_stop = 0: every track uses the whole capacity), with the
+    apex stop (r_stop beyond the chamber), and with fewer steps than one 64-row block."""
+    from paper_1911_09340_b200.binding import OPT_ZGROUP
+    from comet_synth import seed_grid
+    ev = cfg1_event
+    sp = ev.spec
+    seeds = seed_grid(ev, 0, (3, 4, 5, n_z), tuple(sp["p_range"]), ct_hw=sp.get("ct_hw", 0.15))
+    seeds = np.ascontiguousarray(seeds[:, :seeds.shape[1] - cut])
+    ns = ev.n_steps if n_steps is None else n_steps
+    ref = O.scan(seeds, ev.charge, ev.bz, ev.step, ns, r_stop, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, ev.hit_off,
+                 ev.rho, ev.cutoff, want_npts=True)
+    comet.set_option(OPT_ZGROUP, 2)
+    try:
+        o = comet.scan_rss(_dev(seeds), ev.charge, ev.bz, ev.step, ns, r_stop, *_hits(ev), ev.cutoff, z_run=min(n_z, 32))
+        torch.cuda.synchronize()
+    finally:
+        comet.set_option(OPT_ZGROUP, 1)
+    assert np.array_equal(o["n_pts"].cpu().numpy(), ref["n_pts"])
+    assert np.array_equal(o["rss"].cpu().numpy(), ref["rss"])
+
+
+def test_z_run_kernels_without_hits_and_with_empty_wires(comet, cfg1_event):
+    """No fired wire at all (RSS = 0), and a hit list in which some fired wires have no entries (they contribute cutoff^2
+    and are never swept)."""
+    from paper_1911_09340_b200.binding import OPT_ZGROUP
+    ev = cfg1_event
+    seeds, _ = event_seeds(ev, shape=(4, 4, 4, 16))
+    d = _dev(seeds)
+    wa, wb = _dev(ev.geom.wire_a), _dev(ev.geom.wire_b)
+    phys = (ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop)
+    comet.set_option(OPT_ZGROUP, 2)
+    try:
+        e32, ef = torch.zeros(0, dtype=torch.int32, device="cuda"), torch.zeros(0, dtype=torch.float64, device="cuda")
+        o = comet.scan_rss(d, *phys, wa, wb, e32, torch.zeros(1, dtype=torch.int32, device="cuda"), ef, ev.cutoff, z_run=16)
+        torch.cuda.synchronize()
+        ref = O.scan(seeds, *phys, ev.geom.wire_a, ev.geom.wire_b, np.zeros(0, np.int32), np.zeros(1, np.int32), np.zeros(0),
+                     ev.cutoff, want_npts=True)
+        assert np.array_equal(o["rss"].cpu().numpy(), ref["rss"]) and float(o["rss"].abs().max()) == 0.0
+        assert np.array_equal(o["n_pts"].cpu().numpy(), ref["n_pts"])
+        # every third fired wire loses its entries
+        keep = np.ones(ev.n_fired, bool)
+        keep[::3] = False
+        cnt = np.where(keep, np.diff(ev.hit_off), 0)
+        ho = np.zeros(ev.n_fired + 1, np.int32)
+        ho[1:] = np.cumsum(cnt)
+        rho = np.concatenate([ev.rho[ev.hit_off[i]:ev.hit_off[i + 1]] for i in range(ev.n_fired) if keep[i]])
+        o = comet.scan_rss(d, *phys, wa, wb, _dev(ev.fired_wire), _dev(ho), _dev(rho), ev.cutoff, z_run=16)
+        torch.cuda.synchronize()
+        ref = O.scan(seeds, *phys, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, ho, rho, ev.cutoff)
+        assert np.array_equal(o["rss"].cpu().numpy(), ref["rss"])
+    finally:
+        comet.set_option(OPT_ZGROUP, 1)
+
+
 # ------------------------------------------------------------------------------------------------
 # comet_reserve_scan: the first call of a cold context neither allocates nor synchronises -- it can be captured
 # ------------------------------------------------------------------------------------------------
