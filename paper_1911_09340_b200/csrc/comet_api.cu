@@ -57,6 +57,7 @@ struct comet_ctx {
     int opt_lanes;
     int opt_zgroup;              // 1 (default): seeds in z-runs go through the ZG kernels (scan_zgroup.cuh)
     int lanes_set;               // COMET_OPT_LANES was set by the caller
+    int* ref_fb;                 // [COMET_MAX_PARTITIONS] k_select_refs_short: the partition needs the full rule
     unsigned int* zg_flag;       // [COMET_MAX_LANES] run length found by k_zgroup_check
     double* ub;                  // distinct transverse tracks of a slab (k_gen_unique)
     size_t ub_bytes;
@@ -174,6 +175,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     ctx->opt_lanes = COMET_DEFAULT_LANES;
     ctx->opt_zgroup = 1;
     if (e == cudaSuccess) e = cudaMalloc(&ctx->zg_flag, sizeof(unsigned int) * (COMET_MAX_LANES + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->ref_fb, sizeof(int) * COMET_MAX_PARTITIONS);
     {
         int prio_lo = 0, prio_hi = 0;
         if (e == cudaSuccess) e = cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
@@ -229,7 +231,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     if (!ctx) return COMET_EINVAL;
     cudaSetDevice(ctx->device);
     cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
-    cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ub); cudaFree(ctx->npu);
+    cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ref_fb); cudaFree(ctx->ub); cudaFree(ctx->npu);
     for (int j = 0; j < COMET_TEV_RING * 5; ++j) if (ctx->tev[j / 5][j % 5]) cudaEventDestroy(ctx->tev[j / 5][j % 5]);
     cudaFree(ctx->geom_a); cudaFree(ctx->geom_b);
     if (ctx->hstage) cudaFreeHost(ctx->hstage);
@@ -1029,12 +1031,15 @@ extern "C" int comet_select_references(comet_ctx* ctx, const double* seeds, int6
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (n_max <= 16 * COMET_REF_THREADS) {
         k_select_refs<<<n_part, COMET_REF_THREADS, 0, st>>>(seeds, seed_stride, rss, po, box, k_ref, ref_seed);
-    } else if (per <= COMET_REF_SMEM_MAX) {
-        k_select_refs_cluster<true><<<dim3(COMET_REF_CLUSTER, n_part), COMET_REF_THREADS, (size_t)per * sizeof(double), st>>>(
-            seeds, seed_stride, rss, po, box, k_ref, ref_seed);
     } else {
-        k_select_refs_cluster<false><<<dim3(COMET_REF_CLUSTER, n_part), COMET_REF_THREADS, 0, st>>>(
-            seeds, seed_stride, rss, po, box, k_ref, ref_seed);
+        // the seeds of lowest RSS first (k_select_refs_short); the cluster kernel redoes a partition only if they ran out
+        k_select_refs_short<<<n_part, COMET_REF_THREADS, 0, st>>>(seeds, seed_stride, rss, po, box, k_ref, ref_seed, ctx->ref_fb);
+        if (per <= COMET_REF_SMEM_MAX)
+            k_select_refs_cluster<true><<<dim3(COMET_REF_CLUSTER, n_part), COMET_REF_THREADS, (size_t)per * sizeof(double), st>>>(
+                seeds, seed_stride, rss, po, box, k_ref, ref_seed, ctx->ref_fb);
+        else
+            k_select_refs_cluster<false><<<dim3(COMET_REF_CLUSTER, n_part), COMET_REF_THREADS, 0, st>>>(
+                seeds, seed_stride, rss, po, box, k_ref, ref_seed, ctx->ref_fb);
     }
     CU(ctx, cudaGetLastError());
     return COMET_OK;

@@ -142,6 +142,151 @@ k_select_refs(const double* __restrict__ seeds, int64_t stride, const double* __
     }
 }
 
+// Large partitions (the first iteration of a stage: 131072 seeds per partition): the greedy rule visits the seeds in
+// increasing (RSS, index), so only the seeds of lowest RSS matter -- as long as enough of them exist.  One CTA per partition:
+//   1. a threshold key K* from a sample of 2048 seeds (the 16th smallest of their RSS high words, by a radix select in
+//      shared memory): about 1024 seeds lie below it;
+//   2. the candidates: EVERY seed whose key is below K* (they must fit the list of M = COMET_SHORT_M, else fallback),
+//      compacted into shared memory;
+//   3. the greedy rule on the candidates, register-resident as in k_select_refs.
+// The candidates are exactly the seeds the rule visits first, so the references it finds among them are the references of
+// the full rule.  If they run out before k_ref references are found (heavy overlaps, or a partition whose M smallest
+// values are equal), fallback[p] = 1 and k_select_refs_cluster redoes the partition: the result never depends on M.
+#define COMET_SHORT_M 2048
+#define COMET_SHORT_RANK 16
+__device__ __forceinline__ unsigned rss_key(double v)
+{
+    return (v != v) ? 0xffffffffu : (unsigned)__double2hiint(v);        // RSS >= 0: the high word orders like the value
+}
+__global__ void __launch_bounds__(COMET_REF_THREADS)
+k_select_refs_short(const double* __restrict__ seeds, int64_t stride, const double* __restrict__ rss, PartOff po,
+                    RefBox box, int32_t k_ref, int64_t* __restrict__ ref_seed, int* __restrict__ fallback)
+{
+    constexpr int M = COMET_SHORT_M, PER = M / COMET_REF_THREADS;
+    __shared__ unsigned hist[257];
+    __shared__ unsigned s_prefix, s_want, s_cnt;
+    __shared__ int cand[M];
+    __shared__ int64_t sel_idx[COMET_MAX_REFS];
+    __shared__ double sel_c[COMET_MAX_REFS][4];
+    __shared__ double sv[COMET_REF_THREADS / 32];
+    __shared__ int64_t si[COMET_REF_THREADS / 32];
+    __shared__ int64_t s_win;
+    const int p = blockIdx.x;
+    const int64_t lo = po.off[p], hi = po.off[p + 1];
+    const int64_t n = hi - lo;
+    int64_t* out = ref_seed + (size_t)p * k_ref;
+    for (int r = threadIdx.x; r < k_ref; r += blockDim.x) out[r] = -1;
+    if (threadIdx.x == 0) { s_prefix = 0u; s_want = (unsigned)M; s_cnt = 0u; fallback[p] = 0; }
+    __syncthreads();
+    unsigned kstar = 0xffffffffu;                           // n <= M: every seed with a number is a candidate
+    if (n > M) {
+        // threshold from a sample: 2 x 1024 seeds at a stride of n / 2048, the COMET_SHORT_RANK-th smallest of their keys by
+        // a radix select in shared memory.  About COMET_SHORT_RANK n / 2048 seeds lie below it (1024 +- 256 for rank 16):
+        // ANY threshold is correct as long as the list holds every seed below it, which is checked (cnt < M) below.
+        const int64_t sstep = n / (2 * COMET_REF_THREADS);
+        unsigned skey[2];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) skey[j] = rss_key(rss[lo + (int64_t)(threadIdx.x + j * COMET_REF_THREADS) * sstep]);
+        if (threadIdx.x == 0) s_want = COMET_SHORT_RANK;
+        for (int shift = 24; shift >= 0; shift -= 8) {
+            for (int b2 = threadIdx.x; b2 < 257; b2 += blockDim.x) hist[b2] = 0u;
+            __syncthreads();
+            const unsigned prefix = s_prefix;
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {
+                const bool in = shift == 24 || (skey[j] >> (shift + 8)) == (prefix >> (shift + 8));
+                const unsigned digit = in ? ((skey[j] >> shift) & 255u) : 256u;
+                const unsigned peers = __match_any_sync(0xffffffffu, digit);
+                if (in && (int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&hist[digit], (unsigned)__popc(peers));
+            }
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                unsigned want = s_want, cum = 0u;
+                int d = 0;
+                for (; d < 255; ++d) {
+                    if (cum + hist[d] >= want) break;
+                    cum += hist[d];
+                }
+                s_prefix = prefix | ((unsigned)d << shift);
+                s_want = want - cum;
+            }
+            __syncthreads();
+        }
+        kstar = s_prefix;
+    }
+    for (int64_t s = lo + threadIdx.x; s < hi; s += blockDim.x) {
+        if (rss_key(rss[s]) < kstar) {
+            const unsigned pos = atomicAdd(&s_cnt, 1u);
+            if (pos < (unsigned)M) cand[pos] = (int)(s - lo);
+        }
+    }
+    __syncthreads();
+    if (s_cnt >= (unsigned)M && n > M) {                    // (more seeds below the threshold than the list holds: the full rule)
+        if (threadIdx.x == 0) fallback[p] = 1;
+        return;
+    }
+    const int cnt = (int)min(s_cnt, (unsigned)M);
+    // the greedy rule on the candidates (k_select_refs, register-resident branch)
+    double rv[PER], cc[PER][4];                             // RSS and the refined components of the thread's candidates
+    int64_t sj[PER];
+    unsigned dead = 0u;
+#pragma unroll
+    for (int j = 0; j < PER; ++j) {
+        const int q = threadIdx.x + j * COMET_REF_THREADS;
+        sj[j] = q < cnt ? lo + cand[q] : -1;
+        rv[j] = q < cnt ? rss[sj[j]] : 0.0;
+        if (!(q < cnt) || rv[j] != rv[j]) dead |= 1u << j;
+#pragma unroll
+        for (int d = 0; d < 4; ++d) cc[j][d] = q < cnt ? seeds[(size_t)(2 + d) * stride + sj[j]] : 0.0;
+    }
+    int found = 0;
+    for (int r = 0; r < k_ref; ++r) {
+        double v = 0.0;
+        int64_t idx = -1;
+#pragma unroll
+        for (int j = 0; j < PER; ++j)
+            if (!((dead >> j) & 1u)) argmin_merge(v, idx, rv[j], sj[j]);
+        for (int o = 16; o > 0; o >>= 1) {
+            const double v2 = __shfl_down_sync(0xffffffffu, v, o);
+            const int64_t i2 = __shfl_down_sync(0xffffffffu, idx, o);
+            argmin_merge(v, idx, v2, i2);
+        }
+        if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = v; si[threadIdx.x >> 5] = idx; }
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            v = sv[threadIdx.x];
+            idx = si[threadIdx.x];
+            for (int o = 16; o > 0; o >>= 1) {
+                const double v2 = __shfl_down_sync(0xffffffffu, v, o);
+                const int64_t i2 = __shfl_down_sync(0xffffffffu, idx, o);
+                argmin_merge(v, idx, v2, i2);
+            }
+            if (threadIdx.x == 0) {
+                s_win = idx;
+                if (idx >= 0) {
+                    sel_idx[r] = idx;
+                    for (int d = 0; d < 4; ++d) sel_c[r][d] = seeds[(size_t)(2 + d) * stride + idx];
+                    out[r] = idx;
+                }
+            }
+        }
+        __syncthreads();
+        const int64_t win = s_win;
+        if (win < 0) break;
+        found = r + 1;
+        if (r + 1 == k_ref) break;
+#pragma unroll
+        for (int j = 0; j < PER; ++j) {
+            if ((dead >> j) & 1u) continue;
+            const bool ov = fabs(xsub(cc[j][0], sel_c[r][0])) < box.two_hw[0] && fabs(xsub(cc[j][1], sel_c[r][1])) < box.two_hw[1] &&
+                            fabs(xsub(cc[j][2], sel_c[r][2])) < box.two_hw[2] && fabs(xsub(cc[j][3], sel_c[r][3])) < box.two_hw[3];
+            if (ov || sj[j] == win) dead |= 1u << j;
+        }
+    }
+    // the candidates ran out while other seeds exist: the full rule decides
+    if (threadIdx.x == 0 && found < k_ref && n > M) fallback[p] = 1;
+}
+
 // The same selection by a thread-block cluster of COMET_REF_CLUSTER CTAs per partition: every CTA owns a
 // slice of the partition (its RSS values staged once in shared memory when they fit), each round the CTAs
 // publish their candidates in their own shared memory, synchronise the cluster, and every CTA merges the
@@ -153,8 +298,9 @@ k_select_refs(const double* __restrict__ seeds, int64_t stride, const double* __
 template <bool SMEM>
 __global__ void __cluster_dims__(COMET_REF_CLUSTER, 1, 1) __launch_bounds__(COMET_REF_THREADS)
 k_select_refs_cluster(const double* __restrict__ seeds, int64_t stride, const double* __restrict__ rss, PartOff po,
-                      RefBox box, int32_t k_ref, int64_t* __restrict__ ref_seed)
+                      RefBox box, int32_t k_ref, int64_t* __restrict__ ref_seed, const int* __restrict__ only_if = nullptr)
 {
+    if (only_if && !only_if[blockIdx.y]) return;            // (k_select_refs_short has served this partition)
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
     extern __shared__ __align__(16) double srss[];
