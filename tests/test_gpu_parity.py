@@ -693,6 +693,36 @@ def test_select_references_large_partitions(comet, n):
     np.testing.assert_array_equal(ref.cpu().numpy(), O.select_references(s, rss, po, hw, 12))
 
 
+@pytest.mark.parametrize("case", ["all_equal", "few_small", "sample_misses", "one_box", "nan_heavy"])
+def test_select_references_shortlist_fallbacks(comet, case):
+    """Large partitions take their references from the seeds below a sampled RSS threshold (k_select_refs_short) and fall
+    back to the full rule when that list cannot decide: every seed equal, fewer distinct small values than references,
+    a sample that misses the small values (more seeds below the threshold than the list holds), every seed in one box
+    (one reference only), mostly NaN."""
+    rng = np.random.default_rng(7)
+    n = 70000
+    s = np.zeros((6, n))
+    s[2:] = rng.normal(size=(4, n)) * np.array([[3.0], [5.0], [5.0], [8.0]])
+    rss = rng.uniform(0.5, 2.0, n)
+    if case == "all_equal":
+        rss[:] = 0.71
+    elif case == "few_small":
+        rss[:] = 0.71
+        rss[rng.integers(0, n, 5)] = 0.1
+    elif case == "sample_misses":
+        rss[:] = rng.uniform(0.1, 0.2, n)
+        rss[::n // 2048] = 5.0                               # the sampled positions hold the largest values
+    elif case == "one_box":
+        s[2:] = 0.0
+    elif case == "nan_heavy":
+        rss[rng.random(n) < 0.97] = np.nan
+    po = np.array([0, n])
+    hw = np.array([0.5, 1.0, 1.0, 2.0])
+    ref = comet.select_references(_dev(s), _dev(rss), po, hw, 12)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(ref.cpu().numpy(), O.select_references(s, rss, po, hw, 12))
+
+
 def test_select_references_cfg1_rss(comet, cfg1_event):
     ev = cfg1_event
     seeds, po = event_seeds(ev)
