@@ -263,7 +263,7 @@ class Leg:
         self.rss = torch.empty(self.S, dtype=torch.float64, device="cuda")
         self.n_pts = torch.empty(self.S, dtype=torch.int32, device="cuda")
         self.pairs = float(self.S) * ev.n_fired
-        c.reserve_scan(self.S, ev.n_steps, ev.n_fired)
+        c.reserve_scan(self.S, ev.n_steps, ev.n_fired, z_run=self.z_run)
         self.call_events = []
 
     def scan(self):
@@ -510,7 +510,7 @@ def run_ours(args):
         bctx = [Comet(local) for _ in range(n_str)]
         for q in bctx:
             q.set_option(OPT_ZGROUP, 1 if args.zgroup else 0)
-            q.reserve_scan(4 * 131072, bevs[0].n_steps, 250)
+            q.reserve_scan(4 * 131072, bevs[0].n_steps, 250, z_run=16)
         bstr = [torch.cuda.Stream() for _ in range(n_str)]
         dev = leg.dev
         d_wa, d_wb = leg.hits[0], leg.hits[1]

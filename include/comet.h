@@ -73,20 +73,23 @@ int comet_set_option(comet_ctx* ctx, int option, int value);
 int comet_get_option(const comet_ctx* ctx, int option, int* value);
 
 /* Sets the size of the (seed, wire) pair workspace of the pruned search to max_pairs_per_launch
- * pairs (8 bytes each, 12 on the materialised path; default limit 2^28) and allocates it now, so that later comet_dca_rss calls
+ * pairs (8 bytes each, 12 on the materialised path; default limit 2^29) and allocates it now, so that later comet_dca_rss calls
  * never allocate.  comet_dca_rss processes larger problems in seed slabs that fit; without this
  * call the workspace grows on the first comet_dca_rss that needs it (that call synchronises the
  * device). */
 int comet_reserve(comet_ctx* ctx, int64_t max_pairs_per_launch);
 
 /* Sizes every workspace comet_scan_rss (and the calls built on it: comet_scan_stage, comet_scan_turns, the
- * half-track calls) needs for seed sets of up to n_seeds seeds, n_steps steps and n_fired fired wires --
+ * half-track calls) needs for seed sets of up to n_seeds seeds (with the z_run the scans will promise, and for
+ * calls without a promise), n_steps steps and n_fired fired wires --
  * (seed, wire) pair keys, checkpoints, per-seed constants, the distinct-track rows of the z-run kernels --
  * under the current options and field mode, so that those calls never allocate or synchronise afterwards
  * (they can then be captured into a CUDA graph from the first call on).  Larger problems than comet_reserve's
- * pair limit or 8 GiB of checkpoints allow are processed in seed slabs of that size.  Synchronises the device
- * when it reallocates. */
-int comet_reserve_scan(comet_ctx* ctx, int64_t n_seeds, int32_t n_steps, int32_t n_fired);
+ * pair limit (default 2^29 pairs) or 8 GiB of checkpoints allow are processed in seed slabs of that size: with
+ * the run length promised a checkpoint is one z per seed and 8 states, without it (x, T) per seed and 4 states,
+ * so a promised configs[3] scan is one slab and an unpromised one ten.  Synchronises the device when it
+ * reallocates. */
+int comet_reserve_scan(comet_ctx* ctx, int64_t n_seeds, int32_t z_run, int32_t n_steps, int32_t n_fired);
 
 /* With COMET_OPT_TIMING = 1 the pruned comet_dca_rss and comet_scan_rss record CUDA events on the caller's
  * stream around their kernels (once per seed slab; comet_scan_rss then runs its sub-slabs one after the other).

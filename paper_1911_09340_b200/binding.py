@@ -122,7 +122,7 @@ def load_library():
     L.comet_scan_stage.argtypes = [vp, vp, i64, i64, i32, i32, dbl, dbl, i32, dbl,
                                    vp, vp, i32, vp, vp, vp, i32, i32, dbl,
                                    vp, i32, vp, vp, i32, dbl, i32, i32, vp, vp, vp, vp, vp, vp]
-    L.comet_reserve_scan.argtypes = [vp, i64, i32, i32]
+    L.comet_reserve_scan.argtypes = [vp, i64, i32, i32, i32]
     L.comet_seed_grid.argtypes = [vp, vp, i32, i32, i32, i32, i32, vp, i64, vp]
     L.comet_grid_axes_len.argtypes = [i32, i32, i32, i32]
     L.comet_grid_axes_len.restype = sz
@@ -218,9 +218,9 @@ class Comet:
         """Pre-allocates the pruned search's (seed, wire) pair workspace (12 bytes per pair)."""
         self._check(self._L.comet_reserve(self._h, int(max_pairs_per_launch)))
 
-    def reserve_scan(self, n_seeds: int, n_steps: int, n_fired: int):
+    def reserve_scan(self, n_seeds: int, n_steps: int, n_fired: int, z_run: int = 0):
         """comet_reserve_scan: sizes every workspace of comet_scan_rss & co.; later calls do not allocate."""
-        self._check(self._L.comet_reserve_scan(self._h, int(n_seeds), int(n_steps), int(n_fired)))
+        self._check(self._L.comet_reserve_scan(self._h, int(n_seeds), int(z_run), int(n_steps), int(n_fired)))
 
     def read_timing(self, names=("k_coarse_pruned", "k_fine", "k_rss_sum", "k_gen_unique")) -> dict:
         """Mean device milliseconds per kernel of the latest (<= 64) seed slabs of comet_dca_rss (pruned:

@@ -157,7 +157,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaMalloc(&ctx->pi, sizeof(int64_t) * COMET_MAX_PARTITIONS * COMET_ARGMIN_SPLIT);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->stats, sizeof(unsigned long long) * ST_N);
     if (e == cudaSuccess) e = cudaMemset(ctx->stats, 0, sizeof(unsigned long long) * ST_N);
-    ctx->pair_max = (size_t)1 << 28;
+    ctx->pair_max = (size_t)1 << 29;                        // 4 GiB of pair keys: configs[3] (4.2e8 pairs) is one slab
     ctx->ck_max = (size_t)8 << 30;
     ctx->fused_smem = ((COMET_FUSED_WFIELDS + 1) * COMET_FUSED_WCAP + COMET_FUSED_WARPS * COMET_FUSED_TR * 3 * COMET_LANES) * (int)sizeof(double);
     {
@@ -623,8 +623,15 @@ static ScanWs scan_ws(const comet_ctx* ctx, int64_t total_chunks, int32_t n_step
 {
     ScanWs w;
     const bool field = ctx->field.B != nullptr;
+    // (small calls are launch- and latency-bound: the run-length check and the chain of k_gen_unique in front of the
+    // scan cost more than they save below about a thousand chunks -- configs[0], the refined sets of a stage)
+    w.zgroup = !field && ctx->opt_zgroup != 0 && z_run != 1 &&
+               (ctx->opt_zgroup == 2 || total_chunks >= COMET_ZG_MIN_CHUNKS);
+    // checkpoints per chunk: (x, T) every 4th state for the plain kernels; with the run length promised only the
+    // z-run kernels run, which keep one z per seed every COMET_ZR_CK states
     w.n_ck = n_steps / COMET_CK_ROWS(field) + 1;
     w.ck_chunk = (size_t)w.n_ck * COMET_CK_FIELDS(field) * COMET_LANES * sizeof(double);
+    if (w.zgroup && z_run >= COMET_ZG_MIN) w.ck_chunk = (size_t)(n_steps / COMET_ZR_CK + 1) * COMET_LANES * sizeof(double);
     int64_t slab_chunks = total_chunks;
     if (n_fired > 0) {
         const int64_t by_pairs = (int64_t)(ctx->pair_max / ((size_t)COMET_LANES * (size_t)n_fired));
@@ -638,10 +645,6 @@ static ScanWs scan_ws(const comet_ctx* ctx, int64_t total_chunks, int32_t n_step
     w.ck = (size_t)slab_chunks * w.ck_chunk;
     w.cw = (size_t)slab_chunks * COMET_LANES * sizeof(double);
     w.npw = (size_t)slab_chunks * COMET_LANES * sizeof(int32_t);
-    // (small calls are launch- and latency-bound: the run-length check and the chain of k_gen_unique in front of the
-    // scan cost more than they save below about a thousand chunks -- configs[0], the refined sets of a stage)
-    w.zgroup = !field && ctx->opt_zgroup != 0 && z_run != 1 &&
-               (ctx->opt_zgroup == 2 || total_chunks >= COMET_ZG_MIN_CHUNKS);
     // distinct transverse tracks (scan_zgroup.cuh): 32 / run length per chunk (at most 4: runs of >= 8 seeds), each
     // u_rows = n_steps + 1 rounded up to whole 64-row blocks, 32 bytes per row
     w.tpc = (z_run >= COMET_ZG_MIN) ? (z_run >= 32 ? 1 : 32 / z_run) : 4;
@@ -689,16 +692,24 @@ static int scan_ws_grow(comet_ctx* ctx, const ScanWs& w)
     return COMET_OK;
 }
 
-extern "C" int comet_reserve_scan(comet_ctx* ctx, int64_t n_seeds, int32_t n_steps, int32_t n_fired)
+static bool bad_zrun(int32_t z_run) { return z_run < 0 || (z_run > 1 && (z_run < 8 || (z_run & (z_run - 1)) != 0)); }
+
+extern "C" int comet_reserve_scan(comet_ctx* ctx, int64_t n_seeds, int32_t z_run, int32_t n_steps, int32_t n_fired)
 {
-    if (!ctx || n_seeds < 1 || n_steps < 1 || n_steps > COMET_MAX_STEPS || n_fired < 0 || n_fired > ctx->wt_cap)
+    if (!ctx || n_seeds < 1 || n_steps < 1 || n_steps > COMET_MAX_STEPS || n_fired < 0 || n_fired > ctx->wt_cap || bad_zrun(z_run))
         return COMET_EINVAL;
     int rc = set_device(ctx);
     if (rc) return rc;
-    return scan_ws_grow(ctx, scan_ws(ctx, n_chunks_of(n_seeds), n_steps, n_fired, 0));
+    // a workspace that serves the promised run length and the call without a promise (whichever is larger, buffer by buffer)
+    ScanWs w = scan_ws(ctx, n_chunks_of(n_seeds), n_steps, n_fired, z_run);
+    if (z_run != 0) {
+        const ScanWs w0 = scan_ws(ctx, n_chunks_of(n_seeds), n_steps, n_fired, 0);
+        auto mx = [](size_t a, size_t b) { return a > b ? a : b; };
+        w.pairs = mx(w.pairs, w0.pairs); w.ck = mx(w.ck, w0.ck); w.cw = mx(w.cw, w0.cw); w.ub = mx(w.ub, w0.ub);
+        w.npu = mx(w.npu, w0.npu); w.tw = mx(w.tw, w0.tw); w.tm = mx(w.tm, w0.tm); w.npw = mx(w.npw, w0.npw);
+    }
+    return scan_ws_grow(ctx, w);
 }
-
-static bool bad_zrun(int32_t z_run) { return z_run < 0 || (z_run > 1 && (z_run < 8 || (z_run & (z_run - 1)) != 0)); }
 
 // comet_scan_rss; with seeds_host != NULL (HOST SoA [6][n_seeds]) every sub-slab first copies its seeds to
 // `seeds` on its own stream, so the upload of one sub-slab overlaps the kernels of the others

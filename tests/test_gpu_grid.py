@@ -192,7 +192,7 @@ def test_cold_context_first_call_captured_in_a_graph(cfg1_event):
             with torch.cuda.graph(g0, stream=side):
                 cold.scan_rss(seeds, *phys, *hits, ev.cutoff, rss=rss, n_pts=n_pts, z_run=16, stream=side)
         torch.cuda.synchronize()
-        cold.reserve_scan(S, ev.n_steps, ev.n_fired)
+        cold.reserve_scan(S, ev.n_steps, ev.n_fired, z_run=16)
         g = torch.cuda.CUDAGraph()
         with torch.cuda.graph(g, stream=side):
             cold.seed_grid(d_axes, shp, seeds=seeds, stream=side)
@@ -235,7 +235,7 @@ def test_turn_loop_replayed_from_a_graph(cfg1_event):
         cold = Comet(0)
         try:
             seeds = cold.seed_grid(_dev(axes), shp)
-            cold.reserve_scan(int(part_off[1]), ev.n_steps, ev.n_fired)
+            cold.reserve_scan(int(part_off[1]), ev.n_steps, ev.n_fired, z_run=16)
             torch.cuda.synchronize()
             g = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g, stream=side):
@@ -300,7 +300,7 @@ def test_full_cfg2_batch_on_streams_as_benchmarked():
             axes, shp, part_off = event_axes(ev)
             items.append((ev, _dev(axes), shp, part_off, _dev(ev.fired_wire), _dev(ev.hit_off), _dev(ev.rho)))
         for q in ctxs:
-            q.reserve_scan(4 * 131072, events[0].n_steps, 250)
+            q.reserve_scan(4 * 131072, events[0].n_steps, 250, z_run=16)
         torch.cuda.synchronize()
         for k, (ev, d_axes, shp, part_off, fw, ho, rho) in enumerate(items):
             q, st = ctxs[k % n_str], streams[k % n_str]
