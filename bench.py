@@ -568,8 +568,17 @@ def run_ours(args):
         swork = so["work"]
         ms_stage, so = _time_steps(lambda: c.scan_stage(leg.seeds, leg.part_off, *leg.phys, ev.r_stop, *leg.hits, ev.cutoff,
                                                         work=swork, **skw), 5, stream)
+        # the stage only enqueues work: replayed from a CUDA graph the launch gaps go
+        gs, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(gs, stream=side):
+            so_g = c.scan_stage(leg.seeds, leg.part_off, *leg.phys, ev.r_stop, *leg.hits, ev.cutoff, work=swork, stream=side, **skw)
+        gs.replay()
+        ms_stage_graph, _ = _time_steps(gs.replay, 5, stream)
+        assert bool(torch.equal(so_g["final_rss"], so["final_rss"]))
+        del gs, so_g
         g = int(np.prod(STAGE_GRID))
-        stage = {"ms_per_stage": ms_stage, "iterations": 4, "seeds_per_iteration": [leg.S] + [leg.P * 10 * g] * 3,
+        stage = {"ms_per_stage": ms_stage, "ms_per_stage_graph_replay": ms_stage_graph, "iterations": 4, "seeds_per_iteration": [leg.S] + [leg.P * 10 * g] * 3,
                  "dca_evals_per_s": (leg.S + 3 * leg.P * 10 * g) * ev.n_fired / (ms_stage * 1e-3),
                  "best_rss_first_iteration": out["best_rss"].cpu().numpy().tolist(),
                  "best_rss_final": so["final_rss"][:, 0].cpu().numpy().tolist(),

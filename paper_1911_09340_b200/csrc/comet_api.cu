@@ -719,7 +719,8 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                          const double* wire_a, const double* wire_b, int32_t n_wires,
                          const int32_t* fired_wire, const int32_t* hit_off, const double* rho,
                          int32_t n_fired, int32_t n_hits, double cutoff_cm,
-                         double* rss, int32_t* n_pts, void* cuda_stream, const int32_t* dyn = nullptr)
+                         double* rss, int32_t* n_pts, void* cuda_stream, const int32_t* dyn = nullptr,
+                         bool wire_table_ready = false)
 {
     if (!ctx || n_seeds < 0 || seed_stride < n_seeds || bad_physics(charge, bz_tesla, step_cm, n_steps) ||
         !(r_stop_cm >= 0.0) || bad_zrun(z_run) ||
@@ -743,8 +744,11 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
         rc = scan_ws_grow(ctx, ws);
         if (rc) return rc;
     }
-    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
-    if (rc) return rc;
+    // (the later iterations of a stage scan against the same hit list: the table of the first one stands)
+    if (!wire_table_ready) {
+        rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
+        if (rc) return rc;
+    }
     const int32_t n_ck = ws.n_ck;
     const size_t ck_chunk = ws.ck_chunk;
     const int64_t slab_chunks = ws.slab_chunks;
@@ -1218,7 +1222,7 @@ static int scan_stage_impl(comet_ctx* ctx, const double* seeds, int64_t seed_str
         // (the caller's promise is about the seeds it passed: the refined sets are checked on the device)
         rc = scan_rss_impl(ctx, nullptr, nullptr, cur, cur_stride, cur_n, it == 0 ? z_run : 0, charge, bz_tesla, step_cm, n_steps,
                            r_stop_cm, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, n_hits, cutoff_cm, rss, nullptr,
-                           cuda_stream, dyn);
+                           cuda_stream, dyn, it > 0);
         if (rc) return rc;
         if (it == n_iter) break;
         rc = comet_select_references(ctx, cur, cur_stride, cur_n, rss, po_cur, n_part, hw, k_ref, ref, cuda_stream);
