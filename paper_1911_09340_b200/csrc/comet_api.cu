@@ -16,6 +16,7 @@
 #include "scan_fused.cuh"
 #include "scan_zgroup.cuh"
 #include "scan_zrun.cuh"
+#include "scan_small.cuh"
 #include "refine.cuh"
 #include "turns.cuh"
 #include "hough.cuh"
@@ -161,11 +162,10 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     ctx->ck_max = (size_t)8 << 30;
     ctx->fused_smem = ((COMET_FUSED_WFIELDS + 1) * COMET_FUSED_WCAP + COMET_FUSED_WARPS * COMET_FUSED_TR * 3 * COMET_LANES) * (int)sizeof(double);
     {
-        const void* fk[8] = {(const void*)k_scan_fused<false, false>, (const void*)k_scan_fused<true, false>,
+        const void* fk[6] = {(const void*)k_scan_fused<false, false>, (const void*)k_scan_fused<true, false>,
                              (const void*)k_scan_fused<false, true>, (const void*)k_scan_fused<true, true>,
-                             (const void*)k_scan_fused<false, false, true>, (const void*)k_scan_fused<true, false, true>,
                              (const void*)k_scan_fused<false, true, true>, (const void*)k_scan_fused<true, true, true>};
-        for (int j = 0; j < 8 && e == cudaSuccess; ++j) {
+        for (int j = 0; j < 6 && e == cudaSuccess; ++j) {
             e = cudaFuncSetAttribute(fk[j], cudaFuncAttributeMaxDynamicSharedMemorySize, ctx->fused_smem);
             if (e == cudaSuccess) e = cudaFuncSetAttribute(fk[j], cudaFuncAttributePreferredSharedMemoryCarveout, 100);
         }
@@ -825,8 +825,10 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             if (tm && !zgroup) CU(ctx, cudaEventRecord(tev[1], st));    // (no k_gen_unique: an empty slot)
             const int thr = 32 * COMET_FUSED_WARPS;
             // a launch that cannot give every SM two CTAs of four chunks: the CTA's warps share one chunk's wires
-            const bool split = !zgroup && n_fired > 32 && nc < (int64_t)COMET_FUSED_WARPS * ctx->n_sm * 2;
-            const unsigned b1 = split ? (unsigned)nc : b1_packed;
+            const bool small = !zgroup && nc < (int64_t)COMET_FUSED_WARPS * ctx->n_sm * 2;
+            const bool split = small && field && n_fired > 32;   // (field map: the warps of a CTA repeat the chunk's chain)
+            const bool overlap = small && !field;                // uniform field: one generator warp, three search warps (scan_small.cuh)
+            const unsigned b1 = (split || overlap) ? (unsigned)nc : b1_packed;
             a.zg = nullptr;
             a.zrun = zrun_host;
             a.ub = nullptr;
@@ -870,14 +872,12 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             }
             if (zrun_host) {
                 // (the ZG kernels serve the launch: the plain variants are not enqueued)
+            } else if (overlap) {
+                if (a.stats) k_scan_small<true><<<b1, 128, COMET_SMALL_SMEM, s_scan>>>(a);
+                else k_scan_small<false><<<b1, 128, COMET_SMALL_SMEM, s_scan>>>(a);
             } else if (split) {
-                if (field) {
-                    if (a.stats) k_scan_fused<true, true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
-                    else k_scan_fused<false, true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
-                } else {
-                    if (a.stats) k_scan_fused<true, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
-                    else k_scan_fused<false, false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
-                }
+                if (a.stats) k_scan_fused<true, true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
+                else k_scan_fused<false, true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
             } else if (field) {
                 if (a.stats) k_scan_fused<true, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
                 else k_scan_fused<false, true><<<b1, thr, ctx->fused_smem, s_scan>>>(a);
