@@ -77,22 +77,45 @@ __global__ void __launch_bounds__(128, 4) k_scan_small(const FusedArgs a)
     int32_t np = valid ? a.n_steps + 1 : 0;
     const bool use_stop = a.r_stop2 > 0.0;
     double* ckc = a.ck + (size_t)chunk * a.n_ck * (CKF * COMET_LANES) + lane;
+    // The chain of dependent operations of a step is the generator's whole cost, so the stop test does not sit on it: blocks
+    // of 4 steps are taken and stored unconditionally, the first state in the target region is only remembered, and the
+    // rows after it are overwritten with it afterwards (hold-last); a lane that has stopped just repeats its last position.
     auto generate = [&](int t) {
         double* tile = tiles + (t & 1) * (TR * ROW);
         const int r0 = t * TR;
-#pragma unroll 2
-        for (int rr = 0; rr < TR; ++rr) {
-            const int k = r0 + rr;
-            if (k > 0 && active) {
-                rkn4_step(st, a.hk, c);
-                if (use_stop && in_target_region(st, a.r_stop2)) { np = k + 1; active = false; }
-            }
-            if (k >= a.n_steps) active = false;
-            double* tr = tile + rr * ROW + lane;
-            tr[0] = st.x0; tr[32] = st.x1; tr[64] = st.x2;
-            if ((rr & (CK - 1)) == 0 && k <= a.n_steps) {
-                double* o = ckc + (size_t)(k / CK) * (CKF * COMET_LANES);
-                o[0] = st.x0; o[32] = st.x1; o[64] = st.x2; o[96] = st.t0; o[128] = st.t1; o[160] = st.t2;
+#pragma unroll 1
+        for (int b = 0; b < TR; b += 4) {
+            const int k0 = r0 + b;
+            double* tb = tile + b * ROW + lane;
+            if (active) {
+                int first = 4;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int k = k0 + j;
+                    if (k > 0 && k <= a.n_steps) {          // (warp-uniform: row 0 is the seed, rows past the capacity repeat the last state)
+                        rkn4_step(st, a.hk, c);
+                        const double r2 = xadd(xmul(st.x0, st.x0), xmul(st.x1, st.x1));
+                        const double rad = xadd(xmul(st.x0, st.t0), xmul(st.x1, st.t1));
+                        const bool stop = (r2 < a.r_stop2) & (rad < 0.0) & use_stop;
+                        first = (stop & (first == 4)) ? j : first;
+                    }
+                    tb[j * ROW] = st.x0; tb[j * ROW + 32] = st.x1; tb[j * ROW + 64] = st.x2;
+                    if (j == 0 && k <= a.n_steps) {
+                        double* o = ckc + (size_t)(k / CK) * (CKF * COMET_LANES);
+                        o[0] = st.x0; o[32] = st.x1; o[64] = st.x2; o[96] = st.t0; o[128] = st.t1; o[160] = st.t2;
+                    }
+                }
+                if (first < 4) {
+                    np = k0 + first + 1;
+                    active = false;
+                    st.x0 = tb[first * ROW]; st.x1 = tb[first * ROW + 32]; st.x2 = tb[first * ROW + 64];
+                    for (int j = first + 1; j < 4; ++j) { tb[j * ROW] = st.x0; tb[j * ROW + 32] = st.x1; tb[j * ROW + 64] = st.x2; }
+                } else if (k0 + 3 >= a.n_steps) {
+                    active = false;                         // capacity reached: np stays n_steps + 1
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < 4; ++j) { tb[j * ROW] = st.x0; tb[j * ROW + 32] = st.x1; tb[j * ROW + 64] = st.x2; }
             }
         }
         s_np[t & 1][lane] = np;
