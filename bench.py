@@ -267,9 +267,12 @@ class Leg:
         self.call_events = []
 
     def scan(self):
+        self.scan_on(None)
+
+    def scan_on(self, stream):
         ev = self.ev
         self.c.scan_rss(self.seeds, *self.phys, ev.r_stop, *self.hits, ev.cutoff, rss=self.rss, n_pts=self.n_pts,
-                        z_run=self.z_run)
+                        z_run=self.z_run, stream=stream)
 
     def step(self, stream=None):
         ev, torch = self.ev, self.torch
@@ -296,6 +299,16 @@ class Leg:
         self.out = out
         r = {"ms_per_event": ms, "ms_scan_call": ms_call, "dca_evals_per_s": self.pairs / (ms * 1e-3),
              "events_per_s": 1.0 / (ms * 1e-3)}
+        # the step only enqueues work (workspace reserved): replayed from a CUDA graph the launch gaps go
+        g, side = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+        with torch.cuda.graph(g, stream=side):
+            self.scan_on(side)
+            go = c.select_and_classify(self.seeds, *self.phys, self.ev.r_stop, *self.hits, self.ev.cutoff, self.rss, self.part_off,
+                                       stream=side)
+        g.replay()
+        r["ms_per_event_graph_replay"], _ = _time_steps(g.replay, steps, stream)
+        assert bool(torch.equal(go["best_seed"], out["best_seed"])) and bool(torch.equal(go["cls"], out["cls"]))
+        del g, go
         if kernels:
             names = ("k_scan", "k_fine_ck", "k_rss_sum", "k_gen_unique")
             c.set_option(OPT_TIMING, 1)
