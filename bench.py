@@ -662,7 +662,8 @@ def run_ours(args):
         d_layer, d_circ = dev(ev.geom.layer), ho1["circle"][0].contiguous()
         hfn = lambda: c.scan_half_tracks(se, sx, *leg.phys, 1.0e3, *leg.hits, ev.cutoff, d_layer, d_circ, 3.0, 3, **hkw)
         hfn()
-        ms_half, hout_ = _time_steps(hfn, 5, stream)
+        hfn()
+        ms_half, hout_ = min((_time_steps(hfn, 10, stream) for _ in range(3)), key=lambda v: v[0])   # (the call synchronises: host jitter)
         seeding = {"hough": {"events": len(lists), "fired_wires": int(ev_off[-1]), "ms_per_graph_replay": ms_hg,
                              "votes_per_s": float(ev_off[-1]) * HOUGH_N_PHI / (ms_hg * 1e-3), "events_per_s": len(lists) / (ms_hg * 1e-3),
                              "accumulator": "%d directions x %d rho bins per event" % (HOUGH_N_PHI, HOUGH_N_RHO)},
