@@ -239,6 +239,11 @@ int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int
  *   part_off   HOST [n_part+1], non-decreasing, within [0, n_seeds]; read before returning
  *   best_seed  dev [n_part] (global seed index, -1 for an empty partition), best_rss dev [n_part],
  *   best_dca   dev [n_part][n_fired], cls dev [n_part][n_hits]
+ * A NaN in rss follows the serial rule "rss[s] < rss[best]": it wins only at the first seed of a partition.
+ * When the last comet_scan_rss of this ctx scanned exactly this seed set (same buffer, stride, count and physics,
+ * z_run promised, one slab), the winner's (x, y, T_x, T_y) rows are copied from that scan's distinct-track
+ * workspace instead of being stepped again -- the same numbers; the seeds must not have been rewritten in
+ * between (rss would be stale as well).
  * Limits: n_part <= COMET_MAX_PARTITIONS, n_steps <= COMET_MAX_STEPS. */
 int comet_select_and_classify(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
                               int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
