@@ -110,20 +110,38 @@ __global__ void __launch_bounds__(32) k_gen_unique(const FusedArgs a)
     // before) overwrites the rows after its last state with it: the hold-last padding.
     const int n_rows = a.n_steps + 1;
     int k = 0;                                              // first row of the round
+    // A round cannot hold a stop while every lane is farther outside the target region than a round's steps can cover
+    // (a step moves the position by at most 1.001 h) and the capacity is not reached: such a round skips the tests.
+    const double far_r = sqrt(a.r_stop2) + (GR + 1) * 1.001 * a.hk.h;
+    const double far2 = far_r * far_r;
+    bool quiet = false;                                     // (warp-uniform) the next round needs no test
     while (true) {
         const State hold = st;                              // (what a finished lane keeps)
         int first = GR;                                     // row of this round at which the lane stops
+        if (quiet) {
 #pragma unroll
-        for (int j = 0; j < GR; ++j) {
-            if (k + j > 0) {                                // (row 0: the seed state itself; warp-uniform)
+            for (int j = 0; j < GR; ++j) {
                 rkn4_step(st, a.hk, c);
-                // in_target_region without its early exit: no branch waits for this step's position
-                const double r2 = xadd(xmul(st.x0, st.x0), xmul(st.x1, st.x1));
-                const double rad = xadd(xmul(st.x0, st.t0), xmul(st.x1, st.t1));
-                const bool stop = ((r2 < a.r_stop2) & (rad < 0.0) & use_stop) | (k + j == n_rows - 1);
-                first = (stop & (first == GR)) ? j : first;
+                put(j);
             }
-            put(j);
+        } else {
+#pragma unroll
+            for (int j = 0; j < GR; ++j) {
+                if (k + j > 0) {                            // (row 0: the seed state itself; warp-uniform)
+                    rkn4_step(st, a.hk, c);
+                    // in_target_region without its early exit: no branch waits for this step's position
+                    const double r2 = xadd(xmul(st.x0, st.x0), xmul(st.x1, st.x1));
+                    const double rad = xadd(xmul(st.x0, st.t0), xmul(st.x1, st.t1));
+                    const bool stop = ((r2 < a.r_stop2) & (rad < 0.0) & use_stop) | (k + j == n_rows - 1);
+                    first = (stop & (first == GR)) ? j : first;
+                }
+                put(j);
+            }
+        }
+        {
+            const double r2e = fma(st.x0, st.x0, st.x1 * st.x1);
+            const bool lane_quiet = !active || !use_stop || r2e > far2;
+            quiet = __all_sync(FULL, lane_quiet) && (k + 2 * GR < n_rows - 1);
         }
         if (!active) {
             st = hold;
