@@ -52,7 +52,7 @@ struct comet_ctx {
     int32_t* kb;
     double* e2;
     unsigned long long* items;   // [pair_cap / 32] work list of k_fine
-    unsigned int* n_items;       // [COMET_MAX_LANES] (one counter per internal stream lane)
+    unsigned int* n_items;       // [COMET_MAX_LANES][4] per internal stream lane: items listed, items handed out by k_fine_ck
     // comet_scan_rss runs the sub-slabs of a slab concurrently: scan kernels on ls[], the fine stage on
     // the high-priority lf[] so that its CTAs take the slots retiring scan CTAs free
     int opt_lanes;
@@ -171,7 +171,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
         }
     }
     if (e == cudaSuccess) e = cudaMalloc(&ctx->bmax, sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int) * COMET_MAX_LANES);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->n_items, sizeof(unsigned int) * 4 * COMET_MAX_LANES);
     ctx->opt_lanes = COMET_DEFAULT_LANES;
     ctx->opt_zgroup = 1;
     if (e == cudaSuccess) e = cudaMalloc(&ctx->zg_flag, sizeof(unsigned int) * (COMET_MAX_LANES + 1));
@@ -806,7 +806,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             a.cw = ctx->cw + cl * COMET_LANES;
             a.tw = zgroup ? ctx->tw + cl * COMET_LANES : nullptr;
             a.items = ctx->items + (size_t)cl * (size_t)n_fired;
-            a.n_items = ctx->n_items + l;
+            a.n_items = ctx->n_items + 4 * l;
             a.stats = ctx->opt_stats ? ctx->stats : nullptr;
             a.dyn = dyn;
             if (lanes > 1) CU(ctx, cudaStreamWaitEvent(s_scan, ctx->ev_fork, 0));
@@ -814,7 +814,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 for (int j = 0; j < 6; ++j)
                     CU(ctx, cudaMemcpyAsync(seeds_w + (size_t)j * seed_stride + s0, seeds_host + (size_t)j * n_seeds + s0,
                                             sizeof(double) * (size_t)a.n_seeds, cudaMemcpyHostToDevice, s_scan));
-            CU(ctx, cudaMemsetAsync(a.n_items, 0, sizeof(unsigned int), s_scan));
+            CU(ctx, cudaMemsetAsync(a.n_items, 0, 4 * sizeof(unsigned int), s_scan));
             const unsigned b1_packed = (unsigned)((nc + COMET_FUSED_WARPS - 1) / COMET_FUSED_WARPS);
             const int64_t w2 = nc * (int64_t)n_fired;
             const int64_t b2_all = (w2 + COMET_FINE_THREADS / 32 - 1) / (COMET_FINE_THREADS / 32);

@@ -94,7 +94,7 @@ struct FusedArgs {
     double* cw;              // [SP] curvature constant c = kappa q B_z / |p| of every seed, for k_fine_ck
     double* tw;              // [SP] ZG: T_z of every seed, for k_fine_ck
     unsigned long long* items;
-    unsigned int* n_items;
+    unsigned int* n_items;   // [0] items listed by the scan, [1] items handed out by k_fine_ck
     unsigned long long* stats;
     FieldMap F;              // field-map variants (FIELD = true): the map, and qkb = kappa q, hk.h = h_max
     double h_min;            // h_max / 64 (R31)
@@ -430,7 +430,13 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, FIELD ? COMET_FINE_MINB_FI
     const unsigned n_warps = gridDim.x * (COMET_FINE_THREADS / 32);
     const int W = a.W;
     const double lam2 = xmul(a.lambda, a.lambda);
-    for (unsigned it = blockIdx.x * (COMET_FINE_THREADS / 32) + (threadIdx.x >> 5); it < n_items; it += n_warps) {
+    // a warp's first item is its own index; the next ones are handed out by a counter -- asked for before the work on the
+    // current item, so the answer is there when it is needed: items differ in cost (live lanes, iterations of O6) and the
+    // grid is one wave, so a fixed share per warp would leave a fifth of the warp slots idle towards the end
+    unsigned it = blockIdx.x * (COMET_FINE_THREADS / 32) + (threadIdx.x >> 5);
+    while (it < n_items) {
+        unsigned nxt = 0;
+        if (lane == 0) nxt = n_warps + atomicAdd(a.n_items + 1, 1u);
         const unsigned long long item = a.items[it];
         const int64_t chunk = (int64_t)(item >> 16);
         const int i = (int)(item & 0xffffu);
@@ -524,6 +530,7 @@ __global__ void __launch_bounds__(COMET_FINE_THREADS, FIELD ? COMET_FINE_MINB_FI
             e2 = xmul(e, e);
         }
         a.bd[pidx] = e2;
+        it = __shfl_sync(0xffffffffu, nxt, 0);
     }
 }
 
