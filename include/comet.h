@@ -241,9 +241,13 @@ int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int
  *   best_dca   dev [n_part][n_fired], cls dev [n_part][n_hits]
  * A NaN in rss follows the serial rule "rss[s] < rss[best]": it wins only at the first seed of a partition.
  * When the last comet_scan_rss of this ctx scanned exactly this seed set (same buffer, stride, count and physics,
- * z_run promised, one slab), the winner's (x, y, T_x, T_y) rows are copied from that scan's distinct-track
- * workspace instead of being stepped again -- the same numbers; the seeds must not have been rewritten in
- * between (rss would be stale as well).
+ * uniform field, one slab), the winner's track is not stepped again as one chain of n_steps dependent steps: with
+ * z_run promised its (x, y, T_x, T_y) rows are copied from that scan's distinct-track workspace; after the plain
+ * kernels (small sets, z_run = 1) every 4th recorded state is that scan's checkpoint and the three states after
+ * it are stepped by one thread per checkpoint -- the same numbers either way.  If the hit-list arguments are
+ * also that call's (same arrays and sizes, cutoff, step) its wire table is used as it stands.  The seed and
+ * hit-list arrays must not have been rewritten between the two calls (rss would be stale as well).
+ * Partitions of at most 16384 seeds are searched by the classifying CTA itself (one launch).
  * Limits: n_part <= COMET_MAX_PARTITIONS, n_steps <= COMET_MAX_STEPS. */
 int comet_select_and_classify(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,
                               int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,

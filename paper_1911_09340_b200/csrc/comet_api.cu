@@ -23,6 +23,8 @@
 #include "half.cuh"
 #include "seedgrid.cuh"
 
+static_assert(COMET_SEL_CK == COMET_FUSED_CK, "select.cuh steps the states between the checkpoints of scan_fused.cuh");
+
 #ifndef COMET_PRUNED_WT
 #define COMET_PRUNED_WT 3
 #endif
@@ -97,12 +99,21 @@ struct comet_ctx {
     size_t tbuf_bytes;
     // the comet_scan_rss call whose distinct transverse tracks are still in `ub`, one slab, run length promised: the
     // classification of the winners copies their rows instead of stepping them again (select.cuh)
+    // (valid = 2: uniform field, plain kernels: the (x, T) checkpoints of every 4th recorded state are still in `ck`)
     struct {
         const double* seeds;
         int64_t stride, n_seeds;
         double qkb, step, r_stop;
-        int32_t n_steps, zshift, u_rows, valid;
+        int32_t n_steps, zshift, u_rows, n_ck, valid;
     } last;
+    // the hit list the wire table `wt` was last built from (launch_wire_prep): comet_select_and_classify does not build it
+    // again after the comet_scan_rss call it follows
+    struct {
+        const double *wire_a, *wire_b, *rho;
+        const int32_t *fired_wire, *hit_off;
+        int32_t n_wires, n_fired, uniform;
+        double cutoff, step;
+    } wt_of;
     void* hstage;          // pinned host staging of comet_scan_event_grid_host: one copy in, one copy out per event
     size_t hstage_bytes;
     // detector geometry kept on the device for the host-buffer entry points (comet_set_geometry)
@@ -477,10 +488,25 @@ static int launch_wire_prep(comet_ctx* ctx, const double* wire_a, const double* 
 {
     if (n_fired > ctx->wt_cap) return COMET_EINVAL;
     if (n_fired == 0) return COMET_OK;
+    const int32_t uniform = ctx->field.B == nullptr ? 1 : 0;
     k_wire_prep<<<(n_fired + 127) / 128, 128, 0, st>>>(wire_a, wire_b, n_wires, fired_wire, n_fired, hit_off, rho,
-                                                       cutoff_cm, step_cm, ctx->field.B == nullptr ? 1 : 0, ctx->wt);
+                                                       cutoff_cm, step_cm, uniform, ctx->wt);
     CU(ctx, cudaGetLastError());
+    ctx->wt_of.wire_a = wire_a; ctx->wt_of.wire_b = wire_b; ctx->wt_of.rho = rho; ctx->wt_of.fired_wire = fired_wire;
+    ctx->wt_of.hit_off = hit_off; ctx->wt_of.n_wires = n_wires; ctx->wt_of.n_fired = n_fired; ctx->wt_of.uniform = uniform;
+    ctx->wt_of.cutoff = cutoff_cm; ctx->wt_of.step = step_cm;
     return COMET_OK;
+}
+
+// the table in `wt` is the one launch_wire_prep would build from these arguments (same arrays, same sizes)
+static bool wire_table_is(const comet_ctx* ctx, const double* wire_a, const double* wire_b, int32_t n_wires,
+                          const int32_t* fired_wire, const int32_t* hit_off, const double* rho, int32_t n_fired,
+                          double cutoff_cm, double step_cm)
+{
+    return ctx->wt_of.wire_a == wire_a && ctx->wt_of.wire_b == wire_b && ctx->wt_of.rho == rho &&
+           ctx->wt_of.fired_wire == fired_wire && ctx->wt_of.hit_off == hit_off && ctx->wt_of.n_wires == n_wires &&
+           ctx->wt_of.n_fired == n_fired && ctx->wt_of.uniform == (ctx->field.B == nullptr ? 1 : 0) &&
+           ctx->wt_of.cutoff == cutoff_cm && ctx->wt_of.step == step_cm;
 }
 
 static bool bad_hits(const double* wire_a, const double* wire_b, int32_t n_wires, const int32_t* fired_wire,
@@ -909,6 +935,13 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             for (int l = 0; l < used; ++l) CU(ctx, cudaStreamWaitEvent(st, ctx->ev_join[l], 0));
     }
     ctx->last.valid = 0;
+    if (!zgroup && !field && slab_chunks >= total_chunks && !seeds_host) {
+        // plain kernels, uniform field: the checkpoints of the whole seed set are in `ck`, chunk after chunk
+        ctx->last.seeds = seeds; ctx->last.stride = seed_stride; ctx->last.n_seeds = n_seeds;
+        ctx->last.qkb = COMET_KAPPA * (double)charge * bz_tesla; ctx->last.step = step_cm; ctx->last.r_stop = r_stop_cm;
+        ctx->last.n_steps = n_steps; ctx->last.n_ck = n_ck;
+        ctx->last.valid = 2;
+    }
     if (zrun_host && slab_chunks >= total_chunks && !seeds_host) {
         ctx->last.seeds = seeds; ctx->last.stride = seed_stride; ctx->last.n_seeds = n_seeds;
         ctx->last.qkb = COMET_KAPPA * (double)charge * bz_tesla; ctx->last.step = step_cm; ctx->last.r_stop = r_stop_cm;
@@ -959,11 +992,27 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
-    if (rc) return rc;
-    k_argmin_stage1<<<dim3(COMET_ARGMIN_SPLIT, n_part), COMET_ARGMIN_THREADS, 0, st>>>(rss, po, ctx->pv, ctx->pi);
-    CU(ctx, cudaGetLastError());
+    // what the comet_scan_rss call that produced rss left in the ctx, if this is that seed set (same buffer, same physics)
+    const bool field = ctx->field.B != nullptr;
+    const double qkb_u = COMET_KAPPA * (double)charge * bz_tesla;
+    const bool same_scan = !field && ctx->last.valid && ctx->last.seeds == seeds && ctx->last.stride == seed_stride &&
+                           ctx->last.n_seeds == n_seeds && ctx->last.qkb == qkb_u && ctx->last.step == step_cm &&
+                           ctx->last.r_stop == r_stop_cm && ctx->last.n_steps == n_steps;
+    if (!(same_scan && wire_table_is(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm))) {
+        rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
+        if (rc) return rc;
+    }
+    int64_t part_max = 0;
+    for (int p = 0; p < n_part; ++p)
+        if (po.off[p + 1] - po.off[p] > part_max) part_max = po.off[p + 1] - po.off[p];
+    const bool fused_argmin = part_max <= COMET_ARGMIN_FUSED;
+    if (!fused_argmin) {
+        k_argmin_stage1<<<dim3(COMET_ARGMIN_SPLIT, n_part), COMET_ARGMIN_THREADS, 0, st>>>(rss, po, ctx->pv, ctx->pi);
+        CU(ctx, cudaGetLastError());
+    }
     ClassifyArgs a;
+    a.rss = fused_argmin ? rss : nullptr;
+    a.po = po;
     a.seeds = seeds;
     a.stride = seed_stride;
     a.qkb = COMET_KAPPA * (double)charge * bz_tesla;
@@ -982,16 +1031,13 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     a.best_rss = best_rss;
     a.best_dca = best_dca;
     a.cls = cls;
-    const bool field = ctx->field.B != nullptr;
     if (field) a.qkb = COMET_KAPPA * (double)charge;
     a.F = ctx->field;
     a.h_min = step_cm / 64.0;
-    // the tracks of the scan that produced rss, if this is that seed set (same buffer, same physics)
-    a.ub = nullptr; a.np_u = nullptr; a.zshift = 0; a.u_rows = 0; a.dyn = nullptr;
-    if (!field && ctx->last.valid && ctx->last.seeds == seeds && ctx->last.stride == seed_stride && ctx->last.n_seeds == n_seeds &&
-        ctx->last.qkb == a.qkb && ctx->last.step == step_cm && ctx->last.r_stop == r_stop_cm && ctx->last.n_steps == n_steps) {
-        a.ub = ctx->ub; a.np_u = ctx->npu; a.zshift = ctx->last.zshift; a.u_rows = ctx->last.u_rows;
-    }
+    // the winners' tracks: the rows of their distinct transverse tracks, or the checkpoints of the plain kernels
+    a.ub = nullptr; a.np_u = nullptr; a.zshift = 0; a.u_rows = 0; a.dyn = nullptr; a.ck = nullptr; a.n_ck = 0;
+    if (same_scan && ctx->last.valid == 1) { a.ub = ctx->ub; a.np_u = ctx->npu; a.zshift = ctx->last.zshift; a.u_rows = ctx->last.u_rows; }
+    if (same_scan && ctx->last.valid == 2) { a.ck = ctx->ck; a.n_ck = ctx->last.n_ck; }
     const size_t smem = (size_t)(n_steps + 1) * (field ? 7 : 6) * sizeof(double);
     if (field) k_select_classify<true><<<n_part, 256, smem, st>>>(a);
     else k_select_classify<false><<<n_part, 256, smem, st>>>(a);
@@ -1117,6 +1163,8 @@ static int launch_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t se
     a.rho = rho;
     a.n_hits = n_hits;
     a.lambda = cutoff_cm;
+    a.ck = nullptr; a.n_ck = 0; a.rss = nullptr;
+    memset(&a.po, 0, sizeof(a.po));
     const bool field = ctx->field.B != nullptr;
     if (field) a.qkb = COMET_KAPPA * (double)charge;
     a.F = ctx->field;

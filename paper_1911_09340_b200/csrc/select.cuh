@@ -11,6 +11,8 @@ struct PartOff {
 
 #define COMET_ARGMIN_SPLIT 64   // CTAs per partition in the first argmin stage
 #define COMET_ARGMIN_THREADS 256
+#define COMET_ARGMIN_FUSED 16384 // partitions up to this size skip the first stage: the CTA of k_select_classify scans them
+#define COMET_SEL_CK 4           // = COMET_FUSED_CK (scan_fused.cuh; checked there): rows between the scan's checkpoints
 
 // (value, index) ordering of R15: smaller rss wins, equal rss -> lower index.  NaN never wins
 // against a number (the comparison is false), exactly as the serial scan "rss[s] < rss[b]".
@@ -24,17 +26,13 @@ __device__ __forceinline__ void argmin_merge(double& v, int64_t& i, double v2, i
 // position of the partition stays the winner whatever follows, a NaN anywhere else never wins.  Reproduced here by
 // skipping NaNs at s > lo and giving a NaN at lo the value -infinity (RSS is a sum of squares: no number is that
 // small); k_select_classify turns it back into the NaN it stands for.
-__global__ void __launch_bounds__(COMET_ARGMIN_THREADS)
-k_argmin_stage1(const double* __restrict__ rss, PartOff po, double* __restrict__ pv, int64_t* __restrict__ pi)
+// one thread's share [first, first + step, ...) of [.., hi) of the partition that starts at lo, then the warp's minimum
+__device__ __forceinline__ void partition_argmin(const double* __restrict__ rss, int64_t lo, int64_t first, int64_t hi,
+                                                 int64_t step, double& v, int64_t& idx)
 {
-    const int p = blockIdx.y;
-    const int64_t lo = po.off[p], hi = po.off[p + 1];
-    const int64_t n = hi - lo;
-    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
-    const int64_t b = lo + per * blockIdx.x, e = min(hi, b + per);
-    double v = 0.0;
-    int64_t idx = -1;
-    for (int64_t s = b + threadIdx.x; s < e; s += blockDim.x) {
+    v = 0.0;
+    idx = -1;
+    for (int64_t s = first; s < hi; s += step) {
         double r = rss[s];
         if (r != r) {
             if (s != lo) continue;
@@ -47,6 +45,19 @@ k_argmin_stage1(const double* __restrict__ rss, PartOff po, double* __restrict__
         const int64_t i2 = __shfl_down_sync(0xffffffffu, idx, o);
         argmin_merge(v, idx, v2, i2);
     }
+}
+
+__global__ void __launch_bounds__(COMET_ARGMIN_THREADS)
+k_argmin_stage1(const double* __restrict__ rss, PartOff po, double* __restrict__ pv, int64_t* __restrict__ pi)
+{
+    const int p = blockIdx.y;
+    const int64_t lo = po.off[p], hi = po.off[p + 1];
+    const int64_t n = hi - lo;
+    const int64_t per = (n + gridDim.x - 1) / gridDim.x;
+    const int64_t b = lo + per * blockIdx.x, e = min(hi, b + per);
+    double v;
+    int64_t idx;
+    partition_argmin(rss, lo, b + threadIdx.x, e, blockDim.x, v, idx);
     __shared__ double sv[COMET_ARGMIN_THREADS / 32];
     __shared__ int64_t si[COMET_ARGMIN_THREADS / 32];
     if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = v; si[threadIdx.x >> 5] = idx; }
@@ -84,6 +95,12 @@ struct ClassifyArgs {
     const double* ub;          // [track][u_rows][4], nullptr = record the track here
     const int32_t* np_u;
     int32_t zshift, u_rows;
+    // or (uniform field, plain scan kernels) that call's checkpoints: (x, T) of every COMET_SEL_CK-th recorded state of
+    // every seed, [chunk][n_ck][6][32]; the states in between are stepped by one thread per checkpoint
+    const double* ck;          // nullptr = no checkpoints
+    int32_t n_ck;
+    const double* rss;         // partitions of at most COMET_ARGMIN_FUSED seeds: k_select_classify takes the argmin itself
+    PartOff po;
     const int32_t* dyn;        // comet_scan_turns: device {.., .., stop flag}: set = write nothing
 };
 
@@ -123,6 +140,33 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
             double z = st.x2;
             sm[2] = z;
             for (int k = 1; k < np; ++k) { z = xadd(z, hz); sm[(size_t)k * RS + 2] = z; }
+        }
+    } else if (!FIELD && a.ck) {
+        // the same numbers without the chain: thread m starts from checkpoint m (recorded state m CK, bit for bit) and steps
+        // the CK - 1 states after it.  The first state in the target region ends the track (R3); the checkpoints behind it
+        // were never written and whatever those threads compute is not read (pure arithmetic: nothing is addressed by it).
+        constexpr int CK = COMET_SEL_CK;
+        State s0;
+        const double c = seed_init(a.seeds, a.stride, idx, a.qkb, s0);
+        if (threadIdx.x == 0) { s_c = c; s_np = a.n_steps + 1; }
+        __syncthreads();
+        const double* base = a.ck + (size_t)(idx >> 5) * (size_t)a.n_ck * (6 * COMET_LANES) + (idx & 31);
+        const bool use_stop = a.r_stop2 > 0.0;
+        for (int m = threadIdx.x; m * CK <= a.n_steps; m += blockDim.x) {
+            const double* o = base + (size_t)m * (6 * COMET_LANES);
+            State st;
+            st.x0 = o[0]; st.x1 = o[32]; st.x2 = o[64]; st.t0 = o[96]; st.t1 = o[128]; st.t2 = o[160];
+            int first = 1 << 30;
+#pragma unroll
+            for (int j = 0; j < CK; ++j) {
+                const int k = m * CK + j;
+                if (k > a.n_steps) break;
+                if (j > 0) rkn4_step(st, a.hk, c);
+                double* r = sm + (size_t)k * RS;
+                r[0] = st.x0; r[1] = st.x1; r[2] = st.x2; r[3] = st.t0; r[4] = st.t1; r[5] = st.t2;
+                if (use_stop && k > 0 && first > k && in_target_region(st, a.r_stop2)) first = k;
+            }
+            if (first < (1 << 30)) atomicMin(&s_np, first + 1);
         }
     } else
     if (threadIdx.x == 0) {
@@ -225,7 +269,22 @@ __global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
     extern __shared__ __align__(16) double sm[];       // [(n_steps+1)][6]
     __shared__ int64_t s_best;
     const int p = blockIdx.x;
-    if (threadIdx.x == 0) {
+    if (a.rss) {
+        // a small partition: the whole argmin here (same rule as k_argmin_stage1)
+        __shared__ double sv[8];
+        __shared__ int64_t si[8];
+        double v = 0.0;
+        int64_t idx = -1;
+        partition_argmin(a.rss, a.po.off[p], a.po.off[p] + threadIdx.x, a.po.off[p + 1], blockDim.x, v, idx);
+        if ((threadIdx.x & 31) == 0) { sv[threadIdx.x >> 5] = v; si[threadIdx.x >> 5] = idx; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < (int)blockDim.x / 32; ++w) argmin_merge(v, idx, sv[w], si[w]);
+            s_best = idx;
+            a.best_seed[p] = idx;
+            a.best_rss[p] = (idx >= 0 && v != -INFINITY) ? v : __longlong_as_double(0x7ff8000000000000LL);
+        }
+    } else if (threadIdx.x == 0) {
         double v = 0.0;
         int64_t idx = -1;
         for (int b = 0; b < COMET_ARGMIN_SPLIT; ++b)

@@ -339,3 +339,46 @@ def test_full_cfg3_cfg4_grid_path(comet, cfg):
         got = {k: o[k].cpu().numpy() for k in ("best_seed", "best_rss", "best_dca", "cls")}
         check_event_against_oracle(ev, seeds_h, shp, part_off, o["rss"].cpu().numpy(), got, 2048 if cfg == 3 else 1024,
                                    rng, cutoff=lam)
+
+
+# ------------------------------------------------------------------------------------------------
+# step C after a plain scan: the winner's track from the scan's checkpoints (select.cuh)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_steps,r_stop,n_seeds", [(None, None, 997), (41, 0.0, 256), (40, 0.0, 100), (43, None, 64),
+                                                    (None, 70.0, 300), (7, None, 33), (3, 0.0, 32)])
+def test_select_after_a_plain_scan_uses_its_checkpoints(cfg0_event, n_steps, r_stop, n_seeds):
+    """comet_select_and_classify right after comet_scan_rss of the same seed buffer (plain kernels: a small set) rebuilds
+    the winners' tracks from the scan's checkpoints -- one thread per checkpoint instead of one chain -- and skips the wire
+    table and, for small partitions, the first argmin stage.  Same winners, RSS, D and classified sets as a context that
+    has not seen the scan (the chain), and as the oracle; tracks that stop early, at a checkpoint row, one row after it,
+    or fill the capacity; a ragged last chunk; a partition that starts inside a chunk."""
+    from paper_1911_09340_b200 import Comet
+    ev = cfg0_event
+    n_steps = ev.n_steps if n_steps is None else n_steps
+    r_stop = ev.r_stop if r_stop is None else r_stop
+    seeds, _ = event_seeds(ev)
+    rng = np.random.default_rng(11)
+    pick = np.sort(rng.choice(seeds.shape[1], n_seeds, replace=False))
+    seeds = np.ascontiguousarray(seeds[:, pick])
+    part_off = [0, n_seeds // 3 + 1, n_seeds]
+    d, hits = _dev(seeds), _hits(ev)
+    phys = (ev.charge, ev.bz, ev.step, n_steps, r_stop)
+    a, b = Comet(0), Comet(0)
+    try:
+        o = a.scan_rss(d, *phys, *hits, ev.cutoff)
+        sa = a.select_and_classify(d, *phys, *hits, ev.cutoff, o["rss"], part_off)
+        sb = b.select_and_classify(d, *phys, *hits, ev.cutoff, o["rss"], part_off)
+        torch.cuda.synchronize()
+        for k in ("best_seed", "best_rss", "best_dca", "cls"):
+            assert np.array_equal(sa[k].cpu().numpy(), sb[k].cpu().numpy(), equal_nan=True), k
+        ref = O.select_classify(seeds, *phys, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff,
+                                o["rss"].cpu().numpy(), part_off)
+        assert np.array_equal(sa["best_seed"].cpu().numpy(), ref["best_seed"])
+        assert np.array_equal(sa["best_dca"].cpu().numpy(), ref["best_dca"], equal_nan=True)
+        assert np.array_equal(sa["cls"].cpu().numpy().astype(bool), np.asarray(ref["cls"]).astype(bool))
+        # the track lengths the checkpoints stand for span the cases named above
+        np_w = o["n_pts"].cpu().numpy()[ref["best_seed"]]
+        assert np.all(np_w >= 1) and np.all(np_w <= n_steps + 1)
+    finally:
+        a.close()
+        b.close()
