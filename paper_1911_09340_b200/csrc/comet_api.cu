@@ -426,6 +426,12 @@ extern "C" int comet_set_field(comet_ctx* ctx, const double* field_dev, const in
     for (int a = 0; a < 3; ++a) { F.n[a] = n_nodes[a]; F.o[a] = origin_cm[a]; F.d[a] = spacing_cm[a]; }
     F.tol = rkn_tol_cm;
     F.tol32 = rkn_tol_cm / 32.0;
+    F.pow2 = 1;
+    for (int a = 0; a < 3; ++a) {
+        int ex = 0;
+        if (frexp(spacing_cm[a], &ex) != 0.5 || ex < -500 || ex > 500) F.pow2 = 0;
+        F.inv[a] = 1.0 / spacing_cm[a];
+    }
     F.bmax = ctx->bmax;
     k_field_bmax<<<1, 1024, 0, (cudaStream_t)cuda_stream>>>(field_dev, nodes, ctx->bmax);
     CU(ctx, cudaGetLastError());

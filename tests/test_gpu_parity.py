@@ -902,6 +902,31 @@ def test_field_classify_and_stage_match_oracle(field_comet, cfg0_event):
     del keep
 
 
+@pytest.mark.parametrize("spacing", [(3.0, 5.0, 2.5), (4.0, 4.0, 6.0), (2.0, 8.0, 0.5)])
+def test_field_map_spacings_division_and_exact_scaling(field_comet, cfg0_event, spacing):
+    """The cell coordinate (x - o) / d of R29 is an IEEE division; when all three spacings are powers of two the
+    kernels scale by 1 / d instead (the same number, bit for bit).  Both branches, and a map in which only some
+    axes have such a spacing (division), against the oracle's division: RSS, n_pts, winner and classification."""
+    from comet_synth import solenoid_map
+    c, ev = field_comet, cfg0_event
+    seeds, po = event_seeds(ev, shape=(5, 4, 4, 4))
+    d = DevEvent(ev, seeds)
+    F, tol = solenoid_map(spacing=spacing), 1e-7
+    keep = _set_map(c, F, tol)
+    fargs = (ev.charge, F, ev.step, ev.n_steps, ev.r_stop, tol, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire,
+             ev.hit_off, ev.rho, ev.cutoff)
+    out = c.scan_event(d.seeds, po, *d.phys(), ev.r_stop, *d.hits(), ev.cutoff)
+    ref = O.scan_field(seeds, *fargs, want_npts=True)
+    assert np.array_equal(out["rss"].cpu().numpy(), ref["rss"])
+    assert np.array_equal(out["n_pts"].cpu().numpy(), ref["n_pts"])
+    best = int(np.argmin(ref["rss"]))
+    assert out["best_seed"].cpu().tolist() == [best]
+    rc = O.classify_seeds_field(seeds, [best], *fargs)
+    np.testing.assert_array_equal(out["cls"].cpu().numpy()[0], rc["cls"][0])
+    np.testing.assert_array_equal(out["best_dca"].cpu().numpy()[0], rc["dca"][0])
+    del keep
+
+
 def test_field_scan_cfg1_ragged_three_partitions(field_comet, cfg1_event):
     from comet_synth import solenoid_map
     c, ev = field_comet, cfg1_event
