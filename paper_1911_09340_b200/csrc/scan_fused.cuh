@@ -225,7 +225,7 @@ __global__ void __launch_bounds__(32 * COMET_FUSED_WARPS, COMET_FUSED_MINB) k_sc
         const int r0 = t * TR;
         PC_MARK();
         // ---- generate rows r0 .. r0 + TR - 1 (Algorithm 1; finished lanes hold their last state) ------
-#pragma unroll 2
+#pragma unroll (FIELD ? 1 : 2)
         for (int rr = 0; rr < TR; ++rr) {
             const int k = r0 + rr;
             if (k > 0 && active) {
