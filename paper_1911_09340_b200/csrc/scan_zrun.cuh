@@ -275,7 +275,8 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
                         const double aa = fma(a1, a1, a2 * a2), bb = fma(b1, b1, b2 * b2);
                         const double ab = fabs(fma(a1, b1, a2 * b2));
                         // min over |u| <= U of |a + u b|^2 = aa - sv (2 ab - sv) / bb with sv = min(ab, U bb)
-                        const double sv = fmin(ab, U * bb);
+                        const double ubb = U * bb;
+                        const double sv = ab < ubb ? ab : ubb;   // (fmin without its NaN rule: a NaN fails the test below either way)
                         if (fma(aa - thr2, bb, -(sv * fma(2.0, ab, -sv))) <= 0.0) m8 |= 1u << j;
                     }
                     if (STATS) st_cnt[ST_SAMPLES_B] += NSUB;
