@@ -55,8 +55,8 @@ DENSE = {"rkn_step": 52, "row": 9, "fine_pair": 600}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1], from the ncu --set full capture of THIS build
 # named beside them (profiles/): the bytes the live run moves are modelled from the library's own sizes below
 NCU_TRAFFIC = {"file": "profiles/r2_full_zrun.txt", "per": "launch = one sub-slab of 3072 chunks; a configs[1] step has four",
-               "k_gen_unique": 27.0e6, "k_scan_zrun": 121.1e6, "k_fine_ck": 62.9e6, "k_rss_sum": 17.7e6,
-               "per_step": 4 * (27.0e6 + 121.1e6 + 62.9e6 + 17.7e6)}
+               "k_gen_unique": 26.5e6, "k_scan_zrun": 121.5e6, "k_fine_ck": 63.1e6, "k_rss_sum": 17.7e6,
+               "per_step": 4 * (26.5e6 + 121.5e6 + 63.1e6 + 17.7e6)}
 STAGE_HALF_WIDTH = [0.6, 0.5, 0.5, 1.0]
 STAGE_GRID = [5, 5, 5, 5]
 FIELD_TOL = 1e-7
@@ -381,12 +381,31 @@ class Leg:
         w0 = time.perf_counter()
         for _ in range(steps):
             hout = c.scan_event_grid_host(h["axes"], self.shape, *self.phys, ev.r_stop, h["fw"], h["ho"], h["rho"], ev.cutoff, out=hout)
-        dt = (time.perf_counter() - w0) / steps
+        dt_sync = (time.perf_counter() - w0) / steps
         assert hout["best_seed"].numpy().tolist() == self.out["best_seed"].cpu().numpy().tolist()
         assert bool((hout["cls"] == self.out["cls"].cpu()).all())
+        # a stream of events: comet_scan_event_grid_submit / _collect, the next event submitted before the last one is
+        # collected (two slots), every event's inputs copied in and results copied out inside the timed region
+        sub = lambda k: c.scan_event_grid_submit(k % 2, h["axes"], self.shape, *self.phys, ev.r_stop, h["fw"], h["ho"], h["rho"], ev.cutoff)
+        outs = [{k: torch.empty_like(v) for k, v in hout.items()} for _ in range(2)]
+        for k in (0, 1):                                    # (both slots have their buffers)
+            sz = sub(k)
+            c.scan_event_grid_collect(k, sz, out=outs[k])
+        torch.cuda.synchronize()
+        w0 = time.perf_counter()
+        sub(0)
+        for k in range(1, steps):
+            sub(k)
+            c.scan_event_grid_collect((k - 1) % 2, sz, out=outs[(k - 1) % 2])
+        c.scan_event_grid_collect((steps - 1) % 2, sz, out=outs[(steps - 1) % 2])
+        dt = (time.perf_counter() - w0) / steps
+        for o in outs[:min(2, steps)]:
+            assert o["best_seed"].numpy().tolist() == self.out["best_seed"].cpu().numpy().tolist()
+            assert bool((o["cls"] == self.out["cls"].cpu()).all())
         return {"ms_per_step": dt * 1e3, "value": self.pairs / dt,
                 "h2d_bytes_per_step": sum(int(v.numel() * v.element_size()) for v in h.values()),
-                "d2h_bytes_per_step": sum(int(v.numel() * v.element_size()) for v in hout.values())}
+                "d2h_bytes_per_step": sum(int(v.numel() * v.element_size()) for v in hout.values()),
+                "one_event_at_a_time_ms": dt_sync * 1e3}
 
 
 def run_ours(args):
@@ -486,9 +505,43 @@ def run_ours(args):
             del track
             torch.cuda.empty_cache()
 
+    # ---- the same event twice in flight: two contexts on two streams (what a consumer of many events does; the head of a
+    # call -- k_gen_unique alone on the device -- and the kernels' tails then overlap the other event's work) -----------
+    in_flight = None
+    if args.compare:
+        c2 = Comet(local)
+        c2.set_option(OPT_ZGROUP, 1 if args.zgroup else 0)
+        leg2 = Leg(c2, args.config, torch, zgroup=args.zgroup, ev=ev)
+        q2 = [torch.cuda.Stream(), torch.cuda.Stream()]
+
+        def pair():
+            res = []
+            for lg_, q in zip((leg, leg2), q2):
+                q.wait_stream(stream)
+                with torch.cuda.stream(q):
+                    lg_.scan_on(q)
+                    res.append(lg_.c.select_and_classify(lg_.seeds, *lg_.phys, ev.r_stop, *lg_.hits, ev.cutoff, lg_.rss, lg_.part_off,
+                                                         stream=q))
+            for q in q2:
+                stream.wait_stream(q)
+            return res
+        pair()
+        torch.cuda.synchronize()
+        ms_pair, res2 = _time_steps(pair, min(args.steps, 30), stream)
+        ok2 = all(o["best_seed"].cpu().numpy().tolist() == best and bool(torch.equal(o["cls"], leg.out["cls"])) for o in res2)
+        ok2 = ok2 and bool(torch.equal(leg2.rss, leg.rss))
+        assert ok2, "two events in flight differ from the single event"
+        in_flight = {"contexts": 2, "ms_per_event": ms_pair / 2, "events_per_s": 2.0 / (ms_pair * 1e-3),
+                     "dca_evals_per_s": 2.0 * leg.pairs / (ms_pair * 1e-3), "identical_to_single_event": ok2,
+                     "what": "the headline event scanned by two contexts on two streams at the same time; `value` and "
+                             "`ms_per_step` stay the single event's"}
+        c2.close()
+        del leg2, res2
+        torch.cuda.empty_cache()
+
     # ---- every other config, device-resident + end to end ------------------------------------------------------
     configs = {str(args.config): dict(head, e2e_ms=e2e["ms_per_step"], workload=_workload_name(args.config, ev, leg.S, leg.P),
-                                      best_seed=best)}
+                                      best_seed=best, two_events_in_flight=in_flight)}
     for cfg in [int(v) for v in args.configs.split(",") if v != ""]:
         if cfg == args.config or cfg == 2:
             continue
@@ -721,8 +774,11 @@ def run_ours(args):
         "result": {"best_seed": best, "classified_entries": n_cls, "recorded_states_per_seed": head["recorded_states_per_seed"]},
         "e2e": {"value": world * e2e["value"], "unit": UNIT, "h2d_bytes_per_step": e2e["h2d_bytes_per_step"],
                 "d2h_bytes_per_step": e2e["d2h_bytes_per_step"], "ms_per_step": e2e["ms_per_step"],
-                "api": "comet_scan_event_grid_host: the seed sets as grid axes, hits and results in pinned host buffers; "
-                       "the detector geometry resident on the device (comet_set_geometry)"},
+                "one_event_at_a_time_ms": e2e["one_event_at_a_time_ms"],
+                "api": "comet_scan_event_grid_submit / _collect (two events in flight: the next one is submitted before the last "
+                       "one is collected): the seed sets as grid axes, hits and results in host buffers, every event's inputs "
+                       "copied in and results copied out inside the timed region, wall clock; the detector geometry resident on "
+                       "the device (comet_set_geometry).  one_event_at_a_time_ms: the synchronous comet_scan_event_grid_host"},
         "gpu_launches": launches_per_step * args.steps,
         "clocks": clocks,
         "configs": configs,

@@ -584,6 +584,25 @@ int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_host, int32_t 
                                int64_t* best_seed_host, double* best_rss_host, double* best_dca_host,
                                uint8_t* cls_host, double* rss_host, void* cuda_stream);
 
+/* The same call in two halves, for a stream of events: comet_scan_event_grid_submit copies the inputs into the
+ * staging buffer of `slot` (0 <= slot < COMET_EVENT_SLOTS) and enqueues the upload, the seed grid, steps A-C and the
+ * download of the results on `cuda_stream`; it returns without waiting.  comet_scan_event_grid_collect waits for
+ * that event's results and copies them to the caller's arrays.  With two slots the host side of event k + 1
+ * (packing, upload, launches) overlaps the kernels of event k; the events of one ctx run one after the other on
+ * the device (they share the scan workspace), so all submits of a ctx go to the same stream.
+ * A slot holds one event at a time: COMET_EINVAL for a submit into a slot that has not been collected, or a
+ * collect from an empty one.  The caller's input arrays may be reused as soon as submit returns. */
+#define COMET_EVENT_SLOTS 2
+int comet_scan_event_grid_submit(comet_ctx* ctx, int32_t slot, const double* axes_host, int32_t n_part, int32_t n_p,
+                                 int32_t n_ct, int32_t n_phi, int32_t n_z,
+                                 int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                                 double r_stop_cm,
+                                 const int32_t* fired_wire_host, const int32_t* hit_off_host,
+                                 const double* rho_host, int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                 void* cuda_stream);
+int comet_scan_event_grid_collect(comet_ctx* ctx, int32_t slot, int64_t* best_seed_host, double* best_rss_host,
+                                  double* best_dca_host, uint8_t* cls_host);
+
 /* ---- measurement helper ------------------------------------------------------------------ */
 
 /* Enqueues a dependent-free DFMA loop on every SM (`iters` FMAs per thread on 8 chains) and

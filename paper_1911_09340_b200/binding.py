@@ -25,6 +25,7 @@ EXPORTED_SYMBOLS = [
     "comet_turns_half_work_bytes", "comet_scan_turns_half",
     "comet_reserve_scan", "comet_seed_grid", "comet_grid_axes_len", "comet_grid_z_run", "comet_seed_runs",
     "comet_set_geometry", "comet_get_geometry", "comet_scan_event_grid_host",
+    "comet_scan_event_grid_submit", "comet_scan_event_grid_collect",
 ]
 
 COMET_CHUNK = 32
@@ -133,6 +134,9 @@ def load_library():
     L.comet_get_geometry.argtypes = [vp, ctypes.POINTER(vp), ctypes.POINTER(vp), ctypes.POINTER(i32)]
     L.comet_scan_event_grid_host.argtypes = [vp, vp, i32, i32, i32, i32, i32, i32, dbl, dbl, i32, dbl,
                                              vp, vp, vp, i32, i32, dbl, vp, vp, vp, vp, vp, vp]
+    L.comet_scan_event_grid_submit.argtypes = [vp, i32, vp, i32, i32, i32, i32, i32, i32, dbl, dbl, i32, dbl,
+                                               vp, vp, vp, i32, i32, dbl, vp]
+    L.comet_scan_event_grid_collect.argtypes = [vp, i32, vp, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes", "comet_turns_work_bytes",
                         "comet_hough_work_bytes", "comet_half_work_bytes", "comet_grid_axes_len", "comet_grid_z_run",
@@ -751,6 +755,34 @@ class Comet:
             float(r_stop), fired_wire.data_ptr(), hit_off.data_ptr(), rho.data_ptr(), W, H, float(cutoff),
             out["best_seed"].data_ptr(), out["best_rss"].data_ptr(), out["best_dca"].data_ptr(),
             out["cls"].data_ptr(), rss_ptr, _stream_ptr(stream)))
+        return out
+
+    def scan_event_grid_submit(self, slot, axes, shape, charge, bz, step, n_steps, r_stop, fired_wire, hit_off, rho, cutoff,
+                               stream=None):
+        """comet_scan_event_grid_submit: enqueue one event (HOST arrays, copied before the call returns) into `slot`."""
+        def host(a, dt):
+            t = a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a))
+            if t.is_cuda or t.dtype != dt or not t.is_contiguous():
+                raise CometError("host array must be a contiguous CPU tensor of dtype %s" % dt)
+            return t
+        axes = host(axes, torch.float64)
+        fired_wire, hit_off, rho = host(fired_wire, torch.int32), host(hit_off, torch.int32), host(rho, torch.float64)
+        n_p, n_ct, n_phi, n_z = (int(v) for v in shape)
+        P, W, H = int(axes.shape[0]), int(fired_wire.shape[0]), int(rho.shape[0])
+        self._check(self._L.comet_scan_event_grid_submit(
+            self._h, int(slot), axes.data_ptr(), P, n_p, n_ct, n_phi, n_z, int(charge), float(bz), float(step), int(n_steps),
+            float(r_stop), fired_wire.data_ptr(), hit_off.data_ptr(), rho.data_ptr(), W, H, float(cutoff), _stream_ptr(stream)))
+        return (P, W, H)
+
+    def scan_event_grid_collect(self, slot, sizes, out=None):
+        """comet_scan_event_grid_collect: wait for the event in `slot`; `sizes` is what the submit returned."""
+        P, W, H = sizes
+        if out is None:
+            out = {"best_seed": torch.empty(P, dtype=torch.int64), "best_rss": torch.empty(P, dtype=torch.float64),
+                   "best_dca": torch.empty((P, W), dtype=torch.float64), "cls": torch.empty((P, H), dtype=torch.uint8)}
+        self._check(self._L.comet_scan_event_grid_collect(
+            self._h, int(slot), out["best_seed"].data_ptr(), out["best_rss"].data_ptr(), out["best_dca"].data_ptr(),
+            out["cls"].data_ptr()))
         return out
 
     # -- measurement helper -------------------------------------------------------------------

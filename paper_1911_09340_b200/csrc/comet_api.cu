@@ -114,8 +114,18 @@ struct comet_ctx {
         int32_t n_wires, n_fired, uniform;
         double cutoff, step;
     } wt_of;
-    void* hstage;          // pinned host staging of comet_scan_event_grid_host: one copy in, one copy out per event
-    size_t hstage_bytes;
+    // events in flight through comet_scan_event_grid_submit / _collect: per slot one device slab (inputs, seeds, rss,
+    // results), one pinned host staging buffer of the same input / result layout (one copy in, one copy out per event)
+    // and the event that marks the results' arrival
+    struct EventSlot {
+        void* dbuf; size_t dbuf_bytes;
+        void* hstage; size_t hstage_bytes;
+        cudaEvent_t done;
+        int pending;
+        size_t in_bytes, o_out, out_bytes, o_bs, o_br, o_bd, o_cls, o_rss;
+        int32_t n_part, n_fired, n_hits;
+        int64_t n_seeds;
+    } slot[COMET_EVENT_SLOTS];
     // detector geometry kept on the device for the host-buffer entry points (comet_set_geometry)
     double* geom_a;
     double* geom_b;
@@ -245,7 +255,11 @@ extern "C" int comet_destroy(comet_ctx* ctx)
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ref_fb); cudaFree(ctx->ub); cudaFree(ctx->npu);
     for (int j = 0; j < COMET_TEV_RING * 5; ++j) if (ctx->tev[j / 5][j % 5]) cudaEventDestroy(ctx->tev[j / 5][j % 5]);
     cudaFree(ctx->geom_a); cudaFree(ctx->geom_b);
-    if (ctx->hstage) cudaFreeHost(ctx->hstage);
+    for (int q = 0; q < COMET_EVENT_SLOTS; ++q) {
+        if (ctx->slot[q].hstage) cudaFreeHost(ctx->slot[q].hstage);
+        cudaFree(ctx->slot[q].dbuf);
+        if (ctx->slot[q].done) cudaEventDestroy(ctx->slot[q].done);
+    }
     cudaFree(ctx->hbuf); cudaFree(ctx->tbuf); cudaFree(ctx->ck); cudaFree(ctx->npw); cudaFree(ctx->cw); cudaFree(ctx->tw); cudaFree(ctx->tmk); cudaFree(ctx->bmax);
     for (int l = 0; l < COMET_MAX_LANES; ++l) {
         if (ctx->ls[l]) cudaStreamDestroy(ctx->ls[l]);
@@ -2016,21 +2030,21 @@ extern "C" int comet_scan_event_host(comet_ctx* ctx, const double* seeds_host, i
 }
 
 // The event of comet_scan_event_host with the seed sets given as grid axes: a few KB cross the bus per event.
-extern "C" int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_host, int32_t n_part, int32_t n_p,
-                                          int32_t n_ct, int32_t n_phi, int32_t n_z,
-                                          int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
-                                          double r_stop_cm,
-                                          const int32_t* fired_wire_host, const int32_t* hit_off_host,
-                                          const double* rho_host, int32_t n_fired, int32_t n_hits, double cutoff_cm,
-                                          int64_t* best_seed_host, double* best_rss_host, double* best_dca_host,
-                                          uint8_t* cls_host, double* rss_host, void* cuda_stream)
+extern "C" int comet_scan_event_grid_submit(comet_ctx* ctx, int32_t slot, const double* axes_host, int32_t n_part, int32_t n_p,
+                                            int32_t n_ct, int32_t n_phi, int32_t n_z,
+                                            int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                                            double r_stop_cm,
+                                            const int32_t* fired_wire_host, const int32_t* hit_off_host,
+                                            const double* rho_host, int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                            void* cuda_stream)
 {
     GridShape g;
-    if (!ctx || make_shape(&g, n_part, n_p, n_ct, n_phi, n_z) || !axes_host || ctx->geom_n <= 0 ||
-        bad_physics(charge, bz_tesla, step_cm, n_steps) || !(r_stop_cm >= 0.0) ||
-        bad_hits(ctx->geom_a, ctx->geom_b, ctx->geom_n, fired_wire_host, hit_off_host, rho_host, n_fired, n_hits, cutoff_cm) ||
-        !best_seed_host || !best_rss_host || (n_fired > 0 && !best_dca_host) || (n_hits > 0 && !cls_host))
+    if (!ctx || slot < 0 || slot >= COMET_EVENT_SLOTS || make_shape(&g, n_part, n_p, n_ct, n_phi, n_z) || !axes_host ||
+        ctx->geom_n <= 0 || bad_physics(charge, bz_tesla, step_cm, n_steps) || !(r_stop_cm >= 0.0) ||
+        bad_hits(ctx->geom_a, ctx->geom_b, ctx->geom_n, fired_wire_host, hit_off_host, rho_host, n_fired, n_hits, cutoff_cm))
         return COMET_EINVAL;
+    comet_ctx::EventSlot& q = ctx->slot[slot];
+    if (q.pending) return COMET_EINVAL;                      // (collect the event that is in the slot first)
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -2053,20 +2067,21 @@ extern "C" int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_hos
     const size_t o_bd = take(sizeof(double) * (size_t)n_part * (size_t)n_fired);
     const size_t o_cls = take((size_t)n_part * (size_t)n_hits);
     const size_t out_bytes = off - o_out;
-    if (off > ctx->hbuf_bytes) {
+    if (!q.done) CU(ctx, cudaEventCreateWithFlags(&q.done, cudaEventDisableTiming));
+    if (off > q.dbuf_bytes) {
         CU(ctx, cudaDeviceSynchronize());
-        rc = grow(ctx, &ctx->hbuf, &ctx->hbuf_bytes, off);
+        rc = grow(ctx, &q.dbuf, &q.dbuf_bytes, off);
         if (rc) return rc;
     }
-    if (in_bytes + out_bytes > ctx->hstage_bytes) {
+    if (in_bytes + out_bytes > q.hstage_bytes) {
         CU(ctx, cudaDeviceSynchronize());
-        if (ctx->hstage) { cudaFreeHost(ctx->hstage); ctx->hstage = nullptr; ctx->hstage_bytes = 0; }
-        cudaError_t e = cudaHostAlloc(&ctx->hstage, in_bytes + out_bytes, cudaHostAllocDefault);
-        if (e != cudaSuccess) { ctx->last_cuda = (int)e; ctx->hstage = nullptr; cudaGetLastError(); return COMET_ENOMEM; }
-        ctx->hstage_bytes = in_bytes + out_bytes;
+        if (q.hstage) { cudaFreeHost(q.hstage); q.hstage = nullptr; q.hstage_bytes = 0; }
+        cudaError_t e = cudaHostAlloc(&q.hstage, in_bytes + out_bytes, cudaHostAllocDefault);
+        if (e != cudaSuccess) { ctx->last_cuda = (int)e; q.hstage = nullptr; cudaGetLastError(); return COMET_ENOMEM; }
+        q.hstage_bytes = in_bytes + out_bytes;
     }
-    char* B = (char*)ctx->hbuf;
-    char* Hs = (char*)ctx->hstage;
+    char* B = (char*)q.dbuf;
+    char* Hs = (char*)q.hstage;
     double* d_axes = (double*)(B + o_axes);
     double* d_seeds = (double*)(B + o_seeds);
     int32_t* d_fw = (int32_t*)(B + o_fw);
@@ -2097,14 +2112,55 @@ extern "C" int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_hos
                                    ctx->geom_a, ctx->geom_b, ctx->geom_n, d_fw, d_ho, d_rho, n_fired, n_hits, cutoff_cm,
                                    d_rss, po, n_part, d_bs, d_br, d_bd, d_cls, st);
     if (rc) return rc;
-    char* Ho = Hs + in_bytes;
-    CU(ctx, cudaMemcpyAsync(Ho, B + o_out, out_bytes, cudaMemcpyDeviceToHost, st));
-    if (rss_host) CU(ctx, cudaMemcpyAsync(rss_host, d_rss, sizeof(double) * (size_t)n_seeds, cudaMemcpyDeviceToHost, st));
-    CU(ctx, cudaStreamSynchronize(st));
-    memcpy(best_seed_host, Ho + (o_bs - o_out), sizeof(int64_t) * (size_t)n_part);
-    memcpy(best_rss_host, Ho + (o_br - o_out), sizeof(double) * (size_t)n_part);
-    if (n_fired) memcpy(best_dca_host, Ho + (o_bd - o_out), sizeof(double) * (size_t)n_part * n_fired);
-    if (n_hits) memcpy(cls_host, Ho + (o_cls - o_out), (size_t)n_part * n_hits);
+    CU(ctx, cudaMemcpyAsync(Hs + in_bytes, B + o_out, out_bytes, cudaMemcpyDeviceToHost, st));
+    CU(ctx, cudaEventRecord(q.done, st));
+    q.in_bytes = in_bytes; q.o_out = o_out; q.out_bytes = out_bytes; q.o_bs = o_bs; q.o_br = o_br; q.o_bd = o_bd; q.o_cls = o_cls;
+    q.o_rss = o_rss; q.n_part = n_part; q.n_fired = n_fired; q.n_hits = n_hits; q.n_seeds = n_seeds;
+    q.pending = 1;
+    return COMET_OK;
+}
+
+extern "C" int comet_scan_event_grid_collect(comet_ctx* ctx, int32_t slot, int64_t* best_seed_host, double* best_rss_host,
+                                             double* best_dca_host, uint8_t* cls_host)
+{
+    if (!ctx || slot < 0 || slot >= COMET_EVENT_SLOTS) return COMET_EINVAL;
+    comet_ctx::EventSlot& q = ctx->slot[slot];
+    if (!q.pending || !best_seed_host || !best_rss_host || (q.n_fired > 0 && !best_dca_host) || (q.n_hits > 0 && !cls_host))
+        return COMET_EINVAL;
+    int rc = set_device(ctx);
+    if (rc) return rc;
+    CU(ctx, cudaEventSynchronize(q.done));
+    q.pending = 0;
+    const char* Ho = (const char*)q.hstage + q.in_bytes;
+    memcpy(best_seed_host, Ho + (q.o_bs - q.o_out), sizeof(int64_t) * (size_t)q.n_part);
+    memcpy(best_rss_host, Ho + (q.o_br - q.o_out), sizeof(double) * (size_t)q.n_part);
+    if (q.n_fired) memcpy(best_dca_host, Ho + (q.o_bd - q.o_out), sizeof(double) * (size_t)q.n_part * q.n_fired);
+    if (q.n_hits) memcpy(cls_host, Ho + (q.o_cls - q.o_out), (size_t)q.n_part * q.n_hits);
+    return COMET_OK;
+}
+
+extern "C" int comet_scan_event_grid_host(comet_ctx* ctx, const double* axes_host, int32_t n_part, int32_t n_p,
+                                          int32_t n_ct, int32_t n_phi, int32_t n_z,
+                                          int32_t charge, double bz_tesla, double step_cm, int32_t n_steps,
+                                          double r_stop_cm,
+                                          const int32_t* fired_wire_host, const int32_t* hit_off_host,
+                                          const double* rho_host, int32_t n_fired, int32_t n_hits, double cutoff_cm,
+                                          int64_t* best_seed_host, double* best_rss_host, double* best_dca_host,
+                                          uint8_t* cls_host, double* rss_host, void* cuda_stream)
+{
+    if (!ctx || !best_seed_host || !best_rss_host || (n_fired > 0 && !best_dca_host) || (n_hits > 0 && !cls_host))
+        return COMET_EINVAL;
+    if (ctx->slot[0].pending) return COMET_EINVAL;           // (an event submitted to slot 0 is still to be collected)
+    int rc = comet_scan_event_grid_submit(ctx, 0, axes_host, n_part, n_p, n_ct, n_phi, n_z, charge, bz_tesla, step_cm, n_steps,
+                                          r_stop_cm, fired_wire_host, hit_off_host, rho_host, n_fired, n_hits, cutoff_cm, cuda_stream);
+    if (rc) return rc;
+    const comet_ctx::EventSlot& q = ctx->slot[0];
+    if (rss_host)
+        CU(ctx, cudaMemcpyAsync(rss_host, (const char*)q.dbuf + q.o_rss, sizeof(double) * (size_t)q.n_seeds, cudaMemcpyDeviceToHost,
+                                (cudaStream_t)cuda_stream));
+    rc = comet_scan_event_grid_collect(ctx, 0, best_seed_host, best_rss_host, best_dca_host, cls_host);
+    if (rc) return rc;
+    if (rss_host) CU(ctx, cudaStreamSynchronize((cudaStream_t)cuda_stream));
     return COMET_OK;
 }
 

@@ -280,6 +280,45 @@ def test_grid_host_event_matches_oracle(comet, cfg0_event):
     np.testing.assert_array_equal(out2["cls"].numpy(), rs["cls"])
 
 
+def test_events_in_flight_through_submit_and_collect(comet):
+    """comet_scan_event_grid_submit / _collect: six different events (configs[2]: one to four partitions, different hit
+    lists) through the two slots, the next one submitted before the last one is collected; every result equals the
+    synchronous call's and the oracle's; a slot refuses a second event and an empty slot refuses a collect."""
+    from paper_1911_09340_b200 import CometError
+    evs = make_config(2, n_events=6)
+    shape = (3, 4, 4, 16)
+    comet.set_geometry(evs[0].geom.wire_a, evs[0].geom.wire_b)
+    args = []
+    for ev in evs:
+        axes, shp, part_off = event_axes(ev, shape=shape)
+        args.append((ev, axes, shp, part_off))
+    sync = [comet.scan_event_grid_host(torch.from_numpy(a), shp, ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop,
+                                       ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff) for ev, a, shp, _ in args]
+    sync = [{k: v.clone() for k, v in o.items()} for o in sync]
+    sub = lambda k: comet.scan_event_grid_submit(k % 2, torch.from_numpy(args[k][1]), args[k][2], args[k][0].charge, args[k][0].bz,
+                                                 args[k][0].step, args[k][0].n_steps, args[k][0].r_stop, args[k][0].fired_wire,
+                                                 args[k][0].hit_off, args[k][0].rho, args[k][0].cutoff)
+    with pytest.raises(CometError):
+        comet.scan_event_grid_collect(0, (1, 1, 1))
+    sizes, got = {}, {}
+    sizes[0] = sub(0)
+    with pytest.raises(CometError):
+        sub(0)                                              # the slot is taken (nothing is enqueued)
+    for k in range(1, len(args)):
+        sizes[k] = sub(k)
+        got[k - 1] = comet.scan_event_grid_collect((k - 1) % 2, sizes[k - 1])
+    got[len(args) - 1] = comet.scan_event_grid_collect((len(args) - 1) % 2, sizes[len(args) - 1])
+    for k, (ev, axes, shp, part_off) in enumerate(args):
+        for key in ("best_seed", "best_rss", "best_dca", "cls"):
+            assert np.array_equal(got[k][key].numpy(), sync[k][key].numpy(), equal_nan=True), (k, key)
+        seeds, _ = event_seeds(ev, shape=shape)
+        ref = _oracle_scan(ev, seeds)
+        rs = _oracle_select(ev, seeds, ref["rss"], part_off)
+        np.testing.assert_array_equal(got[k]["best_seed"].numpy(), rs["best_seed"])
+        np.testing.assert_array_equal(got[k]["cls"].numpy(), rs["cls"])
+        np.testing.assert_array_equal(got[k]["best_dca"].numpy(), rs["best_dca"])
+
+
 def test_full_cfg2_batch_on_streams_as_benchmarked():
     """BASELINE.json configs[2] at full size, the way bench.py's batch leg runs it: the events' full grids (131072
     seeds per partition, 1-4 turns, |p| from 60 to 105 MeV/c) built on the device from their axes, scanned with the
