@@ -120,13 +120,29 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
         for (int i = threadIdx.x; i < W; i += blockDim.x) dca[i] = __longlong_as_double(0x7ff8000000000000LL);
         return;
     }
-    if (!FIELD && a.ub) {
+    // The scan's tracks are taken only if they ARE this seed's: state 0 of the track / checkpoint 0 must equal the seed's own
+    // initial state bit for bit (the host has compared the physics; a track is a function of its initial state and those).  A
+    // buffer that was rewritten, or reused by the allocator for another seed set, falls through to the chain below.
+    bool rows_ok = false, ck_ok = false;
+    if (!FIELD && (a.ub || a.ck)) {
+        State s0;
+        (void)seed_init(a.seeds, a.stride, idx, a.qkb, s0);
+        if (a.ub) {
+            const double2* g0 = reinterpret_cast<const double2*>(a.ub + (size_t)(idx >> a.zshift) * (size_t)a.u_rows * 4);
+            const double2 xy = __ldg(g0), tt = __ldg(g0 + 1);
+            rows_ok = xy.x == s0.x0 && xy.y == s0.x1 && tt.x == s0.t0 && tt.y == s0.t1;
+        } else {
+            const double* o = a.ck + (size_t)(idx >> 5) * (size_t)a.n_ck * (6 * COMET_LANES) + (idx & 31);
+            ck_ok = o[0] == s0.x0 && o[32] == s0.x1 && o[64] == s0.x2 && o[96] == s0.t0 && o[128] == s0.t1 && o[160] == s0.t2;
+        }
+    }
+    if (rows_ok) {
         // the same numbers without the chain of 400-odd dependent RKN4 steps: (x, y, T_x, T_y) of every recorded state are
         // the rows of the seed's distinct transverse track, z is one addition per step (x_2' = x_2 + h T_2)
         State st;
         const double c = seed_init(a.seeds, a.stride, idx, a.qkb, st);
         const int64_t u = idx >> a.zshift;
-        const int32_t np = __ldg(a.np_u + u);
+        const int32_t np = min(max(__ldg(a.np_u + u), 1), a.n_steps + 1);
         const double2* g = reinterpret_cast<const double2*>(a.ub + (size_t)u * (size_t)a.u_rows * 4);
         for (int k = threadIdx.x; k < np; k += blockDim.x) {
             const double2 xy = __ldg(g + 2 * k), tt = __ldg(g + 2 * k + 1);
@@ -141,7 +157,7 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
             sm[2] = z;
             for (int k = 1; k < np; ++k) { z = xadd(z, hz); sm[(size_t)k * RS + 2] = z; }
         }
-    } else if (!FIELD && a.ck) {
+    } else if (ck_ok) {
         // the same numbers without the chain: thread m starts from checkpoint m (recorded state m CK, bit for bit) and steps
         // the CK - 1 states after it.  The first state in the target region ends the track (R3); the checkpoints behind it
         // were never written and whatever those threads compute is not read (pure arithmetic: nothing is addressed by it).

@@ -280,6 +280,39 @@ def test_grid_host_event_matches_oracle(comet, cfg0_event):
     np.testing.assert_array_equal(out2["cls"].numpy(), rs["cls"])
 
 
+@pytest.mark.parametrize("z_run,shape", [(16, (8, 8, 32, 16)), (1, (4, 4, 4, 4))])
+def test_select_does_not_reuse_tracks_of_rewritten_seeds(cfg1_event, z_run, shape):
+    """The seed buffer of the last scan is rewritten in place (as an allocator that hands the same address out again would
+    do): comet_select_and_classify must not classify with the tracks that scan left in the context.  State 0 of the
+    reused track is compared with the seed itself on the device; the winner's track is stepped again."""
+    from paper_1911_09340_b200 import Comet
+    ev = cfg1_event
+    seeds_a, part_off = event_seeds(ev, shape=shape)
+    # other seeds of the same shape: the grid mirrored in its momentum axis and shifted in z
+    seeds_b = np.ascontiguousarray(seeds_a[:, ::-1]).copy()
+    seeds_b[2] += 0.37
+    d, hits = _dev(seeds_a), _hits(ev)
+    phys = (ev.charge, ev.bz, ev.step, ev.n_steps, ev.r_stop)
+    a, b = Comet(0), Comet(0)
+    try:
+        a.scan_rss(d, *phys, *hits, ev.cutoff, z_run=z_run)
+        torch.cuda.synchronize()
+        d.copy_(_dev(seeds_b))                              # same buffer, other seeds
+        rss_b = b.scan_rss(d, *phys, *hits, ev.cutoff, z_run=1)["rss"]
+        got = a.select_and_classify(d, *phys, *hits, ev.cutoff, rss_b, part_off)
+        ref = b.select_and_classify(d, *phys, *hits, ev.cutoff, rss_b, part_off)
+        torch.cuda.synchronize()
+        for k in ("best_seed", "best_rss", "best_dca", "cls"):
+            assert np.array_equal(got[k].cpu().numpy(), ref[k].cpu().numpy(), equal_nan=True), k
+        win = got["best_seed"].cpu().numpy()
+        rs = O.classify_seeds(seeds_b, win, *phys, ev.geom.wire_a, ev.geom.wire_b, ev.fired_wire, ev.hit_off, ev.rho, ev.cutoff)
+        np.testing.assert_array_equal(got["best_dca"].cpu().numpy(), rs["dca"])
+        np.testing.assert_array_equal(got["cls"].cpu().numpy(), rs["cls"])
+    finally:
+        a.close()
+        b.close()
+
+
 def test_events_in_flight_through_submit_and_collect(comet):
     """comet_scan_event_grid_submit / _collect: six different events (configs[2]: one to four partitions, different hit
     lists) through the two slots, the next one submitted before the last one is collected; every result equals the
