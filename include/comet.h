@@ -244,11 +244,10 @@ int comet_scan_rss(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int
  * uniform field, one slab), the winner's track is not stepped again as one chain of n_steps dependent steps: with
  * z_run promised its (x, y, T_x, T_y) rows are copied from that scan's distinct-track workspace; after the plain
  * kernels (small sets, z_run = 1) every 4th recorded state is that scan's checkpoint and the three states after
- * it are stepped by one thread per checkpoint -- the same numbers either way.  If the hit-list arguments are
- * also that call's (same arrays and sizes, cutoff, step) its wire table is used as it stands.  A reused track
- * is checked on the device: its state 0 must equal the seed's own initial state bit for bit, else the track is
- * stepped again (a seed buffer rewritten in place, or handed out again by an allocator, is harmless).  The
- * hit-list arrays must not have been rewritten in place between the two calls.
+ * it are stepped by one thread per checkpoint -- the same numbers either way.  A reused track is checked on the
+ * device: its state 0 must equal the seed's own initial state bit for bit, else the track is stepped again (a
+ * seed buffer rewritten in place, or handed out again by an allocator, is harmless).  The wire lines (O4) are
+ * formed from wire_a / wire_b by the classifying kernel itself: nothing of an earlier call's hit list is used.
  * Partitions of at most 16384 seeds are searched by the classifying CTA itself (one launch).
  * Limits: n_part <= COMET_MAX_PARTITIONS, n_steps <= COMET_MAX_STEPS. */
 int comet_select_and_classify(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int64_t n_seeds,

@@ -106,14 +106,6 @@ struct comet_ctx {
         double qkb, step, r_stop;
         int32_t n_steps, zshift, u_rows, n_ck, valid;
     } last;
-    // the hit list the wire table `wt` was last built from (launch_wire_prep): comet_select_and_classify does not build it
-    // again after the comet_scan_rss call it follows
-    struct {
-        const double *wire_a, *wire_b, *rho;
-        const int32_t *fired_wire, *hit_off;
-        int32_t n_wires, n_fired, uniform;
-        double cutoff, step;
-    } wt_of;
     // events in flight through comet_scan_event_grid_submit / _collect: per slot one device slab (inputs, seeds, rss,
     // results), one pinned host staging buffer of the same input / result layout (one copy in, one copy out per event)
     // and the event that marks the results' arrival
@@ -512,21 +504,7 @@ static int launch_wire_prep(comet_ctx* ctx, const double* wire_a, const double* 
     k_wire_prep<<<(n_fired + 127) / 128, 128, 0, st>>>(wire_a, wire_b, n_wires, fired_wire, n_fired, hit_off, rho,
                                                        cutoff_cm, step_cm, uniform, ctx->wt);
     CU(ctx, cudaGetLastError());
-    ctx->wt_of.wire_a = wire_a; ctx->wt_of.wire_b = wire_b; ctx->wt_of.rho = rho; ctx->wt_of.fired_wire = fired_wire;
-    ctx->wt_of.hit_off = hit_off; ctx->wt_of.n_wires = n_wires; ctx->wt_of.n_fired = n_fired; ctx->wt_of.uniform = uniform;
-    ctx->wt_of.cutoff = cutoff_cm; ctx->wt_of.step = step_cm;
     return COMET_OK;
-}
-
-// the table in `wt` is the one launch_wire_prep would build from these arguments (same arrays, same sizes)
-static bool wire_table_is(const comet_ctx* ctx, const double* wire_a, const double* wire_b, int32_t n_wires,
-                          const int32_t* fired_wire, const int32_t* hit_off, const double* rho, int32_t n_fired,
-                          double cutoff_cm, double step_cm)
-{
-    return ctx->wt_of.wire_a == wire_a && ctx->wt_of.wire_b == wire_b && ctx->wt_of.rho == rho &&
-           ctx->wt_of.fired_wire == fired_wire && ctx->wt_of.hit_off == hit_off && ctx->wt_of.n_wires == n_wires &&
-           ctx->wt_of.n_fired == n_fired && ctx->wt_of.uniform == (ctx->field.B == nullptr ? 1 : 0) &&
-           ctx->wt_of.cutoff == cutoff_cm && ctx->wt_of.step == step_cm;
 }
 
 static bool bad_hits(const double* wire_a, const double* wire_b, int32_t n_wires, const int32_t* fired_wire,
@@ -1018,10 +996,6 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     const bool same_scan = !field && ctx->last.valid && ctx->last.seeds == seeds && ctx->last.stride == seed_stride &&
                            ctx->last.n_seeds == n_seeds && ctx->last.qkb == qkb_u && ctx->last.step == step_cm &&
                            ctx->last.r_stop == r_stop_cm && ctx->last.n_steps == n_steps;
-    if (!(same_scan && wire_table_is(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm))) {
-        rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
-        if (rc) return rc;
-    }
     int64_t part_max = 0;
     for (int p = 0; p < n_part; ++p)
         if (po.off[p + 1] - po.off[p] > part_max) part_max = po.off[p + 1] - po.off[p];
@@ -1039,7 +1013,7 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     a.hk = make_stepk_host(step_cm);
     a.n_steps = n_steps;
     a.r_stop2 = r_stop_cm * r_stop_cm;
-    a.wt = ctx->wt;
+    a.wire_a = wire_a; a.wire_b = wire_b; a.n_wires = n_wires; a.fired_wire = fired_wire;
     a.W = n_fired;
     a.hit_off = hit_off;
     a.rho = rho;
@@ -1163,6 +1137,7 @@ extern "C" int comet_refine_seeds(comet_ctx* ctx, const double* seeds, int64_t s
 
 static int launch_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t seed_stride, int32_t charge,
                                  double bz_tesla, double step_cm, int32_t n_steps, double r_stop_cm,
+                                 const double* wire_a, const double* wire_b, int32_t n_wires, const int32_t* fired_wire,
                                  const int32_t* hit_off, const double* rho, int32_t n_fired, int32_t n_hits,
                                  double cutoff_cm, const int64_t* seed_idx, int32_t n_sel, const double* rss,
                                  double* dca, uint8_t* cls, double* seed_out, double* rss_out, cudaStream_t st,
@@ -1177,7 +1152,7 @@ static int launch_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t se
     a.hk = make_stepk_host(step_cm);
     a.n_steps = n_steps;
     a.r_stop2 = r_stop_cm * r_stop_cm;
-    a.wt = ctx->wt;
+    a.wire_a = wire_a; a.wire_b = wire_b; a.n_wires = n_wires; a.fired_wire = fired_wire;
     a.W = n_fired;
     a.hit_off = hit_off;
     a.rho = rho;
@@ -1215,9 +1190,8 @@ extern "C" int comet_classify_seeds(comet_ctx* ctx, const double* seeds, int64_t
     int rc = set_device(ctx);
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    rc = launch_wire_prep(ctx, wire_a, wire_b, n_wires, fired_wire, hit_off, rho, n_fired, cutoff_cm, step_cm, st);
-    if (rc) return rc;
-    return launch_classify_seeds(ctx, seeds, seed_stride, charge, bz_tesla, step_cm, n_steps, r_stop_cm, hit_off, rho,
+    return launch_classify_seeds(ctx, seeds, seed_stride, charge, bz_tesla, step_cm, n_steps, r_stop_cm, wire_a, wire_b, n_wires,
+                                 fired_wire, hit_off, rho,
                                  n_fired, n_hits, cutoff_cm, seed_idx, n_sel, nullptr, dca, cls, nullptr, nullptr, st);
 }
 
@@ -1307,7 +1281,8 @@ static int scan_stage_impl(comet_ctx* ctx, const double* seeds, int64_t seed_str
     rc = comet_select_references(ctx, cur, cur_stride, cur_n, rss, po_cur, n_part, hw, k_final, ref, cuda_stream);
     if (rc) return rc;
     // the wire table is the one comet_scan_rss has just written on this stream
-    return launch_classify_seeds(ctx, cur, cur_stride, charge, bz_tesla, step_cm, n_steps, r_stop_cm, hit_off, rho,
+    return launch_classify_seeds(ctx, cur, cur_stride, charge, bz_tesla, step_cm, n_steps, r_stop_cm, wire_a, wire_b, n_wires,
+                                 fired_wire, hit_off, rho,
                                  n_fired, n_hits, cutoff_cm, ref, n_part * k_final, rss, final_dca, cls, final_seed,
                                  final_rss, (cudaStream_t)cuda_stream, dyn);
 }

@@ -132,6 +132,20 @@ struct WireLine {
     double m0, m1, m2, w0, w1, w2;
 };
 
+// O4: the line of wire `wi` from its end points (SoA [3][n_wires]): w = (b - a) / |b - a|, m = (a + b) / 2
+__device__ __forceinline__ WireLine wire_line_of(const double* __restrict__ wire_a, const double* __restrict__ wire_b,
+                                                 int32_t n_wires, int wi)
+{
+    const double a0 = wire_a[wi], a1 = wire_a[(size_t)n_wires + wi], a2 = wire_a[2 * (size_t)n_wires + wi];
+    const double b0 = wire_b[wi], b1 = wire_b[(size_t)n_wires + wi], b2 = wire_b[2 * (size_t)n_wires + wi];
+    const double d0 = xsub(b0, a0), d1 = xsub(b1, a1), d2 = xsub(b2, a2);
+    const double len = xsqrt(xdot3(d0, d1, d2, d0, d1, d2));
+    WireLine wl;
+    wl.w0 = xdiv(d0, len); wl.w1 = xdiv(d1, len); wl.w2 = xdiv(d2, len);
+    wl.m0 = xmul(xadd(a0, b0), 0.5); wl.m1 = xmul(xadd(a1, b1), 0.5); wl.m2 = xmul(xadd(a2, b2), 0.5);
+    return wl;
+}
+
 // exact squared perpendicular distance from the wire line to x (O4/O5)
 __device__ __forceinline__ double perp2_exact(double x0, double x1, double x2, const WireLine& wl,
                                               double& u0, double& u1, double& u2)

@@ -54,14 +54,9 @@ __global__ void k_wire_prep(const double* __restrict__ wire_a, const double* __r
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= W) return;
-    const int wi = fired_wire[i];
-    const double a0 = wire_a[wi], a1 = wire_a[(size_t)n_wires + wi], a2 = wire_a[2 * (size_t)n_wires + wi];
-    const double b0 = wire_b[wi], b1 = wire_b[(size_t)n_wires + wi], b2 = wire_b[2 * (size_t)n_wires + wi];
     // exact line (O4): w = (b-a)/|b-a|, m = (a+b)/2
-    const double d0 = xsub(b0, a0), d1 = xsub(b1, a1), d2 = xsub(b2, a2);
-    const double len = xsqrt(xdot3(d0, d1, d2, d0, d1, d2));
-    const double w0 = xdiv(d0, len), w1 = xdiv(d1, len), w2 = xdiv(d2, len);
-    const double m0 = xmul(xadd(a0, b0), 0.5), m1 = xmul(xadd(a1, b1), 0.5), m2 = xmul(xadd(a2, b2), 0.5);
+    const WireLine wl = wire_line_of(wire_a, wire_b, n_wires, fired_wire[i]);
+    const double w0 = wl.w0, w1 = wl.w1, w2 = wl.w2, m0 = wl.m0, m1 = wl.m1, m2 = wl.m2;
     wt[0 * W + i] = m0; wt[1 * W + i] = m1; wt[2 * W + i] = m2;
     wt[3 * W + i] = w0; wt[4 * W + i] = w1; wt[5 * W + i] = w2;
     // orthonormal basis of the plane perpendicular to w (shortlist only)

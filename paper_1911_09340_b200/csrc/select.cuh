@@ -76,7 +76,10 @@ struct ClassifyArgs {
     StepK hk;
     int32_t n_steps;
     double r_stop2;
-    const double* wt;          // [14][W] from k_wire_prep
+    const double* wire_a;      // [3][n_wires] wire end points: the lines (O4) are formed here, no table of another kernel is read
+    const double* wire_b;
+    int32_t n_wires;
+    const int32_t* fired_wire; // [W]
     int32_t W;
     const int32_t* hit_off;
     const double* rho;
@@ -238,8 +241,7 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
         int ks = 0;
         double bd = 0.0;
         if (on) {
-            wl.m0 = a.wt[wi]; wl.m1 = a.wt[W + wi]; wl.m2 = a.wt[2 * W + wi];
-            wl.w0 = a.wt[3 * W + wi]; wl.w1 = a.wt[4 * W + wi]; wl.w2 = a.wt[5 * W + wi];
+            wl = wire_line_of(a.wire_a, a.wire_b, a.n_wires, a.fired_wire[wi]);
             const int len = (np + NSEG - 1) / NSEG;
             const int kb = seg * len, ke = min(np, kb + len);
             ks = -1;
