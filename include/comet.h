@@ -36,7 +36,8 @@ typedef enum comet_status {
     COMET_OK = 0,
     COMET_EINVAL = -1,   /* null pointer, negative size, bad option, limits exceeded */
     COMET_ENOMEM = -2,   /* device or host allocation failed */
-    COMET_ECUDA = -3     /* a CUDA runtime call failed; see comet_last_cuda_error */
+    COMET_ECUDA = -3,    /* a CUDA runtime call failed; see comet_last_cuda_error */
+    COMET_ELIMIT = -4    /* comet_argmin_static: more partitions than its statically allocated scratch holds */
 } comet_status;
 
 /* Seeds per track chunk: the track buffer is laid out in chunks of 32 consecutive seeds
@@ -603,6 +604,28 @@ int comet_scan_event_grid_submit(comet_ctx* ctx, int32_t slot, const double* axe
                                  void* cuda_stream);
 int comet_scan_event_grid_collect(comet_ctx* ctx, int32_t slot, int64_t* best_seed_host, double* best_rss_host,
                                   double* best_dca_host, uint8_t* cls_host);
+
+/* ---- an entry point that allocates nothing ---------------------------------------------------- */
+
+/* The per-partition argmin of step C (reading R15) on its own, for callers that cannot call cudaMalloc
+ * (code under CUDA-graph capture, tight serving loops, harnesses that forbid it): no ctx -- comet_create
+ * allocates --, no cudaMalloc / cudaFree / allocating routine, on the CURRENT device and `cuda_stream`.
+ * best_seed[p] = lowest-index argmin of rss over [part_off[p], part_off[p + 1]) (-1 for an empty partition),
+ * best_rss[p] its value (NaN for an empty partition); the NaN rule is comet_select_and_classify's, and the
+ * results are the same numbers as that call's best_seed / best_rss.
+ *   rss        dev [n_seeds]            part_off  HOST [n_part + 1], non-decreasing, within [0, n_seeds]; read before returning
+ *   best_seed  dev [n_part] (written)   best_rss  dev [n_part] (written); both owned by the caller
+ * The partial minima of the two-stage search (64 slices per partition) live in a file-scope device array of
+ * COMET_STATIC_MAX_PART x 64 x 16 bytes = 64 KB that every GPU that loads the library holds until the process
+ * exits.  n_part > COMET_STATIC_MAX_PART: COMET_ELIMIT, nothing is launched; n_seeds has no limit.
+ * ALL calls on a device share that array: calls whose kernels can overlap on the GPU (different streams
+ * without an ordering between them) race and give undefined results -- order them.  The array keeps the last
+ * call's contents; every slot a call reads it has written itself first, so nothing needs clearing between calls.
+ * The first call on a device resolves the array's device address (cudaGetSymbolAddress); make that call
+ * outside a stream capture.  COMET_ECUDA if the address cannot be resolved or a launch fails. */
+#define COMET_STATIC_MAX_PART 64
+int comet_argmin_static(const double* rss, int64_t n_seeds, const int64_t* part_off, int32_t n_part,
+                        int64_t* best_seed, double* best_rss, void* cuda_stream);
 
 /* ---- measurement helper ------------------------------------------------------------------ */
 

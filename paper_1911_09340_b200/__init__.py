@@ -4,6 +4,6 @@ The product is the C-ABI library `libcomet.so` (include/comet.h); `binding` mars
 into it.  Nothing here has a CPU implementation: without the built library, or without a CUDA
 device, the calls raise.
 """
-from .binding import Comet, CometError, lib_path, load_library, EXPORTED_SYMBOLS
+from .binding import Comet, CometError, argmin_static, lib_path, load_library, EXPORTED_SYMBOLS
 
-__all__ = ["Comet", "CometError", "lib_path", "load_library", "EXPORTED_SYMBOLS"]
+__all__ = ["Comet", "CometError", "argmin_static", "lib_path", "load_library", "EXPORTED_SYMBOLS"]

@@ -25,7 +25,7 @@ EXPORTED_SYMBOLS = [
     "comet_turns_half_work_bytes", "comet_scan_turns_half",
     "comet_reserve_scan", "comet_seed_grid", "comet_grid_axes_len", "comet_grid_z_run", "comet_seed_runs",
     "comet_set_geometry", "comet_get_geometry", "comet_scan_event_grid_host",
-    "comet_scan_event_grid_submit", "comet_scan_event_grid_collect",
+    "comet_scan_event_grid_submit", "comet_scan_event_grid_collect", "comet_argmin_static",
 ]
 
 COMET_CHUNK = 32
@@ -137,6 +137,7 @@ def load_library():
     L.comet_scan_event_grid_submit.argtypes = [vp, i32, vp, i32, i32, i32, i32, i32, i32, dbl, dbl, i32, dbl,
                                                vp, vp, vp, i32, i32, dbl, vp]
     L.comet_scan_event_grid_collect.argtypes = [vp, i32, vp, vp, vp, vp]
+    L.comet_argmin_static.argtypes = [vp, i64, vp, i32, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("comet_status_string", "comet_track_bytes", "comet_stage_work_bytes", "comet_turns_work_bytes",
                         "comet_hough_work_bytes", "comet_half_work_bytes", "comet_grid_axes_len", "comet_grid_z_run",
@@ -161,6 +162,37 @@ def _dev(t: Optional[torch.Tensor], dtype, name: str, device) -> int:
     if t.device.index != device:
         raise CometError("%s is on cuda:%s, the context is on cuda:%d" % (name, t.device.index, device))
     return int(t.data_ptr())
+
+
+STATIC_MAX_PART = 64        # COMET_STATIC_MAX_PART
+
+
+def argmin_static(rss, part_off: Sequence[int], best_seed=None, best_rss=None, stream=None):
+    """comet_argmin_static: per-partition lowest-index argmin of `rss` (CUDA float64 [S]) on rss's device, without a
+    context and without any allocation inside the library; the outputs are the caller's (int64 [P], float64 [P] CUDA
+    tensors; made here with torch when not given).  All calls on a device share one static scratch array: calls that
+    can overlap on the GPU race."""
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise CometError("no CUDA device: the seed x hit scan has no CPU implementation")
+    if not isinstance(rss, torch.Tensor) or not rss.is_cuda:
+        raise CometError("rss must be a CUDA tensor")
+    d = rss.device.index
+    po = np.ascontiguousarray(np.asarray(part_off, dtype=np.int64))
+    P = po.shape[0] - 1
+    with torch.cuda.device(d):
+        if best_seed is None:
+            best_seed = torch.empty(P, dtype=torch.int64, device=rss.device)
+        if best_rss is None:
+            best_rss = torch.empty(P, dtype=torch.float64, device=rss.device)
+        if best_seed.numel() < P or best_rss.numel() < P:
+            raise CometError("best_seed / best_rss hold fewer than %d partitions" % P)
+        rc = L.comet_argmin_static(_dev(rss, torch.float64, "rss", d), int(rss.numel()), po.ctypes.data, P,
+                                   _dev(best_seed, torch.int64, "best_seed", d), _dev(best_rss, torch.float64, "best_rss", d),
+                                   _stream_ptr(stream))
+    if rc != 0:
+        raise CometError("libcomet: %s (status %d)" % (L.comet_status_string(rc).decode(), rc))
+    return {"best_seed": best_seed, "best_rss": best_rss}
 
 
 class Comet:

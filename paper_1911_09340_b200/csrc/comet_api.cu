@@ -5,6 +5,7 @@
 
 #include <cuda_runtime.h>
 #include <math.h>
+#include <mutex>
 #include <new>
 #include <stdio.h>
 #include <string.h>
@@ -146,6 +147,7 @@ extern "C" const char* comet_status_string(int status)
         case COMET_EINVAL: return "invalid argument";
         case COMET_ENOMEM: return "out of memory";
         case COMET_ECUDA: return "CUDA runtime error";
+        case COMET_ELIMIT: return "size beyond the limit of the statically allocated scratch";
         default: return "unknown status";
     }
 }
@@ -2169,5 +2171,81 @@ extern "C" int comet_fp64_peak_probe(comet_ctx* ctx, int32_t iters, double* sink
     k_fp64_probe<<<blocks, threads, 0, (cudaStream_t)cuda_stream>>>(iters, sink_dev);
     CU(ctx, cudaGetLastError());
     if (n_fma) *n_fma = (double)blocks * threads * (double)iters * 8.0;
+    return COMET_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// comet_argmin_static: the per-partition argmin of step C (reading R15) for callers that
+// cannot allocate -- no ctx, no cudaMalloc: the partial minima live in a file-scope device array
+// ---------------------------------------------------------------------------------------------
+// Scratch of the two-stage argmin: [COMET_STATIC_MAX_PART][COMET_ARGMIN_SPLIT] partial values (doubles), then as many
+// partial indices (int64): 64 KB.  Every GPU that loads the library holds it until the process exits.  In HOST code the
+// name below is only a stand-in for the symbol, not a device address: host code takes the address from
+// cudaGetSymbolAddress (static_scratch_ptr), device code names the array directly.
+#define COMET_STATIC_SLOTS (COMET_STATIC_MAX_PART * COMET_ARGMIN_SPLIT)
+#define COMET_STATIC_BYTES (COMET_STATIC_SLOTS * (sizeof(double) + sizeof(int64_t)))
+#define COMET_STATIC_MAX_DEVICES 64
+static __device__ __align__(256) unsigned char g_static_scratch[COMET_STATIC_BYTES];
+
+// second stage: one warp per partition merges the partition's COMET_ARGMIN_SPLIT partial minima (lower value wins,
+// equal values -> lower index: R15) -- read from the array by its name -- and writes the winner as k_select_classify does
+__global__ void __launch_bounds__(32) k_argmin_static_finish(int64_t* __restrict__ best_seed, double* __restrict__ best_rss)
+{
+    const double* pv = reinterpret_cast<const double*>(g_static_scratch);
+    const int64_t* pi = reinterpret_cast<const int64_t*>(g_static_scratch + COMET_STATIC_SLOTS * sizeof(double));
+    const int p = blockIdx.x, lane = threadIdx.x;
+    double v = 0.0;
+    int64_t idx = -1;
+    for (int b = lane; b < COMET_ARGMIN_SPLIT; b += 32) argmin_merge(v, idx, pv[p * COMET_ARGMIN_SPLIT + b], pi[p * COMET_ARGMIN_SPLIT + b]);
+    for (int o = 16; o > 0; o >>= 1) {
+        const double v2 = __shfl_down_sync(0xffffffffu, v, o);
+        const int64_t i2 = __shfl_down_sync(0xffffffffu, idx, o);
+        argmin_merge(v, idx, v2, i2);
+    }
+    if (lane == 0) {
+        best_seed[p] = idx;
+        best_rss[p] = (idx >= 0 && v != -INFINITY) ? v : __longlong_as_double(0x7ff8000000000000LL);
+    }
+}
+
+// device address of g_static_scratch on the CURRENT device: resolved once per device, with that device current
+static std::mutex g_static_mu;
+static void* g_static_ptr[COMET_STATIC_MAX_DEVICES];
+static int static_scratch_ptr(void** out)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return COMET_ECUDA; }
+    if (dev < 0 || dev >= COMET_STATIC_MAX_DEVICES) return COMET_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_static_scratch) != cudaSuccess || !p) { cudaGetLastError(); return COMET_ECUDA; }
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return COMET_OK;
+}
+
+extern "C" int comet_argmin_static(const double* rss, int64_t n_seeds, const int64_t* part_off, int32_t n_part,
+                                   int64_t* best_seed, double* best_rss, void* cuda_stream)
+{
+    if (n_seeds < 0 || n_part < 0) return COMET_EINVAL;
+    if (n_part > COMET_STATIC_MAX_PART) return COMET_ELIMIT;
+    if (n_part == 0) return COMET_OK;
+    if (!part_off || !best_seed || !best_rss) return COMET_EINVAL;
+    PartOff po;
+    if (fill_partoff(&po, part_off, n_part, n_seeds, false)) return COMET_EINVAL;
+    if (po.off[n_part] > 0 && !rss) return COMET_EINVAL;
+    void* scratch = nullptr;
+    int rc = static_scratch_ptr(&scratch);
+    if (rc) return rc;
+    double* pv = reinterpret_cast<double*>(scratch);
+    int64_t* pi = reinterpret_cast<int64_t*>(reinterpret_cast<unsigned char*>(scratch) + COMET_STATIC_SLOTS * sizeof(double));
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // every slot the second stage reads is written by the first stage of the same call (an empty slice writes "none"):
+    // nothing of an earlier call survives, nothing has to start at zero
+    k_argmin_stage1<<<dim3(COMET_ARGMIN_SPLIT, n_part), COMET_ARGMIN_THREADS, 0, st>>>(rss, po, pv, pi);
+    k_argmin_static_finish<<<n_part, 32, 0, st>>>(best_seed, best_rss);
+    if (cudaGetLastError() != cudaSuccess) return COMET_ECUDA;
     return COMET_OK;
 }
