@@ -756,8 +756,9 @@ def run_ours(args):
     n_sub = 4 if zg_on else 6
     while n_sub > 1 and chunks // n_sub < 4 * n_sm * 2:
         n_sub -= 1
-    # k_wire_prep, per sub-slab (k_gen_unique,) the scan kernel, k_fine_ck, k_rss_sum; k_wire_prep, k_argmin_stage1, k_select_classify
-    launches_per_step = 1 + (4 if zg_on else 3) * n_sub + 3
+    # k_wire_prep, per sub-slab (k_gen_unique,) the scan kernel, k_fine_ck, k_rss_sum; k_argmin_stage1 (partitions of more than
+    # 16384 seeds), k_select_classify
+    launches_per_step = 1 + (4 if zg_on else 3) * n_sub + (2 if leg.S // max(1, leg.P) > 16384 else 1)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
