@@ -11,7 +11,7 @@ _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libcomet.so")
 _SOURCES = ["comet_api.cu"]
 _DEPS = ["comet_api.cu", "common.cuh", "extrapolate.cuh", "dca.cuh", "select.cuh", "scan_fused.cuh",
-         "refine.cuh", "turns.cuh", "hough.cuh", "half.cuh", "scan_zgroup.cuh",
+         "refine.cuh", "turns.cuh", "hough.cuh", "half.cuh", "scan_zgroup.cuh", "scan_zrun.cuh", "scan_small.cuh", "seedgrid.cuh",
          os.path.join("..", "..", "include", "comet.h")]
 
 NVCC_FLAGS = [
