@@ -41,8 +41,9 @@ FP64 = {
     "rkn_step": 50,        # k_gen_unique: RKN4 step of reading R1 in (x, y, T_x, T_y) + target-region test of R3
     "rkn_step_full": 52,   # plain kernels: the same with the z components
     "z_add": 1,            # k_scan_zrun: x_2' = x_2 + h T_2 per (seed, recorded state)
-    "sample_a": 12,        # k_scan_zrun level A / k_scan_fused level 0: one distance + threshold per (wire, sample)
-    "sample_b": 28,        # k_scan_zrun level B: the tangent-line bound per (wire, sub-block, distinct track)
+    "sample_a": 12,        # k_scan_fused level 0: one distance + threshold per (wire, sample)
+    "sample_a_zrun": 0,    # k_scan_zrun levels A and B run in single precision (pruning tests with rounding slack): no FP64-pipe
+    "sample_b": 0,         #   instruction; their FP32 work is listed in `fp32_thread_instr_pruning` (11 / 24 per test), not in `frac`
     "row": 9,              # swept row: two projections, the squared distance, the compare
     "fine_pair": 560,      # k_fine_ck<ZG> per pair that runs the virtual-plane iteration (exact decision between three
                            #   rows, ~2.5 iterations with an RKN4 sub-step each, signed distance, residual; measured with
@@ -332,7 +333,7 @@ class Leg:
         zg = st["unique_states"] > 0
         if zg:
             k = {"k_gen_unique": FP64["rkn_step"] * st["unique_states"],
-                 "k_scan": FP64["z_add"] * n_states + FP64["sample_a"] * st["samples"] + FP64["sample_b"] * st["samples_b"]
+                 "k_scan": FP64["z_add"] * n_states + FP64["sample_a_zrun"] * st["samples"] + FP64["sample_b"] * st["samples_b"]
                            + FP64["row"] * st["rows_executed"],
                  "k_fine_ck": FP64["fine_pair"] * st["fine_needed"]}
             tracks = S / self.z_run
@@ -363,6 +364,7 @@ class Leg:
         peak = FP64_PEAK_NOMINAL_TFLOPS
         bytes_model = sum(traffic.values())
         return {"fp64_thread_instr_executed": executed, "fp64_by_kernel": k,
+                "fp32_thread_instr_pruning": (11.0 * st["samples"] + 24.0 * st.get("samples_b", 0)) if zg else 0.0,
                 "tflops_executed": 2.0 * executed / t / 1e12, "frac_executed": 2.0 * executed / t / 1e12 / peak,
                 "frac_dense_equivalent": 2.0 * dense / t / 1e12 / peak,
                 "traffic_model_bytes": bytes_model, "traffic_model": traffic, "hbm_gbs_model": bytes_model / t / 1e9}

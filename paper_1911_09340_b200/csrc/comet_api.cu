@@ -89,7 +89,8 @@ struct comet_ctx {
     FieldMap field;              // field.B == nullptr: uniform field (the bz_tesla arguments)
     double* bmax;                // device scalar: largest |B| of the map
     // device workspace
-    double* wt;            // wire table [14][wt_cap]
+    double* wt;            // wire table [15][wt_cap]
+    float* wtf;            // single-precision shortlist fields [11][wt_cap]
     int32_t wt_cap;
     double* pv;            // argmin partials [MAX_PART][SPLIT]
     int64_t* pi;
@@ -169,6 +170,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->n_sm, cudaDevAttrMultiProcessorCount, cuda_device);
     ctx->wt_cap = 8192;
     if (e == cudaSuccess) e = cudaMalloc(&ctx->wt, sizeof(double) * COMET_WT_FIELDS * (size_t)ctx->wt_cap);
+    if (e == cudaSuccess) e = cudaMalloc(&ctx->wtf, sizeof(float) * 11 * (size_t)ctx->wt_cap);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->pv, sizeof(double) * COMET_MAX_PARTITIONS * COMET_ARGMIN_SPLIT);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->pi, sizeof(int64_t) * COMET_MAX_PARTITIONS * COMET_ARGMIN_SPLIT);
     if (e == cudaSuccess) e = cudaMalloc(&ctx->stats, sizeof(unsigned long long) * ST_N);
@@ -212,6 +214,18 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_coarse_pruned<COMET_PRUNED_WT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, pr_smem);
     for (int j = 0; j < COMET_TEV_RING * 5 && e == cudaSuccess; ++j) e = cudaEventCreate(&ctx->tev[j / 5][j % 5]);
     // shared-memory opt-ins (done once here, never on the hot path)
+#define COMET_ZRUN_OPTIN(NU)                                                                                                   \
+    do {                                                                                                                       \
+        const int zs = COMET_ZR_SMEM(NU, ctx->wt_cap);                                                                         \
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<false, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, zs); \
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<false, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, zs);  \
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<true, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, zs);  \
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<true, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, zs);   \
+    } while (0)
+    COMET_ZRUN_OPTIN(1);
+    COMET_ZRUN_OPTIN(2);
+    COMET_ZRUN_OPTIN(4);
+#undef COMET_ZRUN_OPTIN
     const int dca_smem = (2 * COMET_KT * 3 * COMET_LANES + COMET_DCA_WARPS * 4 * 32) * (int)sizeof(double);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(k_dca_rss<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, dca_smem);
@@ -233,7 +247,7 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
         e = cudaFuncSetAttribute(k_classify_seeds<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (COMET_MAX_STEPS + 1) * 6 * (int)sizeof(double));
     if (e != cudaSuccess) {
-        cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats); cudaFree(ctx->n_items);
+        cudaFree(ctx->wt); cudaFree(ctx->wtf); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats); cudaFree(ctx->n_items);
         delete ctx;
         return e == cudaErrorMemoryAllocation ? COMET_ENOMEM : COMET_ECUDA;
     }
@@ -245,7 +259,7 @@ extern "C" int comet_destroy(comet_ctx* ctx)
 {
     if (!ctx) return COMET_EINVAL;
     cudaSetDevice(ctx->device);
-    cudaFree(ctx->wt); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
+    cudaFree(ctx->wt); cudaFree(ctx->wtf); cudaFree(ctx->pv); cudaFree(ctx->pi); cudaFree(ctx->stats);
     cudaFree(ctx->kb); cudaFree(ctx->e2); cudaFree(ctx->items); cudaFree(ctx->n_items); cudaFree(ctx->zg_flag); cudaFree(ctx->ref_fb); cudaFree(ctx->ub); cudaFree(ctx->npu);
     for (int j = 0; j < COMET_TEV_RING * 5; ++j) if (ctx->tev[j / 5][j % 5]) cudaEventDestroy(ctx->tev[j / 5][j % 5]);
     cudaFree(ctx->geom_a); cudaFree(ctx->geom_b);
@@ -504,7 +518,7 @@ static int launch_wire_prep(comet_ctx* ctx, const double* wire_a, const double* 
     if (n_fired == 0) return COMET_OK;
     const int32_t uniform = ctx->field.B == nullptr ? 1 : 0;
     k_wire_prep<<<(n_fired + 127) / 128, 128, 0, st>>>(wire_a, wire_b, n_wires, fired_wire, n_fired, hit_off, rho,
-                                                       cutoff_cm, step_cm, uniform, ctx->wt);
+                                                       cutoff_cm, step_cm, uniform, ctx->wt, ctx->wtf);
     CU(ctx, cudaGetLastError());
     return COMET_OK;
 }
@@ -820,6 +834,7 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
             a.n_steps = n_steps;
             a.r_stop2 = r_stop_cm * r_stop_cm;
             a.wt = ctx->wt;
+            a.wtf = ctx->wtf;
             a.W = n_fired;
             a.hit_off = hit_off;
             a.rho = rho;

@@ -50,7 +50,7 @@ namespace comet {
 __global__ void k_wire_prep(const double* __restrict__ wire_a, const double* __restrict__ wire_b,
                             int32_t n_wires, const int32_t* __restrict__ fired_wire, int32_t W,
                             const int32_t* __restrict__ hit_off, const double* __restrict__ rho,
-                            double lambda, double h, int tight, double* __restrict__ wt)
+                            double lambda, double h, int tight, double* __restrict__ wt, float* __restrict__ wtf = nullptr)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= W) return;
@@ -80,6 +80,17 @@ __global__ void k_wire_prep(const double* __restrict__ wire_a, const double* __r
         cap = fmin(cap, eps + sqrt(b * b + 0.2505 * h * h + eps * eps));
     }
     wt[14 * W + i] = (rmax < 0.0) ? -1.0 : cap;
+    // single-precision copy of the shortlist fields for the pruning tests of k_scan_zrun (levels A and B): the basis and
+    // offsets rounded to nearest (the tests carry the rounding as slack), the far radius, sqrt(1 - w_z^2) and |c1| + |c2|
+    // rounded up
+    if (wtf) {
+        const double c1 = -(m0 * p0 + m1 * p1 + m2 * p2), c2 = -(m0 * q0 + m1 * q1 + m2 * q2);
+        wtf[0 * W + i] = (float)p0; wtf[1 * W + i] = (float)p1; wtf[2 * W + i] = (float)p2; wtf[3 * W + i] = (float)c1;
+        wtf[4 * W + i] = (float)q0; wtf[5 * W + i] = (float)q1; wtf[6 * W + i] = (float)q2; wtf[7 * W + i] = (float)c2;
+        wtf[8 * W + i] = (rmax < 0.0) ? -1.f : __double2float_ru(cap);
+        wtf[9 * W + i] = __fsqrt_ru(__double2float_ru(fma(p2, p2, q2 * q2)));
+        wtf[10 * W + i] = __double2float_ru(fabs(c1) + fabs(c2));
+    }
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src)

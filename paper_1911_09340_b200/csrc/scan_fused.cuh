@@ -82,6 +82,7 @@ struct FusedArgs {
     int32_t n_steps;
     double r_stop2;
     const double* wt;        // [15][W]
+    const float* wtf;        // [11][W] single-precision shortlist fields (k_wire_prep), for k_scan_zrun's levels A and B
     int32_t W;
     const int32_t* hit_off;
     const double* rho;

@@ -12,10 +12,10 @@
 //   staging    per 64-row block the (x, y) rows of the chunk's NU tracks (2 KB for NU = 2) and the tangents of the 8
 //              sub-block samples go to the warp's shared memory with cp.async, one block ahead (double buffer), so
 //              the L2 latency of ub is off the path;
-//   level A    per 64-row block and wire: the distance of ONE sample (row 36) of each distinct track, taken at
+//   level A    (float) per 64-row block and wire: the distance of ONE sample (row 36) of each distinct track, taken at
 //              the centre of the run's z range, against R_i + (z half range) sqrt(1 - w_z^2) + 36 L -- the
 //              1-Lipschitz bound of dca.cuh; the wires that pass are compacted into a list;
-//   level B    per listed wire, 8-row sub-block and distinct track: the sample (row 4 of the sub-block) WITH ITS
+//   level B    (float) per listed wire, 8-row sub-block and distinct track: the sample (row 4 of the sub-block) WITH ITS
 //              TANGENT.  The rows of the sub-block lie within U = 4 h of arc of the sample, and a curve of
 //              curvature <= |c| leaves its tangent line by at most |c| U^2 / 2 over that arc, so no row of any seed
 //              of the run is closer to the wire than
@@ -36,6 +36,14 @@
 //              k_fine_ck, the others are dropped; the chunk's mask of rows k_fine_ck will fill goes to memory and
 //              k_rss_sum adds cutoff^2 for every other wire without reading anything.
 //
+// Levels A and B only prune, with slack, so they run in SINGLE precision (north_star: "FP32 for the coarse search"): the
+// 8 samples of a block per track are converted once per block, the wire's shortlist fields come from a float table
+// (k_wire_prep: basis and offsets rounded to nearest, far radius and sqrt(1 - w_z^2) rounded up).  Rounding: a projected
+// offset u = x e_x + y e_y + z e_z + c evaluated in float from rounded inputs is off by less than 5 x 2^-24 S,
+// S = |x| + |y| + |z| + |c|, a distance by sqrt(2) times that, the tangent's projections by 9 x 2^-24, the closed-form minimum
+// by another ~1e-5 cm; every threshold takes 32 x 2^-24 (X + |c1| + |c2|) on top, X >= |x| + |y| + |z| for every state of
+// the chunk (the seeds' largest |x_0|_1 + 3.003 n_steps h), and thr^2 a factor 1 + 2e-6.  The sweeps stay in double
+// precision: they choose the row, and a wrong choice between non-adjacent rows would not be repaired afterwards.
 // Only shortlists are decided here (FMA-form distances, slack 1e-6 cm on every bound): k_fine_ck<ZG> re-decides
 // between rows k-1, k, k+1 with the definition's exact operations, so n_pts and RSS are the bit-identical numbers
 // of the plain path and of the definition.  A chunk with a lane beyond |c| h <= 0.05 opens everything.
@@ -54,10 +62,15 @@ namespace comet {
 #define COMET_ZR_NF (COMET_FUSED_WFIELDS + 1)
 // doubles of shared memory per warp: two staged blocks of (64 rows + 8 sample tangents) x NU tracks x 2, the pass
 // list (64 shorts); the item list of the finish (LCAP shorts = 256 doubles) reuses the staged blocks
-#define COMET_ZR_WSM(NU) (2 * (64 + 8) * (NU) * 2 + 16)
+// + the single-precision samples of the staged block: [8 sub-blocks][NU tracks][x, y, z, T_x, T_y, -, -, -] floats
+#define COMET_ZR_WSM(NU) (2 * (64 + 8) * (NU) * 2 + 16 + 8 * (NU) * 4)
+#define COMET_ZR_FF 11             // fields of the single-precision wire table (k_wire_prep)
 // + the touched-wire mask: one bit per fired wire, rounded up to whole 16 bytes
 #define COMET_ZR_MWD(W) ((((W) + 31) / 32 + 3) / 4 * 2)
-#define COMET_ZR_SMEM(NU, W) ((COMET_ZR_NF * COMET_ZR_WCAP + COMET_ZR_WARPS * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W))) * (int)sizeof(double))
+#define COMET_ZR_SMEM(NU, W) ((COMET_ZR_NF * COMET_ZR_WCAP + COMET_ZR_WARPS * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W))) * (int)sizeof(double) + \
+                              COMET_ZR_FF * COMET_ZR_WCAP * (int)sizeof(float))
+// relative rounding slack of the single-precision tests: 32 x 2^-24 per unit of (|x| + |y| + |z| + |c1| + |c2|)
+#define COMET_ZR_FSLACK 1.9073486e-6f
 #define COMET_ZR_MARGIN 1e-6       // cm, added to every pruning threshold (FMA rounding is ~1e-13)
 
 template <bool BIGW>
@@ -73,6 +86,12 @@ __device__ __forceinline__ void zr_evalc(EvalC& w, const double* wtab, const dou
     w.c1 = zr_const<BIGW>(wtab, wt, W, 3, i);
     w.e2x = zr_const<BIGW>(wtab, wt, W, 4, i); w.e2y = zr_const<BIGW>(wtab, wt, W, 5, i); w.e2z = zr_const<BIGW>(wtab, wt, W, 6, i);
     w.c2 = zr_const<BIGW>(wtab, wt, W, 7, i);
+}
+template <bool BIGW>
+__device__ __forceinline__ float zr_constf(const float* wtabf, const float* __restrict__ wtf, int W, int f, int i)
+{
+    if (!BIGW) return wtabf[f * COMET_ZR_WCAP + i];
+    return (i < COMET_ZR_WCAP) ? wtabf[f * COMET_ZR_WCAP + i] : __ldg(wtf + (size_t)f * W + i);
 }
 template <bool BIGW>
 __device__ __forceinline__ double zr_slope(const double* wtab, const double* __restrict__ wt, int W, int i)
@@ -101,7 +120,9 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     const int MW = (W + 31) / 32;                           // words of the touched-wire mask
     double* stg = zsm + NF * WCAP + warp * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W));   // two staged blocks
     unsigned short* plist = reinterpret_cast<unsigned short*>(stg + 2 * BUFD);     // [64] wires that passed level A
-    unsigned* tmask = reinterpret_cast<unsigned*>(stg + 2 * BUFD + 16);            // [MW] bit i: the key row of wire i exists
+    float* sampf = reinterpret_cast<float*>(stg + 2 * BUFD + 16);                  // [8][NU][8] samples of the current block
+    unsigned* tmask = reinterpret_cast<unsigned*>(stg + 2 * BUFD + 16 + NSUB * NU * 4);   // [MW] bit i: the key row of wire i exists
+    float* wtabf = reinterpret_cast<float*>(zsm + NF * WCAP + COMET_ZR_WARPS * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W)));   // [FF][WCAP]
     unsigned short* lst = reinterpret_cast<unsigned short*>(stg);                  // finish: [<= LCAP] items
     constexpr int LCAPW = (NU == 1) ? (2 * BUFD * 4) : LCAP;                       // shorts the staged blocks hold
     for (int v = threadIdx.x; v < COMET_FUSED_WFIELDS * WCAP; v += 32 * COMET_ZR_WARPS) {
@@ -110,6 +131,10 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     }
     for (int i = threadIdx.x; i < WCAP; i += 32 * COMET_ZR_WARPS)
         wtab[COMET_FUSED_WFIELDS * WCAP + i] = (i < W) ? wire_slope(__ldg(a.wt + (size_t)8 * W + i), __ldg(a.wt + (size_t)12 * W + i)) : 0.0;
+    for (int v = threadIdx.x; v < COMET_ZR_FF * WCAP; v += 32 * COMET_ZR_WARPS) {
+        const int f = v / WCAP, i = v - f * WCAP;
+        wtabf[v] = (i < W) ? __ldg(a.wtf + (size_t)f * W + i) : -1.f;
+    }
     __syncthreads();
     const int64_t chunk = (int64_t)blockIdx.x * COMET_ZR_WARPS + warp;
     if (chunk * COMET_LANES >= a.n_seeds) return;
@@ -170,6 +195,28 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
 #pragma unroll
     for (int t = 0; t < NU; ++t)
         if (np_t[t] > 0) npmin = min(npmin, np_t[t]);
+
+    // Levels A and B are pruning tests with slack: they run in single precision (twice the rate of the FP64 pipe, half the
+    // registers).  Every input is rounded to float and every operation rounds again: a projected offset
+    // u = x e_x + y e_y + z e_z + c is off by less than 8 x 2^-24 (|x| + |y| + |z| + |c|), a distance by less than twice
+    // that; the thresholds take COMET_ZR_FSLACK x (X + |c1| + |c2|) on top, X >= |x| + |y| + |z| of every state of the chunk.
+    float zh_f[NU], tz_f[NU];
+#pragma unroll
+    for (int t = 0; t < NU; ++t) {
+        zh_f[t] = __double2float_ru(zh_t[t]);
+        tz_f[t] = (float)tz_t[t];
+    }
+    float xsum_f;
+    {
+        const float xs = valid ? __double2float_ru(fabs(st.x0) + fabs(st.x1) + fabs(st.x2)) : 0.f;
+        xsum_f = __uint_as_float(__reduce_max_sync(FULL, __float_as_uint(xs))) + __double2float_ru(3.003 * (double)a.n_steps * h);
+    }
+    const float dev_f = __double2float_ru(dev + COMET_ZR_MARGIN), lipA_f = __double2float_ru(SROW * L + COMET_ZR_MARGIN);
+    const float U_f = __double2float_ru(U * 1.000001);
+    // the sample this lane converts per block: sub-block lane / NU of track lane % NU
+    const int tq = lane & (NU - 1);
+    const double zc_q = __shfl_sync(FULL, zc0, tq << ZSH), hz_q = __shfl_sync(FULL, hz, tq << ZSH);
+    const int32_t np_q = __shfl_sync(FULL, np, tq << ZSH);
 
     // staging: lane l copies the pieces p = l, l + 32, ... of a block: always of track l % NU
     const int ts = lane & (NU - 1);
@@ -238,46 +285,53 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
         const bool tail = r0 + BLK > npmin;                 // some track of the chunk ends in this block
         const double r0d = (double)r0;
         const double zb = fma(r0d, hz, z0);                 // the seed's z at row r0 (to rounding: shortlist only)
-        double zcb[NU];                                     // the run centre's z at row r0
-#pragma unroll
-        for (int t = 0; t < NU; ++t) zcb[t] = fma(r0d, hz_t[t], zc_t[t]);
-        // z of a sample: row r0 + kr of track t at the run's centre (a sample past the last state repeats it)
-        auto samp_z = [&](int t, int kr) {
-            if (!tail) return fma((double)kr, hz_t[t], zcb[t]);
-            return fma((double)min(kr, np_t[t] - 1 - r0), hz_t[t], zcb[t]);
-        };
+        // the block's 8 samples per track (row 4 of every sub-block) in single precision: position at the run's centre in z
+        // (a sample past the track's last state repeats it) and tangent
+        if (lane < NSUB * NU) {
+            const int j = lane >> (5 - ZSH);
+            const int kr = j * SUB + SUB / 2;
+            const double2 xy = *reinterpret_cast<const double2*>(rows + (kr * NU + tq) * 2);
+            const double2 tt = *reinterpret_cast<const double2*>(tang + (j * NU + tq) * 2);
+            const double z = fma((double)(r0 + (tail ? min(kr, np_q - 1 - r0) : kr)), hz_q, zc_q);
+            float4 f0;
+            f0.x = (float)xy.x; f0.y = (float)xy.y; f0.z = (float)z; f0.w = (float)tt.x;
+            *reinterpret_cast<float4*>(sampf + (j * NU + tq) * 8) = f0;
+            sampf[(j * NU + tq) * 8 + 4] = (float)tt.y;
+        }
+        __syncwarp();
         int cnt = 0;
         auto level_b = [&](const unsigned short* list, int n) {
             // ---- level B (lane = listed wire): tangent-line bound per (distinct track, sub-block) ------------
             const int i = lane < n ? (int)list[lane] : -1;
             unsigned m8 = 0u;
             if (i >= 0) {
-                EvalC ec;
-                zr_evalc<BIGW>(ec, wtab, a.wt, W, i);
-                const double cap = zr_const<BIGW>(wtab, a.wt, W, 8, i);
-                const double swz = zr_slope<BIGW>(wtab, a.wt, W, i);
+                const float e1x = zr_constf<BIGW>(wtabf, a.wtf, W, 0, i), e1y = zr_constf<BIGW>(wtabf, a.wtf, W, 1, i);
+                const float e1z = zr_constf<BIGW>(wtabf, a.wtf, W, 2, i), c1 = zr_constf<BIGW>(wtabf, a.wtf, W, 3, i);
+                const float e2x = zr_constf<BIGW>(wtabf, a.wtf, W, 4, i), e2y = zr_constf<BIGW>(wtabf, a.wtf, W, 5, i);
+                const float e2z = zr_constf<BIGW>(wtabf, a.wtf, W, 6, i), c2 = zr_constf<BIGW>(wtabf, a.wtf, W, 7, i);
+                const float cap = zr_constf<BIGW>(wtabf, a.wtf, W, 8, i), swz = zr_constf<BIGW>(wtabf, a.wtf, W, 9, i);
+                const float slack = COMET_ZR_FSLACK * (xsum_f + zr_constf<BIGW>(wtabf, a.wtf, W, 10, i));
 #pragma unroll
                 for (int t = 0; t < NU; ++t) {
                     if (np_t[t] <= r0) continue;
-                    const double thr = cap + zh_t[t] * swz + dev + COMET_ZR_MARGIN;
-                    const double thr2 = thr * thr;
-                    const double bz1 = tz_t[t] * ec.e1z, bz2 = tz_t[t] * ec.e2z;
+                    const float thr = fmaf(zh_f[t], swz, cap) + dev_f + slack;
+                    const float thr2 = thr * thr * 1.000002f;
+                    const float bz1 = tz_f[t] * e1z, bz2 = tz_f[t] * e2z;
 #pragma unroll
                     for (int j = 0; j < NSUB; ++j) {
                         if (np_t[t] <= r0 + j * SUB) break;          // the track has no row in this sub-block
-                        const double2 xy = *reinterpret_cast<const double2*>(rows + ((j * SUB + SUB / 2) * NU + t) * 2);
-                        const double2 tt = *reinterpret_cast<const double2*>(tang + (j * NU + t) * 2);
-                        const double z = samp_z(t, j * SUB + SUB / 2);
-                        const double a1 = fma(xy.x, ec.e1x, fma(xy.y, ec.e1y, fma(z, ec.e1z, ec.c1)));
-                        const double a2 = fma(xy.x, ec.e2x, fma(xy.y, ec.e2y, fma(z, ec.e2z, ec.c2)));
-                        const double b1 = fma(tt.x, ec.e1x, fma(tt.y, ec.e1y, bz1));
-                        const double b2 = fma(tt.x, ec.e2x, fma(tt.y, ec.e2y, bz2));
-                        const double aa = fma(a1, a1, a2 * a2), bb = fma(b1, b1, b2 * b2);
-                        const double ab = fabs(fma(a1, b1, a2 * b2));
+                        const float4 p = *reinterpret_cast<const float4*>(sampf + (j * NU + t) * 8);   // x, y, z, T_x
+                        const float ty = sampf[(j * NU + t) * 8 + 4];
+                        const float a1 = fmaf(p.x, e1x, fmaf(p.y, e1y, fmaf(p.z, e1z, c1)));
+                        const float a2 = fmaf(p.x, e2x, fmaf(p.y, e2y, fmaf(p.z, e2z, c2)));
+                        const float b1 = fmaf(p.w, e1x, fmaf(ty, e1y, bz1));
+                        const float b2 = fmaf(p.w, e2x, fmaf(ty, e2y, bz2));
+                        const float aa = fmaf(a1, a1, a2 * a2), bb = fmaf(b1, b1, b2 * b2);
+                        const float ab = fabsf(fmaf(a1, b1, a2 * b2));
                         // min over |u| <= U of |a + u b|^2 = aa - sv (2 ab - sv) / bb with sv = min(ab, U bb)
-                        const double ubb = U * bb;
-                        const double sv = ab < ubb ? ab : ubb;   // (fmin without its NaN rule: a NaN fails the test below either way)
-                        if (fma(aa - thr2, bb, -(sv * fma(2.0, ab, -sv))) <= 0.0) m8 |= 1u << j;
+                        const float ubb = U_f * bb;
+                        const float sv = ab < ubb ? ab : ubb;
+                        if (fmaf(aa - thr2, bb, -(sv * fmaf(2.f, ab, -sv))) <= 0.f) m8 |= 1u << j;
                     }
                     if (STATS) st_cnt[ST_SAMPLES_B] += NSUB;
                 }
@@ -340,27 +394,31 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
             }
         };
         // ---- level A (lane = wire): one sample per distinct track and block ----------------------------------
-        double zs_a[NU];
-#pragma unroll
-        for (int t = 0; t < NU; ++t) zs_a[t] = samp_z(t, SROW);
+        constexpr int JA = SROW / SUB;                        // the sample of level A is sub-block 4's (row 36)
+        static_assert(JA * SUB + SUB / 2 == SROW, "level A takes a sample level B has");
         for (int r = 0; r < n_rounds; ++r) {
             const int i = r * 32 + lane;
             const int ii = min(i, W - 1);
-            EvalC ec;
-            zr_evalc<BIGW>(ec, wtab, a.wt, W, ii);
-            const double cap = (i < W) ? zr_const<BIGW>(wtab, a.wt, W, 8, ii) : -1.0;    // far radius; < 0: no entries
-            const double swz = zr_slope<BIGW>(wtab, a.wt, W, ii);
+            const float e1x = zr_constf<BIGW>(wtabf, a.wtf, W, 0, ii), e1y = zr_constf<BIGW>(wtabf, a.wtf, W, 1, ii);
+            const float e1z = zr_constf<BIGW>(wtabf, a.wtf, W, 2, ii), c1 = zr_constf<BIGW>(wtabf, a.wtf, W, 3, ii);
+            const float e2x = zr_constf<BIGW>(wtabf, a.wtf, W, 4, ii), e2y = zr_constf<BIGW>(wtabf, a.wtf, W, 5, ii);
+            const float e2z = zr_constf<BIGW>(wtabf, a.wtf, W, 6, ii), c2 = zr_constf<BIGW>(wtabf, a.wtf, W, 7, ii);
+            const float cap = (i < W) ? zr_constf<BIGW>(wtabf, a.wtf, W, 8, ii) : -1.f;    // far radius; < 0: no entries
+            const float swz = zr_constf<BIGW>(wtabf, a.wtf, W, 9, ii);
+            const float slack = COMET_ZR_FSLACK * (xsum_f + zr_constf<BIGW>(wtabf, a.wtf, W, 10, ii));
             bool pass = false;
 #pragma unroll
             for (int t = 0; t < NU; ++t) {
                 if (np_t[t] <= r0) continue;
-                const double2 xy = *reinterpret_cast<const double2*>(rows + (SROW * NU + t) * 2);
-                const double thr = cap + zh_t[t] * swz + SROW * L + COMET_ZR_MARGIN;
-                pass = pass || (d2_fma(ec, xy.x, xy.y, zs_a[t]) <= thr * thr);
-                if (STATS && cap >= 0.0) st_cnt[ST_SAMPLES] += 1;
+                const float4 p = *reinterpret_cast<const float4*>(sampf + (JA * NU + t) * 8);
+                const float thr = fmaf(zh_f[t], swz, cap) + lipA_f + slack;
+                const float u1 = fmaf(p.x, e1x, fmaf(p.y, e1y, fmaf(p.z, e1z, c1)));
+                const float u2 = fmaf(p.x, e2x, fmaf(p.y, e2y, fmaf(p.z, e2z, c2)));
+                pass = pass || (fmaf(u1, u1, u2 * u2) <= thr * thr * 1.000002f);
+                if (STATS && cap >= 0.f) st_cnt[ST_SAMPLES] += 1;
             }
             if (any_nolip) pass = true;
-            if (cap < 0.0) pass = false;
+            if (cap < 0.f) pass = false;
             const unsigned pm = __ballot_sync(FULL, pass);
             if (pass) plist[cnt + __popc(pm & ((1u << lane) - 1u))] = (unsigned short)i;
             cnt += __popc(pm);
