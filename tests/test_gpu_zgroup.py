@@ -149,3 +149,32 @@ def test_turn_loop_at_full_size_runs_partitions_through_the_z_run_kernels(comet,
     assert np.array_equal(got["turn_seed"].cpu().numpy(), ref["turn_seed"])
     assert np.array_equal(got["turn_rss"].cpu().numpy(), ref["turn_rss"])
     assert np.array_equal(got["turn_cls"].cpu().numpy(), ref["turn_cls"])
+
+
+@pytest.mark.parametrize("shift", [(0.0, 0.0, 0.0), (3000.0, -2000.0, 5000.0), (-40000.0, 25000.0, 8000.0),
+                                   (1.0e6, -2.0e6, 5.0e5), (1.0e7, 2.0e7, -1.5e7)])
+def test_single_precision_pruning_far_from_the_origin(comet, cfg1_event, shift):
+    """Levels A and B of k_scan_zrun prune in single precision with the rounding carried as slack proportional to the
+    size of the coordinates.  The whole event -- wires and seeds -- is moved away from the origin, up to 2e7 cm, where a
+    float resolves 1-2 cm (the drift circles are 0.1-0.8 cm, the far radii about 1 cm): without the slack the tests drop
+    near pairs there (checked once with COMET_ZR_FSLACK = 0: the last case fails on RSS; the far radius is itself
+    conservative by more than 0.1 cm, so smaller shifts do not show it); with it RSS and n_pts stay bit-identical to the
+    oracle's on the same shifted inputs (no target region: it is centred on the origin).  Up to 4e4 cm the pruning still
+    prunes; at 2e7 cm the slack opens everything (rows of the last 64-row block included), which is the correct answer."""
+    import copy
+    ev = copy.deepcopy(cfg1_event)
+    sp = ev.spec
+    sh = np.asarray(shift)
+    seeds = seed_grid(ev, 1, (8, 4, 4, 16), tuple(sp["p_range"]), ct_hw=sp.get("ct_hw", 0.15))
+    seeds = np.ascontiguousarray(seeds)
+    seeds[0:3] += sh[:, None]
+    ev.geom.wire_a[:] = ev.geom.wire_a + sh[:, None]
+    ev.geom.wire_b[:] = ev.geom.wire_b + sh[:, None]
+    ev.n_steps = 400
+    ref = _oracle(ev, seeds, r_stop=0.0)
+    rss, n_pts, st = _scan(comet, ev, seeds, 1, r_stop=0.0)
+    assert st["unique_states"] > 0                              # the z-run kernels served the launch
+    assert np.array_equal(n_pts, ref["n_pts"])
+    assert np.array_equal(rss, ref["rss"])
+    assert float(np.min(rss)) < ev.n_fired * ev.cutoff ** 2     # some seed is near some wire: the comparison is not vacuous
+    assert st["rows_executed"] < (0.25 if max(abs(v) for v in shift) < 1e5 else 1.2) * seeds.shape[1] * ev.n_fired * 401
