@@ -43,7 +43,7 @@ FP64 = {
     "z_add": 1,            # k_scan_zrun: x_2' = x_2 + h T_2 per (seed, recorded state)
     "sample_a": 12,        # k_scan_fused level 0: one distance + threshold per (wire, sample)
     "sample_a_zrun": 0,    # k_scan_zrun levels A and B run in single precision (pruning tests with rounding slack): no FP64-pipe
-    "sample_b": 0,         #   instruction; their FP32 work is listed in `fp32_thread_instr_pruning` (11 / 24 per test), not in `frac`
+    "sample_b": 0,         #   instruction; their FP32 work is listed in `fp32_thread_instr_pruning` (12 / 28 per test), not in `frac`
     "row": 9,              # swept row: two projections, the squared distance, the compare
     "fine_pair": 560,      # k_fine_ck<ZG> per pair that runs the virtual-plane iteration (exact decision between three
                            #   rows, ~2.5 iterations with an RKN4 sub-step each, signed distance, residual; measured with
@@ -56,8 +56,8 @@ DENSE = {"rkn_step": 52, "row": 9, "fine_pair": 600}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch on configs[1], from the ncu --set full capture of THIS build
 # named beside them (profiles/): the bytes the live run moves are modelled from the library's own sizes below
 NCU_TRAFFIC = {"file": "profiles/r2_full_zrun.txt", "per": "launch = one sub-slab of 3072 chunks; a configs[1] step has four",
-               "k_gen_unique": 26.5e6, "k_scan_zrun": 121.5e6, "k_fine_ck": 63.1e6, "k_rss_sum": 17.7e6,
-               "per_step": 4 * (26.5e6 + 121.5e6 + 63.1e6 + 17.7e6)}
+               "k_gen_unique": 27.2e6, "k_scan_zrun": 119.0e6, "k_fine_ck": 63.0e6, "k_rss_sum": 17.7e6,
+               "per_step": 4 * (27.2e6 + 119.0e6 + 63.0e6 + 17.7e6)}
 STAGE_HALF_WIDTH = [0.6, 0.5, 0.5, 1.0]
 STAGE_GRID = [5, 5, 5, 5]
 FIELD_TOL = 1e-7
@@ -364,7 +364,7 @@ class Leg:
         peak = FP64_PEAK_NOMINAL_TFLOPS
         bytes_model = sum(traffic.values())
         return {"fp64_thread_instr_executed": executed, "fp64_by_kernel": k,
-                "fp32_thread_instr_pruning": (11.0 * st["samples"] + 24.0 * st.get("samples_b", 0)) if zg else 0.0,
+                "fp32_thread_instr_pruning": (12.0 * st["samples"] + 28.0 * st.get("samples_b", 0)) if zg else 0.0,
                 "tflops_executed": 2.0 * executed / t / 1e12, "frac_executed": 2.0 * executed / t / 1e12 / peak,
                 "frac_dense_equivalent": 2.0 * dense / t / 1e12 / peak,
                 "traffic_model_bytes": bytes_model, "traffic_model": traffic, "hbm_gbs_model": bytes_model / t / 1e9}
@@ -609,13 +609,20 @@ def run_ours(args):
         del one
         run_batch()
         torch.cuda.synchronize()
-        ms_batch, res = _time_steps(run_batch, 3, stream)
+        # (the leg is bound by the host's launch rate -- 256 events x ~25 launches from one thread --, which varies with what
+        # else the box's cores do: the median of five repetitions, every one timed with CUDA events; all five are listed)
+        reps = []
+        for _ in range(5):
+            ms_r, res = _time_steps(run_batch, 1, stream)
+            reps.append(ms_r)
+        ms_batch = float(np.median(reps))
         same = all(o["best_seed"].cpu().numpy().tolist() == b and bool((o["cls"].cpu() == cl).all())
                    for o, b, cl in zip(res, ref_best, ref_cls)) and all(bool(torch.equal(o["rss"], r)) for o, r in zip(res, ref_rss))
         b_parts = sum(len(it[2]) - 1 for it in items)
         b_pairs = sum(float(it[1].shape[1]) * it[0].n_fired for it in items)
         batch = {"events": len(items), "partitions": b_parts, "ms_per_batch": ms_batch, "ms_per_event": ms_batch / len(items),
                  "events_per_s": len(items) / (ms_batch * 1e-3), "dca_evals_per_s": b_pairs / (ms_batch * 1e-3),
+                 "ms_per_batch_repetitions": reps, "timed": "median of 5 repetitions (host-launch bound)",
                  "identical_to_single_stream": same, "seconds_to_generate_the_events_on_the_host": t_gen,
                  "workload": "BASELINE.json configs[2]: %d events (1-4 turns, |p| in [60, 105] MeV/c before the preselection, "
                              "131072 seeds per partition, %d partitions, %.0f fired wires on average), device-resident, %d "
@@ -793,6 +800,10 @@ def run_ours(args):
                      "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                      "what": "FP64-pipe instructions EXECUTED (work counters x per-unit SASS counts, `fp64_per_unit`) x 2 flop over the "
                              "device time of the call",
+                     "fp32_pruning": {"thread_instr": head["fp32_thread_instr_pruning"],
+                                      "what": "levels A and B of k_scan_zrun run on the FP32 pipe (pruning tests with rounding slack): not in "
+                                              "`frac`; at the FP32 rate (128 lanes per SM) they are this share of the call's time",
+                                      "share_of_call_at_fp32_peak": head["fp32_thread_instr_pruning"] / (2.0 * peak / 2.0 * 1e12) / (ms_call * 1e-3)},
                      "frac_dense_equivalent": head["frac_dense_equivalent"] * head["ms_scan_call"] / ms_call,
                      "dense_equivalent_is": "SURVEY 8(d)'s unit -- one RKN4 step per (seed, recorded state) although the z-run kernels take it "
                                             "once per distinct transverse track, 600 per fine pair -- over the same time: not pipe work",
