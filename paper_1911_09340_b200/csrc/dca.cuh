@@ -598,13 +598,33 @@ __global__ void __launch_bounds__(256) k_rss_sum(const double* __restrict__ e2, 
     double acc = 0.0;
     // (zg: the run length found on the device -- the mask exists only if the z-run kernel served the launch)
     if (tm && (!zg || *zg >= 8u)) {
+        // (the mask is the chunk's, a warp is one chunk: the control flow below is warp-uniform.  The additions are those of
+        // the plain loop, one per wire in wire order; only the bit tests of the wires without a row go)
         const unsigned int* m = tm + (size_t)(s >> 5) * MW;
         for (int wd = 0; wd * 32 < W; ++wd) {
-            const unsigned bits = __ldg(m + wd);
+            unsigned bits = __ldg(m + wd);
             const int n = min(32, W - wd * 32);
+            if (n < 32) bits &= (1u << n) - 1u;
+            if (__popc(bits) > 6) {                         // many rows: the loads of a batch of wires in flight together
 #pragma unroll 4
-            for (int j = 0; j < n; ++j)
-                acc = xadd(acc, ((bits >> j) & 1u) ? e2[(size_t)(wd * 32 + j) * SP + s] : lam2);
+                for (int q = 0; q < n; ++q)
+                    acc = xadd(acc, ((bits >> q) & 1u) ? e2[(size_t)(wd * 32 + q) * SP + s] : lam2);
+                continue;
+            }
+            int j = 0;
+            while (bits) {
+                const int jn = __ffs(bits) - 1;             // the next wire with a row
+                bits &= bits - 1;
+                for (; j < jn; ++j) acc = xadd(acc, lam2);
+                acc = xadd(acc, e2[(size_t)(wd * 32 + jn) * SP + s]);
+                j = jn + 1;
+            }
+            if (j == 0 && n == 32) {
+#pragma unroll
+                for (int q = 0; q < 32; ++q) acc = xadd(acc, lam2);
+            } else {
+                for (; j < n; ++j) acc = xadd(acc, lam2);
+            }
         }
     } else {
 #pragma unroll 4
