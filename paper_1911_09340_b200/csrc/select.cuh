@@ -32,13 +32,25 @@ __device__ __forceinline__ void partition_argmin(const double* __restrict__ rss,
 {
     v = 0.0;
     idx = -1;
-    for (int64_t s = first; s < hi; s += step) {
-        double r = rss[s];
-        if (r != r) {
-            if (s != lo) continue;
-            r = -INFINITY;
+    // batches of 8 loads in flight (one CTA may scan a whole partition: a load per iteration would serialise the latencies)
+    constexpr int NB = 8;
+    for (int64_t s0 = first; s0 < hi; s0 += NB * step) {
+        double rb[NB];
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {
+            const int64_t s = s0 + q * step;
+            rb[q] = s < hi ? rss[s] : __longlong_as_double(0x7ff8000000000000LL);   // (past the end: a NaN, skipped below)
         }
-        if (idx < 0 || r < v) { v = r; idx = s; }       // increasing s per thread: ties keep lower s
+#pragma unroll
+        for (int q = 0; q < NB; ++q) {
+            const int64_t s = s0 + q * step;
+            double r = rb[q];
+            if (r != r) {
+                if (s != lo || s >= hi) continue;
+                r = -INFINITY;
+            }
+            if (idx < 0 || r < v) { v = r; idx = s; }   // increasing s per thread: ties keep lower s
+        }
     }
     for (int o = 16; o > 0; o >>= 1) {
         const double v2 = __shfl_down_sync(0xffffffffu, v, o);
