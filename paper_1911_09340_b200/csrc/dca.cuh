@@ -627,7 +627,8 @@ __global__ void __launch_bounds__(256) k_rss_sum(const double* __restrict__ e2, 
             }
         }
     } else {
-#pragma unroll 4
+        // (small launches are latency-bound: 16 loads in flight per thread)
+#pragma unroll 16
         for (int i = 0; i < W; ++i) acc = xadd(acc, e2[(size_t)i * SP + s]);
     }
     rss[s] = acc;
