@@ -8,9 +8,9 @@
 //
 //   warp 0        generates the track, tile by tile, into a double-buffered tile in shared memory (the definition's
 //                 RKN4 steps, the target-region test, the checkpoints for k_fine_ck) -- one tile ahead of the search;
-//   warps 1 - 3   search the tile that is ready: the level-0 test of k_scan_fused (lane = wire; every search warp
-//                 evaluates it, it is cheap), then the wires with open sub-blocks are dealt round-robin to the three
-//                 warps, which sweep them (lane = seed) and merge the pair keys with an atomic min;
+//   warps 1 - 3   search the tile that is ready: the level-0 test of k_scan_fused (lane = wire; a search warp takes every
+//                 third wire, so that neighbouring wires -- near the same rows -- go to different warps), then the sweeps
+//                 of the sub-blocks its tests opened (lane = seed), merging the pair keys with an atomic min;
 //   all four      the finish of k_scan_fused, wire groups dealt round-robin.
 //
 // One __syncthreads per tile.  The chain of the generator (about 110 cycles per step) is what is left on the critical
@@ -64,7 +64,6 @@ __global__ void __launch_bounds__(128, 4) k_scan_small(const FusedArgs a)
     const unsigned nolip_mask = __ballot_sync(FULL, valid && !lip_ok);
     unsigned long long* const keys = reinterpret_cast<unsigned long long*>(a.bd);
     for (int i = warp; i < W; i += 4) keys[(size_t)i * a.SP + s] = COMET_KEY_NONE;
-    const int n_rounds = (W + 31) / 32;
     const int n_tiles = (a.n_steps + TR) / TR;
     unsigned long long st_cnt[ST_N];
     if (STATS) {
@@ -155,11 +154,12 @@ __global__ void __launch_bounds__(128, 4) k_scan_small(const FusedArgs a)
                     rz[j] = __uint_as_float(__reduce_max_sync(FULL, __float_as_uint(fz)));
                 }
                 const bool any_nolip = (nolip_mask & live) != 0u;
-                int deal = 0;                               // wires with open sub-blocks seen so far: dealt round-robin
-                for (int r = 0; r < n_rounds; ++r) {
+                // every search warp takes a strided third of the wires (neighbouring wires, which tend to be near the same
+                // rows, go to different warps): its level-0 tests and the sweeps they open
+                for (int r = 0; r * (32 * NSEARCH) < W; ++r) {
                     unsigned sm = 0u;
                     {
-                        const int i = r * 32 + lane;
+                        const int i = NSEARCH * (r * 32 + lane) + (warp - 1);
                         const int ii = min(i, W - 1);
                         EvalC ec;
                         wconst_evalc(ec, wtab, a.wt, W, ii);
@@ -173,15 +173,14 @@ __global__ void __launch_bounds__(128, 4) k_scan_small(const FusedArgs a)
                         }
                         if (any_nolip) sm = (1u << NSUB) - 1u;
                         if (cap < 0.0) sm = 0u;
-                        if (STATS && cap >= 0.0 && warp == 1) st_cnt[ST_SAMPLES] += NSUB;
+                        if (STATS && cap >= 0.0) st_cnt[ST_SAMPLES] += NSUB;
                     }
                     unsigned any = __ballot_sync(FULL, sm != 0u);
                     while (any) {
                         const int wl = __ffs(any) - 1;
                         any &= any - 1;
-                        if ((deal++ % NSEARCH) != warp - 1) continue;
                         unsigned wsub = __shfl_sync(FULL, sm, wl);
-                        const int i = r * 32 + wl;
+                        const int i = NSEARCH * (r * 32 + wl) + (warp - 1);
                         EvalC w;
                         wconst_evalc(w, wtab, a.wt, W, i);
                         double best = INF;
