@@ -1050,8 +1050,12 @@ extern "C" int comet_select_and_classify(comet_ctx* ctx, const double* seeds, in
     if (same_scan && ctx->last.valid == 1) { a.ub = ctx->ub; a.np_u = ctx->npu; a.zshift = ctx->last.zshift; a.u_rows = ctx->last.u_rows; }
     if (same_scan && ctx->last.valid == 2) { a.ck = ctx->ck; a.n_ck = ctx->last.n_ck; }
     const size_t smem = (size_t)(n_steps + 1) * (field ? 7 : 6) * sizeof(double);
-    if (field) k_select_classify<true><<<n_part, 256, smem, st>>>(a);
-    else k_select_classify<false><<<n_part, 256, smem, st>>>(a);
+    // (the search over the winner's states is most of the kernel and a CTA is one SM: groups of about 8 wires per CTA)
+    int n_grp = (n_fired + 7) / 8;
+    if (n_grp > 16) n_grp = 16;
+    if (n_grp < 1) n_grp = 1;
+    if (field) k_select_classify<true><<<dim3(n_part, n_grp), 256, smem, st>>>(a);
+    else k_select_classify<false><<<dim3(n_part, n_grp), 256, smem, st>>>(a);
     CU(ctx, cudaGetLastError());
     return COMET_OK;
 }

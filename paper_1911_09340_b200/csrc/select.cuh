@@ -122,17 +122,25 @@ struct ClassifyArgs {
 // CTA-wide: re-extrapolate seed `idx` into shared memory (state k at sm[k*6..]), then one thread per fired
 // wire does O5..O8 + O11 in exact arithmetic: dca[i] = signed D, cls[j] = 1 for the classified entries
 // (all other entries 0).  idx < 0: NaN / zeros.
+// With n_grp > 1 the CTA is one of n_grp that share a seed: each rebuilds the track for itself and takes the fired wires
+// [grp W / n_grp, (grp + 1) W / n_grp) and their hit entries (the search over the states is the bulk of the work and one
+// CTA uses one SM).
 template <bool FIELD>
 __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx, double* __restrict__ dca,
-                                             uint8_t* __restrict__ cls, double* sm)
+                                             uint8_t* __restrict__ cls, double* sm, int grp = 0, int n_grp = 1)
 {
     constexpr int RS = FIELD ? 7 : 6;                   // row: x, T and, in a field map, the step leaving the state
     __shared__ int32_t s_np;
     __shared__ double s_c;
-    for (int j = threadIdx.x; j < a.n_hits; j += blockDim.x) cls[j] = 0;
     const int W = a.W;
+    const int w0 = (int)((int64_t)W * grp / n_grp), w1 = (int)((int64_t)W * (grp + 1) / n_grp);
+    {
+        // the entries of the group's wires; the first and the last group also take what lies outside every wire's range
+        const int j0 = (grp == 0 || W == 0) ? 0 : a.hit_off[w0], j1 = (grp == n_grp - 1 || W == 0) ? a.n_hits : a.hit_off[w1];
+        for (int j = j0 + (int)threadIdx.x; j < j1; j += blockDim.x) cls[j] = 0;
+    }
     if (idx < 0) {
-        for (int i = threadIdx.x; i < W; i += blockDim.x) dca[i] = __longlong_as_double(0x7ff8000000000000LL);
+        for (int i = w0 + (int)threadIdx.x; i < w1; i += blockDim.x) dca[i] = __longlong_as_double(0x7ff8000000000000LL);
         return;
     }
     // The scan's tracks are taken only if they ARE this seed's: state 0 of the track / checkpoint 0 must equal the seed's own
@@ -244,11 +252,11 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
     __shared__ double s_bd[256];
     __shared__ int s_ks[256];
     const int nthr = blockDim.x;
-    const int Wp = min(W, nthr);
+    const int Wp = min(w1 - w0, nthr);
     const int NSEG = Wp > 0 ? nthr / Wp : 1;
-    for (int i0 = 0; i0 < W; i0 += Wp) {
+    for (int i0 = w0; i0 < w1; i0 += Wp) {
         const int wi = i0 + (int)threadIdx.x % Wp, seg = (int)threadIdx.x / Wp;
-        const bool on = wi < W && seg < NSEG;
+        const bool on = wi < w1 && seg < NSEG;
         WireLine wl;
         int ks = 0;
         double bd = 0.0;
@@ -292,13 +300,14 @@ __device__ __forceinline__ void classify_cta(const ClassifyArgs& a, int64_t idx,
     }
 }
 
-// One CTA per partition: finish the argmin, then classify the winning seed.
+// gridDim.y CTAs per partition: each finishes the argmin, then classifies the winning seed on its share of the wires.
 template <bool FIELD>
 __global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
 {
     extern __shared__ __align__(16) double sm[];       // [(n_steps+1)][6]
     __shared__ int64_t s_best;
     const int p = blockIdx.x;
+    const bool first_grp = blockIdx.y == 0;             // (every group finds the same winner; the first one writes it)
     if (a.rss) {
         // a small partition: the whole argmin here (same rule as k_argmin_stage1)
         __shared__ double sv[8];
@@ -311,8 +320,10 @@ __global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
         if (threadIdx.x == 0) {
             for (int w = 1; w < (int)blockDim.x / 32; ++w) argmin_merge(v, idx, sv[w], si[w]);
             s_best = idx;
-            a.best_seed[p] = idx;
-            a.best_rss[p] = (idx >= 0 && v != -INFINITY) ? v : __longlong_as_double(0x7ff8000000000000LL);
+            if (first_grp) {
+                a.best_seed[p] = idx;
+                a.best_rss[p] = (idx >= 0 && v != -INFINITY) ? v : __longlong_as_double(0x7ff8000000000000LL);
+            }
         }
     } else if (threadIdx.x == 0) {
         double v = 0.0;
@@ -320,11 +331,13 @@ __global__ void __launch_bounds__(256) k_select_classify(const ClassifyArgs a)
         for (int b = 0; b < COMET_ARGMIN_SPLIT; ++b)
             argmin_merge(v, idx, a.pv[p * COMET_ARGMIN_SPLIT + b], a.pi[p * COMET_ARGMIN_SPLIT + b]);
         s_best = idx;
-        a.best_seed[p] = idx;
-        a.best_rss[p] = (idx >= 0 && v != -INFINITY) ? v : __longlong_as_double(0x7ff8000000000000LL);
+        if (first_grp) {
+            a.best_seed[p] = idx;
+            a.best_rss[p] = (idx >= 0 && v != -INFINITY) ? v : __longlong_as_double(0x7ff8000000000000LL);
+        }
     }
     __syncthreads();
-    classify_cta<FIELD>(a, s_best, a.best_dca + (size_t)p * a.W, a.cls + (size_t)p * a.n_hits, sm);
+    classify_cta<FIELD>(a, s_best, a.best_dca + (size_t)p * a.W, a.cls + (size_t)p * a.n_hits, sm, (int)blockIdx.y, (int)gridDim.y);
 }
 
 }  // namespace comet
