@@ -51,6 +51,14 @@ def test_host_only_entry_points(libpath):
     # argument errors are reported before any CUDA call
     assert L.comet_create(None, 0) == -1
     assert L.comet_destroy(None) == -1
+    # comet_argmin_static: more partitions than its static scratch holds is refused with a status of its own, and
+    # negative sizes as invalid arguments -- both before any CUDA call
+    L.comet_argmin_static.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int32, ctypes.c_void_p,
+                                      ctypes.c_void_p, ctypes.c_void_p]
+    assert L.comet_argmin_static(None, 0, None, 65, None, None, None) == -4
+    assert b"statically allocated scratch" in L.comet_status_string(-4)
+    assert L.comet_argmin_static(None, -1, None, 1, None, None, None) == -1
+    assert L.comet_argmin_static(None, 0, None, 0, None, None, None) == 0
 
 
 def test_no_gpu_means_loud_failure(libpath):
