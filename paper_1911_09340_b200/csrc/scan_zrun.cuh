@@ -52,8 +52,12 @@
 
 namespace comet {
 
+#ifndef COMET_ZR_WARPS
 #define COMET_ZR_WARPS 4
+#endif
+#ifndef COMET_ZR_WCAP
 #define COMET_ZR_WCAP 128          // wires whose constants the CTA's shared-memory table holds (the others: L1/L2)
+#endif
 #define COMET_ZR_CK 8              // rows between z checkpoints
 #define COMET_ZR_LCAP 1024         // (chunk, wire) items collected per reservation in the finish
 #ifndef COMET_ZR_MINB
