@@ -216,11 +216,11 @@ extern "C" int comet_create(comet_ctx** out, int cuda_device)
     // shared-memory opt-ins (done once here, never on the hot path)
 #define COMET_ZRUN_OPTIN(NU)                                                                                                   \
     do {                                                                                                                       \
-        const int zs = COMET_ZR_SMEM(NU, ctx->wt_cap);                                                                         \
+        const int zs = COMET_ZR_SMEM(NU, COMET_ZR_WCAP, false), zb = COMET_ZR_SMEM(NU, ctx->wt_cap, true);                     \
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<false, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, zs); \
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<false, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, zs);  \
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<false, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, zb);  \
         if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<true, NU, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, zs);  \
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<true, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, zs);   \
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_scan_zrun<true, NU, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, zb);   \
     } while (0)
     COMET_ZRUN_OPTIN(1);
     COMET_ZRUN_OPTIN(2);
@@ -897,14 +897,15 @@ static int scan_rss_impl(comet_ctx* ctx, double* seeds_w, const double* seeds_ho
                 else k_gen_unique<false><<<bu, 32, 0, s_scan>>>(az);
                 if (tm) CU(ctx, cudaEventRecord(tev[1], st));
                 const bool bigw = n_fired > COMET_ZR_WCAP;
-                const unsigned bz = (unsigned)((nc + COMET_ZR_WARPS - 1) / COMET_ZR_WARPS);
-                const int zthr = 32 * COMET_ZR_WARPS;
+                const int wpc = COMET_ZR_WPC(bigw);              // (many wires: CTAs of one warp, no wire table)
+                const unsigned bz = (unsigned)((nc + wpc - 1) / wpc);
+                const int zthr = 32 * wpc;
 #define COMET_LAUNCH_ZRUN(NU)                                                                                         \
                 do {                                                                                                  \
-                    if (a.stats) { if (bigw) k_scan_zrun<true, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired), s_scan>>>(az);     \
-                                   else k_scan_zrun<true, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired), s_scan>>>(az); }       \
-                    else { if (bigw) k_scan_zrun<false, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired), s_scan>>>(az);            \
-                           else k_scan_zrun<false, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired), s_scan>>>(az); }              \
+                    if (a.stats) { if (bigw) k_scan_zrun<true, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired, true), s_scan>>>(az);     \
+                                   else k_scan_zrun<true, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired, false), s_scan>>>(az); }      \
+                    else { if (bigw) k_scan_zrun<false, NU, true><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired, true), s_scan>>>(az);            \
+                           else k_scan_zrun<false, NU, false><<<bz, zthr, COMET_ZR_SMEM(NU, n_fired, false), s_scan>>>(az); }             \
                 } while (0)
                 if (!zrun_host || zrun_host == 32) COMET_LAUNCH_ZRUN(1);
                 if (!zrun_host || zrun_host == 16) COMET_LAUNCH_ZRUN(2);

@@ -71,8 +71,14 @@ namespace comet {
 #define COMET_ZR_FF 11             // fields of the single-precision wire table (k_wire_prep)
 // + the touched-wire mask: one bit per fired wire, rounded up to whole 16 bytes
 #define COMET_ZR_MWD(W) ((((W) + 31) / 32 + 3) / 4 * 2)
-#define COMET_ZR_SMEM(NU, W) ((COMET_ZR_NF * COMET_ZR_WCAP + COMET_ZR_WARPS * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W))) * (int)sizeof(double) + \
-                              COMET_ZR_FF * COMET_ZR_WCAP * (int)sizeof(float))
+#define COMET_ZR_SMEM_OF(NU, W, WPC, WCAP_) ((COMET_ZR_NF * (WCAP_) + (WPC) * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W))) * (int)sizeof(double) + \
+                                            COMET_ZR_FF * (WCAP_) * (int)sizeof(float))
+// BIGW (more fired wires than the table holds): CTAs of ONE warp and no table at all -- every wire constant comes through L1,
+// 20 CTAs per SM, no warp waits for the slowest of its CTA (measured on configs[4], 972 wires: 0.973 -> 0.919 ms; with a table
+// that serves every wire the four-warp CTA is the faster one: 0.340 against 0.356 ms on configs[1])
+#define COMET_ZR_WPC(BIGW) ((BIGW) ? 1 : COMET_ZR_WARPS)
+#define COMET_ZR_TCAP(BIGW) ((BIGW) ? 0 : COMET_ZR_WCAP)
+#define COMET_ZR_SMEM(NU, W, BIGW) COMET_ZR_SMEM_OF(NU, W, COMET_ZR_WPC(BIGW), COMET_ZR_TCAP(BIGW))
 // relative rounding slack of the single-precision tests: 32 x 2^-24 per unit of (|x| + |y| + |z| + |c1| + |c2|)
 #define COMET_ZR_FSLACK 1.9073486e-6f
 #define COMET_ZR_MARGIN 1e-6       // cm, added to every pruning threshold (FMA rounding is ~1e-13)
@@ -81,7 +87,7 @@ template <bool BIGW>
 __device__ __forceinline__ double zr_const(const double* wtab, const double* __restrict__ wt, int W, int f, int i)
 {
     if (!BIGW) return wtab[f * COMET_ZR_WCAP + i];
-    return (i < COMET_ZR_WCAP) ? wtab[f * COMET_ZR_WCAP + i] : __ldg(wt + (size_t)(6 + f) * W + i);
+    return __ldg(wt + (size_t)(6 + f) * W + i);
 }
 template <bool BIGW>
 __device__ __forceinline__ void zr_evalc(EvalC& w, const double* wtab, const double* __restrict__ wt, int W, int i)
@@ -95,21 +101,21 @@ template <bool BIGW>
 __device__ __forceinline__ float zr_constf(const float* wtabf, const float* __restrict__ wtf, int W, int f, int i)
 {
     if (!BIGW) return wtabf[f * COMET_ZR_WCAP + i];
-    return (i < COMET_ZR_WCAP) ? wtabf[f * COMET_ZR_WCAP + i] : __ldg(wtf + (size_t)f * W + i);
+    return __ldg(wtf + (size_t)f * W + i);
 }
 template <bool BIGW>
 __device__ __forceinline__ double zr_slope(const double* wtab, const double* __restrict__ wt, int W, int i)
 {
-    if (!BIGW || i < COMET_ZR_WCAP) return wtab[COMET_FUSED_WFIELDS * COMET_ZR_WCAP + i];
+    if (!BIGW) return wtab[COMET_FUSED_WFIELDS * COMET_ZR_WCAP + i];
     return wire_slope(__ldg(wt + (size_t)8 * W + i), __ldg(wt + (size_t)12 * W + i));
 }
 
 template <bool STATS, int NU, bool BIGW>
-__global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zrun(const FusedArgs a)
+__global__ void __launch_bounds__(32 * COMET_ZR_WPC(BIGW), BIGW ? 20 : COMET_ZR_MINB) k_scan_zrun(const FusedArgs a)
 {
     static_assert(NU == 1 || NU == 2 || NU == 4, "runs of 32, 16 or 8 seeds");
     constexpr int ZR = 32 / NU, ZSH = (NU == 1 ? 5 : (NU == 2 ? 4 : 3));
-    constexpr int WCAP = COMET_ZR_WCAP, NF = COMET_ZR_NF;
+    constexpr int WCAP = COMET_ZR_TCAP(BIGW), NF = COMET_ZR_NF, WPC = COMET_ZR_WPC(BIGW);
     constexpr int BLK = 64, SUB = 8, NSUB = BLK / SUB, SROW = 36;
     constexpr int CK = COMET_ZR_CK, LCAP = COMET_ZR_LCAP;
     constexpr int BUFD = (BLK + NSUB) * NU * 2;             // doubles per staged block: rows [64][NU][x, y], tangents [8][NU][T_x, T_y]
@@ -126,21 +132,21 @@ __global__ void __launch_bounds__(32 * COMET_ZR_WARPS, COMET_ZR_MINB) k_scan_zru
     unsigned short* plist = reinterpret_cast<unsigned short*>(stg + 2 * BUFD);     // [64] wires that passed level A
     float* sampf = reinterpret_cast<float*>(stg + 2 * BUFD + 16);                  // [8][NU][8] samples of the current block
     unsigned* tmask = reinterpret_cast<unsigned*>(stg + 2 * BUFD + 16 + NSUB * NU * 4);   // [MW] bit i: the key row of wire i exists
-    float* wtabf = reinterpret_cast<float*>(zsm + NF * WCAP + COMET_ZR_WARPS * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W)));   // [FF][WCAP]
+    float* wtabf = reinterpret_cast<float*>(zsm + NF * WCAP + WPC * (COMET_ZR_WSM(NU) + COMET_ZR_MWD(W)));   // [FF][WCAP]
     unsigned short* lst = reinterpret_cast<unsigned short*>(stg);                  // finish: [<= LCAP] items
     constexpr int LCAPW = (NU == 1) ? (2 * BUFD * 4) : LCAP;                       // shorts the staged blocks hold
-    for (int v = threadIdx.x; v < COMET_FUSED_WFIELDS * WCAP; v += 32 * COMET_ZR_WARPS) {
+    for (int v = threadIdx.x; v < COMET_FUSED_WFIELDS * WCAP; v += 32 * WPC) {
         const int f = v / WCAP, i = v - f * WCAP;
         wtab[v] = (i < W) ? __ldg(a.wt + (size_t)(6 + f) * W + i) : -1.0;
     }
-    for (int i = threadIdx.x; i < WCAP; i += 32 * COMET_ZR_WARPS)
+    for (int i = threadIdx.x; i < WCAP; i += 32 * WPC)
         wtab[COMET_FUSED_WFIELDS * WCAP + i] = (i < W) ? wire_slope(__ldg(a.wt + (size_t)8 * W + i), __ldg(a.wt + (size_t)12 * W + i)) : 0.0;
-    for (int v = threadIdx.x; v < COMET_ZR_FF * WCAP; v += 32 * COMET_ZR_WARPS) {
+    for (int v = threadIdx.x; v < COMET_ZR_FF * WCAP; v += 32 * WPC) {
         const int f = v / WCAP, i = v - f * WCAP;
         wtabf[v] = (i < W) ? __ldg(a.wtf + (size_t)f * W + i) : -1.f;
     }
     __syncthreads();
-    const int64_t chunk = (int64_t)blockIdx.x * COMET_ZR_WARPS + warp;
+    const int64_t chunk = (int64_t)blockIdx.x * WPC + warp;
     if (chunk * COMET_LANES >= a.n_seeds) return;
     const int64_t s = chunk * COMET_LANES + lane;
     const bool valid = s < a.n_seeds;
